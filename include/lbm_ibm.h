@@ -1,0 +1,141 @@
+/*
+ * lbm_ibm.h -- C ABI of the B200-native LBM-IBM time-step library (liblbm_ibm_b200.so).
+ *
+ * Method: Beny & Latt, "Efficient LBM on GPUs for dense moving objects using immersed boundary
+ * condition" (arXiv 1904.02108).  "P:NN" = line NN of the paper text; "Rn" = reading n in
+ * DESIGN.md.  One time step is the paper's pseudo-code P:60-66:
+ *   1. rho, U from the populations (eq. (1))            -- only on cells near markers
+ *   2. G = immersedBoundary(object, U) (section 3): multi-direct-forcing loop,
+ *      Peskin 4-point kernel, markers moved by a rigid rotation on the device
+ *   3.-6. D3Q19 BGK collision (eq. (2),(3)) with the body force (Guo term, R3; or the
+ *      paper's velocity shift, as an option) fused with streaming (eq. (4)),
+ *      periodic or half-way bounce-back faces.
+ *
+ * Conventions
+ *  - All entry points are extern "C"; no exceptions or aborts cross the boundary.  Functions
+ *    returning int give 0 on success and a negative LBM_E* code on error; the text of the last
+ *    error of the calling thread is lbm_last_error().  On error the state is unchanged.
+ *  - Every pointer argument marked "host or device" may point to pageable/pinned host memory or
+ *    to device memory of the handle's GPU (detected with cudaPointerGetAttributes).  Pointers
+ *    marked "host" are read on the CPU during the call.
+ *  - The caller owns every buffer it passes; inputs are copied during the call and may be freed
+ *    at once.  The library owns lattice and marker state (device memory of the current device at
+ *    lbm_create time).
+ *  - Field layout: x fastest, then y, then z: index = (z*ny + y)*nx + x; vector fields are three
+ *    such planes [3][nz][ny][nx].  Lattice units; cell centres at integer coordinates 0..n-1; on
+ *    a wall axis the wall planes sit half a link outside the first / last node (R16).
+ *  - All work is enqueued on the handle's stream (lbm_set_stream; default: the legacy default
+ *    stream).  lbm_ibm_step is asynchronous; lbm_read_fields / ibm_read_markers synchronise the
+ *    stream before returning when the destination is host memory.
+ *  - Arithmetic: fp32 on the device (populations are stored as f_i - t_i), fp64 only for the
+ *    per-body rotation tables (R21).
+ */
+#ifndef LBM_IBM_H
+#define LBM_IBM_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lbm lbm_t;
+
+/* Boundary conditions and uniform body acceleration (BASELINE.json configs[1],[2]; R15). */
+typedef struct {
+    int wall_x, wall_y, wall_z; /* per axis: 0 = periodic, 1 = half-way bounce-back on both faces */
+    double gx, gy, gz;          /* uniform body acceleration g_body added to the IBM force (R4)   */
+} lbm_bc_t;
+
+enum {
+    LBM_OK = 0,
+    LBM_EINVAL = -1,  /* bad argument (NULL handle, sizes < 1, tau <= 0.5, n < 0, zero axis ...)   */
+    LBM_ENOMEM = -2,  /* device or host allocation failed                                        */
+    LBM_ECUDA = -3,   /* a CUDA call or kernel failed; text in lbm_last_error()                   */
+    LBM_ERANGE = -4,  /* a marker's 4x4x4 stencil would cross a wall face (R17)                   */
+    LBM_ESTATE = -5   /* call not valid in the current state (e.g. kinematics before markers)    */
+};
+
+/* Options for lbm_set_option. */
+enum {
+    LBM_OPT_SPREAD = 1,   /* 0 = deterministic gather-by-cell (default), 1 = global atomics (the
+                             paper's ib_force2 design; kept as a measured comparison)  */
+    LBM_OPT_FORCING = 2,  /* 0 = Guo source term (default, R3), 1 = paper's shift U + tau G */
+    LBM_OPT_GRAPH = 3,    /* 1 = replay the step as a CUDA graph (default), 0 = plain launches     */
+    LBM_OPT_LBM_KERNEL = 4, /* stream-collide variant: 0 = default (vectorised), 1 = scalar         */
+    LBM_OPT_INTERP = 5    /* interpolation variant: 0 = default, 1 = thread per marker            */
+};
+
+/* Keys for lbm_get_info. */
+enum {
+    LBM_INFO_MARKERS = 1,       /* number of Lagrangian points                                   */
+    LBM_INFO_BODIES = 2,
+    LBM_INFO_STEPS = 3,         /* completed time steps                                           */
+    LBM_INFO_LAUNCHES = 4,      /* kernels launched by this handle so far (graph nodes counted)   */
+    LBM_INFO_ACTIVE_CELLS = 5,  /* cells inside at least one marker's stencil in the last step    */
+    LBM_INFO_DEVICE_BYTES = 6,  /* device memory owned by the handle                              */
+    LBM_INFO_STATUS = 7         /* device-side status word of the last step (0 = OK)              */
+};
+
+/* P:31 + eq.(3): allocate an nx*ny*nz D3Q19 lattice with relaxation time tau on the current CUDA
+ * device and set it to rest (rho = 1, u = 0, i.e. f_i = t_i; R18).  bc may be NULL (periodic, no
+ * body force).  Returns NULL on error (see lbm_last_error). */
+lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc);
+
+/* Free everything the handle owns.  NULL is allowed. */
+void lbm_destroy(lbm_t *h);
+
+/* Use cuda_stream (a cudaStream_t; NULL = legacy default stream) for all later work. */
+int lbm_set_stream(lbm_t *h, void *cuda_stream);
+
+int lbm_set_option(lbm_t *h, int key, int value);
+int lbm_get_info(lbm_t *h, int key, long long *value /* host */);
+
+/* R18: f_i = Eq_i(rho, u) (eq. (3)) on every cell, with u the bare velocity of eq. (1).
+ * rho [nz][ny][nx] or NULL (= 1); u [3][nz][ny][nx] or NULL (= 0); host or device; fp32.
+ * Resets the step counter and the force field to zero. */
+int lbm_set_fields(lbm_t *h, const float *rho, const float *u);
+
+/* P:154 "object": define ONE rigid body of n Lagrangian points and append it to the handle.
+ * pos [n][3] rest positions x(k) (on a periodic axis any real value, it is wrapped; on a wall axis
+ * the stencil floor(x)-1..floor(x)+2 must stay inside 0..n-1, else LBM_ERANGE); vel [n][3]
+ * additional, unrotated point velocity or NULL (= 0) (R14); area [n] the surface area s(k) of P:94.
+ * All host or device, fp32.  Returns the body id (>= 0) or a negative error. */
+int ibm_set_markers(lbm_t *h, const float *pos, const float *vel, const float *area, long long n);
+
+/* P:154, Alg.1: the body most recently defined rotates rigidly with omega rad/step about
+ * the line through center[3] along axis[3] (host, fp64; axis is normalised).  Step n -> n+1 places
+ * point k at c + R(omega (n+1)) (p_k - c) and prescribes u_k = (R(omega (n+1)) - R(omega n))
+ * (p_k - c) + vel_k (R12, R13).  Bodies without kinematics are static (omega = 0).  On a wall axis
+ * the sphere swept by every point must keep its stencil inside the box, else LBM_ERANGE. */
+int ibm_set_kinematics(lbm_t *h, double omega, const double *axis, const double *center);
+
+/* Remove all bodies and markers. */
+int ibm_clear(lbm_t *h);
+
+/* Advance nsteps time steps (pseudo-code P:60-66), each with mdf_iters multi-direct-forcing
+ * iterations (the paper uses 5).  mdf_iters = 0 or no markers = pure LBM.
+ * Asynchronous: returns after enqueueing on the handle's stream. */
+int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters);
+
+/* Canonical read-out (R19): rho [nz][ny][nx] and bare velocity u [3][nz][ny][nx] (eq. (1)) of the
+ * state after the last completed step; force [3][nz][ny][nx] = G of the last step (zero
+ * before any step and away from markers).  Any pointer may be NULL; host or device; fp32. */
+int lbm_read_fields(lbm_t *h, float *rho, float *u, float *force);
+
+/* Marker read-out of the last step, in the caller's original marker order (bodies concatenated):
+ * pos [n][3] current positions; force [n][3] = Delta u(k); cell [n] = linear index
+ * of the owning lattice cell (floor of the position); perm [n]: perm[i] = original index of the
+ * i-th marker after the stable sort by cell (ties by original index).  Any may be NULL;
+ * host or device. */
+int ibm_read_markers(lbm_t *h, float *pos, float *force, int *perm, int *cell);
+
+/* Block until all enqueued work is done; returns LBM_ERANGE if a stencil crossed a wall during
+ * the steps since the last sync (the offending step clamps the stencil instead of faulting). */
+int lbm_sync(lbm_t *h);
+
+/* Text of the last error raised on the calling thread ("" if none). */
+const char *lbm_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBM_IBM_H */

@@ -1,0 +1,102 @@
+// D3Q19 lattice constants and the fp32 BGK collision with body force, in deviation form.
+//
+// Populations are stored as  df_i = f_i - t_i: the rest state is all
+// zeros and the O(1) part of rho never enters an fp32 sum.
+//
+// Direction numbering is lexicographic in (ez, ey, ex) over the 19 vectors with |e|^2 <= 2, so
+// that the opposite of direction i is 18 - i and i = 9 is the rest population (P:35 gives no
+// order; it is internal and never visible at the ABI, reading R2).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace lbmk {
+
+constexpr int NQ = 19;
+
+// e_i as constexpr functions (folded to literals once the direction loops are unrolled).
+__host__ __device__ constexpr int dir_ez(int i) { return i < 5 ? -1 : (i < 14 ? 0 : 1); }
+__host__ __device__ constexpr int dir_ey(int i)
+{
+    return i < 5 ? (i == 0 ? -1 : (i == 4 ? 1 : 0)) : (i < 14 ? ((i - 5) / 3 - 1) : (i == 14 ? -1 : (i == 18 ? 1 : 0)));
+}
+__host__ __device__ constexpr int dir_ex(int i)
+{
+    return i < 5 ? (i == 1 ? -1 : (i == 3 ? 1 : 0)) : (i < 14 ? ((i - 5) % 3 - 1) : (i == 15 ? -1 : (i == 17 ? 1 : 0)));
+}
+__host__ __device__ constexpr int dir_opp(int i) { return NQ - 1 - i; }
+__host__ __device__ constexpr int dir_norm2(int i)
+{
+    return dir_ex(i) * dir_ex(i) + dir_ey(i) * dir_ey(i) + dir_ez(i) * dir_ez(i);
+}
+// t_i: 1/3 (rest), 1/18 (axis), 1/36 (face diagonal); c_s^2 = 1/3.
+__host__ __device__ constexpr float dir_weight(int i)
+{
+    return dir_norm2(i) == 0 ? (1.0f / 3.0f) : (dir_norm2(i) == 1 ? (1.0f / 18.0f) : (1.0f / 36.0f));
+}
+
+// Relaxation and forcing constants, filled on the host from the double-precision tau.
+struct CollisionConst {
+    float omega;       // 1/tau
+    float keep;        // 1 - 1/tau
+    float guo;         // 1 - 1/(2 tau)
+    float tau;
+    float gbx, gby, gbz;  // uniform body acceleration
+    int shift_forcing;    // 0: Guo source term (R3); 1: paper's U + tau*a shift
+};
+
+// Moments of eq. (1), from deviations: rho = 1 + sum df, rho U = sum e_i df (sum e_i t_i = 0).
+__device__ __forceinline__ void moments(const float (&df)[NQ], float &drho, float &ux, float &uy, float &uz)
+{
+    float s = 0.f, jx = 0.f, jy = 0.f, jz = 0.f;
+#pragma unroll
+    for (int i = 0; i < NQ; ++i) {
+        s += df[i];
+        if (dir_ex(i) == 1) jx += df[i];
+        if (dir_ex(i) == -1) jx -= df[i];
+        if (dir_ey(i) == 1) jy += df[i];
+        if (dir_ey(i) == -1) jy -= df[i];
+        if (dir_ez(i) == 1) jz += df[i];
+        if (dir_ez(i) == -1) jz -= df[i];
+    }
+    const float inv = 1.0f / (1.0f + s);
+    drho = s;
+    ux = jx * inv;
+    uy = jy * inv;
+    uz = jz * inv;
+}
+
+// BGK collision, eq. (2),(3) (rho per R1), with acceleration a = G + g_body (R4):
+//   Guo (R3):   u* = U + a/2,  f_i <- f_i - (f_i - Eq_i(rho,u*))/tau
+//                                       + (1 - 1/(2tau)) t_i rho [3 (e_i - u*).a + 9 (e_i.u*)(e_i.a)]
+//   shift:  f_i <- f_i - (f_i - Eq_i(rho, U + tau a))/tau
+// all in deviation form: Eq_i - t_i = t_i [drho + rho (3 e.u + 4.5 (e.u)^2 - 1.5 u.u)].
+__device__ __forceinline__ void collide(float (&df)[NQ], float ax, float ay, float az, const CollisionConst &c)
+{
+    float drho, ux, uy, uz;
+    moments(df, drho, ux, uy, uz);
+    const float rho = 1.0f + drho;
+    const float h = c.shift_forcing ? c.tau : 0.5f;
+    const float vx = fmaf(h, ax, ux), vy = fmaf(h, ay, uy), vz = fmaf(h, az, uz);
+    const float uu15 = 1.5f * (vx * vx + vy * vy + vz * vz);
+    const float va3 = 3.0f * (vx * ax + vy * ay + vz * az);
+    const float sg = c.shift_forcing ? 0.0f : c.guo;
+#pragma unroll
+    for (int i = 0; i < NQ; ++i) {
+        const float eu = dir_ex(i) * vx + dir_ey(i) * vy + dir_ez(i) * vz;
+        const float ea = dir_ex(i) * ax + dir_ey(i) * ay + dir_ez(i) * az;
+        const float w = dir_weight(i);
+        const float eqd = w * fmaf(rho, fmaf(eu, fmaf(4.5f, eu, 3.0f), -uu15), drho);
+        const float src = sg * w * rho * (fmaf(9.0f * eu, ea, 3.0f * ea) - va3);
+        df[i] = fmaf(c.keep, df[i], fmaf(c.omega, eqd, src));
+    }
+}
+
+// Eq_i(rho, u) - t_i, used by lbm_set_fields (R18).
+__device__ __forceinline__ float equilibrium_dev(int i, float drho, float ux, float uy, float uz)
+{
+    const float eu = dir_ex(i) * ux + dir_ey(i) * uy + dir_ez(i) * uz;
+    const float uu15 = 1.5f * (ux * ux + uy * uy + uz * uz);
+    return dir_weight(i) * fmaf(1.0f + drho, fmaf(eu, fmaf(4.5f, eu, 3.0f), -uu15), drho);
+}
+
+}  // namespace lbmk

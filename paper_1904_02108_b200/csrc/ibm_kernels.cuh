@@ -1,0 +1,433 @@
+// Immersed-boundary kernels: rigid-rotation kinematics (a1, a2), bins + active-cell mask (a3),
+// interpolation (a5), direct-forcing correction (a6), spreading (a7).  Section 3 of the paper
+// with the readings R6-R14 of DESIGN.md.
+//
+// Marker position is kept as (integer cell, fractional offset in [0,1)) per axis, so the delta
+// kernel arguments never lose bits to the magnitude of the coordinate.
+#pragma once
+#include "lbm_kernels.cuh"
+
+namespace lbmk {
+
+// per-body constants (host-filled, fp64) and per-step rotation tables (device-filled)
+struct BodyDef {
+    double omega, ax, ay, az;      // unit axis
+    int ci[3];                     // centre = ci + cf, cf in [0,1)
+    float cf[3];
+};
+struct BodyStep {
+    float R[9];    // R(omega (n+1))
+    float dR[9];   // R(omega (n+1)) - R(omega n), formed in fp64 (R12)
+};
+
+struct MarkerIn {                  // original (caller) order, SoA
+    const float *qx, *qy, *qz;     // rest position relative to the body centre, p_k - c (fp64 -> fp32)
+    const float *vx, *vy, *vz;     // extra velocity vel_k (R14)
+    const float *s;                // area s(k)
+    const int *body;
+    int n;
+};
+
+// a1: Rodrigues rotation tables of every body for step n -> n+1, in fp64 (R12, R13).
+// Also re-arms the per-step device counters.
+__global__ void k_kinematics(const BodyDef *__restrict__ defs, BodyStep *__restrict__ out, int nbodies,
+                             const long long *__restrict__ step_ctr, int *__restrict__ n_words)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b == 0) *n_words = 0;
+    if (b >= nbodies) return;
+    const BodyDef d = defs[b];
+    const double n = (double)(*step_ctr);
+    double R1[9], R0[9];
+    for (int which = 0; which < 2; ++which) {
+        const double th = d.omega * (n + (which == 0 ? 1.0 : 0.0));
+        double s, c;
+        sincos(th, &s, &c);
+        const double v = 1.0 - c;
+        double *R = which == 0 ? R1 : R0;
+        R[0] = c + d.ax * d.ax * v;        R[1] = d.ax * d.ay * v - d.az * s; R[2] = d.ax * d.az * v + d.ay * s;
+        R[3] = d.ay * d.ax * v + d.az * s; R[4] = c + d.ay * d.ay * v;        R[5] = d.ay * d.az * v - d.ax * s;
+        R[6] = d.az * d.ax * v - d.ay * s; R[7] = d.az * d.ay * v + d.ax * s; R[8] = c + d.az * d.az * v;
+    }
+    BodyStep o;
+    for (int j = 0; j < 9; ++j) { o.R[j] = (float)R1[j]; o.dR[j] = (float)(R1[j] - R0[j]); }
+    out[b] = o;
+}
+
+struct Placed {
+    int cx, cy, cz;      // owning cell = floor(position), wrapped on periodic axes
+    float fx, fy, fz;    // position - cell, in [0,1)
+    bool bad;            // stencil would cross a wall face (R17); cell clamped
+};
+
+__device__ __forceinline__ void place_axis(float d, int ci, int n, int wall, int &c, float &f, bool &bad)
+{
+    const float fl = floorf(d);
+    f = d - fl;
+    c = ci + (int)fl;
+    if (f >= 1.0f) { f = 0.0f; c += 1; }       // d = -tiny rounds d - floor(d) up to 1
+    if (wall) {
+        if (c < 1 || c > n - 3) { bad = true; c = min(max(c, 1), n - 3); }
+    } else {
+        c %= n;
+        if (c < 0) c += n;
+    }
+}
+
+// a2: x_k = c + R (p_k - c) as (cell, fraction).  Used by BOTH the key kernel and the gather kernel
+// so the two always agree on the owning cell.
+__device__ __forceinline__ Placed place_marker(const BodyDef &d, const BodyStep &t, float qx, float qy, float qz,
+                                               const Geom &g)
+{
+    Placed p;
+    p.bad = false;
+    const float dx = fmaf(t.R[0], qx, fmaf(t.R[1], qy, fmaf(t.R[2], qz, d.cf[0])));
+    const float dy = fmaf(t.R[3], qx, fmaf(t.R[4], qy, fmaf(t.R[5], qz, d.cf[1])));
+    const float dz = fmaf(t.R[6], qx, fmaf(t.R[7], qy, fmaf(t.R[8], qz, d.cf[2])));
+    place_axis(dx, d.ci[0], g.nx, g.wallx, p.cx, p.fx, p.bad);
+    place_axis(dy, d.ci[1], g.ny, g.wally, p.cy, p.fy, p.bad);
+    place_axis(dz, d.ci[2], g.nz, g.wallz, p.cz, p.fz, p.bad);
+    return p;
+}
+
+// a2: cell key of every marker (original order): key = (cz ny + cy) nx + cx  (O3).
+__global__ void __launch_bounds__(256)
+k_marker_keys(MarkerIn m, const BodyDef *__restrict__ defs, const BodyStep *__restrict__ tabs, Geom g,
+              unsigned *__restrict__ keys, int *__restrict__ status)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= m.n) return;
+    const int b = m.body[k];
+    const Placed p = place_marker(defs[b], tabs[b], m.qx[k], m.qy[k], m.qz[k], g);
+    if (p.bad) *status = 1;
+    keys[k] = (unsigned)((p.cz * g.ny + p.cy) * g.nx + p.cx);
+}
+
+// per-marker state in SORTED order
+struct MarkerSorted {
+    float4 *fs;     // (fx, fy, fz, s)
+    float4 *uk;     // prescribed velocity u_k, w unused
+    float4 *sg;     // s * g^m(k)   (what the U update spreads, P:98 + R8)
+    float4 *du;     // Delta u(k)
+};
+
+// a2 (second half): gather into sorted order; u_k = dR (p_k - c) + vel_k (chord velocity, R12).
+__global__ void __launch_bounds__(256)
+k_marker_gather(MarkerIn m, const BodyDef *__restrict__ defs, const BodyStep *__restrict__ tabs, Geom g,
+                const int *__restrict__ perm, MarkerSorted out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m.n) return;
+    const int k = perm[i];
+    const int b = m.body[k];
+    const BodyStep t = tabs[b];
+    const float qx = m.qx[k], qy = m.qy[k], qz = m.qz[k];
+    const Placed p = place_marker(defs[b], t, qx, qy, qz, g);
+    out.fs[i] = make_float4(p.fx, p.fy, p.fz, m.s[k]);
+    const float ux = fmaf(t.dR[0], qx, fmaf(t.dR[1], qy, fmaf(t.dR[2], qz, m.vx[k])));
+    const float uy = fmaf(t.dR[3], qx, fmaf(t.dR[4], qy, fmaf(t.dR[5], qz, m.vy[k])));
+    const float uz = fmaf(t.dR[6], qx, fmaf(t.dR[7], qy, fmaf(t.dR[8], qz, m.vz[k])));
+    out.uk[i] = make_float4(ux, uy, uz, 0.f);
+    out.du[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    out.sg[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
+__device__ __forceinline__ void key_to_cell(unsigned key, const Geom &g, int &cx, int &cy, int &cz)
+{
+    const int row = (int)(key / (unsigned)g.nx);
+    cx = (int)key - row * g.nx;
+    cz = row / g.ny;
+    cy = row - cz * g.ny;
+}
+
+__device__ __forceinline__ int wrap(int i, int n)
+{
+    return i < 0 ? i + n : (i >= n ? i - n : i);
+}
+
+// a3: bins and active cells.  The first marker of every occupied cell ("bin head") records its
+// sorted index in the dense cell -> first-marker map and marks the 4x4x4 cells of its stencil in
+// the active-cell bitmask (one bit per cell, 32 consecutive x per word).  The thread whose
+// atomicOr turns a word from 0 to non-zero appends it to the active-word list (warp-aggregated).
+__global__ void __launch_bounds__(256)
+k_bins(const unsigned *__restrict__ skey, int n, Geom g, int *__restrict__ bin_first, unsigned *__restrict__ amask,
+       int *__restrict__ words, int *__restrict__ n_words)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    bool head = false;
+    int cx = 0, cy = 0, cz = 0;
+    if (i < n) {
+        const unsigned key = skey[i];
+        head = (i == 0) || (skey[i - 1] != key);
+        if (head) {
+            bin_first[key] = i;
+            key_to_cell(key, g, cx, cy, cz);
+        }
+    }
+    // the four x cells cx-1..cx+2 fall into at most two words (two runs when they wrap)
+#pragma unroll 1
+    for (int r = 0; r < 16; ++r) {
+        const int y = wrap(cy - 1 + (r & 3), g.ny);
+        const int z = wrap(cz - 1 + (r >> 2), g.nz);
+        const int rowbase = (z * g.ny + y) * g.nxw;
+        int w0 = -1, w1 = -1;
+        unsigned b0 = 0, b1 = 0;
+        if (head) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int x = wrap(cx - 1 + j, g.nx);
+                const int w = rowbase + (x >> 5);
+                const unsigned bit = 1u << (x & 31);
+                if (w0 < 0 || w == w0) { w0 = w; b0 |= bit; }
+                else { w1 = w; b1 |= bit; }
+            }
+        }
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            const int w = half ? w1 : w0;
+            const unsigned b = half ? b1 : b0;
+            bool fresh = false;
+            if (w >= 0) fresh = (atomicOr(amask + w, b) == 0u);
+            const unsigned vote = __ballot_sync(0xffffffffu, fresh);
+            if (vote) {
+                int base = 0;
+                const int leader = __ffs(vote) - 1;
+                if (lane == leader) base = atomicAdd(n_words, __popc(vote));
+                base = __shfl_sync(0xffffffffu, base, leader);
+                if (fresh) words[base + __popc(vote & ((1u << lane) - 1u))] = w;
+            }
+        }
+    }
+}
+
+// Undo what k_bins of the previous step left behind (bitmask words and cell -> first-marker
+// entries), so neither needs a full-lattice memset per step.
+__global__ void __launch_bounds__(256)
+k_clear_prev(const unsigned *__restrict__ skey_prev, const int *__restrict__ n_prev, int *__restrict__ bin_first,
+             unsigned *__restrict__ amask, const int *__restrict__ words, const int *__restrict__ n_words)
+{
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int stride = gridDim.x * blockDim.x;
+    const int np = *n_prev, nw = *n_words;
+    for (int i = tid; i < np; i += stride) bin_first[skey_prev[i]] = -1;
+    for (int i = tid; i < nw; i += stride) amask[words[i]] = 0u;
+}
+
+// device scalars: mode bit 0: step_ctr = step; bit 1: n_prev = n_prev_val; bit 2: step_ctr += 1
+__global__ void k_set_scalars(long long *step_ctr, long long step, int *n_prev, int n_prev_val, int mode)
+{
+    if (mode & 1) *step_ctr = step;
+    if (mode & 2) *n_prev = n_prev_val;
+    if (mode & 4) *step_ctr += 1;
+}
+
+// Peskin 4-point weights of the cells c-1, c, c+1, c+2 for a point at c + f, 0 <= f < 1 (R6).
+// The four distances 1+f, f, 1-f, 2-f share one square root: 1 + 4r - 4r^2 at r = f or 1-f and
+// -7 + 12r - 4r^2 at r = 1+f or 2-f all equal 1 + 4f - 4f^2.
+__device__ __forceinline__ void peskin4(float f, float (&w)[4])
+{
+    const float q = sqrtf(fmaf(4.0f * f, 1.0f - f, 1.0f));
+    const float a = 3.0f - 2.0f * f, b = 1.0f + 2.0f * f;
+    w[0] = 0.125f * (a - q);
+    w[1] = 0.125f * (a + q);
+    w[2] = 0.125f * (b + q);
+    w[3] = 0.125f * (b - q);
+}
+
+// a5 + a6, thread-per-marker variant over the sorted markers: u^m(k) = sum U^m W;
+// g = u_k - u^m(k); Delta u += s g (R9).
+__global__ void __launch_bounds__(128)
+k_interp_correct(const unsigned *__restrict__ skey, int n, Geom g, const float4 *__restrict__ U, MarkerSorted m)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int cx, cy, cz;
+    key_to_cell(skey[i], g, cx, cy, cz);
+    const float4 fs = m.fs[i];
+    float wx[4], wy[4], wz[4];
+    peskin4(fs.x, wx);
+    peskin4(fs.y, wy);
+    peskin4(fs.z, wz);
+    int xs[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) xs[j] = wrap(cx - 1 + j, g.nx);
+    float ux = 0.f, uy = 0.f, uz = 0.f;
+#pragma unroll
+    for (int jz = 0; jz < 4; ++jz) {
+        const int z = wrap(cz - 1 + jz, g.nz);
+#pragma unroll
+        for (int jy = 0; jy < 4; ++jy) {
+            const int y = wrap(cy - 1 + jy, g.ny);
+            const float wyz = wy[jy] * wz[jz];
+            const float4 *row = U + (size_t)(z * g.ny + y) * g.nx;
+#pragma unroll
+            for (int jx = 0; jx < 4; ++jx) {
+                const float4 v = row[xs[jx]];
+                const float w = wx[jx] * wyz;
+                ux = fmaf(v.x, w, ux);
+                uy = fmaf(v.y, w, uy);
+                uz = fmaf(v.z, w, uz);
+            }
+        }
+    }
+    const float4 uk = m.uk[i];
+    const float gx = uk.x - ux, gy = uk.y - uy, gz = uk.z - uz;
+    float4 du = m.du[i];
+    du.x = fmaf(fs.w, gx, du.x);
+    du.y = fmaf(fs.w, gy, du.y);
+    du.z = fmaf(fs.w, gz, du.z);
+    m.du[i] = du;
+    m.sg[i] = make_float4(fs.w * gx, fs.w * gy, fs.w * gz, 0.f);
+}
+
+// weight of the cell at offset j (0..3 <-> c-1..c+2) only
+__device__ __forceinline__ float peskin1(float f, int j)
+{
+    const float q = sqrtf(fmaf(4.0f * f, 1.0f - f, 1.0f));
+    const float lin = (j < 2) ? (3.0f - 2.0f * f) : (1.0f + 2.0f * f);
+    const float sq = (j == 1 || j == 2) ? q : -q;
+    return 0.125f * (lin + sq);
+}
+
+// a7, deterministic gather-by-cell (reference variant): one warp per active word, one lane per
+// active cell.  The cell visits the 4x4x4 bins whose stencils reach it in a fixed order and, inside
+// a bin, the markers in sorted order, so the sum is order-fixed and free of atomics.
+//   LAST = false:  U^{m+1}(X) = U^m(X) + sum_k s_k g_k W_k(X)      (R8)
+//   LAST = true :  G(X) = sum_k Delta u_k W_k(X)                    (R10, R11)
+template <bool LAST>
+__global__ void __launch_bounds__(256)
+k_spread_gather(const unsigned *__restrict__ skey, int n, Geom g, const int *__restrict__ bin_first,
+                const unsigned *__restrict__ amask, const int *__restrict__ words, const int *__restrict__ n_words,
+                const float4 *__restrict__ fs, const float4 *__restrict__ val, float4 *__restrict__ field)
+{
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    const int nw = *n_words;
+    for (int k = warp; k < nw; k += nwarps) {
+        const int w = __ldg(words + k);
+        const unsigned bits = __ldg(amask + w);
+        if (!((bits >> lane) & 1u)) continue;
+        const int row = w / g.nxw;
+        const int x = (w - row * g.nxw) * 32 + lane;
+        const int z = row / g.ny, y = row - z * g.ny;
+        float sx = 0.f, sy = 0.f, sz = 0.f;
+        // marker cell c = X + 1 - j, j = stencil offset of X inside the marker's block
+#pragma unroll 1
+        for (int jz = 0; jz < 4; ++jz) {
+            int cz = z + 1 - jz;
+            if (g.wallz) { if (cz < 0 || cz >= g.nz) continue; } else cz = wrap(cz, g.nz);
+#pragma unroll 1
+            for (int jy = 0; jy < 4; ++jy) {
+                int cy = y + 1 - jy;
+                if (g.wally) { if (cy < 0 || cy >= g.ny) continue; } else cy = wrap(cy, g.ny);
+#pragma unroll 1
+                for (int jx = 0; jx < 4; ++jx) {
+                    int cx = x + 1 - jx;
+                    if (g.wallx) { if (cx < 0 || cx >= g.nx) continue; } else cx = wrap(cx, g.nx);
+                    const unsigned ckey = (unsigned)((cz * g.ny + cy) * g.nx + cx);
+                    int i = bin_first[ckey];
+                    if (i < 0) continue;
+                    for (; i < n && skey[i] == ckey; ++i) {
+                        const float4 f = fs[i];
+                        const float4 v = val[i];
+                        const float wgt = peskin1(f.x, jx) * peskin1(f.y, jy) * peskin1(f.z, jz);
+                        sx = fmaf(v.x, wgt, sx);
+                        sy = fmaf(v.y, wgt, sy);
+                        sz = fmaf(v.z, wgt, sz);
+                    }
+                }
+            }
+        }
+        const size_t cell = (size_t)row * g.nx + x;
+        if (LAST) {
+            field[cell] = make_float4(sx, sy, sz, 0.f);
+        } else {
+            float4 u = field[cell];
+            u.x += sx; u.y += sy; u.z += sz;
+            field[cell] = u;
+        }
+    }
+}
+
+// a7, atomic variant (the paper's ib_force2 idea, kept as a measured comparison):
+// every marker adds its 64 contributions with global float atomics.  Not deterministic.
+__global__ void __launch_bounds__(128)
+k_spread_atomic(const unsigned *__restrict__ skey, int n, Geom g, const float4 *__restrict__ fs,
+                const float4 *__restrict__ val, float4 *__restrict__ field)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int cx, cy, cz;
+    key_to_cell(skey[i], g, cx, cy, cz);
+    const float4 f = fs[i];
+    const float4 v = val[i];
+    float wx[4], wy[4], wz[4];
+    peskin4(f.x, wx);
+    peskin4(f.y, wy);
+    peskin4(f.z, wz);
+#pragma unroll 1
+    for (int jz = 0; jz < 4; ++jz) {
+        const int z = wrap(cz - 1 + jz, g.nz);
+#pragma unroll 1
+        for (int jy = 0; jy < 4; ++jy) {
+            const int y = wrap(cy - 1 + jy, g.ny);
+            const float wyz = wy[jy] * wz[jz];
+            float *row = reinterpret_cast<float *>(field + (size_t)(z * g.ny + y) * g.nx);
+#pragma unroll
+            for (int jx = 0; jx < 4; ++jx) {
+                const int x = wrap(cx - 1 + jx, g.nx);
+                const float w = wx[jx] * wyz;
+                atomicAdd(row + 4 * x + 0, v.x * w);
+                atomicAdd(row + 4 * x + 1, v.y * w);
+                atomicAdd(row + 4 * x + 2, v.z * w);
+            }
+        }
+    }
+}
+
+// zero G on the active cells (needed before the atomic variant accumulates into it)
+__global__ void __launch_bounds__(256)
+k_zero_active(Geom g, const unsigned *__restrict__ amask, const int *__restrict__ words,
+              const int *__restrict__ n_words, float4 *__restrict__ field)
+{
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    const int nw = *n_words;
+    for (int k = warp; k < nw; k += nwarps) {
+        const int w = words[k];
+        if (!((amask[w] >> lane) & 1u)) continue;
+        const int row = w / g.nxw;
+        const int x = (w - row * g.nxw) * 32 + lane;
+        field[(size_t)row * g.nx + x] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+}
+
+// read-back helpers: scatter sorted per-marker data to the caller's original order
+__global__ void __launch_bounds__(256)
+k_read_markers(const unsigned *__restrict__ skey, const int *__restrict__ perm, int n, Geom g,
+               const float4 *__restrict__ fs, const float4 *__restrict__ du, float *__restrict__ pos,
+               float *__restrict__ force, int *__restrict__ cell)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int k = perm[i];
+    const unsigned key = skey[i];
+    if (pos) {
+        int cx, cy, cz;
+        key_to_cell(key, g, cx, cy, cz);
+        const float4 f = fs[i];
+        pos[3 * k + 0] = (float)cx + f.x;
+        pos[3 * k + 1] = (float)cy + f.y;
+        pos[3 * k + 2] = (float)cz + f.z;
+    }
+    if (force) {
+        const float4 d = du[i];
+        force[3 * k + 0] = d.x; force[3 * k + 1] = d.y; force[3 * k + 2] = d.z;
+    }
+    if (cell) cell[k] = (int)key;
+}
+
+}  // namespace lbmk

@@ -1,0 +1,741 @@
+// C-ABI library of the B200-native LBM-IBM time step (see include/lbm_ibm.h for the contract).
+// Host side: state, marshalling, launch sequencing and CUDA-graph replay.  Every arithmetic step
+// of the hot path runs in the kernels of lbm_kernels.cuh / ibm_kernels.cuh / sort_kernels.cuh.
+#include "../../include/lbm_ibm.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "ibm_kernels.cuh"
+#include "sort_kernels.cuh"
+
+using namespace lbmk;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return code;
+}
+
+#define CK(expr)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (expr);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(e_ == cudaErrorMemoryAllocation ? LBM_ENOMEM : LBM_ECUDA, "%s: %s (%s:%d)", \
+                        #expr, cudaGetErrorString(e_), __FILE__, __LINE__);                        \
+    } while (0)
+
+struct DevScalars {
+    long long step_ctr;  // time step n of the step being computed (kinematics angle)
+    int n_words;         // active words of the current / last IBM step
+    int n_prev;          // sorted markers whose bins are still registered in bin_first
+    int status;          // != 0: a stencil crossed a wall
+    int scratch;
+};
+
+struct HostBody {
+    long long first, count;
+    double omega, axis[3], center[3];
+    bool has_kin;
+};
+
+constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driven kernels
+
+}  // namespace
+
+struct lbm {
+    int device = 0;
+    cudaStream_t stream = nullptr;      // where work is enqueued
+    cudaStream_t cap_stream = nullptr;  // capture-only stream for building graphs
+    Geom g{};
+    CollisionConst cc{};
+    double tau = 1.0;
+    float *f[2] = {nullptr, nullptr};
+    int cur = 0;                        // f[cur] holds the post-collision state to pull from
+    float4 *U = nullptr, *G = nullptr;
+    unsigned *amask = nullptr;
+    int *words = nullptr, *bin_first = nullptr;
+    DevScalars *scal = nullptr;
+    long long steps_done = 0;
+    size_t n_mask_words = 0;
+    bool ibm_dirty = false;             // mask / bin_first hold entries of an earlier IBM step
+    bool force_valid = false;           // G + mask describe the last completed step
+
+    // markers: host mirror (caller order) and device copies
+    std::vector<float> h_pos, h_vel, h_area;   // [n][3], [n][3], [n]
+    std::vector<int> h_body;
+    std::vector<HostBody> bodies;
+    bool markers_stale = true;          // device copies / graphs need rebuilding
+    int nm = 0, nm_cap = 0, nb_cap = 0;
+    float *d_q[3] = {nullptr, nullptr, nullptr}, *d_v[3] = {nullptr, nullptr, nullptr}, *d_s = nullptr;
+    int *d_body = nullptr;
+    BodyDef *d_defs = nullptr;
+    BodyStep *d_tabs = nullptr;
+    unsigned *d_keys[2] = {nullptr, nullptr};
+    int *d_vals[2] = {nullptr, nullptr};
+    int *d_hist = nullptr, *d_total = nullptr;
+    MarkerSorted ms{nullptr, nullptr, nullptr, nullptr};
+    int sort_ipw = 64, sort_tiles = 0, sort_passes = 1;
+
+    int opt_spread = 0, opt_forcing = 0, opt_graph = 1, opt_lbm_kernel = 0, opt_interp = 0;
+    std::map<long long, std::pair<cudaGraphExec_t, int>> graphs;   // key -> (exec, kernel nodes)
+    long long launches = 0;
+    size_t dev_bytes = 0;
+};
+
+namespace {
+
+template <class T>
+int dmalloc(lbm *h, T **p, size_t count)
+{
+    *p = nullptr;
+    if (count == 0) return LBM_OK;
+    CK(cudaMalloc((void **)p, count * sizeof(T)));
+    h->dev_bytes += count * sizeof(T);
+    return LBM_OK;
+}
+template <class T>
+void dfree(lbm *h, T *&p, size_t count)
+{
+    if (p) { cudaFree(p); h->dev_bytes -= count * sizeof(T); }
+    p = nullptr;
+}
+
+bool is_device_ptr(const void *p)
+{
+    cudaPointerAttributes a{};
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+void drop_graphs(lbm *h)
+{
+    for (auto &kv : h->graphs) cudaGraphExecDestroy(kv.second.first);
+    h->graphs.clear();
+}
+
+void free_markers_dev(lbm *h)
+{
+    const size_t c = (size_t)h->nm_cap;
+    for (int a = 0; a < 3; ++a) { dfree(h, h->d_q[a], c); dfree(h, h->d_v[a], c); }
+    dfree(h, h->d_s, c);
+    dfree(h, h->d_body, c);
+    for (int a = 0; a < 2; ++a) { dfree(h, h->d_keys[a], c); dfree(h, h->d_vals[a], c); }
+    dfree(h, h->ms.fs, c); dfree(h, h->ms.uk, c); dfree(h, h->ms.sg, c); dfree(h, h->ms.du, c);
+    dfree(h, h->d_hist, (size_t)RADIX * (size_t)h->sort_tiles);
+    dfree(h, h->d_total, (size_t)RADIX);
+    dfree(h, h->d_defs, (size_t)h->nb_cap);
+    dfree(h, h->d_tabs, (size_t)h->nb_cap);
+    h->nm_cap = 0; h->nb_cap = 0; h->sort_tiles = 0;
+}
+
+dim3 cell_block(const Geom &g)
+{
+    int bx = g.nx >= 256 ? 256 : ((g.nx + 31) / 32) * 32;
+    int by = 256 / bx; if (by < 1) by = 1;
+    return dim3(bx, by, 1);
+}
+dim3 cell_grid(const Geom &g, dim3 b) { return dim3((g.nx + b.x - 1) / b.x, (g.ny + b.y - 1) / b.y, g.nz); }
+
+// ---- remove what the last IBM step registered in the dense maps (outside any graph) -----------
+int flush_ibm(lbm *h)
+{
+    if (!h->ibm_dirty) return LBM_OK;
+    const unsigned *skey = h->d_keys[h->sort_passes & 1];
+    k_clear_prev<<<LIST_GRID, 256, 0, h->stream>>>(skey, &h->scal->n_prev, h->bin_first, h->amask, h->words,
+                                                    &h->scal->n_words);
+    k_set_scalars<<<1, 1, 0, h->stream>>>(&h->scal->step_ctr, h->steps_done, &h->scal->n_prev, 0, 1 | 2);
+    CK(cudaMemsetAsync(&h->scal->n_words, 0, sizeof(int), h->stream));
+    CK(cudaGetLastError());
+    h->launches += 2;
+    h->ibm_dirty = false;
+    h->force_valid = false;
+    return LBM_OK;
+}
+
+// ---- (re)build the device copies of the markers -------------------------------------------------
+int upload_markers(lbm *h)
+{
+    if (!h->markers_stale) return LBM_OK;
+    int rc = flush_ibm(h);
+    if (rc) return rc;
+    CK(cudaStreamSynchronize(h->stream));
+    drop_graphs(h);
+    const int n = (int)h->h_area.size();
+    const int nb = (int)h->bodies.size();
+    if (n > h->nm_cap || nb > h->nb_cap) {
+        free_markers_dev(h);
+        const size_t c = (size_t)n;
+        for (int a = 0; a < 3; ++a) {
+            if ((rc = dmalloc(h, &h->d_q[a], c))) return rc;
+            if ((rc = dmalloc(h, &h->d_v[a], c))) return rc;
+        }
+        if ((rc = dmalloc(h, &h->d_s, c))) return rc;
+        if ((rc = dmalloc(h, &h->d_body, c))) return rc;
+        for (int a = 0; a < 2; ++a) {
+            if ((rc = dmalloc(h, &h->d_keys[a], c))) return rc;
+            if ((rc = dmalloc(h, &h->d_vals[a], c))) return rc;
+        }
+        if ((rc = dmalloc(h, &h->ms.fs, c))) return rc;
+        if ((rc = dmalloc(h, &h->ms.uk, c))) return rc;
+        if ((rc = dmalloc(h, &h->ms.sg, c))) return rc;
+        if ((rc = dmalloc(h, &h->ms.du, c))) return rc;
+        if ((rc = dmalloc(h, &h->d_total, (size_t)RADIX))) return rc;
+        if ((rc = dmalloc(h, &h->d_defs, (size_t)nb))) return rc;
+        if ((rc = dmalloc(h, &h->d_tabs, (size_t)nb))) return rc;
+        h->nm_cap = n; h->nb_cap = nb;
+    }
+    h->nm = n;
+    // sort geometry
+    int ipw = ((n / (148 * 32)) + 31) / 32 * 32;
+    if (ipw < 64) ipw = 64;
+    if (ipw > 2048) ipw = 2048;
+    const int tiles = n > 0 ? (n + ipw - 1) / ipw : 0;
+    if (tiles > h->sort_tiles) {
+        dfree(h, h->d_hist, (size_t)RADIX * (size_t)h->sort_tiles);
+        if ((rc = dmalloc(h, &h->d_hist, (size_t)RADIX * (size_t)tiles))) return rc;
+    }
+    h->sort_ipw = ipw; h->sort_tiles = tiles;
+    int bits = 1;
+    while (bits < 32 && ((long long)1 << bits) < h->g.cells) ++bits;
+    h->sort_passes = (bits + 7) / 8;
+    if (n == 0) { h->markers_stale = false; return LBM_OK; }
+
+    // body tables; rest positions relative to the body centre, formed in fp64
+    std::vector<BodyDef> defs((size_t)nb);
+    std::vector<float> q[3], v[3];
+    for (int a = 0; a < 3; ++a) { q[a].resize((size_t)n); v[a].resize((size_t)n); }
+    for (int b = 0; b < nb; ++b) {
+        const HostBody &B = h->bodies[(size_t)b];
+        BodyDef d{};
+        d.omega = B.omega; d.ax = B.axis[0]; d.ay = B.axis[1]; d.az = B.axis[2];
+        for (int a = 0; a < 3; ++a) {
+            const double fl = std::floor(B.center[a]);
+            d.ci[a] = (int)fl;
+            d.cf[a] = (float)(B.center[a] - fl);
+            if (d.cf[a] >= 1.0f) { d.cf[a] = 0.0f; d.ci[a] += 1; }
+        }
+        defs[(size_t)b] = d;
+        for (long long k = B.first; k < B.first + B.count; ++k)
+            for (int a = 0; a < 3; ++a) {
+                q[a][(size_t)k] = (float)((double)h->h_pos[(size_t)(3 * k + a)] - B.center[a]);
+                v[a][(size_t)k] = h->h_vel[(size_t)(3 * k + a)];
+            }
+    }
+    for (int a = 0; a < 3; ++a) {
+        CK(cudaMemcpyAsync(h->d_q[a], q[a].data(), sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, h->stream));
+        CK(cudaMemcpyAsync(h->d_v[a], v[a].data(), sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, h->stream));
+    }
+    CK(cudaMemcpyAsync(h->d_s, h->h_area.data(), sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaMemcpyAsync(h->d_body, h->h_body.data(), sizeof(int) * (size_t)n, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaMemcpyAsync(h->d_defs, defs.data(), sizeof(BodyDef) * (size_t)nb, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaStreamSynchronize(h->stream));   // staging vectors die here
+    h->markers_stale = false;
+    return LBM_OK;
+}
+
+// ---- enqueue one time step on stream s (plain launches; also what graph capture records) -------
+int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, int *n_kernels)
+{
+    const float *src = h->f[parity];
+    float *dst = h->f[parity ^ 1];
+    const Geom &g = h->g;
+    int nk = 0;
+    if (ibm) {
+        const int n = h->nm;
+        const int mb = (n + 255) / 256;
+        DevScalars *sc = h->scal;
+        unsigned *skey = h->d_keys[h->sort_passes & 1];
+        int *perm = h->d_vals[h->sort_passes & 1];
+        MarkerIn mi{h->d_q[0], h->d_q[1], h->d_q[2], h->d_v[0], h->d_v[1], h->d_v[2], h->d_s, h->d_body, n};
+
+        k_clear_prev<<<LIST_GRID, 256, 0, s>>>(skey, &sc->n_prev, h->bin_first, h->amask, h->words, &sc->n_words);
+        const int nb = (int)h->bodies.size();
+        k_kinematics<<<(nb + 127) / 128, 128, 0, s>>>(h->d_defs, h->d_tabs, nb, &sc->step_ctr, &sc->n_words);
+        k_marker_keys<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, h->d_keys[0], &sc->status);
+        nk += 3;
+        const int sb = (h->sort_tiles + SORT_WARPS - 1) / SORT_WARPS;
+        for (int p = 0; p < h->sort_passes; ++p) {
+            const unsigned *kin = h->d_keys[p & 1];
+            unsigned *kout = h->d_keys[(p + 1) & 1];
+            const int *vin = p == 0 ? nullptr : h->d_vals[p & 1];
+            int *vout = h->d_vals[(p + 1) & 1];
+            k_radix_hist<<<sb, SORT_BLOCK, 0, s>>>(kin, n, h->sort_ipw, h->sort_tiles, 8 * p, h->d_hist);
+            k_radix_scan<<<RADIX, SORT_BLOCK, 0, s>>>(h->d_hist, h->sort_tiles, h->d_total);
+            k_radix_scatter<<<sb, SORT_BLOCK, 0, s>>>(kin, vin, kout, vout, n, h->sort_ipw, h->sort_tiles, 8 * p,
+                                                       h->d_hist, h->d_total);
+            nk += 3;
+        }
+        k_marker_gather<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, perm, h->ms);
+        k_bins<<<mb, 256, 0, s>>>(skey, n, g, h->bin_first, h->amask, h->words, &sc->n_words);
+        k_set_scalars<<<1, 1, 0, s>>>(&sc->step_ctr, 0, &sc->n_prev, n, 2 | 4);
+        k_moments_active<<<LIST_GRID, 256, 0, s>>>(src, g, h->amask, h->words, &sc->n_words, h->U);
+        nk += 4;
+        for (int m = 0; m < mdf_iters; ++m) {
+            const bool last = (m == mdf_iters - 1);
+            k_interp_correct<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, h->U, h->ms);
+            ++nk;
+            if (h->opt_spread == 0) {
+                if (last)
+                    k_spread_gather<true><<<LIST_GRID, 256, 0, s>>>(skey, n, g, h->bin_first, h->amask, h->words,
+                                                                     &sc->n_words, h->ms.fs, h->ms.du, h->G);
+                else
+                    k_spread_gather<false><<<LIST_GRID, 256, 0, s>>>(skey, n, g, h->bin_first, h->amask, h->words,
+                                                                      &sc->n_words, h->ms.fs, h->ms.sg, h->U);
+                ++nk;
+            } else {
+                if (last) {
+                    k_zero_active<<<LIST_GRID, 256, 0, s>>>(g, h->amask, h->words, &sc->n_words, h->G);
+                    k_spread_atomic<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, h->ms.fs, h->ms.du, h->G);
+                    nk += 2;
+                } else {
+                    k_spread_atomic<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, h->ms.fs, h->ms.sg, h->U);
+                    ++nk;
+                }
+            }
+        }
+    }
+    CollisionConst cc = h->cc;
+    cc.shift_forcing = h->opt_forcing;
+    const bool vec = (h->opt_lbm_kernel == 0) && (g.nx % 4 == 0);
+    if (vec) {
+        const int nx4 = g.nx / 4;
+        int bx = 1;
+        while (bx < nx4 && bx < 64) bx <<= 1;
+        dim3 b(bx, 256 / bx, 1);
+        dim3 gr((nx4 + b.x - 1) / b.x, (g.ny + b.y - 1) / b.y, g.nz);
+        if (ibm) k_stream_collide_vec4<true><<<gr, b, 0, s>>>(src, dst, g, cc, h->amask, h->G);
+        else k_stream_collide_vec4<false><<<gr, b, 0, s>>>(src, dst, g, cc, nullptr, nullptr);
+    } else {
+        dim3 b = cell_block(g);
+        dim3 gr = cell_grid(g, b);
+        if (ibm) k_stream_collide_scalar<true><<<gr, b, 0, s>>>(src, dst, g, cc, h->amask, h->G);
+        else k_stream_collide_scalar<false><<<gr, b, 0, s>>>(src, dst, g, cc, nullptr, nullptr);
+    }
+    ++nk;
+    CK(cudaGetLastError());
+    *n_kernels = nk;
+    return LBM_OK;
+}
+
+int get_graph(lbm *h, int parity, int mdf_iters, bool ibm, cudaGraphExec_t *exec, int *n_kernels)
+{
+    const long long key = ((long long)mdf_iters << 8) | (ibm ? 2 : 0) | parity | ((long long)h->opt_spread << 40) |
+                          ((long long)h->opt_forcing << 44) | ((long long)h->opt_lbm_kernel << 48) |
+                          ((long long)h->opt_interp << 52);
+    auto it = h->graphs.find(key);
+    if (it != h->graphs.end()) { *exec = it->second.first; *n_kernels = it->second.second; return LBM_OK; }
+    cudaGraph_t graph = nullptr;
+    CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+    int nk = 0;
+    int rc = enqueue_step(h, h->cap_stream, parity, mdf_iters, ibm, &nk);
+    cudaError_t e = cudaStreamEndCapture(h->cap_stream, &graph);
+    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) return fail(LBM_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
+    cudaGraphExec_t ex = nullptr;
+    e = cudaGraphInstantiate(&ex, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) return fail(LBM_ECUDA, "graph instantiate failed: %s", cudaGetErrorString(e));
+    h->graphs[key] = std::make_pair(ex, nk);
+    *exec = ex; *n_kernels = nk;
+    return LBM_OK;
+}
+
+// copy caller data (host or device) into a host vector
+int to_host(const float *src, size_t count, std::vector<float> &dst)
+{
+    dst.resize(count);
+    if (count == 0) return LBM_OK;
+    if (is_device_ptr(src)) CK(cudaMemcpy(dst.data(), src, count * sizeof(float), cudaMemcpyDeviceToHost));
+    else std::memcpy(dst.data(), src, count * sizeof(float));
+    return LBM_OK;
+}
+
+// R17: the 4-cell stencil floor(x)-1 .. floor(x)+2 must stay inside 0..n-1 on wall axes
+bool stencil_inside(const lbm *h, const double lo[3], const double hi[3])
+{
+    const int n[3] = {h->g.nx, h->g.ny, h->g.nz};
+    const int wall[3] = {h->g.wallx, h->g.wally, h->g.wallz};
+    for (int a = 0; a < 3; ++a) {
+        if (!wall[a]) continue;
+        if (std::floor(lo[a]) < 1.0 || std::floor(hi[a]) > (double)(n[a] - 3)) return false;
+    }
+    return true;
+}
+
+__global__ void k_count_active(const unsigned *amask, const int *words, const int *n_words, int *out)
+{
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    int c = 0;
+    for (int i = tid; i < *n_words; i += gridDim.x * blockDim.x) c += __popc(amask[words[i]]);
+    if (c) atomicAdd(out, c);
+}
+
+}  // namespace
+
+// =================================================================================================
+extern "C" {
+
+const char *lbm_last_error(void) { return g_err.c_str(); }
+
+lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || !(tau > 0.5) || !std::isfinite(tau)) {
+        fail(LBM_EINVAL, "lbm_create: need nx,ny,nz >= 1 and tau > 0.5 (got %d %d %d %g)", nx, ny, nz, tau);
+        return nullptr;
+    }
+    if ((long long)nx * ny * nz > 0x7fffffffLL / 2) {
+        fail(LBM_EINVAL, "lbm_create: lattice too large for 32-bit cell keys");
+        return nullptr;
+    }
+    lbm *h = new (std::nothrow) lbm();
+    if (!h) { fail(LBM_ENOMEM, "lbm_create: host allocation failed"); return nullptr; }
+    auto bail = [&](const char *what) -> lbm_t * {
+        std::string msg = g_err;
+        lbm_destroy(h);
+        fail(LBM_ENOMEM, "lbm_create: %s: %s", what, msg.c_str());
+        return nullptr;
+    };
+    if (cudaGetDevice(&h->device) != cudaSuccess) return bail("no CUDA device");
+    h->g.nx = nx; h->g.ny = ny; h->g.nz = nz;
+    h->g.nxw = (nx + 31) / 32;
+    h->g.cells = (long long)nx * ny * nz;
+    h->g.wallx = bc ? (bc->wall_x != 0) : 0;
+    h->g.wally = bc ? (bc->wall_y != 0) : 0;
+    h->g.wallz = bc ? (bc->wall_z != 0) : 0;
+    h->tau = tau;
+    h->cc.omega = (float)(1.0 / tau);
+    h->cc.keep = (float)(1.0 - 1.0 / tau);
+    h->cc.guo = (float)(1.0 - 0.5 / tau);
+    h->cc.tau = (float)tau;
+    h->cc.gbx = bc ? (float)bc->gx : 0.f;
+    h->cc.gby = bc ? (float)bc->gy : 0.f;
+    h->cc.gbz = bc ? (float)bc->gz : 0.f;
+    h->cc.shift_forcing = 0;
+    const size_t cells = (size_t)h->g.cells;
+    h->n_mask_words = (size_t)h->g.nxw * ny * nz;
+    if (cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return bail("stream");
+    if (dmalloc(h, &h->f[0], cells * NQ) || dmalloc(h, &h->f[1], cells * NQ)) return bail("populations");
+    if (dmalloc(h, &h->U, cells) || dmalloc(h, &h->G, cells)) return bail("U/G fields");
+    if (dmalloc(h, &h->amask, h->n_mask_words) || dmalloc(h, &h->words, h->n_mask_words)) return bail("active mask");
+    if (dmalloc(h, &h->bin_first, cells)) return bail("bin map");
+    if (dmalloc(h, &h->scal, (size_t)1)) return bail("scalars");
+    bool ok = true;
+    ok &= cudaMemset(h->f[0], 0, cells * NQ * sizeof(float)) == cudaSuccess;   // rest state: f_i - t_i = 0
+    ok &= cudaMemset(h->f[1], 0, cells * NQ * sizeof(float)) == cudaSuccess;
+    ok &= cudaMemset(h->amask, 0, h->n_mask_words * sizeof(unsigned)) == cudaSuccess;
+    ok &= cudaMemset(h->bin_first, 0xff, cells * sizeof(int)) == cudaSuccess;
+    ok &= cudaMemset(h->scal, 0, sizeof(DevScalars)) == cudaSuccess;
+    ok &= cudaDeviceSynchronize() == cudaSuccess;
+    if (!ok) { fail(LBM_ECUDA, "%s", cudaGetErrorString(cudaGetLastError())); return bail("memset"); }
+    g_err.clear();
+    return h;
+}
+
+void lbm_destroy(lbm_t *h)
+{
+    if (!h) return;
+    cudaDeviceSynchronize();
+    drop_graphs(h);
+    free_markers_dev(h);
+    cudaFree(h->f[0]); cudaFree(h->f[1]); cudaFree(h->U); cudaFree(h->G);
+    cudaFree(h->amask); cudaFree(h->words); cudaFree(h->bin_first); cudaFree(h->scal);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    delete h;
+}
+
+int lbm_set_stream(lbm_t *h, void *cuda_stream)
+{
+    if (!h) return fail(LBM_EINVAL, "lbm_set_stream: NULL handle");
+    if (h->stream != (cudaStream_t)cuda_stream) CK(cudaStreamSynchronize(h->stream));
+    h->stream = (cudaStream_t)cuda_stream;
+    return LBM_OK;
+}
+
+int lbm_set_option(lbm_t *h, int key, int value)
+{
+    if (!h) return fail(LBM_EINVAL, "lbm_set_option: NULL handle");
+    switch (key) {
+        case LBM_OPT_SPREAD: if (value < 0 || value > 1) break; h->opt_spread = value; return LBM_OK;
+        case LBM_OPT_FORCING: if (value < 0 || value > 1) break; h->opt_forcing = value; return LBM_OK;
+        case LBM_OPT_GRAPH: if (value < 0 || value > 1) break; h->opt_graph = value; return LBM_OK;
+        case LBM_OPT_LBM_KERNEL: if (value < 0 || value > 1) break; h->opt_lbm_kernel = value; return LBM_OK;
+        case LBM_OPT_INTERP: if (value < 0 || value > 1) break; h->opt_interp = value; return LBM_OK;
+        default: return fail(LBM_EINVAL, "lbm_set_option: unknown key %d", key);
+    }
+    return fail(LBM_EINVAL, "lbm_set_option: value %d out of range for key %d", value, key);
+}
+
+int lbm_get_info(lbm_t *h, int key, long long *value)
+{
+    if (!h || !value) return fail(LBM_EINVAL, "lbm_get_info: NULL argument");
+    switch (key) {
+        case LBM_INFO_MARKERS: *value = (long long)h->h_area.size(); return LBM_OK;
+        case LBM_INFO_BODIES: *value = (long long)h->bodies.size(); return LBM_OK;
+        case LBM_INFO_STEPS: *value = h->steps_done; return LBM_OK;
+        case LBM_INFO_LAUNCHES: *value = h->launches; return LBM_OK;
+        case LBM_INFO_DEVICE_BYTES: *value = (long long)h->dev_bytes; return LBM_OK;
+        case LBM_INFO_ACTIVE_CELLS: {
+            int r = 0;
+            if (h->force_valid) {
+                CK(cudaMemsetAsync(&h->scal->scratch, 0, sizeof(int), h->stream));
+                k_count_active<<<256, 256, 0, h->stream>>>(h->amask, h->words, &h->scal->n_words, &h->scal->scratch);
+                CK(cudaMemcpyAsync(&r, &h->scal->scratch, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+                CK(cudaStreamSynchronize(h->stream));
+            }
+            *value = r;
+            return LBM_OK;
+        }
+        case LBM_INFO_STATUS: {
+            int st = 0;
+            CK(cudaMemcpyAsync(&st, &h->scal->status, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+            CK(cudaStreamSynchronize(h->stream));
+            *value = st;
+            return LBM_OK;
+        }
+        default: return fail(LBM_EINVAL, "lbm_get_info: unknown key %d", key);
+    }
+}
+
+int lbm_set_fields(lbm_t *h, const float *rho, const float *u)
+{
+    if (!h) return fail(LBM_EINVAL, "lbm_set_fields: NULL handle");
+    int rc = flush_ibm(h);
+    if (rc) return rc;
+    const size_t cells = (size_t)h->g.cells;
+    float *d_rho = nullptr, *d_u = nullptr;
+    const float *p_rho = rho, *p_u = u;
+    if (rho && !is_device_ptr(rho)) {
+        CK(cudaMalloc((void **)&d_rho, cells * sizeof(float)));
+        CK(cudaMemcpyAsync(d_rho, rho, cells * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+        p_rho = d_rho;
+    }
+    if (u && !is_device_ptr(u)) {
+        CK(cudaMalloc((void **)&d_u, 3 * cells * sizeof(float)));
+        CK(cudaMemcpyAsync(d_u, u, 3 * cells * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+        p_u = d_u;
+    }
+    dim3 b = cell_block(h->g);
+    k_init_fields<<<cell_grid(h->g, b), b, 0, h->stream>>>(h->f[h->cur], h->g, p_rho, p_u);
+    h->launches += 1;
+    cudaError_t e = cudaStreamSynchronize(h->stream);
+    if (d_rho) cudaFree(d_rho);
+    if (d_u) cudaFree(d_u);
+    if (e != cudaSuccess) return fail(LBM_ECUDA, "lbm_set_fields: %s", cudaGetErrorString(e));
+    h->steps_done = 0;
+    h->force_valid = false;
+    return LBM_OK;
+}
+
+int ibm_set_markers(lbm_t *h, const float *pos, const float *vel, const float *area, long long n)
+{
+    if (!h) return fail(LBM_EINVAL, "ibm_set_markers: NULL handle");
+    if (n < 0 || (n > 0 && (!pos || !area))) return fail(LBM_EINVAL, "ibm_set_markers: bad arguments");
+    if ((long long)h->h_area.size() + n > 0x7fffffffLL / 4) return fail(LBM_EINVAL, "ibm_set_markers: too many markers");
+    if (n > 0 && (h->g.nx < 4 || h->g.ny < 4 || h->g.nz < 4))
+        return fail(LBM_EINVAL, "ibm_set_markers: the lattice must be at least 4 cells wide on every axis");
+    std::vector<float> p, v, s;
+    int rc;
+    if ((rc = to_host(pos, (size_t)(3 * n), p))) return rc;
+    if ((rc = to_host(area, (size_t)n, s))) return rc;
+    if (vel) { if ((rc = to_host(vel, (size_t)(3 * n), v))) return rc; }
+    else v.assign((size_t)(3 * n), 0.f);
+    // static body until ibm_set_kinematics: centre := centroid (only used to keep fp32 offsets small)
+    HostBody B{};
+    B.first = (long long)h->h_area.size(); B.count = n; B.omega = 0.0;
+    B.axis[0] = 0.0; B.axis[1] = 0.0; B.axis[2] = 1.0; B.has_kin = false;
+    double c[3] = {0, 0, 0};
+    for (long long k = 0; k < n; ++k) {
+        double x[3] = {p[(size_t)(3 * k)], p[(size_t)(3 * k + 1)], p[(size_t)(3 * k + 2)]};
+        if (!std::isfinite(x[0]) || !std::isfinite(x[1]) || !std::isfinite(x[2]) || !std::isfinite(s[(size_t)k]))
+            return fail(LBM_EINVAL, "ibm_set_markers: non-finite input at marker %lld", k);
+        if (!stencil_inside(h, x, x))
+            return fail(LBM_ERANGE, "ibm_set_markers: stencil of marker %lld (%.3f %.3f %.3f) crosses a wall", k,
+                        x[0], x[1], x[2]);
+        for (int a = 0; a < 3; ++a) c[a] += x[a];
+    }
+    for (int a = 0; a < 3; ++a) B.center[a] = n > 0 ? c[a] / (double)n : 0.0;
+    h->h_pos.insert(h->h_pos.end(), p.begin(), p.end());
+    h->h_vel.insert(h->h_vel.end(), v.begin(), v.end());
+    h->h_area.insert(h->h_area.end(), s.begin(), s.end());
+    h->h_body.insert(h->h_body.end(), (size_t)n, (int)h->bodies.size());
+    h->bodies.push_back(B);
+    h->markers_stale = true;
+    return (int)h->bodies.size() - 1;
+}
+
+int ibm_set_kinematics(lbm_t *h, double omega, const double *axis, const double *center)
+{
+    if (!h || !axis || !center) return fail(LBM_EINVAL, "ibm_set_kinematics: NULL argument");
+    if (h->bodies.empty()) return fail(LBM_ESTATE, "ibm_set_kinematics: no body defined yet");
+    const double nrm = std::sqrt(axis[0] * axis[0] + axis[1] * axis[1] + axis[2] * axis[2]);
+    if (!(nrm > 0.0) || !std::isfinite(nrm) || !std::isfinite(omega))
+        return fail(LBM_EINVAL, "ibm_set_kinematics: axis must be non-zero and finite");
+    HostBody &B = h->bodies.back();
+    if (omega != 0.0) {
+        // every point stays on a sphere of radius |p - c| about c
+        for (long long k = B.first; k < B.first + B.count; ++k) {
+            double r2 = 0.0;
+            for (int a = 0; a < 3; ++a) {
+                const double d = (double)h->h_pos[(size_t)(3 * k + a)] - center[a];
+                r2 += d * d;
+            }
+            const double r = std::sqrt(r2);
+            const double lo[3] = {center[0] - r, center[1] - r, center[2] - r};
+            const double hi[3] = {center[0] + r, center[1] + r, center[2] + r};
+            if (!stencil_inside(h, lo, hi))
+                return fail(LBM_ERANGE, "ibm_set_kinematics: marker %lld (radius %.3f) can reach a wall", k, r);
+        }
+    }
+    B.omega = omega;
+    for (int a = 0; a < 3; ++a) { B.axis[a] = axis[a] / nrm; B.center[a] = center[a]; }
+    B.has_kin = true;
+    h->markers_stale = true;
+    return LBM_OK;
+}
+
+int ibm_clear(lbm_t *h)
+{
+    if (!h) return fail(LBM_EINVAL, "ibm_clear: NULL handle");
+    int rc = flush_ibm(h);
+    if (rc) return rc;
+    h->h_pos.clear(); h->h_vel.clear(); h->h_area.clear(); h->h_body.clear(); h->bodies.clear();
+    h->markers_stale = true;
+    return LBM_OK;
+}
+
+int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
+{
+    if (!h) return fail(LBM_EINVAL, "lbm_ibm_step: NULL handle");
+    if (nsteps < 0 || mdf_iters < 0) return fail(LBM_EINVAL, "lbm_ibm_step: negative count");
+    if (nsteps == 0) return LBM_OK;
+    int rc = upload_markers(h);
+    if (rc) return rc;
+    const bool ibm = (h->nm > 0 && mdf_iters > 0);
+    if (!ibm) { if ((rc = flush_ibm(h))) return rc; }
+    if (ibm) {
+        k_set_scalars<<<1, 1, 0, h->stream>>>(&h->scal->step_ctr, h->steps_done, &h->scal->n_prev, 0, 1);
+        h->launches += 1;
+    }
+    for (int s = 0; s < nsteps; ++s) {
+        int nk = 0;
+        if (h->opt_graph) {
+            cudaGraphExec_t ex = nullptr;
+            if ((rc = get_graph(h, h->cur, mdf_iters, ibm, &ex, &nk))) return rc;
+            CK(cudaGraphLaunch(ex, h->stream));
+        } else {
+            if ((rc = enqueue_step(h, h->stream, h->cur, mdf_iters, ibm, &nk))) return rc;
+        }
+        h->launches += nk;
+        h->cur ^= 1;
+        h->steps_done += 1;
+        if (ibm) { h->ibm_dirty = true; h->force_valid = true; }
+    }
+    return LBM_OK;
+}
+
+int lbm_read_fields(lbm_t *h, float *rho, float *u, float *force)
+{
+    if (!h) return fail(LBM_EINVAL, "lbm_read_fields: NULL handle");
+    if (!rho && !u && !force) return LBM_OK;
+    const size_t cells = (size_t)h->g.cells;
+    float *out[3] = {rho, u, force};
+    const size_t cnt[3] = {cells, 3 * cells, 3 * cells};
+    float *dev[3] = {nullptr, nullptr, nullptr};
+    bool tmp[3] = {false, false, false};
+    for (int a = 0; a < 3; ++a) {
+        if (!out[a]) continue;
+        if (is_device_ptr(out[a])) dev[a] = out[a];
+        else {
+            if (cudaMalloc((void **)&dev[a], cnt[a] * sizeof(float)) != cudaSuccess) {
+                for (int b = 0; b < a; ++b) if (tmp[b]) cudaFree(dev[b]);
+                return fail(LBM_ENOMEM, "lbm_read_fields: staging allocation failed");
+            }
+            tmp[a] = true;
+        }
+    }
+    dim3 b = cell_block(h->g);
+    k_read_fields<<<cell_grid(h->g, b), b, 0, h->stream>>>(h->f[h->cur], h->g, h->force_valid ? h->amask : nullptr,
+                                                            h->G, dev[0], dev[1], dev[2]);
+    h->launches += 1;
+    cudaError_t e = cudaGetLastError();
+    bool any_tmp = false;
+    for (int a = 0; a < 3 && e == cudaSuccess; ++a)
+        if (tmp[a]) {
+            any_tmp = true;
+            e = cudaMemcpyAsync(out[a], dev[a], cnt[a] * sizeof(float), cudaMemcpyDeviceToHost, h->stream);
+        }
+    if (any_tmp && e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    for (int a = 0; a < 3; ++a) if (tmp[a]) cudaFree(dev[a]);
+    if (e != cudaSuccess) return fail(LBM_ECUDA, "lbm_read_fields: %s", cudaGetErrorString(e));
+    return LBM_OK;
+}
+
+int ibm_read_markers(lbm_t *h, float *pos, float *force, int *perm, int *cell)
+{
+    if (!h) return fail(LBM_EINVAL, "ibm_read_markers: NULL handle");
+    const int n = (int)h->h_area.size();
+    if (n == 0 || (!pos && !force && !perm && !cell)) return LBM_OK;
+    if (!h->ibm_dirty || h->markers_stale)
+        return fail(LBM_ESTATE, "ibm_read_markers: no IBM step has been run with the current markers");
+    const unsigned *skey = h->d_keys[h->sort_passes & 1];
+    const int *dperm = h->d_vals[h->sort_passes & 1];
+    void *out[3] = {pos, force, cell};
+    const size_t bytes[3] = {sizeof(float) * 3 * (size_t)n, sizeof(float) * 3 * (size_t)n, sizeof(int) * (size_t)n};
+    void *dev[3] = {nullptr, nullptr, nullptr};
+    bool tmp[3] = {false, false, false};
+    for (int a = 0; a < 3; ++a) {
+        if (!out[a]) continue;
+        if (is_device_ptr(out[a])) dev[a] = out[a];
+        else { CK(cudaMalloc(&dev[a], bytes[a])); tmp[a] = true; }
+    }
+    k_read_markers<<<(n + 255) / 256, 256, 0, h->stream>>>(skey, dperm, n, h->g, h->ms.fs, h->ms.du, (float *)dev[0],
+                                                            (float *)dev[1], (int *)dev[2]);
+    h->launches += 1;
+    cudaError_t e = cudaGetLastError();
+    bool need_sync = false;
+    for (int a = 0; a < 3 && e == cudaSuccess; ++a)
+        if (tmp[a]) { need_sync = true; e = cudaMemcpyAsync(out[a], dev[a], bytes[a], cudaMemcpyDeviceToHost, h->stream); }
+    if (perm && e == cudaSuccess) {
+        const bool dv = is_device_ptr(perm);
+        e = cudaMemcpyAsync(perm, dperm, sizeof(int) * (size_t)n, dv ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost,
+                            h->stream);
+        need_sync |= !dv;
+    }
+    if (need_sync && e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    for (int a = 0; a < 3; ++a) if (tmp[a]) cudaFree(dev[a]);
+    if (e != cudaSuccess) return fail(LBM_ECUDA, "ibm_read_markers: %s", cudaGetErrorString(e));
+    return LBM_OK;
+}
+
+int lbm_sync(lbm_t *h)
+{
+    if (!h) return fail(LBM_EINVAL, "lbm_sync: NULL handle");
+    int st = 0;
+    CK(cudaMemcpyAsync(&st, &h->scal->status, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    if (st) {
+        CK(cudaMemsetAsync(&h->scal->status, 0, sizeof(int), h->stream));
+        return fail(LBM_ERANGE, "lbm_sync: a marker stencil crossed a wall face during the last steps");
+    }
+    return LBM_OK;
+}
+
+}  // extern "C"

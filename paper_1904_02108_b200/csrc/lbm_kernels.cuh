@@ -1,0 +1,301 @@
+// Lattice kernels: fused pull-stream + BGK collide + force (row a8 of SURVEY.md section 8),
+// moments on active cells (a4), field initialisation and canonical read-out (a9).
+//
+// Storage: two SoA buffers of 19 fp32 planes, plane i = df_i[z][y][x] (x fastest).  A buffer
+// holds POST-collision populations (R19); the canonical (post-stream, pre-collision) state of
+// P:31 is what a pull from that buffer yields:
+//     f_i(x, n+1) = f'_i(x - e_i)                       eq. (4), P:49 (indices wrapped if periodic)
+//     f_i(x, n+1) = f'_{opp i}(x)   if x - e_i lies behind a wall face (half-way bounce-back, R16)
+#pragma once
+#include "d3q19.cuh"
+
+namespace lbmk {
+
+struct Geom {
+    int nx, ny, nz;
+    int nxw;             // 32-cell words per x-row of the active-cell bitmask
+    long long cells;
+    int wallx, wally, wallz;
+};
+
+// The neighbourhood of one cell for the pull: wrapped neighbour coordinates and, per axis, whether
+// stepping -1 / +1 leaves the domain through a wall.
+struct Nbr {
+    int xm, xp, ym, yp, zm, zp;
+    bool wxm, wxp, wym, wyp, wzm, wzp;
+};
+
+__device__ __forceinline__ Nbr neighbours(const Geom &g, int x, int y, int z)
+{
+    Nbr n;
+    n.xm = (x == 0) ? g.nx - 1 : x - 1;
+    n.xp = (x == g.nx - 1) ? 0 : x + 1;
+    n.ym = (y == 0) ? g.ny - 1 : y - 1;
+    n.yp = (y == g.ny - 1) ? 0 : y + 1;
+    n.zm = (z == 0) ? g.nz - 1 : z - 1;
+    n.zp = (z == g.nz - 1) ? 0 : z + 1;
+    n.wxm = g.wallx && x == 0;
+    n.wxp = g.wallx && x == g.nx - 1;
+    n.wym = g.wally && y == 0;
+    n.wyp = g.wally && y == g.ny - 1;
+    n.wzm = g.wallz && z == 0;
+    n.wzp = g.wallz && z == g.nz - 1;
+    return n;
+}
+
+// Pull the 19 canonical populations of cell (x,y,z) out of a post-collision buffer.
+__device__ __forceinline__ void pull_cell(const float *__restrict__ src, const Geom &g, const Nbr &n, int x, int y,
+                                          int z, float (&df)[NQ])
+{
+    const size_t cells = (size_t)g.cells;
+    const int self = (z * g.ny + y) * g.nx + x;
+#pragma unroll
+    for (int i = 0; i < NQ; ++i) {
+        // source cell x - e_i
+        const int sx = dir_ex(i) == 1 ? n.xm : (dir_ex(i) == -1 ? n.xp : x);
+        const int sy = dir_ey(i) == 1 ? n.ym : (dir_ey(i) == -1 ? n.yp : y);
+        const int sz = dir_ez(i) == 1 ? n.zm : (dir_ez(i) == -1 ? n.zp : z);
+        bool behind_wall = false;
+        if (dir_ex(i) == 1) behind_wall |= n.wxm;
+        if (dir_ex(i) == -1) behind_wall |= n.wxp;
+        if (dir_ey(i) == 1) behind_wall |= n.wym;
+        if (dir_ey(i) == -1) behind_wall |= n.wyp;
+        if (dir_ez(i) == 1) behind_wall |= n.wzm;
+        if (dir_ez(i) == -1) behind_wall |= n.wzp;
+        const int cell = behind_wall ? self : (sz * g.ny + sy) * g.nx + sx;
+        const int plane = behind_wall ? dir_opp(i) : i;
+        df[i] = __ldg(src + (size_t)plane * cells + cell);
+    }
+}
+
+__device__ __forceinline__ bool cell_is_active(const unsigned *__restrict__ amask, const Geom &g, int x, int y, int z)
+{
+    const unsigned w = __ldg(amask + (size_t)(z * g.ny + y) * g.nxw + (x >> 5));
+    return (w >> (x & 31)) & 1u;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a8, scalar variant: one thread per cell, x along threadIdx.x (coalesced 128 B per warp and plane).
+// IBM = true reads one bitmask word per warp-row and G only where a marker stencil reaches.
+template <bool IBM>
+__global__ void __launch_bounds__(256)
+k_stream_collide_scalar(const float *__restrict__ src, float *__restrict__ dst, Geom g, CollisionConst cc,
+                        const unsigned *__restrict__ amask, const float4 *__restrict__ G)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= g.nx || y >= g.ny) return;
+
+    const Nbr n = neighbours(g, x, y, z);
+    float df[NQ];
+    pull_cell(src, g, n, x, y, z, df);
+
+    float ax = cc.gbx, ay = cc.gby, az = cc.gbz;
+    const int self = (z * g.ny + y) * g.nx + x;
+    if (IBM) {
+        if (cell_is_active(amask, g, x, y, z)) {
+            const float4 gv = __ldg(G + self);
+            ax += gv.x; ay += gv.y; az += gv.z;
+        }
+    }
+    collide(df, ax, ay, az, cc);
+    const size_t cells = (size_t)g.cells;
+#pragma unroll
+    for (int i = 0; i < NQ; ++i) __stcs(dst + (size_t)i * cells + self, df[i]);
+}
+
+// ---------------------------------------------------------------------------------------------
+// a8, vectorised variant: one thread per 4 consecutive x cells; every plane is read and written
+// with 128-bit accesses.  Directions with e_x = 0 are plain aligned float4 loads of the source
+// row; directions with e_x = +-1 need the row shifted by one cell: three of the four values come
+// from the thread's own aligned float4 and the fourth from the neighbouring lane's float4 via a
+// warp shuffle (lanes at a warp or row edge fetch that one value with a scalar load instead).
+// Requires nx % 4 == 0.
+template <bool IBM>
+__global__ void __launch_bounds__(256)
+k_stream_collide_vec4(const float *__restrict__ src, float *__restrict__ dst, Geom g, CollisionConst cc,
+                      const unsigned *__restrict__ amask, const float4 *__restrict__ G)
+{
+    const int nx4 = g.nx >> 2;
+    const int x4 = blockIdx.x * blockDim.x + threadIdx.x;   // index of the 4-cell group in the row
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    const bool live = (x4 < nx4) && (y < g.ny);
+    const size_t cells = (size_t)g.cells;
+    const unsigned lane = (threadIdx.y * blockDim.x + threadIdx.x) & 31u;
+
+    // clamp dead threads onto a valid cell so that shuffles stay convergent; they do not store
+    const int xg = live ? x4 : 0;
+    const int yy = live ? y : 0;
+    const int x0 = xg << 2;
+    const Nbr n = neighbours(g, x0, yy, z);   // y/z neighbours and wall flags of the row
+    const bool wall_lo = g.wallx && x0 == 0;             // cell x0 has the low-x wall behind it
+    const bool wall_hi = g.wallx && x0 + 4 == g.nx;      // cell x0+3 has the high-x wall behind it
+    const int self = (z * g.ny + yy) * g.nx + x0;
+
+    // do my lane neighbours hold the adjacent 4-cell groups of the same row?
+    const int lane_x4_dn = __shfl_up_sync(0xffffffffu, xg, 1);
+    const int lane_y_dn = __shfl_up_sync(0xffffffffu, yy, 1);
+    const int lane_x4_up = __shfl_down_sync(0xffffffffu, xg, 1);
+    const int lane_y_up = __shfl_down_sync(0xffffffffu, yy, 1);
+    const bool have_dn = lane > 0 && lane_x4_dn == xg - 1 && lane_y_dn == yy;
+    const bool have_up = lane < 31 && lane_x4_up == xg + 1 && lane_y_up == yy;
+
+    float df[4][NQ];
+#pragma unroll
+    for (int i = 0; i < NQ; ++i) {
+        const int sy = dir_ey(i) == 1 ? n.ym : (dir_ey(i) == -1 ? n.yp : yy);
+        const int sz = dir_ez(i) == 1 ? n.zm : (dir_ez(i) == -1 ? n.zp : z);
+        bool row_behind_wall = false;       // the whole source row lies behind a y or z wall
+        if (dir_ey(i) == 1) row_behind_wall |= n.wym;
+        if (dir_ey(i) == -1) row_behind_wall |= n.wyp;
+        if (dir_ez(i) == 1) row_behind_wall |= n.wzm;
+        if (dir_ez(i) == -1) row_behind_wall |= n.wzp;
+        if (dir_ex(i) == 0) {
+            const int cell = row_behind_wall ? self : (sz * g.ny + sy) * g.nx + x0;
+            const int plane = row_behind_wall ? dir_opp(i) : i;
+            const float4 v = __ldg(reinterpret_cast<const float4 *>(src + (size_t)plane * cells + cell));
+            df[0][i] = v.x; df[1][i] = v.y; df[2][i] = v.z; df[3][i] = v.w;
+        } else {
+            // bounce-back rows read plane opp(i) at the cell itself (no x shift); regular rows
+            // read plane i shifted by -e_x.
+            const int rowbase = row_behind_wall ? (z * g.ny + yy) * g.nx : (sz * g.ny + sy) * g.nx;
+            const int plane = row_behind_wall ? dir_opp(i) : i;
+            const float *__restrict__ p = src + (size_t)plane * cells + rowbase;
+            const float4 v = __ldg(reinterpret_cast<const float4 *>(p + x0));
+            if (dir_ex(i) == 1) {
+                // regular: cells x0..x0+3 take p[x0-1 .. x0+2]
+                float edge = __shfl_up_sync(0xffffffffu, v.w, 1);
+                if (!have_dn) edge = __ldg(p + n.xm);
+                float a0 = edge, a1 = v.x, a2 = v.y, a3 = v.z;
+                if (row_behind_wall) { a0 = v.x; a1 = v.y; a2 = v.z; a3 = v.w; }
+                else if (wall_lo) a0 = __ldg(src + (size_t)dir_opp(i) * cells + self);
+                df[0][i] = a0; df[1][i] = a1; df[2][i] = a2; df[3][i] = a3;
+            } else {
+                // regular: cells x0..x0+3 take p[x0+1 .. x0+4]
+                float edge = __shfl_down_sync(0xffffffffu, v.x, 1);
+                const int xp3 = (x0 + 4 == g.nx) ? 0 : x0 + 4;
+                if (!have_up) edge = __ldg(p + xp3);
+                float a0 = v.y, a1 = v.z, a2 = v.w, a3 = edge;
+                if (row_behind_wall) { a0 = v.x; a1 = v.y; a2 = v.z; a3 = v.w; }
+                else if (wall_hi) a3 = __ldg(src + (size_t)dir_opp(i) * cells + self + 3);
+                df[0][i] = a0; df[1][i] = a1; df[2][i] = a2; df[3][i] = a3;
+            }
+        }
+    }
+    if (!live) return;
+
+    float ax[4], ay[4], az[4];
+#pragma unroll
+    for (int c = 0; c < 4; ++c) { ax[c] = cc.gbx; ay[c] = cc.gby; az[c] = cc.gbz; }
+    if (IBM) {
+        const unsigned w = __ldg(amask + (size_t)(z * g.ny + yy) * g.nxw + (x0 >> 5));
+        const unsigned bits = (w >> (x0 & 31)) & 0xFu;
+        if (bits) {
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+                if ((bits >> c) & 1u) {
+                    const float4 gv = __ldg(G + self + c);
+                    ax[c] += gv.x; ay[c] += gv.y; az[c] += gv.z;
+                }
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c) collide(df[c], ax[c], ay[c], az[c], cc);
+#pragma unroll
+    for (int i = 0; i < NQ; ++i)
+        __stcs(reinterpret_cast<float4 *>(dst + (size_t)i * cells + self),
+               make_float4(df[0][i], df[1][i], df[2][i], df[3][i]));
+}
+
+// ---------------------------------------------------------------------------------------------
+// R18: f = Eq(rho0, u0) as the canonical state, stored so that the pull of the next step (and of
+// the read-out) recovers it: the value f_i(x) goes to plane i of cell x - e_i, or, when that cell
+// lies behind a wall, to plane opp(i) of x itself (the inverse of the two pull rules above).
+__global__ void __launch_bounds__(256)
+k_init_fields(float *__restrict__ buf, Geom g, const float *__restrict__ rho0, const float *__restrict__ u0)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= g.nx || y >= g.ny) return;
+    const size_t cells = (size_t)g.cells;
+    const int self = (z * g.ny + y) * g.nx + x;
+    const float drho = rho0 ? (rho0[self] - 1.0f) : 0.0f;
+    const float ux = u0 ? u0[self] : 0.0f;
+    const float uy = u0 ? u0[cells + self] : 0.0f;
+    const float uz = u0 ? u0[2 * cells + self] : 0.0f;
+    const Nbr n = neighbours(g, x, y, z);
+#pragma unroll
+    for (int i = 0; i < NQ; ++i) {
+        const int sx = dir_ex(i) == 1 ? n.xm : (dir_ex(i) == -1 ? n.xp : x);
+        const int sy = dir_ey(i) == 1 ? n.ym : (dir_ey(i) == -1 ? n.yp : y);
+        const int sz = dir_ez(i) == 1 ? n.zm : (dir_ez(i) == -1 ? n.zp : z);
+        bool behind_wall = false;
+        if (dir_ex(i) == 1) behind_wall |= n.wxm;
+        if (dir_ex(i) == -1) behind_wall |= n.wxp;
+        if (dir_ey(i) == 1) behind_wall |= n.wym;
+        if (dir_ey(i) == -1) behind_wall |= n.wyp;
+        if (dir_ez(i) == 1) behind_wall |= n.wzm;
+        if (dir_ez(i) == -1) behind_wall |= n.wzp;
+        const int cell = behind_wall ? self : (sz * g.ny + sy) * g.nx + sx;
+        const int plane = behind_wall ? dir_opp(i) : i;
+        buf[(size_t)plane * cells + cell] = equilibrium_dev(i, drho, ux, uy, uz);
+    }
+}
+
+// a9 / O8: canonical rho, bare U (eq. (1)) of every cell; force = G where a stencil reached in
+// the last step, zero elsewhere.  Output planes [nz][ny][nx]; any output may be NULL.
+__global__ void __launch_bounds__(256)
+k_read_fields(const float *__restrict__ src, Geom g, const unsigned *__restrict__ amask_last,
+              const float4 *__restrict__ G, float *__restrict__ rho, float *__restrict__ u, float *__restrict__ force)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= g.nx || y >= g.ny) return;
+    const size_t cells = (size_t)g.cells;
+    const int self = (z * g.ny + y) * g.nx + x;
+    if (rho || u) {
+        const Nbr n = neighbours(g, x, y, z);
+        float df[NQ], drho, ux, uy, uz;
+        pull_cell(src, g, n, x, y, z, df);
+        moments(df, drho, ux, uy, uz);
+        if (rho) rho[self] = 1.0f + drho;
+        if (u) { u[self] = ux; u[cells + self] = uy; u[2 * cells + self] = uz; }
+    }
+    if (force) {
+        float4 gv = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (amask_last && cell_is_active(amask_last, g, x, y, z)) gv = G[self];
+        force[self] = gv.x; force[cells + self] = gv.y; force[2 * cells + self] = gv.z;
+    }
+}
+
+// a4: rho, U of eq. (1) for the cells of the active words only (the paper's "kernel strategy",
+// P:215, de-duplicated): one warp per 32-cell word of the bitmask, lanes whose bit is set pull
+// their 19 populations.  U is stored as float4 (Ux, Uy, Uz, rho).
+__global__ void __launch_bounds__(256)
+k_moments_active(const float *__restrict__ src, Geom g, const unsigned *__restrict__ amask,
+                 const int *__restrict__ words, const int *__restrict__ n_words, float4 *__restrict__ U)
+{
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    const int nw = *n_words;
+    for (int k = warp; k < nw; k += nwarps) {
+        const int w = __ldg(words + k);
+        const unsigned bits = __ldg(amask + w);
+        if (!((bits >> lane) & 1u)) continue;
+        const int row = w / g.nxw;
+        const int x = (w - row * g.nxw) * 32 + lane;
+        const int z = row / g.ny, y = row - z * g.ny;
+        const Nbr n = neighbours(g, x, y, z);
+        float df[NQ], drho, ux, uy, uz;
+        pull_cell(src, g, n, x, y, z, df);
+        moments(df, drho, ux, uy, uz);
+        U[(size_t)row * g.nx + x] = make_float4(ux, uy, uz, 1.0f + drho);
+    }
+}
+
+}  // namespace lbmk
