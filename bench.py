@@ -1,0 +1,348 @@
+#!/usr/bin/env python
+"""bench.py -- coupled LBM-IBM MLUPS on one B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload W4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path: one time step of the coupled scheme (kinematics, marker
+sort + bins, moments on active cells, mdf_iters x (interpolate, correct, spread), fused
+stream-collide-force).  The default workload is W4 (BASELINE.json configs[3], 256^3 periodic, 64
+three-blade propellers, ~1.18 M markers, 5 MDF iterations): the coupled configuration on the same
+256^3 lattice as the pure-LBM bandwidth case configs[1] (W2), which is timed alongside and reported
+under "pure_lbm".  All inputs are seeded synthetic (paper_1904_02108_b200/workloads.py).
+
+N > 1: "replicas only": every rank runs the same workload on its own GPU, no data-path
+collective; value = units of all ranks / max-over-ranks time.
+
+--impl reference times the fp64 CPU oracle (oracle/) on the host cores on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "coupled LBM-IBM MLUPS"
+UNIT = "MLUPS"
+BYTES_PER_LUP = 152.0          # 19 fp32 loads + 19 fp32 stores per lattice update
+G_BYTES_PER_ACTIVE = 12.0      # G read on active cells
+NOMINAL_HBM_GBS = 8000.0       # north_star's denominator
+
+
+def measured_peak_gbs():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def traffic_from_profile(workload):
+    """dram bytes per launch of the stream-collide kernel from the committed ncu capture, or None"""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            return json.load(fh).get(workload)
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.QUERY}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            # under load = the upper half of the samples (the sampler also sees idle gaps)
+            s = sorted(sm)
+            out["sm_mhz"] = float(np.median(s[len(s) // 2:]))
+            out["sm_max_mhz"] = float(max(mx))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def time_steps(torch, sim, stream, steps, mdf):
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with torch.cuda.stream(stream):
+        e0.record(stream)
+        sim.step(steps, mdf)
+        e1.record(stream)
+    stream.synchronize()
+    return e0.elapsed_time(e1)          # ms
+
+
+def oracle_sample(workload_name, seed, budget_steps):
+    """The oracle as it stands on a bounded sample of the same workload (host cores)."""
+    import oracle
+    from paper_1904_02108_b200 import workloads
+    if workload_name in ("W4", "W4lit"):
+        wl = workloads.w4(seed, 8 if workload_name == "W4" else 1, n=128)
+        sample = f"{workload_name} recipe on a 128^3 box (8 propellers, {wl.n_markers} markers), {budget_steps} steps"
+    elif workload_name in ("W5", "W5lit"):
+        wl = workloads.w5(seed, 12 if workload_name == "W5" else 1, n=128)
+        sample = f"{workload_name} recipe on a 128^3 box ({len(wl.bodies)} propellers, {wl.n_markers} markers), {budget_steps} steps"
+    elif workload_name == "W2":
+        wl = workloads.w2(seed, n=128)
+        sample = f"W2 recipe on a 128^3 channel, {budget_steps} steps"
+    else:
+        wl = workloads.get(workload_name, seed)
+        sample = f"{workload_name} full size, {budget_steps} steps"
+    ref = oracle.from_workload(wl)
+    return ref, wl, sample
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cores = os.cpu_count() or 1
+    ref, wl, sample = oracle_sample(args.workload, args.seed, args.steps)
+    ref.step(args.warmup, wl.mdf_iters)
+    t0 = time.perf_counter()
+    ref.step(args.steps, wl.mdf_iters)
+    dt = time.perf_counter() - t0
+    mlups = wl.cells * args.steps / dt / 1e6
+    line = {
+        "impl": "reference", "metric": METRIC, "value": mlups, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded)",
+        "config": {"workload": args.workload, "sample": sample, "mdf_iters": wl.mdf_iters, "markers": wl.n_markers},
+        "cpu_baseline": {"value": mlups, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": mlups, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    if not torch.cuda.is_available():
+        print(json.dumps({"error": "no CUDA device: this library has no CPU fallback"}))
+        return 2
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
+
+    from paper_1904_02108_b200 import api, workloads
+    wl = workloads.get(args.workload, args.seed)
+    mdf = wl.mdf_iters
+    stream = torch.cuda.Stream()
+    sim = api.from_workload(wl, stream=stream)
+    if args.spread == "atomic":
+        sim.set_option(api.OPT_SPREAD, api.SPREAD_ATOMIC)
+    if args.lbm_kernel == "scalar":
+        sim.set_option(api.OPT_LBM_KERNEL, 1)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing (the headline `value`) ------------------------------------------
+    sim.step(args.warmup, mdf)
+    barrier()
+    l0 = sim.get_info(api.INFO_LAUNCHES)
+    sampler = ClockSampler(local) if rank == 0 else None
+    ms = time_steps(torch, sim, stream, args.steps, mdf)
+    barrier()
+    launches = sim.get_info(api.INFO_LAUNCHES) - l0
+    clocks = sampler.stop() if sampler else {}
+    sim.sync()
+    t = torch.tensor([ms], device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = world * wl.cells * args.steps / (ms * 1e-3) / 1e6
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic (seeded)",
+        "config": {"workload": wl.name, "lattice": [wl.nx, wl.ny, wl.nz], "tau": wl.tau, "markers": wl.n_markers,
+                   "bodies": len(wl.bodies), "mdf_iters": mdf, "spread": args.spread, "lbm_kernel": args.lbm_kernel,
+                   "parallelism": "replicas" if world > 1 else "single-gpu",
+                   "l2": "inputs larger than L2 (populations %.0f MB per buffer)" % (wl.cells * 76 / 1e6)},
+        "clocks": clocks, "gpu_launches": int(launches),
+    }
+
+    if rank == 0:
+        # ---- per-phase device time with CUDA events on the launching stream ----------------------
+        n_ph = max(3, min(args.steps, 20))
+        sim.set_option(api.OPT_TIMING, 1)
+        sim.step(n_ph, mdf)
+        ph = sim.phase_ms()
+        sim.set_option(api.OPT_TIMING, 0)
+        n_active = sim.get_info(api.INFO_ACTIVE_CELLS) if wl.n_markers else 0
+        lbm_ms = ph["lbm"] / n_ph
+        tot = sum(ph.values()) / n_ph
+        peak, how = measured_peak_gbs()
+        alg_bytes = BYTES_PER_LUP * wl.cells + G_BYTES_PER_ACTIVE * n_active
+        achieved = alg_bytes / (lbm_ms * 1e-3) / 1e9
+        line["roofline"] = {"bound": "hbm", "kernel": "k_stream_collide (a8)", "achieved": achieved, "peak": peak,
+                            "unit": "GB/s", "frac": achieved / peak, "traffic": traffic_from_profile(wl.name),
+                            "peak_source": how, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                            "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": lbm_ms}
+        line["phases_ms_per_step"] = {k: v / n_ph for k, v in ph.items()}
+        line["ibm_share"] = (tot - lbm_ms) / tot if tot > 0 else 0.0
+        line["active_cells"] = int(n_active)
+
+        # ---- pure LBM on the same lattice and on configs[1] (W2) ---------------------------------
+        sim.step(3, 0)
+        ms_p = time_steps(torch, sim, stream, args.steps, 0)
+        pure_same = wl.cells * args.steps / (ms_p * 1e-3) / 1e6
+        line["pure_lbm"] = {"same_lattice_mlups": pure_same,
+                            "frac_of_measured": pure_same * 1e6 * BYTES_PER_LUP / 1e9 / peak,
+                            "frac_of_nominal_8TBs": pure_same * 1e6 * BYTES_PER_LUP / 1e9 / NOMINAL_HBM_GBS,
+                            "coupled_over_pure": value / world / pure_same}
+        if wl.name != "W2" and not args.quick:
+            w2 = workloads.get("W2", args.seed)
+            s2 = api.from_workload(w2, stream=stream)
+            if args.lbm_kernel == "scalar":
+                s2.set_option(api.OPT_LBM_KERNEL, 1)
+            s2.step(max(3, args.warmup), 0)
+            stream.synchronize()
+            ms2 = time_steps(torch, s2, stream, args.steps, 0)
+            v2 = w2.cells * args.steps / (ms2 * 1e-3) / 1e6
+            line["pure_lbm"].update({"W2_mlups": v2, "W2_frac_of_measured": v2 * 1e6 * BYTES_PER_LUP / 1e9 / peak,
+                                     "W2_frac_of_nominal_8TBs": v2 * 1e6 * BYTES_PER_LUP / 1e9 / NOMINAL_HBM_GBS})
+            s2.close()
+            del s2
+
+    # ---- end to end through the public API with host buffers (all ranks) ---------------------------
+    # every step: H2D = the per-body kinematics table a host controller sets (ibm_update_kinematics),
+    # D2H = the marker forces Delta u(k) into pinned host memory (ibm_read_markers); the fields stay
+    # resident, as the method intends ("fully performed within the GPU's memory").
+    e2e_steps = max(3, min(args.steps, 20))
+    if wl.n_markers:
+        nb = len(wl.bodies)
+        om = np.array([b.omega for b in wl.bodies]); ax = np.stack([b.axis for b in wl.bodies])
+        force_host = torch.empty((wl.n_markers, 3), dtype=torch.float32, pin_memory=True)
+        out = {"force": force_host.numpy()}
+        h2d, d2h = nb * 56, wl.n_markers * 12
+
+        def e2e_step():
+            sim.update_kinematics(0, om, ax)
+            sim.step(1, mdf)
+            sim.read_markers(pos=False, perm=False, cell=False, out=out)
+    else:
+        rho_host = torch.empty((wl.nz, wl.ny, wl.nx), dtype=torch.float32, pin_memory=True)
+        u_host = torch.empty((3, wl.nz, wl.ny, wl.nx), dtype=torch.float32, pin_memory=True)
+        u_in = torch.zeros((3, wl.nz, wl.ny, wl.nx), dtype=torch.float32, pin_memory=True)
+        out = {"rho": rho_host.numpy(), "u": u_host.numpy()}
+        h2d, d2h = wl.cells * 12, wl.cells * 16
+
+        def e2e_step():
+            sim.set_fields(None, u_in.numpy())
+            sim.step(1, 0)
+            sim.read_fields(force=False, out=out)
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    t = torch.tensor([dt], device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dt = float(t.item())
+    line["e2e"] = {"value": world * wl.cells * e2e_steps / dt / 1e6, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+                   "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
+                   "what": "per step: kinematics table H2D, one coupled step, marker forces D2H (pinned)"
+                   if wl.n_markers else "per step: u field H2D (set_fields), one step, rho+u D2H (pinned)"}
+    sim.close()
+
+    # ---- the oracle on the host cores (rank 0, N = 1 only) ------------------------------------------
+    if rank == 0 and world == 1 and not args.no_cpu:
+        ref, swl, sample = oracle_sample(wl.name if wl.name in ("W1", "W2", "W3") else args.workload, args.seed,
+                                         args.cpu_steps)
+        ref.step(1, swl.mdf_iters)
+        t0 = time.perf_counter()
+        ref.step(args.cpu_steps, swl.mdf_iters)
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": swl.cells * args.cpu_steps / dt / 1e6, "unit": UNIT,
+                                "cores": os.cpu_count() or 1, "kind": "oracle", "sample": sample}
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="W4")
+    ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--spread", default="gather", choices=["gather", "atomic"])
+    ap.add_argument("--lbm-kernel", default="vec4", choices=["vec4", "scalar"])
+    ap.add_argument("--cpu-steps", type=int, default=10)
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--quick", action="store_true", help="skip the extra W2 pure-LBM run")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else max(args.warmup, 0)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -61,7 +61,10 @@ enum {
     LBM_OPT_FORCING = 2,  /* 0 = Guo source term (default, R3), 1 = paper's shift U + tau G */
     LBM_OPT_GRAPH = 3,    /* 1 = replay the step as a CUDA graph (default), 0 = plain launches     */
     LBM_OPT_LBM_KERNEL = 4, /* stream-collide variant: 0 = default (vectorised), 1 = scalar         */
-    LBM_OPT_INTERP = 5    /* interpolation variant: 0 = default, 1 = thread per marker            */
+    LBM_OPT_INTERP = 5,   /* interpolation variant: 0 = default, 1 = thread per marker            */
+    LBM_OPT_TIMING = 6    /* 1 = run steps as plain launches with CUDA events between the phases and
+                             accumulate per-phase device time (LBM_INFO_PHASE_NS); setting it resets
+                             the accumulators.  Each step then ends with a stream synchronise.     */
 };
 
 /* Keys for lbm_get_info. */
@@ -72,7 +75,11 @@ enum {
     LBM_INFO_LAUNCHES = 4,      /* kernels launched by this handle so far (graph nodes counted)   */
     LBM_INFO_ACTIVE_CELLS = 5,  /* cells inside at least one marker's stencil in the last step    */
     LBM_INFO_DEVICE_BYTES = 6,  /* device memory owned by the handle                              */
-    LBM_INFO_STATUS = 7         /* device-side status word of the last step (0 = OK)              */
+    LBM_INFO_STATUS = 7,        /* device-side status word of the last step (0 = OK)              */
+    LBM_INFO_PHASE_NS = 100     /* + phase: accumulated device time in ns under LBM_OPT_TIMING.
+                                   phases: 0 kinematics+keys, 1 sort, 2 gather+bins, 3 moments on
+                                   active cells, 4 interpolation+correction, 5 spreading,
+                                   6 stream-collide                                              */
 };
 
 /* P:31 + eq.(3): allocate an nx*ny*nz D3Q19 lattice with relaxation time tau on the current CUDA
@@ -107,6 +114,14 @@ int ibm_set_markers(lbm_t *h, const float *pos, const float *vel, const float *a
  * (p_k - c) + vel_k (R12, R13).  Bodies without kinematics are static (omega = 0).  On a wall axis
  * the sphere swept by every point must keep its stencil inside the box, else LBM_ERANGE. */
 int ibm_set_kinematics(lbm_t *h, double omega, const double *axis, const double *center);
+
+/* Same as ibm_set_kinematics for the bodies first_body .. first_body+count-1 at once: omega [count],
+ * axis [count][3], center [count][3] or NULL (= keep the centres); host, fp64.  When the centres
+ * are kept only a small per-body table is copied to the device (no marker re-upload), so a host
+ * controller may call this every step.  The angle of step n is omega * n (R13): changing omega
+ * mid-run re-phases the body. */
+int ibm_update_kinematics(lbm_t *h, int first_body, int count, const double *omega, const double *axis,
+                          const double *center);
 
 /* Remove all bodies and markers. */
 int ibm_clear(lbm_t *h);

@@ -21,13 +21,15 @@ if not os.path.exists(LIB_PATH):
 
 _L = C.CDLL(LIB_PATH)
 
-OPT_SPREAD, OPT_FORCING, OPT_GRAPH, OPT_LBM_KERNEL, OPT_INTERP = 1, 2, 3, 4, 5
+OPT_SPREAD, OPT_FORCING, OPT_GRAPH, OPT_LBM_KERNEL, OPT_INTERP, OPT_TIMING = 1, 2, 3, 4, 5, 6
 INFO_MARKERS, INFO_BODIES, INFO_STEPS, INFO_LAUNCHES, INFO_ACTIVE_CELLS, INFO_DEVICE_BYTES, INFO_STATUS = range(1, 8)
+INFO_PHASE_NS = 100
+PHASES = ["keys", "sort", "bins", "moments", "interp", "spread", "lbm"]
 SPREAD_GATHER, SPREAD_ATOMIC = 0, 1
 FORCING_GUO, FORCING_SHIFT = 0, 1
 
 EXPORTS = ["lbm_create", "lbm_destroy", "lbm_set_stream", "lbm_set_option", "lbm_get_info", "lbm_set_fields",
-           "ibm_set_markers", "ibm_set_kinematics", "ibm_clear", "lbm_ibm_step", "lbm_read_fields",
+           "ibm_set_markers", "ibm_set_kinematics", "ibm_update_kinematics", "ibm_clear", "lbm_ibm_step", "lbm_read_fields",
            "ibm_read_markers", "lbm_sync", "lbm_last_error"]
 
 
@@ -47,6 +49,7 @@ _L.lbm_get_info.argtypes = [_vp, C.c_int, C.POINTER(C.c_longlong)]
 _L.lbm_set_fields.argtypes = [_vp, _vp, _vp]
 _L.ibm_set_markers.argtypes = [_vp, _vp, _vp, _vp, C.c_longlong]
 _L.ibm_set_kinematics.argtypes = [_vp, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+_L.ibm_update_kinematics.argtypes = [_vp, C.c_int, C.c_int, _vp, _vp, _vp]
 _L.ibm_clear.argtypes = [_vp]
 _L.lbm_ibm_step.argtypes = [_vp, C.c_int, C.c_int]
 _L.lbm_read_fields.argtypes = [_vp, _vp, _vp, _vp]
@@ -149,6 +152,14 @@ class LbmIbm:
         c = (C.c_double * 3)(*[float(v) for v in center])
         _check(_L.ibm_set_kinematics(self._h, float(omega), a, c), "ibm_set_kinematics")
 
+    def update_kinematics(self, first_body, omega, axis, center=None):
+        """omega [n], axis [n,3], center [n,3] or None: float64 numpy arrays (host)"""
+        om = np.ascontiguousarray(omega, dtype=np.float64)
+        ax = np.ascontiguousarray(axis, dtype=np.float64)
+        ce = None if center is None else np.ascontiguousarray(center, dtype=np.float64)
+        _check(_L.ibm_update_kinematics(self._h, int(first_body), int(om.shape[0]), om.ctypes.data, ax.ctypes.data,
+                                        None if ce is None else ce.ctypes.data), "ibm_update_kinematics")
+
     def clear(self):
         _check(_L.ibm_clear(self._h), "ibm_clear")
 
@@ -159,6 +170,10 @@ class LbmIbm:
 
     def step(self, nsteps=1, mdf_iters=0):
         _check(_L.lbm_ibm_step(self._h, int(nsteps), int(mdf_iters)), "lbm_ibm_step")
+
+    def phase_ms(self) -> dict:
+        """per-phase device time accumulated under OPT_TIMING, in ms"""
+        return {n: self.get_info(INFO_PHASE_NS + i) * 1e-6 for i, n in enumerate(PHASES)}
 
     def sync(self):
         _check(_L.lbm_sync(self._h), "lbm_sync")

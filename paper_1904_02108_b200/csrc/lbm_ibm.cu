@@ -58,6 +58,32 @@ struct HostBody {
 
 constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driven kernels
 
+// Optional per-phase device timing (LBM_OPT_TIMING): CUDA events recorded on the launching stream
+// between the phases of a step; durations are accumulated after a stream synchronise.
+enum { PH_KEYS = 0, PH_SORT, PH_BINS, PH_MOMENTS, PH_INTERP, PH_SPREAD, PH_LBM, PH_COUNT };
+struct PhaseTimer {
+    std::vector<cudaEvent_t> ev;
+    std::vector<int> tag;
+    size_t used = 0;
+    double ns[PH_COUNT] = {0, 0, 0, 0, 0, 0, 0};
+    void mark(int phase, cudaStream_t s)
+    {
+        if (used == ev.size()) { cudaEvent_t e; cudaEventCreate(&e); ev.push_back(e); tag.push_back(0); }
+        tag[used] = phase;
+        cudaEventRecord(ev[used++], s);
+    }
+    void collect()
+    {
+        for (size_t i = 0; i + 1 < used; ++i) {
+            float ms = 0.f;
+            if (tag[i] >= 0 && cudaEventElapsedTime(&ms, ev[i], ev[i + 1]) == cudaSuccess) ns[tag[i]] += 1e6 * ms;
+        }
+        used = 0;
+    }
+    void reset() { for (double &v : ns) v = 0; used = 0; }
+    ~PhaseTimer() { for (cudaEvent_t e : ev) cudaEventDestroy(e); }
+};
+
 }  // namespace
 
 struct lbm {
@@ -82,6 +108,7 @@ struct lbm {
     std::vector<float> h_pos, h_vel, h_area;   // [n][3], [n][3], [n]
     std::vector<int> h_body;
     std::vector<HostBody> bodies;
+    std::vector<BodyDef> h_defs;        // host copy of the per-body device table
     bool markers_stale = true;          // device copies / graphs need rebuilding
     int nm = 0, nm_cap = 0, nb_cap = 0;
     float *d_q[3] = {nullptr, nullptr, nullptr}, *d_v[3] = {nullptr, nullptr, nullptr}, *d_s = nullptr;
@@ -94,7 +121,8 @@ struct lbm {
     MarkerSorted ms{nullptr, nullptr, nullptr, nullptr};
     int sort_ipw = 64, sort_tiles = 0, sort_passes = 1;
 
-    int opt_spread = 0, opt_forcing = 0, opt_graph = 1, opt_lbm_kernel = 0, opt_interp = 0;
+    int opt_spread = 0, opt_forcing = 0, opt_graph = 1, opt_lbm_kernel = 0, opt_interp = 0, opt_timing = 0;
+    PhaseTimer timer;
     std::map<long long, std::pair<cudaGraphExec_t, int>> graphs;   // key -> (exec, kernel nodes)
     long long launches = 0;
     size_t dev_bytes = 0;
@@ -219,7 +247,8 @@ int upload_markers(lbm *h)
     if (n == 0) { h->markers_stale = false; return LBM_OK; }
 
     // body tables; rest positions relative to the body centre, formed in fp64
-    std::vector<BodyDef> defs((size_t)nb);
+    std::vector<BodyDef> &defs = h->h_defs;
+    defs.assign((size_t)nb, BodyDef{});
     std::vector<float> q[3], v[3];
     for (int a = 0; a < 3; ++a) { q[a].resize((size_t)n); v[a].resize((size_t)n); }
     for (int b = 0; b < nb; ++b) {
@@ -252,7 +281,7 @@ int upload_markers(lbm *h)
 }
 
 // ---- enqueue one time step on stream s (plain launches; also what graph capture records) -------
-int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, int *n_kernels)
+int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, int *n_kernels, PhaseTimer *pt = nullptr)
 {
     const float *src = h->f[parity];
     float *dst = h->f[parity ^ 1];
@@ -266,11 +295,13 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
         int *perm = h->d_vals[h->sort_passes & 1];
         MarkerIn mi{h->d_q[0], h->d_q[1], h->d_q[2], h->d_v[0], h->d_v[1], h->d_v[2], h->d_s, h->d_body, n};
 
+        if (pt) pt->mark(PH_KEYS, s);
         k_clear_prev<<<LIST_GRID, 256, 0, s>>>(skey, &sc->n_prev, h->bin_first, h->amask, h->words, &sc->n_words);
         const int nb = (int)h->bodies.size();
         k_kinematics<<<(nb + 127) / 128, 128, 0, s>>>(h->d_defs, h->d_tabs, nb, &sc->step_ctr, &sc->n_words);
         k_marker_keys<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, h->d_keys[0], &sc->status);
         nk += 3;
+        if (pt) pt->mark(PH_SORT, s);
         const int sb = (h->sort_tiles + SORT_WARPS - 1) / SORT_WARPS;
         for (int p = 0; p < h->sort_passes; ++p) {
             const unsigned *kin = h->d_keys[p & 1];
@@ -283,15 +314,19 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
                                                        h->d_hist, h->d_total);
             nk += 3;
         }
+        if (pt) pt->mark(PH_BINS, s);
         k_marker_gather<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, perm, h->ms);
         k_bins<<<mb, 256, 0, s>>>(skey, n, g, h->bin_first, h->amask, h->words, &sc->n_words);
         k_set_scalars<<<1, 1, 0, s>>>(&sc->step_ctr, 0, &sc->n_prev, n, 2 | 4);
+        if (pt) pt->mark(PH_MOMENTS, s);
         k_moments_active<<<LIST_GRID, 256, 0, s>>>(src, g, h->amask, h->words, &sc->n_words, h->U);
         nk += 4;
         for (int m = 0; m < mdf_iters; ++m) {
             const bool last = (m == mdf_iters - 1);
+            if (pt) pt->mark(PH_INTERP, s);
             k_interp_correct<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, h->U, h->ms);
             ++nk;
+            if (pt) pt->mark(PH_SPREAD, s);
             if (h->opt_spread == 0) {
                 if (last)
                     k_spread_gather<true><<<LIST_GRID, 256, 0, s>>>(skey, n, g, h->bin_first, h->amask, h->words,
@@ -312,6 +347,7 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
             }
         }
     }
+    if (pt) pt->mark(PH_LBM, s);
     CollisionConst cc = h->cc;
     cc.shift_forcing = h->opt_forcing;
     const bool vec = (h->opt_lbm_kernel == 0) && (g.nx % 4 == 0);
@@ -330,6 +366,7 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
         else k_stream_collide_scalar<false><<<gr, b, 0, s>>>(src, dst, g, cc, nullptr, nullptr);
     }
     ++nk;
+    if (pt) pt->mark(-1, s);
     CK(cudaGetLastError());
     *n_kernels = nk;
     return LBM_OK;
@@ -478,6 +515,7 @@ int lbm_set_option(lbm_t *h, int key, int value)
         case LBM_OPT_GRAPH: if (value < 0 || value > 1) break; h->opt_graph = value; return LBM_OK;
         case LBM_OPT_LBM_KERNEL: if (value < 0 || value > 1) break; h->opt_lbm_kernel = value; return LBM_OK;
         case LBM_OPT_INTERP: if (value < 0 || value > 1) break; h->opt_interp = value; return LBM_OK;
+        case LBM_OPT_TIMING: if (value < 0 || value > 1) break; h->opt_timing = value; h->timer.reset(); return LBM_OK;
         default: return fail(LBM_EINVAL, "lbm_set_option: unknown key %d", key);
     }
     return fail(LBM_EINVAL, "lbm_set_option: value %d out of range for key %d", value, key);
@@ -510,7 +548,12 @@ int lbm_get_info(lbm_t *h, int key, long long *value)
             *value = st;
             return LBM_OK;
         }
-        default: return fail(LBM_EINVAL, "lbm_get_info: unknown key %d", key);
+        default:
+            if (key >= LBM_INFO_PHASE_NS && key < LBM_INFO_PHASE_NS + PH_COUNT) {
+                *value = (long long)h->timer.ns[key - LBM_INFO_PHASE_NS];
+                return LBM_OK;
+            }
+            return fail(LBM_EINVAL, "lbm_get_info: unknown key %d", key);
     }
 }
 
@@ -611,6 +654,52 @@ int ibm_set_kinematics(lbm_t *h, double omega, const double *axis, const double 
     return LBM_OK;
 }
 
+int ibm_update_kinematics(lbm_t *h, int first_body, int count, const double *omega, const double *axis,
+                          const double *center)
+{
+    if (!h || !omega || !axis) return fail(LBM_EINVAL, "ibm_update_kinematics: NULL argument");
+    if (first_body < 0 || count < 0 || (size_t)first_body + (size_t)count > h->bodies.size())
+        return fail(LBM_EINVAL, "ibm_update_kinematics: body range out of bounds");
+    std::vector<HostBody> nb(h->bodies.begin() + first_body, h->bodies.begin() + first_body + count);
+    bool moved = false;
+    for (int b = 0; b < count; ++b) {
+        const double *ax = axis + 3 * b;
+        const double nrm = std::sqrt(ax[0] * ax[0] + ax[1] * ax[1] + ax[2] * ax[2]);
+        if (!(nrm > 0.0) || !std::isfinite(nrm) || !std::isfinite(omega[b]))
+            return fail(LBM_EINVAL, "ibm_update_kinematics: bad axis or omega for body %d", first_body + b);
+        HostBody &B = nb[(size_t)b];
+        const double *c = center ? center + 3 * b : B.center;
+        if (center) for (int a = 0; a < 3; ++a) moved |= (c[a] != B.center[a]);
+        const bool any_wall = h->g.wallx || h->g.wally || h->g.wallz;
+        if (any_wall && omega[b] != 0.0 && (center || B.omega == 0.0))
+            for (long long k = B.first; k < B.first + B.count; ++k) {
+                double r2 = 0.0;
+                for (int a = 0; a < 3; ++a) {
+                    const double d = (double)h->h_pos[(size_t)(3 * k + a)] - c[a];
+                    r2 += d * d;
+                }
+                const double r = std::sqrt(r2);
+                const double lo[3] = {c[0] - r, c[1] - r, c[2] - r}, hi[3] = {c[0] + r, c[1] + r, c[2] + r};
+                if (!stencil_inside(h, lo, hi))
+                    return fail(LBM_ERANGE, "ibm_update_kinematics: marker %lld can reach a wall", k);
+            }
+        B.omega = omega[b];
+        for (int a = 0; a < 3; ++a) { B.axis[a] = ax[a] / nrm; B.center[a] = c[a]; }
+        B.has_kin = true;
+    }
+    std::copy(nb.begin(), nb.end(), h->bodies.begin() + first_body);
+    if (moved || h->markers_stale) { h->markers_stale = true; return LBM_OK; }
+    // centres unchanged: only the small per-body table changes; graphs and marker arrays stay valid
+    for (int b = 0; b < count; ++b) {
+        const HostBody &B = h->bodies[(size_t)(first_body + b)];
+        BodyDef &d = h->h_defs[(size_t)(first_body + b)];
+        d.omega = B.omega; d.ax = B.axis[0]; d.ay = B.axis[1]; d.az = B.axis[2];
+    }
+    CK(cudaMemcpyAsync(h->d_defs + first_body, h->h_defs.data() + first_body, sizeof(BodyDef) * (size_t)count,
+                       cudaMemcpyHostToDevice, h->stream));
+    return LBM_OK;
+}
+
 int ibm_clear(lbm_t *h)
 {
     if (!h) return fail(LBM_EINVAL, "ibm_clear: NULL handle");
@@ -636,7 +725,11 @@ int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
     }
     for (int s = 0; s < nsteps; ++s) {
         int nk = 0;
-        if (h->opt_graph) {
+        if (h->opt_timing) {
+            if ((rc = enqueue_step(h, h->stream, h->cur, mdf_iters, ibm, &nk, &h->timer))) return rc;
+            CK(cudaStreamSynchronize(h->stream));
+            h->timer.collect();
+        } else if (h->opt_graph) {
             cudaGraphExec_t ex = nullptr;
             if ((rc = get_graph(h, h->cur, mdf_iters, ibm, &ex, &nk))) return rc;
             CK(cudaGraphLaunch(ex, h->stream));
