@@ -181,10 +181,8 @@ def run_ours(args):
     mdf = wl.mdf_iters
     stream = torch.cuda.Stream()
     sim = api.from_workload(wl, stream=stream)
-    if args.spread == "atomic":
-        sim.set_option(api.OPT_SPREAD, api.SPREAD_ATOMIC)
-    if args.lbm_kernel == "scalar":
-        sim.set_option(api.OPT_LBM_KERNEL, 1)
+    sim.set_option(api.OPT_SPREAD, {"gather": 0, "atomic": 1, "plain": 2}[args.spread])
+    sim.set_option(api.OPT_LBM_KERNEL, {"auto": 0, "scalar": 1, "vec4": 2}[args.lbm_kernel])
 
     def barrier():
         torch.cuda.synchronize()
@@ -251,8 +249,7 @@ def run_ours(args):
         if wl.name != "W2" and not args.quick:
             w2 = workloads.get("W2", args.seed)
             s2 = api.from_workload(w2, stream=stream)
-            if args.lbm_kernel == "scalar":
-                s2.set_option(api.OPT_LBM_KERNEL, 1)
+            s2.set_option(api.OPT_LBM_KERNEL, {"auto": 0, "scalar": 1, "vec4": 2}[args.lbm_kernel])
             s2.step(max(3, args.warmup), 0)
             stream.synchronize()
             ms2 = time_steps(torch, s2, stream, args.steps, 0)
@@ -332,8 +329,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="W4")
     ap.add_argument("--seed", type=int, default=0)
-    ap.add_argument("--spread", default="gather", choices=["gather", "atomic"])
-    ap.add_argument("--lbm-kernel", default="vec4", choices=["vec4", "scalar"])
+    ap.add_argument("--spread", default="gather", choices=["gather", "atomic", "plain"])
+    ap.add_argument("--lbm-kernel", default="auto", choices=["auto", "vec4", "scalar"])
     ap.add_argument("--cpu-steps", type=int, default=10)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--quick", action="store_true", help="skip the extra W2 pure-LBM run")

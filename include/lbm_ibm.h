@@ -56,11 +56,13 @@ enum {
 
 /* Options for lbm_set_option. */
 enum {
-    LBM_OPT_SPREAD = 1,   /* 0 = deterministic gather-by-cell (default), 1 = global atomics (the
-                             paper's ib_force2 design; kept as a measured comparison)  */
+    LBM_OPT_SPREAD = 1,   /* 0 = deterministic run-sweep + gather-by-cell (default), 1 = global atomics
+                             (the paper's ib_force2 design; kept as a measured comparison),
+                             2 = plain gather-by-cell over the bins (slow reference variant)        */
     LBM_OPT_FORCING = 2,  /* 0 = Guo source term (default, R3), 1 = paper's shift U + tau G */
     LBM_OPT_GRAPH = 3,    /* 1 = replay the step as a CUDA graph (default), 0 = plain launches     */
-    LBM_OPT_LBM_KERNEL = 4, /* stream-collide variant: 0 = default (vectorised), 1 = scalar         */
+    LBM_OPT_LBM_KERNEL = 4, /* stream-collide variant: 0 = default (the faster one), 1 = one cell per
+                             thread, 2 = four cells per thread with 128-bit accesses (nx % 4 == 0)    */
     LBM_OPT_INTERP = 5,   /* interpolation variant: 0 = default, 1 = thread per marker            */
     LBM_OPT_TIMING = 6    /* 1 = run steps as plain launches with CUDA events between the phases and
                              accumulate per-phase device time (LBM_INFO_PHASE_NS); setting it resets

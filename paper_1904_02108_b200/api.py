@@ -25,7 +25,7 @@ OPT_SPREAD, OPT_FORCING, OPT_GRAPH, OPT_LBM_KERNEL, OPT_INTERP, OPT_TIMING = 1, 
 INFO_MARKERS, INFO_BODIES, INFO_STEPS, INFO_LAUNCHES, INFO_ACTIVE_CELLS, INFO_DEVICE_BYTES, INFO_STATUS = range(1, 8)
 INFO_PHASE_NS = 100
 PHASES = ["keys", "sort", "bins", "moments", "interp", "spread", "lbm"]
-SPREAD_GATHER, SPREAD_ATOMIC = 0, 1
+SPREAD_GATHER, SPREAD_ATOMIC, SPREAD_GATHER_PLAIN = 0, 1, 2
 FORCING_GUO, FORCING_SHIFT = 0, 1
 
 EXPORTS = ["lbm_create", "lbm_destroy", "lbm_set_stream", "lbm_set_option", "lbm_get_info", "lbm_set_fields",

@@ -31,10 +31,11 @@ struct MarkerIn {                  // original (caller) order, SoA
 // a1: Rodrigues rotation tables of every body for step n -> n+1, in fp64 (R12, R13).
 // Also re-arms the per-step device counters.
 __global__ void k_kinematics(const BodyDef *__restrict__ defs, BodyStep *__restrict__ out, int nbodies,
-                             const long long *__restrict__ step_ctr, int *__restrict__ n_words)
+                             const long long *__restrict__ step_ctr, int *__restrict__ n_words,
+                             int *__restrict__ n_runs, int *__restrict__ t_count)
 {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b == 0) *n_words = 0;
+    if (b == 0) { *n_words = 0; *n_runs = 0; *t_count = 0; }
     if (b >= nbodies) return;
     const BodyDef d = defs[b];
     const double n = (double)(*step_ctr);
@@ -53,6 +54,11 @@ __global__ void k_kinematics(const BodyDef *__restrict__ defs, BodyStep *__restr
     for (int j = 0; j < 9; ++j) { o.R[j] = (float)R1[j]; o.dR[j] = (float)(R1[j] - R0[j]); }
     out[b] = o;
 }
+
+// Peskin 4-point kernel (R6): the four distances 1+f, f, 1-f, 2-f of a point at c + f to the
+// cells c-1 .. c+2 share one square root, because 1 + 4r - 4r^2 at r = f or 1-f and -7 + 12r - 4r^2
+// at r = 1+f or 2-f all equal 1 + 4f(1 - f).
+__device__ __forceinline__ float peskin_root(float f) { return sqrtf(fmaf(4.0f * f, 1.0f - f, 1.0f)); }
 
 struct Placed {
     int cx, cy, cz;      // owning cell = floor(position), wrapped on periodic axes
@@ -106,6 +112,7 @@ k_marker_keys(MarkerIn m, const BodyDef *__restrict__ defs, const BodyStep *__re
 // per-marker state in SORTED order
 struct MarkerSorted {
     float4 *fs;     // (fx, fy, fz, s)
+    float4 *fq;     // (qx, qy, qz, -), q = sqrt(1 + 4f - 4f^2): the one square root of the four weights
     float4 *uk;     // prescribed velocity u_k, w unused
     float4 *sg;     // s * g^m(k)   (what the U update spreads, P:98 + R8)
     float4 *du;     // Delta u(k)
@@ -124,6 +131,7 @@ k_marker_gather(MarkerIn m, const BodyDef *__restrict__ defs, const BodyStep *__
     const float qx = m.qx[k], qy = m.qy[k], qz = m.qz[k];
     const Placed p = place_marker(defs[b], t, qx, qy, qz, g);
     out.fs[i] = make_float4(p.fx, p.fy, p.fz, m.s[k]);
+    out.fq[i] = make_float4(peskin_root(p.fx), peskin_root(p.fy), peskin_root(p.fz), 0.f);
     const float ux = fmaf(t.dR[0], qx, fmaf(t.dR[1], qy, fmaf(t.dR[2], qz, m.vx[k])));
     const float uy = fmaf(t.dR[3], qx, fmaf(t.dR[4], qy, fmaf(t.dR[5], qz, m.vy[k])));
     const float uz = fmaf(t.dR[6], qx, fmaf(t.dR[7], qy, fmaf(t.dR[8], qz, m.vz[k])));
@@ -205,13 +213,19 @@ k_bins(const unsigned *__restrict__ skey, int n, Geom g, int *__restrict__ bin_f
 // entries), so neither needs a full-lattice memset per step.
 __global__ void __launch_bounds__(256)
 k_clear_prev(const unsigned *__restrict__ skey_prev, const int *__restrict__ n_prev, int *__restrict__ bin_first,
-             unsigned *__restrict__ amask, const int *__restrict__ words, const int *__restrict__ n_words)
+             unsigned *__restrict__ amask, const int *__restrict__ words, const int *__restrict__ n_words,
+             int *__restrict__ tslot, const int *__restrict__ run_slot0, const int *__restrict__ run_nent,
+             const int *__restrict__ n_runs)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     const int stride = gridDim.x * blockDim.x;
-    const int np = *n_prev, nw = *n_words;
+    const int np = *n_prev, nw = *n_words, nr = *n_runs;
     for (int i = tid; i < np; i += stride) bin_first[skey_prev[i]] = -1;
     for (int i = tid; i < nw; i += stride) amask[words[i]] = 0u;
+    for (int r = tid; r < nr; r += stride) {
+        const int s0 = run_slot0[r], ne = run_nent[r];
+        for (int j = 0; j < ne; ++j) tslot[s0 + j] = -1;
+    }
 }
 
 // device scalars: mode bit 0: step_ctr = step; bit 1: n_prev = n_prev_val; bit 2: step_ctr += 1
@@ -227,7 +241,7 @@ __global__ void k_set_scalars(long long *step_ctr, long long step, int *n_prev, 
 // -7 + 12r - 4r^2 at r = 1+f or 2-f all equal 1 + 4f - 4f^2.
 __device__ __forceinline__ void peskin4(float f, float (&w)[4])
 {
-    const float q = sqrtf(fmaf(4.0f * f, 1.0f - f, 1.0f));
+    const float q = peskin_root(f);
     const float a = 3.0f - 2.0f * f, b = 1.0f + 2.0f * f;
     w[0] = 0.125f * (a - q);
     w[1] = 0.125f * (a + q);
@@ -284,13 +298,13 @@ k_interp_correct(const unsigned *__restrict__ skey, int n, Geom g, const float4 
 // weight of the cell at offset j (0..3 <-> c-1..c+2) only
 __device__ __forceinline__ float peskin1(float f, int j)
 {
-    const float q = sqrtf(fmaf(4.0f * f, 1.0f - f, 1.0f));
+    const float q = peskin_root(f);
     const float lin = (j < 2) ? (3.0f - 2.0f * f) : (1.0f + 2.0f * f);
     const float sq = (j == 1 || j == 2) ? q : -q;
     return 0.125f * (lin + sq);
 }
 
-// a7, deterministic gather-by-cell (reference variant): one warp per active word, one lane per
+// a7, plain gather-by-cell (reference variant, slow; kept for cross-checks): one warp per active word, one lane per
 // active cell.  The cell visits the 4x4x4 bins whose stencils reach it in a fixed order and, inside
 // a bin, the markers in sorted order, so the sum is order-fixed and free of atomics.
 //   LAST = false:  U^{m+1}(X) = U^m(X) + sum_k s_k g_k W_k(X)      (R8)
@@ -336,6 +350,196 @@ k_spread_gather(const unsigned *__restrict__ skey, int n, Geom g, const int *__r
                         sx = fmaf(v.x, wgt, sx);
                         sy = fmaf(v.y, wgt, sy);
                         sz = fmaf(v.z, wgt, sz);
+                    }
+                }
+            }
+        }
+        const size_t cell = (size_t)row * g.nx + x;
+        if (LAST) {
+            field[cell] = make_float4(sx, sy, sz, 0.f);
+        } else {
+            float4 u = field[cell];
+            u.x += sx; u.y += sy; u.z += sz;
+            field[cell] = u;
+        }
+    }
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// a7, product path: deterministic spreading in two stages, no atomics on the field.
+//
+// A "run" is a maximal stretch of sorted markers in one lattice row (same cy, cz) whose owning
+// cells are less than 4 apart in x, i.e. whose stencils chain together along x.  Runs of one row
+// never touch the same cell, and a marker of source row (cy, cz) reaches the 16 target rows
+// (cy-1+jy, cz-1+jz).  Stage A sweeps every run once, in sorted order, and produces for each of the
+// 16 (jy, jz) offsets the x-profile  T[entry][jy*4+jz] = sum_k v_k w_y(jy) w_z(jz) w_x(X - cx_k + 1)
+// over the run's x extent (entries cx_first-1 .. cx_last+2).  Stage B lets every active cell add
+// up, in fixed order, the <= 16 profiles that reach it (one per source row).  All sums have a fixed
+// order, so the result is bitwise reproducible.
+
+struct RunTable {
+    int *first, *end;   // sorted-marker range [first, end) of the run
+    int *base;          // first T entry of the run
+    int *slot0;         // index into tslot of the run's first entry
+    int *nent;          // number of entries = cx_last - cx_first + 4
+};
+
+// tslot is a dense map [row][X + 1], X = -1 .. nx+1 (unwrapped x, so that runs at a periodic seam
+// keep their own entries), holding the T entry or -1.
+__device__ __forceinline__ int tslot_pitch(const Geom &g) { return g.nx + 3; }
+
+// a3 (third part): find the runs, give each its block of T entries and publish them in tslot.
+__global__ void __launch_bounds__(256)
+k_runs(const unsigned *__restrict__ skey, int n, Geom g, RunTable rt, int *__restrict__ tslot,
+       int *__restrict__ n_runs, int *__restrict__ t_count)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    bool head = false;
+    int row = 0, cx = 0, end = 0, nent = 0;
+    if (i < n) {
+        const unsigned key = skey[i];
+        row = (int)(key / (unsigned)g.nx);
+        cx = (int)key - row * g.nx;
+        if (i == 0) head = true;
+        else {
+            const unsigned pk = skey[i - 1];
+            const int prow = (int)(pk / (unsigned)g.nx);
+            head = (prow != row) || (cx - ((int)pk - prow * g.nx) >= 4);
+        }
+        if (head) {
+            int j = i + 1, last = cx;
+            while (j < n) {
+                const unsigned k2 = skey[j];
+                const int r2 = (int)(k2 / (unsigned)g.nx);
+                const int c2 = (int)k2 - r2 * g.nx;
+                if (r2 != row || c2 - last >= 4) break;
+                last = c2;
+                ++j;
+            }
+            end = j;
+            nent = last - cx + 4;
+        }
+    }
+    const unsigned vote = __ballot_sync(0xffffffffu, head);
+    if (!vote) return;
+    int incl = nent;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    const int total = __shfl_sync(0xffffffffu, incl, 31);
+    int rbase = 0, tbase = 0;
+    if (lane == 0) { rbase = atomicAdd(n_runs, __popc(vote)); tbase = atomicAdd(t_count, total); }
+    rbase = __shfl_sync(0xffffffffu, rbase, 0);
+    tbase = __shfl_sync(0xffffffffu, tbase, 0);
+    if (head) {
+        const int r = rbase + __popc(vote & ((1u << lane) - 1u));
+        const int base = tbase + incl - nent;
+        const int s0 = row * tslot_pitch(g) + cx;        // X = cx - 1  ->  column X + 1 = cx
+        rt.first[r] = i; rt.end[r] = end; rt.base[r] = base; rt.slot0[r] = s0; rt.nent[r] = nent;
+        for (int j = 0; j < nent; ++j) tslot[s0 + j] = base + j;
+    }
+}
+
+// Stage A: one half-warp per run, lane l = jy*4 + jz owns the profile of target-row offset (jy, jz)
+// and keeps a sliding window of four x cells (cxw-1 .. cxw+2) in registers; cells that fall out of
+// the window as the sweep advances are final and are written to T (16 lanes x float4 = 256 B).
+__global__ void __launch_bounds__(256)
+k_spread_rows(const unsigned *__restrict__ skey, Geom g, RunTable rt, const int *__restrict__ n_runs,
+              const float4 *__restrict__ fs, const float4 *__restrict__ fq, const float4 *__restrict__ val,
+              float4 *__restrict__ T)
+{
+    const int l = threadIdx.x & 15;
+    const int jy = l >> 2, jz = l & 3;
+    // w_j(f) = 1/8 (A + B f + C q):  j=0: (3,-2,-1)  1: (3,-2,+1)  2: (1,+2,+1)  3: (1,+2,-1)
+    const float ay = (jy < 2) ? 0.375f : 0.125f, by = (jy < 2) ? -0.25f : 0.25f, cy = (jy == 1 || jy == 2) ? 0.125f : -0.125f;
+    const float az = (jz < 2) ? 0.375f : 0.125f, bz = (jz < 2) ? -0.25f : 0.25f, cz = (jz == 1 || jz == 2) ? 0.125f : -0.125f;
+    const int hw = (blockIdx.x * blockDim.x + threadIdx.x) >> 4;
+    const int nhw = (gridDim.x * blockDim.x) >> 4;
+    const int nr = *n_runs;
+    for (int r = hw; r < nr; r += nhw) {
+        const int i0 = rt.first[r], i1 = rt.end[r];
+        size_t e = (size_t)rt.base[r];
+        const unsigned key0 = skey[i0];
+        const int rowx = (int)(key0 / (unsigned)g.nx) * g.nx;
+        int cxw = (int)key0 - rowx;
+        float a0x = 0.f, a0y = 0.f, a0z = 0.f, a1x = 0.f, a1y = 0.f, a1z = 0.f;
+        float a2x = 0.f, a2y = 0.f, a2z = 0.f, a3x = 0.f, a3y = 0.f, a3z = 0.f;
+        for (int i = i0; i < i1; ++i) {
+            const int cx = (int)skey[i] - rowx;
+            const float4 f = fs[i];
+            const float4 q = fq[i];
+            const float4 v = val[i];
+            while (cxw < cx) {
+                T[e * 16 + l] = make_float4(a0x, a0y, a0z, 0.f);
+                a0x = a1x; a0y = a1y; a0z = a1z;
+                a1x = a2x; a1y = a2y; a1z = a2z;
+                a2x = a3x; a2y = a3y; a2z = a3z;
+                a3x = 0.f; a3y = 0.f; a3z = 0.f;
+                ++e; ++cxw;
+            }
+            const float wyz = fmaf(cy, q.y, fmaf(by, f.y, ay)) * fmaf(cz, q.z, fmaf(bz, f.z, az));
+            const float vx = v.x * wyz, vy = v.y * wyz, vz = v.z * wyz;
+            const float lo = fmaf(-0.25f, f.x, 0.375f), hi = fmaf(0.25f, f.x, 0.125f), qq = 0.125f * q.x;
+            const float w0 = lo - qq, w1 = lo + qq, w2 = hi + qq, w3 = hi - qq;
+            a0x = fmaf(w0, vx, a0x); a0y = fmaf(w0, vy, a0y); a0z = fmaf(w0, vz, a0z);
+            a1x = fmaf(w1, vx, a1x); a1y = fmaf(w1, vy, a1y); a1z = fmaf(w1, vz, a1z);
+            a2x = fmaf(w2, vx, a2x); a2y = fmaf(w2, vy, a2y); a2z = fmaf(w2, vz, a2z);
+            a3x = fmaf(w3, vx, a3x); a3y = fmaf(w3, vy, a3y); a3z = fmaf(w3, vz, a3z);
+        }
+        T[e * 16 + l] = make_float4(a0x, a0y, a0z, 0.f);
+        T[(e + 1) * 16 + l] = make_float4(a1x, a1y, a1z, 0.f);
+        T[(e + 2) * 16 + l] = make_float4(a2x, a2y, a2z, 0.f);
+        T[(e + 3) * 16 + l] = make_float4(a3x, a3y, a3z, 0.f);
+    }
+}
+
+// Stage B: one warp per active word, one lane per active cell: add the profiles of the source rows
+// (y+1-jy, z+1-jz) at this x, jy and jz ascending (fixed order).
+//   LAST = false:  U^{m+1}(X) = U^m(X) + sum   (R8)      LAST = true:  G(X) = sum
+template <bool LAST>
+__global__ void __launch_bounds__(256)
+k_spread_collect(Geom g, const int *__restrict__ tslot, const float4 *__restrict__ T,
+                 const unsigned *__restrict__ amask, const int *__restrict__ words, const int *__restrict__ n_words,
+                 float4 *__restrict__ field)
+{
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    const int nw = *n_words;
+    const int pitch = tslot_pitch(g);
+    for (int k = warp; k < nw; k += nwarps) {
+        const int w = __ldg(words + k);
+        const unsigned bits = __ldg(amask + w);
+        if (!((bits >> lane) & 1u)) continue;
+        const int row = w / g.nxw;
+        const int x = (w - row * g.nxw) * 32 + lane;
+        const int z = row / g.ny, y = row - z * g.ny;
+        // ghost columns of a periodic x axis: X = x + nx (for x <= 1) and X = -1 (for x = nx-1)
+        const int ghost = g.wallx ? -1 : (x <= 1 ? x + g.nx + 1 : (x == g.nx - 1 ? 0 : -1));
+        float sx = 0.f, sy = 0.f, sz = 0.f;
+#pragma unroll
+        for (int jy = 0; jy < 4; ++jy) {
+            int cy = y + 1 - jy;
+            if (g.wally) { if (cy < 0 || cy >= g.ny) continue; } else cy = wrap(cy, g.ny);
+#pragma unroll
+            for (int jz = 0; jz < 4; ++jz) {
+                int cz = z + 1 - jz;
+                if (g.wallz) { if (cz < 0 || cz >= g.nz) continue; } else cz = wrap(cz, g.nz);
+                const int *trow = tslot + (size_t)(cz * g.ny + cy) * pitch;
+                const int e = __ldg(trow + x + 1);
+                if (e >= 0) {
+                    const float4 t = T[(size_t)e * 16 + (jy * 4 + jz)];
+                    sx += t.x; sy += t.y; sz += t.z;
+                }
+                if (ghost >= 0) {
+                    const int e2 = __ldg(trow + ghost);
+                    if (e2 >= 0) {
+                        const float4 t = T[(size_t)e2 * 16 + (jy * 4 + jz)];
+                        sx += t.x; sy += t.y; sz += t.z;
                     }
                 }
             }

@@ -5,6 +5,7 @@
 
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -48,6 +49,8 @@ struct DevScalars {
     int n_prev;          // sorted markers whose bins are still registered in bin_first
     int status;          // != 0: a stencil crossed a wall
     int scratch;
+    int n_runs;          // runs of the current / last IBM step
+    int t_count;         // T entries handed out in the current / last IBM step
 };
 
 struct HostBody {
@@ -118,7 +121,11 @@ struct lbm {
     unsigned *d_keys[2] = {nullptr, nullptr};
     int *d_vals[2] = {nullptr, nullptr};
     int *d_hist = nullptr, *d_total = nullptr;
-    MarkerSorted ms{nullptr, nullptr, nullptr, nullptr};
+    MarkerSorted ms{nullptr, nullptr, nullptr, nullptr, nullptr};
+    RunTable rt{nullptr, nullptr, nullptr, nullptr, nullptr};
+    int *tslot = nullptr;               // dense [row][X+1] -> T entry map (pitch nx+3)
+    float4 *T = nullptr;                // run profiles, 16 float4 per entry
+    size_t t_cap = 0, tslot_count = 0;
     int sort_ipw = 64, sort_tiles = 0, sort_passes = 1;
 
     int opt_spread = 0, opt_forcing = 0, opt_graph = 1, opt_lbm_kernel = 0, opt_interp = 0, opt_timing = 0;
@@ -166,7 +173,10 @@ void free_markers_dev(lbm *h)
     dfree(h, h->d_s, c);
     dfree(h, h->d_body, c);
     for (int a = 0; a < 2; ++a) { dfree(h, h->d_keys[a], c); dfree(h, h->d_vals[a], c); }
-    dfree(h, h->ms.fs, c); dfree(h, h->ms.uk, c); dfree(h, h->ms.sg, c); dfree(h, h->ms.du, c);
+    dfree(h, h->ms.fs, c); dfree(h, h->ms.fq, c); dfree(h, h->ms.uk, c); dfree(h, h->ms.sg, c); dfree(h, h->ms.du, c);
+    dfree(h, h->rt.first, c); dfree(h, h->rt.end, c); dfree(h, h->rt.base, c); dfree(h, h->rt.slot0, c);
+    dfree(h, h->rt.nent, c);
+    dfree(h, h->T, h->t_cap * 16); h->t_cap = 0;
     dfree(h, h->d_hist, (size_t)RADIX * (size_t)h->sort_tiles);
     dfree(h, h->d_total, (size_t)RADIX);
     dfree(h, h->d_defs, (size_t)h->nb_cap);
@@ -188,9 +198,11 @@ int flush_ibm(lbm *h)
     if (!h->ibm_dirty) return LBM_OK;
     const unsigned *skey = h->d_keys[h->sort_passes & 1];
     k_clear_prev<<<LIST_GRID, 256, 0, h->stream>>>(skey, &h->scal->n_prev, h->bin_first, h->amask, h->words,
-                                                    &h->scal->n_words);
+                                                    &h->scal->n_words, h->tslot, h->rt.slot0, h->rt.nent,
+                                                    &h->scal->n_runs);
     k_set_scalars<<<1, 1, 0, h->stream>>>(&h->scal->step_ctr, h->steps_done, &h->scal->n_prev, 0, 1 | 2);
     CK(cudaMemsetAsync(&h->scal->n_words, 0, sizeof(int), h->stream));
+    CK(cudaMemsetAsync(&h->scal->n_runs, 0, sizeof(int), h->stream));
     CK(cudaGetLastError());
     h->launches += 2;
     h->ibm_dirty = false;
@@ -222,6 +234,14 @@ int upload_markers(lbm *h)
             if ((rc = dmalloc(h, &h->d_vals[a], c))) return rc;
         }
         if ((rc = dmalloc(h, &h->ms.fs, c))) return rc;
+        if ((rc = dmalloc(h, &h->ms.fq, c))) return rc;
+        if ((rc = dmalloc(h, &h->rt.first, c))) return rc;
+        if ((rc = dmalloc(h, &h->rt.end, c))) return rc;
+        if ((rc = dmalloc(h, &h->rt.base, c))) return rc;
+        if ((rc = dmalloc(h, &h->rt.slot0, c))) return rc;
+        if ((rc = dmalloc(h, &h->rt.nent, c))) return rc;
+        h->t_cap = std::min((size_t)4 * c, h->tslot_count);
+        if ((rc = dmalloc(h, &h->T, h->t_cap * 16))) return rc;
         if ((rc = dmalloc(h, &h->ms.uk, c))) return rc;
         if ((rc = dmalloc(h, &h->ms.sg, c))) return rc;
         if ((rc = dmalloc(h, &h->ms.du, c))) return rc;
@@ -296,9 +316,11 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
         MarkerIn mi{h->d_q[0], h->d_q[1], h->d_q[2], h->d_v[0], h->d_v[1], h->d_v[2], h->d_s, h->d_body, n};
 
         if (pt) pt->mark(PH_KEYS, s);
-        k_clear_prev<<<LIST_GRID, 256, 0, s>>>(skey, &sc->n_prev, h->bin_first, h->amask, h->words, &sc->n_words);
+        k_clear_prev<<<LIST_GRID, 256, 0, s>>>(skey, &sc->n_prev, h->bin_first, h->amask, h->words, &sc->n_words,
+                                               h->tslot, h->rt.slot0, h->rt.nent, &sc->n_runs);
         const int nb = (int)h->bodies.size();
-        k_kinematics<<<(nb + 127) / 128, 128, 0, s>>>(h->d_defs, h->d_tabs, nb, &sc->step_ctr, &sc->n_words);
+        k_kinematics<<<(nb + 127) / 128, 128, 0, s>>>(h->d_defs, h->d_tabs, nb, &sc->step_ctr, &sc->n_words, &sc->n_runs,
+                                                      &sc->t_count);
         k_marker_keys<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, h->d_keys[0], &sc->status);
         nk += 3;
         if (pt) pt->mark(PH_SORT, s);
@@ -317,6 +339,7 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
         if (pt) pt->mark(PH_BINS, s);
         k_marker_gather<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, perm, h->ms);
         k_bins<<<mb, 256, 0, s>>>(skey, n, g, h->bin_first, h->amask, h->words, &sc->n_words);
+        if (h->opt_spread == 0) { k_runs<<<mb, 256, 0, s>>>(skey, n, g, h->rt, h->tslot, &sc->n_runs, &sc->t_count); ++nk; }
         k_set_scalars<<<1, 1, 0, s>>>(&sc->step_ctr, 0, &sc->n_prev, n, 2 | 4);
         if (pt) pt->mark(PH_MOMENTS, s);
         k_moments_active<<<LIST_GRID, 256, 0, s>>>(src, g, h->amask, h->words, &sc->n_words, h->U);
@@ -328,6 +351,16 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
             ++nk;
             if (pt) pt->mark(PH_SPREAD, s);
             if (h->opt_spread == 0) {
+                k_spread_rows<<<LIST_GRID, 256, 0, s>>>(skey, g, h->rt, &sc->n_runs, h->ms.fs, h->ms.fq,
+                                                        last ? h->ms.du : h->ms.sg, h->T);
+                if (last)
+                    k_spread_collect<true><<<LIST_GRID, 256, 0, s>>>(g, h->tslot, h->T, h->amask, h->words,
+                                                                      &sc->n_words, h->G);
+                else
+                    k_spread_collect<false><<<LIST_GRID, 256, 0, s>>>(g, h->tslot, h->T, h->amask, h->words,
+                                                                       &sc->n_words, h->U);
+                nk += 2;
+            } else if (h->opt_spread == 2) {
                 if (last)
                     k_spread_gather<true><<<LIST_GRID, 256, 0, s>>>(skey, n, g, h->bin_first, h->amask, h->words,
                                                                      &sc->n_words, h->ms.fs, h->ms.du, h->G);
@@ -350,7 +383,7 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
     if (pt) pt->mark(PH_LBM, s);
     CollisionConst cc = h->cc;
     cc.shift_forcing = h->opt_forcing;
-    const bool vec = (h->opt_lbm_kernel == 0) && (g.nx % 4 == 0);
+    const bool vec = (h->opt_lbm_kernel == 2) && (g.nx % 4 == 0);
     if (vec) {
         const int nx4 = g.nx / 4;
         int bx = 1;
@@ -473,12 +506,15 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
     if (dmalloc(h, &h->U, cells) || dmalloc(h, &h->G, cells)) return bail("U/G fields");
     if (dmalloc(h, &h->amask, h->n_mask_words) || dmalloc(h, &h->words, h->n_mask_words)) return bail("active mask");
     if (dmalloc(h, &h->bin_first, cells)) return bail("bin map");
+    h->tslot_count = (size_t)(nx + 3) * ny * nz;
+    if (dmalloc(h, &h->tslot, h->tslot_count)) return bail("run slot map");
     if (dmalloc(h, &h->scal, (size_t)1)) return bail("scalars");
     bool ok = true;
     ok &= cudaMemset(h->f[0], 0, cells * NQ * sizeof(float)) == cudaSuccess;   // rest state: f_i - t_i = 0
     ok &= cudaMemset(h->f[1], 0, cells * NQ * sizeof(float)) == cudaSuccess;
     ok &= cudaMemset(h->amask, 0, h->n_mask_words * sizeof(unsigned)) == cudaSuccess;
     ok &= cudaMemset(h->bin_first, 0xff, cells * sizeof(int)) == cudaSuccess;
+    ok &= cudaMemset(h->tslot, 0xff, h->tslot_count * sizeof(int)) == cudaSuccess;
     ok &= cudaMemset(h->scal, 0, sizeof(DevScalars)) == cudaSuccess;
     ok &= cudaDeviceSynchronize() == cudaSuccess;
     if (!ok) { fail(LBM_ECUDA, "%s", cudaGetErrorString(cudaGetLastError())); return bail("memset"); }
@@ -493,7 +529,7 @@ void lbm_destroy(lbm_t *h)
     drop_graphs(h);
     free_markers_dev(h);
     cudaFree(h->f[0]); cudaFree(h->f[1]); cudaFree(h->U); cudaFree(h->G);
-    cudaFree(h->amask); cudaFree(h->words); cudaFree(h->bin_first); cudaFree(h->scal);
+    cudaFree(h->amask); cudaFree(h->words); cudaFree(h->bin_first); cudaFree(h->scal); cudaFree(h->tslot);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     delete h;
 }
@@ -510,10 +546,10 @@ int lbm_set_option(lbm_t *h, int key, int value)
 {
     if (!h) return fail(LBM_EINVAL, "lbm_set_option: NULL handle");
     switch (key) {
-        case LBM_OPT_SPREAD: if (value < 0 || value > 1) break; h->opt_spread = value; return LBM_OK;
+        case LBM_OPT_SPREAD: if (value < 0 || value > 2) break; h->opt_spread = value; return LBM_OK;
         case LBM_OPT_FORCING: if (value < 0 || value > 1) break; h->opt_forcing = value; return LBM_OK;
         case LBM_OPT_GRAPH: if (value < 0 || value > 1) break; h->opt_graph = value; return LBM_OK;
-        case LBM_OPT_LBM_KERNEL: if (value < 0 || value > 1) break; h->opt_lbm_kernel = value; return LBM_OK;
+        case LBM_OPT_LBM_KERNEL: if (value < 0 || value > 2) break; h->opt_lbm_kernel = value; return LBM_OK;
         case LBM_OPT_INTERP: if (value < 0 || value > 1) break; h->opt_interp = value; return LBM_OK;
         case LBM_OPT_TIMING: if (value < 0 || value > 1) break; h->opt_timing = value; h->timer.reset(); return LBM_OK;
         default: return fail(LBM_EINVAL, "lbm_set_option: unknown key %d", key);

@@ -74,7 +74,7 @@ def test_rest_state_is_bitwise_invariant(api):
     sim.close()
 
 
-@pytest.mark.parametrize("kernel", [0, 1])
+@pytest.mark.parametrize("kernel", [1, 2])
 @pytest.mark.parametrize("shape,wall", [((32, 16, 12), (0, 0, 0)), ((36, 10, 9), (1, 0, 1)),
                                         ((20, 7, 6), (1, 1, 1)), ((130, 5, 4), (0, 1, 0)),
                                         ((8, 8, 8), (1, 1, 0))])
@@ -143,7 +143,7 @@ def test_w1_atomic_variant_matches_and_gather_is_deterministic(api, orc):
     from paper_1904_02108_b200 import workloads
     wl = workloads.get("W1")
     outs = []
-    for variant in (api.SPREAD_GATHER, api.SPREAD_GATHER, api.SPREAD_ATOMIC):
+    for variant in (api.SPREAD_GATHER, api.SPREAD_GATHER, api.SPREAD_ATOMIC, api.SPREAD_GATHER_PLAIN):
         sim = api.from_workload(wl, stream=_stream())
         sim.set_option(api.OPT_SPREAD, variant)
         sim.step(20, wl.mdf_iters)
@@ -153,6 +153,8 @@ def test_w1_atomic_variant_matches_and_gather_is_deterministic(api, orc):
         assert np.array_equal(a, b)                 # bitwise run-to-run determinism of the gather path
     assert np.abs(outs[0][1] - outs[2][1]).max() <= 5e-7      # atomic variant: same physics
     assert np.abs(outs[0][3] - outs[2][3]).max() <= 1e-5 * np.abs(outs[0][3]).max()
+    assert np.abs(outs[0][1] - outs[3][1]).max() <= 5e-7      # plain gather-by-cell: same physics
+    assert np.abs(outs[0][3] - outs[3][3]).max() <= 1e-5 * np.abs(outs[0][3]).max()
 
 
 def test_static_markers_with_prescribed_velocity_and_walls(api, orc):
@@ -197,3 +199,48 @@ def test_error_paths(api):
     sim.step(2, 2)
     sim.sync()
     sim.close()
+
+
+# ---- medium-size parity: the five configs' recipes at sizes the oracle finishes in a minute -------
+def _run_pair(api, orc, wl, steps, check_markers=True):
+    sim = api.from_workload(wl, stream=_stream())
+    ref = orc.from_workload(wl)
+    sim.step(steps, wl.mdf_iters)
+    ref.step(steps, wl.mdf_iters)
+    sim.sync()
+    e = _compare_fields(sim, ref)
+    if check_markers and wl.n_markers:
+        _check_markers(sim, ref, orc, wl)
+        _, _, f = sim.read_fields()
+        _, _, rf = ref.read_fields()
+        assert np.abs(f - rf).max() <= 1e-5 * np.abs(rf).max()
+    sim.close()
+    ref.close()
+    return e
+
+
+def test_w2_recipe_128_pure_lbm_100_steps(api, orc):
+    from paper_1904_02108_b200 import workloads
+    e = _run_pair(api, orc, workloads.w2(0, n=128), 100)
+    print("W2-128 errors:", e)
+
+
+def test_w3_full_size_100_steps(api, orc):
+    """configs[2] at full size (128^3, walls on all faces, 15360 markers, 5 MDF iterations)."""
+    from paper_1904_02108_b200 import workloads
+    e = _run_pair(api, orc, workloads.get("W3"), 100)
+    print("W3 errors:", e)
+
+
+def test_w4_recipe_128_100_steps(api, orc):
+    """configs[3] recipe on a 128^3 box: 8 propellers x 8 layers = 147456 markers, periodic."""
+    from paper_1904_02108_b200 import workloads
+    e = _run_pair(api, orc, workloads.w4(0, 8, n=128), 100)
+    print("W4-128 errors:", e)
+
+
+def test_w5_recipe_128_100_steps(api, orc):
+    """configs[4] recipe on a 128^3 box: 8 propellers x 12 layers = 184320 markers, overlapping supports."""
+    from paper_1904_02108_b200 import workloads
+    e = _run_pair(api, orc, workloads.w5(0, 12, n=128), 100)
+    print("W5-128 errors:", e)
