@@ -237,6 +237,9 @@ def run_ours(args):
         line["phases_ms_per_step"] = {k: v / n_ph for k, v in ph.items()}
         line["ibm_share"] = (tot - lbm_ms) / tot if tot > 0 else 0.0
         line["active_cells"] = int(n_active)
+        if wl.n_markers:
+            line["runs"] = sim.get_info(api.INFO_RUNS)
+            line["run_entries"] = sim.get_info(api.INFO_RUN_ENTRIES)
 
         # ---- pure LBM on the same lattice and on configs[1] (W2) ---------------------------------
         sim.step(3, 0)

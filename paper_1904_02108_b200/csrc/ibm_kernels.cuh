@@ -31,11 +31,10 @@ struct MarkerIn {                  // original (caller) order, SoA
 // a1: Rodrigues rotation tables of every body for step n -> n+1, in fp64 (R12, R13).
 // Also re-arms the per-step device counters.
 __global__ void k_kinematics(const BodyDef *__restrict__ defs, BodyStep *__restrict__ out, int nbodies,
-                             const long long *__restrict__ step_ctr, int *__restrict__ n_words,
-                             int *__restrict__ n_runs, int *__restrict__ t_count)
+                             const long long *__restrict__ step_ctr, int *__restrict__ counters, int n_counters)
 {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b == 0) { *n_words = 0; *n_runs = 0; *t_count = 0; }
+    if (b < n_counters) counters[b] = 0;
     if (b >= nbodies) return;
     const BodyDef d = defs[b];
     const double n = (double)(*step_ctr);
@@ -389,38 +388,66 @@ struct RunTable {
 // keep their own entries), holding the T entry or -1.
 __device__ __forceinline__ int tslot_pitch(const Geom &g) { return g.nx + 3; }
 
-// a3 (third part): find the runs, give each its block of T entries and publish them in tslot.
+// a3 (second part): one bit per sorted marker, set where a run starts.  Bits at and beyond n are
+// set as well, so a forward search for the next run start always terminates.
 __global__ void __launch_bounds__(256)
-k_runs(const unsigned *__restrict__ skey, int n, Geom g, RunTable rt, int *__restrict__ tslot,
-       int *__restrict__ n_runs, int *__restrict__ t_count)
+k_run_heads(const unsigned *__restrict__ skey, int n, Geom g, unsigned *__restrict__ headbits)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool head = true;
+    if (i > 0 && i < n) {
+        const unsigned key = skey[i], pk = skey[i - 1];
+        const int row = (int)(key / (unsigned)g.nx), prow = (int)(pk / (unsigned)g.nx);
+        head = (prow != row) || (((int)key - row * g.nx) - ((int)pk - prow * g.nx) >= 4);
+    }
+    const unsigned vote = __ballot_sync(0xffffffffu, head);
+    if ((threadIdx.x & 31) == 0) headbits[i >> 5] = vote;
+}
+
+// set the bits x0..x1 (inclusive, 0 <= x0 <= x1 < nx) of one row of the active-cell mask; the
+// thread that turns a word non-zero appends it to the word list
+__device__ __forceinline__ void mark_span(unsigned *__restrict__ amask, int rowbase, int x0, int x1,
+                                          int *__restrict__ words, int *__restrict__ n_words)
+{
+    for (int w = x0 >> 5; w <= (x1 >> 5); ++w) {
+        const int lo = max(x0 - (w << 5), 0), hi = min(x1 - (w << 5), 31);
+        const unsigned bits = (0xffffffffu >> (31 - hi)) & (0xffffffffu << lo);
+        if (atomicOr(amask + rowbase + w, bits) == 0u) {
+            const unsigned act = __activemask();
+            const int lane = threadIdx.x & 31;
+            const int leader = __ffs(act) - 1;
+            int base = 0;
+            if (lane == leader) base = atomicAdd(n_words, __popc(act));
+            base = __shfl_sync(act, base, leader);
+            words[base + __popc(act & ((1u << lane) - 1u))] = rowbase + w;
+        }
+    }
+}
+
+// a3 (third part): the first marker of every run finds the run's end, takes a block of T entries,
+// publishes them in tslot and marks the run's cells -- the whole x span cx_first-1 .. cx_last+2 in
+// each of the 16 target rows -- in the active-cell bitmask.
+__global__ void __launch_bounds__(256)
+k_runs(const unsigned *__restrict__ skey, int n, Geom g, const unsigned *__restrict__ headbits, RunTable rt,
+       int *__restrict__ tslot, int *__restrict__ n_runs, int *__restrict__ t_count, unsigned *__restrict__ amask,
+       int *__restrict__ words, int *__restrict__ n_words)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
-    bool head = false;
+    const unsigned myword = (i < n) ? headbits[i >> 5] : 0u;
+    const bool head = (myword >> lane) & 1u;
     int row = 0, cx = 0, end = 0, nent = 0;
-    if (i < n) {
-        const unsigned key = skey[i];
+    if (head) {
+        // next set bit after i
+        int wi = i >> 5;
+        unsigned w = (lane == 31) ? 0u : (myword & (0xffffffffu << (lane + 1)));
+        while (w == 0u) w = headbits[++wi];
+        end = (wi << 5) + __ffs(w) - 1;
+        if (end > n) end = n;
+        const unsigned key = skey[i], lk = skey[end - 1];
         row = (int)(key / (unsigned)g.nx);
         cx = (int)key - row * g.nx;
-        if (i == 0) head = true;
-        else {
-            const unsigned pk = skey[i - 1];
-            const int prow = (int)(pk / (unsigned)g.nx);
-            head = (prow != row) || (cx - ((int)pk - prow * g.nx) >= 4);
-        }
-        if (head) {
-            int j = i + 1, last = cx;
-            while (j < n) {
-                const unsigned k2 = skey[j];
-                const int r2 = (int)(k2 / (unsigned)g.nx);
-                const int c2 = (int)k2 - r2 * g.nx;
-                if (r2 != row || c2 - last >= 4) break;
-                last = c2;
-                ++j;
-            }
-            end = j;
-            nent = last - cx + 4;
-        }
+        nent = ((int)lk - row * g.nx) - cx + 4;
     }
     const unsigned vote = __ballot_sync(0xffffffffu, head);
     if (!vote) return;
@@ -435,88 +462,152 @@ k_runs(const unsigned *__restrict__ skey, int n, Geom g, RunTable rt, int *__res
     if (lane == 0) { rbase = atomicAdd(n_runs, __popc(vote)); tbase = atomicAdd(t_count, total); }
     rbase = __shfl_sync(0xffffffffu, rbase, 0);
     tbase = __shfl_sync(0xffffffffu, tbase, 0);
-    if (head) {
-        const int r = rbase + __popc(vote & ((1u << lane) - 1u));
-        const int base = tbase + incl - nent;
-        const int s0 = row * tslot_pitch(g) + cx;        // X = cx - 1  ->  column X + 1 = cx
-        rt.first[r] = i; rt.end[r] = end; rt.base[r] = base; rt.slot0[r] = s0; rt.nent[r] = nent;
-        for (int j = 0; j < nent; ++j) tslot[s0 + j] = base + j;
+    if (!head) return;
+    const int r = rbase + __popc(vote & ((1u << lane) - 1u));
+    const int base = tbase + incl - nent;
+    const int s0 = row * tslot_pitch(g) + cx;        // X = cx - 1  ->  column X + 1 = cx
+    rt.first[r] = i; rt.end[r] = end; rt.base[r] = base; rt.slot0[r] = s0; rt.nent[r] = nent;
+    for (int j = 0; j < nent; ++j) tslot[s0 + j] = base + j;
+    // active cells: x span [cx-1, cx+nent-2], wrapped on a periodic axis (inside the box on a wall axis)
+    const int cz = row / g.ny, cy = row - cz * g.ny;
+    int xa = cx - 1, xb = cx + nent - 2;
+    int x0a, x1a, x0b = 0, x1b = -1;
+    if (nent >= g.nx) { x0a = 0; x1a = g.nx - 1; }
+    else if (xa < 0) { x0a = xa + g.nx; x1a = g.nx - 1; x0b = 0; x1b = xb; }
+    else if (xb >= g.nx) { x0a = xa; x1a = g.nx - 1; x0b = 0; x1b = xb - g.nx; }
+    else { x0a = xa; x1a = xb; }
+    for (int rr = 0; rr < 16; ++rr) {
+        const int y = wrap(cy - 1 + (rr & 3), g.ny);
+        const int z = wrap(cz - 1 + (rr >> 2), g.nz);
+        const int rowbase = (z * g.ny + y) * g.nxw;
+        mark_span(amask, rowbase, x0a, x1a, words, n_words);
+        if (x1b >= x0b) mark_span(amask, rowbase, x0b, x1b, words, n_words);
+    }
+}
+
+// a3 (last part): expand the active words into a list of active cell indices (order arbitrary; every
+// consumer treats the cells independently).
+__global__ void __launch_bounds__(256)
+k_active_cells(Geom g, const unsigned *__restrict__ amask, const int *__restrict__ words,
+               const int *__restrict__ n_words, int *__restrict__ cells, int *__restrict__ n_cells)
+{
+    const int lane = threadIdx.x & 31;
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int stride = gridDim.x * blockDim.x;
+    const int nw = *n_words;
+    for (int k0 = tid - lane; k0 < nw; k0 += stride) {
+        const int k = k0 + lane;
+        int w = 0;
+        unsigned bits = 0u;
+        if (k < nw) { w = words[k]; bits = amask[w]; }
+        const int cnt = __popc(bits);
+        int incl = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        const int total = __shfl_sync(0xffffffffu, incl, 31);
+        int base = 0;
+        if (lane == 0 && total) base = atomicAdd(n_cells, total);
+        base = __shfl_sync(0xffffffffu, base, 0) + incl - cnt;
+        const int row = w / g.nxw;
+        const int cell0 = row * g.nx + (w - row * g.nxw) * 32;
+        while (bits) {
+            const int b = __ffs(bits) - 1;
+            bits &= bits - 1;
+            cells[base++] = cell0 + b;
+        }
     }
 }
 
 // Stage A: one half-warp per run, lane l = jy*4 + jz owns the profile of target-row offset (jy, jz)
 // and keeps a sliding window of four x cells (cxw-1 .. cxw+2) in registers; cells that fall out of
 // the window as the sweep advances are final and are written to T (16 lanes x float4 = 256 B).
+// Runs are handed out through an atomic cursor (they differ a lot in length); the data of marker
+// i+1 is fetched while marker i is accumulated.
+struct Acc3 { float x, y, z; };
+
 __global__ void __launch_bounds__(256)
 k_spread_rows(const unsigned *__restrict__ skey, Geom g, RunTable rt, const int *__restrict__ n_runs,
-              const float4 *__restrict__ fs, const float4 *__restrict__ fq, const float4 *__restrict__ val,
-              float4 *__restrict__ T)
+              int *__restrict__ cursor, const float4 *__restrict__ fs, const float4 *__restrict__ fq,
+              const float4 *__restrict__ val, float4 *__restrict__ T)
 {
-    const int l = threadIdx.x & 15;
+    const int lane = threadIdx.x & 31;
+    const int l = lane & 15;
+    const unsigned hmask = 0xffffu << (lane & 16);
     const int jy = l >> 2, jz = l & 3;
     // w_j(f) = 1/8 (A + B f + C q):  j=0: (3,-2,-1)  1: (3,-2,+1)  2: (1,+2,+1)  3: (1,+2,-1)
     const float ay = (jy < 2) ? 0.375f : 0.125f, by = (jy < 2) ? -0.25f : 0.25f, cy = (jy == 1 || jy == 2) ? 0.125f : -0.125f;
     const float az = (jz < 2) ? 0.375f : 0.125f, bz = (jz < 2) ? -0.25f : 0.25f, cz = (jz == 1 || jz == 2) ? 0.125f : -0.125f;
-    const int hw = (blockIdx.x * blockDim.x + threadIdx.x) >> 4;
-    const int nhw = (gridDim.x * blockDim.x) >> 4;
     const int nr = *n_runs;
-    for (int r = hw; r < nr; r += nhw) {
+    for (;;) {
+        int r = 0;
+        if (l == 0) r = atomicAdd(cursor, 1);
+        r = __shfl_sync(hmask, r, lane & 16);
+        if (r >= nr) break;
         const int i0 = rt.first[r], i1 = rt.end[r];
-        size_t e = (size_t)rt.base[r];
+        float4 *out = T + (size_t)rt.base[r] * 16 + l;
         const unsigned key0 = skey[i0];
         const int rowx = (int)(key0 / (unsigned)g.nx) * g.nx;
         int cxw = (int)key0 - rowx;
-        float a0x = 0.f, a0y = 0.f, a0z = 0.f, a1x = 0.f, a1y = 0.f, a1z = 0.f;
-        float a2x = 0.f, a2y = 0.f, a2z = 0.f, a3x = 0.f, a3y = 0.f, a3z = 0.f;
+        Acc3 a0{0.f, 0.f, 0.f}, a1{0.f, 0.f, 0.f}, a2{0.f, 0.f, 0.f}, a3{0.f, 0.f, 0.f};
+        // software pipeline: (cx, f, q, v) of the next marker
+        int ncx = cxw;
+        float4 nf = fs[i0], nq = fq[i0], nv = val[i0];
         for (int i = i0; i < i1; ++i) {
-            const int cx = (int)skey[i] - rowx;
-            const float4 f = fs[i];
-            const float4 q = fq[i];
-            const float4 v = val[i];
-            while (cxw < cx) {
-                T[e * 16 + l] = make_float4(a0x, a0y, a0z, 0.f);
-                a0x = a1x; a0y = a1y; a0z = a1z;
-                a1x = a2x; a1y = a2y; a1z = a2z;
-                a2x = a3x; a2y = a3y; a2z = a3z;
-                a3x = 0.f; a3y = 0.f; a3z = 0.f;
-                ++e; ++cxw;
+            const int cx = ncx;
+            const float4 f = nf, q = nq, v = nv;
+            if (i + 1 < i1) {
+                ncx = (int)skey[i + 1] - rowx;
+                nf = fs[i + 1]; nq = fq[i + 1]; nv = val[i + 1];
+            }
+            if (cx != cxw) {
+                // the window moves right by 1..3 cells: its leftmost cells are complete
+                const int sh = cx - cxw;
+                out[0] = make_float4(a0.x, a0.y, a0.z, 0.f);
+                if (sh > 1) out[16] = make_float4(a1.x, a1.y, a1.z, 0.f);
+                if (sh > 2) out[32] = make_float4(a2.x, a2.y, a2.z, 0.f);
+                const Acc3 zero{0.f, 0.f, 0.f};
+                const Acc3 b0 = sh == 1 ? a1 : (sh == 2 ? a2 : a3);
+                const Acc3 b1 = sh == 1 ? a2 : (sh == 2 ? a3 : zero);
+                const Acc3 b2 = sh == 1 ? a3 : zero;
+                a0 = b0; a1 = b1; a2 = b2; a3 = zero;
+                out += 16 * sh;
+                cxw = cx;
             }
             const float wyz = fmaf(cy, q.y, fmaf(by, f.y, ay)) * fmaf(cz, q.z, fmaf(bz, f.z, az));
             const float vx = v.x * wyz, vy = v.y * wyz, vz = v.z * wyz;
             const float lo = fmaf(-0.25f, f.x, 0.375f), hi = fmaf(0.25f, f.x, 0.125f), qq = 0.125f * q.x;
             const float w0 = lo - qq, w1 = lo + qq, w2 = hi + qq, w3 = hi - qq;
-            a0x = fmaf(w0, vx, a0x); a0y = fmaf(w0, vy, a0y); a0z = fmaf(w0, vz, a0z);
-            a1x = fmaf(w1, vx, a1x); a1y = fmaf(w1, vy, a1y); a1z = fmaf(w1, vz, a1z);
-            a2x = fmaf(w2, vx, a2x); a2y = fmaf(w2, vy, a2y); a2z = fmaf(w2, vz, a2z);
-            a3x = fmaf(w3, vx, a3x); a3y = fmaf(w3, vy, a3y); a3z = fmaf(w3, vz, a3z);
+            a0.x = fmaf(w0, vx, a0.x); a0.y = fmaf(w0, vy, a0.y); a0.z = fmaf(w0, vz, a0.z);
+            a1.x = fmaf(w1, vx, a1.x); a1.y = fmaf(w1, vy, a1.y); a1.z = fmaf(w1, vz, a1.z);
+            a2.x = fmaf(w2, vx, a2.x); a2.y = fmaf(w2, vy, a2.y); a2.z = fmaf(w2, vz, a2.z);
+            a3.x = fmaf(w3, vx, a3.x); a3.y = fmaf(w3, vy, a3.y); a3.z = fmaf(w3, vz, a3.z);
         }
-        T[e * 16 + l] = make_float4(a0x, a0y, a0z, 0.f);
-        T[(e + 1) * 16 + l] = make_float4(a1x, a1y, a1z, 0.f);
-        T[(e + 2) * 16 + l] = make_float4(a2x, a2y, a2z, 0.f);
-        T[(e + 3) * 16 + l] = make_float4(a3x, a3y, a3z, 0.f);
+        out[0] = make_float4(a0.x, a0.y, a0.z, 0.f);
+        out[16] = make_float4(a1.x, a1.y, a1.z, 0.f);
+        out[32] = make_float4(a2.x, a2.y, a2.z, 0.f);
+        out[48] = make_float4(a3.x, a3.y, a3.z, 0.f);
     }
 }
 
-// Stage B: one warp per active word, one lane per active cell: add the profiles of the source rows
-// (y+1-jy, z+1-jz) at this x, jy and jz ascending (fixed order).
+// Stage B: one thread per active cell: add the profiles of the source rows (y+1-jy, z+1-jz) at this
+// x, jy and jz ascending (fixed order).
 //   LAST = false:  U^{m+1}(X) = U^m(X) + sum   (R8)      LAST = true:  G(X) = sum
 template <bool LAST>
 __global__ void __launch_bounds__(256)
 k_spread_collect(Geom g, const int *__restrict__ tslot, const float4 *__restrict__ T,
-                 const unsigned *__restrict__ amask, const int *__restrict__ words, const int *__restrict__ n_words,
-                 float4 *__restrict__ field)
+                 const int *__restrict__ cells, const int *__restrict__ n_cells, float4 *__restrict__ field)
 {
-    const int lane = threadIdx.x & 31;
-    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int nwarps = (gridDim.x * blockDim.x) >> 5;
-    const int nw = *n_words;
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int stride = gridDim.x * blockDim.x;
+    const int nc = *n_cells;
     const int pitch = tslot_pitch(g);
-    for (int k = warp; k < nw; k += nwarps) {
-        const int w = __ldg(words + k);
-        const unsigned bits = __ldg(amask + w);
-        if (!((bits >> lane) & 1u)) continue;
-        const int row = w / g.nxw;
-        const int x = (w - row * g.nxw) * 32 + lane;
+    for (int k = tid; k < nc; k += stride) {
+        const int cell = __ldg(cells + k);
+        const int row = cell / g.nx;
+        const int x = cell - row * g.nx;
         const int z = row / g.ny, y = row - z * g.ny;
         // ghost columns of a periodic x axis: X = x + nx (for x <= 1) and X = -1 (for x = nx-1)
         const int ghost = g.wallx ? -1 : (x <= 1 ? x + g.nx + 1 : (x == g.nx - 1 ? 0 : -1));
@@ -544,7 +635,6 @@ k_spread_collect(Geom g, const int *__restrict__ tslot, const float4 *__restrict
                 }
             }
         }
-        const size_t cell = (size_t)row * g.nx + x;
         if (LAST) {
             field[cell] = make_float4(sx, sy, sz, 0.f);
         } else {

@@ -43,15 +43,21 @@ int fail(int code, const char *fmt, ...)
                         #expr, cudaGetErrorString(e_), __FILE__, __LINE__);                        \
     } while (0)
 
+constexpr int MAX_MDF = 64;
+
 struct DevScalars {
     long long step_ctr;  // time step n of the step being computed (kinematics angle)
-    int n_words;         // active words of the current / last IBM step
     int n_prev;          // sorted markers whose bins are still registered in bin_first
     int status;          // != 0: a stencil crossed a wall
     int scratch;
+    // ---- zeroed at the start of every IBM step (k_kinematics), after k_clear_prev has used them
+    int n_words;         // active words of the current / last IBM step
     int n_runs;          // runs of the current / last IBM step
     int t_count;         // T entries handed out in the current / last IBM step
+    int n_cells;         // active cells of the current / last IBM step
+    int cursor[MAX_MDF]; // work cursors of the run sweeps, one per MDF iteration
 };
+constexpr int N_STEP_COUNTERS = 4 + MAX_MDF;
 
 struct HostBody {
     long long first, count;
@@ -124,8 +130,12 @@ struct lbm {
     MarkerSorted ms{nullptr, nullptr, nullptr, nullptr, nullptr};
     RunTable rt{nullptr, nullptr, nullptr, nullptr, nullptr};
     int *tslot = nullptr;               // dense [row][X+1] -> T entry map (pitch nx+3)
+    int *cells = nullptr;               // active-cell list
+    unsigned *headbits = nullptr;       // one bit per sorted marker: starts a run
+    size_t cells_cap = 0, headbits_cap = 0;
     float4 *T = nullptr;                // run profiles, 16 float4 per entry
     size_t t_cap = 0, tslot_count = 0;
+    int rows_grid = 148;                // persistent grid of the run sweep (blocks resident at once)
     int sort_ipw = 64, sort_tiles = 0, sort_passes = 1;
 
     int opt_spread = 0, opt_forcing = 0, opt_graph = 1, opt_lbm_kernel = 0, opt_interp = 0, opt_timing = 0;
@@ -177,6 +187,8 @@ void free_markers_dev(lbm *h)
     dfree(h, h->rt.first, c); dfree(h, h->rt.end, c); dfree(h, h->rt.base, c); dfree(h, h->rt.slot0, c);
     dfree(h, h->rt.nent, c);
     dfree(h, h->T, h->t_cap * 16); h->t_cap = 0;
+    dfree(h, h->cells, h->cells_cap); h->cells_cap = 0;
+    dfree(h, h->headbits, h->headbits_cap); h->headbits_cap = 0;
     dfree(h, h->d_hist, (size_t)RADIX * (size_t)h->sort_tiles);
     dfree(h, h->d_total, (size_t)RADIX);
     dfree(h, h->d_defs, (size_t)h->nb_cap);
@@ -203,6 +215,7 @@ int flush_ibm(lbm *h)
     k_set_scalars<<<1, 1, 0, h->stream>>>(&h->scal->step_ctr, h->steps_done, &h->scal->n_prev, 0, 1 | 2);
     CK(cudaMemsetAsync(&h->scal->n_words, 0, sizeof(int), h->stream));
     CK(cudaMemsetAsync(&h->scal->n_runs, 0, sizeof(int), h->stream));
+    CK(cudaMemsetAsync(&h->scal->n_cells, 0, sizeof(int), h->stream));
     CK(cudaGetLastError());
     h->launches += 2;
     h->ibm_dirty = false;
@@ -242,6 +255,10 @@ int upload_markers(lbm *h)
         if ((rc = dmalloc(h, &h->rt.nent, c))) return rc;
         h->t_cap = std::min((size_t)4 * c, h->tslot_count);
         if ((rc = dmalloc(h, &h->T, h->t_cap * 16))) return rc;
+        h->cells_cap = std::min((size_t)64 * c, (size_t)h->g.cells);
+        if ((rc = dmalloc(h, &h->cells, h->cells_cap))) return rc;
+        h->headbits_cap = c / 32 + 16;
+        if ((rc = dmalloc(h, &h->headbits, h->headbits_cap))) return rc;
         if ((rc = dmalloc(h, &h->ms.uk, c))) return rc;
         if ((rc = dmalloc(h, &h->ms.sg, c))) return rc;
         if ((rc = dmalloc(h, &h->ms.du, c))) return rc;
@@ -319,8 +336,8 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
         k_clear_prev<<<LIST_GRID, 256, 0, s>>>(skey, &sc->n_prev, h->bin_first, h->amask, h->words, &sc->n_words,
                                                h->tslot, h->rt.slot0, h->rt.nent, &sc->n_runs);
         const int nb = (int)h->bodies.size();
-        k_kinematics<<<(nb + 127) / 128, 128, 0, s>>>(h->d_defs, h->d_tabs, nb, &sc->step_ctr, &sc->n_words, &sc->n_runs,
-                                                      &sc->t_count);
+        k_kinematics<<<(std::max(nb, N_STEP_COUNTERS) + 127) / 128, 128, 0, s>>>(h->d_defs, h->d_tabs, nb, &sc->step_ctr,
+                                                                                  &sc->n_words, N_STEP_COUNTERS);
         k_marker_keys<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, h->d_keys[0], &sc->status);
         nk += 3;
         if (pt) pt->mark(PH_SORT, s);
@@ -338,11 +355,19 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
         }
         if (pt) pt->mark(PH_BINS, s);
         k_marker_gather<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, perm, h->ms);
-        k_bins<<<mb, 256, 0, s>>>(skey, n, g, h->bin_first, h->amask, h->words, &sc->n_words);
-        if (h->opt_spread == 0) { k_runs<<<mb, 256, 0, s>>>(skey, n, g, h->rt, h->tslot, &sc->n_runs, &sc->t_count); ++nk; }
+        if (h->opt_spread == 0) {
+            k_run_heads<<<(n + 32 + 255) / 256, 256, 0, s>>>(skey, n, g, h->headbits);
+            k_runs<<<mb, 256, 0, s>>>(skey, n, g, h->headbits, h->rt, h->tslot, &sc->n_runs, &sc->t_count, h->amask,
+                                      h->words, &sc->n_words);
+            ++nk;
+        } else {
+            k_bins<<<mb, 256, 0, s>>>(skey, n, g, h->bin_first, h->amask, h->words, &sc->n_words);
+        }
+        k_active_cells<<<LIST_GRID, 256, 0, s>>>(g, h->amask, h->words, &sc->n_words, h->cells, &sc->n_cells);
+        ++nk;
         k_set_scalars<<<1, 1, 0, s>>>(&sc->step_ctr, 0, &sc->n_prev, n, 2 | 4);
         if (pt) pt->mark(PH_MOMENTS, s);
-        k_moments_active<<<LIST_GRID, 256, 0, s>>>(src, g, h->amask, h->words, &sc->n_words, h->U);
+        k_moments_active<<<LIST_GRID, 256, 0, s>>>(src, g, h->cells, &sc->n_cells, h->U);
         nk += 4;
         for (int m = 0; m < mdf_iters; ++m) {
             const bool last = (m == mdf_iters - 1);
@@ -351,14 +376,12 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
             ++nk;
             if (pt) pt->mark(PH_SPREAD, s);
             if (h->opt_spread == 0) {
-                k_spread_rows<<<LIST_GRID, 256, 0, s>>>(skey, g, h->rt, &sc->n_runs, h->ms.fs, h->ms.fq,
-                                                        last ? h->ms.du : h->ms.sg, h->T);
+                k_spread_rows<<<h->rows_grid, 256, 0, s>>>(skey, g, h->rt, &sc->n_runs, &sc->cursor[m], h->ms.fs,
+                                                           h->ms.fq, last ? h->ms.du : h->ms.sg, h->T);
                 if (last)
-                    k_spread_collect<true><<<LIST_GRID, 256, 0, s>>>(g, h->tslot, h->T, h->amask, h->words,
-                                                                      &sc->n_words, h->G);
+                    k_spread_collect<true><<<LIST_GRID, 256, 0, s>>>(g, h->tslot, h->T, h->cells, &sc->n_cells, h->G);
                 else
-                    k_spread_collect<false><<<LIST_GRID, 256, 0, s>>>(g, h->tslot, h->T, h->amask, h->words,
-                                                                       &sc->n_words, h->U);
+                    k_spread_collect<false><<<LIST_GRID, 256, 0, s>>>(g, h->tslot, h->T, h->cells, &sc->n_cells, h->U);
                 nk += 2;
             } else if (h->opt_spread == 2) {
                 if (last)
@@ -393,10 +416,24 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
         if (ibm) k_stream_collide_vec4<true><<<gr, b, 0, s>>>(src, dst, g, cc, h->amask, h->G);
         else k_stream_collide_vec4<false><<<gr, b, 0, s>>>(src, dst, g, cc, nullptr, nullptr);
     } else {
-        dim3 b = cell_block(g);
-        dim3 gr = cell_grid(g, b);
-        if (ibm) k_stream_collide_scalar<true><<<gr, b, 0, s>>>(src, dst, g, cc, h->amask, h->G);
-        else k_stream_collide_scalar<false><<<gr, b, 0, s>>>(src, dst, g, cc, nullptr, nullptr);
+        // variants of the one-cell-per-thread kernel: (threads per block, min blocks per SM)
+        auto launch = [&](auto kern_ibm, auto kern_pure, int threads) {
+            int bx = g.nx >= threads ? threads : ((g.nx + 31) / 32) * 32;
+            int by = threads / bx; if (by < 1) by = 1;
+            dim3 b(bx, by, 1);
+            dim3 gr = cell_grid(g, b);
+            if (ibm) kern_ibm<<<gr, b, 0, s>>>(src, dst, g, cc, h->amask, h->G);
+            else kern_pure<<<gr, b, 0, s>>>(src, dst, g, cc, nullptr, nullptr);
+        };
+        switch (h->opt_lbm_kernel) {
+            case 3: launch(k_stream_collide_scalar<true, 256, 5>, k_stream_collide_scalar<false, 256, 5>, 256); break;
+            case 4: launch(k_stream_collide_scalar<true, 256, 6>, k_stream_collide_scalar<false, 256, 6>, 256); break;
+            case 5: launch(k_stream_collide_scalar<true, 128, 8>, k_stream_collide_scalar<false, 128, 8>, 128); break;
+            case 6: launch(k_stream_collide_scalar<true, 128, 10>, k_stream_collide_scalar<false, 128, 10>, 128); break;
+            case 7: launch(k_stream_collide_scalar<true, 512, 2>, k_stream_collide_scalar<false, 512, 2>, 512); break;
+            case 8: launch(k_stream_collide_scalar<true, 128, 12>, k_stream_collide_scalar<false, 128, 12>, 128); break;
+            default: launch(k_stream_collide_scalar<true, 256, 4>, k_stream_collide_scalar<false, 256, 4>, 256); break;
+        }
     }
     ++nk;
     if (pt) pt->mark(-1, s);
@@ -448,14 +485,6 @@ bool stencil_inside(const lbm *h, const double lo[3], const double hi[3])
         if (std::floor(lo[a]) < 1.0 || std::floor(hi[a]) > (double)(n[a] - 3)) return false;
     }
     return true;
-}
-
-__global__ void k_count_active(const unsigned *amask, const int *words, const int *n_words, int *out)
-{
-    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
-    int c = 0;
-    for (int i = tid; i < *n_words; i += gridDim.x * blockDim.x) c += __popc(amask[words[i]]);
-    if (c) atomicAdd(out, c);
 }
 
 }  // namespace
@@ -518,6 +547,12 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
     ok &= cudaMemset(h->scal, 0, sizeof(DevScalars)) == cudaSuccess;
     ok &= cudaDeviceSynchronize() == cudaSuccess;
     if (!ok) { fail(LBM_ECUDA, "%s", cudaGetErrorString(cudaGetLastError())); return bail("memset"); }
+    {
+        int per_sm = 0, sms = 148;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spread_rows, 256, 0);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device);
+        h->rows_grid = std::max(1, per_sm) * sms;
+    }
     g_err.clear();
     return h;
 }
@@ -549,7 +584,7 @@ int lbm_set_option(lbm_t *h, int key, int value)
         case LBM_OPT_SPREAD: if (value < 0 || value > 2) break; h->opt_spread = value; return LBM_OK;
         case LBM_OPT_FORCING: if (value < 0 || value > 1) break; h->opt_forcing = value; return LBM_OK;
         case LBM_OPT_GRAPH: if (value < 0 || value > 1) break; h->opt_graph = value; return LBM_OK;
-        case LBM_OPT_LBM_KERNEL: if (value < 0 || value > 2) break; h->opt_lbm_kernel = value; return LBM_OK;
+        case LBM_OPT_LBM_KERNEL: if (value < 0 || value > 8) break; h->opt_lbm_kernel = value; return LBM_OK;
         case LBM_OPT_INTERP: if (value < 0 || value > 1) break; h->opt_interp = value; return LBM_OK;
         case LBM_OPT_TIMING: if (value < 0 || value > 1) break; h->opt_timing = value; h->timer.reset(); return LBM_OK;
         default: return fail(LBM_EINVAL, "lbm_set_option: unknown key %d", key);
@@ -569,9 +604,17 @@ int lbm_get_info(lbm_t *h, int key, long long *value)
         case LBM_INFO_ACTIVE_CELLS: {
             int r = 0;
             if (h->force_valid) {
-                CK(cudaMemsetAsync(&h->scal->scratch, 0, sizeof(int), h->stream));
-                k_count_active<<<256, 256, 0, h->stream>>>(h->amask, h->words, &h->scal->n_words, &h->scal->scratch);
-                CK(cudaMemcpyAsync(&r, &h->scal->scratch, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+                CK(cudaMemcpyAsync(&r, &h->scal->n_cells, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+                CK(cudaStreamSynchronize(h->stream));
+            }
+            *value = r;
+            return LBM_OK;
+        }
+        case LBM_INFO_RUNS: case LBM_INFO_RUN_ENTRIES: {
+            int r = 0;
+            if (h->force_valid) {
+                CK(cudaMemcpyAsync(&r, key == LBM_INFO_RUNS ? &h->scal->n_runs : &h->scal->t_count, sizeof(int),
+                                   cudaMemcpyDeviceToHost, h->stream));
                 CK(cudaStreamSynchronize(h->stream));
             }
             *value = r;
@@ -750,6 +793,7 @@ int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
 {
     if (!h) return fail(LBM_EINVAL, "lbm_ibm_step: NULL handle");
     if (nsteps < 0 || mdf_iters < 0) return fail(LBM_EINVAL, "lbm_ibm_step: negative count");
+    if (mdf_iters > MAX_MDF) return fail(LBM_EINVAL, "lbm_ibm_step: at most %d MDF iterations", MAX_MDF);
     if (nsteps == 0) return LBM_OK;
     int rc = upload_markers(h);
     if (rc) return rc;

@@ -74,11 +74,38 @@ __device__ __forceinline__ bool cell_is_active(const unsigned *__restrict__ amas
     return (w >> (x & 31)) & 1u;
 }
 
+// Pull for a cell whose y and z neighbours are plain lattice rows (no wrap, no wall): every source
+// row sits at a constant offset from the cell's own row; only x needs the wrapped neighbour, and an
+// x wall the bounce-back select.
+__device__ __forceinline__ void pull_cell_inner(const float *__restrict__ src, const Geom &g, int x, int self,
+                                                float (&df)[NQ])
+{
+    const size_t cells = (size_t)g.cells;
+    const int dxm = (x == 0) ? g.nx - 1 : -1;          // offset to the cell at x-1 (wrapped)
+    const int dxp = (x == g.nx - 1) ? 1 - g.nx : 1;    // offset to the cell at x+1 (wrapped)
+    const bool wlo = g.wallx && x == 0, whi = g.wallx && x == g.nx - 1;
+    const int sy = g.nx, sz = g.nx * g.ny;
+    const float *__restrict__ p = src + self;
+#pragma unroll
+    for (int i = 0; i < NQ; ++i) {
+        const int off = (dir_ex(i) == 1 ? dxm : (dir_ex(i) == -1 ? dxp : 0)) - dir_ey(i) * sy - dir_ez(i) * sz;
+        if (dir_ex(i) == 0) {
+            df[i] = __ldg(p + ((size_t)i * cells + off));
+        } else {
+            const bool behind = dir_ex(i) == 1 ? wlo : whi;
+            const long long o = behind ? (long long)((size_t)dir_opp(i) * cells) : (long long)((size_t)i * cells) + off;
+            df[i] = __ldg(p + o);
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------
-// a8, scalar variant: one thread per cell, x along threadIdx.x (coalesced 128 B per warp and plane).
-// IBM = true reads one bitmask word per warp-row and G only where a marker stencil reaches.
-template <bool IBM>
-__global__ void __launch_bounds__(256)
+// a8, one thread per cell, x along threadIdx.x (coalesced 128 B per warp and plane), one x-row
+// segment per block so that "is this an interior row" is block-uniform.  IBM = true reads one
+// bitmask word per warp and G only where a marker stencil reaches; both are issued before the
+// population loads so their latency overlaps.
+template <bool IBM, int THREADS, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
 k_stream_collide_scalar(const float *__restrict__ src, float *__restrict__ dst, Geom g, CollisionConst cc,
                         const unsigned *__restrict__ amask, const float4 *__restrict__ G)
 {
@@ -86,23 +113,27 @@ k_stream_collide_scalar(const float *__restrict__ src, float *__restrict__ dst, 
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
     const int z = blockIdx.z;
     if (x >= g.nx || y >= g.ny) return;
-
-    const Nbr n = neighbours(g, x, y, z);
-    float df[NQ];
-    pull_cell(src, g, n, x, y, z, df);
+    const int self = (z * g.ny + y) * g.nx + x;
 
     float ax = cc.gbx, ay = cc.gby, az = cc.gbz;
-    const int self = (z * g.ny + y) * g.nx + x;
     if (IBM) {
         if (cell_is_active(amask, g, x, y, z)) {
             const float4 gv = __ldg(G + self);
             ax += gv.x; ay += gv.y; az += gv.z;
         }
     }
+    float df[NQ];
+    if (y > 0 && y < g.ny - 1 && z > 0 && z < g.nz - 1) {
+        pull_cell_inner(src, g, x, self, df);
+    } else {
+        const Nbr n = neighbours(g, x, y, z);
+        pull_cell(src, g, n, x, y, z, df);
+    }
     collide(df, ax, ay, az, cc);
     const size_t cells = (size_t)g.cells;
+    float *__restrict__ q = dst + self;
 #pragma unroll
-    for (int i = 0; i < NQ; ++i) __stcs(dst + (size_t)i * cells + self, df[i]);
+    for (int i = 0; i < NQ; ++i) __stcs(q + (size_t)i * cells, df[i]);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -272,29 +303,26 @@ k_read_fields(const float *__restrict__ src, Geom g, const unsigned *__restrict_
     }
 }
 
-// a4: rho, U of eq. (1) for the cells of the active words only (the paper's "kernel strategy",
-// P:215, de-duplicated): one warp per 32-cell word of the bitmask, lanes whose bit is set pull
-// their 19 populations.  U is stored as float4 (Ux, Uy, Uz, rho).
+// a4: rho, U of eq. (1) for the active cells only (the paper's "kernel strategy", P:215,
+// de-duplicated): one thread per entry of the active-cell list pulls its 19 populations.
+// U is stored as float4 (Ux, Uy, Uz, rho).
 __global__ void __launch_bounds__(256)
-k_moments_active(const float *__restrict__ src, Geom g, const unsigned *__restrict__ amask,
-                 const int *__restrict__ words, const int *__restrict__ n_words, float4 *__restrict__ U)
+k_moments_active(const float *__restrict__ src, Geom g, const int *__restrict__ cells,
+                 const int *__restrict__ n_cells, float4 *__restrict__ U)
 {
-    const int lane = threadIdx.x & 31;
-    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int nwarps = (gridDim.x * blockDim.x) >> 5;
-    const int nw = *n_words;
-    for (int k = warp; k < nw; k += nwarps) {
-        const int w = __ldg(words + k);
-        const unsigned bits = __ldg(amask + w);
-        if (!((bits >> lane) & 1u)) continue;
-        const int row = w / g.nxw;
-        const int x = (w - row * g.nxw) * 32 + lane;
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int stride = gridDim.x * blockDim.x;
+    const int nc = *n_cells;
+    for (int k = tid; k < nc; k += stride) {
+        const int cell = __ldg(cells + k);
+        const int row = cell / g.nx;
+        const int x = cell - row * g.nx;
         const int z = row / g.ny, y = row - z * g.ny;
         const Nbr n = neighbours(g, x, y, z);
         float df[NQ], drho, ux, uy, uz;
         pull_cell(src, g, n, x, y, z, df);
         moments(df, drho, ux, uy, uz);
-        U[(size_t)row * g.nx + x] = make_float4(ux, uy, uz, 1.0f + drho);
+        U[cell] = make_float4(ux, uy, uz, 1.0f + drho);
     }
 }
 
