@@ -108,10 +108,25 @@ k_marker_keys(MarkerIn m, const BodyDef *__restrict__ defs, const BodyStep *__re
     keys[k] = (unsigned)((p.cz * g.ny + p.cy) * g.nx + p.cx);
 }
 
+// Peskin 4-point weights of the cells c-1, c, c+1, c+2 for a point at c + f, 0 <= f < 1 (P:84, R6).
+// The four distances 1+f, f, 1-f, 2-f share one square root: 1 + 4r - 4r^2 at r = f or 1-f and
+// -7 + 12r - 4r^2 at r = 1+f or 2-f all equal 1 + 4f - 4f^2.
+__device__ __forceinline__ void peskin4(float f, float (&w)[4])
+{
+    const float q = peskin_root(f);
+    const float a = 3.0f - 2.0f * f, b = 1.0f + 2.0f * f;
+    w[0] = 0.125f * (a - q);
+    w[1] = 0.125f * (a + q);
+    w[2] = 0.125f * (b + q);
+    w[3] = 0.125f * (b - q);
+}
+
 // per-marker state in SORTED order
 struct MarkerSorted {
     float4 *fs;     // (fx, fy, fz, s)
-    float4 *fq;     // (qx, qy, qz, -), q = sqrt(1 + 4f - 4f^2): the one square root of the four weights
+    float4 *wx;     // the four x weights w(x_k - X), X = cx-1 .. cx+2
+    float *wyz;     // [16] per marker: w_y(jy) w_z(jz) at index jy*4+jz
+                    // sg.w and du.w carry the marker's cell x index (int bits) for the run sweep
     float4 *uk;     // prescribed velocity u_k, w unused
     float4 *sg;     // s * g^m(k)   (what the U update spreads, P:98 + R8)
     float4 *du;     // Delta u(k)
@@ -130,13 +145,22 @@ k_marker_gather(MarkerIn m, const BodyDef *__restrict__ defs, const BodyStep *__
     const float qx = m.qx[k], qy = m.qy[k], qz = m.qz[k];
     const Placed p = place_marker(defs[b], t, qx, qy, qz, g);
     out.fs[i] = make_float4(p.fx, p.fy, p.fz, m.s[k]);
-    out.fq[i] = make_float4(peskin_root(p.fx), peskin_root(p.fy), peskin_root(p.fz), 0.f);
+
     const float ux = fmaf(t.dR[0], qx, fmaf(t.dR[1], qy, fmaf(t.dR[2], qz, m.vx[k])));
     const float uy = fmaf(t.dR[3], qx, fmaf(t.dR[4], qy, fmaf(t.dR[5], qz, m.vy[k])));
     const float uz = fmaf(t.dR[6], qx, fmaf(t.dR[7], qy, fmaf(t.dR[8], qz, m.vz[k])));
     out.uk[i] = make_float4(ux, uy, uz, 0.f);
-    out.du[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    out.sg[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    out.du[i] = make_float4(0.f, 0.f, 0.f, __int_as_float(p.cx));
+    out.sg[i] = make_float4(0.f, 0.f, 0.f, __int_as_float(p.cx));
+    // per-step weight tables of the run sweep (the position does not change during the MDF loop)
+    float wx[4], wy[4], wz[4];
+    peskin4(p.fx, wx);
+    peskin4(p.fy, wy);
+    peskin4(p.fz, wz);
+    out.wx[i] = make_float4(wx[0], wx[1], wx[2], wx[3]);
+    float4 *w16 = reinterpret_cast<float4 *>(out.wyz + (size_t)i * 16);
+#pragma unroll
+    for (int jy = 0; jy < 4; ++jy) w16[jy] = make_float4(wy[jy] * wz[0], wy[jy] * wz[1], wy[jy] * wz[2], wy[jy] * wz[3]);
 }
 
 __device__ __forceinline__ void key_to_cell(unsigned key, const Geom &g, int &cx, int &cy, int &cz)
@@ -235,19 +259,6 @@ __global__ void k_set_scalars(long long *step_ctr, long long step, int *n_prev, 
     if (mode & 4) *step_ctr += 1;
 }
 
-// Peskin 4-point weights of the cells c-1, c, c+1, c+2 for a point at c + f, 0 <= f < 1 (P:84, R6).
-// The four distances 1+f, f, 1-f, 2-f share one square root: 1 + 4r - 4r^2 at r = f or 1-f and
-// -7 + 12r - 4r^2 at r = 1+f or 2-f all equal 1 + 4f - 4f^2.
-__device__ __forceinline__ void peskin4(float f, float (&w)[4])
-{
-    const float q = peskin_root(f);
-    const float a = 3.0f - 2.0f * f, b = 1.0f + 2.0f * f;
-    w[0] = 0.125f * (a - q);
-    w[1] = 0.125f * (a + q);
-    w[2] = 0.125f * (b + q);
-    w[3] = 0.125f * (b - q);
-}
-
 // a5 + a6, thread-per-marker variant over the sorted markers: u^m(k) = sum U^m W;
 // g = u_k - u^m(k); Delta u += s g (R9).
 __global__ void __launch_bounds__(128)
@@ -290,8 +301,8 @@ k_interp_correct(const unsigned *__restrict__ skey, int n, Geom g, const float4 
     du.x = fmaf(fs.w, gx, du.x);
     du.y = fmaf(fs.w, gy, du.y);
     du.z = fmaf(fs.w, gz, du.z);
-    m.du[i] = du;
-    m.sg[i] = make_float4(fs.w * gx, fs.w * gy, fs.w * gz, 0.f);
+    m.du[i] = du;                                    // du.w keeps the cell x index
+    m.sg[i] = make_float4(fs.w * gx, fs.w * gy, fs.w * gz, du.w);
 }
 
 // weight of the cell at offset j (0..3 <-> c-1..c+2) only
@@ -424,13 +435,10 @@ __device__ __forceinline__ void mark_span(unsigned *__restrict__ amask, int rowb
     }
 }
 
-// a3 (third part): the first marker of every run finds the run's end, takes a block of T entries,
-// publishes them in tslot and marks the run's cells -- the whole x span cx_first-1 .. cx_last+2 in
-// each of the 16 target rows -- in the active-cell bitmask.
+// a3 (third part): the first marker of every run finds the run's end and takes a block of T entries.
 __global__ void __launch_bounds__(256)
 k_runs(const unsigned *__restrict__ skey, int n, Geom g, const unsigned *__restrict__ headbits, RunTable rt,
-       int *__restrict__ tslot, int *__restrict__ n_runs, int *__restrict__ t_count, unsigned *__restrict__ amask,
-       int *__restrict__ words, int *__restrict__ n_words)
+       int *__restrict__ n_runs, int *__restrict__ t_count)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
@@ -467,18 +475,35 @@ k_runs(const unsigned *__restrict__ skey, int n, Geom g, const unsigned *__restr
     const int base = tbase + incl - nent;
     const int s0 = row * tslot_pitch(g) + cx;        // X = cx - 1  ->  column X + 1 = cx
     rt.first[r] = i; rt.end[r] = end; rt.base[r] = base; rt.slot0[r] = s0; rt.nent[r] = nent;
-    for (int j = 0; j < nent; ++j) tslot[s0 + j] = base + j;
-    // active cells: x span [cx-1, cx+nent-2], wrapped on a periodic axis (inside the box on a wall axis)
-    const int cz = row / g.ny, cy = row - cz * g.ny;
-    int xa = cx - 1, xb = cx + nent - 2;
-    int x0a, x1a, x0b = 0, x1b = -1;
-    if (nent >= g.nx) { x0a = 0; x1a = g.nx - 1; }
-    else if (xa < 0) { x0a = xa + g.nx; x1a = g.nx - 1; x0b = 0; x1b = xb; }
-    else if (xb >= g.nx) { x0a = xa; x1a = g.nx - 1; x0b = 0; x1b = xb - g.nx; }
-    else { x0a = xa; x1a = xb; }
-    for (int rr = 0; rr < 16; ++rr) {
-        const int y = wrap(cy - 1 + (rr & 3), g.ny);
-        const int z = wrap(cz - 1 + (rr >> 2), g.nz);
+}
+
+// a3 (fourth part): one half-warp per run publishes the run: its T entries go into tslot and its
+// cells -- the whole x span cx_first-1 .. cx_last+2 in each of the 16 target rows, one row per lane
+// -- are marked in the active-cell bitmask.
+__global__ void __launch_bounds__(256)
+k_run_publish(Geom g, RunTable rt, const int *__restrict__ n_runs, int *__restrict__ tslot,
+              unsigned *__restrict__ amask, int *__restrict__ words, int *__restrict__ n_words)
+{
+    const int l = threadIdx.x & 15;
+    const int hw = (blockIdx.x * blockDim.x + threadIdx.x) >> 4;
+    const int nhw = (gridDim.x * blockDim.x) >> 4;
+    const int nr = *n_runs;
+    const int pitch = tslot_pitch(g);
+    for (int r = hw; r < nr; r += nhw) {
+        const int s0 = rt.slot0[r], nent = rt.nent[r], base = rt.base[r];
+        for (int j = l; j < nent; j += 16) tslot[s0 + j] = base + j;
+        const int row = s0 / pitch;
+        const int cx = s0 - row * pitch;
+        const int cz = row / g.ny, cy = row - cz * g.ny;
+        // x span [cx-1, cx+nent-2], wrapped on a periodic axis (inside the box on a wall axis)
+        const int xa = cx - 1, xb = cx + nent - 2;
+        int x0a, x1a, x0b = 0, x1b = -1;
+        if (nent >= g.nx) { x0a = 0; x1a = g.nx - 1; }
+        else if (xa < 0) { x0a = xa + g.nx; x1a = g.nx - 1; x0b = 0; x1b = xb; }
+        else if (xb >= g.nx) { x0a = xa; x1a = g.nx - 1; x0b = 0; x1b = xb - g.nx; }
+        else { x0a = xa; x1a = xb; }
+        const int y = wrap(cy - 1 + (l >> 2), g.ny);
+        const int z = wrap(cz - 1 + (l & 3), g.nz);
         const int rowbase = (z * g.ny + y) * g.nxw;
         mark_span(amask, rowbase, x0a, x1a, words, n_words);
         if (x1b >= x0b) mark_span(amask, rowbase, x0b, x1b, words, n_words);
@@ -529,17 +554,13 @@ k_active_cells(Geom g, const unsigned *__restrict__ amask, const int *__restrict
 struct Acc3 { float x, y, z; };
 
 __global__ void __launch_bounds__(256)
-k_spread_rows(const unsigned *__restrict__ skey, Geom g, RunTable rt, const int *__restrict__ n_runs,
-              int *__restrict__ cursor, const float4 *__restrict__ fs, const float4 *__restrict__ fq,
-              const float4 *__restrict__ val, float4 *__restrict__ T)
+k_spread_rows(RunTable rt, const int *__restrict__ n_runs, int *__restrict__ cursor,
+              const float4 *__restrict__ wx4, const float *__restrict__ wyz16, const float4 *__restrict__ val,
+              float4 *__restrict__ T)
 {
     const int lane = threadIdx.x & 31;
     const int l = lane & 15;
     const unsigned hmask = 0xffffu << (lane & 16);
-    const int jy = l >> 2, jz = l & 3;
-    // w_j(f) = 1/8 (A + B f + C q):  j=0: (3,-2,-1)  1: (3,-2,+1)  2: (1,+2,+1)  3: (1,+2,-1)
-    const float ay = (jy < 2) ? 0.375f : 0.125f, by = (jy < 2) ? -0.25f : 0.25f, cy = (jy == 1 || jy == 2) ? 0.125f : -0.125f;
-    const float az = (jz < 2) ? 0.375f : 0.125f, bz = (jz < 2) ? -0.25f : 0.25f, cz = (jz == 1 || jz == 2) ? 0.125f : -0.125f;
     const int nr = *n_runs;
     for (;;) {
         int r = 0;
@@ -548,20 +569,18 @@ k_spread_rows(const unsigned *__restrict__ skey, Geom g, RunTable rt, const int 
         if (r >= nr) break;
         const int i0 = rt.first[r], i1 = rt.end[r];
         float4 *out = T + (size_t)rt.base[r] * 16 + l;
-        const unsigned key0 = skey[i0];
-        const int rowx = (int)(key0 / (unsigned)g.nx) * g.nx;
-        int cxw = (int)key0 - rowx;
         Acc3 a0{0.f, 0.f, 0.f}, a1{0.f, 0.f, 0.f}, a2{0.f, 0.f, 0.f}, a3{0.f, 0.f, 0.f};
-        // software pipeline: (cx, f, q, v) of the next marker
-        int ncx = cxw;
-        float4 nf = fs[i0], nq = fq[i0], nv = val[i0];
+        // software pipeline: the data of marker i+1 is in flight while marker i is accumulated
+        const float4 *pv = val + i0, *pw = wx4 + i0;
+        const float *pz = wyz16 + (size_t)i0 * 16 + l;
+        float4 nv = *pv, nw = *pw;
+        float nz = *pz;
+        int cxw = __float_as_int(nv.w);
         for (int i = i0; i < i1; ++i) {
-            const int cx = ncx;
-            const float4 f = nf, q = nq, v = nv;
-            if (i + 1 < i1) {
-                ncx = (int)skey[i + 1] - rowx;
-                nf = fs[i + 1]; nq = fq[i + 1]; nv = val[i + 1];
-            }
+            const float4 v = nv, w = nw;
+            const float wyz = nz;
+            if (i + 1 < i1) { nv = *++pv; nw = *++pw; pz += 16; nz = *pz; }
+            const int cx = __float_as_int(v.w);
             if (cx != cxw) {
                 // the window moves right by 1..3 cells: its leftmost cells are complete
                 const int sh = cx - cxw;
@@ -576,14 +595,11 @@ k_spread_rows(const unsigned *__restrict__ skey, Geom g, RunTable rt, const int 
                 out += 16 * sh;
                 cxw = cx;
             }
-            const float wyz = fmaf(cy, q.y, fmaf(by, f.y, ay)) * fmaf(cz, q.z, fmaf(bz, f.z, az));
             const float vx = v.x * wyz, vy = v.y * wyz, vz = v.z * wyz;
-            const float lo = fmaf(-0.25f, f.x, 0.375f), hi = fmaf(0.25f, f.x, 0.125f), qq = 0.125f * q.x;
-            const float w0 = lo - qq, w1 = lo + qq, w2 = hi + qq, w3 = hi - qq;
-            a0.x = fmaf(w0, vx, a0.x); a0.y = fmaf(w0, vy, a0.y); a0.z = fmaf(w0, vz, a0.z);
-            a1.x = fmaf(w1, vx, a1.x); a1.y = fmaf(w1, vy, a1.y); a1.z = fmaf(w1, vz, a1.z);
-            a2.x = fmaf(w2, vx, a2.x); a2.y = fmaf(w2, vy, a2.y); a2.z = fmaf(w2, vz, a2.z);
-            a3.x = fmaf(w3, vx, a3.x); a3.y = fmaf(w3, vy, a3.y); a3.z = fmaf(w3, vz, a3.z);
+            a0.x = fmaf(w.x, vx, a0.x); a0.y = fmaf(w.x, vy, a0.y); a0.z = fmaf(w.x, vz, a0.z);
+            a1.x = fmaf(w.y, vx, a1.x); a1.y = fmaf(w.y, vy, a1.y); a1.z = fmaf(w.y, vz, a1.z);
+            a2.x = fmaf(w.z, vx, a2.x); a2.y = fmaf(w.z, vy, a2.y); a2.z = fmaf(w.z, vz, a2.z);
+            a3.x = fmaf(w.w, vx, a3.x); a3.y = fmaf(w.w, vy, a3.y); a3.z = fmaf(w.w, vz, a3.z);
         }
         out[0] = make_float4(a0.x, a0.y, a0.z, 0.f);
         out[16] = make_float4(a1.x, a1.y, a1.z, 0.f);

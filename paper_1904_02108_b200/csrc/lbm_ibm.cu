@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <new>
@@ -127,7 +128,7 @@ struct lbm {
     unsigned *d_keys[2] = {nullptr, nullptr};
     int *d_vals[2] = {nullptr, nullptr};
     int *d_hist = nullptr, *d_total = nullptr;
-    MarkerSorted ms{nullptr, nullptr, nullptr, nullptr, nullptr};
+    MarkerSorted ms{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     RunTable rt{nullptr, nullptr, nullptr, nullptr, nullptr};
     int *tslot = nullptr;               // dense [row][X+1] -> T entry map (pitch nx+3)
     int *cells = nullptr;               // active-cell list
@@ -183,7 +184,7 @@ void free_markers_dev(lbm *h)
     dfree(h, h->d_s, c);
     dfree(h, h->d_body, c);
     for (int a = 0; a < 2; ++a) { dfree(h, h->d_keys[a], c); dfree(h, h->d_vals[a], c); }
-    dfree(h, h->ms.fs, c); dfree(h, h->ms.fq, c); dfree(h, h->ms.uk, c); dfree(h, h->ms.sg, c); dfree(h, h->ms.du, c);
+    dfree(h, h->ms.fs, c); dfree(h, h->ms.wx, c); dfree(h, h->ms.wyz, 16 * c); dfree(h, h->ms.uk, c); dfree(h, h->ms.sg, c); dfree(h, h->ms.du, c);
     dfree(h, h->rt.first, c); dfree(h, h->rt.end, c); dfree(h, h->rt.base, c); dfree(h, h->rt.slot0, c);
     dfree(h, h->rt.nent, c);
     dfree(h, h->T, h->t_cap * 16); h->t_cap = 0;
@@ -247,7 +248,8 @@ int upload_markers(lbm *h)
             if ((rc = dmalloc(h, &h->d_vals[a], c))) return rc;
         }
         if ((rc = dmalloc(h, &h->ms.fs, c))) return rc;
-        if ((rc = dmalloc(h, &h->ms.fq, c))) return rc;
+        if ((rc = dmalloc(h, &h->ms.wx, c))) return rc;
+        if ((rc = dmalloc(h, &h->ms.wyz, 16 * c))) return rc;
         if ((rc = dmalloc(h, &h->rt.first, c))) return rc;
         if ((rc = dmalloc(h, &h->rt.end, c))) return rc;
         if ((rc = dmalloc(h, &h->rt.base, c))) return rc;
@@ -357,9 +359,9 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
         k_marker_gather<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, perm, h->ms);
         if (h->opt_spread == 0) {
             k_run_heads<<<(n + 32 + 255) / 256, 256, 0, s>>>(skey, n, g, h->headbits);
-            k_runs<<<mb, 256, 0, s>>>(skey, n, g, h->headbits, h->rt, h->tslot, &sc->n_runs, &sc->t_count, h->amask,
-                                      h->words, &sc->n_words);
-            ++nk;
+            k_runs<<<mb, 256, 0, s>>>(skey, n, g, h->headbits, h->rt, &sc->n_runs, &sc->t_count);
+            k_run_publish<<<LIST_GRID, 256, 0, s>>>(g, h->rt, &sc->n_runs, h->tslot, h->amask, h->words, &sc->n_words);
+            nk += 2;
         } else {
             k_bins<<<mb, 256, 0, s>>>(skey, n, g, h->bin_first, h->amask, h->words, &sc->n_words);
         }
@@ -376,8 +378,8 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
             ++nk;
             if (pt) pt->mark(PH_SPREAD, s);
             if (h->opt_spread == 0) {
-                k_spread_rows<<<h->rows_grid, 256, 0, s>>>(skey, g, h->rt, &sc->n_runs, &sc->cursor[m], h->ms.fs,
-                                                           h->ms.fq, last ? h->ms.du : h->ms.sg, h->T);
+                k_spread_rows<<<h->rows_grid, 256, 0, s>>>(h->rt, &sc->n_runs, &sc->cursor[m], h->ms.wx, h->ms.wyz,
+                                                           last ? h->ms.du : h->ms.sg, h->T);
                 if (last)
                     k_spread_collect<true><<<LIST_GRID, 256, 0, s>>>(g, h->tslot, h->T, h->cells, &sc->n_cells, h->G);
                 else
@@ -516,6 +518,14 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
     h->g.nx = nx; h->g.ny = ny; h->g.nz = nz;
     h->g.nxw = (nx + 31) / 32;
     h->g.cells = (long long)nx * ny * nz;
+    {
+        // plane padding: 0 by default; LBM_PLANE_PAD (floats, multiple of 4) for experiments
+        long long pad = 0;
+        if (const char *e = std::getenv("LBM_PLANE_PAD")) pad = std::atoll(e);
+        if (pad < 0) pad = 0;
+        pad = (pad + 3) / 4 * 4;
+        h->g.pitch = (h->g.cells + 3) / 4 * 4 + pad;
+    }
     h->g.wallx = bc ? (bc->wall_x != 0) : 0;
     h->g.wally = bc ? (bc->wall_y != 0) : 0;
     h->g.wallz = bc ? (bc->wall_z != 0) : 0;
@@ -531,7 +541,8 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
     const size_t cells = (size_t)h->g.cells;
     h->n_mask_words = (size_t)h->g.nxw * ny * nz;
     if (cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return bail("stream");
-    if (dmalloc(h, &h->f[0], cells * NQ) || dmalloc(h, &h->f[1], cells * NQ)) return bail("populations");
+    const size_t fcount = (size_t)h->g.pitch * NQ;
+    if (dmalloc(h, &h->f[0], fcount) || dmalloc(h, &h->f[1], fcount)) return bail("populations");
     if (dmalloc(h, &h->U, cells) || dmalloc(h, &h->G, cells)) return bail("U/G fields");
     if (dmalloc(h, &h->amask, h->n_mask_words) || dmalloc(h, &h->words, h->n_mask_words)) return bail("active mask");
     if (dmalloc(h, &h->bin_first, cells)) return bail("bin map");
@@ -539,8 +550,8 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
     if (dmalloc(h, &h->tslot, h->tslot_count)) return bail("run slot map");
     if (dmalloc(h, &h->scal, (size_t)1)) return bail("scalars");
     bool ok = true;
-    ok &= cudaMemset(h->f[0], 0, cells * NQ * sizeof(float)) == cudaSuccess;   // rest state: f_i - t_i = 0
-    ok &= cudaMemset(h->f[1], 0, cells * NQ * sizeof(float)) == cudaSuccess;
+    ok &= cudaMemset(h->f[0], 0, fcount * sizeof(float)) == cudaSuccess;   // rest state: f_i - t_i = 0
+    ok &= cudaMemset(h->f[1], 0, fcount * sizeof(float)) == cudaSuccess;
     ok &= cudaMemset(h->amask, 0, h->n_mask_words * sizeof(unsigned)) == cudaSuccess;
     ok &= cudaMemset(h->bin_first, 0xff, cells * sizeof(int)) == cudaSuccess;
     ok &= cudaMemset(h->tslot, 0xff, h->tslot_count * sizeof(int)) == cudaSuccess;

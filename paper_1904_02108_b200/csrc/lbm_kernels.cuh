@@ -9,12 +9,43 @@
 #pragma once
 #include "d3q19.cuh"
 
+// cache operators of the population streams (each value is read once and written once per step);
+// the modes exist for measurement builds, the defaults are the ones measured fastest.
+#ifndef LBM_LD_MODE
+#define LBM_LD_MODE 0
+#endif
+#ifndef LBM_ST_MODE
+#define LBM_ST_MODE 0
+#endif
+#if LBM_LD_MODE == 1
+#define LBM_LOAD(p) __ldcs(p)
+#elif LBM_LD_MODE == 2
+#define LBM_LOAD(p) __ldlu(p)
+#elif LBM_LD_MODE == 3
+#define LBM_LOAD(p) __ldcg(p)
+#elif LBM_LD_MODE == 4
+#define LBM_LOAD(p) (*(p))
+#else
+#define LBM_LOAD(p) __ldg(p)
+#endif
+#if LBM_ST_MODE == 1
+#define LBM_STORE(p, v) (*(p) = (v))
+#elif LBM_ST_MODE == 2
+#define LBM_STORE(p, v) __stcg(p, v)
+#elif LBM_ST_MODE == 3
+#define LBM_STORE(p, v) __stwt(p, v)
+#else
+#define LBM_STORE(p, v) __stcs(p, v)
+#endif
+
 namespace lbmk {
 
 struct Geom {
     int nx, ny, nz;
     int nxw;             // 32-cell words per x-row of the active-cell bitmask
     long long cells;
+    long long pitch;     // floats between two population planes (>= cells; padding staggers the
+                         // 19 read and 19 write streams over the memory channels)
     int wallx, wally, wallz;
 };
 
@@ -47,7 +78,7 @@ __device__ __forceinline__ Nbr neighbours(const Geom &g, int x, int y, int z)
 __device__ __forceinline__ void pull_cell(const float *__restrict__ src, const Geom &g, const Nbr &n, int x, int y,
                                           int z, float (&df)[NQ])
 {
-    const size_t cells = (size_t)g.cells;
+    const size_t cells = (size_t)g.pitch;
     const int self = (z * g.ny + y) * g.nx + x;
 #pragma unroll
     for (int i = 0; i < NQ; ++i) {
@@ -64,7 +95,7 @@ __device__ __forceinline__ void pull_cell(const float *__restrict__ src, const G
         if (dir_ez(i) == -1) behind_wall |= n.wzp;
         const int cell = behind_wall ? self : (sz * g.ny + sy) * g.nx + sx;
         const int plane = behind_wall ? dir_opp(i) : i;
-        df[i] = __ldg(src + (size_t)plane * cells + cell);
+        df[i] = LBM_LOAD(src + (size_t)plane * cells + cell);
     }
 }
 
@@ -80,7 +111,7 @@ __device__ __forceinline__ bool cell_is_active(const unsigned *__restrict__ amas
 __device__ __forceinline__ void pull_cell_inner(const float *__restrict__ src, const Geom &g, int x, int self,
                                                 float (&df)[NQ])
 {
-    const size_t cells = (size_t)g.cells;
+    const size_t cells = (size_t)g.pitch;
     const int dxm = (x == 0) ? g.nx - 1 : -1;          // offset to the cell at x-1 (wrapped)
     const int dxp = (x == g.nx - 1) ? 1 - g.nx : 1;    // offset to the cell at x+1 (wrapped)
     const bool wlo = g.wallx && x == 0, whi = g.wallx && x == g.nx - 1;
@@ -90,11 +121,11 @@ __device__ __forceinline__ void pull_cell_inner(const float *__restrict__ src, c
     for (int i = 0; i < NQ; ++i) {
         const int off = (dir_ex(i) == 1 ? dxm : (dir_ex(i) == -1 ? dxp : 0)) - dir_ey(i) * sy - dir_ez(i) * sz;
         if (dir_ex(i) == 0) {
-            df[i] = __ldg(p + ((size_t)i * cells + off));
+            df[i] = LBM_LOAD(p + ((size_t)i * cells + off));
         } else {
             const bool behind = dir_ex(i) == 1 ? wlo : whi;
             const long long o = behind ? (long long)((size_t)dir_opp(i) * cells) : (long long)((size_t)i * cells) + off;
-            df[i] = __ldg(p + o);
+            df[i] = LBM_LOAD(p + o);
         }
     }
 }
@@ -130,10 +161,10 @@ k_stream_collide_scalar(const float *__restrict__ src, float *__restrict__ dst, 
         pull_cell(src, g, n, x, y, z, df);
     }
     collide(df, ax, ay, az, cc);
-    const size_t cells = (size_t)g.cells;
+    const size_t cells = (size_t)g.pitch;
     float *__restrict__ q = dst + self;
 #pragma unroll
-    for (int i = 0; i < NQ; ++i) __stcs(q + (size_t)i * cells, df[i]);
+    for (int i = 0; i < NQ; ++i) LBM_STORE(q + (size_t)i * cells, df[i]);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -153,7 +184,7 @@ k_stream_collide_vec4(const float *__restrict__ src, float *__restrict__ dst, Ge
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
     const int z = blockIdx.z;
     const bool live = (x4 < nx4) && (y < g.ny);
-    const size_t cells = (size_t)g.cells;
+    const size_t cells = (size_t)g.pitch;
     const unsigned lane = (threadIdx.y * blockDim.x + threadIdx.x) & 31u;
 
     // clamp dead threads onto a valid cell so that shuffles stay convergent; they do not store
@@ -252,6 +283,7 @@ k_init_fields(float *__restrict__ buf, Geom g, const float *__restrict__ rho0, c
     const int z = blockIdx.z;
     if (x >= g.nx || y >= g.ny) return;
     const size_t cells = (size_t)g.cells;
+    const size_t pitch = (size_t)g.pitch;
     const int self = (z * g.ny + y) * g.nx + x;
     const float drho = rho0 ? (rho0[self] - 1.0f) : 0.0f;
     const float ux = u0 ? u0[self] : 0.0f;
@@ -272,7 +304,7 @@ k_init_fields(float *__restrict__ buf, Geom g, const float *__restrict__ rho0, c
         if (dir_ez(i) == -1) behind_wall |= n.wzp;
         const int cell = behind_wall ? self : (sz * g.ny + sy) * g.nx + sx;
         const int plane = behind_wall ? dir_opp(i) : i;
-        buf[(size_t)plane * cells + cell] = equilibrium_dev(i, drho, ux, uy, uz);
+        buf[(size_t)plane * pitch + cell] = equilibrium_dev(i, drho, ux, uy, uz);
     }
 }
 
