@@ -570,36 +570,46 @@ k_spread_rows(RunTable rt, const int *__restrict__ n_runs, int *__restrict__ cur
         const int i0 = rt.first[r], i1 = rt.end[r];
         float4 *out = T + (size_t)rt.base[r] * 16 + l;
         Acc3 a0{0.f, 0.f, 0.f}, a1{0.f, 0.f, 0.f}, a2{0.f, 0.f, 0.f}, a3{0.f, 0.f, 0.f};
-        // software pipeline: the data of marker i+1 is in flight while marker i is accumulated
-        const float4 *pv = val + i0, *pw = wx4 + i0;
-        const float *pz = wyz16 + (size_t)i0 * 16 + l;
-        float4 nv = *pv, nw = *pw;
-        float nz = *pz;
-        int cxw = __float_as_int(nv.w);
-        for (int i = i0; i < i1; ++i) {
-            const float4 v = nv, w = nw;
-            const float wyz = nz;
-            if (i + 1 < i1) { nv = *++pv; nw = *++pw; pz += 16; nz = *pz; }
-            const int cx = __float_as_int(v.w);
-            if (cx != cxw) {
-                // the window moves right by 1..3 cells: its leftmost cells are complete
-                const int sh = cx - cxw;
-                out[0] = make_float4(a0.x, a0.y, a0.z, 0.f);
-                if (sh > 1) out[16] = make_float4(a1.x, a1.y, a1.z, 0.f);
-                if (sh > 2) out[32] = make_float4(a2.x, a2.y, a2.z, 0.f);
-                const Acc3 zero{0.f, 0.f, 0.f};
-                const Acc3 b0 = sh == 1 ? a1 : (sh == 2 ? a2 : a3);
-                const Acc3 b1 = sh == 1 ? a2 : (sh == 2 ? a3 : zero);
-                const Acc3 b2 = sh == 1 ? a3 : zero;
-                a0 = b0; a1 = b1; a2 = b2; a3 = zero;
-                out += 16 * sh;
-                cxw = cx;
+        // markers are taken in batches of RB: all loads of a batch are issued before the first
+        // marker is accumulated, so the memory latency is paid once per batch, not once per marker
+        constexpr int RB = 4;
+        int cxw = __float_as_int(val[i0].w);
+        for (int ib = i0; ib < i1; ib += RB) {
+            float4 bv[RB], bw[RB];
+            float bz[RB];
+#pragma unroll
+            for (int j = 0; j < RB; ++j) {
+                const int i = min(ib + j, i1 - 1);
+                bv[j] = val[i];
+                bw[j] = wx4[i];
+                bz[j] = wyz16[(size_t)i * 16 + l];
             }
-            const float vx = v.x * wyz, vy = v.y * wyz, vz = v.z * wyz;
-            a0.x = fmaf(w.x, vx, a0.x); a0.y = fmaf(w.x, vy, a0.y); a0.z = fmaf(w.x, vz, a0.z);
-            a1.x = fmaf(w.y, vx, a1.x); a1.y = fmaf(w.y, vy, a1.y); a1.z = fmaf(w.y, vz, a1.z);
-            a2.x = fmaf(w.z, vx, a2.x); a2.y = fmaf(w.z, vy, a2.y); a2.z = fmaf(w.z, vz, a2.z);
-            a3.x = fmaf(w.w, vx, a3.x); a3.y = fmaf(w.w, vy, a3.y); a3.z = fmaf(w.w, vz, a3.z);
+#pragma unroll
+            for (int j = 0; j < RB; ++j) {
+                if (ib + j < i1) {
+                    const float4 v = bv[j], w = bw[j];
+                    const int cx = __float_as_int(v.w);
+                    if (cx != cxw) {
+                        // the window moves right by 1..3 cells: its leftmost cells are complete
+                        const int sh = cx - cxw;
+                        out[0] = make_float4(a0.x, a0.y, a0.z, 0.f);
+                        if (sh > 1) out[16] = make_float4(a1.x, a1.y, a1.z, 0.f);
+                        if (sh > 2) out[32] = make_float4(a2.x, a2.y, a2.z, 0.f);
+                        const Acc3 zero{0.f, 0.f, 0.f};
+                        const Acc3 b0 = sh == 1 ? a1 : (sh == 2 ? a2 : a3);
+                        const Acc3 b1 = sh == 1 ? a2 : (sh == 2 ? a3 : zero);
+                        const Acc3 b2 = sh == 1 ? a3 : zero;
+                        a0 = b0; a1 = b1; a2 = b2; a3 = zero;
+                        out += 16 * sh;
+                        cxw = cx;
+                    }
+                    const float vx = v.x * bz[j], vy = v.y * bz[j], vz = v.z * bz[j];
+                    a0.x = fmaf(w.x, vx, a0.x); a0.y = fmaf(w.x, vy, a0.y); a0.z = fmaf(w.x, vz, a0.z);
+                    a1.x = fmaf(w.y, vx, a1.x); a1.y = fmaf(w.y, vy, a1.y); a1.z = fmaf(w.y, vz, a1.z);
+                    a2.x = fmaf(w.z, vx, a2.x); a2.y = fmaf(w.z, vy, a2.y); a2.z = fmaf(w.z, vz, a2.z);
+                    a3.x = fmaf(w.w, vx, a3.x); a3.y = fmaf(w.w, vy, a3.y); a3.z = fmaf(w.w, vz, a3.z);
+                }
+            }
         }
         out[0] = make_float4(a0.x, a0.y, a0.z, 0.f);
         out[16] = make_float4(a1.x, a1.y, a1.z, 0.f);

@@ -428,13 +428,13 @@ int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, in
             else kern_pure<<<gr, b, 0, s>>>(src, dst, g, cc, nullptr, nullptr);
         };
         switch (h->opt_lbm_kernel) {
-            case 3: launch(k_stream_collide_scalar<true, 256, 5>, k_stream_collide_scalar<false, 256, 5>, 256); break;
+            case 3: launch(k_stream_collide_scalar<true, 256, 4>, k_stream_collide_scalar<false, 256, 4>, 256); break;
             case 4: launch(k_stream_collide_scalar<true, 256, 6>, k_stream_collide_scalar<false, 256, 6>, 256); break;
             case 5: launch(k_stream_collide_scalar<true, 128, 8>, k_stream_collide_scalar<false, 128, 8>, 128); break;
             case 6: launch(k_stream_collide_scalar<true, 128, 10>, k_stream_collide_scalar<false, 128, 10>, 128); break;
             case 7: launch(k_stream_collide_scalar<true, 512, 2>, k_stream_collide_scalar<false, 512, 2>, 512); break;
             case 8: launch(k_stream_collide_scalar<true, 128, 12>, k_stream_collide_scalar<false, 128, 12>, 128); break;
-            default: launch(k_stream_collide_scalar<true, 256, 4>, k_stream_collide_scalar<false, 256, 4>, 256); break;
+            default: launch(k_stream_collide_scalar<true, 256, 5>, k_stream_collide_scalar<false, 256, 5>, 256); break;
         }
     }
     ++nk;

@@ -15,7 +15,7 @@
 #define LBM_LD_MODE 0
 #endif
 #ifndef LBM_ST_MODE
-#define LBM_ST_MODE 0
+#define LBM_ST_MODE 1
 #endif
 #if LBM_LD_MODE == 1
 #define LBM_LOAD(p) __ldcs(p)
@@ -29,7 +29,7 @@
 #define LBM_LOAD(p) __ldg(p)
 #endif
 #if LBM_ST_MODE == 1
-#define LBM_STORE(p, v) (*(p) = (v))
+#define LBM_STORE(p, v) (*(p) = (v))      /* plain write-back stores: measured 2-3 % faster than .cs */
 #elif LBM_ST_MODE == 2
 #define LBM_STORE(p, v) __stcg(p, v)
 #elif LBM_ST_MODE == 3
