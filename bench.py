@@ -47,12 +47,20 @@ def measured_peak_gbs():
 
 
 def traffic_from_profile(workload):
-    """dram bytes per launch of the stream-collide kernel from the committed ncu capture, or None"""
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stream-collide kernel from the
+    newest committed ncu --set full summary (profiles/traffic_rNN.csv), or None"""
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
-            return json.load(fh).get(workload)
+        pdir = os.path.join(ROOT, "profiles")
+        files = sorted(f for f in os.listdir(pdir) if f.startswith("traffic_r") and f.endswith(".csv"))
+        for name in reversed(files):
+            with open(os.path.join(pdir, name)) as fh:
+                for line in fh.read().splitlines()[1:]:
+                    w, _, b = line.rsplit(",", 2)[0].split(",", 1)[0], None, line.rsplit(",", 1)[1]
+                    if w == workload:
+                        return float(b)
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
