@@ -61,12 +61,19 @@ enum {
                              2 = plain gather-by-cell over the bins (slow reference variant)        */
     LBM_OPT_FORCING = 2,  /* 0 = Guo source term (default, R3), 1 = paper's shift U + tau G */
     LBM_OPT_GRAPH = 3,    /* 1 = replay the step as a CUDA graph (default), 0 = plain launches     */
-    LBM_OPT_LBM_KERNEL = 4, /* stream-collide variant: 0 = default (the faster one), 1 = one cell per
-                             thread, 2 = four cells per thread with 128-bit accesses (nx % 4 == 0)    */
+    LBM_OPT_LBM_KERNEL = 4, /* stream-collide variant: 0 = default, 1 = one cell per thread (the default),
+                             2 = four cells per thread with 128-bit accesses (nx % 4 == 0; comparison;
+                             used for the pure and the serial fused pass only)                     */
     LBM_OPT_INTERP = 5,   /* interpolation variant: 0 = default, 1 = thread per marker            */
-    LBM_OPT_TIMING = 6    /* 1 = run steps as plain launches with CUDA events between the phases and
+    LBM_OPT_TIMING = 6,   /* 1 = run steps as plain launches with CUDA events between the phases and
                              accumulate per-phase device time (LBM_INFO_PHASE_NS); setting it resets
                              the accumulators.  Each step then ends with a stream synchronise.     */
+    LBM_OPT_OVERLAP = 7   /* 1 (default) = a coupled step runs as three concurrent graph branches: the
+                             MDF loop, the stream-collide of every cell outside the marker stencils
+                             (it needs no IBM force), and the binning of the NEXT step's markers (P:154:
+                             positions depend on time only); the cells inside the stencils are updated
+                             after the join.  0 = the same step as one serial chain with a single fused
+                             stream-collide pass (measured comparison).  Results are identical.        */
 };
 
 /* Keys for lbm_get_info. */
@@ -83,7 +90,8 @@ enum {
     LBM_INFO_PHASE_NS = 100     /* + phase: accumulated device time in ns under LBM_OPT_TIMING.
                                    phases: 0 kinematics+keys, 1 sort, 2 gather+bins, 3 moments on
                                    active cells, 4 interpolation+correction, 5 spreading,
-                                   6 stream-collide                                              */
+                                   6 stream-collide (with LBM_OPT_OVERLAP: the pass over the cells
+                                   outside the stencils), 7 stream-collide of the active cells     */
 };
 
 /* P:31 + eq.(3): allocate an nx*ny*nz D3Q19 lattice with relaxation time tau on the current CUDA

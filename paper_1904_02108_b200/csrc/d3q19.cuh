@@ -58,7 +58,7 @@ __device__ __forceinline__ void moments(const float (&df)[NQ], float &drho, floa
         if (dir_ez(i) == 1) jz += df[i];
         if (dir_ez(i) == -1) jz -= df[i];
     }
-    const float inv = 1.0f / (1.0f + s);
+    const float inv = __fdividef(1.0f, 1.0f + s);   // MUFU.RCP, relative error < 2^-22
     drho = s;
     ux = jx * inv;
     uy = jy * inv;
@@ -77,17 +77,27 @@ __device__ __forceinline__ void collide(float (&df)[NQ], float ax, float ay, flo
     const float rho = 1.0f + drho;
     const float h = c.shift_forcing ? c.tau : 0.5f;
     const float vx = fmaf(h, ax, ux), vy = fmaf(h, ay, uy), vz = fmaf(h, az, uz);
-    const float uu15 = 1.5f * (vx * vx + vy * vy + vz * vz);
-    const float va3 = 3.0f * (vx * ax + vy * ay + vz * az);
-    const float sg = c.shift_forcing ? 0.0f : c.guo;
+    // The update of direction i splits into a part even in e_i and a part odd in e_i, shared by the
+    // pair (i, opp i) = (i, 18 - i).  With A = rho/tau, B = (1 - 1/(2 tau)) rho (B = 0 for the shift):
+    //   even_i = t_i [ drho/tau - 1.5 A v.v - 3 B v.a + (e.v) (e.(4.5 A v + 9 B a)) ]
+    //   odd_i  = t_i  e.(3 A v + 3 B a)
+    //   f_i <- keep f_i + even_i + odd_i,   f_opp <- keep f_opp + even_i - odd_i
+    const float A = c.omega * rho;
+    const float B = c.shift_forcing ? 0.0f : c.guo * rho;
+    const float c0 = fmaf(c.omega, drho, -(1.5f * A * (vx * vx + vy * vy + vz * vz) + 3.0f * B * (vx * ax + vy * ay + vz * az)));
+    const float qx = fmaf(4.5f * A, vx, 9.0f * B * ax), qy = fmaf(4.5f * A, vy, 9.0f * B * ay), qz = fmaf(4.5f * A, vz, 9.0f * B * az);
+    const float px = 3.0f * fmaf(A, vx, B * ax), py = 3.0f * fmaf(A, vy, B * ay), pz = 3.0f * fmaf(A, vz, B * az);
+    df[9] = fmaf(c.keep, df[9], dir_weight(9) * c0);
 #pragma unroll
-    for (int i = 0; i < NQ; ++i) {
-        const float eu = dir_ex(i) * vx + dir_ey(i) * vy + dir_ez(i) * vz;
-        const float ea = dir_ex(i) * ax + dir_ey(i) * ay + dir_ez(i) * az;
+    for (int i = 0; i < 9; ++i) {
         const float w = dir_weight(i);
-        const float eqd = w * fmaf(rho, fmaf(eu, fmaf(4.5f, eu, 3.0f), -uu15), drho);
-        const float src = sg * w * rho * (fmaf(9.0f * eu, ea, 3.0f * ea) - va3);
-        df[i] = fmaf(c.keep, df[i], fmaf(c.omega, eqd, src));
+        const float ev = dir_ex(i) * vx + dir_ey(i) * vy + dir_ez(i) * vz;
+        const float eq = dir_ex(i) * qx + dir_ey(i) * qy + dir_ez(i) * qz;
+        const float ep = dir_ex(i) * px + dir_ey(i) * py + dir_ez(i) * pz;
+        const float even = w * fmaf(ev, eq, c0);
+        const float odd = w * ep;
+        df[i] = fmaf(c.keep, df[i], even + odd);
+        df[dir_opp(i)] = fmaf(c.keep, df[dir_opp(i)], even - odd);
     }
 }
 

@@ -29,15 +29,17 @@ struct MarkerIn {                  // original (caller) order, SoA
 };
 
 // a1: Rodrigues rotation tables of every body for step n -> n+1, in fp64 (R12, R13).
-// Also re-arms the per-step device counters.
+// Also re-arms the per-step device counters of the marker set being prepared.  step_offset = 1
+// when the tables of the NEXT step are prepared while the current one is still running.
 __global__ void k_kinematics(const BodyDef *__restrict__ defs, BodyStep *__restrict__ out, int nbodies,
-                             const long long *__restrict__ step_ctr, int *__restrict__ counters, int n_counters)
+                             const long long *__restrict__ step_ctr, int step_offset, int *__restrict__ counters,
+                             int n_counters)
 {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b < n_counters) counters[b] = 0;
     if (b >= nbodies) return;
     const BodyDef d = defs[b];
-    const double n = (double)(*step_ctr);
+    const double n = (double)(*step_ctr + step_offset);
     double R1[9], R0[9];
     for (int which = 0; which < 2; ++which) {
         const double th = d.omega * (n + (which == 0 ? 1.0 : 0.0));
@@ -243,7 +245,7 @@ k_clear_prev(const unsigned *__restrict__ skey_prev, const int *__restrict__ n_p
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     const int stride = gridDim.x * blockDim.x;
     const int np = *n_prev, nw = *n_words, nr = *n_runs;
-    for (int i = tid; i < np; i += stride) bin_first[skey_prev[i]] = -1;
+    if (bin_first) for (int i = tid; i < np; i += stride) bin_first[skey_prev[i]] = -1;
     for (int i = tid; i < nw; i += stride) amask[words[i]] = 0u;
     for (int r = tid; r < nr; r += stride) {
         const int s0 = run_slot0[r], ne = run_nent[r];

@@ -46,16 +46,20 @@ int fail(int code, const char *fmt, ...)
 
 constexpr int MAX_MDF = 64;
 
+// device scalars shared by both marker sets
 struct DevScalars {
     long long step_ctr;  // time step n of the step being computed (kinematics angle)
-    int n_prev;          // sorted markers whose bins are still registered in bin_first
     int status;          // != 0: a stencil crossed a wall
     int scratch;
-    // ---- zeroed at the start of every IBM step (k_kinematics), after k_clear_prev has used them
-    int n_words;         // active words of the current / last IBM step
-    int n_runs;          // runs of the current / last IBM step
-    int t_count;         // T entries handed out in the current / last IBM step
-    int n_cells;         // active cells of the current / last IBM step
+};
+// device scalars of one marker set (see PrepSet)
+struct SetScalars {
+    int n_prev;          // sorted markers whose bins are still registered in bin_first
+    // ---- zeroed at the start of every preparation (k_kinematics), after k_clear_prev has used them
+    int n_words;         // active words
+    int n_runs;          // runs
+    int t_count;         // T entries handed out
+    int n_cells;         // active cells
     int cursor[MAX_MDF]; // work cursors of the run sweeps, one per MDF iteration
 };
 constexpr int N_STEP_COUNTERS = 4 + MAX_MDF;
@@ -70,12 +74,12 @@ constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driv
 
 // Optional per-phase device timing (LBM_OPT_TIMING): CUDA events recorded on the launching stream
 // between the phases of a step; durations are accumulated after a stream synchronise.
-enum { PH_KEYS = 0, PH_SORT, PH_BINS, PH_MOMENTS, PH_INTERP, PH_SPREAD, PH_LBM, PH_COUNT };
+enum { PH_KEYS = 0, PH_SORT, PH_BINS, PH_MOMENTS, PH_INTERP, PH_SPREAD, PH_LBM, PH_LBM_ACTIVE, PH_COUNT };
 struct PhaseTimer {
     std::vector<cudaEvent_t> ev;
     std::vector<int> tag;
     size_t used = 0;
-    double ns[PH_COUNT] = {0, 0, 0, 0, 0, 0, 0};
+    double ns[PH_COUNT] = {0, 0, 0, 0, 0, 0, 0, 0};
     void mark(int phase, cudaStream_t s)
     {
         if (used == ev.size()) { cudaEvent_t e; cudaEventCreate(&e); ev.push_back(e); tag.push_back(0); }
@@ -96,23 +100,48 @@ struct PhaseTimer {
 
 }  // namespace
 
+// Everything the binning stage (a1-a3) produces for ONE time step.  There are two sets: while the
+// MDF loop and the stream-collide of step n use set n & 1, the side stream prepares step n + 1 in
+// the other set (the marker positions depend on time only, not on the fluid).
+struct PrepSet {
+    unsigned *keys[2] = {nullptr, nullptr};   // radix ping-pong; the sorted keys end in keys[sort_passes & 1]
+    int *vals[2] = {nullptr, nullptr};        // the permutation, same ping-pong
+    MarkerSorted ms{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    RunTable rt{nullptr, nullptr, nullptr, nullptr, nullptr};
+    unsigned *headbits = nullptr;             // one bit per sorted marker: starts a run
+    int *cells = nullptr;                     // active-cell list
+    // dense maps, cleared incrementally by the set's next preparation (k_clear_prev)
+    unsigned *amask = nullptr;                // active-cell bitmask, 32 consecutive x per word
+    int *words = nullptr;                     // list of non-zero mask words
+    int *tslot = nullptr;                     // [row][X+1] -> T entry (pitch nx+3)
+    int *bin_first = nullptr;                 // cell -> first sorted marker (comparison spreads only; lazy)
+    SetScalars *scal = nullptr;
+    bool dirty = false;                       // the dense maps hold entries of a preparation
+    long long step = -1;                      // time step the set is prepared for (-1: none)
+    int spread = -1;                          // LBM_OPT_SPREAD the preparation was made for
+};
+
 struct lbm {
     int device = 0;
     cudaStream_t stream = nullptr;      // where work is enqueued
-    cudaStream_t cap_stream = nullptr;  // capture-only stream for building graphs
+    cudaStream_t cap_stream = nullptr;  // capture-only streams for building graphs: the MDF chain (high priority),
+    cudaStream_t cap_bulk = nullptr;    //   the bulk stream-collide (low priority),
+    cudaStream_t cap_prep = nullptr;    //   the preparation of the next step
+    cudaEvent_t ev_fork = nullptr, ev_bulk = nullptr, ev_prep = nullptr;
     Geom g{};
     CollisionConst cc{};
+    PlaneOffsets po{};
     double tau = 1.0;
     float *f[2] = {nullptr, nullptr};
     int cur = 0;                        // f[cur] holds the post-collision state to pull from
     float4 *U = nullptr, *G = nullptr;
-    unsigned *amask = nullptr;
-    int *words = nullptr, *bin_first = nullptr;
     DevScalars *scal = nullptr;
     long long steps_done = 0;
     size_t n_mask_words = 0;
-    bool ibm_dirty = false;             // mask / bin_first hold entries of an earlier IBM step
-    bool force_valid = false;           // G + mask describe the last completed step
+    PrepSet set[2];
+    int cur_set = 0;                    // set the next IBM step uses
+    int last_set = -1;                  // set of the last completed IBM step (G, mask, marker read-out), -1: none
+    bool force_valid = false;           // G + mask of last_set describe the last completed step
 
     // markers: host mirror (caller order) and device copies
     std::vector<float> h_pos, h_vel, h_area;   // [n][3], [n][3], [n]
@@ -125,21 +154,16 @@ struct lbm {
     int *d_body = nullptr;
     BodyDef *d_defs = nullptr;
     BodyStep *d_tabs = nullptr;
-    unsigned *d_keys[2] = {nullptr, nullptr};
-    int *d_vals[2] = {nullptr, nullptr};
     int *d_hist = nullptr, *d_total = nullptr;
-    MarkerSorted ms{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    RunTable rt{nullptr, nullptr, nullptr, nullptr, nullptr};
-    int *tslot = nullptr;               // dense [row][X+1] -> T entry map (pitch nx+3)
-    int *cells = nullptr;               // active-cell list
-    unsigned *headbits = nullptr;       // one bit per sorted marker: starts a run
     size_t cells_cap = 0, headbits_cap = 0;
     float4 *T = nullptr;                // run profiles, 16 float4 per entry
     size_t t_cap = 0, tslot_count = 0;
     int rows_grid = 148;                // persistent grid of the run sweep (blocks resident at once)
+    int words_grid = 148, moments_grid = 148;   // same for the active-word stream-collide and the moments kernel
     int sort_ipw = 64, sort_tiles = 0, sort_passes = 1;
 
     int opt_spread = 0, opt_forcing = 0, opt_graph = 1, opt_lbm_kernel = 0, opt_interp = 0, opt_timing = 0;
+    int opt_overlap = 1;
     PhaseTimer timer;
     std::map<long long, std::pair<cudaGraphExec_t, int>> graphs;   // key -> (exec, kernel nodes)
     long long launches = 0;
@@ -177,19 +201,28 @@ void drop_graphs(lbm *h)
     h->graphs.clear();
 }
 
+void free_set(lbm *h, PrepSet &S)
+{
+    const size_t c = (size_t)h->nm_cap;
+    for (int a = 0; a < 2; ++a) { dfree(h, S.keys[a], c); dfree(h, S.vals[a], c); }
+    dfree(h, S.ms.fs, c); dfree(h, S.ms.wx, c); dfree(h, S.ms.wyz, 16 * c); dfree(h, S.ms.uk, c);
+    dfree(h, S.ms.sg, c); dfree(h, S.ms.du, c);
+    dfree(h, S.rt.first, c); dfree(h, S.rt.end, c); dfree(h, S.rt.base, c); dfree(h, S.rt.slot0, c);
+    dfree(h, S.rt.nent, c);
+    dfree(h, S.cells, h->cells_cap);
+    dfree(h, S.headbits, h->headbits_cap);
+    S.step = -1;
+}
+
 void free_markers_dev(lbm *h)
 {
     const size_t c = (size_t)h->nm_cap;
     for (int a = 0; a < 3; ++a) { dfree(h, h->d_q[a], c); dfree(h, h->d_v[a], c); }
     dfree(h, h->d_s, c);
     dfree(h, h->d_body, c);
-    for (int a = 0; a < 2; ++a) { dfree(h, h->d_keys[a], c); dfree(h, h->d_vals[a], c); }
-    dfree(h, h->ms.fs, c); dfree(h, h->ms.wx, c); dfree(h, h->ms.wyz, 16 * c); dfree(h, h->ms.uk, c); dfree(h, h->ms.sg, c); dfree(h, h->ms.du, c);
-    dfree(h, h->rt.first, c); dfree(h, h->rt.end, c); dfree(h, h->rt.base, c); dfree(h, h->rt.slot0, c);
-    dfree(h, h->rt.nent, c);
+    for (PrepSet &S : h->set) free_set(h, S);
+    h->cells_cap = 0; h->headbits_cap = 0;
     dfree(h, h->T, h->t_cap * 16); h->t_cap = 0;
-    dfree(h, h->cells, h->cells_cap); h->cells_cap = 0;
-    dfree(h, h->headbits, h->headbits_cap); h->headbits_cap = 0;
     dfree(h, h->d_hist, (size_t)RADIX * (size_t)h->sort_tiles);
     dfree(h, h->d_total, (size_t)RADIX);
     dfree(h, h->d_defs, (size_t)h->nb_cap);
@@ -205,22 +238,41 @@ dim3 cell_block(const Geom &g)
 }
 dim3 cell_grid(const Geom &g, dim3 b) { return dim3((g.nx + b.x - 1) / b.x, (g.ny + b.y - 1) / b.y, g.nz); }
 
-// ---- remove what the last IBM step registered in the dense maps (outside any graph) -----------
+const unsigned *sorted_keys(const lbm *h, const PrepSet &S) { return S.keys[h->sort_passes & 1]; }
+const int *sorted_perm(const lbm *h, const PrepSet &S) { return S.vals[h->sort_passes & 1]; }
+
+// the dense cell -> first-marker map is needed by the comparison spreads only
+int ensure_bin_first(lbm *h, PrepSet &S)
+{
+    if (S.bin_first) return LBM_OK;
+    int rc = dmalloc(h, &S.bin_first, (size_t)h->g.cells);
+    if (rc) return rc;
+    CK(cudaMemsetAsync(S.bin_first, 0xff, (size_t)h->g.cells * sizeof(int), h->stream));
+    return LBM_OK;
+}
+
+// ---- remove what the preparations registered in the dense maps (outside any graph) -------------
+int flush_set(lbm *h, PrepSet &S)
+{
+    S.step = -1;
+    if (!S.dirty) return LBM_OK;
+    k_clear_prev<<<LIST_GRID, 256, 0, h->stream>>>(sorted_keys(h, S), &S.scal->n_prev, S.bin_first, S.amask, S.words,
+                                                    &S.scal->n_words, S.tslot, S.rt.slot0, S.rt.nent, &S.scal->n_runs);
+    CK(cudaMemsetAsync(S.scal, 0, sizeof(SetScalars), h->stream));
+    CK(cudaGetLastError());
+    h->launches += 1;
+    S.dirty = false;
+    return LBM_OK;
+}
+
 int flush_ibm(lbm *h)
 {
-    if (!h->ibm_dirty) return LBM_OK;
-    const unsigned *skey = h->d_keys[h->sort_passes & 1];
-    k_clear_prev<<<LIST_GRID, 256, 0, h->stream>>>(skey, &h->scal->n_prev, h->bin_first, h->amask, h->words,
-                                                    &h->scal->n_words, h->tslot, h->rt.slot0, h->rt.nent,
-                                                    &h->scal->n_runs);
-    k_set_scalars<<<1, 1, 0, h->stream>>>(&h->scal->step_ctr, h->steps_done, &h->scal->n_prev, 0, 1 | 2);
-    CK(cudaMemsetAsync(&h->scal->n_words, 0, sizeof(int), h->stream));
-    CK(cudaMemsetAsync(&h->scal->n_runs, 0, sizeof(int), h->stream));
-    CK(cudaMemsetAsync(&h->scal->n_cells, 0, sizeof(int), h->stream));
-    CK(cudaGetLastError());
-    h->launches += 2;
-    h->ibm_dirty = false;
+    for (PrepSet &S : h->set) {
+        int rc = flush_set(h, S);
+        if (rc) return rc;
+    }
     h->force_valid = false;
+    h->last_set = -1;
     return LBM_OK;
 }
 
@@ -243,27 +295,29 @@ int upload_markers(lbm *h)
         }
         if ((rc = dmalloc(h, &h->d_s, c))) return rc;
         if ((rc = dmalloc(h, &h->d_body, c))) return rc;
-        for (int a = 0; a < 2; ++a) {
-            if ((rc = dmalloc(h, &h->d_keys[a], c))) return rc;
-            if ((rc = dmalloc(h, &h->d_vals[a], c))) return rc;
+        h->cells_cap = std::min((size_t)64 * c, (size_t)h->g.cells);
+        h->headbits_cap = c / 32 + 16;
+        for (PrepSet &S : h->set) {
+            for (int a = 0; a < 2; ++a) {
+                if ((rc = dmalloc(h, &S.keys[a], c))) return rc;
+                if ((rc = dmalloc(h, &S.vals[a], c))) return rc;
+            }
+            if ((rc = dmalloc(h, &S.ms.fs, c))) return rc;
+            if ((rc = dmalloc(h, &S.ms.wx, c))) return rc;
+            if ((rc = dmalloc(h, &S.ms.wyz, 16 * c))) return rc;
+            if ((rc = dmalloc(h, &S.ms.uk, c))) return rc;
+            if ((rc = dmalloc(h, &S.ms.sg, c))) return rc;
+            if ((rc = dmalloc(h, &S.ms.du, c))) return rc;
+            if ((rc = dmalloc(h, &S.rt.first, c))) return rc;
+            if ((rc = dmalloc(h, &S.rt.end, c))) return rc;
+            if ((rc = dmalloc(h, &S.rt.base, c))) return rc;
+            if ((rc = dmalloc(h, &S.rt.slot0, c))) return rc;
+            if ((rc = dmalloc(h, &S.rt.nent, c))) return rc;
+            if ((rc = dmalloc(h, &S.cells, h->cells_cap))) return rc;
+            if ((rc = dmalloc(h, &S.headbits, h->headbits_cap))) return rc;
         }
-        if ((rc = dmalloc(h, &h->ms.fs, c))) return rc;
-        if ((rc = dmalloc(h, &h->ms.wx, c))) return rc;
-        if ((rc = dmalloc(h, &h->ms.wyz, 16 * c))) return rc;
-        if ((rc = dmalloc(h, &h->rt.first, c))) return rc;
-        if ((rc = dmalloc(h, &h->rt.end, c))) return rc;
-        if ((rc = dmalloc(h, &h->rt.base, c))) return rc;
-        if ((rc = dmalloc(h, &h->rt.slot0, c))) return rc;
-        if ((rc = dmalloc(h, &h->rt.nent, c))) return rc;
         h->t_cap = std::min((size_t)4 * c, h->tslot_count);
         if ((rc = dmalloc(h, &h->T, h->t_cap * 16))) return rc;
-        h->cells_cap = std::min((size_t)64 * c, (size_t)h->g.cells);
-        if ((rc = dmalloc(h, &h->cells, h->cells_cap))) return rc;
-        h->headbits_cap = c / 32 + 16;
-        if ((rc = dmalloc(h, &h->headbits, h->headbits_cap))) return rc;
-        if ((rc = dmalloc(h, &h->ms.uk, c))) return rc;
-        if ((rc = dmalloc(h, &h->ms.sg, c))) return rc;
-        if ((rc = dmalloc(h, &h->ms.du, c))) return rc;
         if ((rc = dmalloc(h, &h->d_total, (size_t)RADIX))) return rc;
         if ((rc = dmalloc(h, &h->d_defs, (size_t)nb))) return rc;
         if ((rc = dmalloc(h, &h->d_tabs, (size_t)nb))) return rc;
@@ -319,147 +373,252 @@ int upload_markers(lbm *h)
     return LBM_OK;
 }
 
-// ---- enqueue one time step on stream s (plain launches; also what graph capture records) -------
-int enqueue_step(lbm *h, cudaStream_t s, int parity, int mdf_iters, bool ibm, int *n_kernels, PhaseTimer *pt = nullptr)
-{
-    const float *src = h->f[parity];
-    float *dst = h->f[parity ^ 1];
-    const Geom &g = h->g;
-    int nk = 0;
-    if (ibm) {
-        const int n = h->nm;
-        const int mb = (n + 255) / 256;
-        DevScalars *sc = h->scal;
-        unsigned *skey = h->d_keys[h->sort_passes & 1];
-        int *perm = h->d_vals[h->sort_passes & 1];
-        MarkerIn mi{h->d_q[0], h->d_q[1], h->d_q[2], h->d_v[0], h->d_v[1], h->d_v[2], h->d_s, h->d_body, n};
+// ---- launch helpers (plain launches on stream s; also what graph capture records) --------------
 
-        if (pt) pt->mark(PH_KEYS, s);
-        k_clear_prev<<<LIST_GRID, 256, 0, s>>>(skey, &sc->n_prev, h->bin_first, h->amask, h->words, &sc->n_words,
-                                               h->tslot, h->rt.slot0, h->rt.nent, &sc->n_runs);
-        const int nb = (int)h->bodies.size();
-        k_kinematics<<<(std::max(nb, N_STEP_COUNTERS) + 127) / 128, 128, 0, s>>>(h->d_defs, h->d_tabs, nb, &sc->step_ctr,
-                                                                                  &sc->n_words, N_STEP_COUNTERS);
-        k_marker_keys<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, h->d_keys[0], &sc->status);
+// a1-a3 for the time step (device step counter + step_offset) into marker set S.
+int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_kernels, PhaseTimer *pt)
+{
+    const Geom &g = h->g;
+    const int n = h->nm;
+    const int mb = (n + 255) / 256;
+    SetScalars *sc = S.scal;
+    unsigned *skey = S.keys[h->sort_passes & 1];
+    int *perm = S.vals[h->sort_passes & 1];
+    MarkerIn mi{h->d_q[0], h->d_q[1], h->d_q[2], h->d_v[0], h->d_v[1], h->d_v[2], h->d_s, h->d_body, n};
+    int nk = 0;
+
+    if (pt) pt->mark(PH_KEYS, s);
+    k_clear_prev<<<LIST_GRID, 256, 0, s>>>(skey, &sc->n_prev, S.bin_first, S.amask, S.words, &sc->n_words, S.tslot,
+                                           S.rt.slot0, S.rt.nent, &sc->n_runs);
+    const int nb = (int)h->bodies.size();
+    k_kinematics<<<(std::max(nb, N_STEP_COUNTERS) + 127) / 128, 128, 0, s>>>(h->d_defs, h->d_tabs, nb, &h->scal->step_ctr,
+                                                                              step_offset, &sc->n_words, N_STEP_COUNTERS);
+    k_marker_keys<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, S.keys[0], &h->scal->status);
+    nk += 3;
+    if (pt) pt->mark(PH_SORT, s);
+    const int sb = (h->sort_tiles + SORT_WARPS - 1) / SORT_WARPS;
+    for (int p = 0; p < h->sort_passes; ++p) {
+        const unsigned *kin = S.keys[p & 1];
+        unsigned *kout = S.keys[(p + 1) & 1];
+        const int *vin = p == 0 ? nullptr : S.vals[p & 1];
+        int *vout = S.vals[(p + 1) & 1];
+        k_radix_hist<<<sb, SORT_BLOCK, 0, s>>>(kin, n, h->sort_ipw, h->sort_tiles, 8 * p, h->d_hist);
+        k_radix_scan<<<RADIX, SORT_BLOCK, 0, s>>>(h->d_hist, h->sort_tiles, h->d_total);
+        k_radix_scatter<<<sb, SORT_BLOCK, 0, s>>>(kin, vin, kout, vout, n, h->sort_ipw, h->sort_tiles, 8 * p, h->d_hist,
+                                                   h->d_total);
         nk += 3;
-        if (pt) pt->mark(PH_SORT, s);
-        const int sb = (h->sort_tiles + SORT_WARPS - 1) / SORT_WARPS;
-        for (int p = 0; p < h->sort_passes; ++p) {
-            const unsigned *kin = h->d_keys[p & 1];
-            unsigned *kout = h->d_keys[(p + 1) & 1];
-            const int *vin = p == 0 ? nullptr : h->d_vals[p & 1];
-            int *vout = h->d_vals[(p + 1) & 1];
-            k_radix_hist<<<sb, SORT_BLOCK, 0, s>>>(kin, n, h->sort_ipw, h->sort_tiles, 8 * p, h->d_hist);
-            k_radix_scan<<<RADIX, SORT_BLOCK, 0, s>>>(h->d_hist, h->sort_tiles, h->d_total);
-            k_radix_scatter<<<sb, SORT_BLOCK, 0, s>>>(kin, vin, kout, vout, n, h->sort_ipw, h->sort_tiles, 8 * p,
-                                                       h->d_hist, h->d_total);
-            nk += 3;
-        }
-        if (pt) pt->mark(PH_BINS, s);
-        k_marker_gather<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, perm, h->ms);
-        if (h->opt_spread == 0) {
-            k_run_heads<<<(n + 32 + 255) / 256, 256, 0, s>>>(skey, n, g, h->headbits);
-            k_runs<<<mb, 256, 0, s>>>(skey, n, g, h->headbits, h->rt, &sc->n_runs, &sc->t_count);
-            k_run_publish<<<LIST_GRID, 256, 0, s>>>(g, h->rt, &sc->n_runs, h->tslot, h->amask, h->words, &sc->n_words);
-            nk += 2;
-        } else {
-            k_bins<<<mb, 256, 0, s>>>(skey, n, g, h->bin_first, h->amask, h->words, &sc->n_words);
-        }
-        k_active_cells<<<LIST_GRID, 256, 0, s>>>(g, h->amask, h->words, &sc->n_words, h->cells, &sc->n_cells);
+    }
+    if (pt) pt->mark(PH_BINS, s);
+    k_marker_gather<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, perm, S.ms);
+    ++nk;
+    if (h->opt_spread == 0) {
+        k_run_heads<<<(n + 32 + 255) / 256, 256, 0, s>>>(skey, n, g, S.headbits);
+        k_runs<<<mb, 256, 0, s>>>(skey, n, g, S.headbits, S.rt, &sc->n_runs, &sc->t_count);
+        k_run_publish<<<LIST_GRID, 256, 0, s>>>(g, S.rt, &sc->n_runs, S.tslot, S.amask, S.words, &sc->n_words);
+        nk += 3;
+    } else {
+        k_bins<<<mb, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask, S.words, &sc->n_words);
         ++nk;
-        k_set_scalars<<<1, 1, 0, s>>>(&sc->step_ctr, 0, &sc->n_prev, n, 2 | 4);
-        if (pt) pt->mark(PH_MOMENTS, s);
-        k_moments_active<<<LIST_GRID, 256, 0, s>>>(src, g, h->cells, &sc->n_cells, h->U);
-        nk += 4;
-        for (int m = 0; m < mdf_iters; ++m) {
-            const bool last = (m == mdf_iters - 1);
-            if (pt) pt->mark(PH_INTERP, s);
-            k_interp_correct<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, h->U, h->ms);
+    }
+    k_active_cells<<<LIST_GRID, 256, 0, s>>>(g, S.amask, S.words, &sc->n_words, S.cells, &sc->n_cells);
+    k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, &sc->n_prev, n, 2);
+    nk += 2;
+    CK(cudaGetLastError());
+    *n_kernels += nk;
+    return LBM_OK;
+}
+
+// a4-a7: moments on the active cells of set S, then the MDF loop; leaves G on the active cells.
+int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_iters, int *n_kernels, PhaseTimer *pt)
+{
+    const Geom &g = h->g;
+    const int n = h->nm;
+    SetScalars *sc = S.scal;
+    const unsigned *skey = sorted_keys(h, S);
+    int nk = 0;
+    if (pt) pt->mark(PH_MOMENTS, s);
+    k_moments_active<<<h->moments_grid, 256, 0, s>>>(src, g, h->po, S.cells, &sc->n_cells, h->U);
+    ++nk;
+    for (int m = 0; m < mdf_iters; ++m) {
+        const bool last = (m == mdf_iters - 1);
+        if (pt) pt->mark(PH_INTERP, s);
+        k_interp_correct<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, h->U, S.ms);
+        ++nk;
+        if (pt) pt->mark(PH_SPREAD, s);
+        if (h->opt_spread == 0) {
+            k_spread_rows<<<h->rows_grid, 256, 0, s>>>(S.rt, &sc->n_runs, &sc->cursor[m], S.ms.wx, S.ms.wyz,
+                                                       last ? S.ms.du : S.ms.sg, h->T);
+            if (last) k_spread_collect<true><<<LIST_GRID, 256, 0, s>>>(g, S.tslot, h->T, S.cells, &sc->n_cells, h->G);
+            else k_spread_collect<false><<<LIST_GRID, 256, 0, s>>>(g, S.tslot, h->T, S.cells, &sc->n_cells, h->U);
+            nk += 2;
+        } else if (h->opt_spread == 2) {
+            if (last)
+                k_spread_gather<true><<<LIST_GRID, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask, S.words, &sc->n_words,
+                                                                 S.ms.fs, S.ms.du, h->G);
+            else
+                k_spread_gather<false><<<LIST_GRID, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask, S.words, &sc->n_words,
+                                                                  S.ms.fs, S.ms.sg, h->U);
             ++nk;
-            if (pt) pt->mark(PH_SPREAD, s);
-            if (h->opt_spread == 0) {
-                k_spread_rows<<<h->rows_grid, 256, 0, s>>>(h->rt, &sc->n_runs, &sc->cursor[m], h->ms.wx, h->ms.wyz,
-                                                           last ? h->ms.du : h->ms.sg, h->T);
-                if (last)
-                    k_spread_collect<true><<<LIST_GRID, 256, 0, s>>>(g, h->tslot, h->T, h->cells, &sc->n_cells, h->G);
-                else
-                    k_spread_collect<false><<<LIST_GRID, 256, 0, s>>>(g, h->tslot, h->T, h->cells, &sc->n_cells, h->U);
+        } else {
+            if (last) {
+                k_zero_active<<<LIST_GRID, 256, 0, s>>>(g, S.amask, S.words, &sc->n_words, h->G);
+                k_spread_atomic<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, S.ms.fs, S.ms.du, h->G);
                 nk += 2;
-            } else if (h->opt_spread == 2) {
-                if (last)
-                    k_spread_gather<true><<<LIST_GRID, 256, 0, s>>>(skey, n, g, h->bin_first, h->amask, h->words,
-                                                                     &sc->n_words, h->ms.fs, h->ms.du, h->G);
-                else
-                    k_spread_gather<false><<<LIST_GRID, 256, 0, s>>>(skey, n, g, h->bin_first, h->amask, h->words,
-                                                                      &sc->n_words, h->ms.fs, h->ms.sg, h->U);
-                ++nk;
             } else {
-                if (last) {
-                    k_zero_active<<<LIST_GRID, 256, 0, s>>>(g, h->amask, h->words, &sc->n_words, h->G);
-                    k_spread_atomic<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, h->ms.fs, h->ms.du, h->G);
-                    nk += 2;
-                } else {
-                    k_spread_atomic<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, h->ms.fs, h->ms.sg, h->U);
-                    ++nk;
-                }
+                k_spread_atomic<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, S.ms.fs, S.ms.sg, h->U);
+                ++nk;
             }
         }
     }
-    if (pt) pt->mark(PH_LBM, s);
+    CK(cudaGetLastError());
+    *n_kernels += nk;
+    return LBM_OK;
+}
+
+CollisionConst collision_const(const lbm *h)
+{
     CollisionConst cc = h->cc;
     cc.shift_forcing = h->opt_forcing;
-    const bool vec = (h->opt_lbm_kernel == 2) && (g.nx % 4 == 0);
+    return cc;
+}
+
+// a8 in one pass over the whole lattice: mode LBM_PURE, LBM_FUSED (mask + G) or LBM_BULK (skip active cells)
+int enqueue_lbm_pass(lbm *h, cudaStream_t s, const float *src, float *dst, int mode, const unsigned *amask)
+{
+    const Geom &g = h->g;
+    const CollisionConst cc = collision_const(h);
+    const bool vec = (h->opt_lbm_kernel == 2) && (g.nx % 4 == 0) && (mode == LBM_PURE || mode == LBM_FUSED);
     if (vec) {
         const int nx4 = g.nx / 4;
         int bx = 1;
         while (bx < nx4 && bx < 64) bx <<= 1;
         dim3 b(bx, 256 / bx, 1);
         dim3 gr((nx4 + b.x - 1) / b.x, (g.ny + b.y - 1) / b.y, g.nz);
-        if (ibm) k_stream_collide_vec4<true><<<gr, b, 0, s>>>(src, dst, g, cc, h->amask, h->G);
+        if (mode == LBM_FUSED) k_stream_collide_vec4<true><<<gr, b, 0, s>>>(src, dst, g, cc, amask, h->G);
         else k_stream_collide_vec4<false><<<gr, b, 0, s>>>(src, dst, g, cc, nullptr, nullptr);
     } else {
-        // variants of the one-cell-per-thread kernel: (threads per block, min blocks per SM)
-        auto launch = [&](auto kern_ibm, auto kern_pure, int threads) {
-            int bx = g.nx >= threads ? threads : ((g.nx + 31) / 32) * 32;
-            int by = threads / bx; if (by < 1) by = 1;
-            dim3 b(bx, by, 1);
-            dim3 gr = cell_grid(g, b);
-            if (ibm) kern_ibm<<<gr, b, 0, s>>>(src, dst, g, cc, h->amask, h->G);
-            else kern_pure<<<gr, b, 0, s>>>(src, dst, g, cc, nullptr, nullptr);
-        };
-        switch (h->opt_lbm_kernel) {
-            case 3: launch(k_stream_collide_scalar<true, 256, 4>, k_stream_collide_scalar<false, 256, 4>, 256); break;
-            case 4: launch(k_stream_collide_scalar<true, 256, 6>, k_stream_collide_scalar<false, 256, 6>, 256); break;
-            case 5: launch(k_stream_collide_scalar<true, 128, 8>, k_stream_collide_scalar<false, 128, 8>, 128); break;
-            case 6: launch(k_stream_collide_scalar<true, 128, 10>, k_stream_collide_scalar<false, 128, 10>, 128); break;
-            case 7: launch(k_stream_collide_scalar<true, 512, 2>, k_stream_collide_scalar<false, 512, 2>, 512); break;
-            case 8: launch(k_stream_collide_scalar<true, 128, 12>, k_stream_collide_scalar<false, 128, 12>, 128); break;
-            default: launch(k_stream_collide_scalar<true, 256, 5>, k_stream_collide_scalar<false, 256, 5>, 256); break;
-        }
+        const dim3 b = cell_block(g);
+        const dim3 gr = cell_grid(g, b);
+        if (mode == LBM_FUSED) k_stream_collide_scalar<LBM_FUSED, 256, 5><<<gr, b, 0, s>>>(src, dst, g, cc, h->po, amask, h->G);
+        else if (mode == LBM_BULK) k_stream_collide_scalar<LBM_BULK, 256, 5><<<gr, b, 0, s>>>(src, dst, g, cc, h->po, amask, nullptr);
+        else k_stream_collide_scalar<LBM_PURE, 256, 5><<<gr, b, 0, s>>>(src, dst, g, cc, h->po, nullptr, nullptr);
     }
-    ++nk;
+    CK(cudaGetLastError());
+    return LBM_OK;
+}
+
+int enqueue_lbm_active(lbm *h, cudaStream_t s, const float *src, float *dst, PrepSet &S)
+{
+    k_stream_collide_words<<<h->words_grid, 256, 0, s>>>(src, dst, h->g, collision_const(h), h->po, S.amask, S.words,
+                                                      &S.scal->n_words, h->G);
+    CK(cudaGetLastError());
+    return LBM_OK;
+}
+
+// ---- one time step, serial on stream s ----------------------------------------------------------
+// prep: 0 = set S is already prepared for this step; 1 = prepare it first.
+int enqueue_step_serial(lbm *h, cudaStream_t s, int parity, PrepSet *S, bool prep, int mdf_iters, int *n_kernels,
+                        PhaseTimer *pt = nullptr)
+{
+    const float *src = h->f[parity];
+    float *dst = h->f[parity ^ 1];
+    int nk = 0, rc;
+    if (S) {
+        if (prep && (rc = enqueue_prep(h, s, *S, 0, &nk, pt))) return rc;
+        if ((rc = enqueue_mdf(h, s, *S, src, mdf_iters, &nk, pt))) return rc;
+        if (h->opt_overlap) {
+            if (pt) pt->mark(PH_LBM, s);
+            if ((rc = enqueue_lbm_pass(h, s, src, dst, LBM_BULK, S->amask))) return rc;
+            if (pt) pt->mark(PH_LBM_ACTIVE, s);
+            if ((rc = enqueue_lbm_active(h, s, src, dst, *S))) return rc;
+            nk += 2;
+        } else {
+            if (pt) pt->mark(PH_LBM, s);
+            if ((rc = enqueue_lbm_pass(h, s, src, dst, LBM_FUSED, S->amask))) return rc;
+            ++nk;
+        }
+        k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, nullptr, 0, 4);
+        ++nk;
+    } else {
+        if (pt) pt->mark(PH_LBM, s);
+        if ((rc = enqueue_lbm_pass(h, s, src, dst, LBM_PURE, nullptr))) return rc;
+        ++nk;
+    }
     if (pt) pt->mark(-1, s);
     CK(cudaGetLastError());
     *n_kernels = nk;
     return LBM_OK;
 }
 
-int get_graph(lbm *h, int parity, int mdf_iters, bool ibm, cudaGraphExec_t *exec, int *n_kernels)
+// ---- one time step as three concurrent branches (captured into a graph) --------------------------
+//   main (high priority): moments + MDF loop on set S          -> G
+//   bulk (low priority) : stream-collide of every cell outside S's active mask (needs no G)
+//   prep                : a1-a3 of the NEXT step into the other set (depends on time only)
+//   join, then the stream-collide of the active cells with G, then step counter + 1.
+int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, int mdf_iters, int *n_kernels)
 {
-    const long long key = ((long long)mdf_iters << 8) | (ibm ? 2 : 0) | parity | ((long long)h->opt_spread << 40) |
-                          ((long long)h->opt_forcing << 44) | ((long long)h->opt_lbm_kernel << 48) |
-                          ((long long)h->opt_interp << 52);
+    const float *src = h->f[parity];
+    float *dst = h->f[parity ^ 1];
+    cudaStream_t s = h->cap_stream;
+    int nk = 0, rc;
+    CK(cudaEventRecord(h->ev_fork, s));
+    CK(cudaStreamWaitEvent(h->cap_bulk, h->ev_fork, 0));
+    CK(cudaStreamWaitEvent(h->cap_prep, h->ev_fork, 0));
+    if ((rc = enqueue_lbm_pass(h, h->cap_bulk, src, dst, LBM_BULK, S.amask))) return rc;
+    ++nk;
+    if ((rc = enqueue_mdf(h, s, S, src, mdf_iters, &nk, nullptr))) return rc;
+    if ((rc = enqueue_prep(h, h->cap_prep, N, 1, &nk, nullptr))) return rc;
+    CK(cudaEventRecord(h->ev_bulk, h->cap_bulk));
+    CK(cudaEventRecord(h->ev_prep, h->cap_prep));
+    CK(cudaStreamWaitEvent(s, h->ev_bulk, 0));
+    CK(cudaStreamWaitEvent(s, h->ev_prep, 0));
+    if ((rc = enqueue_lbm_active(h, s, src, dst, S))) return rc;
+    k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, nullptr, 0, 4);
+    nk += 2;
+    CK(cudaGetLastError());
+    *n_kernels = nk;
+    return LBM_OK;
+}
+
+// kind: 0 = pure LBM, 1 = serial IBM step that prepares its own set, 2 = overlapped IBM step
+int get_graph(lbm *h, int kind, int parity, int set, int mdf_iters, cudaGraphExec_t *exec, int *n_kernels)
+{
+    const long long key = ((long long)mdf_iters << 8) | ((long long)kind << 4) | (set << 1) | parity |
+                          ((long long)h->opt_spread << 40) | ((long long)h->opt_forcing << 44) |
+                          ((long long)h->opt_lbm_kernel << 48) | ((long long)h->opt_interp << 52) |
+                          ((long long)h->opt_overlap << 56);
     auto it = h->graphs.find(key);
     if (it != h->graphs.end()) { *exec = it->second.first; *n_kernels = it->second.second; return LBM_OK; }
     cudaGraph_t graph = nullptr;
     CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
-    int nk = 0;
-    int rc = enqueue_step(h, h->cap_stream, parity, mdf_iters, ibm, &nk);
+    int nk = 0, rc;
+    if (kind == 2) rc = enqueue_step_overlapped(h, parity, h->set[set], h->set[set ^ 1], mdf_iters, &nk);
+    else rc = enqueue_step_serial(h, h->cap_stream, parity, kind ? &h->set[set] : nullptr, true, mdf_iters, &nk);
     cudaError_t e = cudaStreamEndCapture(h->cap_stream, &graph);
     if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
     if (e != cudaSuccess) return fail(LBM_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
+    if (kind == 2) {
+        // node priorities: the lattice-wide bulk pass yields to every other kernel of the step, so that the short
+        // IBM kernels are placed on the SMs as soon as bulk blocks retire instead of queueing behind the whole grid
+        int lo = 0, hi = 0;
+        cudaDeviceGetStreamPriorityRange(&lo, &hi);
+        size_t nn = 0;
+        CK(cudaGraphGetNodes(graph, nullptr, &nn));
+        std::vector<cudaGraphNode_t> nodes(nn);
+        CK(cudaGraphGetNodes(graph, nodes.data(), &nn));
+        const void *bulk_fn = (const void *)k_stream_collide_scalar<LBM_BULK, 256, 5>;
+        for (cudaGraphNode_t nd : nodes) {
+            cudaGraphNodeType ty;
+            if (cudaGraphNodeGetType(nd, &ty) != cudaSuccess || ty != cudaGraphNodeTypeKernel) continue;
+            cudaKernelNodeParams kp{};
+            if (cudaGraphKernelNodeGetParams(nd, &kp) != cudaSuccess) continue;
+            cudaLaunchAttributeValue v{};
+            v.priority = (kp.func == bulk_fn) ? lo : hi;
+            CK(cudaGraphKernelNodeSetAttribute(nd, cudaLaunchAttributePriority, &v));
+        }
+    }
     cudaGraphExec_t ex = nullptr;
-    e = cudaGraphInstantiate(&ex, graph, 0);
+    e = cudaGraphInstantiate(&ex, graph, kind == 2 ? cudaGraphInstantiateFlagUseNodePriority : 0);
     cudaGraphDestroy(graph);
     if (e != cudaSuccess) return fail(LBM_ECUDA, "graph instantiate failed: %s", cudaGetErrorString(e));
     h->graphs[key] = std::make_pair(ex, nk);
@@ -540,29 +699,48 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
     h->cc.shift_forcing = 0;
     const size_t cells = (size_t)h->g.cells;
     h->n_mask_words = (size_t)h->g.nxw * ny * nz;
-    if (cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) return bail("stream");
+    {
+        // capture streams: the MDF chain gets the highest priority, the bulk stream-collide the lowest, so the
+        // short latency-bound IBM kernels are scheduled ahead of the lattice-wide pass they run beside
+        int lo = 0, hi = 0;
+        cudaDeviceGetStreamPriorityRange(&lo, &hi);
+        bool ok = cudaStreamCreateWithPriority(&h->cap_stream, cudaStreamNonBlocking, hi) == cudaSuccess;
+        ok &= cudaStreamCreateWithPriority(&h->cap_prep, cudaStreamNonBlocking, hi) == cudaSuccess;
+        ok &= cudaStreamCreateWithPriority(&h->cap_bulk, cudaStreamNonBlocking, lo) == cudaSuccess;
+        ok &= cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) == cudaSuccess;
+        ok &= cudaEventCreateWithFlags(&h->ev_bulk, cudaEventDisableTiming) == cudaSuccess;
+        ok &= cudaEventCreateWithFlags(&h->ev_prep, cudaEventDisableTiming) == cudaSuccess;
+        if (!ok) { fail(LBM_ECUDA, "%s", cudaGetErrorString(cudaGetLastError())); return bail("streams"); }
+    }
+    h->po = plane_offsets(h->g);
     const size_t fcount = (size_t)h->g.pitch * NQ;
     if (dmalloc(h, &h->f[0], fcount) || dmalloc(h, &h->f[1], fcount)) return bail("populations");
     if (dmalloc(h, &h->U, cells) || dmalloc(h, &h->G, cells)) return bail("U/G fields");
-    if (dmalloc(h, &h->amask, h->n_mask_words) || dmalloc(h, &h->words, h->n_mask_words)) return bail("active mask");
-    if (dmalloc(h, &h->bin_first, cells)) return bail("bin map");
-    h->tslot_count = (size_t)(nx + 3) * ny * nz;
-    if (dmalloc(h, &h->tslot, h->tslot_count)) return bail("run slot map");
     if (dmalloc(h, &h->scal, (size_t)1)) return bail("scalars");
+    h->tslot_count = (size_t)(nx + 3) * ny * nz;
     bool ok = true;
+    for (PrepSet &S : h->set) {
+        if (dmalloc(h, &S.amask, h->n_mask_words) || dmalloc(h, &S.words, h->n_mask_words)) return bail("active mask");
+        if (dmalloc(h, &S.tslot, h->tslot_count)) return bail("run slot map");
+        if (dmalloc(h, &S.scal, (size_t)1)) return bail("set scalars");
+        ok &= cudaMemset(S.amask, 0, h->n_mask_words * sizeof(unsigned)) == cudaSuccess;
+        ok &= cudaMemset(S.tslot, 0xff, h->tslot_count * sizeof(int)) == cudaSuccess;
+        ok &= cudaMemset(S.scal, 0, sizeof(SetScalars)) == cudaSuccess;
+    }
     ok &= cudaMemset(h->f[0], 0, fcount * sizeof(float)) == cudaSuccess;   // rest state: f_i - t_i = 0
     ok &= cudaMemset(h->f[1], 0, fcount * sizeof(float)) == cudaSuccess;
-    ok &= cudaMemset(h->amask, 0, h->n_mask_words * sizeof(unsigned)) == cudaSuccess;
-    ok &= cudaMemset(h->bin_first, 0xff, cells * sizeof(int)) == cudaSuccess;
-    ok &= cudaMemset(h->tslot, 0xff, h->tslot_count * sizeof(int)) == cudaSuccess;
     ok &= cudaMemset(h->scal, 0, sizeof(DevScalars)) == cudaSuccess;
     ok &= cudaDeviceSynchronize() == cudaSuccess;
     if (!ok) { fail(LBM_ECUDA, "%s", cudaGetErrorString(cudaGetLastError())); return bail("memset"); }
     {
         int per_sm = 0, sms = 148;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spread_rows, 256, 0);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spread_rows, 256, 0);
         h->rows_grid = std::max(1, per_sm) * sms;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_stream_collide_words, 256, 0);
+        h->words_grid = std::max(1, per_sm) * sms;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moments_active, 256, 0);
+        h->moments_grid = std::max(1, per_sm) * sms;
     }
     g_err.clear();
     return h;
@@ -574,9 +752,16 @@ void lbm_destroy(lbm_t *h)
     cudaDeviceSynchronize();
     drop_graphs(h);
     free_markers_dev(h);
-    cudaFree(h->f[0]); cudaFree(h->f[1]); cudaFree(h->U); cudaFree(h->G);
-    cudaFree(h->amask); cudaFree(h->words); cudaFree(h->bin_first); cudaFree(h->scal); cudaFree(h->tslot);
+    cudaFree(h->f[0]); cudaFree(h->f[1]); cudaFree(h->U); cudaFree(h->G); cudaFree(h->scal);
+    for (PrepSet &S : h->set) {
+        cudaFree(S.amask); cudaFree(S.words); cudaFree(S.tslot); cudaFree(S.bin_first); cudaFree(S.scal);
+    }
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    if (h->cap_bulk) cudaStreamDestroy(h->cap_bulk);
+    if (h->cap_prep) cudaStreamDestroy(h->cap_prep);
+    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    if (h->ev_bulk) cudaEventDestroy(h->ev_bulk);
+    if (h->ev_prep) cudaEventDestroy(h->ev_prep);
     delete h;
 }
 
@@ -595,7 +780,8 @@ int lbm_set_option(lbm_t *h, int key, int value)
         case LBM_OPT_SPREAD: if (value < 0 || value > 2) break; h->opt_spread = value; return LBM_OK;
         case LBM_OPT_FORCING: if (value < 0 || value > 1) break; h->opt_forcing = value; return LBM_OK;
         case LBM_OPT_GRAPH: if (value < 0 || value > 1) break; h->opt_graph = value; return LBM_OK;
-        case LBM_OPT_LBM_KERNEL: if (value < 0 || value > 8) break; h->opt_lbm_kernel = value; return LBM_OK;
+        case LBM_OPT_LBM_KERNEL: if (value < 0 || value > 2) break; h->opt_lbm_kernel = value; return LBM_OK;
+        case LBM_OPT_OVERLAP: if (value < 0 || value > 1) break; h->opt_overlap = value; return LBM_OK;
         case LBM_OPT_INTERP: if (value < 0 || value > 1) break; h->opt_interp = value; return LBM_OK;
         case LBM_OPT_TIMING: if (value < 0 || value > 1) break; h->opt_timing = value; h->timer.reset(); return LBM_OK;
         default: return fail(LBM_EINVAL, "lbm_set_option: unknown key %d", key);
@@ -612,20 +798,12 @@ int lbm_get_info(lbm_t *h, int key, long long *value)
         case LBM_INFO_STEPS: *value = h->steps_done; return LBM_OK;
         case LBM_INFO_LAUNCHES: *value = h->launches; return LBM_OK;
         case LBM_INFO_DEVICE_BYTES: *value = (long long)h->dev_bytes; return LBM_OK;
-        case LBM_INFO_ACTIVE_CELLS: {
+        case LBM_INFO_ACTIVE_CELLS: case LBM_INFO_RUNS: case LBM_INFO_RUN_ENTRIES: {
             int r = 0;
-            if (h->force_valid) {
-                CK(cudaMemcpyAsync(&r, &h->scal->n_cells, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
-                CK(cudaStreamSynchronize(h->stream));
-            }
-            *value = r;
-            return LBM_OK;
-        }
-        case LBM_INFO_RUNS: case LBM_INFO_RUN_ENTRIES: {
-            int r = 0;
-            if (h->force_valid) {
-                CK(cudaMemcpyAsync(&r, key == LBM_INFO_RUNS ? &h->scal->n_runs : &h->scal->t_count, sizeof(int),
-                                   cudaMemcpyDeviceToHost, h->stream));
+            if (h->force_valid && h->last_set >= 0) {
+                const SetScalars *sc = h->set[h->last_set].scal;
+                const int *p = key == LBM_INFO_ACTIVE_CELLS ? &sc->n_cells : (key == LBM_INFO_RUNS ? &sc->n_runs : &sc->t_count);
+                CK(cudaMemcpyAsync(&r, p, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
                 CK(cudaStreamSynchronize(h->stream));
             }
             *value = r;
@@ -777,8 +955,15 @@ int ibm_update_kinematics(lbm_t *h, int first_body, int count, const double *ome
         for (int a = 0; a < 3; ++a) { B.axis[a] = ax[a] / nrm; B.center[a] = c[a]; }
         B.has_kin = true;
     }
+    bool changed = moved;
+    for (int b = 0; b < count && !changed; ++b) {
+        const HostBody &o = h->bodies[(size_t)(first_body + b)], &n = nb[(size_t)b];
+        changed = o.omega != n.omega || o.axis[0] != n.axis[0] || o.axis[1] != n.axis[1] || o.axis[2] != n.axis[2];
+    }
     std::copy(nb.begin(), nb.end(), h->bodies.begin() + first_body);
     if (moved || h->markers_stale) { h->markers_stale = true; return LBM_OK; }
+    // a set prepared ahead for the next step used the old table
+    if (changed) for (PrepSet &S : h->set) if (S.step >= h->steps_done) S.step = -1;
     // centres unchanged: only the small per-body table changes; graphs and marker arrays stay valid
     for (int b = 0; b < count; ++b) {
         const HostBody &B = h->bodies[(size_t)(first_body + b)];
@@ -811,26 +996,47 @@ int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
     const bool ibm = (h->nm > 0 && mdf_iters > 0);
     if (!ibm) { if ((rc = flush_ibm(h))) return rc; }
     if (ibm) {
-        k_set_scalars<<<1, 1, 0, h->stream>>>(&h->scal->step_ctr, h->steps_done, &h->scal->n_prev, 0, 1);
+        k_set_scalars<<<1, 1, 0, h->stream>>>(&h->scal->step_ctr, h->steps_done, nullptr, 0, 1);
         h->launches += 1;
+        if (h->opt_spread != 0)
+            for (PrepSet &S : h->set) if ((rc = ensure_bin_first(h, S))) return rc;
     }
+    const bool overlapped = ibm && h->opt_overlap && h->opt_graph && !h->opt_timing;
     for (int s = 0; s < nsteps; ++s) {
         int nk = 0;
-        if (h->opt_timing) {
-            if ((rc = enqueue_step(h, h->stream, h->cur, mdf_iters, ibm, &nk, &h->timer))) return rc;
-            CK(cudaStreamSynchronize(h->stream));
-            h->timer.collect();
-        } else if (h->opt_graph) {
-            cudaGraphExec_t ex = nullptr;
-            if ((rc = get_graph(h, h->cur, mdf_iters, ibm, &ex, &nk))) return rc;
+        cudaGraphExec_t ex = nullptr;
+        PrepSet *S = ibm ? &h->set[h->cur_set] : nullptr;
+        if (overlapped) {
+            if (S->step != h->steps_done || S->spread != h->opt_spread) {
+                // first step of a run (or the kinematics changed): prepare this step's set in line
+                int np = 0;
+                if ((rc = enqueue_prep(h, h->stream, *S, 0, &np, nullptr))) return rc;
+                h->launches += np;
+                S->step = h->steps_done; S->spread = h->opt_spread; S->dirty = true;
+            }
+            if ((rc = get_graph(h, 2, h->cur, h->cur_set, mdf_iters, &ex, &nk))) return rc;
             CK(cudaGraphLaunch(ex, h->stream));
+            PrepSet &N = h->set[h->cur_set ^ 1];
+            N.step = h->steps_done + 1; N.spread = h->opt_spread; N.dirty = true;
+            h->last_set = h->cur_set;
+            h->cur_set ^= 1;
         } else {
-            if ((rc = enqueue_step(h, h->stream, h->cur, mdf_iters, ibm, &nk))) return rc;
+            if (h->opt_timing) {
+                if ((rc = enqueue_step_serial(h, h->stream, h->cur, S, true, mdf_iters, &nk, &h->timer))) return rc;
+                CK(cudaStreamSynchronize(h->stream));
+                h->timer.collect();
+            } else if (h->opt_graph) {
+                if ((rc = get_graph(h, ibm ? 1 : 0, h->cur, h->cur_set, mdf_iters, &ex, &nk))) return rc;
+                CK(cudaGraphLaunch(ex, h->stream));
+            } else {
+                if ((rc = enqueue_step_serial(h, h->stream, h->cur, S, true, mdf_iters, &nk))) return rc;
+            }
+            if (S) { S->step = h->steps_done; S->spread = h->opt_spread; S->dirty = true; h->last_set = h->cur_set; }
         }
         h->launches += nk;
         h->cur ^= 1;
         h->steps_done += 1;
-        if (ibm) { h->ibm_dirty = true; h->force_valid = true; }
+        if (ibm) h->force_valid = true;
     }
     return LBM_OK;
 }
@@ -856,8 +1062,8 @@ int lbm_read_fields(lbm_t *h, float *rho, float *u, float *force)
         }
     }
     dim3 b = cell_block(h->g);
-    k_read_fields<<<cell_grid(h->g, b), b, 0, h->stream>>>(h->f[h->cur], h->g, h->force_valid ? h->amask : nullptr,
-                                                            h->G, dev[0], dev[1], dev[2]);
+    const unsigned *mask = (h->force_valid && h->last_set >= 0) ? h->set[h->last_set].amask : nullptr;
+    k_read_fields<<<cell_grid(h->g, b), b, 0, h->stream>>>(h->f[h->cur], h->g, mask, h->G, dev[0], dev[1], dev[2]);
     h->launches += 1;
     cudaError_t e = cudaGetLastError();
     bool any_tmp = false;
@@ -877,10 +1083,11 @@ int ibm_read_markers(lbm_t *h, float *pos, float *force, int *perm, int *cell)
     if (!h) return fail(LBM_EINVAL, "ibm_read_markers: NULL handle");
     const int n = (int)h->h_area.size();
     if (n == 0 || (!pos && !force && !perm && !cell)) return LBM_OK;
-    if (!h->ibm_dirty || h->markers_stale)
+    if (h->last_set < 0 || h->markers_stale)
         return fail(LBM_ESTATE, "ibm_read_markers: no IBM step has been run with the current markers");
-    const unsigned *skey = h->d_keys[h->sort_passes & 1];
-    const int *dperm = h->d_vals[h->sort_passes & 1];
+    const PrepSet &S = h->set[h->last_set];
+    const unsigned *skey = sorted_keys(h, S);
+    const int *dperm = sorted_perm(h, S);
     void *out[3] = {pos, force, cell};
     const size_t bytes[3] = {sizeof(float) * 3 * (size_t)n, sizeof(float) * 3 * (size_t)n, sizeof(int) * (size_t)n};
     void *dev[3] = {nullptr, nullptr, nullptr};
@@ -890,7 +1097,7 @@ int ibm_read_markers(lbm_t *h, float *pos, float *force, int *perm, int *cell)
         if (is_device_ptr(out[a])) dev[a] = out[a];
         else { CK(cudaMalloc(&dev[a], bytes[a])); tmp[a] = true; }
     }
-    k_read_markers<<<(n + 255) / 256, 256, 0, h->stream>>>(skey, dperm, n, h->g, h->ms.fs, h->ms.du, (float *)dev[0],
+    k_read_markers<<<(n + 255) / 256, 256, 0, h->stream>>>(skey, dperm, n, h->g, S.ms.fs, S.ms.du, (float *)dev[0],
                                                             (float *)dev[1], (int *)dev[2]);
     h->launches += 1;
     cudaError_t e = cudaGetLastError();

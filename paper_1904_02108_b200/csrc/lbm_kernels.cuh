@@ -105,39 +105,56 @@ __device__ __forceinline__ bool cell_is_active(const unsigned *__restrict__ amas
     return (w >> (x & 31)) & 1u;
 }
 
-// Pull for a cell whose y and z neighbours are plain lattice rows (no wrap, no wall): every source
-// row sits at a constant offset from the cell's own row; only x needs the wrapped neighbour, and an
-// x wall the bounce-back select.
-__device__ __forceinline__ void pull_cell_inner(const float *__restrict__ src, const Geom &g, int x, int self,
-                                                float (&df)[NQ])
+// Byte offsets of the interior pull and of the stores, the same for every interior cell; filled on
+// the host (plane_offsets) so that each access costs one 64-bit add of a constant-bank operand.
+struct PlaneOffsets {
+    long long ld[NQ];    // (i pitch - e_y nx - e_z nx ny) * 4: source of direction i relative to the cell (x handled apart)
+    long long st[NQ];    // (i pitch) * 4
+};
+
+inline PlaneOffsets plane_offsets(const Geom &g)
 {
-    const size_t cells = (size_t)g.pitch;
-    const int dxm = (x == 0) ? g.nx - 1 : -1;          // offset to the cell at x-1 (wrapped)
-    const int dxp = (x == g.nx - 1) ? 1 - g.nx : 1;    // offset to the cell at x+1 (wrapped)
-    const bool wlo = g.wallx && x == 0, whi = g.wallx && x == g.nx - 1;
-    const int sy = g.nx, sz = g.nx * g.ny;
-    const float *__restrict__ p = src + self;
+    PlaneOffsets o;
+    for (int i = 0; i < NQ; ++i) {
+        o.ld[i] = 4 * ((long long)i * g.pitch - (long long)dir_ey(i) * g.nx - (long long)dir_ez(i) * g.nx * g.ny);
+        o.st[i] = 4 * ((long long)i * g.pitch);
+    }
+    return o;
+}
+
+// Pull for a cell whose y and z neighbours are plain lattice rows (no wrap, no wall) and that has
+// no x wall behind it: every source sits at a kernel-uniform byte offset (plane + row shift) from
+// one of three per-thread pointers (the cell itself, its wrapped x-1 and x+1 neighbours).
+__device__ __forceinline__ void pull_cell_inner(const float *__restrict__ src, const Geom &g, const PlaneOffsets &po,
+                                                int x, int self, float (&df)[NQ])
+{
+    const char *__restrict__ p0 = reinterpret_cast<const char *>(src + self);
+    const char *__restrict__ pm = p0 + 4 * ((x == 0) ? g.nx - 1 : -1);          // cell at x-1 (wrapped)
+    const char *__restrict__ pp = p0 + 4 * ((x == g.nx - 1) ? 1 - g.nx : 1);    // cell at x+1 (wrapped)
 #pragma unroll
     for (int i = 0; i < NQ; ++i) {
-        const int off = (dir_ex(i) == 1 ? dxm : (dir_ex(i) == -1 ? dxp : 0)) - dir_ey(i) * sy - dir_ez(i) * sz;
-        if (dir_ex(i) == 0) {
-            df[i] = LBM_LOAD(p + ((size_t)i * cells + off));
-        } else {
-            const bool behind = dir_ex(i) == 1 ? wlo : whi;
-            const long long o = behind ? (long long)((size_t)dir_opp(i) * cells) : (long long)((size_t)i * cells) + off;
-            df[i] = LBM_LOAD(p + o);
-        }
+        const char *__restrict__ b = dir_ex(i) == 1 ? pm : (dir_ex(i) == -1 ? pp : p0);
+        df[i] = LBM_LOAD(reinterpret_cast<const float *>(b + po.ld[i]));
     }
 }
 
 // ---------------------------------------------------------------------------------------------
 // a8, one thread per cell, x along threadIdx.x (coalesced 128 B per warp and plane), one x-row
-// segment per block so that "is this an interior row" is block-uniform.  IBM = true reads one
-// bitmask word per warp and G only where a marker stencil reaches; both are issued before the
-// population loads so their latency overlaps.
-template <bool IBM, int THREADS, int MINB>
+// segment per block so that "is this an interior row" is block-uniform.
+//   MODE 0: pure LBM (a = g_body everywhere).
+//   MODE 1: fused IBM pass: one bitmask word per warp, G read only where a marker stencil reaches
+//           (both issued before the population loads so their latency overlaps).
+//   MODE 2: bulk pass of the overlapped step: a warp covers exactly the 32 cells of one mask word;
+//           warps whose word is non-zero are SKIPPED as a whole (k_stream_collide_words updates
+//           them once G is known), so both passes write whole 128-byte lines (measured: skipping
+//           8-cell groups instead leaves less for the second pass but is slower overall).
+//           Everywhere else a = g_body: this pass needs nothing from the IBM and runs beside it.
+enum { LBM_PURE = 0, LBM_FUSED = 1, LBM_BULK = 2 };
+
+template <int MODE, int THREADS, int MINB>
 __global__ void __launch_bounds__(THREADS, MINB)
-k_stream_collide_scalar(const float *__restrict__ src, float *__restrict__ dst, Geom g, CollisionConst cc,
+k_stream_collide_scalar(const float *__restrict__ src, float *__restrict__ dst, const __grid_constant__ Geom g,
+                        const __grid_constant__ CollisionConst cc, const __grid_constant__ PlaneOffsets po,
                         const unsigned *__restrict__ amask, const float4 *__restrict__ G)
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
@@ -147,24 +164,75 @@ k_stream_collide_scalar(const float *__restrict__ src, float *__restrict__ dst, 
     const int self = (z * g.ny + y) * g.nx + x;
 
     float ax = cc.gbx, ay = cc.gby, az = cc.gbz;
-    if (IBM) {
+    if (MODE == LBM_FUSED) {
         if (cell_is_active(amask, g, x, y, z)) {
             const float4 gv = __ldg(G + self);
             ax += gv.x; ay += gv.y; az += gv.z;
         }
     }
+    if (MODE == LBM_BULK) {
+        if (__ldg(amask + (size_t)(z * g.ny + y) * g.nxw + (x >> 5)) != 0u) return;
+    }
     float df[NQ];
-    if (y > 0 && y < g.ny - 1 && z > 0 && z < g.nz - 1) {
-        pull_cell_inner(src, g, x, self, df);
+    const bool xwall = g.wallx && (x == 0 || x == g.nx - 1);
+    if (y > 0 && y < g.ny - 1 && z > 0 && z < g.nz - 1 && !xwall) {
+        pull_cell_inner(src, g, po, x, self, df);
     } else {
         const Nbr n = neighbours(g, x, y, z);
         pull_cell(src, g, n, x, y, z, df);
     }
     collide(df, ax, ay, az, cc);
-    const size_t cells = (size_t)g.pitch;
-    float *__restrict__ q = dst + self;
+    char *__restrict__ q = reinterpret_cast<char *>(dst + self);
 #pragma unroll
-    for (int i = 0; i < NQ; ++i) LBM_STORE(q + (size_t)i * cells, df[i]);
+    for (int i = 0; i < NQ; ++i) LBM_STORE(reinterpret_cast<float *>(q + po.st[i]), df[i]);
+}
+
+// a8 on the words the bulk pass skipped (second pass of the overlapped step): one warp per entry of
+// the active-word list, lane = cell of the word; a = G + g_body where the cell's bit is set, g_body
+// on the other cells of the word.
+__global__ void __launch_bounds__(256)
+k_stream_collide_words(const float *__restrict__ src, float *__restrict__ dst, const __grid_constant__ Geom g,
+                       const __grid_constant__ CollisionConst cc, const __grid_constant__ PlaneOffsets po,
+                       const unsigned *__restrict__ amask, const int *__restrict__ words,
+                       const int *__restrict__ n_words, const float4 *__restrict__ G)
+{
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    const int nw = *n_words;
+    // the word and its mask bits of the next round are fetched while this round's cells are updated
+    int w_next = warp < nw ? __ldg(words + warp) : 0;
+    unsigned bits_next = warp < nw ? __ldg(amask + w_next) : 0u;
+    for (int k = warp; k < nw; k += nwarps) {
+        const int w = w_next;
+        const unsigned bits = bits_next;
+        if (k + nwarps < nw) {
+            w_next = __ldg(words + k + nwarps);
+            bits_next = __ldg(amask + w_next);
+        }
+        const int row = w / g.nxw;
+        const int x = (w - row * g.nxw) * 32 + lane;
+        if (x >= g.nx) continue;
+        const int z = row / g.ny, y = row - z * g.ny;
+        const int self = row * g.nx + x;
+        float ax = cc.gbx, ay = cc.gby, az = cc.gbz;
+        if ((bits >> lane) & 1u) {
+            const float4 gv = __ldg(G + self);
+            ax += gv.x; ay += gv.y; az += gv.z;
+        }
+        float df[NQ];
+        const bool xwall = g.wallx && (x == 0 || x == g.nx - 1);
+        if (y > 0 && y < g.ny - 1 && z > 0 && z < g.nz - 1 && !xwall) {
+            pull_cell_inner(src, g, po, x, self, df);
+        } else {
+            const Nbr n = neighbours(g, x, y, z);
+            pull_cell(src, g, n, x, y, z, df);
+        }
+        collide(df, ax, ay, az, cc);
+        char *__restrict__ q = reinterpret_cast<char *>(dst + self);
+#pragma unroll
+        for (int i = 0; i < NQ; ++i) LBM_STORE(reinterpret_cast<float *>(q + po.st[i]), df[i]);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -339,7 +407,8 @@ k_read_fields(const float *__restrict__ src, Geom g, const unsigned *__restrict_
 // de-duplicated): one thread per entry of the active-cell list pulls its 19 populations.
 // U is stored as float4 (Ux, Uy, Uz, rho).
 __global__ void __launch_bounds__(256)
-k_moments_active(const float *__restrict__ src, Geom g, const int *__restrict__ cells,
+k_moments_active(const float *__restrict__ src, const __grid_constant__ Geom g,
+                 const __grid_constant__ PlaneOffsets po, const int *__restrict__ cells,
                  const int *__restrict__ n_cells, float4 *__restrict__ U)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -350,9 +419,14 @@ k_moments_active(const float *__restrict__ src, Geom g, const int *__restrict__ 
         const int row = cell / g.nx;
         const int x = cell - row * g.nx;
         const int z = row / g.ny, y = row - z * g.ny;
-        const Nbr n = neighbours(g, x, y, z);
         float df[NQ], drho, ux, uy, uz;
-        pull_cell(src, g, n, x, y, z, df);
+        const bool xwall = g.wallx && (x == 0 || x == g.nx - 1);
+        if (y > 0 && y < g.ny - 1 && z > 0 && z < g.nz - 1 && !xwall) {
+            pull_cell_inner(src, g, po, x, cell, df);
+        } else {
+            const Nbr n = neighbours(g, x, y, z);
+            pull_cell(src, g, n, x, y, z, df);
+        }
         moments(df, drho, ux, uy, uz);
         U[cell] = make_float4(ux, uy, uz, 1.0f + drho);
     }

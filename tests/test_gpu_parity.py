@@ -157,6 +157,68 @@ def test_w1_atomic_variant_matches_and_gather_is_deterministic(api, orc):
     assert np.abs(outs[0][3] - outs[3][3]).max() <= 1e-5 * np.abs(outs[0][3]).max()
 
 
+def _run_w1(api, steps_per_call, overlap, graph=1, reads=False, retune_at=None):
+    """W1 for sum(steps_per_call) steps; returns (rho, u, G, marker forces, perm)."""
+    from paper_1904_02108_b200 import workloads
+    wl = workloads.get("W1")
+    sim = api.from_workload(wl, stream=_stream())
+    sim.set_option(api.OPT_OVERLAP, overlap)
+    sim.set_option(api.OPT_GRAPH, graph)
+    done = 0
+    for n in steps_per_call:
+        if retune_at is not None and done == retune_at:
+            b = wl.bodies[0]
+            sim.update_kinematics(0, np.array([2.0 * b.omega]), np.array([b.axis]))
+        sim.step(n, wl.mdf_iters)
+        done += n
+        if reads:
+            sim.read_markers()
+            sim.read_fields()
+    mk = sim.read_markers()
+    out = sim.read_fields() + (mk["force"], mk["perm"])
+    sim.sync()
+    sim.close()
+    return out
+
+
+def test_overlapped_step_equals_serial_step_bitwise(api):
+    """LBM_OPT_OVERLAP only reorders independent work (bulk stream-collide beside the MDF loop, the
+    next step's binning ahead of time): every output must be bit-identical to the serial chain,
+    whatever the split into calls, with read-outs in between, and with plain launches."""
+    ref = _run_w1(api, [12], overlap=0)
+    for kw in (dict(steps_per_call=[12], overlap=1), dict(steps_per_call=[1, 2, 1, 5, 3], overlap=1, reads=True),
+               dict(steps_per_call=[5, 7], overlap=1, graph=0), dict(steps_per_call=[3, 9], overlap=0, graph=0)):
+        got = _run_w1(api, **kw)
+        for a, b in zip(ref, got):
+            assert np.array_equal(a, b), kw
+
+
+def test_kinematics_change_discards_the_set_prepared_ahead(api):
+    """the overlapped step bins the markers of step n+1 during step n; a new omega before step n+1
+    must win over that prepared set (compare with the serial chain, which never prepares ahead)."""
+    ref = _run_w1(api, [4, 6], overlap=0, retune_at=4)
+    got = _run_w1(api, [4, 6], overlap=1, retune_at=4)
+    same = _run_w1(api, [4, 6], overlap=1)
+    for a, b in zip(ref, got):
+        assert np.array_equal(a, b)
+    assert not np.array_equal(same[3], got[3])
+
+
+def test_pure_and_coupled_steps_interleave(api, orc):
+    """mdf_iters = 0 calls between coupled calls (flushes the marker sets, flips the buffer parity)."""
+    from paper_1904_02108_b200 import workloads
+    wl = workloads.get("W1")
+    sim = api.from_workload(wl, stream=_stream())
+    ref = orc.from_workload(wl)
+    for n, mdf in ((3, wl.mdf_iters), (2, 0), (1, wl.mdf_iters), (1, 0), (4, wl.mdf_iters)):
+        sim.step(n, mdf)
+        ref.step(n, mdf)
+    sim.sync()
+    _compare_fields(sim, ref)
+    _check_markers(sim, ref, orc, wl)
+    sim.close()
+
+
 def test_static_markers_with_prescribed_velocity_and_walls(api, orc):
     """omega = 0 bodies (R14), two bodies, walls on z, markers near (but legally off) the walls."""
     rng = np.random.default_rng(21)
