@@ -128,7 +128,7 @@ struct MarkerSorted {
     float4 *fs;     // (fx, fy, fz, s)
     float4 *wx;     // the four x weights w(x_k - X), X = cx-1 .. cx+2
     float *wyz;     // [16] per marker: w_y(jy) w_z(jz) at index jy*4+jz
-                    // sg.w and du.w carry the marker's cell x index (int bits) for the run sweep
+                    // sg.w and du.w carry the marker's cell x index (int bits) for the chunk sweep
     float4 *uk;     // prescribed velocity u_k, w unused
     float4 *sg;     // s * g^m(k)   (what the U update spreads, P:98 + R8)
     float4 *du;     // Delta u(k)
@@ -234,23 +234,19 @@ k_bins(const unsigned *__restrict__ skey, int n, Geom g, int *__restrict__ bin_f
     }
 }
 
-// Undo what k_bins of the previous step left behind (bitmask words and cell -> first-marker
-// entries), so neither needs a full-lattice memset per step.
+// Undo what the previous preparation of this marker set left in the dense maps (bitmask words, chunk
+// registrations, cell -> first-marker entries), so none of them needs a full memset per step.
 __global__ void __launch_bounds__(256)
 k_clear_prev(const unsigned *__restrict__ skey_prev, const int *__restrict__ n_prev, int *__restrict__ bin_first,
              unsigned *__restrict__ amask, const int *__restrict__ words, const int *__restrict__ n_words,
-             int *__restrict__ tslot, const int *__restrict__ run_slot0, const int *__restrict__ run_nent,
-             const int *__restrict__ n_runs)
+             int *__restrict__ chunk_of, const int *__restrict__ chunk_slot, const int *__restrict__ n_chunks, int cap)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     const int stride = gridDim.x * blockDim.x;
-    const int np = *n_prev, nw = *n_words, nr = *n_runs;
+    const int np = *n_prev, nw = *n_words, nc = min(*n_chunks, cap);
     if (bin_first) for (int i = tid; i < np; i += stride) bin_first[skey_prev[i]] = -1;
     for (int i = tid; i < nw; i += stride) amask[words[i]] = 0u;
-    for (int r = tid; r < nr; r += stride) {
-        const int s0 = run_slot0[r], ne = run_nent[r];
-        for (int j = 0; j < ne; ++j) tslot[s0 + j] = -1;
-    }
+    for (int c = tid; c < nc; c += stride) chunk_of[chunk_slot[c]] = -1;
 }
 
 // device scalars: mode bit 0: step_ctr = step; bit 1: n_prev = n_prev_val; bit 2: step_ctr += 1
@@ -381,37 +377,63 @@ k_spread_gather(const unsigned *__restrict__ skey, int n, Geom g, const int *__r
 // ---------------------------------------------------------------------------------------------
 // a7, product path: deterministic spreading in two stages, no atomics on the field.
 //
-// A "run" is a maximal stretch of sorted markers in one lattice row (same cy, cz) whose owning
-// cells are less than 4 apart in x, i.e. whose stencils chain together along x.  Runs of one row
-// never touch the same cell, and a marker of source row (cy, cz) reaches the 16 target rows
-// (cy-1+jy, cz-1+jz).  Stage A sweeps every run once, in sorted order, and produces for each of the
-// 16 (jy, jz) offsets the x-profile  T[entry][jy*4+jz] = sum_k v_k w_y(jy) w_z(jz) w_x(X - cx_k + 1)
-// over the run's x extent (entries cx_first-1 .. cx_last+2).  Stage B lets every active cell add
-// up, in fixed order, the <= 16 profiles that reach it (one per source row).  All sums have a fixed
-// order, so the result is bitwise reproducible.
+// A "chunk" is the stretch of sorted markers that lie in one lattice row (same cy, cz) and in one
+// aligned block of CHUNK_W = 8 cells in x.  A marker of source row (cy, cz) reaches the 16 target
+// rows (cy-1+jy, cz-1+jz) and, in x, the cells cx-1 .. cx+2, so a chunk of block j touches the
+// window X = 8j-1 .. 8j+9 (CHUNK_W + 3 "entries") of each target row.  Stage A sweeps every chunk
+// once, in sorted order, and produces for each of the 16 (jy, jz) offsets the x-profile
+//     T[chunk][jy*4+jz][e] = sum_k v_k w_y(jy) w_z(jz) w_x(X_e - cx_k + 1),   X_e = 8j - 1 + e.
+// Stage B lets every active cell add up, in fixed order, the profiles that reach it: per source row
+// at most two chunks (the blocks holding cx = X-2 and cx = X+1).  All sums have a fixed order, so
+// the result is bitwise reproducible.  Chunks are short (<= 8 cells wide), uniform in cost and
+// plentiful, which is what keeps 148 SMs busy on a single propeller as well as on 12 M markers.
 
-struct RunTable {
-    int *first, *end;   // sorted-marker range [first, end) of the run
-    int *base;          // first T entry of the run
-    int *slot0;         // index into tslot of the run's first entry
-    int *nent;          // number of entries = cx_last - cx_first + 4
+constexpr int CHUNK_W = 8;
+constexpr int CHUNK_ENT_MAX = 14;     // widest window: a last block widened to 11 cells (see ChunkGeom)
+
+// Blocks in x: 8 cells each; when nx % 8 is 1..3 the remainder joins the last block (width 9..11), so
+// that every block is at least 4 wide and four consecutive cells (periodic or not) meet at most two
+// blocks.  ent = widest window = widest block + 3.
+struct ChunkGeom {
+    int nbx;     // blocks per row
+    int ent;     // entries per (chunk, jy, jz) profile (row pitch of T)
 };
 
-// tslot is a dense map [row][X + 1], X = -1 .. nx+1 (unwrapped x, so that runs at a periodic seam
-// keep their own entries), holding the T entry or -1.
-__device__ __forceinline__ int tslot_pitch(const Geom &g) { return g.nx + 3; }
+inline ChunkGeom chunk_geom(int nx)
+{
+    ChunkGeom c;
+    const int rem = nx % CHUNK_W;
+    c.nbx = nx / CHUNK_W + ((rem >= 4 || nx < CHUNK_W) ? 1 : 0);
+    if (c.nbx < 1) c.nbx = 1;
+    const int last_w = nx - (c.nbx - 1) * CHUNK_W;
+    c.ent = (last_w > CHUNK_W ? last_w : CHUNK_W) + 3;
+    return c;
+}
 
-// a3 (second part): one bit per sorted marker, set where a run starts.  Bits at and beyond n are
-// set as well, so a forward search for the next run start always terminates.
+__device__ __forceinline__ int chunk_block(int cx, int nbx) { return min(cx >> 3, nbx - 1); }
+
+// chunk_of[row * nbx + block] packs (chunk id, first entry lo, last entry hi) of the chunk registered there,
+// or -1:  id in bits 0..22, lo in bits 23..26, hi in bits 27..30.
+constexpr int CHUNK_ID_BITS = 23;
+constexpr int CHUNK_ID_MAX = (1 << CHUNK_ID_BITS) - 1;
+__device__ __forceinline__ int chunk_pack(int id, int lo, int hi) { return id | (lo << 23) | (hi << 27); }
+
+struct ChunkTable {
+    int *first, *end;   // sorted-marker range [first, end) of the chunk
+    int *slot;          // index into chunk_of (= row * nbx + block)
+};
+
+// a3 (second part): one bit per sorted marker, set where a chunk starts.  Bits at and beyond n are
+// set as well, so a forward search for the next chunk start always terminates.
 __global__ void __launch_bounds__(256)
-k_run_heads(const unsigned *__restrict__ skey, int n, Geom g, unsigned *__restrict__ headbits)
+k_chunk_heads(const unsigned *__restrict__ skey, int n, Geom g, ChunkGeom cg, unsigned *__restrict__ headbits)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool head = true;
     if (i > 0 && i < n) {
         const unsigned key = skey[i], pk = skey[i - 1];
         const int row = (int)(key / (unsigned)g.nx), prow = (int)(pk / (unsigned)g.nx);
-        head = (prow != row) || (((int)key - row * g.nx) - ((int)pk - prow * g.nx) >= 4);
+        head = (prow != row) || (chunk_block((int)key - row * g.nx, cg.nbx) != chunk_block((int)pk - prow * g.nx, cg.nbx));
     }
     const unsigned vote = __ballot_sync(0xffffffffu, head);
     if ((threadIdx.x & 31) == 0) headbits[i >> 5] = vote;
@@ -437,16 +459,18 @@ __device__ __forceinline__ void mark_span(unsigned *__restrict__ amask, int rowb
     }
 }
 
-// a3 (third part): the first marker of every run finds the run's end and takes a block of T entries.
+// a3 (third part): the first marker of every chunk finds the chunk's end, takes a chunk id and
+// registers the chunk in chunk_of.  Chunks beyond `cap` are dropped and flagged in *status (bit 1).
 __global__ void __launch_bounds__(256)
-k_runs(const unsigned *__restrict__ skey, int n, Geom g, const unsigned *__restrict__ headbits, RunTable rt,
-       int *__restrict__ n_runs, int *__restrict__ t_count)
+k_chunks(const unsigned *__restrict__ skey, int n, Geom g, ChunkGeom cg, const unsigned *__restrict__ headbits,
+         ChunkTable ct, int cap, int *__restrict__ n_chunks, int *__restrict__ n_entries, int *__restrict__ chunk_of,
+         int *__restrict__ status)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     const unsigned myword = (i < n) ? headbits[i >> 5] : 0u;
     const bool head = (myword >> lane) & 1u;
-    int row = 0, cx = 0, end = 0, nent = 0;
+    int slot = 0, end = 0, lo = 0, hi = 0;
     if (head) {
         // next set bit after i
         int wi = i >> 5;
@@ -455,52 +479,58 @@ k_runs(const unsigned *__restrict__ skey, int n, Geom g, const unsigned *__restr
         end = (wi << 5) + __ffs(w) - 1;
         if (end > n) end = n;
         const unsigned key = skey[i], lk = skey[end - 1];
-        row = (int)(key / (unsigned)g.nx);
-        cx = (int)key - row * g.nx;
-        nent = ((int)lk - row * g.nx) - cx + 4;
+        const int row = (int)(key / (unsigned)g.nx);
+        const int cx = (int)key - row * g.nx;
+        const int blk = chunk_block(cx, cg.nbx);
+        slot = row * cg.nbx + blk;
+        lo = cx - blk * CHUNK_W;                                   // window of the first marker starts at entry lo
+        hi = ((int)lk - row * g.nx) - blk * CHUNK_W + 3;           // window of the last marker ends at entry hi
     }
+    // chunk ids: one atomic per block (warp counts -> block scan), ids ascend with the marker index inside a block
+    __shared__ int s_cnt[8], s_ent[8], s_base;
+    const int wib = threadIdx.x >> 5;
     const unsigned vote = __ballot_sync(0xffffffffu, head);
-    if (!vote) return;
-    int incl = nent;
+    int ne = head ? hi - lo + 1 : 0;
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int t = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += t;
+    for (int o = 16; o > 0; o >>= 1) ne += __shfl_xor_sync(0xffffffffu, ne, o);
+    if (lane == 0) { s_cnt[wib] = __popc(vote); s_ent[wib] = ne; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int tc = 0, te = 0;
+        for (int w = 0; w < 8; ++w) { const int t = s_cnt[w]; s_cnt[w] = tc; tc += t; te += s_ent[w]; }
+        s_base = tc ? atomicAdd(n_chunks, tc) : 0;
+        if (te) atomicAdd(n_entries, te);
     }
-    const int total = __shfl_sync(0xffffffffu, incl, 31);
-    int rbase = 0, tbase = 0;
-    if (lane == 0) { rbase = atomicAdd(n_runs, __popc(vote)); tbase = atomicAdd(t_count, total); }
-    rbase = __shfl_sync(0xffffffffu, rbase, 0);
-    tbase = __shfl_sync(0xffffffffu, tbase, 0);
+    __syncthreads();
     if (!head) return;
-    const int r = rbase + __popc(vote & ((1u << lane) - 1u));
-    const int base = tbase + incl - nent;
-    const int s0 = row * tslot_pitch(g) + cx;        // X = cx - 1  ->  column X + 1 = cx
-    rt.first[r] = i; rt.end[r] = end; rt.base[r] = base; rt.slot0[r] = s0; rt.nent[r] = nent;
+    const int c = s_base + s_cnt[wib] + __popc(vote & ((1u << lane) - 1u));
+    if (c >= cap) { atomicOr(status, 2); return; }
+    ct.first[c] = i; ct.end[c] = end; ct.slot[c] = slot;
+    chunk_of[slot] = chunk_pack(c, lo, hi);
 }
 
-// a3 (fourth part): one half-warp per run publishes the run: its T entries go into tslot and its
-// cells -- the whole x span cx_first-1 .. cx_last+2 in each of the 16 target rows, one row per lane
-// -- are marked in the active-cell bitmask.
+// a3 (fourth part): one half-warp per chunk marks the chunk's cells -- the x span cx_first-1 ..
+// cx_last+2 in each of the 16 target rows, one row per lane -- in the active-cell bitmask.
 __global__ void __launch_bounds__(256)
-k_run_publish(Geom g, RunTable rt, const int *__restrict__ n_runs, int *__restrict__ tslot,
-              unsigned *__restrict__ amask, int *__restrict__ words, int *__restrict__ n_words)
+k_chunk_publish(Geom g, ChunkGeom cg, ChunkTable ct, const int *__restrict__ n_chunks, int cap,
+                const int *__restrict__ chunk_of, unsigned *__restrict__ amask, int *__restrict__ words,
+                int *__restrict__ n_words)
 {
     const int l = threadIdx.x & 15;
     const int hw = (blockIdx.x * blockDim.x + threadIdx.x) >> 4;
     const int nhw = (gridDim.x * blockDim.x) >> 4;
-    const int nr = *n_runs;
-    const int pitch = tslot_pitch(g);
-    for (int r = hw; r < nr; r += nhw) {
-        const int s0 = rt.slot0[r], nent = rt.nent[r], base = rt.base[r];
-        for (int j = l; j < nent; j += 16) tslot[s0 + j] = base + j;
-        const int row = s0 / pitch;
-        const int cx = s0 - row * pitch;
+    const int nc = min(*n_chunks, cap);
+    for (int c = hw; c < nc; c += nhw) {
+        const int slot = ct.slot[c];
+        const int packed = chunk_of[slot];
+        const int lo = (packed >> 23) & 15, hi = (packed >> 27) & 15;
+        const int row = slot / cg.nbx;
+        const int blk = slot - row * cg.nbx;
         const int cz = row / g.ny, cy = row - cz * g.ny;
-        // x span [cx-1, cx+nent-2], wrapped on a periodic axis (inside the box on a wall axis)
-        const int xa = cx - 1, xb = cx + nent - 2;
+        // x span [xa, xb] = entries lo..hi, entry e <-> X = 8 blk - 1 + e; wrapped on a periodic axis
+        const int xa = blk * CHUNK_W - 1 + lo, xb = blk * CHUNK_W - 1 + hi;
         int x0a, x1a, x0b = 0, x1b = -1;
-        if (nent >= g.nx) { x0a = 0; x1a = g.nx - 1; }
+        if (xb - xa + 1 >= g.nx) { x0a = 0; x1a = g.nx - 1; }
         else if (xa < 0) { x0a = xa + g.nx; x1a = g.nx - 1; x0b = 0; x1b = xb; }
         else if (xb >= g.nx) { x0a = xa; x1a = g.nx - 1; x0b = 0; x1b = xb - g.nx; }
         else { x0a = xa; x1a = xb; }
@@ -548,120 +578,148 @@ k_active_cells(Geom g, const unsigned *__restrict__ amask, const int *__restrict
     }
 }
 
-// Stage A: one half-warp per run, lane l = jy*4 + jz owns the profile of target-row offset (jy, jz)
-// and keeps a sliding window of four x cells (cxw-1 .. cxw+2) in registers; cells that fall out of
-// the window as the sweep advances are final and are written to T (16 lanes x float4 = 256 B).
-// Runs are handed out through an atomic cursor (they differ a lot in length); the data of marker
-// i+1 is fetched while marker i is accumulated.
+// Stage A: one warp per chunk.  Lane = h*16 + l: l = jy*4 + jz is the target-row offset whose
+// profile the lane accumulates, h the half of the 4-cell x window it owns (h = 0: the two left
+// cells, h = 1: the two right cells), both in registers.  When the sweep moves on to the next cell
+// the leftmost window cell is final: it is written to T and the window shifts by one (the cell that
+// crosses from the right half to the left half travels by shuffle).  Control flow is uniform across
+// the warp; chunks are handed out through an atomic cursor.
 struct Acc3 { float x, y, z; };
 
 __global__ void __launch_bounds__(256)
-k_spread_rows(RunTable rt, const int *__restrict__ n_runs, int *__restrict__ cursor,
-              const float4 *__restrict__ wx4, const float *__restrict__ wyz16, const float4 *__restrict__ val,
-              float4 *__restrict__ T)
+k_spread_chunks(ChunkTable ct, const int *__restrict__ n_chunks, int cap, int *__restrict__ cursor,
+                const int *__restrict__ chunk_of, ChunkGeom cg, const float2 *__restrict__ wx2,
+                const float *__restrict__ wyz16, const float4 *__restrict__ val, float4 *__restrict__ T)
 {
     const int lane = threadIdx.x & 31;
-    const int l = lane & 15;
-    const unsigned hmask = 0xffffu << (lane & 16);
-    const int nr = *n_runs;
+    const int l = lane & 15, h = lane >> 4;
+    const int nc = min(*n_chunks, cap);
     for (;;) {
-        int r = 0;
-        if (l == 0) r = atomicAdd(cursor, 1);
-        r = __shfl_sync(hmask, r, lane & 16);
-        if (r >= nr) break;
-        const int i0 = rt.first[r], i1 = rt.end[r];
-        float4 *out = T + (size_t)rt.base[r] * 16 + l;
-        Acc3 a0{0.f, 0.f, 0.f}, a1{0.f, 0.f, 0.f}, a2{0.f, 0.f, 0.f}, a3{0.f, 0.f, 0.f};
-        // markers are taken in batches of RB: all loads of a batch are issued before the first
-        // marker is accumulated, so the memory latency is paid once per batch, not once per marker
+        int c = 0;
+        if (lane == 0) c = atomicAdd(cursor, 1);
+        c = __shfl_sync(0xffffffffu, c, 0);
+        if (c >= nc) break;
+        const int i0 = ct.first[c], i1 = ct.end[c];
+        const int slot = ct.slot[c];
+        const int blk = slot % cg.nbx;
+        const int x0 = blk * CHUNK_W;                       // entry e <-> cell X = x0 - 1 + e
+        float4 *out = T + ((size_t)c * 16 + l) * cg.ent;    // profile row of this lane
+        Acc3 p{0.f, 0.f, 0.f}, q{0.f, 0.f, 0.f};            // window cells (e + 2h, e + 2h + 1)
+        const float4 *__restrict__ pv = val + i0;
+        const float2 *__restrict__ pw = wx2 + 2 * (size_t)i0 + h;
+        const float *__restrict__ pz = wyz16 + 16 * (size_t)i0 + l;
+        int e = __float_as_int(pv->w) - x0;                 // window start = entry of the first marker's cx - 1
+        auto add_marker = [&](const float4 v, const float2 w, const float wz) {
+            const int em = __float_as_int(v.w) - x0;
+            if (em != e) {                                  // warp-uniform: the sweep moves on to another cell
+#pragma unroll 1
+                do {                                        // the leftmost window cell is complete
+                    if (h == 0) out[e] = make_float4(p.x, p.y, p.z, 0.f);
+                    const float tx = __shfl_down_sync(0xffffffffu, p.x, 16);
+                    const float ty = __shfl_down_sync(0xffffffffu, p.y, 16);
+                    const float tz = __shfl_down_sync(0xffffffffu, p.z, 16);
+                    p = q;
+                    q.x = h ? 0.f : tx; q.y = h ? 0.f : ty; q.z = h ? 0.f : tz;
+                } while (++e < em);
+            }
+            const float vx = v.x * wz, vy = v.y * wz, vz = v.z * wz;
+            p.x = fmaf(w.x, vx, p.x); p.y = fmaf(w.x, vy, p.y); p.z = fmaf(w.x, vz, p.z);
+            q.x = fmaf(w.y, vx, q.x); q.y = fmaf(w.y, vy, q.y); q.z = fmaf(w.y, vz, q.z);
+        };
+        // full batches of RB markers: all loads of a batch are issued (at immediate offsets from three
+        // running pointers) before the first marker is accumulated, so the memory latency is paid once
+        // per batch, not once per marker; then the remaining markers one by one
         constexpr int RB = 4;
-        int cxw = __float_as_int(val[i0].w);
-        for (int ib = i0; ib < i1; ib += RB) {
-            float4 bv[RB], bw[RB];
+        int left = i1 - i0;
+        for (; left >= RB; left -= RB, pv += RB, pw += 2 * RB, pz += 16 * RB) {
+            float4 bv[RB];
+            float2 bw[RB];
             float bz[RB];
 #pragma unroll
-            for (int j = 0; j < RB; ++j) {
-                const int i = min(ib + j, i1 - 1);
-                bv[j] = val[i];
-                bw[j] = wx4[i];
-                bz[j] = wyz16[(size_t)i * 16 + l];
-            }
+            for (int j = 0; j < RB; ++j) { bv[j] = pv[j]; bw[j] = pw[2 * j]; bz[j] = pz[16 * j]; }
 #pragma unroll
-            for (int j = 0; j < RB; ++j) {
-                if (ib + j < i1) {
-                    const float4 v = bv[j], w = bw[j];
-                    const int cx = __float_as_int(v.w);
-                    if (cx != cxw) {
-                        // the window moves right by 1..3 cells: its leftmost cells are complete
-                        const int sh = cx - cxw;
-                        out[0] = make_float4(a0.x, a0.y, a0.z, 0.f);
-                        if (sh > 1) out[16] = make_float4(a1.x, a1.y, a1.z, 0.f);
-                        if (sh > 2) out[32] = make_float4(a2.x, a2.y, a2.z, 0.f);
-                        const Acc3 zero{0.f, 0.f, 0.f};
-                        const Acc3 b0 = sh == 1 ? a1 : (sh == 2 ? a2 : a3);
-                        const Acc3 b1 = sh == 1 ? a2 : (sh == 2 ? a3 : zero);
-                        const Acc3 b2 = sh == 1 ? a3 : zero;
-                        a0 = b0; a1 = b1; a2 = b2; a3 = zero;
-                        out += 16 * sh;
-                        cxw = cx;
-                    }
-                    const float vx = v.x * bz[j], vy = v.y * bz[j], vz = v.z * bz[j];
-                    a0.x = fmaf(w.x, vx, a0.x); a0.y = fmaf(w.x, vy, a0.y); a0.z = fmaf(w.x, vz, a0.z);
-                    a1.x = fmaf(w.y, vx, a1.x); a1.y = fmaf(w.y, vy, a1.y); a1.z = fmaf(w.y, vz, a1.z);
-                    a2.x = fmaf(w.z, vx, a2.x); a2.y = fmaf(w.z, vy, a2.y); a2.z = fmaf(w.z, vz, a2.z);
-                    a3.x = fmaf(w.w, vx, a3.x); a3.y = fmaf(w.w, vy, a3.y); a3.z = fmaf(w.w, vz, a3.z);
-                }
-            }
+            for (int j = 0; j < RB; ++j) add_marker(bv[j], bw[j], bz[j]);
         }
-        out[0] = make_float4(a0.x, a0.y, a0.z, 0.f);
-        out[16] = make_float4(a1.x, a1.y, a1.z, 0.f);
-        out[32] = make_float4(a2.x, a2.y, a2.z, 0.f);
-        out[48] = make_float4(a3.x, a3.y, a3.z, 0.f);
+#pragma unroll 1
+        for (; left > 0; --left, ++pv, pw += 2, pz += 16) add_marker(*pv, *pw, *pz);
+        // the last window: entries e .. e+3 (= hi)
+        out[e + 2 * h] = make_float4(p.x, p.y, p.z, 0.f);
+        out[e + 2 * h + 1] = make_float4(q.x, q.y, q.z, 0.f);
     }
 }
 
-// Stage B: one thread per active cell: add the profiles of the source rows (y+1-jy, z+1-jz) at this
-// x, jy and jz ascending (fixed order).
+// Stage B: one thread per active cell X of target row (y, z): for the source rows (y+1-jy, z+1-jz),
+// jy and jz ascending, add the profile entry of X from the chunk of the block that holds cx = X-2
+// and then from the chunk of the block that holds cx = X+1 (if it is another block).  Fixed order.
 //   LAST = false:  U^{m+1}(X) = U^m(X) + sum   (R8)      LAST = true:  G(X) = sum
-template <bool LAST>
+template <bool NARROW>
+__device__ __forceinline__ void collect_one(const float4 *__restrict__ T, int packed, int l, int ent, int e, int nx,
+                                            float &sx, float &sy, float &sz)
+{
+    if (packed < 0) return;
+    const int lo = (packed >> 23) & 15, hi = (packed >> 27) & 15;
+    const float4 *__restrict__ row = T + ((size_t)(packed & CHUNK_ID_MAX) * 16 + l) * ent;
+    if ((unsigned)(e - lo) <= (unsigned)(hi - lo)) { const float4 t = row[e]; sx += t.x; sy += t.y; sz += t.z; }
+    if (NARROW) {
+        // a lattice narrower than the window: the same cell can appear once more, one period away
+        if (e + nx <= hi) { const float4 t = row[e + nx]; sx += t.x; sy += t.y; sz += t.z; }
+        if (e - nx >= lo) { const float4 t = row[e - nx]; sx += t.x; sy += t.y; sz += t.z; }
+    }
+}
+
+// NARROW: nx < CHUNK_ENT_MAX (a window can wrap onto itself); only tiny test lattices need it.
+template <bool LAST, bool NARROW>
 __global__ void __launch_bounds__(256)
-k_spread_collect(Geom g, const int *__restrict__ tslot, const float4 *__restrict__ T,
+k_collect_chunks(Geom g, ChunkGeom cg, const int *__restrict__ chunk_of, const float4 *__restrict__ T,
                  const int *__restrict__ cells, const int *__restrict__ n_cells, float4 *__restrict__ field)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     const int stride = gridDim.x * blockDim.x;
     const int nc = *n_cells;
-    const int pitch = tslot_pitch(g);
     for (int k = tid; k < nc; k += stride) {
         const int cell = __ldg(cells + k);
         const int row = cell / g.nx;
         const int x = cell - row * g.nx;
         const int z = row / g.ny, y = row - z * g.ny;
-        // ghost columns of a periodic x axis: X = x + nx (for x <= 1) and X = -1 (for x = nx-1)
-        const int ghost = g.wallx ? -1 : (x <= 1 ? x + g.nx + 1 : (x == g.nx - 1 ? 0 : -1));
-        float sx = 0.f, sy = 0.f, sz = 0.f;
+        // blocks that can hold markers reaching X: the one of cx = X-2 and the one of cx = X+1
+        int xa = x - 2, xb = x + 1;
+        if (g.wallx) { xa = max(xa, 0); xb = min(xb, g.nx - 1); }
+        else { xa = wrap(xa, g.nx); xb = wrap(xb, g.nx); }
+        const int ja = chunk_block(xa, cg.nbx), jb = chunk_block(xb, cg.nbx);
+        // entry of X in the window of block j: X - (8 j - 1), taken modulo nx on a periodic axis
+        int ea = x - ja * CHUNK_W + 1, eb = x - jb * CHUNK_W + 1;
+        if (!g.wallx) {
+            if (ea < 0) ea += g.nx;
+            if (eb < 0) eb += g.nx; else if (eb >= g.nx) eb -= g.nx;
+        }
+        // source rows (y+1-jy, z+1-jz): offsets into chunk_of, -1 behind a wall
+        int ry[4], rz[4];
 #pragma unroll
-        for (int jy = 0; jy < 4; ++jy) {
-            int cy = y + 1 - jy;
-            if (g.wally) { if (cy < 0 || cy >= g.ny) continue; } else cy = wrap(cy, g.ny);
+        for (int j = 0; j < 4; ++j) {
+            int cy = y + 1 - j, cz = z + 1 - j;
+            if (g.wally) { if (cy < 0 || cy >= g.ny) cy = -1; } else cy = wrap(cy, g.ny);
+            if (g.wallz) { if (cz < 0 || cz >= g.nz) cz = -1; } else cz = wrap(cz, g.nz);
+            ry[j] = cy; rz[j] = cz;
+        }
+        // all chunk look-ups first (independent loads), then the profile entries
+        int pa[16], pb[16];
+#pragma unroll
+        for (int jy = 0; jy < 4; ++jy)
 #pragma unroll
             for (int jz = 0; jz < 4; ++jz) {
-                int cz = z + 1 - jz;
-                if (g.wallz) { if (cz < 0 || cz >= g.nz) continue; } else cz = wrap(cz, g.nz);
-                const int *trow = tslot + (size_t)(cz * g.ny + cy) * pitch;
-                const int e = __ldg(trow + x + 1);
-                if (e >= 0) {
-                    const float4 t = T[(size_t)e * 16 + (jy * 4 + jz)];
-                    sx += t.x; sy += t.y; sz += t.z;
-                }
-                if (ghost >= 0) {
-                    const int e2 = __ldg(trow + ghost);
-                    if (e2 >= 0) {
-                        const float4 t = T[(size_t)e2 * 16 + (jy * 4 + jz)];
-                        sx += t.x; sy += t.y; sz += t.z;
-                    }
+                const int lidx = jy * 4 + jz;
+                pa[lidx] = -1; pb[lidx] = -1;
+                if (ry[jy] >= 0 && rz[jz] >= 0) {
+                    const int *__restrict__ crow = chunk_of + (size_t)(rz[jz] * g.ny + ry[jy]) * cg.nbx;
+                    pa[lidx] = __ldg(crow + ja);
+                    if (jb != ja) pb[lidx] = __ldg(crow + jb);
                 }
             }
+        float sx = 0.f, sy = 0.f, sz = 0.f;
+#pragma unroll
+        for (int lidx = 0; lidx < 16; ++lidx) {
+            collect_one<NARROW>(T, pa[lidx], lidx, cg.ent, ea, g.nx, sx, sy, sz);
+            collect_one<NARROW>(T, pb[lidx], lidx, cg.ent, eb, g.nx, sx, sy, sz);
         }
         if (LAST) {
             field[cell] = make_float4(sx, sy, sz, 0.f);

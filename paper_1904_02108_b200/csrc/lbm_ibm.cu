@@ -57,8 +57,8 @@ struct SetScalars {
     int n_prev;          // sorted markers whose bins are still registered in bin_first
     // ---- zeroed at the start of every preparation (k_kinematics), after k_clear_prev has used them
     int n_words;         // active words
-    int n_runs;          // runs
-    int t_count;         // T entries handed out
+    int n_chunks;        // chunks (may exceed the capacity: the excess is dropped and flagged)
+    int n_entries;       // profile entries (window cells) over all chunks
     int n_cells;         // active cells
     int cursor[MAX_MDF]; // work cursors of the run sweeps, one per MDF iteration
 };
@@ -107,13 +107,13 @@ struct PrepSet {
     unsigned *keys[2] = {nullptr, nullptr};   // radix ping-pong; the sorted keys end in keys[sort_passes & 1]
     int *vals[2] = {nullptr, nullptr};        // the permutation, same ping-pong
     MarkerSorted ms{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    RunTable rt{nullptr, nullptr, nullptr, nullptr, nullptr};
+    ChunkTable ct{nullptr, nullptr, nullptr};
     unsigned *headbits = nullptr;             // one bit per sorted marker: starts a run
     int *cells = nullptr;                     // active-cell list
     // dense maps, cleared incrementally by the set's next preparation (k_clear_prev)
     unsigned *amask = nullptr;                // active-cell bitmask, 32 consecutive x per word
     int *words = nullptr;                     // list of non-zero mask words
-    int *tslot = nullptr;                     // [row][X+1] -> T entry (pitch nx+3)
+    int *chunk_of = nullptr;                  // [row][x block] -> packed (chunk id, lo, hi) or -1
     int *bin_first = nullptr;                 // cell -> first sorted marker (comparison spreads only; lazy)
     SetScalars *scal = nullptr;
     bool dirty = false;                       // the dense maps hold entries of a preparation
@@ -156,8 +156,10 @@ struct lbm {
     BodyStep *d_tabs = nullptr;
     int *d_hist = nullptr, *d_total = nullptr;
     size_t cells_cap = 0, headbits_cap = 0;
-    float4 *T = nullptr;                // run profiles, 16 float4 per entry
-    size_t t_cap = 0, tslot_count = 0;
+    float4 *T = nullptr;                // chunk profiles [chunk][16][cg.ent]
+    ChunkGeom cg{1, CHUNK_W + 3};
+    int chunk_cap = 0;                  // chunks T has room for
+    size_t chunk_slots = 0;             // entries of chunk_of
     int rows_grid = 148;                // persistent grid of the run sweep (blocks resident at once)
     int words_grid = 148, moments_grid = 148;   // same for the active-word stream-collide and the moments kernel
     int sort_ipw = 64, sort_tiles = 0, sort_passes = 1;
@@ -207,8 +209,8 @@ void free_set(lbm *h, PrepSet &S)
     for (int a = 0; a < 2; ++a) { dfree(h, S.keys[a], c); dfree(h, S.vals[a], c); }
     dfree(h, S.ms.fs, c); dfree(h, S.ms.wx, c); dfree(h, S.ms.wyz, 16 * c); dfree(h, S.ms.uk, c);
     dfree(h, S.ms.sg, c); dfree(h, S.ms.du, c);
-    dfree(h, S.rt.first, c); dfree(h, S.rt.end, c); dfree(h, S.rt.base, c); dfree(h, S.rt.slot0, c);
-    dfree(h, S.rt.nent, c);
+    dfree(h, S.ct.first, (size_t)h->chunk_cap); dfree(h, S.ct.end, (size_t)h->chunk_cap);
+    dfree(h, S.ct.slot, (size_t)h->chunk_cap);
     dfree(h, S.cells, h->cells_cap);
     dfree(h, S.headbits, h->headbits_cap);
     S.step = -1;
@@ -222,7 +224,7 @@ void free_markers_dev(lbm *h)
     dfree(h, h->d_body, c);
     for (PrepSet &S : h->set) free_set(h, S);
     h->cells_cap = 0; h->headbits_cap = 0;
-    dfree(h, h->T, h->t_cap * 16); h->t_cap = 0;
+    dfree(h, h->T, (size_t)h->chunk_cap * 16 * (size_t)h->cg.ent); h->chunk_cap = 0;
     dfree(h, h->d_hist, (size_t)RADIX * (size_t)h->sort_tiles);
     dfree(h, h->d_total, (size_t)RADIX);
     dfree(h, h->d_defs, (size_t)h->nb_cap);
@@ -257,7 +259,8 @@ int flush_set(lbm *h, PrepSet &S)
     S.step = -1;
     if (!S.dirty) return LBM_OK;
     k_clear_prev<<<LIST_GRID, 256, 0, h->stream>>>(sorted_keys(h, S), &S.scal->n_prev, S.bin_first, S.amask, S.words,
-                                                    &S.scal->n_words, S.tslot, S.rt.slot0, S.rt.nent, &S.scal->n_runs);
+                                                    &S.scal->n_words, S.chunk_of, S.ct.slot, &S.scal->n_chunks,
+                                                    h->chunk_cap);
     CK(cudaMemsetAsync(S.scal, 0, sizeof(SetScalars), h->stream));
     CK(cudaGetLastError());
     h->launches += 1;
@@ -295,6 +298,11 @@ int upload_markers(lbm *h)
         }
         if ((rc = dmalloc(h, &h->d_s, c))) return rc;
         if ((rc = dmalloc(h, &h->d_body, c))) return rc;
+        // T has room for every chunk that can exist (one per marker, one per (row, block) slot, CHUNK_ID_MAX)
+        // up to 8 GB; beyond that the capacity is capped and an overflow is flagged on the device
+        size_t ccap = std::min(std::min(c, h->chunk_slots), (size_t)CHUNK_ID_MAX);
+        const size_t chunk_bytes = (size_t)16 * (size_t)h->cg.ent * sizeof(float4);
+        ccap = std::max((size_t)1, std::min(ccap, ((size_t)8 << 30) / chunk_bytes));
         h->cells_cap = std::min((size_t)64 * c, (size_t)h->g.cells);
         h->headbits_cap = c / 32 + 16;
         for (PrepSet &S : h->set) {
@@ -308,16 +316,14 @@ int upload_markers(lbm *h)
             if ((rc = dmalloc(h, &S.ms.uk, c))) return rc;
             if ((rc = dmalloc(h, &S.ms.sg, c))) return rc;
             if ((rc = dmalloc(h, &S.ms.du, c))) return rc;
-            if ((rc = dmalloc(h, &S.rt.first, c))) return rc;
-            if ((rc = dmalloc(h, &S.rt.end, c))) return rc;
-            if ((rc = dmalloc(h, &S.rt.base, c))) return rc;
-            if ((rc = dmalloc(h, &S.rt.slot0, c))) return rc;
-            if ((rc = dmalloc(h, &S.rt.nent, c))) return rc;
+            if ((rc = dmalloc(h, &S.ct.first, (size_t)ccap))) return rc;
+            if ((rc = dmalloc(h, &S.ct.end, (size_t)ccap))) return rc;
+            if ((rc = dmalloc(h, &S.ct.slot, (size_t)ccap))) return rc;
             if ((rc = dmalloc(h, &S.cells, h->cells_cap))) return rc;
             if ((rc = dmalloc(h, &S.headbits, h->headbits_cap))) return rc;
         }
-        h->t_cap = std::min((size_t)4 * c, h->tslot_count);
-        if ((rc = dmalloc(h, &h->T, h->t_cap * 16))) return rc;
+        if ((rc = dmalloc(h, &h->T, ccap * 16 * (size_t)h->cg.ent))) return rc;
+        h->chunk_cap = (int)ccap;
         if ((rc = dmalloc(h, &h->d_total, (size_t)RADIX))) return rc;
         if ((rc = dmalloc(h, &h->d_defs, (size_t)nb))) return rc;
         if ((rc = dmalloc(h, &h->d_tabs, (size_t)nb))) return rc;
@@ -388,8 +394,8 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
     int nk = 0;
 
     if (pt) pt->mark(PH_KEYS, s);
-    k_clear_prev<<<LIST_GRID, 256, 0, s>>>(skey, &sc->n_prev, S.bin_first, S.amask, S.words, &sc->n_words, S.tslot,
-                                           S.rt.slot0, S.rt.nent, &sc->n_runs);
+    k_clear_prev<<<LIST_GRID, 256, 0, s>>>(skey, &sc->n_prev, S.bin_first, S.amask, S.words, &sc->n_words, S.chunk_of,
+                                           S.ct.slot, &sc->n_chunks, h->chunk_cap);
     const int nb = (int)h->bodies.size();
     k_kinematics<<<(std::max(nb, N_STEP_COUNTERS) + 127) / 128, 128, 0, s>>>(h->d_defs, h->d_tabs, nb, &h->scal->step_ctr,
                                                                               step_offset, &sc->n_words, N_STEP_COUNTERS);
@@ -412,9 +418,11 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
     k_marker_gather<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, perm, S.ms);
     ++nk;
     if (h->opt_spread == 0) {
-        k_run_heads<<<(n + 32 + 255) / 256, 256, 0, s>>>(skey, n, g, S.headbits);
-        k_runs<<<mb, 256, 0, s>>>(skey, n, g, S.headbits, S.rt, &sc->n_runs, &sc->t_count);
-        k_run_publish<<<LIST_GRID, 256, 0, s>>>(g, S.rt, &sc->n_runs, S.tslot, S.amask, S.words, &sc->n_words);
+        k_chunk_heads<<<(n + 32 + 255) / 256, 256, 0, s>>>(skey, n, g, h->cg, S.headbits);
+        k_chunks<<<mb, 256, 0, s>>>(skey, n, g, h->cg, S.headbits, S.ct, h->chunk_cap, &sc->n_chunks, &sc->n_entries,
+                                    S.chunk_of, &h->scal->status);
+        k_chunk_publish<<<LIST_GRID, 256, 0, s>>>(g, h->cg, S.ct, &sc->n_chunks, h->chunk_cap, S.chunk_of, S.amask, S.words,
+                                                  &sc->n_words);
         nk += 3;
     } else {
         k_bins<<<mb, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask, S.words, &sc->n_words);
@@ -446,10 +454,13 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
         ++nk;
         if (pt) pt->mark(PH_SPREAD, s);
         if (h->opt_spread == 0) {
-            k_spread_rows<<<h->rows_grid, 256, 0, s>>>(S.rt, &sc->n_runs, &sc->cursor[m], S.ms.wx, S.ms.wyz,
-                                                       last ? S.ms.du : S.ms.sg, h->T);
-            if (last) k_spread_collect<true><<<LIST_GRID, 256, 0, s>>>(g, S.tslot, h->T, S.cells, &sc->n_cells, h->G);
-            else k_spread_collect<false><<<LIST_GRID, 256, 0, s>>>(g, S.tslot, h->T, S.cells, &sc->n_cells, h->U);
+            k_spread_chunks<<<h->rows_grid, 256, 0, s>>>(S.ct, &sc->n_chunks, h->chunk_cap, &sc->cursor[m], S.chunk_of, h->cg,
+                                                         reinterpret_cast<const float2 *>(S.ms.wx), S.ms.wyz,
+                                                         last ? S.ms.du : S.ms.sg, h->T);
+            const bool narrow = g.nx < CHUNK_ENT_MAX;
+            auto collect = last ? (narrow ? k_collect_chunks<true, true> : k_collect_chunks<true, false>)
+                                : (narrow ? k_collect_chunks<false, true> : k_collect_chunks<false, false>);
+            collect<<<LIST_GRID, 256, 0, s>>>(g, h->cg, S.chunk_of, h->T, S.cells, &sc->n_cells, last ? h->G : h->U);
             nk += 2;
         } else if (h->opt_spread == 2) {
             if (last)
@@ -717,14 +728,15 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
     if (dmalloc(h, &h->f[0], fcount) || dmalloc(h, &h->f[1], fcount)) return bail("populations");
     if (dmalloc(h, &h->U, cells) || dmalloc(h, &h->G, cells)) return bail("U/G fields");
     if (dmalloc(h, &h->scal, (size_t)1)) return bail("scalars");
-    h->tslot_count = (size_t)(nx + 3) * ny * nz;
+    h->cg = chunk_geom(nx);
+    h->chunk_slots = (size_t)h->cg.nbx * ny * nz;
     bool ok = true;
     for (PrepSet &S : h->set) {
         if (dmalloc(h, &S.amask, h->n_mask_words) || dmalloc(h, &S.words, h->n_mask_words)) return bail("active mask");
-        if (dmalloc(h, &S.tslot, h->tslot_count)) return bail("run slot map");
+        if (dmalloc(h, &S.chunk_of, h->chunk_slots)) return bail("chunk map");
         if (dmalloc(h, &S.scal, (size_t)1)) return bail("set scalars");
         ok &= cudaMemset(S.amask, 0, h->n_mask_words * sizeof(unsigned)) == cudaSuccess;
-        ok &= cudaMemset(S.tslot, 0xff, h->tslot_count * sizeof(int)) == cudaSuccess;
+        ok &= cudaMemset(S.chunk_of, 0xff, h->chunk_slots * sizeof(int)) == cudaSuccess;
         ok &= cudaMemset(S.scal, 0, sizeof(SetScalars)) == cudaSuccess;
     }
     ok &= cudaMemset(h->f[0], 0, fcount * sizeof(float)) == cudaSuccess;   // rest state: f_i - t_i = 0
@@ -735,7 +747,7 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
     {
         int per_sm = 0, sms = 148;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spread_rows, 256, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spread_chunks, 256, 0);
         h->rows_grid = std::max(1, per_sm) * sms;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_stream_collide_words, 256, 0);
         h->words_grid = std::max(1, per_sm) * sms;
@@ -754,7 +766,7 @@ void lbm_destroy(lbm_t *h)
     free_markers_dev(h);
     cudaFree(h->f[0]); cudaFree(h->f[1]); cudaFree(h->U); cudaFree(h->G); cudaFree(h->scal);
     for (PrepSet &S : h->set) {
-        cudaFree(S.amask); cudaFree(S.words); cudaFree(S.tslot); cudaFree(S.bin_first); cudaFree(S.scal);
+        cudaFree(S.amask); cudaFree(S.words); cudaFree(S.chunk_of); cudaFree(S.bin_first); cudaFree(S.scal);
     }
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     if (h->cap_bulk) cudaStreamDestroy(h->cap_bulk);
@@ -802,7 +814,7 @@ int lbm_get_info(lbm_t *h, int key, long long *value)
             int r = 0;
             if (h->force_valid && h->last_set >= 0) {
                 const SetScalars *sc = h->set[h->last_set].scal;
-                const int *p = key == LBM_INFO_ACTIVE_CELLS ? &sc->n_cells : (key == LBM_INFO_RUNS ? &sc->n_runs : &sc->t_count);
+                const int *p = key == LBM_INFO_ACTIVE_CELLS ? &sc->n_cells : (key == LBM_INFO_RUNS ? &sc->n_chunks : &sc->n_entries);
                 CK(cudaMemcpyAsync(&r, p, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
                 CK(cudaStreamSynchronize(h->stream));
             }
