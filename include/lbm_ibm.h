@@ -85,8 +85,9 @@ enum {
     LBM_INFO_ACTIVE_CELLS = 5,  /* cells inside at least one marker's stencil in the last step    */
     LBM_INFO_DEVICE_BYTES = 6,  /* device memory owned by the handle                              */
     LBM_INFO_STATUS = 7,        /* device-side status word of the last step (0 = OK)              */
-    LBM_INFO_RUNS = 8,          /* marker runs (x-chained stencils of one row) in the last step   */
-    LBM_INFO_RUN_ENTRIES = 9,   /* run-profile entries written per spreading pass in the last step */
+    LBM_INFO_RUNS = 8,          /* marker chunks (markers of one row and one 8-cell x block) in the last step */
+    LBM_INFO_RUN_ENTRIES = 9,   /* window cells (profile entries) over all chunks in the last step  */
+    LBM_INFO_TILES = 10,        /* tiles (chunks of one x block and one 4x4 block of rows) in the last step */
     LBM_INFO_PHASE_NS = 100     /* + phase: accumulated device time in ns under LBM_OPT_TIMING.
                                    phases: 0 kinematics+keys, 1 sort, 2 gather+bins, 3 moments on
                                    active cells, 4 interpolation+correction, 5 spreading,

@@ -239,7 +239,9 @@ k_bins(const unsigned *__restrict__ skey, int n, Geom g, int *__restrict__ bin_f
 __global__ void __launch_bounds__(256)
 k_clear_prev(const unsigned *__restrict__ skey_prev, const int *__restrict__ n_prev, int *__restrict__ bin_first,
              unsigned *__restrict__ amask, const int *__restrict__ words, const int *__restrict__ n_words,
-             int *__restrict__ chunk_of, const int *__restrict__ chunk_slot, const int *__restrict__ n_chunks, int cap)
+             int *__restrict__ chunk_of, const int *__restrict__ chunk_slot, const int *__restrict__ n_chunks, int cap,
+             unsigned *__restrict__ tile_mask, const int *__restrict__ tile_slot, const int *__restrict__ n_tiles,
+             int tile_cap)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     const int stride = gridDim.x * blockDim.x;
@@ -247,6 +249,8 @@ k_clear_prev(const unsigned *__restrict__ skey_prev, const int *__restrict__ n_p
     if (bin_first) for (int i = tid; i < np; i += stride) bin_first[skey_prev[i]] = -1;
     for (int i = tid; i < nw; i += stride) amask[words[i]] = 0u;
     for (int c = tid; c < nc; c += stride) chunk_of[chunk_slot[c]] = -1;
+    const int nt = min(*n_tiles, tile_cap);
+    for (int c = tid; c < nt; c += stride) tile_mask[tile_slot[c]] = 0u;
 }
 
 // device scalars: mode bit 0: step_ctr = step; bit 1: n_prev = n_prev_val; bit 2: step_ctr += 1
@@ -578,100 +582,318 @@ k_active_cells(Geom g, const unsigned *__restrict__ amask, const int *__restrict
     }
 }
 
-// Stage A: one warp per chunk.  Lane = h*16 + l: l = jy*4 + jz is the target-row offset whose
-// profile the lane accumulates, h the half of the 4-cell x window it owns (h = 0: the two left
-// cells, h = 1: the two right cells), both in registers.  When the sweep moves on to the next cell
-// the leftmost window cell is final: it is written to T and the window shifts by one (the cell that
-// crosses from the right half to the left half travels by shuffle).  Control flow is uniform across
-// the warp; chunks are handed out through an atomic cursor.
 struct Acc3 { float x, y, z; };
 
-__global__ void __launch_bounds__(256)
-k_spread_chunks(ChunkTable ct, const int *__restrict__ n_chunks, int cap, int *__restrict__ cursor,
-                const int *__restrict__ chunk_of, ChunkGeom cg, const float2 *__restrict__ wx2,
-                const float *__restrict__ wyz16, const float4 *__restrict__ val, float4 *__restrict__ T)
+// ---- tiles ---------------------------------------------------------------------------------------
+// A "tile" groups the chunks of one x block whose source rows lie in one aligned 4 x 4 block of
+// (y, z): up to 16 chunks.  Their 16 x 16 profiles overlap on a footprint of 7 x 7 target rows, so
+// one thread block sweeps the chunks of a tile into shared memory, adds the profiles that fall on
+// the same target row there (fixed order) and writes ONE footprint  F[tile][fy][fz][e]  (fy, fz =
+// 0..6 <-> target row 4 ty - 1 + fy, 4 tz - 1 + fz; e as in the chunk window).  Stage B then reads
+// about 4 footprints per cell instead of 22 profiles, and the profile traffic shrinks ~7x.
+//
+// tile_mask[tile slot] = x entries (bits 0..13) | y rows (bits 14..20) | z rows (bits 21..27) that
+// some chunk of the tile reaches; a footprint element is valid iff its three bits are set (a
+// superset of the cells actually reached; the rest is written as zeros).
+constexpr int TILE_R = 4;                  // source rows per tile in y and in z
+constexpr int TILE_F = TILE_R + 3;         // footprint rows per tile in y and in z
+
+struct TileGeom {
+    int nty, ntz;        // tiles in y and z
+};
+inline TileGeom tile_geom(int ny, int nz)
 {
-    const int lane = threadIdx.x & 31;
-    const int l = lane & 15, h = lane >> 4;
+    TileGeom t;
+    t.nty = (ny + TILE_R - 1) / TILE_R;
+    t.ntz = (nz + TILE_R - 1) / TILE_R;
+    return t;
+}
+
+struct TileTable {
+    unsigned *mask;      // [tile slots] dense, 0 = no tile
+    int *id;             // [tile slots] dense: footprint index of the tile (valid where mask != 0)
+    int *slot;           // [tile ids] -> tile slot
+    int2 *rec;           // [tile ids][16]: sorted-marker range [first, end) of the chunk in source row sy + 4 sz, (0,0) = none
+};
+
+__device__ __forceinline__ int tile_slot_of(int blk, int ty, int tz, const ChunkGeom &cg, const TileGeom &tg)
+{
+    return (tz * tg.nty + ty) * cg.nbx + blk;
+}
+
+// a3: register every chunk in its tile (bits it reaches); the chunk that finds the mask empty
+// allocates the tile's footprint index.  One thread per chunk.
+__global__ void __launch_bounds__(256)
+k_tiles(Geom g, ChunkGeom cg, TileGeom tg, ChunkTable ct, const int *__restrict__ n_chunks, int cap,
+        const int *__restrict__ chunk_of, TileTable tt, int tile_cap, int *__restrict__ n_tiles, int *__restrict__ status)
+{
     const int nc = min(*n_chunks, cap);
-    for (;;) {
-        int c = 0;
-        if (lane == 0) c = atomicAdd(cursor, 1);
-        c = __shfl_sync(0xffffffffu, c, 0);
-        if (c >= nc) break;
-        const int i0 = ct.first[c], i1 = ct.end[c];
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
         const int slot = ct.slot[c];
-        const int blk = slot % cg.nbx;
-        const int x0 = blk * CHUNK_W;                       // entry e <-> cell X = x0 - 1 + e
-        float4 *out = T + ((size_t)c * 16 + l) * cg.ent;    // profile row of this lane
-        Acc3 p{0.f, 0.f, 0.f}, q{0.f, 0.f, 0.f};            // window cells (e + 2h, e + 2h + 1)
-        const float4 *__restrict__ pv = val + i0;
-        const float2 *__restrict__ pw = wx2 + 2 * (size_t)i0 + h;
-        const float *__restrict__ pz = wyz16 + 16 * (size_t)i0 + l;
-        int e = __float_as_int(pv->w) - x0;                 // window start = entry of the first marker's cx - 1
-        auto add_marker = [&](const float4 v, const float2 w, const float wz) {
-            const int em = __float_as_int(v.w) - x0;
-            if (em != e) {                                  // warp-uniform: the sweep moves on to another cell
-#pragma unroll 1
-                do {                                        // the leftmost window cell is complete
-                    if (h == 0) out[e] = make_float4(p.x, p.y, p.z, 0.f);
-                    const float tx = __shfl_down_sync(0xffffffffu, p.x, 16);
-                    const float ty = __shfl_down_sync(0xffffffffu, p.y, 16);
-                    const float tz = __shfl_down_sync(0xffffffffu, p.z, 16);
-                    p = q;
-                    q.x = h ? 0.f : tx; q.y = h ? 0.f : ty; q.z = h ? 0.f : tz;
-                } while (++e < em);
-            }
-            const float vx = v.x * wz, vy = v.y * wz, vz = v.z * wz;
-            p.x = fmaf(w.x, vx, p.x); p.y = fmaf(w.x, vy, p.y); p.z = fmaf(w.x, vz, p.z);
-            q.x = fmaf(w.y, vx, q.x); q.y = fmaf(w.y, vy, q.y); q.z = fmaf(w.y, vz, q.z);
-        };
-        // full batches of RB markers: all loads of a batch are issued (at immediate offsets from three
-        // running pointers) before the first marker is accumulated, so the memory latency is paid once
-        // per batch, not once per marker; then the remaining markers one by one
-        constexpr int RB = 4;
-        int left = i1 - i0;
-        for (; left >= RB; left -= RB, pv += RB, pw += 2 * RB, pz += 16 * RB) {
-            float4 bv[RB];
-            float2 bw[RB];
-            float bz[RB];
+        const int packed = chunk_of[slot];
+        const int lo = (packed >> 23) & 15, hi = (packed >> 27) & 15;
+        const int row = slot / cg.nbx;
+        const int blk = slot - row * cg.nbx;
+        const int cz = row / g.ny, cy = row - cz * g.ny;
+        const unsigned xbits = ((1u << (hi - lo + 1)) - 1u) << lo;
+        const unsigned ybits = 0xFu << (cy & (TILE_R - 1)), zbits = 0xFu << (cz & (TILE_R - 1));
+        const int ts = tile_slot_of(blk, cy / TILE_R, cz / TILE_R, cg, tg);
+        const unsigned old = atomicOr(tt.mask + ts, xbits | (ybits << 14) | (zbits << 21));
+        if (old == 0u) {
+            const int id = atomicAdd(n_tiles, 1);
+            if (id < tile_cap) {
+                tt.slot[id] = ts; tt.id[ts] = id;
+                int4 *z = reinterpret_cast<int4 *>(tt.rec + (size_t)id * 16);
 #pragma unroll
-            for (int j = 0; j < RB; ++j) { bv[j] = pv[j]; bw[j] = pw[2 * j]; bz[j] = pz[16 * j]; }
-#pragma unroll
-            for (int j = 0; j < RB; ++j) add_marker(bv[j], bw[j], bz[j]);
+                for (int i = 0; i < 8; ++i) z[i] = make_int4(0, 0, 0, 0);
+            } else { tt.id[ts] = -1; atomicOr(status, 2); }
         }
-#pragma unroll 1
-        for (; left > 0; --left, ++pv, pw += 2, pz += 16) add_marker(*pv, *pw, *pz);
-        // the last window: entries e .. e+3 (= hi)
-        out[e + 2 * h] = make_float4(p.x, p.y, p.z, 0.f);
-        out[e + 2 * h + 1] = make_float4(q.x, q.y, q.z, 0.f);
     }
 }
 
-// Stage B: one thread per active cell X of target row (y, z): for the source rows (y+1-jy, z+1-jz),
-// jy and jz ascending, add the profile entry of X from the chunk of the block that holds cx = X-2
-// and then from the chunk of the block that holds cx = X+1 (if it is another block).  Fixed order.
-//   LAST = false:  U^{m+1}(X) = U^m(X) + sum   (P:98, P:108, R8)      LAST = true:  G(X) = sum  (P:114)
-template <bool NARROW>
-__device__ __forceinline__ void collect_one(const float4 *__restrict__ T, int packed, int l, int ent, int e, int nx,
-                                            float &sx, float &sy, float &sz)
-{
-    if (packed < 0) return;
-    const int lo = (packed >> 23) & 15, hi = (packed >> 27) & 15;
-    const float4 *__restrict__ row = T + ((size_t)(packed & CHUNK_ID_MAX) * 16 + l) * ent;
-    if ((unsigned)(e - lo) <= (unsigned)(hi - lo)) { const float4 t = row[e]; sx += t.x; sy += t.y; sz += t.z; }
-    if (NARROW) {
-        // a lattice narrower than the window: the same cell can appear once more, one period away
-        if (e + nx <= hi) { const float4 t = row[e + nx]; sx += t.x; sy += t.y; sz += t.z; }
-        if (e - nx >= lo) { const float4 t = row[e - nx]; sx += t.x; sy += t.y; sz += t.z; }
-    }
-}
-
-// NARROW: nx < CHUNK_ENT_MAX (a window can wrap onto itself); only tiny test lattices need it.
-template <bool LAST, bool NARROW>
+// a3: every chunk writes its marker range into the record of its tile (after k_tiles has handed out the ids).
 __global__ void __launch_bounds__(256)
-k_collect_chunks(Geom g, ChunkGeom cg, const int *__restrict__ chunk_of, const float4 *__restrict__ T,
-                 const int *__restrict__ cells, const int *__restrict__ n_cells, float4 *__restrict__ field)
+k_tile_fill(Geom g, ChunkGeom cg, TileGeom tg, ChunkTable ct, const int *__restrict__ n_chunks, int cap, TileTable tt)
+{
+    const int nc = min(*n_chunks, cap);
+    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
+        const int slot = ct.slot[c];
+        const int row = slot / cg.nbx;
+        const int blk = slot - row * cg.nbx;
+        const int cz = row / g.ny, cy = row - cz * g.ny;
+        const int id = tt.id[tile_slot_of(blk, cy / TILE_R, cz / TILE_R, cg, tg)];
+        if (id >= 0) tt.rec[(size_t)id * 16 + (cy & (TILE_R - 1)) + 4 * (cz & (TILE_R - 1))] = make_int2(ct.first[c], ct.end[c]);
+    }
+}
+
+// ---- asynchronous bulk copies global -> shared (TMA, 1-D) completing on an mbarrier ---------------
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+
+// Stage A: one thread block (8 warps) per tile.  The source rows of the tile that hold a chunk are
+// dealt to the warps.  A warp brings its chunk's marker data (value, x weights, y-z weights: three
+// contiguous ranges of the sorted arrays) into its own shared-memory buffers with asynchronous bulk
+// copies, SPREAD_PIECE markers at a time and double-buffered, so the sweep never waits on a global
+// load per marker.  It sweeps the chunk with lane = h*16 + l: l = jy*4 + jz is the target-row
+// offset whose profile the lane accumulates, h the half of the 4-cell x window it owns (h = 0: the
+// two left cells, h = 1: the two right cells), both in registers.  When the sweep moves on to the
+// next cell the leftmost window cell is final: it goes to the row's private profile in shared memory
+// and the window shifts by one (the cell that crosses from the right half to the left half travels
+// by shuffle).  Control flow is uniform across the warp.  After a barrier the block adds, for every
+// footprint element, the profiles of the source rows that reach it (sz, then sy ascending: fixed
+// order) and writes the footprint.  Tiles are handed out through an atomic cursor whose next value
+// is fetched one tile ahead.
+//
+// Shared memory (dynamic): prof[16 source rows][16 l][3 components][EP*4 entries] floats (EP =
+// ceil(ent/4)), so that the reduction reads four consecutive entries of one component with one
+// 128-bit load; then per warp 2 x { val[PIECE] float4, wx[PIECE] float4, wyz[PIECE][16] float }.
+// measured on B200 (W4, W3, W4lit): 8 warps, 4 blocks per SM, pieces of 16 markers beat 4/16 warps, 2-5 blocks and
+// pieces of 32 (more resident blocks hide the barrier between sweep and reduction)
+#ifndef TILE_WARPS_CFG
+#define TILE_WARPS_CFG 8
+#define TILE_MINB_CFG 4
+#define SPREAD_PIECE_CFG 16
+#endif
+constexpr int TILE_WARPS = TILE_WARPS_CFG;
+constexpr int SPREAD_PIECE = SPREAD_PIECE_CFG;
+constexpr int SPREAD_PIECE_BYTES = SPREAD_PIECE * 96;
+
+inline size_t spread_tiles_smem(const ChunkGeom &cg)
+{
+    return (size_t)16 * 16 * 3 * (size_t)((cg.ent + 3) / 4 * 4) * sizeof(float) + (size_t)TILE_WARPS * 2 * SPREAD_PIECE_BYTES;
+}
+
+__global__ void __launch_bounds__(TILE_WARPS * 32, TILE_MINB_CFG)
+k_spread_tiles(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int *__restrict__ tile_slot,
+               const unsigned *__restrict__ tile_mask, const int *__restrict__ n_tiles, int tile_cap,
+               int *__restrict__ cursor, const float4 *__restrict__ wx4, const float *__restrict__ wyz16,
+               const float4 *__restrict__ val, float4 *__restrict__ F)
+{
+    extern __shared__ __align__(128) float4 smem4[];
+    __shared__ unsigned long long s_bar[TILE_WARPS][2];
+    __shared__ int s_tile[2];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int l = lane & 15, h = lane >> 4;
+    const int nt = min(*n_tiles, tile_cap);
+    const int ent = cg.ent;
+    const int EP = (ent + 3) >> 2, E4 = EP * 4;          // entries per profile row in shared memory
+    const int rowf = 16 * 3 * E4;                        // floats per source row
+    float *prof = reinterpret_cast<float *>(smem4);
+    char *stage = reinterpret_cast<char *>(smem4) + (size_t)16 * rowf * sizeof(float) + (size_t)warp * 2 * SPREAD_PIECE_BYTES;
+    unsigned long long *bar = s_bar[warp];
+    if (lane == 0) { mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); }
+    unsigned phase = 0u;                                 // bit b: parity the next wait on bar[b] uses
+    // the footprint element group (fy, fz, 4 entries) this thread reduces, fixed for the whole kernel
+    const bool red = (int)threadIdx.x < TILE_F * TILE_F * EP;
+    const int r_e4 = threadIdx.x % EP, r_fyz = threadIdx.x / EP;
+    const int r_fz = r_fyz % TILE_F, r_fy = r_fyz / TILE_F;
+    if (threadIdx.x == 0) s_tile[0] = atomicAdd(cursor, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncthreads();
+    for (int it = 0;; ++it) {
+        const int t = s_tile[it & 1];
+        if (t >= nt) break;
+        if (threadIdx.x == 0) s_tile[(it + 1) & 1] = atomicAdd(cursor, 1);    // consumed after the next barrier pair
+        // lane r < 16: sorted-marker range of the chunk in source row r = sy + 4 sz ((0,0) = none)
+        const int2 rec = __ldg(tile_rec + (size_t)t * 16 + l);
+        const unsigned present = __ballot_sync(0xffffffffu, rec.y > rec.x) & 0xffffu;
+        const int x0 = (__ldg(tile_slot + t) % cg.nbx) * CHUNK_W;
+        // the present source rows, dealt round-robin to the warps
+        int taken = 0;
+        for (unsigned rest = present; rest; rest &= rest - 1, ++taken) {
+            if ((taken & (TILE_WARPS - 1)) != warp) continue;
+            const int r = __ffs(rest) - 1;
+            const int i0 = __shfl_sync(0xffffffffu, rec.x, r), i1 = __shfl_sync(0xffffffffu, rec.y, r);
+            const int npieces = (i1 - i0 + SPREAD_PIECE - 1) / SPREAD_PIECE;
+            auto issue = [&](int k) {                    // lane 0: bulk copies of piece k into buffer k & 1
+                const int b = k & 1;
+                const int j0 = i0 + k * SPREAD_PIECE;
+                const int n = min(SPREAD_PIECE, i1 - j0);
+                char *dst = stage + b * SPREAD_PIECE_BYTES;
+                mbar_expect_tx(&bar[b], (unsigned)n * 96u);
+                bulk_g2s(dst, val + j0, (unsigned)n * 16u, &bar[b]);
+                bulk_g2s(dst + SPREAD_PIECE * 16, wx4 + j0, (unsigned)n * 16u, &bar[b]);
+                bulk_g2s(dst + SPREAD_PIECE * 32, wyz16 + (size_t)j0 * 16, (unsigned)n * 64u, &bar[b]);
+            };
+            if (lane == 0) issue(0);
+            // zero the row's profiles (entries outside the chunk's window stay zero) while the copy is in flight
+            float4 *z4 = smem4 + (size_t)r * (rowf / 4);
+            for (int i = lane; i < rowf / 4; i += 32) z4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+            __syncwarp();
+            float *out = prof + (size_t)r * rowf + l * 3 * E4;   // out[c * E4 + e]
+            Acc3 p{0.f, 0.f, 0.f}, q{0.f, 0.f, 0.f};            // window cells (e + 2h, e + 2h + 1)
+            int e = -1000;
+            for (int k = 0; k < npieces; ++k) {
+                const int b = k & 1;
+                if (k + 1 < npieces && lane == 0) issue(k + 1);   // buffer (k+1)&1 was released by the __syncwarp below
+                mbar_wait(&bar[b], (phase >> b) & 1u);
+                phase ^= 1u << b;
+                const char *src = stage + b * SPREAD_PIECE_BYTES;
+                const float4 *sv = reinterpret_cast<const float4 *>(src);
+                const float2 *sw = reinterpret_cast<const float2 *>(src + SPREAD_PIECE * 16) + h;
+                const float *sz = reinterpret_cast<const float *>(src + SPREAD_PIECE * 32) + l;
+                const int n = min(SPREAD_PIECE, i1 - i0 - k * SPREAD_PIECE);
+                if (k == 0) e = __float_as_int(sv[0].w) - x0;   // window start = entry of the first marker's cx - 1
+#pragma unroll 4
+                for (int j = 0; j < n; ++j) {
+                    const float4 v = sv[j];
+                    const float2 w = sw[2 * j];
+                    const float wz = sz[16 * j];
+                    const int em = __float_as_int(v.w) - x0;
+                    if (em != e) {                              // warp-uniform: the sweep moves on to another cell
+#pragma unroll 1
+                        do {                                    // the leftmost window cell is complete
+                            if (h == 0) { out[e] = p.x; out[E4 + e] = p.y; out[2 * E4 + e] = p.z; }
+                            const float tx = __shfl_down_sync(0xffffffffu, p.x, 16);
+                            const float ty = __shfl_down_sync(0xffffffffu, p.y, 16);
+                            const float tz = __shfl_down_sync(0xffffffffu, p.z, 16);
+                            p = q;
+                            q.x = h ? 0.f : tx; q.y = h ? 0.f : ty; q.z = h ? 0.f : tz;
+                        } while (++e < em);
+                    }
+                    const float vx = v.x * wz, vy = v.y * wz, vz = v.z * wz;
+                    p.x = fmaf(w.x, vx, p.x); p.y = fmaf(w.x, vy, p.y); p.z = fmaf(w.x, vz, p.z);
+                    q.x = fmaf(w.y, vx, q.x); q.y = fmaf(w.y, vy, q.y); q.z = fmaf(w.y, vz, q.z);
+                }
+                __syncwarp();                                   // every lane is done with buffer b
+            }
+            // the last window: entries e .. e+3 (= hi)
+            const int ee = e + 2 * h;
+            out[ee] = p.x; out[E4 + ee] = p.y; out[2 * E4 + ee] = p.z;
+            out[ee + 1] = q.x; out[E4 + ee + 1] = q.y; out[2 * E4 + ee + 1] = q.z;
+        }
+        __syncthreads();
+        // footprint: element (fy, fz, e) <- sum over the present source rows (sy, sz) with 0 <= fy - sy <= 3,
+        // 0 <= fz - sz <= 3 of their profile l = (fy - sy) * 4 + (fz - sz); four entries per thread
+        if (red) {
+            const unsigned m = __ldg(tile_mask + __ldg(tile_slot + t));
+            if ((m >> (14 + r_fy)) & (m >> (21 + r_fz)) & 1u) {
+                float4 ax = make_float4(0.f, 0.f, 0.f, 0.f), ay = ax, az = ax;
+                for (int sz = max(0, r_fz - 3); sz <= min(3, r_fz); ++sz)
+                    for (int sy = max(0, r_fy - 3); sy <= min(3, r_fy); ++sy) {
+                        const int r = sy + 4 * sz;
+                        if (!((present >> r) & 1u)) continue;
+                        const float4 *v = smem4 + ((size_t)r * rowf + ((r_fy - sy) * 4 + (r_fz - sz)) * 3 * E4) / 4 + r_e4;
+                        const float4 vx = v[0], vy = v[EP], vz = v[2 * EP];
+                        ax.x += vx.x; ax.y += vx.y; ax.z += vx.z; ax.w += vx.w;
+                        ay.x += vy.x; ay.y += vy.y; ay.z += vy.z; ay.w += vy.w;
+                        az.x += vz.x; az.y += vz.y; az.z += vz.z; az.w += vz.w;
+                    }
+                float4 *__restrict__ Ft = F + ((size_t)t * (TILE_F * TILE_F) + r_fy * TILE_F + r_fz) * ent + 4 * r_e4;
+                const unsigned mx = m >> (4 * r_e4);
+                if (mx & 1u) Ft[0] = make_float4(ax.x, ay.x, az.x, 0.f);
+                if (mx & 2u) Ft[1] = make_float4(ax.y, ay.y, az.y, 0.f);
+                if (mx & 4u) Ft[2] = make_float4(ax.z, ay.z, az.z, 0.f);
+                if (mx & 8u) Ft[3] = make_float4(ax.w, ay.w, az.w, 0.f);
+            }
+        }
+        __syncthreads();   // the next tile must not overwrite prof before every thread has read it
+    }
+}
+
+// Stage B: one thread per active cell X of target row (y, z).  The markers that reach it sit in the
+// source cells (X+1-jx, y+1-jy, z+1-jz); per axis these four coordinates meet one or two tiles
+// (blocks in x), found here as the distinct (tile, footprint coordinate) pairs.  The cell adds the
+// footprint elements of every tile in that small product, in fixed order.
+//   LAST = false:  U^{m+1}(X) = U^m(X) + sum   (P:98, P:108, R8)      LAST = true:  G(X) = sum  (P:114)
+// MAXC = 2 covers every lattice with nx >= 14 (or an x wall) and ny, nz multiples of 4 (or walls);
+// MAXC = 4 is the general case (tiny or odd-sized periodic lattices, where a window can wrap onto
+// its own tile or meet a third, narrow tile).
+template <int MAXC>
+struct AxisCand { int t[MAXC], f[MAXC], n; };
+
+// candidates along one axis: source coordinate c = X + 1 - j (wrapped, or skipped outside a wall axis);
+// tile = c / tile width (blocks in x: chunk_block), footprint coordinate = offset of c in its tile + j
+template <bool IS_X, int MAXC>
+__device__ __forceinline__ void axis_candidates(int X, int n, int wall, int nbx, AxisCand<MAXC> &a)
+{
+    a.n = 0;
+    int pt = -1, pf = -1;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        int c = X + 1 - j;
+        if (wall) { if (c < 0 || c >= n) continue; } else c = wrap(c, n);
+        const int t = IS_X ? chunk_block(c, nbx) : c / TILE_R;
+        const int f = c - t * (IS_X ? CHUNK_W : TILE_R) + j;
+        if (t != pt || f != pf) {
+#pragma unroll
+            for (int i = 0; i < MAXC; ++i) if (i == a.n) { a.t[i] = t; a.f[i] = f; }
+            ++a.n; pt = t; pf = f;
+        }
+    }
+}
+
+template <bool LAST, int MAXC>
+__global__ void __launch_bounds__(256)
+k_collect_tiles(Geom g, ChunkGeom cg, TileGeom tg, TileTable tt, const float4 *__restrict__ F,
+                const int *__restrict__ cells, const int *__restrict__ n_cells, float4 *__restrict__ field)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     const int stride = gridDim.x * blockDim.x;
@@ -681,46 +903,26 @@ k_collect_chunks(Geom g, ChunkGeom cg, const int *__restrict__ chunk_of, const f
         const int row = cell / g.nx;
         const int x = cell - row * g.nx;
         const int z = row / g.ny, y = row - z * g.ny;
-        // blocks that can hold markers reaching X: the one of cx = X-2 and the one of cx = X+1
-        int xa = x - 2, xb = x + 1;
-        if (g.wallx) { xa = max(xa, 0); xb = min(xb, g.nx - 1); }
-        else { xa = wrap(xa, g.nx); xb = wrap(xb, g.nx); }
-        const int ja = chunk_block(xa, cg.nbx), jb = chunk_block(xb, cg.nbx);
-        // entry of X in the window of block j: X - (8 j - 1), taken modulo nx on a periodic axis
-        int ea = x - ja * CHUNK_W + 1, eb = x - jb * CHUNK_W + 1;
-        if (!g.wallx) {
-            if (ea < 0) ea += g.nx;
-            if (eb < 0) eb += g.nx; else if (eb >= g.nx) eb -= g.nx;
-        }
-        // source rows (y+1-jy, z+1-jz): offsets into chunk_of, -1 behind a wall
-        int ry[4], rz[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            int cy = y + 1 - j, cz = z + 1 - j;
-            if (g.wally) { if (cy < 0 || cy >= g.ny) cy = -1; } else cy = wrap(cy, g.ny);
-            if (g.wallz) { if (cz < 0 || cz >= g.nz) cz = -1; } else cz = wrap(cz, g.nz);
-            ry[j] = cy; rz[j] = cz;
-        }
-        // all chunk look-ups first (independent loads), then the profile entries
-        int pa[16], pb[16];
-#pragma unroll
-        for (int jy = 0; jy < 4; ++jy)
-#pragma unroll
-            for (int jz = 0; jz < 4; ++jz) {
-                const int lidx = jy * 4 + jz;
-                pa[lidx] = -1; pb[lidx] = -1;
-                if (ry[jy] >= 0 && rz[jz] >= 0) {
-                    const int *__restrict__ crow = chunk_of + (size_t)(rz[jz] * g.ny + ry[jy]) * cg.nbx;
-                    pa[lidx] = __ldg(crow + ja);
-                    if (jb != ja) pb[lidx] = __ldg(crow + jb);
-                }
-            }
+        AxisCand<MAXC> ax, ay, az;
+        axis_candidates<true, MAXC>(x, g.nx, g.wallx, cg.nbx, ax);
+        axis_candidates<false, MAXC>(y, g.ny, g.wally, 0, ay);
+        axis_candidates<false, MAXC>(z, g.nz, g.wallz, 0, az);
         float sx = 0.f, sy = 0.f, sz = 0.f;
 #pragma unroll
-        for (int lidx = 0; lidx < 16; ++lidx) {
-            collect_one<NARROW>(T, pa[lidx], lidx, cg.ent, ea, g.nx, sx, sy, sz);
-            collect_one<NARROW>(T, pb[lidx], lidx, cg.ent, eb, g.nx, sx, sy, sz);
-        }
+        for (int iz = 0; iz < MAXC; ++iz)
+#pragma unroll
+            for (int iy = 0; iy < MAXC; ++iy)
+#pragma unroll
+                for (int ix = 0; ix < MAXC; ++ix) {
+                    if (iz >= az.n || iy >= ay.n || ix >= ax.n) continue;
+                    const int ts = tile_slot_of(ax.t[ix], ay.t[iy], az.t[iz], cg, tg);
+                    const unsigned m = __ldg(tt.mask + ts);
+                    if (!((m >> ax.f[ix]) & (m >> (14 + ay.f[iy])) & (m >> (21 + az.f[iz])) & 1u)) continue;
+                    const int id = __ldg(tt.id + ts);
+                    if (id < 0) continue;
+                    const float4 v = F[((size_t)id * (TILE_F * TILE_F) + ay.f[iy] * TILE_F + az.f[iz]) * cg.ent + ax.f[ix]];
+                    sx += v.x; sy += v.y; sz += v.z;
+                }
         if (LAST) {
             field[cell] = make_float4(sx, sy, sz, 0.f);
         } else {

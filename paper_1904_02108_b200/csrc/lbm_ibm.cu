@@ -60,9 +60,10 @@ struct SetScalars {
     int n_chunks;        // chunks (may exceed the capacity: the excess is dropped and flagged)
     int n_entries;       // profile entries (window cells) over all chunks
     int n_cells;         // active cells
-    int cursor[MAX_MDF]; // work cursors of the run sweeps, one per MDF iteration
+    int n_tiles;         // tiles (may exceed the capacity: the excess is dropped and flagged)
+    int cursor[MAX_MDF]; // work cursors of the tile sweeps, one per MDF iteration
 };
-constexpr int N_STEP_COUNTERS = 4 + MAX_MDF;
+constexpr int N_STEP_COUNTERS = 5 + MAX_MDF;
 
 struct HostBody {
     long long first, count;
@@ -108,6 +109,7 @@ struct PrepSet {
     int *vals[2] = {nullptr, nullptr};        // the permutation, same ping-pong
     MarkerSorted ms{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     ChunkTable ct{nullptr, nullptr, nullptr};
+    TileTable tt{nullptr, nullptr, nullptr, nullptr};  // mask, id: dense over the tile slots; slot, rec: per tile
     unsigned *headbits = nullptr;             // one bit per sorted marker: starts a run
     int *cells = nullptr;                     // active-cell list
     // dense maps, cleared incrementally by the set's next preparation (k_clear_prev)
@@ -156,10 +158,11 @@ struct lbm {
     BodyStep *d_tabs = nullptr;
     int *d_hist = nullptr, *d_total = nullptr;
     size_t cells_cap = 0, headbits_cap = 0;
-    float4 *T = nullptr;                // chunk profiles [chunk][16][cg.ent]
+    float4 *F = nullptr;                // tile footprints [tile][7][7][cg.ent]
     ChunkGeom cg{1, CHUNK_W + 3};
-    int chunk_cap = 0;                  // chunks T has room for
-    size_t chunk_slots = 0;             // entries of chunk_of
+    TileGeom tg{1, 1};
+    int chunk_cap = 0, tile_cap = 0;    // capacity of the chunk table / of F
+    size_t chunk_slots = 0, tile_slots = 0;   // entries of chunk_of / of the dense tile maps
     int rows_grid = 148;                // persistent grid of the run sweep (blocks resident at once)
     int words_grid = 148, moments_grid = 148;   // same for the active-word stream-collide and the moments kernel
     int sort_ipw = 64, sort_tiles = 0, sort_passes = 1;
@@ -211,6 +214,8 @@ void free_set(lbm *h, PrepSet &S)
     dfree(h, S.ms.sg, c); dfree(h, S.ms.du, c);
     dfree(h, S.ct.first, (size_t)h->chunk_cap); dfree(h, S.ct.end, (size_t)h->chunk_cap);
     dfree(h, S.ct.slot, (size_t)h->chunk_cap);
+    dfree(h, S.tt.slot, (size_t)h->tile_cap);
+    dfree(h, S.tt.rec, (size_t)h->tile_cap * 16);
     dfree(h, S.cells, h->cells_cap);
     dfree(h, S.headbits, h->headbits_cap);
     S.step = -1;
@@ -224,7 +229,7 @@ void free_markers_dev(lbm *h)
     dfree(h, h->d_body, c);
     for (PrepSet &S : h->set) free_set(h, S);
     h->cells_cap = 0; h->headbits_cap = 0;
-    dfree(h, h->T, (size_t)h->chunk_cap * 16 * (size_t)h->cg.ent); h->chunk_cap = 0;
+    dfree(h, h->F, (size_t)h->tile_cap * (TILE_F * TILE_F) * (size_t)h->cg.ent); h->chunk_cap = 0; h->tile_cap = 0;
     dfree(h, h->d_hist, (size_t)RADIX * (size_t)h->sort_tiles);
     dfree(h, h->d_total, (size_t)RADIX);
     dfree(h, h->d_defs, (size_t)h->nb_cap);
@@ -260,7 +265,7 @@ int flush_set(lbm *h, PrepSet &S)
     if (!S.dirty) return LBM_OK;
     k_clear_prev<<<LIST_GRID, 256, 0, h->stream>>>(sorted_keys(h, S), &S.scal->n_prev, S.bin_first, S.amask, S.words,
                                                     &S.scal->n_words, S.chunk_of, S.ct.slot, &S.scal->n_chunks,
-                                                    h->chunk_cap);
+                                                    h->chunk_cap, S.tt.mask, S.tt.slot, &S.scal->n_tiles, h->tile_cap);
     CK(cudaMemsetAsync(S.scal, 0, sizeof(SetScalars), h->stream));
     CK(cudaGetLastError());
     h->launches += 1;
@@ -298,11 +303,12 @@ int upload_markers(lbm *h)
         }
         if ((rc = dmalloc(h, &h->d_s, c))) return rc;
         if ((rc = dmalloc(h, &h->d_body, c))) return rc;
-        // T has room for every chunk that can exist (one per marker, one per (row, block) slot, CHUNK_ID_MAX)
-        // up to 8 GB; beyond that the capacity is capped and an overflow is flagged on the device
-        size_t ccap = std::min(std::min(c, h->chunk_slots), (size_t)CHUNK_ID_MAX);
-        const size_t chunk_bytes = (size_t)16 * (size_t)h->cg.ent * sizeof(float4);
-        ccap = std::max((size_t)1, std::min(ccap, ((size_t)8 << 30) / chunk_bytes));
+        // every chunk that can exist gets a table entry (one per marker, one per (row, block) slot, CHUNK_ID_MAX);
+        // F has room for every tile that can exist up to 12 GB, beyond that the capacity is capped and an
+        // overflow is flagged on the device (LBM_ENOMEM at lbm_sync)
+        const size_t ccap = std::max((size_t)1, std::min(std::min(c, h->chunk_slots), (size_t)CHUNK_ID_MAX));
+        const size_t tile_bytes = (size_t)(TILE_F * TILE_F) * (size_t)h->cg.ent * sizeof(float4);
+        const size_t tcap = std::max((size_t)1, std::min(std::min(c, h->tile_slots), ((size_t)12 << 30) / tile_bytes));
         h->cells_cap = std::min((size_t)64 * c, (size_t)h->g.cells);
         h->headbits_cap = c / 32 + 16;
         for (PrepSet &S : h->set) {
@@ -319,11 +325,13 @@ int upload_markers(lbm *h)
             if ((rc = dmalloc(h, &S.ct.first, (size_t)ccap))) return rc;
             if ((rc = dmalloc(h, &S.ct.end, (size_t)ccap))) return rc;
             if ((rc = dmalloc(h, &S.ct.slot, (size_t)ccap))) return rc;
+            if ((rc = dmalloc(h, &S.tt.slot, tcap))) return rc;
+            if ((rc = dmalloc(h, &S.tt.rec, tcap * 16))) return rc;
             if ((rc = dmalloc(h, &S.cells, h->cells_cap))) return rc;
             if ((rc = dmalloc(h, &S.headbits, h->headbits_cap))) return rc;
         }
-        if ((rc = dmalloc(h, &h->T, ccap * 16 * (size_t)h->cg.ent))) return rc;
-        h->chunk_cap = (int)ccap;
+        if ((rc = dmalloc(h, &h->F, tcap * (TILE_F * TILE_F) * (size_t)h->cg.ent))) return rc;
+        h->chunk_cap = (int)ccap; h->tile_cap = (int)tcap;
         if ((rc = dmalloc(h, &h->d_total, (size_t)RADIX))) return rc;
         if ((rc = dmalloc(h, &h->d_defs, (size_t)nb))) return rc;
         if ((rc = dmalloc(h, &h->d_tabs, (size_t)nb))) return rc;
@@ -395,7 +403,7 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
 
     if (pt) pt->mark(PH_KEYS, s);
     k_clear_prev<<<LIST_GRID, 256, 0, s>>>(skey, &sc->n_prev, S.bin_first, S.amask, S.words, &sc->n_words, S.chunk_of,
-                                           S.ct.slot, &sc->n_chunks, h->chunk_cap);
+                                           S.ct.slot, &sc->n_chunks, h->chunk_cap, S.tt.mask, S.tt.slot, &sc->n_tiles, h->tile_cap);
     const int nb = (int)h->bodies.size();
     k_kinematics<<<(std::max(nb, N_STEP_COUNTERS) + 127) / 128, 128, 0, s>>>(h->d_defs, h->d_tabs, nb, &h->scal->step_ctr,
                                                                               step_offset, &sc->n_words, N_STEP_COUNTERS);
@@ -423,7 +431,10 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
                                     S.chunk_of, &h->scal->status);
         k_chunk_publish<<<LIST_GRID, 256, 0, s>>>(g, h->cg, S.ct, &sc->n_chunks, h->chunk_cap, S.chunk_of, S.amask, S.words,
                                                   &sc->n_words);
-        nk += 3;
+        k_tiles<<<LIST_GRID, 256, 0, s>>>(g, h->cg, h->tg, S.ct, &sc->n_chunks, h->chunk_cap, S.chunk_of, S.tt, h->tile_cap,
+                                          &sc->n_tiles, &h->scal->status);
+        k_tile_fill<<<LIST_GRID, 256, 0, s>>>(g, h->cg, h->tg, S.ct, &sc->n_chunks, h->chunk_cap, S.tt);
+        nk += 5;
     } else {
         k_bins<<<mb, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask, S.words, &sc->n_words);
         ++nk;
@@ -454,13 +465,14 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
         ++nk;
         if (pt) pt->mark(PH_SPREAD, s);
         if (h->opt_spread == 0) {
-            k_spread_chunks<<<h->rows_grid, 256, 0, s>>>(S.ct, &sc->n_chunks, h->chunk_cap, &sc->cursor[m], S.chunk_of, h->cg,
-                                                         reinterpret_cast<const float2 *>(S.ms.wx), S.ms.wyz,
-                                                         last ? S.ms.du : S.ms.sg, h->T);
-            const bool narrow = g.nx < CHUNK_ENT_MAX;
-            auto collect = last ? (narrow ? k_collect_chunks<true, true> : k_collect_chunks<true, false>)
-                                : (narrow ? k_collect_chunks<false, true> : k_collect_chunks<false, false>);
-            collect<<<LIST_GRID, 256, 0, s>>>(g, h->cg, S.chunk_of, h->T, S.cells, &sc->n_cells, last ? h->G : h->U);
+            k_spread_tiles<<<h->rows_grid, TILE_WARPS * 32, spread_tiles_smem(h->cg), s>>>(
+                h->cg, S.tt.rec, S.tt.slot, S.tt.mask, &sc->n_tiles, h->tile_cap, &sc->cursor[m], S.ms.wx, S.ms.wyz,
+                last ? S.ms.du : S.ms.sg, h->F);
+            const bool two = (g.wallx || g.nx >= CHUNK_ENT_MAX) && (g.wally || g.ny % TILE_R == 0) &&
+                             (g.wallz || g.nz % TILE_R == 0);
+            auto collect = last ? (two ? k_collect_tiles<true, 2> : k_collect_tiles<true, 4>)
+                                : (two ? k_collect_tiles<false, 2> : k_collect_tiles<false, 4>);
+            collect<<<LIST_GRID, 256, 0, s>>>(g, h->cg, h->tg, S.tt, h->F, S.cells, &sc->n_cells, last ? h->G : h->U);
             nk += 2;
         } else if (h->opt_spread == 2) {
             if (last)
@@ -730,13 +742,17 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
     if (dmalloc(h, &h->scal, (size_t)1)) return bail("scalars");
     h->cg = chunk_geom(nx);
     h->chunk_slots = (size_t)h->cg.nbx * ny * nz;
+    h->tg = tile_geom(ny, nz);
+    h->tile_slots = (size_t)h->cg.nbx * h->tg.nty * h->tg.ntz;
     bool ok = true;
     for (PrepSet &S : h->set) {
         if (dmalloc(h, &S.amask, h->n_mask_words) || dmalloc(h, &S.words, h->n_mask_words)) return bail("active mask");
         if (dmalloc(h, &S.chunk_of, h->chunk_slots)) return bail("chunk map");
+        if (dmalloc(h, &S.tt.mask, h->tile_slots) || dmalloc(h, &S.tt.id, h->tile_slots)) return bail("tile maps");
         if (dmalloc(h, &S.scal, (size_t)1)) return bail("set scalars");
         ok &= cudaMemset(S.amask, 0, h->n_mask_words * sizeof(unsigned)) == cudaSuccess;
         ok &= cudaMemset(S.chunk_of, 0xff, h->chunk_slots * sizeof(int)) == cudaSuccess;
+        ok &= cudaMemset(S.tt.mask, 0, h->tile_slots * sizeof(unsigned)) == cudaSuccess;
         ok &= cudaMemset(S.scal, 0, sizeof(SetScalars)) == cudaSuccess;
     }
     ok &= cudaMemset(h->f[0], 0, fcount * sizeof(float)) == cudaSuccess;   // rest state: f_i - t_i = 0
@@ -747,7 +763,9 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
     {
         int per_sm = 0, sms = 148;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spread_chunks, 256, 0);
+        cudaFuncSetAttribute(k_spread_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             16 * 16 * 3 * 16 * (int)sizeof(float) + TILE_WARPS * 2 * SPREAD_PIECE_BYTES);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spread_tiles, TILE_WARPS * 32, spread_tiles_smem(h->cg));
         h->rows_grid = std::max(1, per_sm) * sms;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_stream_collide_words, 256, 0);
         h->words_grid = std::max(1, per_sm) * sms;
@@ -767,6 +785,7 @@ void lbm_destroy(lbm_t *h)
     cudaFree(h->f[0]); cudaFree(h->f[1]); cudaFree(h->U); cudaFree(h->G); cudaFree(h->scal);
     for (PrepSet &S : h->set) {
         cudaFree(S.amask); cudaFree(S.words); cudaFree(S.chunk_of); cudaFree(S.bin_first); cudaFree(S.scal);
+        cudaFree(S.tt.mask); cudaFree(S.tt.id);
     }
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     if (h->cap_bulk) cudaStreamDestroy(h->cap_bulk);
@@ -810,11 +829,11 @@ int lbm_get_info(lbm_t *h, int key, long long *value)
         case LBM_INFO_STEPS: *value = h->steps_done; return LBM_OK;
         case LBM_INFO_LAUNCHES: *value = h->launches; return LBM_OK;
         case LBM_INFO_DEVICE_BYTES: *value = (long long)h->dev_bytes; return LBM_OK;
-        case LBM_INFO_ACTIVE_CELLS: case LBM_INFO_RUNS: case LBM_INFO_RUN_ENTRIES: {
+        case LBM_INFO_ACTIVE_CELLS: case LBM_INFO_RUNS: case LBM_INFO_RUN_ENTRIES: case LBM_INFO_TILES: {
             int r = 0;
             if (h->force_valid && h->last_set >= 0) {
                 const SetScalars *sc = h->set[h->last_set].scal;
-                const int *p = key == LBM_INFO_ACTIVE_CELLS ? &sc->n_cells : (key == LBM_INFO_RUNS ? &sc->n_chunks : &sc->n_entries);
+                const int *p = key == LBM_INFO_ACTIVE_CELLS ? &sc->n_cells : (key == LBM_INFO_RUNS ? &sc->n_chunks : (key == LBM_INFO_TILES ? &sc->n_tiles : &sc->n_entries));
                 CK(cudaMemcpyAsync(&r, p, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
                 CK(cudaStreamSynchronize(h->stream));
             }
