@@ -587,8 +587,8 @@ struct Acc3 { float x, y, z; };
 // ---- tiles ---------------------------------------------------------------------------------------
 // A "tile" groups the chunks of one x block whose source rows lie in one aligned 4 x 4 block of
 // (y, z): up to 16 chunks.  Their 16 x 16 profiles overlap on a footprint of 7 x 7 target rows, so
-// one thread block sweeps the chunks of a tile into shared memory, adds the profiles that fall on
-// the same target row there (fixed order) and writes ONE footprint  F[tile][fy][fz][e]  (fy, fz =
+// one warp sweeps the chunks of a tile one after the other, adds their profiles up in a footprint it
+// keeps in shared memory (fixed order) and writes ONE footprint  F[tile][fy][fz][e]  (fy, fz =
 // 0..6 <-> target row 4 ty - 1 + fy, 4 tz - 1 + fz; e as in the chunk window).  Stage B then reads
 // about 4 footprints per cell instead of 22 profiles, and the profile traffic shrinks ~7x.
 //
@@ -697,10 +697,177 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned pari
         : "memory");
 }
 
-// Stage A: one thread block (8 warps) per tile.  The source rows of the tile that hold a chunk are
+// Stage A: one WARP per tile, no block-level synchronisation at all.  The warp walks through the
+// source rows of its tile that hold a chunk, in ascending order, and sweeps each chunk with
+// lane = h*16 + l: l = jy*4 + jz is the target-row offset whose profile the lane accumulates, h the
+// half of the 4-cell x window it owns (h = 0: the two left cells, h = 1: the two right cells), both
+// in registers.  When the sweep moves on to the next cell the leftmost window cell is final: the
+// lane adds it to the tile's footprint, which the warp keeps in shared memory (the 16 lanes of a
+// chunk hit 16 different footprint rows, and chunks follow one another, so there is no conflict and
+// the order of every sum is fixed), and the window shifts by one (the cell that crosses from the
+// right half to the left half travels by shuffle).  Control flow is uniform across the warp.
+//
+// The marker data of a chunk (value, x weights, y-z weights: three contiguous ranges of the sorted
+// arrays) comes through the warp's own shared-memory buffers by asynchronous bulk copies (TMA),
+// SPREAD_PIECE markers at a time through a ring of SPREAD_STAGES buffers that runs ACROSS chunks, so the sweep never waits on a
+// global load per marker.  Tiles are handed out through an atomic cursor.
+//
+// Shared memory (dynamic), per warp: footprint [7*7][ent][3] floats, then STAGES x { val[PIECE] float4,
+// wx[PIECE] float4, wyz[PIECE][16] float }.
+#ifndef TILE_WARPS_CFG
+#define TILE_WARPS_CFG 4
+#define TILE_MINB_CFG 5
+#define SPREAD_PIECE_CFG 16
+#define SPREAD_STAGES_CFG 2
+#endif
+constexpr int TILE_WARPS = TILE_WARPS_CFG;
+constexpr int SPREAD_PIECE = SPREAD_PIECE_CFG;
+constexpr int SPREAD_STAGES = SPREAD_STAGES_CFG;     // ring of staging buffers per warp: STAGES - 1 pieces in flight
+constexpr int SPREAD_PIECE_BYTES = SPREAD_PIECE * 96;
+
+inline size_t spread_warp_smem(const ChunkGeom &cg)
+{
+    const size_t foot = ((size_t)TILE_F * TILE_F * (size_t)cg.ent * 3 * sizeof(float) + 127) / 128 * 128;
+    return foot + SPREAD_STAGES * SPREAD_PIECE_BYTES;
+}
+inline size_t spread_tiles_smem(const ChunkGeom &cg) { return (size_t)TILE_WARPS * spread_warp_smem(cg); }
+
+__global__ void __launch_bounds__(TILE_WARPS * 32, TILE_MINB_CFG)
+k_spread_tiles(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int *__restrict__ tile_slot,
+               const unsigned *__restrict__ tile_mask, const int *__restrict__ n_tiles, int tile_cap,
+               int *__restrict__ cursor, const float4 *__restrict__ wx4, const float *__restrict__ wyz16,
+               const float4 *__restrict__ val, float4 *__restrict__ F, int warp_smem)
+{
+    extern __shared__ __align__(128) char smem[];
+    __shared__ unsigned long long s_bar[TILE_WARPS][SPREAD_STAGES];
+    __shared__ int s_n[TILE_WARPS][SPREAD_STAGES];     // markers in the piece a stage holds
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int l = lane & 15, h = lane >> 4;
+    const int nt = min(*n_tiles, tile_cap);
+    const int ent = cg.ent;
+    float *foot = reinterpret_cast<float *>(smem + (size_t)warp * warp_smem);
+    char *stage = smem + (size_t)warp * warp_smem + (warp_smem - SPREAD_STAGES * SPREAD_PIECE_BYTES);
+    unsigned long long *bar = s_bar[warp];
+    if (lane < SPREAD_STAGES) mbar_init(&bar[lane], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncwarp();
+    unsigned phase = 0u;                                 // bit b: parity the next wait on bar[b] uses
+    const int nfoot = TILE_F * TILE_F * ent;             // footprint elements
+    const int jy = l >> 2, jz = l & 3;
+    for (;;) {
+        int t = 0;
+        if (lane == 0) t = atomicAdd(cursor, 1);
+        t = __shfl_sync(0xffffffffu, t, 0);
+        if (t >= nt) break;
+        // lane r < 16: sorted-marker range of the chunk in source row r = sy + 4 sz ((0,0) = none)
+        const int2 rec = __ldg(tile_rec + (size_t)t * 16 + l);
+        const unsigned present = __ballot_sync(0xffffffffu, rec.y > rec.x) & 0xffffu;
+        const int ts = __ldg(tile_slot + t);
+        const int x0 = (ts % cg.nbx) * CHUNK_W;
+        // piece stream over the chunks of the tile: (row, offset) of the next piece to issue
+        unsigned irest = present;
+        int ioff = 0;
+        int n_issued = 0;
+        auto issue = [&]() {                             // next piece of the stream into stage n_issued % STAGES
+            if (!irest) return;
+            const int b = n_issued % SPREAD_STAGES;
+            const int r = __ffs(irest) - 1;
+            const int first = __shfl_sync(0xffffffffu, rec.x, r), end = __shfl_sync(0xffffffffu, rec.y, r);
+            const int j0 = first + ioff;
+            const int n = min(SPREAD_PIECE, end - j0);
+            if (lane == 0) {
+                char *dst = stage + b * SPREAD_PIECE_BYTES;
+                s_n[warp][b] = n;
+                mbar_expect_tx(&bar[b], (unsigned)n * 96u);
+                bulk_g2s(dst, val + j0, (unsigned)n * 16u, &bar[b]);
+                bulk_g2s(dst + SPREAD_PIECE * 16, wx4 + j0, (unsigned)n * 16u, &bar[b]);
+                bulk_g2s(dst + SPREAD_PIECE * 32, wyz16 + (size_t)j0 * 16, (unsigned)n * 64u, &bar[b]);
+            }
+            ioff += n;
+            if (j0 + n == end) { irest &= irest - 1; ioff = 0; }
+            ++n_issued;
+        };
+#pragma unroll
+        for (int i = 0; i < SPREAD_STAGES - 1; ++i) issue();
+        // zero the footprint while the first piece is in flight
+        for (int i = lane; i < (nfoot * 3 + 3) / 4; i += 32) reinterpret_cast<float4 *>(foot)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        __syncwarp();
+        // consumer state: row being swept and how many of its markers are still to come
+        unsigned crest = present;
+        int cleft = 0;
+        float *frow = foot;
+        Acc3 p{0.f, 0.f, 0.f}, q{0.f, 0.f, 0.f};         // window cells (e + 2h, e + 2h + 1)
+        int e = 0;
+        for (int k = 0; k < n_issued; ++k) {
+            issue();                                     // into the stage the previous round released (__syncwarp below)
+            const int b = k % SPREAD_STAGES;
+            mbar_wait(&bar[b], (phase >> b) & 1u);
+            phase ^= 1u << b;
+            const int n_cur = s_n[warp][b];
+            const char *src = stage + b * SPREAD_PIECE_BYTES;
+            const float4 *sv = reinterpret_cast<const float4 *>(src);
+            const float2 *sw = reinterpret_cast<const float2 *>(src + SPREAD_PIECE * 16) + h;
+            const float *sz = reinterpret_cast<const float *>(src + SPREAD_PIECE * 32) + l;
+            if (cleft == 0) {                            // this piece starts a new source row
+                const int r = __ffs(crest) - 1;
+                crest &= crest - 1;
+                cleft = __shfl_sync(0xffffffffu, rec.y - rec.x, r);
+                frow = foot + (((r & 3) + jy) * TILE_F + ((r >> 2) + jz)) * ent * 3;
+                p = Acc3{0.f, 0.f, 0.f}; q = Acc3{0.f, 0.f, 0.f};
+                e = __float_as_int(sv[0].w) - x0;        // window start = entry of the first marker's cx - 1
+            }
+            auto flush = [&](int ee, const Acc3 &a) {
+                float *d = frow + ee * 3;
+                d[0] += a.x; d[1] += a.y; d[2] += a.z;
+            };
+#pragma unroll 4
+            for (int j = 0; j < n_cur; ++j) {
+                const float4 v = sv[j];
+                const float2 w = sw[2 * j];
+                const float wz = sz[16 * j];
+                const int em = __float_as_int(v.w) - x0;
+                if (em != e) {                           // warp-uniform: the sweep moves on to another cell
+#pragma unroll 1
+                    do {                                 // the leftmost window cell is complete
+                        if (h == 0) flush(e, p);
+                        const float tx = __shfl_down_sync(0xffffffffu, p.x, 16);
+                        const float ty = __shfl_down_sync(0xffffffffu, p.y, 16);
+                        const float tz = __shfl_down_sync(0xffffffffu, p.z, 16);
+                        p = q;
+                        q.x = h ? 0.f : tx; q.y = h ? 0.f : ty; q.z = h ? 0.f : tz;
+                    } while (++e < em);
+                }
+                const float vx = v.x * wz, vy = v.y * wz, vz = v.z * wz;
+                p.x = fmaf(w.x, vx, p.x); p.y = fmaf(w.x, vy, p.y); p.z = fmaf(w.x, vz, p.z);
+                q.x = fmaf(w.y, vx, q.x); q.y = fmaf(w.y, vy, q.y); q.z = fmaf(w.y, vz, q.z);
+            }
+            cleft -= n_cur;
+            if (cleft == 0) {                            // the row's last window: entries e .. e+3 (= hi)
+                flush(e + 2 * h, p);
+                flush(e + 2 * h + 1, q);
+            }
+            __syncwarp();                                // every lane is done with stage b (and with the footprint row)
+        }
+        // write the footprint elements some chunk of the tile can reach (mask product); the rest is never read
+        const unsigned m = __ldg(tile_mask + ts);
+        float4 *__restrict__ Ft = F + (size_t)t * nfoot;
+        for (int idx = lane; idx < nfoot; idx += 32) {
+            const int fyz = idx / ent, ee = idx - fyz * ent;
+            const int fy = fyz / TILE_F, fz = fyz - fy * TILE_F;
+            if ((m >> ee) & (m >> (14 + fy)) & (m >> (21 + fz)) & 1u) {
+                const float *s = foot + idx * 3;
+                Ft[idx] = make_float4(s[0], s[1], s[2], 0.f);
+            }
+        }
+        __syncwarp();
+    }
+}
+
+// Stage A, variant for FEW tiles (small marker sets): one thread block (8 warps) per tile, so that a single
+// propeller still spreads over all SMs.  The source rows of the tile that hold a chunk are
 // dealt to the warps.  A warp brings its chunk's marker data (value, x weights, y-z weights: three
 // contiguous ranges of the sorted arrays) into its own shared-memory buffers with asynchronous bulk
-// copies, SPREAD_PIECE markers at a time and double-buffered, so the sweep never waits on a global
+// copies, BTILE_PIECE markers at a time and double-buffered, so the sweep never waits on a global
 // load per marker.  It sweeps the chunk with lane = h*16 + l: l = jy*4 + jz is the target-row
 // offset whose profile the lane accumulates, h the half of the 4-cell x window it owns (h = 0: the
 // two left cells, h = 1: the two right cells), both in registers.  When the sweep moves on to the
@@ -714,30 +881,24 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned pari
 // Shared memory (dynamic): prof[16 source rows][16 l][3 components][EP*4 entries] floats (EP =
 // ceil(ent/4)), so that the reduction reads four consecutive entries of one component with one
 // 128-bit load; then per warp 2 x { val[PIECE] float4, wx[PIECE] float4, wyz[PIECE][16] float }.
-// measured on B200 (W4, W3, W4lit): 8 warps, 4 blocks per SM, pieces of 16 markers beat 4/16 warps, 2-5 blocks and
-// pieces of 32 (more resident blocks hide the barrier between sweep and reduction)
-#ifndef TILE_WARPS_CFG
-#define TILE_WARPS_CFG 8
-#define TILE_MINB_CFG 4
-#define SPREAD_PIECE_CFG 16
-#endif
-constexpr int TILE_WARPS = TILE_WARPS_CFG;
-constexpr int SPREAD_PIECE = SPREAD_PIECE_CFG;
-constexpr int SPREAD_PIECE_BYTES = SPREAD_PIECE * 96;
+// measured on B200: 8 warps, 4 blocks per SM, pieces of 16 markers beat 4/16 warps, 2-5 blocks and pieces of 32
+constexpr int BTILE_WARPS = 8;
+constexpr int BTILE_PIECE = 16;
+constexpr int BTILE_PIECE_BYTES = BTILE_PIECE * 96;
 
-inline size_t spread_tiles_smem(const ChunkGeom &cg)
+inline size_t spread_tiles_block_smem(const ChunkGeom &cg)
 {
-    return (size_t)16 * 16 * 3 * (size_t)((cg.ent + 3) / 4 * 4) * sizeof(float) + (size_t)TILE_WARPS * 2 * SPREAD_PIECE_BYTES;
+    return (size_t)16 * 16 * 3 * (size_t)((cg.ent + 3) / 4 * 4) * sizeof(float) + (size_t)BTILE_WARPS * 2 * BTILE_PIECE_BYTES;
 }
 
-__global__ void __launch_bounds__(TILE_WARPS * 32, TILE_MINB_CFG)
-k_spread_tiles(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int *__restrict__ tile_slot,
+__global__ void __launch_bounds__(BTILE_WARPS * 32, 4)
+k_spread_tiles_block(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int *__restrict__ tile_slot,
                const unsigned *__restrict__ tile_mask, const int *__restrict__ n_tiles, int tile_cap,
                int *__restrict__ cursor, const float4 *__restrict__ wx4, const float *__restrict__ wyz16,
                const float4 *__restrict__ val, float4 *__restrict__ F)
 {
     extern __shared__ __align__(128) float4 smem4[];
-    __shared__ unsigned long long s_bar[TILE_WARPS][2];
+    __shared__ unsigned long long s_bar[BTILE_WARPS][2];
     __shared__ int s_tile[2];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int l = lane & 15, h = lane >> 4;
@@ -746,7 +907,7 @@ k_spread_tiles(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int *__res
     const int EP = (ent + 3) >> 2, E4 = EP * 4;          // entries per profile row in shared memory
     const int rowf = 16 * 3 * E4;                        // floats per source row
     float *prof = reinterpret_cast<float *>(smem4);
-    char *stage = reinterpret_cast<char *>(smem4) + (size_t)16 * rowf * sizeof(float) + (size_t)warp * 2 * SPREAD_PIECE_BYTES;
+    char *stage = reinterpret_cast<char *>(smem4) + (size_t)16 * rowf * sizeof(float) + (size_t)warp * 2 * BTILE_PIECE_BYTES;
     unsigned long long *bar = s_bar[warp];
     if (lane == 0) { mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); }
     unsigned phase = 0u;                                 // bit b: parity the next wait on bar[b] uses
@@ -768,19 +929,19 @@ k_spread_tiles(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int *__res
         // the present source rows, dealt round-robin to the warps
         int taken = 0;
         for (unsigned rest = present; rest; rest &= rest - 1, ++taken) {
-            if ((taken & (TILE_WARPS - 1)) != warp) continue;
+            if ((taken & (BTILE_WARPS - 1)) != warp) continue;
             const int r = __ffs(rest) - 1;
             const int i0 = __shfl_sync(0xffffffffu, rec.x, r), i1 = __shfl_sync(0xffffffffu, rec.y, r);
-            const int npieces = (i1 - i0 + SPREAD_PIECE - 1) / SPREAD_PIECE;
+            const int npieces = (i1 - i0 + BTILE_PIECE - 1) / BTILE_PIECE;
             auto issue = [&](int k) {                    // lane 0: bulk copies of piece k into buffer k & 1
                 const int b = k & 1;
-                const int j0 = i0 + k * SPREAD_PIECE;
-                const int n = min(SPREAD_PIECE, i1 - j0);
-                char *dst = stage + b * SPREAD_PIECE_BYTES;
+                const int j0 = i0 + k * BTILE_PIECE;
+                const int n = min(BTILE_PIECE, i1 - j0);
+                char *dst = stage + b * BTILE_PIECE_BYTES;
                 mbar_expect_tx(&bar[b], (unsigned)n * 96u);
                 bulk_g2s(dst, val + j0, (unsigned)n * 16u, &bar[b]);
-                bulk_g2s(dst + SPREAD_PIECE * 16, wx4 + j0, (unsigned)n * 16u, &bar[b]);
-                bulk_g2s(dst + SPREAD_PIECE * 32, wyz16 + (size_t)j0 * 16, (unsigned)n * 64u, &bar[b]);
+                bulk_g2s(dst + BTILE_PIECE * 16, wx4 + j0, (unsigned)n * 16u, &bar[b]);
+                bulk_g2s(dst + BTILE_PIECE * 32, wyz16 + (size_t)j0 * 16, (unsigned)n * 64u, &bar[b]);
             };
             if (lane == 0) issue(0);
             // zero the row's profiles (entries outside the chunk's window stay zero) while the copy is in flight
@@ -795,11 +956,11 @@ k_spread_tiles(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int *__res
                 if (k + 1 < npieces && lane == 0) issue(k + 1);   // buffer (k+1)&1 was released by the __syncwarp below
                 mbar_wait(&bar[b], (phase >> b) & 1u);
                 phase ^= 1u << b;
-                const char *src = stage + b * SPREAD_PIECE_BYTES;
+                const char *src = stage + b * BTILE_PIECE_BYTES;
                 const float4 *sv = reinterpret_cast<const float4 *>(src);
-                const float2 *sw = reinterpret_cast<const float2 *>(src + SPREAD_PIECE * 16) + h;
-                const float *sz = reinterpret_cast<const float *>(src + SPREAD_PIECE * 32) + l;
-                const int n = min(SPREAD_PIECE, i1 - i0 - k * SPREAD_PIECE);
+                const float2 *sw = reinterpret_cast<const float2 *>(src + BTILE_PIECE * 16) + h;
+                const float *sz = reinterpret_cast<const float *>(src + BTILE_PIECE * 32) + l;
+                const int n = min(BTILE_PIECE, i1 - i0 - k * BTILE_PIECE);
                 if (k == 0) e = __float_as_int(sv[0].w) - x0;   // window start = entry of the first marker's cx - 1
 #pragma unroll 4
                 for (int j = 0; j < n; ++j) {

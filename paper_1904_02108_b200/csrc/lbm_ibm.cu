@@ -72,6 +72,7 @@ struct HostBody {
 };
 
 constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driven kernels
+constexpr int SPREAD_BLOCK_BELOW = 100000;   // marker count below which the block-per-tile sweep is used (measured: W3 vs W4lit)
 
 // Optional per-phase device timing (LBM_OPT_TIMING): CUDA events recorded on the launching stream
 // between the phases of a step; durations are accumulated after a stream synchronise.
@@ -163,7 +164,7 @@ struct lbm {
     TileGeom tg{1, 1};
     int chunk_cap = 0, tile_cap = 0;    // capacity of the chunk table / of F
     size_t chunk_slots = 0, tile_slots = 0;   // entries of chunk_of / of the dense tile maps
-    int rows_grid = 148;                // persistent grid of the run sweep (blocks resident at once)
+    int rows_grid = 148, rows_block_grid = 148;   // persistent grids of the two tile sweeps (blocks resident at once)
     int words_grid = 148, moments_grid = 148;   // same for the active-word stream-collide and the moments kernel
     int sort_ipw = 64, sort_tiles = 0, sort_passes = 1;
 
@@ -465,9 +466,15 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
         ++nk;
         if (pt) pt->mark(PH_SPREAD, s);
         if (h->opt_spread == 0) {
-            k_spread_tiles<<<h->rows_grid, TILE_WARPS * 32, spread_tiles_smem(h->cg), s>>>(
-                h->cg, S.tt.rec, S.tt.slot, S.tt.mask, &sc->n_tiles, h->tile_cap, &sc->cursor[m], S.ms.wx, S.ms.wyz,
-                last ? S.ms.du : S.ms.sg, h->F);
+            // few markers (a single propeller): one block per tile keeps all SMs busy; many: one warp per tile
+            if (n < SPREAD_BLOCK_BELOW)
+                k_spread_tiles_block<<<h->rows_block_grid, BTILE_WARPS * 32, spread_tiles_block_smem(h->cg), s>>>(
+                    h->cg, S.tt.rec, S.tt.slot, S.tt.mask, &sc->n_tiles, h->tile_cap, &sc->cursor[m], S.ms.wx, S.ms.wyz,
+                    last ? S.ms.du : S.ms.sg, h->F);
+            else
+                k_spread_tiles<<<h->rows_grid, TILE_WARPS * 32, spread_tiles_smem(h->cg), s>>>(
+                    h->cg, S.tt.rec, S.tt.slot, S.tt.mask, &sc->n_tiles, h->tile_cap, &sc->cursor[m], S.ms.wx, S.ms.wyz,
+                    last ? S.ms.du : S.ms.sg, h->F, (int)spread_warp_smem(h->cg));
             const bool two = (g.wallx || g.nx >= CHUNK_ENT_MAX) && (g.wally || g.ny % TILE_R == 0) &&
                              (g.wallz || g.nz % TILE_R == 0);
             auto collect = last ? (two ? k_collect_tiles<true, 2> : k_collect_tiles<true, 4>)
@@ -764,9 +771,14 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
         int per_sm = 0, sms = 148;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device);
         cudaFuncSetAttribute(k_spread_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             16 * 16 * 3 * 16 * (int)sizeof(float) + TILE_WARPS * 2 * SPREAD_PIECE_BYTES);
+                             (int)spread_tiles_smem(ChunkGeom{1, CHUNK_ENT_MAX}));
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spread_tiles, TILE_WARPS * 32, spread_tiles_smem(h->cg));
         h->rows_grid = std::max(1, per_sm) * sms;
+        cudaFuncSetAttribute(k_spread_tiles_block, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)spread_tiles_block_smem(ChunkGeom{1, CHUNK_ENT_MAX}));
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spread_tiles_block, BTILE_WARPS * 32,
+                                                      spread_tiles_block_smem(h->cg));
+        h->rows_block_grid = std::max(1, per_sm) * sms;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_stream_collide_words, 256, 0);
         h->words_grid = std::max(1, per_sm) * sms;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moments_active, 256, 0);
