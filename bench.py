@@ -4,8 +4,9 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload W4] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path: one time step of the coupled scheme (kinematics, marker
-sort + bins, moments on active cells, mdf_iters x (interpolate, correct, spread), fused
-stream-collide-force).  The default workload is W4 (BASELINE.json configs[3], 256^3 periodic, 64
+sort + chunks + tiles, moments on active cells, mdf_iters x (interpolate, correct, spread), fused
+stream-collide-force), replayed as one CUDA graph whose branches overlap the MDF loop, the
+stream-collide of the cells outside the marker stencils and the binning of the next step.  The default workload is W4 (BASELINE.json configs[3], 256^3 periodic, 64
 three-blade propellers, ~1.18 M markers, 5 MDF iterations): the coupled configuration on the same
 256^3 lattice as the pure-LBM bandwidth case configs[1] (W2), which is timed alongside and reported
 under "pure_lbm".  All inputs are seeded synthetic (paper_1904_02108_b200/workloads.py).
@@ -178,11 +179,8 @@ def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", local))
+    from paper_1904_02108_b200 import replicas
+    dist = replicas.init("nccl", rank, world, device=torch.device("cuda", local))
 
     from paper_1904_02108_b200 import api, workloads
     wl = workloads.get(args.workload, args.seed)
@@ -194,8 +192,7 @@ def run_ours(args):
 
     def barrier():
         torch.cuda.synchronize()
-        if dist is not None:
-            dist.barrier()
+        replicas.barrier(dist)
         torch.cuda.synchronize()
 
     # ---- device-resident timing (the headline `value`) ------------------------------------------
@@ -208,11 +205,8 @@ def run_ours(args):
     launches = sim.get_info(api.INFO_LAUNCHES) - l0
     clocks = sampler.stop() if sampler else {}
     sim.sync()
-    t = torch.tensor([ms], device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
-    value = world * wl.cells * args.steps / (ms * 1e-3) / 1e6
+    ms = replicas.max_over_ranks(ms, dist, device="cuda")
+    value = replicas.whole_job_mlups(wl.cells, args.steps, world, ms)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -226,28 +220,45 @@ def run_ours(args):
     }
 
     if rank == 0:
-        # ---- per-phase device time with CUDA events on the launching stream ----------------------
+        # ---- the same step as one serial chain with a single fused stream-collide pass (comparison) -----
+        if wl.n_markers:
+            sim.set_option(api.OPT_OVERLAP, 0)
+            sim.step(3, mdf)
+            ms_serial = time_steps(torch, sim, stream, args.steps, mdf)
+            sim.set_option(api.OPT_OVERLAP, 1)
+            line["serial_chain"] = {"value": wl.cells * args.steps / (ms_serial * 1e-3) / 1e6, "unit": UNIT,
+                                    "ms_per_step": ms_serial / args.steps,
+                                    "what": "LBM_OPT_OVERLAP=0: one stream, one fused stream-collide pass"}
+        # ---- per-phase device time with CUDA events on the launching stream (phases run one after the other) --
         n_ph = max(3, min(args.steps, 20))
         sim.set_option(api.OPT_TIMING, 1)
         sim.step(n_ph, mdf)
         ph = sim.phase_ms()
         sim.set_option(api.OPT_TIMING, 0)
         n_active = sim.get_info(api.INFO_ACTIVE_CELLS) if wl.n_markers else 0
+        n_words = sim.get_info(api.INFO_ACTIVE_WORDS) if wl.n_markers else 0
         lbm_ms = ph["lbm"] / n_ph
         tot = sum(ph.values()) / n_ph
         peak, how = measured_peak_gbs()
-        alg_bytes = BYTES_PER_LUP * wl.cells + G_BYTES_PER_ACTIVE * n_active
+        # the dominant kernel is the stream-collide pass over every 32-cell word without an active cell
+        # (k_stream_collide_scalar<LBM_BULK>; with no markers: <LBM_PURE> over all cells): 152 B per cell it updates
+        word_cells = min(wl.cells, n_words * 32)
+        alg_bytes = BYTES_PER_LUP * (wl.cells - word_cells)
         achieved = alg_bytes / (lbm_ms * 1e-3) / 1e9
-        line["roofline"] = {"bound": "hbm", "kernel": "k_stream_collide (a8)", "achieved": achieved, "peak": peak,
+        line["roofline"] = {"bound": "hbm", "kernel": "k_stream_collide_scalar<%s> (a8)" % ("LBM_BULK" if wl.n_markers else "LBM_PURE"),
+                            "achieved": achieved, "peak": peak,
                             "unit": "GB/s", "frac": achieved / peak, "traffic": traffic_from_profile(wl.name),
                             "peak_source": how, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
-                            "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": lbm_ms}
+                            "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": lbm_ms,
+                            "cells_per_launch": int(wl.cells - word_cells)}
         line["phases_ms_per_step"] = {k: v / n_ph for k, v in ph.items()}
-        line["ibm_share"] = (tot - lbm_ms) / tot if tot > 0 else 0.0
+        line["phases_note"] = "phases timed one after the other (LBM_OPT_TIMING); in the timed step they overlap"
         line["active_cells"] = int(n_active)
+        line["active_word_cells"] = int(word_cells)
         if wl.n_markers:
-            line["runs"] = sim.get_info(api.INFO_RUNS)
-            line["run_entries"] = sim.get_info(api.INFO_RUN_ENTRIES)
+            line["chunks"] = sim.get_info(api.INFO_RUNS)
+            line["chunk_entries"] = sim.get_info(api.INFO_RUN_ENTRIES)
+            line["tiles"] = sim.get_info(api.INFO_TILES)
 
         # ---- pure LBM on the same lattice and on configs[1] (W2) ---------------------------------
         sim.step(3, 0)
@@ -257,6 +268,8 @@ def run_ours(args):
                             "frac_of_measured": pure_same * 1e6 * BYTES_PER_LUP / 1e9 / peak,
                             "frac_of_nominal_8TBs": pure_same * 1e6 * BYTES_PER_LUP / 1e9 / NOMINAL_HBM_GBS,
                             "coupled_over_pure": value / world / pure_same}
+        # share of the coupled step that the IBM adds on top of a pure-LBM step of the same lattice
+        line["ibm_share"] = max(0.0, 1.0 - (ms_p / args.steps) / (ms / args.steps))
         if wl.name != "W2" and not args.quick:
             w2 = workloads.get("W2", args.seed)
             s2 = api.from_workload(w2, stream=stream)
@@ -304,11 +317,8 @@ def run_ours(args):
         e2e_step()
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
-    t = torch.tensor([dt], device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    dt = float(t.item())
-    line["e2e"] = {"value": world * wl.cells * e2e_steps / dt / 1e6, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+    dt = replicas.max_over_ranks(dt, dist, device="cuda")
+    line["e2e"] = {"value": replicas.whole_job_mlups(wl.cells, e2e_steps, world, dt * 1e3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                    "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
                    "what": "per step: kinematics table H2D, one coupled step, marker forces D2H (pinned)"
                    if wl.n_markers else "per step: u field H2D (set_fields), one step, rho+u D2H (pinned)"}
@@ -326,9 +336,7 @@ def run_ours(args):
                                 "cores": os.cpu_count() or 1, "kind": "oracle", "sample": sample}
     if rank == 0:
         print(json.dumps(line))
-    if dist is not None:
-        dist.barrier()
-        dist.destroy_process_group()
+    replicas.finish(dist)
     return 0
 
 

@@ -88,6 +88,8 @@ enum {
     LBM_INFO_RUNS = 8,          /* marker chunks (markers of one row and one 8-cell x block) in the last step */
     LBM_INFO_RUN_ENTRIES = 9,   /* window cells (profile entries) over all chunks in the last step  */
     LBM_INFO_TILES = 10,        /* tiles (chunks of one x block and one 4x4 block of rows) in the last step */
+    LBM_INFO_ACTIVE_WORDS = 11, /* 32-cell words of the active mask that hold an active cell (the cells the
+                                   second stream-collide pass of the overlapped step updates)          */
     LBM_INFO_PHASE_NS = 100     /* + phase: accumulated device time in ns under LBM_OPT_TIMING.
                                    phases: 0 kinematics+keys, 1 sort, 2 gather+bins, 3 moments on
                                    active cells, 4 interpolation+correction, 5 spreading,

@@ -23,7 +23,7 @@ _L = C.CDLL(LIB_PATH)
 
 OPT_SPREAD, OPT_FORCING, OPT_GRAPH, OPT_LBM_KERNEL, OPT_INTERP, OPT_TIMING, OPT_OVERLAP = 1, 2, 3, 4, 5, 6, 7
 INFO_MARKERS, INFO_BODIES, INFO_STEPS, INFO_LAUNCHES, INFO_ACTIVE_CELLS, INFO_DEVICE_BYTES, INFO_STATUS = range(1, 8)
-INFO_RUNS, INFO_RUN_ENTRIES, INFO_TILES = 8, 9, 10
+INFO_RUNS, INFO_RUN_ENTRIES, INFO_TILES, INFO_ACTIVE_WORDS = 8, 9, 10, 11
 INFO_PHASE_NS = 100
 PHASES = ["keys", "sort", "bins", "moments", "interp", "spread", "lbm", "lbm_active"]
 SPREAD_GATHER, SPREAD_ATOMIC, SPREAD_GATHER_PLAIN = 0, 1, 2

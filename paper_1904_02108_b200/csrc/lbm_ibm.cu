@@ -841,11 +841,12 @@ int lbm_get_info(lbm_t *h, int key, long long *value)
         case LBM_INFO_STEPS: *value = h->steps_done; return LBM_OK;
         case LBM_INFO_LAUNCHES: *value = h->launches; return LBM_OK;
         case LBM_INFO_DEVICE_BYTES: *value = (long long)h->dev_bytes; return LBM_OK;
-        case LBM_INFO_ACTIVE_CELLS: case LBM_INFO_RUNS: case LBM_INFO_RUN_ENTRIES: case LBM_INFO_TILES: {
+        case LBM_INFO_ACTIVE_CELLS: case LBM_INFO_RUNS: case LBM_INFO_RUN_ENTRIES: case LBM_INFO_TILES:
+        case LBM_INFO_ACTIVE_WORDS: {
             int r = 0;
             if (h->force_valid && h->last_set >= 0) {
                 const SetScalars *sc = h->set[h->last_set].scal;
-                const int *p = key == LBM_INFO_ACTIVE_CELLS ? &sc->n_cells : (key == LBM_INFO_RUNS ? &sc->n_chunks : (key == LBM_INFO_TILES ? &sc->n_tiles : &sc->n_entries));
+                const int *p = key == LBM_INFO_ACTIVE_CELLS ? &sc->n_cells : (key == LBM_INFO_RUNS ? &sc->n_chunks : (key == LBM_INFO_TILES ? &sc->n_tiles : (key == LBM_INFO_ACTIVE_WORDS ? &sc->n_words : &sc->n_entries)));
                 CK(cudaMemcpyAsync(&r, p, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
                 CK(cudaStreamSynchronize(h->stream));
             }

@@ -70,9 +70,8 @@ def _frame_from_axis(axis: np.ndarray) -> np.ndarray:
 
 
 def propeller(n_blades: int, radius: float, width: float, layers: int, psi0: float,
-              axis, center, omega: float) -> Body:
-    """Flat-plate propeller markers in the lab frame (see module docstring)."""
-    h = H_SPACING
+              axis, center, omega: float, h: float = H_SPACING) -> Body:
+    """Flat-plate propeller markers in the lab frame (see module docstring); h = marker spacing."""
     beta = np.deg2rad(PITCH_DEG)
     na = int(round(radius / h))
     nb = int(round(width / h))
@@ -197,8 +196,26 @@ def w5(seed: int = 0, layers: int = 12, n: int = 512, n_bodies: int | None = Non
                     note="configs[4]: extreme density, periodic")
 
 
+def paper_case(n_bodies: int, seed: int = 0) -> Workload:
+    """the shape of the paper's own test cases: a 160 x 160 x 320 lattice
+    with 1, 6 or 18 rotating propellers of about 3930 Lagrangian points each whose area is about one
+    cell face (spacing 1, s = 1), 5 MDF iterations.  The paper's Blender mesh is not in the
+    container: a three-blade flat-plate propeller (R = 41, w = 32: 3936 points) stands in for it; the
+    bodies sit on the long axis of the box at equal distances, as in the paper's Fig. 4.  The paper
+    states neither tau, omega nor the boundary: tau = 0.7, omega = 0.002, periodic (R15)."""
+    rng = np.random.default_rng(seed)
+    bodies = []
+    for i in range(n_bodies):
+        c = np.array([80.0, 80.0, 320.0 * (i + 0.5) / n_bodies])
+        psi0 = float(rng.uniform(0.0, 2.0 * np.pi))
+        bodies.append(propeller(3, 41.0, 32.0, 1, psi0, [0.0, 0.0, 1.0], c, 0.002 * (1 if i % 2 == 0 else -1), h=1.0))
+    return Workload(f"P{n_bodies}", 160, 160, 320, 0.7, (0, 0, 0), (0.0, 0.0, 0.0), bodies, steps=1000, mdf_iters=5,
+                    note="SURVEY 8(f3): paper-shaped case, 160x160x320, %d propellers x 3936 points" % n_bodies)
+
+
 def get(name: str, seed: int = 0) -> Workload:
-    """Named workloads: W1, W2, W3, W3lit, W4, W4lit, W5, W5lit (lit = single layer, 'literal')."""
+    """Named workloads: W1, W2, W3, W3lit, W4, W4lit, W5, W5lit (lit = single layer, 'literal');
+    P1, P6, P18 = the paper-shaped cases of SURVEY 8(f3)."""
     table = {
         "W1": lambda: w1(seed),
         "W2": lambda: w2(seed),
@@ -208,6 +225,9 @@ def get(name: str, seed: int = 0) -> Workload:
         "W4lit": lambda: w4(seed, 1),
         "W5": lambda: w5(seed, 12),
         "W5lit": lambda: w5(seed, 1),
+        "P1": lambda: paper_case(1, seed),
+        "P6": lambda: paper_case(6, seed),
+        "P18": lambda: paper_case(18, seed),
     }
     if name not in table:
         raise KeyError(f"unknown workload {name!r}; choose from {sorted(table)}")

@@ -115,3 +115,15 @@ def test_w5_full_512_parity_5_steps_and_properties(api):
     e = _parity(api, wl, 5)
     print("W5 full errors (u, rho):", e)
     _properties(api, wl, 20)
+
+
+def test_paper_shaped_case_p6_parity_and_p18_properties(api):
+    """the paper's 160 x 160 x 320 box with 6 propellers of 3936 points
+    (spacing 1, s = 1): 20 steps against the oracle on every cell and marker; 18 propellers (the
+    paper's extreme case, 70,848 points): properties over 50 steps.  nx = 160 is a multiple of 32,
+    ny = 160, nz = 320 of 4: the two-candidate collect path; s = 1 makes the MDF iteration matrix
+    the stiffest of all workloads."""
+    from paper_1904_02108_b200 import workloads
+    e = _parity(api, workloads.get("P6"), 20)
+    print("P6 errors (u, rho):", e)
+    _properties(api, workloads.get("P18"), 50)

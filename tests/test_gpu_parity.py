@@ -241,6 +241,52 @@ def test_static_markers_with_prescribed_velocity_and_walls(api, orc):
     sim.close()
 
 
+@pytest.mark.parametrize("shape,wall", [((19, 13, 10), (0, 0, 0)),     # nx % 8 = 3: widened last x block; ny % 4 = 1, nz % 4 = 2: third tile
+                                        ((9, 5, 6), (0, 0, 0)),       # narrower than a chunk window: windows wrap onto themselves
+                                        ((27, 9, 18), (0, 1, 0)),     # wall on y with ny % 4 = 1
+                                        ((40, 8, 4), (0, 0, 0)),      # one tile in z, periodic
+                                        ((12, 12, 12), (1, 1, 1))])   # all walls, one and a half x blocks
+def test_odd_lattices_chunk_and_tile_edges(api, orc, shape, wall):
+    """moving and static markers everywhere in small, odd-sized boxes: every wrap / widened-block /
+    third-tile branch of the chunk and tile code against the oracle (and the atomic variant)."""
+    rng = np.random.default_rng(5)
+    nx, ny, nz = shape
+    lo = [1.0 if w else 0.0 for w in wall]
+    hi = [n - 2.001 if w else float(n) for n, w in zip(shape, wall)]
+    outs = []
+    for variant in (api.SPREAD_GATHER, api.SPREAD_ATOMIC):
+        sim = api.LbmIbm(nx, ny, nz, 0.8, wall=wall, stream=_stream())
+        sim.set_option(api.OPT_SPREAD, variant)
+        ref = orc.Oracle(nx, ny, nz, 0.8, wall=wall) if variant == api.SPREAD_GATHER else None
+        rng = np.random.default_rng(5)
+        for b in range(3):
+            n = 120
+            pos = np.stack([rng.uniform(lo[a], hi[a], n) for a in range(3)], axis=1).astype(np.float32)
+            vel = rng.normal(scale=0.02, size=(n, 3)).astype(np.float32)
+            area = rng.uniform(0.05, 0.2, size=n).astype(np.float32)
+            sim.set_markers(pos, vel, area)
+            if ref is not None:
+                ref.set_markers(pos, vel, area)
+            if b == 2 and not any(wall):
+                c = np.array([nx / 2.0, ny / 2.0, nz / 2.0])
+                sim.set_kinematics(0.01, [0.3, -0.5, 0.8], c)
+                if ref is not None:
+                    ref.set_kinematics(0.01, [0.3, -0.5, 0.8], c)
+        sim.step(12, 3)
+        sim.sync()
+        if ref is not None:
+            ref.step(12, 3)
+            _compare_fields(sim, ref)
+            mk, rm = sim.read_markers(), ref.read_markers()
+            assert np.abs(mk["force"] - rm["du"]).max() <= TOL_F * np.abs(rm["du"]).max()
+            _, _, f = sim.read_fields()
+            _, _, rf = ref.read_fields()
+            assert np.abs(f - rf).max() <= 1e-5 * np.abs(rf).max()
+        outs.append(sim.read_fields()[1])
+        sim.close()
+    assert np.abs(outs[0] - outs[1]).max() <= 5e-7
+
+
 def test_error_paths(api):
     with pytest.raises(api.LbmError):
         api.LbmIbm(8, 8, 8, 0.5)
