@@ -1008,7 +1008,7 @@ k_spread_tiles_block(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int 
                         az.x += vz.x; az.y += vz.y; az.z += vz.z; az.w += vz.w;
                     }
                 float4 *__restrict__ Ft = F + ((size_t)t * (TILE_F * TILE_F) + r_fy * TILE_F + r_fz) * ent + 4 * r_e4;
-                const unsigned mx = m >> (4 * r_e4);
+                const unsigned mx = (m & ((1u << ent) - 1u)) >> (4 * r_e4);   // x bits only (bits 14.. are rows)
                 if (mx & 1u) Ft[0] = make_float4(ax.x, ay.x, az.x, 0.f);
                 if (mx & 2u) Ft[1] = make_float4(ax.y, ay.y, az.y, 0.f);
                 if (mx & 4u) Ft[2] = make_float4(ax.z, ay.z, az.z, 0.f);
