@@ -666,6 +666,39 @@ k_tile_fill(Geom g, ChunkGeom cg, TileGeom tg, ChunkTable ct, const int *__restr
     }
 }
 
+// a3: order the tiles by decreasing marker count (8 size classes: >= 1024, >= 512, ... , < 16), so that the
+// sweep, which hands tiles out through a cursor, starts the long ones first and ends on short ones
+// (longest-processing-time-first; the order inside a class is arbitrary).  Two passes: count per
+// class, then place.  bucket[0..7] = class counts, bucket[8..15] = fill cursors.
+__device__ __forceinline__ int tile_size_class(const int2 *__restrict__ rec)
+{
+    int n = 0;
+#pragma unroll
+    for (int r = 0; r < 16; ++r) { const int2 v = __ldg(rec + r); n += v.y - v.x; }
+    const int c = 27 - __clz(max(n, 1));       // floor(log2 n) - 4
+    return 7 - min(max(c, 0), 7);              // class 0 = largest
+}
+
+__global__ void __launch_bounds__(256)
+k_tile_count(TileTable tt, const int *__restrict__ n_tiles, int tile_cap, int *__restrict__ bucket)
+{
+    const int nt = min(*n_tiles, tile_cap);
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < nt; t += gridDim.x * blockDim.x)
+        atomicAdd(bucket + tile_size_class(tt.rec + (size_t)t * 16), 1);
+}
+
+__global__ void __launch_bounds__(256)
+k_tile_place(TileTable tt, const int *__restrict__ n_tiles, int tile_cap, int *__restrict__ bucket, int *__restrict__ order)
+{
+    const int nt = min(*n_tiles, tile_cap);
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < nt; t += gridDim.x * blockDim.x) {
+        const int c = tile_size_class(tt.rec + (size_t)t * 16);
+        int base = 0;
+        for (int q = 0; q < c; ++q) base += bucket[q];
+        order[base + atomicAdd(bucket + 8 + c, 1)] = t;
+    }
+}
+
 // ---- asynchronous bulk copies global -> shared (TMA, 1-D) completing on an mbarrier ---------------
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned long long *bar, int count)
@@ -735,8 +768,8 @@ inline size_t spread_tiles_smem(const ChunkGeom &cg) { return (size_t)TILE_WARPS
 __global__ void __launch_bounds__(TILE_WARPS * 32, TILE_MINB_CFG)
 k_spread_tiles(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int *__restrict__ tile_slot,
                const unsigned *__restrict__ tile_mask, const int *__restrict__ n_tiles, int tile_cap,
-               int *__restrict__ cursor, const float4 *__restrict__ wx4, const float *__restrict__ wyz16,
-               const float4 *__restrict__ val, float4 *__restrict__ F, int warp_smem)
+               int *__restrict__ cursor, const int *__restrict__ order, const float4 *__restrict__ wx4,
+               const float *__restrict__ wyz16, const float4 *__restrict__ val, float4 *__restrict__ F, int warp_smem)
 {
     extern __shared__ __align__(128) char smem[];
     __shared__ unsigned long long s_bar[TILE_WARPS][SPREAD_STAGES];
@@ -756,7 +789,7 @@ k_spread_tiles(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int *__res
     const int jy = l >> 2, jz = l & 3;
     for (;;) {
         int t = 0;
-        if (lane == 0) t = atomicAdd(cursor, 1);
+        if (lane == 0) { t = atomicAdd(cursor, 1); t = t < nt ? __ldg(order + t) : nt; }
         t = __shfl_sync(0xffffffffu, t, 0);
         if (t >= nt) break;
         // lane r < 16: sorted-marker range of the chunk in source row r = sy + 4 sz ((0,0) = none)

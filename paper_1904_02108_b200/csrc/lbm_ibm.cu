@@ -62,8 +62,9 @@ struct SetScalars {
     int n_cells;         // active cells
     int n_tiles;         // tiles (may exceed the capacity: the excess is dropped and flagged)
     int cursor[MAX_MDF]; // work cursors of the tile sweeps, one per MDF iteration
+    int bucket[16];      // tile size classes: counts [0..7] and fill cursors [8..15] (k_tile_count / k_tile_place)
 };
-constexpr int N_STEP_COUNTERS = 5 + MAX_MDF;
+constexpr int N_STEP_COUNTERS = 5 + MAX_MDF + 16;
 
 struct HostBody {
     long long first, count;
@@ -111,6 +112,7 @@ struct PrepSet {
     MarkerSorted ms{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     ChunkTable ct{nullptr, nullptr, nullptr};
     TileTable tt{nullptr, nullptr, nullptr, nullptr};  // mask, id: dense over the tile slots; slot, rec: per tile
+    int *tile_order = nullptr;                // tiles by decreasing marker count (size classes)
     unsigned *headbits = nullptr;             // one bit per sorted marker: starts a run
     int *cells = nullptr;                     // active-cell list
     // dense maps, cleared incrementally by the set's next preparation (k_clear_prev)
@@ -217,6 +219,7 @@ void free_set(lbm *h, PrepSet &S)
     dfree(h, S.ct.slot, (size_t)h->chunk_cap);
     dfree(h, S.tt.slot, (size_t)h->tile_cap);
     dfree(h, S.tt.rec, (size_t)h->tile_cap * 16);
+    dfree(h, S.tile_order, (size_t)h->tile_cap);
     dfree(h, S.cells, h->cells_cap);
     dfree(h, S.headbits, h->headbits_cap);
     S.step = -1;
@@ -328,6 +331,7 @@ int upload_markers(lbm *h)
             if ((rc = dmalloc(h, &S.ct.slot, (size_t)ccap))) return rc;
             if ((rc = dmalloc(h, &S.tt.slot, tcap))) return rc;
             if ((rc = dmalloc(h, &S.tt.rec, tcap * 16))) return rc;
+            if ((rc = dmalloc(h, &S.tile_order, tcap))) return rc;
             if ((rc = dmalloc(h, &S.cells, h->cells_cap))) return rc;
             if ((rc = dmalloc(h, &S.headbits, h->headbits_cap))) return rc;
         }
@@ -435,7 +439,9 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
         k_tiles<<<LIST_GRID, 256, 0, s>>>(g, h->cg, h->tg, S.ct, &sc->n_chunks, h->chunk_cap, S.chunk_of, S.tt, h->tile_cap,
                                           &sc->n_tiles, &h->scal->status);
         k_tile_fill<<<LIST_GRID, 256, 0, s>>>(g, h->cg, h->tg, S.ct, &sc->n_chunks, h->chunk_cap, S.tt);
-        nk += 5;
+        k_tile_count<<<LIST_GRID, 256, 0, s>>>(S.tt, &sc->n_tiles, h->tile_cap, sc->bucket);
+        k_tile_place<<<LIST_GRID, 256, 0, s>>>(S.tt, &sc->n_tiles, h->tile_cap, sc->bucket, S.tile_order);
+        nk += 7;
     } else {
         k_bins<<<mb, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask, S.words, &sc->n_words);
         ++nk;
@@ -473,8 +479,8 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
                     last ? S.ms.du : S.ms.sg, h->F);
             else
                 k_spread_tiles<<<h->rows_grid, TILE_WARPS * 32, spread_tiles_smem(h->cg), s>>>(
-                    h->cg, S.tt.rec, S.tt.slot, S.tt.mask, &sc->n_tiles, h->tile_cap, &sc->cursor[m], S.ms.wx, S.ms.wyz,
-                    last ? S.ms.du : S.ms.sg, h->F, (int)spread_warp_smem(h->cg));
+                    h->cg, S.tt.rec, S.tt.slot, S.tt.mask, &sc->n_tiles, h->tile_cap, &sc->cursor[m], S.tile_order, S.ms.wx,
+                    S.ms.wyz, last ? S.ms.du : S.ms.sg, h->F, (int)spread_warp_smem(h->cg));
             const bool two = (g.wallx || g.nx >= CHUNK_ENT_MAX) && (g.wally || g.ny % TILE_R == 0) &&
                              (g.wallz || g.nz % TILE_R == 0);
             auto collect = last ? (two ? k_collect_tiles<true, 2> : k_collect_tiles<true, 4>)
