@@ -229,6 +229,28 @@ def run_ours(args):
             line["serial_chain"] = {"value": wl.cells * args.steps / (ms_serial * 1e-3) / 1e6, "unit": UNIT,
                                     "ms_per_step": ms_serial / args.steps,
                                     "what": "LBM_OPT_OVERLAP=0: one stream, one fused stream-collide pass"}
+        # ---- the paper's own kernel designs on the same step, one option at a time ---------
+        if wl.n_markers and args.compare:
+            cmp_steps = max(3, min(args.steps, 20))
+            variants = [("moments_box(P:209)", {api.OPT_MOMENTS: api.MOMENTS_BOX}),
+                        ("moments_block_per_marker(P:215)", {api.OPT_MOMENTS: api.MOMENTS_PER_MARKER}),
+                        ("interp_caller_order(ib_force1)", {api.OPT_INTERP: api.INTERP_CALLER_ORDER}),
+                        ("spread_atomic_thread_per_marker", {api.OPT_SPREAD: api.SPREAD_ATOMIC}),
+                        ("spread_block125_atomic(ib_force2)", {api.OPT_SPREAD: api.SPREAD_BLOCK125}),
+                        ("paper_pipeline(box+ib_force1+ib_force2,serial)",
+                         {api.OPT_MOMENTS: api.MOMENTS_BOX, api.OPT_INTERP: api.INTERP_CALLER_ORDER,
+                          api.OPT_SPREAD: api.SPREAD_BLOCK125, api.OPT_OVERLAP: 0})]
+            defaults = {api.OPT_MOMENTS: 0, api.OPT_INTERP: 0, api.OPT_SPREAD: 0, api.OPT_OVERLAP: 1}
+            comp = {"default": ms / args.steps}
+            for name, opts in variants:
+                for k, v in opts.items():
+                    sim.set_option(k, v)
+                sim.step(3, mdf)
+                comp[name] = time_steps(torch, sim, stream, cmp_steps, mdf) / cmp_steps
+                for k, v in defaults.items():
+                    sim.set_option(k, v)
+            sim.step(2, mdf)
+            line["comparisons_ms_per_step"] = comp
         # ---- per-phase device time with CUDA events on the launching stream (phases run one after the other) --
         n_ph = max(3, min(args.steps, 20))
         sim.set_option(api.OPT_TIMING, 1)
@@ -353,6 +375,8 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=10)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--quick", action="store_true", help="skip the extra W2 pure-LBM run")
+    ap.add_argument("--compare", action="store_true",
+                    help="also time the paper's own kernel designs (box / per-marker U precompute, ib_force1, ib_force2)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else max(args.warmup, 0)
     if args.impl == "reference":

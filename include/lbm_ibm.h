@@ -56,24 +56,32 @@ enum {
 
 /* Options for lbm_set_option. */
 enum {
-    LBM_OPT_SPREAD = 1,   /* 0 = deterministic run-sweep + gather-by-cell (default), 1 = global atomics
-                             (the paper's ib_force2 design; kept as a measured comparison),
-                             2 = plain gather-by-cell over the bins (slow reference variant)        */
+    LBM_OPT_SPREAD = 1,   /* 0 = deterministic chunk sweep + tile footprints + gather-by-cell (default),
+                             1 = global atomics, one thread per marker (measured comparison),
+                             2 = plain gather-by-cell over the bins (slow reference variant),
+                             3 = the paper's ib_force2 as printed: a block of 5^3 threads per marker with
+                             atomicAdd (Alg.2; measured comparison)                      */
     LBM_OPT_FORCING = 2,  /* 0 = Guo source term (default, R3), 1 = paper's shift U + tau G */
     LBM_OPT_GRAPH = 3,    /* 1 = replay the step as a CUDA graph (default), 0 = plain launches     */
     LBM_OPT_LBM_KERNEL = 4, /* stream-collide variant: 0 = default, 1 = one cell per thread (the default),
                              2 = four cells per thread with 128-bit accesses (nx % 4 == 0; comparison;
                              used for the pure and the serial fused pass only)                     */
-    LBM_OPT_INTERP = 5,   /* interpolation variant: 0 = default, 1 = thread per marker            */
+    LBM_OPT_INTERP = 5,   /* interpolation: 0 = thread per marker in sorted order (default), 1 = the paper's
+                             ib_force1 access pattern: thread per marker in the caller's order, no reordering
+                             (Alg.1; measured comparison)                                  */
     LBM_OPT_TIMING = 6,   /* 1 = run steps as plain launches with CUDA events between the phases and
                              accumulate per-phase device time (LBM_INFO_PHASE_NS); setting it resets
                              the accumulators.  Each step then ends with a stream synchronise.     */
-    LBM_OPT_OVERLAP = 7   /* 1 (default) = a coupled step runs as three concurrent graph branches: the
+    LBM_OPT_OVERLAP = 7,  /* 1 (default) = a coupled step runs as three concurrent graph branches: the
                              MDF loop, the stream-collide of every cell outside the marker stencils
                              (it needs no IBM force), and the binning of the NEXT step's markers (P:154:
                              positions depend on time only); the cells inside the stencils are updated
                              after the join.  0 = the same step as one serial chain with a single fused
                              stream-collide pass (measured comparison).  Results are identical.        */
+    LBM_OPT_MOMENTS = 8   /* where U is precomputed for the IBM: 0 = the de-duplicated list of
+                             cells inside a marker stencil (default), 1 = the paper's box strategy (bounding
+                             box of every body), 2 = the paper's kernel strategy (a block per Lagrangian
+                             point, duplicates included).  Results are identical.                      */
 };
 
 /* Keys for lbm_get_info. */

@@ -21,12 +21,14 @@ if not os.path.exists(LIB_PATH):
 
 _L = C.CDLL(LIB_PATH)
 
-OPT_SPREAD, OPT_FORCING, OPT_GRAPH, OPT_LBM_KERNEL, OPT_INTERP, OPT_TIMING, OPT_OVERLAP = 1, 2, 3, 4, 5, 6, 7
+OPT_SPREAD, OPT_FORCING, OPT_GRAPH, OPT_LBM_KERNEL, OPT_INTERP, OPT_TIMING, OPT_OVERLAP, OPT_MOMENTS = 1, 2, 3, 4, 5, 6, 7, 8
 INFO_MARKERS, INFO_BODIES, INFO_STEPS, INFO_LAUNCHES, INFO_ACTIVE_CELLS, INFO_DEVICE_BYTES, INFO_STATUS = range(1, 8)
 INFO_RUNS, INFO_RUN_ENTRIES, INFO_TILES, INFO_ACTIVE_WORDS = 8, 9, 10, 11
 INFO_PHASE_NS = 100
 PHASES = ["keys", "sort", "bins", "moments", "interp", "spread", "lbm", "lbm_active"]
-SPREAD_GATHER, SPREAD_ATOMIC, SPREAD_GATHER_PLAIN = 0, 1, 2
+SPREAD_GATHER, SPREAD_ATOMIC, SPREAD_GATHER_PLAIN, SPREAD_BLOCK125 = 0, 1, 2, 3
+MOMENTS_LIST, MOMENTS_BOX, MOMENTS_PER_MARKER = 0, 1, 2
+INTERP_SORTED, INTERP_CALLER_ORDER = 0, 1
 FORCING_GUO, FORCING_SHIFT = 0, 1
 
 EXPORTS = ["lbm_create", "lbm_destroy", "lbm_set_stream", "lbm_set_option", "lbm_get_info", "lbm_set_fields",

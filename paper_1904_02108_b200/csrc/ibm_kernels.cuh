@@ -1206,4 +1206,172 @@ k_read_markers(const unsigned *__restrict__ skey, const int *__restrict__ perm, 
     if (cell) cell[k] = (int)key;
 }
 
+// =================================================================================================
+// The paper's own kernel designs, kept as measured comparisons; none of them
+// is on the default path.  They produce the same fields as the product kernels (U bit-identical,
+// atomics up to summation order).
+
+// general Peskin 4-point kernel w(r) (R6), used where the stencil offset is not known at compile time
+__device__ __forceinline__ float peskin_w(float r)
+{
+    const float a = fabsf(r);
+    if (a >= 2.0f) return 0.0f;
+    if (a <= 1.0f) return 0.125f * (3.0f - 2.0f * a + sqrtf(fmaf(4.0f * a, 1.0f - a, 1.0f)));
+    return 0.125f * (5.0f - 2.0f * a - sqrtf(fmaf(-4.0f * a, a, fmaf(12.0f, a, -7.0f))));
+}
+
+// inverse of the sort permutation: inv[original index] = sorted index
+__global__ void __launch_bounds__(256)
+k_invert_perm(const int *__restrict__ perm, int n, int *__restrict__ inv)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) inv[perm[i]] = i;
+}
+
+// f4, ib_force1 as the paper has it (Alg.1): one thread per Lagrangian point in the
+// CALLER's order, no reordering, so neighbouring threads gather from unrelated places (P:152
+// "memory accesses are often not coalesced").  Same arithmetic as k_interp_correct.
+__global__ void __launch_bounds__(128)
+k_interp_caller_order(const unsigned *__restrict__ skey, const int *__restrict__ inv, int n, Geom g,
+                      const float4 *__restrict__ U, MarkerSorted m)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const int i = inv[k];
+    int cx, cy, cz;
+    key_to_cell(skey[i], g, cx, cy, cz);
+    const float4 fs = m.fs[i];
+    float wx[4], wy[4], wz[4];
+    peskin4(fs.x, wx);
+    peskin4(fs.y, wy);
+    peskin4(fs.z, wz);
+    float ux = 0.f, uy = 0.f, uz = 0.f;
+#pragma unroll
+    for (int jz = 0; jz < 4; ++jz) {
+        const int z = wrap(cz - 1 + jz, g.nz);
+#pragma unroll
+        for (int jy = 0; jy < 4; ++jy) {
+            const int y = wrap(cy - 1 + jy, g.ny);
+            const float wyz = wy[jy] * wz[jz];
+            const float4 *row = U + (size_t)(z * g.ny + y) * g.nx;
+#pragma unroll
+            for (int jx = 0; jx < 4; ++jx) {
+                const float4 v = row[wrap(cx - 1 + jx, g.nx)];
+                const float w = wx[jx] * wyz;
+                ux = fmaf(v.x, w, ux);
+                uy = fmaf(v.y, w, uy);
+                uz = fmaf(v.z, w, uz);
+            }
+        }
+    }
+    const float4 uk = m.uk[i];
+    const float gx = uk.x - ux, gy = uk.y - uy, gz = uk.z - uz;
+    float4 du = m.du[i];
+    du.x = fmaf(fs.w, gx, du.x);
+    du.y = fmaf(fs.w, gy, du.y);
+    du.z = fmaf(fs.w, gz, du.z);
+    m.du[i] = du;
+    m.sg[i] = make_float4(fs.w * gx, fs.w * gy, fs.w * gz, du.w);
+}
+
+// f4, ib_force2 as the paper has it (Alg.2): one CUDA block of 5 x 5 x 5 threads per
+// Lagrangian point, thread (a,b,c) adds the contribution to the cell round(x) + (a,b,c) - 2 with
+// atomicAdd.  At most 4 of the 5 weights per axis are non-zero (R7).
+__global__ void __launch_bounds__(125)
+k_spread_block125(const unsigned *__restrict__ skey, int n, Geom g, const float4 *__restrict__ fs,
+                  const float4 *__restrict__ val, float4 *__restrict__ field)
+{
+    const int i = blockIdx.x;
+    if (i >= n) return;
+    int cx, cy, cz;
+    key_to_cell(skey[i], g, cx, cy, cz);
+    const float4 f = fs[i];
+    const float4 v = val[i];
+    const int a = threadIdx.x % 5, b = (threadIdx.x / 5) % 5, c = threadIdx.x / 25;
+    // nearest cell round(x) = cell + (fraction >= 1/2); distance of the point to the thread's cell
+    const int rx = f.x >= 0.5f ? 1 : 0, ry = f.y >= 0.5f ? 1 : 0, rz = f.z >= 0.5f ? 1 : 0;
+    const int ox = rx + a - 2, oy = ry + b - 2, oz = rz + c - 2;
+    const float w = peskin_w(f.x - (float)ox) * peskin_w(f.y - (float)oy) * peskin_w(f.z - (float)oz);
+    if (w == 0.0f) return;
+    const int x = wrap(cx + ox, g.nx), y = wrap(cy + oy, g.ny), z = wrap(cz + oz, g.nz);
+    float *dst = reinterpret_cast<float *>(field + (size_t)(z * g.ny + y) * g.nx + x);
+    atomicAdd(dst + 0, v.x * w);
+    atomicAdd(dst + 1, v.y * w);
+    atomicAdd(dst + 2, v.z * w);
+}
+
+// f2, lbm_u_start "kernel strategy" as the paper has it: one CUDA block per Lagrangian
+// point computes U on the point's 4 x 4 x 4 neighbourhood; the same U(X) is computed by every
+// point whose neighbourhood holds X.
+__global__ void __launch_bounds__(64)
+k_moments_per_marker(const float *__restrict__ src, const __grid_constant__ Geom g, const unsigned *__restrict__ skey,
+                     int n, float4 *__restrict__ U)
+{
+    const int i = blockIdx.x;
+    if (i >= n) return;
+    int cx, cy, cz;
+    key_to_cell(skey[i], g, cx, cy, cz);
+    const int x = wrap(cx - 1 + (threadIdx.x & 3), g.nx);
+    const int y = wrap(cy - 1 + ((threadIdx.x >> 2) & 3), g.ny);
+    const int z = wrap(cz - 1 + (threadIdx.x >> 4), g.nz);
+    const Nbr nb = neighbours(g, x, y, z);
+    float df[NQ], drho, ux, uy, uz;
+    pull_cell(src, g, nb, x, y, z, df);
+    moments(df, drho, ux, uy, uz);
+    U[(size_t)(z * g.ny + y) * g.nx + x] = make_float4(ux, uy, uz, 1.0f + drho);
+}
+
+// f2, lbm_u_start "box strategy": U on the bounding box of every body.  The paper
+// transforms the rest-pose box; here the box is taken from the cells the body's markers occupy in
+// this step (tighter), widened by the stencil.  Boxes are kept unwrapped (they may straddle a
+// periodic face); box[b] = {xlo, ylo, zlo, xhi, yhi, zhi}.
+__global__ void __launch_bounds__(256)
+k_body_boxes(MarkerIn m, const BodyDef *__restrict__ defs, const BodyStep *__restrict__ tabs, int *__restrict__ box)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= m.n) return;
+    const int b = m.body[k];
+    const BodyDef d = defs[b];
+    const BodyStep t = tabs[b];
+    const float qx = m.qx[k], qy = m.qy[k], qz = m.qz[k];
+    const float dx = fmaf(t.R[0], qx, fmaf(t.R[1], qy, fmaf(t.R[2], qz, d.cf[0])));
+    const float dy = fmaf(t.R[3], qx, fmaf(t.R[4], qy, fmaf(t.R[5], qz, d.cf[1])));
+    const float dz = fmaf(t.R[6], qx, fmaf(t.R[7], qy, fmaf(t.R[8], qz, d.cf[2])));
+    const int cx = d.ci[0] + (int)floorf(dx), cy = d.ci[1] + (int)floorf(dy), cz = d.ci[2] + (int)floorf(dz);
+    int *bx = box + 6 * b;
+    atomicMin(bx + 0, cx - 1); atomicMin(bx + 1, cy - 1); atomicMin(bx + 2, cz - 1);
+    atomicMax(bx + 3, cx + 3); atomicMax(bx + 4, cy + 3); atomicMax(bx + 5, cz + 3);   // + 3: rounding of d - floor(d) (place_axis)
+}
+
+__global__ void k_reset_boxes(int *__restrict__ box, int nbodies)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nbodies) return;
+    for (int a = 0; a < 3; ++a) { box[6 * b + a] = 0x7fffffff; box[6 * b + 3 + a] = -0x7fffffff; }
+}
+
+// grid (blocks per body, bodies): the blocks of a body stride over the cells of its box
+__global__ void __launch_bounds__(256)
+k_moments_box(const float *__restrict__ src, const __grid_constant__ Geom g, const int *__restrict__ box,
+              float4 *__restrict__ U)
+{
+    const int *bx = box + 6 * blockIdx.y;
+    const int x0 = bx[0], y0 = bx[1], z0 = bx[2];
+    const int ex = min(bx[3] - x0 + 1, g.nx), ey = min(bx[4] - y0 + 1, g.ny), ez = min(bx[5] - z0 + 1, g.nz);
+    if (ex <= 0 || ey <= 0 || ez <= 0) return;
+    const long long total = (long long)ex * ey * ez;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < total; c += (long long)gridDim.x * blockDim.x) {
+        const int ix = (int)(c % ex), iy = (int)((c / ex) % ey), iz = (int)(c / ((long long)ex * ey));
+        int x = (x0 + ix) % g.nx, y = (y0 + iy) % g.ny, z = (z0 + iz) % g.nz;
+        if (x < 0) x += g.nx;
+        if (y < 0) y += g.ny;
+        if (z < 0) z += g.nz;
+        const Nbr nb = neighbours(g, x, y, z);
+        float df[NQ], drho, ux, uy, uz;
+        pull_cell(src, g, nb, x, y, z, df);
+        moments(df, drho, ux, uy, uz);
+        U[(size_t)(z * g.ny + y) * g.nx + x] = make_float4(ux, uy, uz, 1.0f + drho);
+    }
+}
+
 }  // namespace lbmk

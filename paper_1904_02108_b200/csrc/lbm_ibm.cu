@@ -73,7 +73,7 @@ struct HostBody {
 };
 
 constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driven kernels
-constexpr int SPREAD_BLOCK_BELOW = 100000;   // marker count below which the block-per-tile sweep is used (measured: W3 vs W4lit)
+constexpr int SPREAD_WARP_FROM_TILES = 1200;   // tile count from which the warp-per-tile sweep is used (W3: 160 tiles -> block, P6: 1460 -> warp)
 
 // Optional per-phase device timing (LBM_OPT_TIMING): CUDA events recorded on the launching stream
 // between the phases of a step; durations are accumulated after a stream synchronise.
@@ -113,6 +113,7 @@ struct PrepSet {
     ChunkTable ct{nullptr, nullptr, nullptr};
     TileTable tt{nullptr, nullptr, nullptr, nullptr};  // mask, id: dense over the tile slots; slot, rec: per tile
     int *tile_order = nullptr;                // tiles by decreasing marker count (size classes)
+    int *inv = nullptr;                       // inverse permutation (comparison LBM_OPT_INTERP = 1 only; lazy)
     unsigned *headbits = nullptr;             // one bit per sorted marker: starts a run
     int *cells = nullptr;                     // active-cell list
     // dense maps, cleared incrementally by the set's next preparation (k_clear_prev)
@@ -171,7 +172,9 @@ struct lbm {
     int sort_ipw = 64, sort_tiles = 0, sort_passes = 1;
 
     int opt_spread = 0, opt_forcing = 0, opt_graph = 1, opt_lbm_kernel = 0, opt_interp = 0, opt_timing = 0;
-    int opt_overlap = 1;
+    int opt_overlap = 1, opt_moments = 0;
+    int tiles_hint = -1;                // tile count of the first preparation after a marker upload (-1: not known yet)
+    int *d_box = nullptr;               // per-body bounding boxes (comparison LBM_OPT_MOMENTS = 1 only; lazy)
     PhaseTimer timer;
     std::map<long long, std::pair<cudaGraphExec_t, int>> graphs;   // key -> (exec, kernel nodes)
     long long launches = 0;
@@ -220,6 +223,7 @@ void free_set(lbm *h, PrepSet &S)
     dfree(h, S.tt.slot, (size_t)h->tile_cap);
     dfree(h, S.tt.rec, (size_t)h->tile_cap * 16);
     dfree(h, S.tile_order, (size_t)h->tile_cap);
+    dfree(h, S.inv, c);
     dfree(h, S.cells, h->cells_cap);
     dfree(h, S.headbits, h->headbits_cap);
     S.step = -1;
@@ -236,6 +240,7 @@ void free_markers_dev(lbm *h)
     dfree(h, h->F, (size_t)h->tile_cap * (TILE_F * TILE_F) * (size_t)h->cg.ent); h->chunk_cap = 0; h->tile_cap = 0;
     dfree(h, h->d_hist, (size_t)RADIX * (size_t)h->sort_tiles);
     dfree(h, h->d_total, (size_t)RADIX);
+    dfree(h, h->d_box, (size_t)6 * (size_t)h->nb_cap);
     dfree(h, h->d_defs, (size_t)h->nb_cap);
     dfree(h, h->d_tabs, (size_t)h->nb_cap);
     h->nm_cap = 0; h->nb_cap = 0; h->sort_tiles = 0;
@@ -259,6 +264,16 @@ int ensure_bin_first(lbm *h, PrepSet &S)
     int rc = dmalloc(h, &S.bin_first, (size_t)h->g.cells);
     if (rc) return rc;
     CK(cudaMemsetAsync(S.bin_first, 0xff, (size_t)h->g.cells * sizeof(int), h->stream));
+    return LBM_OK;
+}
+
+// arrays only the comparison variants need
+int ensure_comparison_arrays(lbm *h)
+{
+    int rc;
+    if (h->opt_interp == 1)
+        for (PrepSet &S : h->set) if (!S.inv && (rc = dmalloc(h, &S.inv, (size_t)h->nm_cap))) return rc;
+    if (h->opt_moments == 1 && !h->d_box && (rc = dmalloc(h, &h->d_box, (size_t)6 * (size_t)h->nb_cap))) return rc;
     return LBM_OK;
 }
 
@@ -389,6 +404,7 @@ int upload_markers(lbm *h)
     CK(cudaMemcpyAsync(h->d_defs, defs.data(), sizeof(BodyDef) * (size_t)nb, cudaMemcpyHostToDevice, h->stream));
     CK(cudaStreamSynchronize(h->stream));   // staging vectors die here
     h->markers_stale = false;
+    h->tiles_hint = -1;
     return LBM_OK;
 }
 
@@ -430,6 +446,7 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
     if (pt) pt->mark(PH_BINS, s);
     k_marker_gather<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, perm, S.ms);
     ++nk;
+    if (h->opt_interp == 1) { k_invert_perm<<<mb, 256, 0, s>>>(perm, n, S.inv); ++nk; }
     if (h->opt_spread == 0) {
         k_chunk_heads<<<(n + 32 + 255) / 256, 256, 0, s>>>(skey, n, g, h->cg, S.headbits);
         k_chunks<<<mb, 256, 0, s>>>(skey, n, g, h->cg, S.headbits, S.ct, h->chunk_cap, &sc->n_chunks, &sc->n_entries,
@@ -463,17 +480,33 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
     const unsigned *skey = sorted_keys(h, S);
     int nk = 0;
     if (pt) pt->mark(PH_MOMENTS, s);
-    k_moments_active<<<h->moments_grid, 256, 0, s>>>(src, g, h->po, S.cells, &sc->n_cells, h->U);
-    ++nk;
+    if (h->opt_moments == 1) {
+        // the paper's box strategy: U on the bounding box of every body
+        const int nb = (int)h->bodies.size();
+        MarkerIn mi{h->d_q[0], h->d_q[1], h->d_q[2], h->d_v[0], h->d_v[1], h->d_v[2], h->d_s, h->d_body, n};
+        k_reset_boxes<<<(nb + 127) / 128, 128, 0, s>>>(h->d_box, nb);
+        k_body_boxes<<<(n + 255) / 256, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, h->d_box);
+        k_moments_box<<<dim3(64, nb), 256, 0, s>>>(src, g, h->d_box, h->U);
+        nk += 3;
+    } else if (h->opt_moments == 2) {
+        // the paper's kernel strategy: a block per Lagrangian point, duplicates included
+        k_moments_per_marker<<<n, 64, 0, s>>>(src, g, skey, n, h->U);
+        ++nk;
+    } else {
+        k_moments_active<<<h->moments_grid, 256, 0, s>>>(src, g, h->po, S.cells, &sc->n_cells, h->U);
+        ++nk;
+    }
     for (int m = 0; m < mdf_iters; ++m) {
         const bool last = (m == mdf_iters - 1);
         if (pt) pt->mark(PH_INTERP, s);
-        k_interp_correct<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, h->U, S.ms);
+        if (h->opt_interp == 1) k_interp_caller_order<<<(n + 127) / 128, 128, 0, s>>>(skey, S.inv, n, g, h->U, S.ms);
+        else k_interp_correct<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, h->U, S.ms);
         ++nk;
         if (pt) pt->mark(PH_SPREAD, s);
         if (h->opt_spread == 0) {
-            // few markers (a single propeller): one block per tile keeps all SMs busy; many: one warp per tile
-            if (n < SPREAD_BLOCK_BELOW)
+            // few tiles (a single propeller): one block per tile keeps all SMs busy; many: one warp per tile
+            // (tiles_hint = the tile count read back once after the first preparation of the current markers)
+            if (h->tiles_hint >= 0 && h->tiles_hint < SPREAD_WARP_FROM_TILES)
                 k_spread_tiles_block<<<h->rows_block_grid, BTILE_WARPS * 32, spread_tiles_block_smem(h->cg), s>>>(
                     h->cg, S.tt.rec, S.tt.slot, S.tt.mask, &sc->n_tiles, h->tile_cap, &sc->cursor[m], S.ms.wx, S.ms.wyz,
                     last ? S.ms.du : S.ms.sg, h->F);
@@ -496,14 +529,13 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
                                                                   S.ms.fs, S.ms.sg, h->U);
             ++nk;
         } else {
-            if (last) {
-                k_zero_active<<<LIST_GRID, 256, 0, s>>>(g, S.amask, S.words, &sc->n_words, h->G);
-                k_spread_atomic<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, S.ms.fs, S.ms.du, h->G);
-                nk += 2;
-            } else {
-                k_spread_atomic<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, S.ms.fs, S.ms.sg, h->U);
-                ++nk;
-            }
+            // global atomics: thread per marker (1) or the paper's block of 5^3 threads per marker (3)
+            if (last) { k_zero_active<<<LIST_GRID, 256, 0, s>>>(g, S.amask, S.words, &sc->n_words, h->G); ++nk; }
+            const float4 *v = last ? S.ms.du : S.ms.sg;
+            float4 *field = last ? h->G : h->U;
+            if (h->opt_spread == 3) k_spread_block125<<<n, 125, 0, s>>>(skey, n, g, S.ms.fs, v, field);
+            else k_spread_atomic<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, S.ms.fs, v, field);
+            ++nk;
         }
     }
     CK(cudaGetLastError());
@@ -622,7 +654,8 @@ int get_graph(lbm *h, int kind, int parity, int set, int mdf_iters, cudaGraphExe
     const long long key = ((long long)mdf_iters << 8) | ((long long)kind << 4) | (set << 1) | parity |
                           ((long long)h->opt_spread << 40) | ((long long)h->opt_forcing << 44) |
                           ((long long)h->opt_lbm_kernel << 48) | ((long long)h->opt_interp << 52) |
-                          ((long long)h->opt_overlap << 56);
+                          ((long long)h->opt_overlap << 56) | ((long long)h->opt_moments << 58) |
+                          ((long long)(h->tiles_hint >= 0 && h->tiles_hint < SPREAD_WARP_FROM_TILES) << 60);
     auto it = h->graphs.find(key);
     if (it != h->graphs.end()) { *exec = it->second.first; *n_kernels = it->second.second; return LBM_OK; }
     cudaGraph_t graph = nullptr;
@@ -826,11 +859,12 @@ int lbm_set_option(lbm_t *h, int key, int value)
 {
     if (!h) return fail(LBM_EINVAL, "lbm_set_option: NULL handle");
     switch (key) {
-        case LBM_OPT_SPREAD: if (value < 0 || value > 2) break; h->opt_spread = value; return LBM_OK;
+        case LBM_OPT_SPREAD: if (value < 0 || value > 3) break; h->opt_spread = value; return LBM_OK;
         case LBM_OPT_FORCING: if (value < 0 || value > 1) break; h->opt_forcing = value; return LBM_OK;
         case LBM_OPT_GRAPH: if (value < 0 || value > 1) break; h->opt_graph = value; return LBM_OK;
         case LBM_OPT_LBM_KERNEL: if (value < 0 || value > 2) break; h->opt_lbm_kernel = value; return LBM_OK;
         case LBM_OPT_OVERLAP: if (value < 0 || value > 1) break; h->opt_overlap = value; return LBM_OK;
+        case LBM_OPT_MOMENTS: if (value < 0 || value > 2) break; h->opt_moments = value; return LBM_OK;
         case LBM_OPT_INTERP: if (value < 0 || value > 1) break; h->opt_interp = value; return LBM_OK;
         case LBM_OPT_TIMING: if (value < 0 || value > 1) break; h->opt_timing = value; h->timer.reset(); return LBM_OK;
         default: return fail(LBM_EINVAL, "lbm_set_option: unknown key %d", key);
@@ -1050,8 +1084,21 @@ int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
         h->launches += 1;
         if (h->opt_spread != 0)
             for (PrepSet &S : h->set) if ((rc = ensure_bin_first(h, S))) return rc;
+        if ((rc = ensure_comparison_arrays(h))) return rc;
     }
     const bool overlapped = ibm && h->opt_overlap && h->opt_graph && !h->opt_timing;
+    if (ibm && h->opt_spread == 0 && h->tiles_hint < 0) {
+        // once per marker upload: prepare the first step now and read the tile count back (one stream
+        // synchronise); it only picks the sweep variant, results do not depend on it
+        PrepSet &S = h->set[h->cur_set];
+        int np = 0, nt = 0;
+        if ((rc = enqueue_prep(h, h->stream, S, 0, &np, nullptr))) return rc;
+        h->launches += np;
+        S.step = h->steps_done; S.spread = h->opt_spread; S.dirty = true;
+        CK(cudaMemcpyAsync(&nt, &S.scal->n_tiles, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+        CK(cudaStreamSynchronize(h->stream));
+        h->tiles_hint = nt;
+    }
     for (int s = 0; s < nsteps; ++s) {
         int nk = 0;
         cudaGraphExec_t ex = nullptr;

@@ -219,6 +219,38 @@ def test_pure_and_coupled_steps_interleave(api, orc):
     sim.close()
 
 
+def test_paper_kernel_designs_give_the_same_fields(api):
+    """the paper's own designs kept as measured comparisons -- box / per-marker U
+    precompute, ib_force1's caller-order gather (Alg.1), ib_force2's block of 5^3 threads
+    with atomicAdd (Alg.2) -- must reproduce the default path: bit for bit where only the traversal
+    differs, to summation order where atomics are involved."""
+    from paper_1904_02108_b200 import workloads
+    wl = workloads.get("W1")
+
+    def run(opts=None):
+        opts = opts or {}
+        sim = api.from_workload(wl, stream=_stream())
+        for k, v in opts.items():
+            sim.set_option(k, v)
+        sim.step(15, wl.mdf_iters)
+        out = sim.read_fields() + (sim.read_markers()["force"],)
+        sim.sync()
+        sim.close()
+        return out
+
+    ref = run()
+    for opts in ({api.OPT_MOMENTS: api.MOMENTS_BOX}, {api.OPT_MOMENTS: api.MOMENTS_PER_MARKER},
+                 {api.OPT_INTERP: api.INTERP_CALLER_ORDER},
+                 {api.OPT_MOMENTS: api.MOMENTS_BOX, api.OPT_OVERLAP: 0, api.OPT_GRAPH: 0}):
+        got = run(opts)
+        for a, b in zip(ref, got):
+            assert np.array_equal(a, b), opts
+    got = run({api.OPT_SPREAD: api.SPREAD_BLOCK125, api.OPT_INTERP: api.INTERP_CALLER_ORDER,
+               api.OPT_MOMENTS: api.MOMENTS_PER_MARKER})              # the paper's pipeline as a whole
+    assert np.abs(ref[1] - got[1]).max() <= 5e-7
+    assert np.abs(ref[3] - got[3]).max() <= 1e-5 * np.abs(ref[3]).max()
+
+
 def test_static_markers_with_prescribed_velocity_and_walls(api, orc):
     """omega = 0 bodies (R14), two bodies, walls on z, markers near (but legally off) the walls."""
     rng = np.random.default_rng(21)
