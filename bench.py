@@ -219,6 +219,11 @@ def run_ours(args):
         "clocks": clocks, "gpu_launches": int(launches),
     }
 
+    paper = {"P1": 893.0, "P6": 650.0, "P18": 344.2}.get(wl.name)
+    if paper is not None:
+        # context, not a baseline: the paper's own MLUPS for the case this synthetic workload is shaped after
+        line["config"]["paper_context"] = {"mlups": paper, "hardware": "Tesla P100-PCIE (P:229-237)",
+                                           "note": "paper's Blender mesh replaced by a synthetic propeller of the same point count"}
     if rank == 0:
         # ---- the same step as one serial chain with a single fused stream-collide pass (comparison) -----
         if wl.n_markers:
