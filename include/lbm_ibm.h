@@ -167,7 +167,9 @@ int lbm_read_fields(lbm_t *h, float *rho, float *u, float *force);
 int ibm_read_markers(lbm_t *h, float *pos, float *force, int *perm, int *cell);
 
 /* Block until all enqueued work is done; returns LBM_ERANGE if a stencil crossed a wall during
- * the steps since the last sync (the offending step clamps the stencil instead of faulting). */
+ * the steps since the last sync (the offending step clamps the stencil instead of faulting), and
+ * LBM_ENOMEM if the markers formed more chunks or tiles than the device tables hold (only possible
+ * beyond the 12 GB footprint cap; the excess chunks were dropped). */
 int lbm_sync(lbm_t *h);
 
 /* Text of the last error raised on the calling thread ("" if none). */

@@ -180,14 +180,11 @@ __device__ __forceinline__ int wrap(int i, int n)
 
 // a3: bins and active cells.  The first marker of every occupied cell ("bin head") records its
 // sorted index in the dense cell -> first-marker map and marks the 4x4x4 cells of its stencil in
-// the active-cell bitmask (one bit per cell, 32 consecutive x per word).  The thread whose
-// atomicOr turns a word from 0 to non-zero appends it to the active-word list (warp-aggregated).
+// the active-cell bitmask (one bit per cell, 32 consecutive x per word).
 __global__ void __launch_bounds__(256)
-k_bins(const unsigned *__restrict__ skey, int n, Geom g, int *__restrict__ bin_first, unsigned *__restrict__ amask,
-       int *__restrict__ words, int *__restrict__ n_words)
+k_bins(const unsigned *__restrict__ skey, int n, Geom g, int *__restrict__ bin_first, unsigned *__restrict__ amask)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const int lane = threadIdx.x & 31;
     bool head = false;
     int cx = 0, cy = 0, cz = 0;
     if (i < n) {
@@ -216,21 +213,8 @@ k_bins(const unsigned *__restrict__ skey, int n, Geom g, int *__restrict__ bin_f
                 else { w1 = w; b1 |= bit; }
             }
         }
-#pragma unroll
-        for (int half = 0; half < 2; ++half) {
-            const int w = half ? w1 : w0;
-            const unsigned b = half ? b1 : b0;
-            bool fresh = false;
-            if (w >= 0) fresh = (atomicOr(amask + w, b) == 0u);
-            const unsigned vote = __ballot_sync(0xffffffffu, fresh);
-            if (vote) {
-                int base = 0;
-                const int leader = __ffs(vote) - 1;
-                if (lane == leader) base = atomicAdd(n_words, __popc(vote));
-                base = __shfl_sync(0xffffffffu, base, leader);
-                if (fresh) words[base + __popc(vote & ((1u << lane) - 1u))] = w;
-            }
-        }
+        if (w0 >= 0) atomicOr(amask + w0, b0);
+        if (w1 >= 0) atomicOr(amask + w1, b1);
     }
 }
 
@@ -443,23 +427,36 @@ k_chunk_heads(const unsigned *__restrict__ skey, int n, Geom g, ChunkGeom cg, un
     if ((threadIdx.x & 31) == 0) headbits[i >> 5] = vote;
 }
 
-// set the bits x0..x1 (inclusive, 0 <= x0 <= x1 < nx) of one row of the active-cell mask; the
-// thread that turns a word non-zero appends it to the word list
-__device__ __forceinline__ void mark_span(unsigned *__restrict__ amask, int rowbase, int x0, int x1,
-                                          int *__restrict__ words, int *__restrict__ n_words)
+// set the bits x0..x1 (inclusive, 0 <= x0 <= x1 < nx) of one row of the active-cell mask
+__device__ __forceinline__ void mark_span(unsigned *__restrict__ amask, int rowbase, int x0, int x1)
 {
     for (int w = x0 >> 5; w <= (x1 >> 5); ++w) {
         const int lo = max(x0 - (w << 5), 0), hi = min(x1 - (w << 5), 31);
-        const unsigned bits = (0xffffffffu >> (31 - hi)) & (0xffffffffu << lo);
-        if (atomicOr(amask + rowbase + w, bits) == 0u) {
-            const unsigned act = __activemask();
-            const int lane = threadIdx.x & 31;
-            const int leader = __ffs(act) - 1;
-            int base = 0;
-            if (lane == leader) base = atomicAdd(n_words, __popc(act));
-            base = __shfl_sync(act, base, leader);
-            words[base + __popc(act & ((1u << lane) - 1u))] = rowbase + w;
-        }
+        atomicOr(amask + rowbase + w, (0xffffffffu >> (31 - hi)) & (0xffffffffu << lo));
+    }
+}
+
+// a3: list of the non-zero words of the active-cell mask, in (nearly) ascending order: every warp
+// scans a contiguous stretch of the mask 32 words at a time and appends its hits in order.  The
+// spatial order is what makes the list-driven passes (moments, collect, stream-collide of the active
+// words) touch neighbouring lines one after the other.
+__global__ void __launch_bounds__(256)
+k_compact_words(const unsigned *__restrict__ amask, int n_mask_words, int *__restrict__ words, int *__restrict__ n_words)
+{
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    const int per = ((n_mask_words + nwarps - 1) / nwarps + 31) & ~31;      // words per warp, multiple of 32
+    const int beg = warp * per, end = min(beg + per, n_mask_words);
+    for (int k0 = beg; k0 < end; k0 += 32) {
+        const int k = k0 + lane;
+        const bool nz = k < end && amask[k] != 0u;
+        const unsigned vote = __ballot_sync(0xffffffffu, nz);
+        if (!vote) continue;
+        int base = 0;
+        if (lane == 0) base = atomicAdd(n_words, __popc(vote));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (nz) words[base + __popc(vote & ((1u << lane) - 1u))] = k;
     }
 }
 
@@ -517,8 +514,7 @@ k_chunks(const unsigned *__restrict__ skey, int n, Geom g, ChunkGeom cg, const u
 // cx_last+2 in each of the 16 target rows, one row per lane -- in the active-cell bitmask.
 __global__ void __launch_bounds__(256)
 k_chunk_publish(Geom g, ChunkGeom cg, ChunkTable ct, const int *__restrict__ n_chunks, int cap,
-                const int *__restrict__ chunk_of, unsigned *__restrict__ amask, int *__restrict__ words,
-                int *__restrict__ n_words)
+                const int *__restrict__ chunk_of, unsigned *__restrict__ amask)
 {
     const int l = threadIdx.x & 15;
     const int hw = (blockIdx.x * blockDim.x + threadIdx.x) >> 4;
@@ -541,8 +537,8 @@ k_chunk_publish(Geom g, ChunkGeom cg, ChunkTable ct, const int *__restrict__ n_c
         const int y = wrap(cy - 1 + (l >> 2), g.ny);
         const int z = wrap(cz - 1 + (l & 3), g.nz);
         const int rowbase = (z * g.ny + y) * g.nxw;
-        mark_span(amask, rowbase, x0a, x1a, words, n_words);
-        if (x1b >= x0b) mark_span(amask, rowbase, x0b, x1b, words, n_words);
+        mark_span(amask, rowbase, x0a, x1a);
+        if (x1b >= x0b) mark_span(amask, rowbase, x0b, x1b);
     }
 }
 

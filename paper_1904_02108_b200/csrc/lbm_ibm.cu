@@ -451,8 +451,7 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
         k_chunk_heads<<<(n + 32 + 255) / 256, 256, 0, s>>>(skey, n, g, h->cg, S.headbits);
         k_chunks<<<mb, 256, 0, s>>>(skey, n, g, h->cg, S.headbits, S.ct, h->chunk_cap, &sc->n_chunks, &sc->n_entries,
                                     S.chunk_of, &h->scal->status);
-        k_chunk_publish<<<LIST_GRID, 256, 0, s>>>(g, h->cg, S.ct, &sc->n_chunks, h->chunk_cap, S.chunk_of, S.amask, S.words,
-                                                  &sc->n_words);
+        k_chunk_publish<<<LIST_GRID, 256, 0, s>>>(g, h->cg, S.ct, &sc->n_chunks, h->chunk_cap, S.chunk_of, S.amask);
         k_tiles<<<LIST_GRID, 256, 0, s>>>(g, h->cg, h->tg, S.ct, &sc->n_chunks, h->chunk_cap, S.chunk_of, S.tt, h->tile_cap,
                                           &sc->n_tiles, &h->scal->status);
         k_tile_fill<<<LIST_GRID, 256, 0, s>>>(g, h->cg, h->tg, S.ct, &sc->n_chunks, h->chunk_cap, S.tt);
@@ -460,12 +459,13 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
         k_tile_place<<<LIST_GRID, 256, 0, s>>>(S.tt, &sc->n_tiles, h->tile_cap, sc->bucket, S.tile_order);
         nk += 7;
     } else {
-        k_bins<<<mb, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask, S.words, &sc->n_words);
+        k_bins<<<mb, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask);
         ++nk;
     }
+    k_compact_words<<<LIST_GRID, 256, 0, s>>>(S.amask, (int)h->n_mask_words, S.words, &sc->n_words);
     k_active_cells<<<LIST_GRID, 256, 0, s>>>(g, S.amask, S.words, &sc->n_words, S.cells, &sc->n_cells);
     k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, &sc->n_prev, n, 2);
-    nk += 2;
+    nk += 3;
     CK(cudaGetLastError());
     *n_kernels += nk;
     return LBM_OK;
@@ -1221,6 +1221,9 @@ int lbm_sync(lbm_t *h)
     CK(cudaStreamSynchronize(h->stream));
     if (st) {
         CK(cudaMemsetAsync(&h->scal->status, 0, sizeof(int), h->stream));
+        if (st & 2)
+            return fail(LBM_ENOMEM, "lbm_sync: more marker chunks / tiles than the tables hold (%d / %d) during the last steps",
+                        h->chunk_cap, h->tile_cap);
         return fail(LBM_ERANGE, "lbm_sync: a marker stencil crossed a wall face during the last steps");
     }
     return LBM_OK;
