@@ -113,6 +113,12 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc);
 /* Free everything the handle owns.  NULL is allowed. */
 void lbm_destroy(lbm_t *h);
 
+/* Host-only helper (no GPU needed): how an nx*ny*nz lattice is cut for the marker binning (DESIGN.md
+ * section 5).  out[8] (host) = { x blocks per row, window entries per chunk profile, tiles in y,
+ * tiles in z, 32-cell mask words per row, nominal block width (8), tile rows (4), largest window }.
+ * Blocks are 8 cells wide; when nx % 8 is 1..3 the remainder joins the last block. */
+int lbm_query_layout(int nx, int ny, int nz, int *out);
+
 /* Use cuda_stream (a cudaStream_t; NULL = legacy default stream) for all later work. */
 int lbm_set_stream(lbm_t *h, void *cuda_stream);
 

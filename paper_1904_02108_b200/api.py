@@ -31,7 +31,7 @@ MOMENTS_LIST, MOMENTS_BOX, MOMENTS_PER_MARKER = 0, 1, 2
 INTERP_SORTED, INTERP_CALLER_ORDER = 0, 1
 FORCING_GUO, FORCING_SHIFT = 0, 1
 
-EXPORTS = ["lbm_create", "lbm_destroy", "lbm_set_stream", "lbm_set_option", "lbm_get_info", "lbm_set_fields",
+EXPORTS = ["lbm_create", "lbm_destroy", "lbm_query_layout", "lbm_set_stream", "lbm_set_option", "lbm_get_info", "lbm_set_fields",
            "ibm_set_markers", "ibm_set_kinematics", "ibm_update_kinematics", "ibm_clear", "lbm_ibm_step", "lbm_read_fields",
            "ibm_read_markers", "lbm_sync", "lbm_last_error"]
 
@@ -46,6 +46,7 @@ _L.lbm_create.restype = _vp
 _L.lbm_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.POINTER(_Bc)]
 _L.lbm_destroy.restype = None
 _L.lbm_destroy.argtypes = [_vp]
+_L.lbm_query_layout.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int)]
 _L.lbm_set_stream.argtypes = [_vp, _vp]
 _L.lbm_set_option.argtypes = [_vp, C.c_int, C.c_int]
 _L.lbm_get_info.argtypes = [_vp, C.c_int, C.POINTER(C.c_longlong)]
@@ -91,6 +92,14 @@ def _ptr(a, dtype, keep):
     b = np.ascontiguousarray(np.asarray(a), dtype=dtype)
     keep.append(b)
     return b.ctypes.data
+
+
+def query_layout(nx, ny, nz) -> dict:
+    """lbm_query_layout: host-only, needs no GPU"""
+    out = (C.c_int * 8)()
+    _check(_L.lbm_query_layout(int(nx), int(ny), int(nz), out), "lbm_query_layout")
+    keys = ["x_blocks", "entries", "tiles_y", "tiles_z", "mask_words_per_row", "block_width", "tile_rows", "entries_max"]
+    return dict(zip(keys, [int(v) for v in out]))
 
 
 class LbmIbm:

@@ -847,6 +847,16 @@ void lbm_destroy(lbm_t *h)
     delete h;
 }
 
+int lbm_query_layout(int nx, int ny, int nz, int *out)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || !out) return fail(LBM_EINVAL, "lbm_query_layout: bad arguments");
+    const ChunkGeom cg = chunk_geom(nx);
+    const TileGeom tg = tile_geom(ny, nz);
+    out[0] = cg.nbx; out[1] = cg.ent; out[2] = tg.nty; out[3] = tg.ntz; out[4] = (nx + 31) / 32;
+    out[5] = CHUNK_W; out[6] = TILE_R; out[7] = CHUNK_ENT_MAX;
+    return LBM_OK;
+}
+
 int lbm_set_stream(lbm_t *h, void *cuda_stream)
 {
     if (!h) return fail(LBM_EINVAL, "lbm_set_stream: NULL handle");
