@@ -154,7 +154,7 @@ k_marker_gather(MarkerIn m, const BodyDef *__restrict__ defs, const BodyStep *__
     out.uk[i] = make_float4(ux, uy, uz, 0.f);
     out.du[i] = make_float4(0.f, 0.f, 0.f, __int_as_float(p.cx));
     out.sg[i] = make_float4(0.f, 0.f, 0.f, __int_as_float(p.cx));
-    // per-step weight tables of the run sweep (the position does not change during the MDF loop)
+    // per-step weight tables of the chunk sweep (the position does not change during the MDF loop)
     float wx[4], wy[4], wz[4];
     peskin4(p.fx, wx);
     peskin4(p.fy, wy);

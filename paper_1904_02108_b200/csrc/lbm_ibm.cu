@@ -124,7 +124,7 @@ struct PrepSet {
     SetScalars *scal = nullptr;
     bool dirty = false;                       // the dense maps hold entries of a preparation
     long long step = -1;                      // time step the set is prepared for (-1: none)
-    int spread = -1;                          // LBM_OPT_SPREAD the preparation was made for
+    int spread = -1;                          // prep_signature() the preparation was made for
 };
 
 struct lbm {
@@ -253,6 +253,9 @@ dim3 cell_block(const Geom &g)
     return dim3(bx, by, 1);
 }
 dim3 cell_grid(const Geom &g, dim3 b) { return dim3((g.nx + b.x - 1) / b.x, (g.ny + b.y - 1) / b.y, g.nz); }
+
+// the options a preparation depends on (which tables it builds)
+int prep_signature(const lbm *h) { return h->opt_spread | (h->opt_interp << 4); }
 
 const unsigned *sorted_keys(const lbm *h, const PrepSet &S) { return S.keys[h->sort_passes & 1]; }
 const int *sorted_perm(const lbm *h, const PrepSet &S) { return S.vals[h->sort_passes & 1]; }
@@ -1104,7 +1107,7 @@ int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
         int np = 0, nt = 0;
         if ((rc = enqueue_prep(h, h->stream, S, 0, &np, nullptr))) return rc;
         h->launches += np;
-        S.step = h->steps_done; S.spread = h->opt_spread; S.dirty = true;
+        S.step = h->steps_done; S.spread = prep_signature(h); S.dirty = true;
         CK(cudaMemcpyAsync(&nt, &S.scal->n_tiles, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
         CK(cudaStreamSynchronize(h->stream));
         h->tiles_hint = nt;
@@ -1114,17 +1117,17 @@ int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
         cudaGraphExec_t ex = nullptr;
         PrepSet *S = ibm ? &h->set[h->cur_set] : nullptr;
         if (overlapped) {
-            if (S->step != h->steps_done || S->spread != h->opt_spread) {
+            if (S->step != h->steps_done || S->spread != prep_signature(h)) {
                 // first step of a run (or the kinematics changed): prepare this step's set in line
                 int np = 0;
                 if ((rc = enqueue_prep(h, h->stream, *S, 0, &np, nullptr))) return rc;
                 h->launches += np;
-                S->step = h->steps_done; S->spread = h->opt_spread; S->dirty = true;
+                S->step = h->steps_done; S->spread = prep_signature(h); S->dirty = true;
             }
             if ((rc = get_graph(h, 2, h->cur, h->cur_set, mdf_iters, &ex, &nk))) return rc;
             CK(cudaGraphLaunch(ex, h->stream));
             PrepSet &N = h->set[h->cur_set ^ 1];
-            N.step = h->steps_done + 1; N.spread = h->opt_spread; N.dirty = true;
+            N.step = h->steps_done + 1; N.spread = prep_signature(h); N.dirty = true;
             h->last_set = h->cur_set;
             h->cur_set ^= 1;
         } else {
@@ -1138,7 +1141,7 @@ int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
             } else {
                 if ((rc = enqueue_step_serial(h, h->stream, h->cur, S, true, mdf_iters, &nk))) return rc;
             }
-            if (S) { S->step = h->steps_done; S->spread = h->opt_spread; S->dirty = true; h->last_set = h->cur_set; }
+            if (S) { S->step = h->steps_done; S->spread = prep_signature(h); S->dirty = true; h->last_set = h->cur_set; }
         }
         h->launches += nk;
         h->cur ^= 1;
