@@ -581,7 +581,7 @@ int enqueue_lbm_pass(lbm *h, cudaStream_t s, const float *src, float *dst, int m
 int enqueue_lbm_active(lbm *h, cudaStream_t s, const float *src, float *dst, PrepSet &S)
 {
     k_stream_collide_words<<<h->words_grid, 256, 0, s>>>(src, dst, h->g, collision_const(h), h->po, S.amask, S.words,
-                                                      &S.scal->n_words, h->G);
+                                                      &S.scal->n_words, h->G, &h->scal->step_ctr);
     CK(cudaGetLastError());
     return LBM_OK;
 }
@@ -601,15 +601,14 @@ int enqueue_step_serial(lbm *h, cudaStream_t s, int parity, PrepSet *S, bool pre
             if (pt) pt->mark(PH_LBM, s);
             if ((rc = enqueue_lbm_pass(h, s, src, dst, LBM_BULK, S->amask))) return rc;
             if (pt) pt->mark(PH_LBM_ACTIVE, s);
-            if ((rc = enqueue_lbm_active(h, s, src, dst, *S))) return rc;
+            if ((rc = enqueue_lbm_active(h, s, src, dst, *S))) return rc;     // also advances the step counter
             nk += 2;
         } else {
             if (pt) pt->mark(PH_LBM, s);
             if ((rc = enqueue_lbm_pass(h, s, src, dst, LBM_FUSED, S->amask))) return rc;
-            ++nk;
+            k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, nullptr, 0, 4);
+            nk += 2;
         }
-        k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, nullptr, 0, 4);
-        ++nk;
     } else {
         if (pt) pt->mark(PH_LBM, s);
         if ((rc = enqueue_lbm_pass(h, s, src, dst, LBM_PURE, nullptr))) return rc;
@@ -643,9 +642,8 @@ int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, int mdf_
     CK(cudaEventRecord(h->ev_prep, h->cap_prep));
     CK(cudaStreamWaitEvent(s, h->ev_bulk, 0));
     CK(cudaStreamWaitEvent(s, h->ev_prep, 0));
-    if ((rc = enqueue_lbm_active(h, s, src, dst, S))) return rc;
-    k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, nullptr, 0, 4);
-    nk += 2;
+    if ((rc = enqueue_lbm_active(h, s, src, dst, S))) return rc;               // also advances the step counter
+    ++nk;
     CK(cudaGetLastError());
     *n_kernels = nk;
     return LBM_OK;

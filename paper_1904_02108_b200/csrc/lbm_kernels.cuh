@@ -194,8 +194,10 @@ __global__ void __launch_bounds__(256)
 k_stream_collide_words(const float *__restrict__ src, float *__restrict__ dst, const __grid_constant__ Geom g,
                        const __grid_constant__ CollisionConst cc, const __grid_constant__ PlaneOffsets po,
                        const unsigned *__restrict__ amask, const int *__restrict__ words,
-                       const int *__restrict__ n_words, const float4 *__restrict__ G)
+                       const int *__restrict__ n_words, const float4 *__restrict__ G, long long *__restrict__ step_ctr)
 {
+    // last kernel of a coupled step: advance the device-side time-step counter (read by k_kinematics)
+    if (step_ctr && blockIdx.x == 0 && threadIdx.x == 0) *step_ctr += 1;
     const int lane = threadIdx.x & 31;
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int nwarps = (gridDim.x * blockDim.x) >> 5;
