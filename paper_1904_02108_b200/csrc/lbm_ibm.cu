@@ -673,18 +673,22 @@ int get_graph(lbm *h, int kind, int parity, int set, int mdf_iters, cudaGraphExe
         int lo = 0, hi = 0;
         cudaDeviceGetStreamPriorityRange(&lo, &hi);
         size_t nn = 0;
-        CK(cudaGraphGetNodes(graph, nullptr, &nn));
+        e = cudaGraphGetNodes(graph, nullptr, &nn);
         std::vector<cudaGraphNode_t> nodes(nn);
-        CK(cudaGraphGetNodes(graph, nodes.data(), &nn));
+        if (e == cudaSuccess) e = cudaGraphGetNodes(graph, nodes.data(), &nn);
         const void *bulk_fn = (const void *)k_stream_collide_scalar<LBM_BULK, 256, 5>;
-        for (cudaGraphNode_t nd : nodes) {
+        for (size_t i = 0; i < nn && e == cudaSuccess; ++i) {
             cudaGraphNodeType ty;
-            if (cudaGraphNodeGetType(nd, &ty) != cudaSuccess || ty != cudaGraphNodeTypeKernel) continue;
+            if (cudaGraphNodeGetType(nodes[i], &ty) != cudaSuccess || ty != cudaGraphNodeTypeKernel) continue;
             cudaKernelNodeParams kp{};
-            if (cudaGraphKernelNodeGetParams(nd, &kp) != cudaSuccess) continue;
+            if (cudaGraphKernelNodeGetParams(nodes[i], &kp) != cudaSuccess) continue;
             cudaLaunchAttributeValue v{};
             v.priority = (kp.func == bulk_fn) ? lo : hi;
-            CK(cudaGraphKernelNodeSetAttribute(nd, cudaLaunchAttributePriority, &v));
+            e = cudaGraphKernelNodeSetAttribute(nodes[i], cudaLaunchAttributePriority, &v);
+        }
+        if (e != cudaSuccess) {
+            cudaGraphDestroy(graph);
+            return fail(LBM_ECUDA, "setting graph node priorities failed: %s", cudaGetErrorString(e));
         }
     }
     cudaGraphExec_t ex = nullptr;
