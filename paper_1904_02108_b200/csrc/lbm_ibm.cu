@@ -179,6 +179,10 @@ struct lbm {
     std::map<long long, std::pair<cudaGraphExec_t, int>> graphs;   // key -> (exec, kernel nodes)
     long long launches = 0;
     size_t dev_bytes = 0;
+    // staging buffers for host destinations / sources, kept between calls (a host controller reads the marker
+    // forces every step: no cudaMalloc / cudaFree, which synchronise the device, on that path)
+    void *stage[3] = {nullptr, nullptr, nullptr};
+    size_t stage_cap[3] = {0, 0, 0};
 };
 
 namespace {
@@ -197,6 +201,25 @@ void dfree(lbm *h, T *&p, size_t count)
 {
     if (p) { cudaFree(p); h->dev_bytes -= count * sizeof(T); }
     p = nullptr;
+}
+
+// device staging buffer `slot` of at least `bytes` bytes; buffers up to 1 GB are kept for the next call
+constexpr size_t STAGE_KEEP = (size_t)1 << 30;
+void *stage_get(lbm *h, int slot, size_t bytes)
+{
+    if (h->stage_cap[slot] >= bytes) return h->stage[slot];
+    if (h->stage[slot]) { cudaFree(h->stage[slot]); h->dev_bytes -= h->stage_cap[slot]; h->stage[slot] = nullptr; h->stage_cap[slot] = 0; }
+    void *p = nullptr;
+    if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    h->stage[slot] = p; h->stage_cap[slot] = bytes; h->dev_bytes += bytes;
+    return p;
+}
+void stage_release(lbm *h)
+{
+    for (int a = 0; a < 3; ++a)
+        if (h->stage[a] && h->stage_cap[a] > STAGE_KEEP) {
+            cudaFree(h->stage[a]); h->dev_bytes -= h->stage_cap[a]; h->stage[a] = nullptr; h->stage_cap[a] = 0;
+        }
 }
 
 bool is_device_ptr(const void *p)
@@ -843,6 +866,7 @@ void lbm_destroy(lbm_t *h)
         cudaFree(S.amask); cudaFree(S.words); cudaFree(S.chunk_of); cudaFree(S.bin_first); cudaFree(S.scal);
         cudaFree(S.tt.mask); cudaFree(S.tt.id);
     }
+    for (int a = 0; a < 3; ++a) cudaFree(h->stage[a]);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     if (h->cap_bulk) cudaStreamDestroy(h->cap_bulk);
     if (h->cap_prep) cudaStreamDestroy(h->cap_prep);
@@ -1166,8 +1190,8 @@ int lbm_read_fields(lbm_t *h, float *rho, float *u, float *force)
         if (!out[a]) continue;
         if (is_device_ptr(out[a])) dev[a] = out[a];
         else {
-            if (cudaMalloc((void **)&dev[a], cnt[a] * sizeof(float)) != cudaSuccess) {
-                for (int b = 0; b < a; ++b) if (tmp[b]) cudaFree(dev[b]);
+            if (!(dev[a] = (float *)stage_get(h, a, cnt[a] * sizeof(float)))) {
+                stage_release(h);
                 return fail(LBM_ENOMEM, "lbm_read_fields: staging allocation failed");
             }
             tmp[a] = true;
@@ -1185,7 +1209,7 @@ int lbm_read_fields(lbm_t *h, float *rho, float *u, float *force)
             e = cudaMemcpyAsync(out[a], dev[a], cnt[a] * sizeof(float), cudaMemcpyDeviceToHost, h->stream);
         }
     if (any_tmp && e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-    for (int a = 0; a < 3; ++a) if (tmp[a]) cudaFree(dev[a]);
+    stage_release(h);
     if (e != cudaSuccess) return fail(LBM_ECUDA, "lbm_read_fields: %s", cudaGetErrorString(e));
     return LBM_OK;
 }
@@ -1207,7 +1231,10 @@ int ibm_read_markers(lbm_t *h, float *pos, float *force, int *perm, int *cell)
     for (int a = 0; a < 3; ++a) {
         if (!out[a]) continue;
         if (is_device_ptr(out[a])) dev[a] = out[a];
-        else { CK(cudaMalloc(&dev[a], bytes[a])); tmp[a] = true; }
+        else {
+            if (!(dev[a] = stage_get(h, a, bytes[a]))) return fail(LBM_ENOMEM, "ibm_read_markers: staging allocation failed");
+            tmp[a] = true;
+        }
     }
     k_read_markers<<<(n + 255) / 256, 256, 0, h->stream>>>(skey, dperm, n, h->g, S.ms.fs, S.ms.du, (float *)dev[0],
                                                             (float *)dev[1], (int *)dev[2]);
@@ -1223,7 +1250,7 @@ int ibm_read_markers(lbm_t *h, float *pos, float *force, int *perm, int *cell)
         need_sync |= !dv;
     }
     if (need_sync && e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-    for (int a = 0; a < 3; ++a) if (tmp[a]) cudaFree(dev[a]);
+    stage_release(h);
     if (e != cudaSuccess) return fail(LBM_ECUDA, "ibm_read_markers: %s", cudaGetErrorString(e));
     return LBM_OK;
 }
