@@ -944,13 +944,15 @@ k_spread_tiles_block(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int 
     const bool red = (int)threadIdx.x < TILE_F * TILE_F * EP;
     const int r_e4 = threadIdx.x % EP, r_fyz = threadIdx.x / EP;
     const int r_fz = r_fyz % TILE_F, r_fy = r_fyz / TILE_F;
-    if (threadIdx.x == 0) s_tile[0] = atomicAdd(cursor, 1);
+    // no more tiles than blocks (the usual case for this variant): block b takes tile b, no cursor round trip
+    const bool one_each = nt <= (int)gridDim.x;
+    if (threadIdx.x == 0) s_tile[0] = one_each ? (int)blockIdx.x : atomicAdd(cursor, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
     for (int it = 0;; ++it) {
         const int t = s_tile[it & 1];
         if (t >= nt) break;
-        if (threadIdx.x == 0) s_tile[(it + 1) & 1] = atomicAdd(cursor, 1);    // consumed after the next barrier pair
+        if (threadIdx.x == 0) s_tile[(it + 1) & 1] = one_each ? nt : atomicAdd(cursor, 1);   // consumed after the next barrier pair
         // lane r < 16: sorted-marker range of the chunk in source row r = sy + 4 sz ((0,0) = none)
         const int2 rec = __ldg(tile_rec + (size_t)t * 16 + l);
         const unsigned present = __ballot_sync(0xffffffffu, rec.y > rec.x) & 0xffffu;

@@ -1,0 +1,34 @@
+"""bench.py prints ONE JSON line with the keys the driver reads (pytest -m gpu; small workload)."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_bench_line_has_the_contract_keys():
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--workload", "W3", "--steps", "20", "--warmup", "3",
+                        "--cpu-steps", "1", "--quick", "--compare"], capture_output=True, text=True, timeout=900)
+    assert p.returncode == 0, p.stderr[-2000:]
+    lines = [l for l in p.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "clocks", "gpu_launches", "roofline", "cpu_baseline", "e2e"):
+        assert k in d, k
+    assert d["unit"] == "MLUPS" and d["n_gpus"] == 1 and d["steps"] == 20 and d["dtype"] == "f32" and d["vs_baseline"] is None
+    assert d["config"]["workload"] == "W3" and "model" not in d["config"]
+    assert d["gpu_launches"] > 20 * 20                 # a coupled step is ~40 kernels of this library
+    r = d["roofline"]
+    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
+    assert 0.3 < r["frac"] < 1.2
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1 and d["cpu_baseline"]["value"] > 0
+    e = d["e2e"]
+    assert e["unit"] == "MLUPS" and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
+    assert 0 < e["value"] <= d["value"] * 1.05          # end to end cannot beat the resident step
+    assert d["serial_chain"]["value"] > 0 and 0.0 <= d["ibm_share"] < 1.0
+    assert d["comparisons_ms_per_step"]["default"] > 0
