@@ -172,6 +172,17 @@ int lbm_read_fields(lbm_t *h, float *rho, float *u, float *force);
  * host or device. */
 int ibm_read_markers(lbm_t *h, float *pos, float *force, int *perm, int *cell);
 
+/* The per-step result for a host controller, without stalling the time loop: enqueue the read-out of
+ * the marker forces Delta u(k) of the last step (caller's order, force [n][3]) into HOST memory
+ * (pinned for a truly asynchronous copy) and return at once.  Packing runs on the work stream, the
+ * device-to-host copy on a stream of its own, so the next lbm_ibm_step overlaps it; the forces of
+ * step n stay valid on the device until step n+2 is prepared.  `force` may be read after
+ * ibm_wait_markers (or lbm_sync) returns; at most one read-out is in flight per handle: a second
+ * call orders itself behind the first one's copy, so use a different `force` buffer if the first
+ * has not been consumed. */
+int ibm_read_markers_async(lbm_t *h, float *force /* host */);
+int ibm_wait_markers(lbm_t *h);
+
 /* Block until all enqueued work is done; returns LBM_ERANGE if a stencil crossed a wall during
  * the steps since the last sync (the offending step clamps the stencil instead of faulting), and
  * LBM_ENOMEM if the markers formed more chunks or tiles than the device tables hold (only possible

@@ -33,7 +33,7 @@ FORCING_GUO, FORCING_SHIFT = 0, 1
 
 EXPORTS = ["lbm_create", "lbm_destroy", "lbm_query_layout", "lbm_set_stream", "lbm_set_option", "lbm_get_info", "lbm_set_fields",
            "ibm_set_markers", "ibm_set_kinematics", "ibm_update_kinematics", "ibm_clear", "lbm_ibm_step", "lbm_read_fields",
-           "ibm_read_markers", "lbm_sync", "lbm_last_error"]
+           "ibm_read_markers", "ibm_read_markers_async", "ibm_wait_markers", "lbm_sync", "lbm_last_error"]
 
 
 class _Bc(C.Structure):
@@ -58,6 +58,8 @@ _L.ibm_clear.argtypes = [_vp]
 _L.lbm_ibm_step.argtypes = [_vp, C.c_int, C.c_int]
 _L.lbm_read_fields.argtypes = [_vp, _vp, _vp, _vp]
 _L.ibm_read_markers.argtypes = [_vp, _vp, _vp, _vp, _vp]
+_L.ibm_read_markers_async.argtypes = [_vp, _vp]
+_L.ibm_wait_markers.argtypes = [_vp]
 _L.lbm_sync.argtypes = [_vp]
 _L.lbm_last_error.restype = C.c_char_p
 _L.lbm_last_error.argtypes = []
@@ -228,6 +230,15 @@ class LbmIbm:
         _check(_L.ibm_read_markers(self._h, ptrs["pos"], ptrs["force"], ptrs["perm"], ptrs["cell"]),
                "ibm_read_markers")
         return bufs
+
+    def read_markers_async(self, force_out):
+        """ibm_read_markers_async: force_out = host buffer [n,3] float32 (a numpy view of pinned memory or a
+        pinned torch tensor); valid after wait_markers() / sync()"""
+        ptr = force_out.ctypes.data if isinstance(force_out, np.ndarray) else force_out.data_ptr()
+        _check(_L.ibm_read_markers_async(self._h, ptr), "ibm_read_markers_async")
+
+    def wait_markers(self):
+        _check(_L.ibm_wait_markers(self._h), "ibm_wait_markers")
 
 
 def from_workload(wl, stream=None) -> LbmIbm:

@@ -183,6 +183,12 @@ struct lbm {
     // forces every step: no cudaMalloc / cudaFree, which synchronise the device, on that path)
     void *stage[3] = {nullptr, nullptr, nullptr};
     size_t stage_cap[3] = {0, 0, 0};
+    // asynchronous marker-force read-back (ibm_read_markers_async): packing on the work stream, D2H on a copy stream
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_pack = nullptr, ev_copy = nullptr;
+    float *async_stage = nullptr;
+    size_t async_cap = 0;
+    bool copy_pending = false;
 };
 
 namespace {
@@ -867,6 +873,10 @@ void lbm_destroy(lbm_t *h)
         cudaFree(S.tt.mask); cudaFree(S.tt.id);
     }
     for (int a = 0; a < 3; ++a) cudaFree(h->stage[a]);
+    cudaFree(h->async_stage);
+    if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+    if (h->ev_pack) cudaEventDestroy(h->ev_pack);
+    if (h->ev_copy) cudaEventDestroy(h->ev_copy);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     if (h->cap_bulk) cudaStreamDestroy(h->cap_bulk);
     if (h->cap_prep) cudaStreamDestroy(h->cap_prep);
@@ -1255,12 +1265,54 @@ int ibm_read_markers(lbm_t *h, float *pos, float *force, int *perm, int *cell)
     return LBM_OK;
 }
 
+int ibm_read_markers_async(lbm_t *h, float *force)
+{
+    if (!h || !force) return fail(LBM_EINVAL, "ibm_read_markers_async: NULL argument");
+    const int n = (int)h->h_area.size();
+    if (n == 0) return LBM_OK;
+    if (h->last_set < 0 || h->markers_stale)
+        return fail(LBM_ESTATE, "ibm_read_markers_async: no IBM step has been run with the current markers");
+    if (!h->copy_stream) {
+        CK(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+        CK(cudaEventCreateWithFlags(&h->ev_pack, cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&h->ev_copy, cudaEventDisableTiming));
+    }
+    const size_t bytes = sizeof(float) * 3 * (size_t)n;
+    if (h->async_cap < bytes) {
+        if (h->copy_pending) CK(cudaEventSynchronize(h->ev_copy));
+        if (h->async_stage) { cudaFree(h->async_stage); h->dev_bytes -= h->async_cap; h->async_stage = nullptr; h->async_cap = 0; }
+        CK(cudaMalloc((void **)&h->async_stage, bytes));
+        h->async_cap = bytes; h->dev_bytes += bytes;
+    }
+    // the packing kernel must not overwrite the staging buffer while the previous copy still reads it
+    if (h->copy_pending) CK(cudaStreamWaitEvent(h->stream, h->ev_copy, 0));
+    const PrepSet &S = h->set[h->last_set];
+    k_read_markers<<<(n + 255) / 256, 256, 0, h->stream>>>(sorted_keys(h, S), sorted_perm(h, S), n, h->g, S.ms.fs, S.ms.du,
+                                                            nullptr, h->async_stage, nullptr);
+    h->launches += 1;
+    CK(cudaGetLastError());
+    CK(cudaEventRecord(h->ev_pack, h->stream));
+    CK(cudaStreamWaitEvent(h->copy_stream, h->ev_pack, 0));
+    CK(cudaMemcpyAsync(force, h->async_stage, bytes, cudaMemcpyDeviceToHost, h->copy_stream));
+    CK(cudaEventRecord(h->ev_copy, h->copy_stream));
+    h->copy_pending = true;
+    return LBM_OK;
+}
+
+int ibm_wait_markers(lbm_t *h)
+{
+    if (!h) return fail(LBM_EINVAL, "ibm_wait_markers: NULL handle");
+    if (h->copy_pending) { CK(cudaEventSynchronize(h->ev_copy)); h->copy_pending = false; }
+    return LBM_OK;
+}
+
 int lbm_sync(lbm_t *h)
 {
     if (!h) return fail(LBM_EINVAL, "lbm_sync: NULL handle");
     int st = 0;
     CK(cudaMemcpyAsync(&st, &h->scal->status, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
+    if (h->copy_pending) { CK(cudaEventSynchronize(h->ev_copy)); h->copy_pending = false; }
     if (st) {
         CK(cudaMemsetAsync(&h->scal->status, 0, sizeof(int), h->stream));
         if (st & 2)

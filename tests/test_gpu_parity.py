@@ -251,6 +251,33 @@ def test_paper_kernel_designs_give_the_same_fields(api):
     assert np.abs(ref[3] - got[3]).max() <= 1e-5 * np.abs(ref[3]).max()
 
 
+def test_async_marker_readout_equals_the_blocking_one(api):
+    """ibm_read_markers_async + ibm_wait_markers: same forces as ibm_read_markers, step after step, while
+    the next step is already running (the forces of step n live in the marker set step n+1 does not touch)."""
+    import torch
+    from paper_1904_02108_b200 import workloads
+    wl = workloads.get("W1")
+    sim = api.from_workload(wl, stream=_stream())
+    bufs = [torch.empty((wl.n_markers, 3), dtype=torch.float32, pin_memory=True) for _ in range(2)]
+    want = []
+    for k in range(6):
+        sim.step(1, wl.mdf_iters)
+        sim.read_markers_async(bufs[k & 1])
+        if k >= 1:
+            # the copy of step k-1 was ordered before this one: after waiting, both buffers are final
+            pass
+        sim.step(1, wl.mdf_iters)                       # runs while the copy is in flight
+        sim.wait_markers()
+        got = bufs[k & 1].numpy().copy()
+        ref = api.from_workload(wl, stream=_stream())
+        ref.step(2 * k + 1, wl.mdf_iters)
+        want = ref.read_markers(pos=False, perm=False, cell=False)["force"]
+        ref.close()
+        assert np.array_equal(got, want), k
+    sim.sync()
+    sim.close()
+
+
 def test_static_markers_with_prescribed_velocity_and_walls(api, orc):
     """omega = 0 bodies (R14), two bodies, walls on z, markers near (but legally off) the walls."""
     rng = np.random.default_rng(21)
