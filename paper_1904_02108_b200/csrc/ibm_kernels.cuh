@@ -368,13 +368,12 @@ k_spread_gather(const unsigned *__restrict__ skey, int n, Geom g, const int *__r
 // A "chunk" is the stretch of sorted markers that lie in one lattice row (same cy, cz) and in one
 // aligned block of CHUNK_W = 8 cells in x.  A marker of source row (cy, cz) reaches the 16 target
 // rows (cy-1+jy, cz-1+jz) and, in x, the cells cx-1 .. cx+2, so a chunk of block j touches the
-// window X = 8j-1 .. 8j+9 (CHUNK_W + 3 "entries") of each target row.  Stage A sweeps every chunk
-// once, in sorted order, and produces for each of the 16 (jy, jz) offsets the x-profile
-//     T[chunk][jy*4+jz][e] = sum_k v_k w_y(jy) w_z(jz) w_x(X_e - cx_k + 1),   X_e = 8j - 1 + e.
-// Stage B lets every active cell add up, in fixed order, the profiles that reach it: per source row
-// at most two chunks (the blocks holding cx = X-2 and cx = X+1).  All sums have a fixed order, so
-// the result is bitwise reproducible.  Chunks are short (<= 8 cells wide), uniform in cost and
-// plentiful, which is what keeps 148 SMs busy on a single propeller as well as on 12 M markers.
+// window X = 8j-1 .. 8j+9 (CHUNK_W + 3 "entries") of each target row: 16 x-profiles
+//     sum_k v_k w_y(jy) w_z(jz) w_x(X_e - cx_k + 1),   X_e = 8j - 1 + e,   one per (jy, jz).
+// Stage A sweeps every chunk once, in sorted order, and adds its profiles, together with those of
+// the other chunks of its TILE (see below), into the tile's footprint.  Stage B lets every active
+// cell add up, in fixed order, the footprints that hold it.  All sums have a fixed order, so the
+// result is bitwise reproducible.  Chunks are short (<= 8 cells wide) and uniform in cost.
 
 constexpr int CHUNK_W = 8;
 constexpr int CHUNK_ENT_MAX = 14;     // widest window: a last block widened to 11 cells (see ChunkGeom)
@@ -738,8 +737,9 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned pari
 //
 // The marker data of a chunk (value, x weights, y-z weights: three contiguous ranges of the sorted
 // arrays) comes through the warp's own shared-memory buffers by asynchronous bulk copies (TMA),
-// SPREAD_PIECE markers at a time through a ring of SPREAD_STAGES buffers that runs ACROSS chunks, so the sweep never waits on a
-// global load per marker.  Tiles are handed out through an atomic cursor.
+// SPREAD_PIECE markers at a time through a ring of SPREAD_STAGES buffers that runs ACROSS chunks, so
+// the sweep never waits on a global load per marker.  Tiles are handed out, longest first, through an
+// atomic cursor.
 //
 // Shared memory (dynamic), per warp: footprint [7*7][ent][3] floats, then STAGES x { val[PIECE] float4,
 // wx[PIECE] float4, wyz[PIECE][16] float }.
