@@ -359,7 +359,8 @@ int upload_markers(lbm *h)
         // overflow is flagged on the device (LBM_ENOMEM at lbm_sync)
         const size_t ccap = std::max((size_t)1, std::min(std::min(c, h->chunk_slots), (size_t)CHUNK_ID_MAX));
         const size_t tile_bytes = (size_t)(TILE_F * TILE_F) * (size_t)h->cg.ent * sizeof(float4);
-        const size_t tcap = std::max((size_t)1, std::min(std::min(c, h->tile_slots), ((size_t)12 << 30) / tile_bytes));
+        size_t tcap = std::max((size_t)1, std::min(std::min(c, h->tile_slots), ((size_t)12 << 30) / tile_bytes));
+        if (const char *e = std::getenv("LBM_TEST_TILE_CAP")) tcap = std::max((size_t)1, std::min(tcap, (size_t)std::atoll(e)));   // tests: force the overflow path
         h->cells_cap = std::min((size_t)64 * c, (size_t)h->g.cells);
         h->headbits_cap = c / 32 + 16;
         for (PrepSet &S : h->set) {

@@ -346,6 +346,24 @@ def test_odd_lattices_chunk_and_tile_edges(api, orc, shape, wall):
     assert np.abs(outs[0] - outs[1]).max() <= 5e-7
 
 
+def test_tile_table_overflow_is_flagged_not_fatal(api, monkeypatch):
+    """more tiles than the footprint table holds (forced here through LBM_TEST_TILE_CAP): the excess tiles are
+    dropped on the device, the step completes, and lbm_sync reports LBM_ENOMEM; the handle stays usable."""
+    from paper_1904_02108_b200 import workloads
+    wl = workloads.get("W1")
+    monkeypatch.setenv("LBM_TEST_TILE_CAP", "5")
+    sim = api.from_workload(wl, stream=_stream())
+    sim.step(3, wl.mdf_iters)
+    with pytest.raises(api.LbmError) as ei:
+        sim.sync()
+    assert ei.value.code == -2
+    rho, u, f = sim.read_fields()
+    assert np.isfinite(u).all() and np.isfinite(f).all()
+    sim.step(2, 0)                      # pure LBM still runs, and the flag was cleared by the failed sync
+    sim.sync()
+    sim.close()
+
+
 def test_error_paths(api):
     with pytest.raises(api.LbmError):
         api.LbmIbm(8, 8, 8, 0.5)
