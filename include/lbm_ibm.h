@@ -68,7 +68,8 @@ enum {
                              used for the pure and the serial fused pass only)                     */
     LBM_OPT_INTERP = 5,   /* interpolation: 0 = thread per marker in sorted order (default), 1 = the paper's
                              ib_force1 access pattern: thread per marker in the caller's order, no reordering
-                             (Alg.1; measured comparison)                                  */
+                             (Alg.1; measured comparison), 2 = one warp per marker with a shuffle
+                             reduction (the warp-cooperative design; measured comparison)             */
     LBM_OPT_TIMING = 6,   /* 1 = run steps as plain launches with CUDA events between the phases and
                              accumulate per-phase device time (LBM_INFO_PHASE_NS); setting it resets
                              the accumulators.  Each step then ends with a stream synchronise.     */

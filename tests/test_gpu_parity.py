@@ -245,6 +245,9 @@ def test_paper_kernel_designs_give_the_same_fields(api):
         got = run(opts)
         for a, b in zip(ref, got):
             assert np.array_equal(a, b), opts
+    got = run({api.OPT_INTERP: api.INTERP_WARP_PER_MARKER})        # other summation order inside the interpolation
+    assert np.abs(ref[1] - got[1]).max() <= 5e-7
+    assert np.abs(ref[3] - got[3]).max() <= 1e-5 * np.abs(ref[3]).max()
     got = run({api.OPT_SPREAD: api.SPREAD_BLOCK125, api.OPT_INTERP: api.INTERP_CALLER_ORDER,
                api.OPT_MOMENTS: api.MOMENTS_PER_MARKER})              # the paper's pipeline as a whole
     assert np.abs(ref[1] - got[1]).max() <= 5e-7
