@@ -241,6 +241,7 @@ def run_ours(args):
                         ("moments_block_per_marker(P:215)", {api.OPT_MOMENTS: api.MOMENTS_PER_MARKER}),
                         ("interp_caller_order(ib_force1)", {api.OPT_INTERP: api.INTERP_CALLER_ORDER}),
                         ("interp_warp_per_marker(shuffle_reduce)", {api.OPT_INTERP: api.INTERP_WARP_PER_MARKER}),
+                        ("interp_chunk_window_in_smem", {api.OPT_INTERP: api.INTERP_CHUNK_SMEM}),
                         ("spread_atomic_thread_per_marker", {api.OPT_SPREAD: api.SPREAD_ATOMIC}),
                         ("spread_block125_atomic(ib_force2)", {api.OPT_SPREAD: api.SPREAD_BLOCK125}),
                         ("paper_pipeline(box+ib_force1+ib_force2,serial)",

@@ -69,7 +69,9 @@ enum {
     LBM_OPT_INTERP = 5,   /* interpolation: 0 = thread per marker in sorted order (default), 1 = the paper's
                              ib_force1 access pattern: thread per marker in the caller's order, no reordering
                              (Alg.1; measured comparison), 2 = one warp per marker with a shuffle
-                             reduction (the warp-cooperative design; measured comparison)             */
+                             reduction (the warp-cooperative design; measured comparison), 3 = one warp per
+                             chunk with the chunk's U window staged in shared memory (measured comparison;
+                             with LBM_OPT_SPREAD = 0 only)                                             */
     LBM_OPT_TIMING = 6,   /* 1 = run steps as plain launches with CUDA events between the phases and
                              accumulate per-phase device time (LBM_INFO_PHASE_NS); setting it resets
                              the accumulators.  Each step then ends with a stream synchronise.     */

@@ -28,7 +28,7 @@ INFO_PHASE_NS = 100
 PHASES = ["keys", "sort", "bins", "moments", "interp", "spread", "lbm", "lbm_active"]
 SPREAD_GATHER, SPREAD_ATOMIC, SPREAD_GATHER_PLAIN, SPREAD_BLOCK125 = 0, 1, 2, 3
 MOMENTS_LIST, MOMENTS_BOX, MOMENTS_PER_MARKER = 0, 1, 2
-INTERP_SORTED, INTERP_CALLER_ORDER, INTERP_WARP_PER_MARKER = 0, 1, 2
+INTERP_SORTED, INTERP_CALLER_ORDER, INTERP_WARP_PER_MARKER, INTERP_CHUNK_SMEM = 0, 1, 2, 3
 FORCING_GUO, FORCING_SHIFT = 0, 1
 
 EXPORTS = ["lbm_create", "lbm_destroy", "lbm_query_layout", "lbm_set_stream", "lbm_set_option", "lbm_get_info", "lbm_set_fields",

@@ -579,6 +579,83 @@ k_active_cells(Geom g, const unsigned *__restrict__ amask, const int *__restrict
 
 struct Acc3 { float x, y, z; };
 
+// a5 + a6, by chunk (LBM_OPT_INTERP = 3, a measured comparison: north_star's "stage the stencil in shared
+// memory"): one warp per chunk (chunks dealt by an atomic cursor).  All stencils of a chunk lie
+// in the chunk's window: 16 rows (jy, jz) x (CHUNK_W + 3) cells of U, 2.8 KB.  The warp stages that
+// window in shared memory with one round of coalesced loads (two rows per round, a half-warp each) and
+// then every lane interpolates one marker of the chunk from shared memory: the 64 gathers of a marker
+// are shared-memory reads instead of L1 / L2 round trips.  Measured slower than the lane-per-sorted-marker
+// gather (W4 0.38 vs 0.31 ms per step, W4lit 0.18 vs 0.08): a chunk fills 23 of 32 lanes on W4 and 5 on W4lit.
+constexpr int ICHUNK_WARPS = 4;
+
+__global__ void __launch_bounds__(ICHUNK_WARPS * 32)
+k_interp_chunks(const unsigned *__restrict__ skey, Geom g, ChunkGeom cg, ChunkTable ct, const int *__restrict__ n_chunks,
+                int cap, int *__restrict__ cursor, const float4 *__restrict__ U, MarkerSorted m)
+{
+    __shared__ float4 s_win[ICHUNK_WARPS][16 * CHUNK_ENT_MAX];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int l = lane & 15, h = lane >> 4;
+    const int nc = min(*n_chunks, cap);
+    const int ent = cg.ent;
+    float4 *win = s_win[warp];
+    for (;;) {
+        int c = 0;
+        if (lane == 0) c = atomicAdd(cursor, 1);
+        c = __shfl_sync(0xffffffffu, c, 0);
+        if (c >= nc) break;
+        const int i0 = __ldg(ct.first + c), i1 = __ldg(ct.end + c), slot = __ldg(ct.slot + c);
+        const int row = slot / cg.nbx;
+        const int x0 = (slot - row * cg.nbx) * CHUNK_W;
+        const int cz = row / g.ny, cy = row - cz * g.ny;
+        // stage the window: row r = jz*4 + jy, entry e <-> cell X = x0 - 1 + e (wrapped; out-of-range cells of a
+        // wall axis are never used)
+        if (l < ent) {
+            const int x = wrap(x0 - 1 + l, g.nx);
+#pragma unroll
+            for (int r2 = 0; r2 < 8; ++r2) {
+                const int r = 2 * r2 + h;
+                const int y = wrap(cy - 1 + (r & 3), g.ny), z = wrap(cz - 1 + (r >> 2), g.nz);
+                win[r * ent + l] = U[(size_t)(z * g.ny + y) * g.nx + x];
+            }
+        }
+        __syncwarp();
+        for (int i = i0 + lane; i < i1; i += 32) {
+            const unsigned key = skey[i];
+            const int ex = (int)(key - (unsigned)row * (unsigned)g.nx) - x0;     // entry of cell cx - 1
+            const float4 fs = m.fs[i];
+            float wx[4], wy[4], wz[4];
+            peskin4(fs.x, wx);
+            peskin4(fs.y, wy);
+            peskin4(fs.z, wz);
+            float ux = 0.f, uy = 0.f, uz = 0.f;
+#pragma unroll
+            for (int jz = 0; jz < 4; ++jz)
+#pragma unroll
+                for (int jy = 0; jy < 4; ++jy) {
+                    const float wyz = wy[jy] * wz[jz];
+                    const float4 *rowp = win + (jz * 4 + jy) * ent + ex;
+#pragma unroll
+                    for (int jx = 0; jx < 4; ++jx) {
+                        const float4 v = rowp[jx];
+                        const float w = wx[jx] * wyz;
+                        ux = fmaf(v.x, w, ux);
+                        uy = fmaf(v.y, w, uy);
+                        uz = fmaf(v.z, w, uz);
+                    }
+                }
+            const float4 uk = m.uk[i];
+            const float gx = uk.x - ux, gy = uk.y - uy, gz = uk.z - uz;
+            float4 du = m.du[i];
+            du.x = fmaf(fs.w, gx, du.x);
+            du.y = fmaf(fs.w, gy, du.y);
+            du.z = fmaf(fs.w, gz, du.z);
+            m.du[i] = du;                                // du.w keeps the cell x index
+            m.sg[i] = make_float4(fs.w * gx, fs.w * gy, fs.w * gz, du.w);
+        }
+        __syncwarp();
+    }
+}
+
 // ---- tiles ---------------------------------------------------------------------------------------
 // A "tile" groups the chunks of one x block whose source rows lie in one aligned 4 x 4 block of
 // (y, z): up to 16 chunks.  Their 16 x 16 profiles overlap on a footprint of 7 x 7 target rows, so

@@ -63,8 +63,9 @@ struct SetScalars {
     int n_tiles;         // tiles (may exceed the capacity: the excess is dropped and flagged)
     int cursor[MAX_MDF]; // work cursors of the tile sweeps, one per MDF iteration
     int bucket[16];      // tile size classes: counts [0..7] and fill cursors [8..15] (k_tile_count / k_tile_place)
+    int icursor[MAX_MDF];// work cursors of the chunk-wise interpolation, one per MDF iteration
 };
-constexpr int N_STEP_COUNTERS = 5 + MAX_MDF + 16;
+constexpr int N_STEP_COUNTERS = 5 + MAX_MDF + 16 + MAX_MDF;
 
 struct HostBody {
     long long first, count;
@@ -534,6 +535,9 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
         if (pt) pt->mark(PH_INTERP, s);
         if (h->opt_interp == 1) k_interp_caller_order<<<(n + 127) / 128, 128, 0, s>>>(skey, S.inv, n, g, h->U, S.ms);
         else if (h->opt_interp == 2) k_interp_warp_per_marker<<<(int)(((long long)n * 32 + 255) / 256), 256, 0, s>>>(skey, n, g, h->U, S.ms);
+        else if (h->opt_interp == 3 && h->opt_spread == 0)
+            k_interp_chunks<<<148 * 8, ICHUNK_WARPS * 32, 0, s>>>(skey, g, h->cg, S.ct, &sc->n_chunks, h->chunk_cap, &sc->icursor[m],
+                                                                  h->U, S.ms);
         else k_interp_correct<<<(n + 127) / 128, 128, 0, s>>>(skey, n, g, h->U, S.ms);
         ++nk;
         if (pt) pt->mark(PH_SPREAD, s);
@@ -916,7 +920,7 @@ int lbm_set_option(lbm_t *h, int key, int value)
         case LBM_OPT_LBM_KERNEL: if (value < 0 || value > 2) break; h->opt_lbm_kernel = value; return LBM_OK;
         case LBM_OPT_OVERLAP: if (value < 0 || value > 1) break; h->opt_overlap = value; return LBM_OK;
         case LBM_OPT_MOMENTS: if (value < 0 || value > 2) break; h->opt_moments = value; return LBM_OK;
-        case LBM_OPT_INTERP: if (value < 0 || value > 2) break; h->opt_interp = value; return LBM_OK;
+        case LBM_OPT_INTERP: if (value < 0 || value > 3) break; h->opt_interp = value; return LBM_OK;
         case LBM_OPT_TIMING: if (value < 0 || value > 1) break; h->opt_timing = value; h->timer.reset(); return LBM_OK;
         default: return fail(LBM_EINVAL, "lbm_set_option: unknown key %d", key);
     }

@@ -240,7 +240,7 @@ def test_paper_kernel_designs_give_the_same_fields(api):
 
     ref = run()
     for opts in ({api.OPT_MOMENTS: api.MOMENTS_BOX}, {api.OPT_MOMENTS: api.MOMENTS_PER_MARKER},
-                 {api.OPT_INTERP: api.INTERP_CALLER_ORDER},
+                 {api.OPT_INTERP: api.INTERP_CALLER_ORDER}, {api.OPT_INTERP: api.INTERP_CHUNK_SMEM},
                  {api.OPT_MOMENTS: api.MOMENTS_BOX, api.OPT_OVERLAP: 0, api.OPT_GRAPH: 0}):
         got = run(opts)
         for a, b in zip(ref, got):
