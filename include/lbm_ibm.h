@@ -56,7 +56,7 @@ enum {
 
 /* Options for lbm_set_option. */
 enum {
-    LBM_OPT_SPREAD = 1,   /* 0 = deterministic chunk sweep + tile footprints + gather-by-cell (default),
+    LBM_OPT_SPREAD = 1,   /* 0 = deterministic tile pass + tile footprints + gather-by-cell (default),
                              1 = global atomics, one thread per marker (measured comparison),
                              2 = plain gather-by-cell over the bins (slow reference variant),
                              3 = the paper's ib_force2 as printed: a block of 5^3 threads per marker with
@@ -66,7 +66,9 @@ enum {
     LBM_OPT_LBM_KERNEL = 4, /* stream-collide variant: 0 = default, 1 = one cell per thread (the default),
                              2 = four cells per thread with 128-bit accesses (nx % 4 == 0; comparison;
                              used for the pure and the serial fused pass only)                     */
-    LBM_OPT_INTERP = 5,   /* interpolation: 0 = thread per marker in sorted order (default), 1 = the paper's
+    LBM_OPT_INTERP = 5,   /* interpolation: 0 = inside the fused tile pass, from the tile's U window in shared
+                             memory (default; with LBM_OPT_FUSED = 0: a kernel of its own, thread per marker
+                             in sorted order), 1 = the paper's
                              ib_force1 access pattern: thread per marker in the caller's order, no reordering
                              (Alg.1; measured comparison), 2 = one warp per marker with a shuffle
                              reduction (the warp-cooperative design; measured comparison), 3 = one warp per
@@ -81,10 +83,24 @@ enum {
                              positions depend on time only); the cells inside the stencils are updated
                              after the join.  0 = the same step as one serial chain with a single fused
                              stream-collide pass (measured comparison).  Results are identical.        */
-    LBM_OPT_MOMENTS = 8   /* where U is precomputed for the IBM: 0 = the de-duplicated list of
+    LBM_OPT_MOMENTS = 8,  /* where U is precomputed for the IBM: 0 = the de-duplicated list of
                              cells inside a marker stencil (default), 1 = the paper's box strategy (bounding
                              box of every body), 2 = the paper's kernel strategy (a block per Lagrangian
                              point, duplicates included).  Results are identical.                      */
+    LBM_OPT_FUSED = 9,    /* 1 (default) = one MDF iteration is ONE tile pass that interpolates,
+                             corrects and spreads (s g never leaves the SM) plus the collect; 0 = the
+                             round-1 pipeline: interpolation kernel, TMA-fed tile sweep, collect (measured
+                             comparison).  Only with LBM_OPT_SPREAD = 0 and LBM_OPT_INTERP = 0.           */
+    LBM_OPT_TILE_ROWS = 10, /* source rows per tile in y and z for the fused path: 0 = automatic (1 for marker
+                             sets up to 100,000 points, else 4), or 1, 2, 4.  Changing it rebuilds the
+                             tile tables at the next step.  Results agree to rounding (summation order).  */
+    LBM_OPT_PERSISTENT = 11, /* the fused MDF loop (moments + N x (tile pass, collect)) as ONE persistent kernel
+                             with grid-wide barriers instead of 2 N + 1 launches: 0 = automatic (marker sets up
+                             to 100,000 points), 1 = always, 2 = never.  Results are bit-identical.         */
+    LBM_OPT_TILE_CAP = 12 /* > 0: cap the number of tile footprints (default 0 = room for every tile that can
+                             exist, up to 12 GB).  More tiles than the cap are dropped for that step and
+                             lbm_sync reports LBM_ENOMEM; later steps that fit are complete again.  Takes
+                             effect at the next step (the tables are re-allocated).                    */
 };
 
 /* Keys for lbm_get_info. */
@@ -98,12 +114,13 @@ enum {
     LBM_INFO_STATUS = 7,        /* device-side status word of the last step (0 = OK)              */
     LBM_INFO_RUNS = 8,          /* marker chunks (markers of one row and one 8-cell x block) in the last step */
     LBM_INFO_RUN_ENTRIES = 9,   /* window cells (profile entries) over all chunks in the last step  */
-    LBM_INFO_TILES = 10,        /* tiles (chunks of one x block and one 4x4 block of rows) in the last step */
+    LBM_INFO_TILES = 10,        /* tiles (chunks of one x block and one block of tile-rows x tile-rows source rows) in the last step */
     LBM_INFO_ACTIVE_WORDS = 11, /* 32-cell words of the active mask that hold an active cell (the cells the
                                    second stream-collide pass of the overlapped step updates)          */
     LBM_INFO_PHASE_NS = 100     /* + phase: accumulated device time in ns under LBM_OPT_TIMING.
                                    phases: 0 kinematics+keys, 1 sort, 2 gather+bins, 3 moments on
-                                   active cells, 4 interpolation+correction, 5 spreading,
+                                   active cells, 4 interpolation+correction (fused path: the whole tile
+                                   pass, sweep included), 5 spreading (fused path: the collect only),
                                    6 stream-collide (with LBM_OPT_OVERLAP: the pass over the cells
                                    outside the stencils), 7 stream-collide of the active cells     */
 };

@@ -126,11 +126,11 @@ __device__ __forceinline__ void peskin4(float f, float (&w)[4])
 // per-marker state in SORTED order
 struct MarkerSorted {
     float4 *fs;     // (fx, fy, fz, s)
-    float4 *wx;     // the four x weights w(x_k - X), X = cx-1 .. cx+2
-    float *wyz;     // [16] per marker: w_y(jy) w_z(jz) at index jy*4+jz
+    float4 *wx;     // the four x weights w(x_k - X), X = cx-1 .. cx+2       (unfused comparison path only, else NULL)
+    float *wyz;     // [16] per marker: w_y(jy) w_z(jz) at index jy*4+jz     (unfused comparison path only, else NULL)
                     // sg.w and du.w carry the marker's cell x index (int bits) for the chunk sweep
     float4 *uk;     // prescribed velocity u_k, w unused
-    float4 *sg;     // s * g^m(k)   (what the U update spreads, P:98 + R8)
+    float4 *sg;     // s * g^m(k)   (what the U update spreads, P:98 + R8)   (comparison paths only, else NULL)
     float4 *du;     // Delta u(k)
 };
 
@@ -153,8 +153,10 @@ k_marker_gather(MarkerIn m, const BodyDef *__restrict__ defs, const BodyStep *__
     const float uz = fmaf(t.dR[6], qx, fmaf(t.dR[7], qy, fmaf(t.dR[8], qz, m.vz[k])));
     out.uk[i] = make_float4(ux, uy, uz, 0.f);
     out.du[i] = make_float4(0.f, 0.f, 0.f, __int_as_float(p.cx));
+    if (!out.sg) return;                             // the fused tile pass (mdf_kernels.cuh) needs no tables
     out.sg[i] = make_float4(0.f, 0.f, 0.f, __int_as_float(p.cx));
-    // per-step weight tables of the chunk sweep (the position does not change during the MDF loop)
+    if (!out.wx) return;
+    // per-step weight tables of the round-1 chunk sweep (the position does not change during the MDF loop)
     float wx[4], wy[4], wz[4];
     peskin4(p.fx, wx);
     peskin4(p.fy, wy);
@@ -225,7 +227,7 @@ k_clear_prev(const unsigned *__restrict__ skey_prev, const int *__restrict__ n_p
              unsigned *__restrict__ amask, const int *__restrict__ words, const int *__restrict__ n_words,
              int *__restrict__ chunk_of, const int *__restrict__ chunk_slot, const int *__restrict__ n_chunks, int cap,
              unsigned *__restrict__ tile_mask, const int *__restrict__ tile_slot, const int *__restrict__ n_tiles,
-             int tile_cap)
+             int tile_cap, const int *__restrict__ ovf_slot, const int *__restrict__ n_ovf, int ovf_cap, int n_tile_slots)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     const int stride = gridDim.x * blockDim.x;
@@ -235,6 +237,11 @@ k_clear_prev(const unsigned *__restrict__ skey_prev, const int *__restrict__ n_p
     for (int c = tid; c < nc; c += stride) chunk_of[chunk_slot[c]] = -1;
     const int nt = min(*n_tiles, tile_cap);
     for (int c = tid; c < nt; c += stride) tile_mask[tile_slot[c]] = 0u;
+    // tile slots that were registered without a footprint (tile table overflow) are listed apart; when even that
+    // list overflowed, every slot is cleared
+    const int no = *n_ovf;
+    if (no <= ovf_cap) { for (int c = tid; c < no; c += stride) tile_mask[ovf_slot[c]] = 0u; }
+    else { for (int c = tid; c < n_tile_slots; c += stride) tile_mask[c] = 0u; }
 }
 
 // device scalars: mode bit 0: step_ctr = step; bit 1: n_prev = n_prev_val; bit 2: step_ctr += 1
@@ -667,17 +674,22 @@ k_interp_chunks(const unsigned *__restrict__ skey, Geom g, ChunkGeom cg, ChunkTa
 // tile_mask[tile slot] = x entries (bits 0..13) | y rows (bits 14..20) | z rows (bits 21..27) that
 // some chunk of the tile reaches; a footprint element is valid iff its three bits are set (a
 // superset of the cells actually reached; the rest is written as zeros).
-constexpr int TILE_R = 4;                  // source rows per tile in y and in z
+constexpr int TILE_R = 4;                  // source rows per tile in y and in z (large marker sets; the round-1 sweep)
 constexpr int TILE_F = TILE_R + 3;         // footprint rows per tile in y and in z
+constexpr int TILE_R_MAX = 4;
 
+// The tile edge is a property of the marker set (tr = 4, 2 or 1 source rows in y and in z): small sets use
+// tiles of a single source row so that a few thousand markers still make enough tiles for all SMs.
 struct TileGeom {
     int nty, ntz;        // tiles in y and z
+    int tr;              // source rows per tile in y and in z
 };
-inline TileGeom tile_geom(int ny, int nz)
+inline TileGeom tile_geom(int ny, int nz, int tr = TILE_R)
 {
     TileGeom t;
-    t.nty = (ny + TILE_R - 1) / TILE_R;
-    t.ntz = (nz + TILE_R - 1) / TILE_R;
+    t.tr = tr;
+    t.nty = (ny + tr - 1) / tr;
+    t.ntz = (nz + tr - 1) / tr;
     return t;
 }
 
@@ -685,7 +697,7 @@ struct TileTable {
     unsigned *mask;      // [tile slots] dense, 0 = no tile
     int *id;             // [tile slots] dense: footprint index of the tile (valid where mask != 0)
     int *slot;           // [tile ids] -> tile slot
-    int2 *rec;           // [tile ids][16]: sorted-marker range [first, end) of the chunk in source row sy + 4 sz, (0,0) = none
+    int2 *rec;           // [tile ids][tr*tr]: sorted-marker range [first, end) of the chunk in source row sy + tr sz, (0,0) = none
 };
 
 __device__ __forceinline__ int tile_slot_of(int blk, int ty, int tz, const ChunkGeom &cg, const TileGeom &tg)
@@ -697,7 +709,8 @@ __device__ __forceinline__ int tile_slot_of(int blk, int ty, int tz, const Chunk
 // allocates the tile's footprint index.  One thread per chunk.
 __global__ void __launch_bounds__(256)
 k_tiles(Geom g, ChunkGeom cg, TileGeom tg, ChunkTable ct, const int *__restrict__ n_chunks, int cap,
-        const int *__restrict__ chunk_of, TileTable tt, int tile_cap, int *__restrict__ n_tiles, int *__restrict__ status)
+        const int *__restrict__ chunk_of, TileTable tt, int tile_cap, int *__restrict__ n_tiles, int *__restrict__ ovf_slot,
+        int ovf_cap, int *__restrict__ n_ovf, int *__restrict__ status)
 {
     const int nc = min(*n_chunks, cap);
     for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
@@ -708,17 +721,24 @@ k_tiles(Geom g, ChunkGeom cg, TileGeom tg, ChunkTable ct, const int *__restrict_
         const int blk = slot - row * cg.nbx;
         const int cz = row / g.ny, cy = row - cz * g.ny;
         const unsigned xbits = ((1u << (hi - lo + 1)) - 1u) << lo;
-        const unsigned ybits = 0xFu << (cy & (TILE_R - 1)), zbits = 0xFu << (cz & (TILE_R - 1));
-        const int ts = tile_slot_of(blk, cy / TILE_R, cz / TILE_R, cg, tg);
+        const unsigned ybits = 0xFu << (cy % tg.tr), zbits = 0xFu << (cz % tg.tr);
+        const int ts = tile_slot_of(blk, cy / tg.tr, cz / tg.tr, cg, tg);
         const unsigned old = atomicOr(tt.mask + ts, xbits | (ybits << 14) | (zbits << 21));
         if (old == 0u) {
             const int id = atomicAdd(n_tiles, 1);
             if (id < tile_cap) {
                 tt.slot[id] = ts; tt.id[ts] = id;
-                int4 *z = reinterpret_cast<int4 *>(tt.rec + (size_t)id * 16);
-#pragma unroll
-                for (int i = 0; i < 8; ++i) z[i] = make_int4(0, 0, 0, 0);
-            } else { tt.id[ts] = -1; atomicOr(status, 2); }
+                int2 *z = tt.rec + (size_t)id * (tg.tr * tg.tr);
+                for (int i = 0; i < tg.tr * tg.tr; ++i) z[i] = make_int2(0, 0);
+            } else {
+                // no footprint left: undo the registration so that the slot is not stuck with a stale mask once a
+                // later step fits again (chunks that find the slot non-empty below re-register into id = -1 and are
+                // dropped for this step only; k_clear_prev clears the slots listed in ovf_slot)
+                tt.id[ts] = -1;
+                const int o = atomicAdd(n_ovf, 1);
+                if (o < ovf_cap) ovf_slot[o] = ts;
+                atomicOr(status, 2);
+            }
         }
     }
 }
@@ -733,8 +753,8 @@ k_tile_fill(Geom g, ChunkGeom cg, TileGeom tg, ChunkTable ct, const int *__restr
         const int row = slot / cg.nbx;
         const int blk = slot - row * cg.nbx;
         const int cz = row / g.ny, cy = row - cz * g.ny;
-        const int id = tt.id[tile_slot_of(blk, cy / TILE_R, cz / TILE_R, cg, tg)];
-        if (id >= 0) tt.rec[(size_t)id * 16 + (cy & (TILE_R - 1)) + 4 * (cz & (TILE_R - 1))] = make_int2(ct.first[c], ct.end[c]);
+        const int id = tt.id[tile_slot_of(blk, cy / tg.tr, cz / tg.tr, cg, tg)];
+        if (id >= 0) tt.rec[(size_t)id * (tg.tr * tg.tr) + (cy % tg.tr) + tg.tr * (cz % tg.tr)] = make_int2(ct.first[c], ct.end[c]);
     }
 }
 
@@ -742,29 +762,28 @@ k_tile_fill(Geom g, ChunkGeom cg, TileGeom tg, ChunkTable ct, const int *__restr
 // sweep, which hands tiles out through a cursor, starts the long ones first and ends on short ones
 // (longest-processing-time-first; the order inside a class is arbitrary).  Two passes: count per
 // class, then place.  bucket[0..7] = class counts, bucket[8..15] = fill cursors.
-__device__ __forceinline__ int tile_size_class(const int2 *__restrict__ rec)
+__device__ __forceinline__ int tile_size_class(const int2 *__restrict__ rec, int nr)
 {
     int n = 0;
-#pragma unroll
-    for (int r = 0; r < 16; ++r) { const int2 v = __ldg(rec + r); n += v.y - v.x; }
+    for (int r = 0; r < nr; ++r) { const int2 v = __ldg(rec + r); n += v.y - v.x; }
     const int c = 27 - __clz(max(n, 1));       // floor(log2 n) - 4
     return 7 - min(max(c, 0), 7);              // class 0 = largest
 }
 
 __global__ void __launch_bounds__(256)
-k_tile_count(TileTable tt, const int *__restrict__ n_tiles, int tile_cap, int *__restrict__ bucket)
+k_tile_count(TileTable tt, int nr, const int *__restrict__ n_tiles, int tile_cap, int *__restrict__ bucket)
 {
     const int nt = min(*n_tiles, tile_cap);
     for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < nt; t += gridDim.x * blockDim.x)
-        atomicAdd(bucket + tile_size_class(tt.rec + (size_t)t * 16), 1);
+        atomicAdd(bucket + tile_size_class(tt.rec + (size_t)t * nr, nr), 1);
 }
 
 __global__ void __launch_bounds__(256)
-k_tile_place(TileTable tt, const int *__restrict__ n_tiles, int tile_cap, int *__restrict__ bucket, int *__restrict__ order)
+k_tile_place(TileTable tt, int nr, const int *__restrict__ n_tiles, int tile_cap, int *__restrict__ bucket, int *__restrict__ order)
 {
     const int nt = min(*n_tiles, tile_cap);
     for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < nt; t += gridDim.x * blockDim.x) {
-        const int c = tile_size_class(tt.rec + (size_t)t * 16);
+        const int c = tile_size_class(tt.rec + (size_t)t * nr, nr);
         int base = 0;
         for (int q = 0; q < c; ++q) base += bucket[q];
         order[base + atomicAdd(bucket + 8 + c, 1)] = t;
@@ -842,7 +861,8 @@ __global__ void __launch_bounds__(TILE_WARPS * 32, TILE_MINB_CFG)
 k_spread_tiles(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int *__restrict__ tile_slot,
                const unsigned *__restrict__ tile_mask, const int *__restrict__ n_tiles, int tile_cap,
                int *__restrict__ cursor, const int *__restrict__ order, const float4 *__restrict__ wx4,
-               const float *__restrict__ wyz16, const float4 *__restrict__ val, float4 *__restrict__ F, int warp_smem)
+               const float *__restrict__ wyz16, const float4 *__restrict__ val, const int *__restrict__ fdst,
+               float4 *__restrict__ F, int warp_smem)
 {
     extern __shared__ __align__(128) char smem[];
     __shared__ unsigned long long s_bar[TILE_WARPS][SPREAD_STAGES];
@@ -954,251 +974,20 @@ k_spread_tiles(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int *__res
             }
             __syncwarp();                                // every lane is done with stage b (and with the footprint row)
         }
-        // write the footprint elements some chunk of the tile can reach (mask product); the rest is never read
+        // hand the footprint elements some chunk of the tile can reach (mask product) to the cells that consume
+        // them (collect plan fdst, mdf_kernels.cuh); the rest is never read
         const unsigned m = __ldg(tile_mask + ts);
-        float4 *__restrict__ Ft = F + (size_t)t * nfoot;
+        const int *__restrict__ dst = fdst + (size_t)t * nfoot;
         for (int idx = lane; idx < nfoot; idx += 32) {
             const int fyz = idx / ent, ee = idx - fyz * ent;
             const int fy = fyz / TILE_F, fz = fyz - fy * TILE_F;
             if ((m >> ee) & (m >> (14 + fy)) & (m >> (21 + fz)) & 1u) {
+                const int o = __ldg(dst + idx);
                 const float *s = foot + idx * 3;
-                Ft[idx] = make_float4(s[0], s[1], s[2], 0.f);
+                if (o >= 0) F[o] = make_float4(s[0], s[1], s[2], 0.f);
             }
         }
         __syncwarp();
-    }
-}
-
-// Stage A, variant for FEW tiles (small marker sets): one thread block (8 warps) per tile, so that a single
-// propeller still spreads over all SMs.  The source rows of the tile that hold a chunk are
-// dealt to the warps.  A warp brings its chunk's marker data (value, x weights, y-z weights: three
-// contiguous ranges of the sorted arrays) into its own shared-memory buffers with asynchronous bulk
-// copies, BTILE_PIECE markers at a time and double-buffered, so the sweep never waits on a global
-// load per marker.  It sweeps the chunk with lane = h*16 + l: l = jy*4 + jz is the target-row
-// offset whose profile the lane accumulates, h the half of the 4-cell x window it owns (h = 0: the
-// two left cells, h = 1: the two right cells), both in registers.  When the sweep moves on to the
-// next cell the leftmost window cell is final: it goes to the row's private profile in shared memory
-// and the window shifts by one (the cell that crosses from the right half to the left half travels
-// by shuffle).  Control flow is uniform across the warp.  After a barrier the block adds, for every
-// footprint element, the profiles of the source rows that reach it (sz, then sy ascending: fixed
-// order) and writes the footprint.  Tiles are handed out through an atomic cursor whose next value
-// is fetched one tile ahead.
-//
-// Shared memory (dynamic): prof[16 source rows][16 l][3 components][EP*4 entries] floats (EP =
-// ceil(ent/4)), so that the reduction reads four consecutive entries of one component with one
-// 128-bit load; then per warp 2 x { val[PIECE] float4, wx[PIECE] float4, wyz[PIECE][16] float }.
-// measured on B200: 8 warps, 4 blocks per SM, pieces of 16 markers beat 4/16 warps, 2-5 blocks and pieces of 32
-constexpr int BTILE_WARPS = 8;
-constexpr int BTILE_PIECE = 16;
-constexpr int BTILE_PIECE_BYTES = BTILE_PIECE * 96;
-
-inline size_t spread_tiles_block_smem(const ChunkGeom &cg)
-{
-    return (size_t)16 * 16 * 3 * (size_t)((cg.ent + 3) / 4 * 4) * sizeof(float) + (size_t)BTILE_WARPS * 2 * BTILE_PIECE_BYTES;
-}
-
-__global__ void __launch_bounds__(BTILE_WARPS * 32, 4)
-k_spread_tiles_block(ChunkGeom cg, const int2 *__restrict__ tile_rec, const int *__restrict__ tile_slot,
-               const unsigned *__restrict__ tile_mask, const int *__restrict__ n_tiles, int tile_cap,
-               int *__restrict__ cursor, const float4 *__restrict__ wx4, const float *__restrict__ wyz16,
-               const float4 *__restrict__ val, float4 *__restrict__ F)
-{
-    extern __shared__ __align__(128) float4 smem4[];
-    __shared__ unsigned long long s_bar[BTILE_WARPS][2];
-    __shared__ int s_tile[2];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int l = lane & 15, h = lane >> 4;
-    const int nt = min(*n_tiles, tile_cap);
-    const int ent = cg.ent;
-    const int EP = (ent + 3) >> 2, E4 = EP * 4;          // entries per profile row in shared memory
-    const int rowf = 16 * 3 * E4;                        // floats per source row
-    float *prof = reinterpret_cast<float *>(smem4);
-    char *stage = reinterpret_cast<char *>(smem4) + (size_t)16 * rowf * sizeof(float) + (size_t)warp * 2 * BTILE_PIECE_BYTES;
-    unsigned long long *bar = s_bar[warp];
-    if (lane == 0) { mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); }
-    unsigned phase = 0u;                                 // bit b: parity the next wait on bar[b] uses
-    // the footprint element group (fy, fz, 4 entries) this thread reduces, fixed for the whole kernel
-    const bool red = (int)threadIdx.x < TILE_F * TILE_F * EP;
-    const int r_e4 = threadIdx.x % EP, r_fyz = threadIdx.x / EP;
-    const int r_fz = r_fyz % TILE_F, r_fy = r_fyz / TILE_F;
-    // no more tiles than blocks (the usual case for this variant): block b takes tile b, no cursor round trip
-    const bool one_each = nt <= (int)gridDim.x;
-    if (threadIdx.x == 0) s_tile[0] = one_each ? (int)blockIdx.x : atomicAdd(cursor, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    __syncthreads();
-    for (int it = 0;; ++it) {
-        const int t = s_tile[it & 1];
-        if (t >= nt) break;
-        if (threadIdx.x == 0) s_tile[(it + 1) & 1] = one_each ? nt : atomicAdd(cursor, 1);   // consumed after the next barrier pair
-        // lane r < 16: sorted-marker range of the chunk in source row r = sy + 4 sz ((0,0) = none)
-        const int2 rec = __ldg(tile_rec + (size_t)t * 16 + l);
-        const unsigned present = __ballot_sync(0xffffffffu, rec.y > rec.x) & 0xffffu;
-        const int x0 = (__ldg(tile_slot + t) % cg.nbx) * CHUNK_W;
-        // the present source rows, dealt round-robin to the warps
-        int taken = 0;
-        for (unsigned rest = present; rest; rest &= rest - 1, ++taken) {
-            if ((taken & (BTILE_WARPS - 1)) != warp) continue;
-            const int r = __ffs(rest) - 1;
-            const int i0 = __shfl_sync(0xffffffffu, rec.x, r), i1 = __shfl_sync(0xffffffffu, rec.y, r);
-            const int npieces = (i1 - i0 + BTILE_PIECE - 1) / BTILE_PIECE;
-            auto issue = [&](int k) {                    // lane 0: bulk copies of piece k into buffer k & 1
-                const int b = k & 1;
-                const int j0 = i0 + k * BTILE_PIECE;
-                const int n = min(BTILE_PIECE, i1 - j0);
-                char *dst = stage + b * BTILE_PIECE_BYTES;
-                mbar_expect_tx(&bar[b], (unsigned)n * 96u);
-                bulk_g2s(dst, val + j0, (unsigned)n * 16u, &bar[b]);
-                bulk_g2s(dst + BTILE_PIECE * 16, wx4 + j0, (unsigned)n * 16u, &bar[b]);
-                bulk_g2s(dst + BTILE_PIECE * 32, wyz16 + (size_t)j0 * 16, (unsigned)n * 64u, &bar[b]);
-            };
-            if (lane == 0) issue(0);
-            // zero the row's profiles (entries outside the chunk's window stay zero) while the copy is in flight
-            float4 *z4 = smem4 + (size_t)r * (rowf / 4);
-            for (int i = lane; i < rowf / 4; i += 32) z4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-            __syncwarp();
-            float *out = prof + (size_t)r * rowf + l * 3 * E4;   // out[c * E4 + e]
-            Acc3 p{0.f, 0.f, 0.f}, q{0.f, 0.f, 0.f};            // window cells (e + 2h, e + 2h + 1)
-            int e = -1000;
-            for (int k = 0; k < npieces; ++k) {
-                const int b = k & 1;
-                if (k + 1 < npieces && lane == 0) issue(k + 1);   // buffer (k+1)&1 was released by the __syncwarp below
-                mbar_wait(&bar[b], (phase >> b) & 1u);
-                phase ^= 1u << b;
-                const char *src = stage + b * BTILE_PIECE_BYTES;
-                const float4 *sv = reinterpret_cast<const float4 *>(src);
-                const float2 *sw = reinterpret_cast<const float2 *>(src + BTILE_PIECE * 16) + h;
-                const float *sz = reinterpret_cast<const float *>(src + BTILE_PIECE * 32) + l;
-                const int n = min(BTILE_PIECE, i1 - i0 - k * BTILE_PIECE);
-                if (k == 0) e = __float_as_int(sv[0].w) - x0;   // window start = entry of the first marker's cx - 1
-#pragma unroll 4
-                for (int j = 0; j < n; ++j) {
-                    const float4 v = sv[j];
-                    const float2 w = sw[2 * j];
-                    const float wz = sz[16 * j];
-                    const int em = __float_as_int(v.w) - x0;
-                    if (em != e) {                              // warp-uniform: the sweep moves on to another cell
-#pragma unroll 1
-                        do {                                    // the leftmost window cell is complete
-                            if (h == 0) { out[e] = p.x; out[E4 + e] = p.y; out[2 * E4 + e] = p.z; }
-                            const float tx = __shfl_down_sync(0xffffffffu, p.x, 16);
-                            const float ty = __shfl_down_sync(0xffffffffu, p.y, 16);
-                            const float tz = __shfl_down_sync(0xffffffffu, p.z, 16);
-                            p = q;
-                            q.x = h ? 0.f : tx; q.y = h ? 0.f : ty; q.z = h ? 0.f : tz;
-                        } while (++e < em);
-                    }
-                    const float vx = v.x * wz, vy = v.y * wz, vz = v.z * wz;
-                    p.x = fmaf(w.x, vx, p.x); p.y = fmaf(w.x, vy, p.y); p.z = fmaf(w.x, vz, p.z);
-                    q.x = fmaf(w.y, vx, q.x); q.y = fmaf(w.y, vy, q.y); q.z = fmaf(w.y, vz, q.z);
-                }
-                __syncwarp();                                   // every lane is done with buffer b
-            }
-            // the last window: entries e .. e+3 (= hi)
-            const int ee = e + 2 * h;
-            out[ee] = p.x; out[E4 + ee] = p.y; out[2 * E4 + ee] = p.z;
-            out[ee + 1] = q.x; out[E4 + ee + 1] = q.y; out[2 * E4 + ee + 1] = q.z;
-        }
-        __syncthreads();
-        // footprint: element (fy, fz, e) <- sum over the present source rows (sy, sz) with 0 <= fy - sy <= 3,
-        // 0 <= fz - sz <= 3 of their profile l = (fy - sy) * 4 + (fz - sz); four entries per thread
-        if (red) {
-            const unsigned m = __ldg(tile_mask + __ldg(tile_slot + t));
-            if ((m >> (14 + r_fy)) & (m >> (21 + r_fz)) & 1u) {
-                float4 ax = make_float4(0.f, 0.f, 0.f, 0.f), ay = ax, az = ax;
-                for (int sz = max(0, r_fz - 3); sz <= min(3, r_fz); ++sz)
-                    for (int sy = max(0, r_fy - 3); sy <= min(3, r_fy); ++sy) {
-                        const int r = sy + 4 * sz;
-                        if (!((present >> r) & 1u)) continue;
-                        const float4 *v = smem4 + ((size_t)r * rowf + ((r_fy - sy) * 4 + (r_fz - sz)) * 3 * E4) / 4 + r_e4;
-                        const float4 vx = v[0], vy = v[EP], vz = v[2 * EP];
-                        ax.x += vx.x; ax.y += vx.y; ax.z += vx.z; ax.w += vx.w;
-                        ay.x += vy.x; ay.y += vy.y; ay.z += vy.z; ay.w += vy.w;
-                        az.x += vz.x; az.y += vz.y; az.z += vz.z; az.w += vz.w;
-                    }
-                float4 *__restrict__ Ft = F + ((size_t)t * (TILE_F * TILE_F) + r_fy * TILE_F + r_fz) * ent + 4 * r_e4;
-                const unsigned mx = (m & ((1u << ent) - 1u)) >> (4 * r_e4);   // x bits only (bits 14.. are rows)
-                if (mx & 1u) Ft[0] = make_float4(ax.x, ay.x, az.x, 0.f);
-                if (mx & 2u) Ft[1] = make_float4(ax.y, ay.y, az.y, 0.f);
-                if (mx & 4u) Ft[2] = make_float4(ax.z, ay.z, az.z, 0.f);
-                if (mx & 8u) Ft[3] = make_float4(ax.w, ay.w, az.w, 0.f);
-            }
-        }
-        __syncthreads();   // the next tile must not overwrite prof before every thread has read it
-    }
-}
-
-// Stage B: one thread per active cell X of target row (y, z).  The markers that reach it sit in the
-// source cells (X+1-jx, y+1-jy, z+1-jz); per axis these four coordinates meet one or two tiles
-// (blocks in x), found here as the distinct (tile, footprint coordinate) pairs.  The cell adds the
-// footprint elements of every tile in that small product, in fixed order.
-//   LAST = false:  U^{m+1}(X) = U^m(X) + sum   (R8)      LAST = true:  G(X) = sum
-// MAXC = 2 covers every lattice with nx >= 14 (or an x wall) and ny, nz multiples of 4 (or walls);
-// MAXC = 4 is the general case (tiny or odd-sized periodic lattices, where a window can wrap onto
-// its own tile or meet a third, narrow tile).
-template <int MAXC>
-struct AxisCand { int t[MAXC], f[MAXC], n; };
-
-// candidates along one axis: source coordinate c = X + 1 - j (wrapped, or skipped outside a wall axis);
-// tile = c / tile width (blocks in x: chunk_block), footprint coordinate = offset of c in its tile + j
-template <bool IS_X, int MAXC>
-__device__ __forceinline__ void axis_candidates(int X, int n, int wall, int nbx, AxisCand<MAXC> &a)
-{
-    a.n = 0;
-    int pt = -1, pf = -1;
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        int c = X + 1 - j;
-        if (wall) { if (c < 0 || c >= n) continue; } else c = wrap(c, n);
-        const int t = IS_X ? chunk_block(c, nbx) : c / TILE_R;
-        const int f = c - t * (IS_X ? CHUNK_W : TILE_R) + j;
-        if (t != pt || f != pf) {
-#pragma unroll
-            for (int i = 0; i < MAXC; ++i) if (i == a.n) { a.t[i] = t; a.f[i] = f; }
-            ++a.n; pt = t; pf = f;
-        }
-    }
-}
-
-template <bool LAST, int MAXC>
-__global__ void __launch_bounds__(256)
-k_collect_tiles(Geom g, ChunkGeom cg, TileGeom tg, TileTable tt, const float4 *__restrict__ F,
-                const int *__restrict__ cells, const int *__restrict__ n_cells, float4 *__restrict__ field)
-{
-    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
-    const int stride = gridDim.x * blockDim.x;
-    const int nc = *n_cells;
-    for (int k = tid; k < nc; k += stride) {
-        const int cell = __ldg(cells + k);
-        const int row = cell / g.nx;
-        const int x = cell - row * g.nx;
-        const int z = row / g.ny, y = row - z * g.ny;
-        AxisCand<MAXC> ax, ay, az;
-        axis_candidates<true, MAXC>(x, g.nx, g.wallx, cg.nbx, ax);
-        axis_candidates<false, MAXC>(y, g.ny, g.wally, 0, ay);
-        axis_candidates<false, MAXC>(z, g.nz, g.wallz, 0, az);
-        float sx = 0.f, sy = 0.f, sz = 0.f;
-#pragma unroll
-        for (int iz = 0; iz < MAXC; ++iz)
-#pragma unroll
-            for (int iy = 0; iy < MAXC; ++iy)
-#pragma unroll
-                for (int ix = 0; ix < MAXC; ++ix) {
-                    if (iz >= az.n || iy >= ay.n || ix >= ax.n) continue;
-                    const int ts = tile_slot_of(ax.t[ix], ay.t[iy], az.t[iz], cg, tg);
-                    const unsigned m = __ldg(tt.mask + ts);
-                    if (!((m >> ax.f[ix]) & (m >> (14 + ay.f[iy])) & (m >> (21 + az.f[iz])) & 1u)) continue;
-                    const int id = __ldg(tt.id + ts);
-                    if (id < 0) continue;
-                    const float4 v = F[((size_t)id * (TILE_F * TILE_F) + ay.f[iy] * TILE_F + az.f[iz]) * cg.ent + ax.f[ix]];
-                    sx += v.x; sy += v.y; sz += v.z;
-                }
-        if (LAST) {
-            field[cell] = make_float4(sx, sy, sz, 0.f);
-        } else {
-            float4 u = field[cell];
-            u.x += sx; u.y += sy; u.z += sz;
-            field[cell] = u;
-        }
     }
 }
 

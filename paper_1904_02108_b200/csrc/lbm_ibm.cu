@@ -16,7 +16,10 @@
 #include <string>
 #include <vector>
 
+#include <cstddef>
+
 #include "ibm_kernels.cuh"
+#include "mdf_kernels.cuh"
 #include "sort_kernels.cuh"
 
 using namespace lbmk;
@@ -61,11 +64,15 @@ struct SetScalars {
     int n_entries;       // profile entries (window cells) over all chunks
     int n_cells;         // active cells
     int n_tiles;         // tiles (may exceed the capacity: the excess is dropped and flagged)
-    int cursor[MAX_MDF]; // work cursors of the tile sweeps, one per MDF iteration
+    int n_ovf;           // tile slots registered beyond the capacity (listed in PrepSet::ovf_slot)
+    int n_felem;         // footprint elements handed out by the collect plan
+    unsigned gbar;       // grid-wide barrier of the persistent MDF kernel (monotonic within a step)
+    int cursor[MAX_MDF]; // work cursors of the tile passes, one per MDF iteration
     int bucket[16];      // tile size classes: counts [0..7] and fill cursors [8..15] (k_tile_count / k_tile_place)
     int icursor[MAX_MDF];// work cursors of the chunk-wise interpolation, one per MDF iteration
 };
-constexpr int N_STEP_COUNTERS = 5 + MAX_MDF + 16 + MAX_MDF;
+constexpr int N_STEP_COUNTERS = (int)((sizeof(SetScalars) - offsetof(SetScalars, n_words)) / sizeof(int));
+constexpr int OVF_CAP = 4096;        // tile slots of a table overflow that are undone one by one
 
 struct HostBody {
     long long first, count;
@@ -74,7 +81,9 @@ struct HostBody {
 };
 
 constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driven kernels
-constexpr int SPREAD_WARP_FROM_TILES = 1200;   // tile count from which the warp-per-tile sweep is used (W3: 160 tiles -> block, P6: 1460 -> warp)
+// Marker sets up to this size run the MDF loop as one persistent kernel on single-row tiles (LBM_OPT_TILE_ROWS,
+// LBM_OPT_PERSISTENT = 0): W1 / W3 / P1-P18 (<= 70,848 markers) fall below, W4lit (147,456) and up above.
+constexpr int SMALL_SET_MARKERS = 100000;
 
 // Optional per-phase device timing (LBM_OPT_TIMING): CUDA events recorded on the launching stream
 // between the phases of a step; durations are accumulated after a stream synchronise.
@@ -114,6 +123,9 @@ struct PrepSet {
     ChunkTable ct{nullptr, nullptr, nullptr};
     TileTable tt{nullptr, nullptr, nullptr, nullptr};  // mask, id: dense over the tile slots; slot, rec: per tile
     int *tile_order = nullptr;                // tiles by decreasing marker count (size classes)
+    int *ovf_slot = nullptr;                  // tile slots registered without a footprint (table overflow), OVF_CAP entries
+    int *fdst = nullptr;                      // collect plan: [tile][footprint element] -> index into F or -1
+    int2 *cell_run = nullptr;                 // collect plan: [active cell] (first element in F, count)
     int *inv = nullptr;                       // inverse permutation (comparison LBM_OPT_INTERP = 1 only; lazy)
     unsigned *headbits = nullptr;             // one bit per sorted marker: starts a run
     int *cells = nullptr;                     // active-cell list
@@ -168,13 +180,18 @@ struct lbm {
     TileGeom tg{1, 1};
     int chunk_cap = 0, tile_cap = 0;    // capacity of the chunk table / of F
     size_t chunk_slots = 0, tile_slots = 0;   // entries of chunk_of / of the dense tile maps
-    int rows_grid = 148, rows_block_grid = 148;   // persistent grids of the two tile sweeps (blocks resident at once)
+    int rows_grid = 148;                // persistent grid of the round-1 tile sweep (blocks resident at once)
+    int sms = 148;
+    int tr = 0;                         // tile edge (source rows in y and z) the tile tables are built for; 0 = none yet
+    int mdf_grid = 148, mdfp_grid = 148;   // grids of the fused tile pass / of the persistent MDF kernel
+    size_t mdf_wsmem = 0;               // shared memory per warp of the tile pass for (tr, cg)
     int words_grid = 148, moments_grid = 148;   // same for the active-word stream-collide and the moments kernel
     int sort_ipw = 64, sort_tiles = 0, sort_passes = 1;
 
     int opt_spread = 0, opt_forcing = 0, opt_graph = 1, opt_lbm_kernel = 0, opt_interp = 0, opt_timing = 0;
     int opt_overlap = 1, opt_moments = 0;
-    int tiles_hint = -1;                // tile count of the first preparation after a marker upload (-1: not known yet)
+    int opt_fused = 1, opt_tile_rows = 0, opt_persistent = 0, opt_tile_cap = 0;
+    bool realloc_tables = false;        // LBM_OPT_TILE_CAP changed: the tile tables are re-allocated at the next step
     int *d_box = nullptr;               // per-body bounding boxes (comparison LBM_OPT_MOMENTS = 1 only; lazy)
     PhaseTimer timer;
     std::map<long long, std::pair<cudaGraphExec_t, int>> graphs;   // key -> (exec, kernel nodes)
@@ -251,8 +268,12 @@ void free_set(lbm *h, PrepSet &S)
     dfree(h, S.ct.first, (size_t)h->chunk_cap); dfree(h, S.ct.end, (size_t)h->chunk_cap);
     dfree(h, S.ct.slot, (size_t)h->chunk_cap);
     dfree(h, S.tt.slot, (size_t)h->tile_cap);
-    dfree(h, S.tt.rec, (size_t)h->tile_cap * 16);
+    dfree(h, S.tt.rec, (size_t)h->tile_cap * (size_t)(h->tr * h->tr));
     dfree(h, S.tile_order, (size_t)h->tile_cap);
+    dfree(h, S.ovf_slot, (size_t)OVF_CAP);
+    dfree(h, S.fdst, (size_t)h->tile_cap * (size_t)((h->tr + 3) * (h->tr + 3)) * (size_t)h->cg.ent);
+    dfree(h, S.cell_run, h->cells_cap);
+    dfree(h, S.tt.mask, h->tile_slots); dfree(h, S.tt.id, h->tile_slots);
     dfree(h, S.inv, c);
     dfree(h, S.cells, h->cells_cap);
     dfree(h, S.headbits, h->headbits_cap);
@@ -267,7 +288,8 @@ void free_markers_dev(lbm *h)
     dfree(h, h->d_body, c);
     for (PrepSet &S : h->set) free_set(h, S);
     h->cells_cap = 0; h->headbits_cap = 0;
-    dfree(h, h->F, (size_t)h->tile_cap * (TILE_F * TILE_F) * (size_t)h->cg.ent); h->chunk_cap = 0; h->tile_cap = 0;
+    dfree(h, h->F, (size_t)h->tile_cap * (size_t)((h->tr + 3) * (h->tr + 3)) * (size_t)h->cg.ent);
+    h->chunk_cap = 0; h->tile_cap = 0; h->tile_slots = 0; h->tr = 0;
     dfree(h, h->d_hist, (size_t)RADIX * (size_t)h->sort_tiles);
     dfree(h, h->d_total, (size_t)RADIX);
     dfree(h, h->d_box, (size_t)6 * (size_t)h->nb_cap);
@@ -284,8 +306,28 @@ dim3 cell_block(const Geom &g)
 }
 dim3 cell_grid(const Geom &g, dim3 b) { return dim3((g.nx + b.x - 1) / b.x, (g.ny + b.y - 1) / b.y, g.nz); }
 
+// the product path: fused tile pass + collect (mdf_kernels.cuh); everything else is a measured comparison
+bool fused_path(const lbm *h) { return h->opt_fused && h->opt_spread == 0 && h->opt_interp == 0; }
+
+// tile edge for the current markers and options: the comparison paths are written for 4 x 4 rows; the fused
+// path uses single-row tiles for small marker sets (enough tiles for all SMs) unless LBM_OPT_TILE_ROWS says otherwise
+int effective_tr(const lbm *h)
+{
+    if (!fused_path(h)) return TILE_R;
+    if (h->opt_tile_rows) return h->opt_tile_rows;
+    return (int)h->h_area.size() <= SMALL_SET_MARKERS ? 1 : TILE_R;
+}
+
+// the whole MDF loop as one persistent kernel (small marker sets: launch latency dominates otherwise)
+bool use_persistent(const lbm *h)
+{
+    if (!fused_path(h) || h->opt_moments != 0 || h->opt_timing) return false;
+    if (h->opt_persistent) return h->opt_persistent == 1;
+    return h->nm <= SMALL_SET_MARKERS;
+}
+
 // the options a preparation depends on (which tables it builds)
-int prep_signature(const lbm *h) { return h->opt_spread | (h->opt_interp << 4); }
+int prep_signature(const lbm *h) { return h->opt_spread | (h->opt_interp << 4) | (h->tr << 8) | ((int)fused_path(h) << 12); }
 
 const unsigned *sorted_keys(const lbm *h, const PrepSet &S) { return S.keys[h->sort_passes & 1]; }
 const int *sorted_perm(const lbm *h, const PrepSet &S) { return S.vals[h->sort_passes & 1]; }
@@ -307,6 +349,17 @@ int ensure_comparison_arrays(lbm *h)
     if (h->opt_interp == 1)
         for (PrepSet &S : h->set) if (!S.inv && (rc = dmalloc(h, &S.inv, (size_t)h->nm_cap))) return rc;
     if (h->opt_moments == 1 && !h->d_box && (rc = dmalloc(h, &h->d_box, (size_t)6 * (size_t)h->nb_cap))) return rc;
+    if (!fused_path(h))
+        for (PrepSet &S : h->set) {
+            // s g per marker; the round-1 sweep also reads per-marker weight tables.  A set prepared without them is stale.
+            const size_t c = (size_t)h->nm_cap;
+            if (!S.ms.sg) { if ((rc = dmalloc(h, &S.ms.sg, c))) return rc; S.step = -1; }
+            if (h->opt_spread == 0 && !S.ms.wx) {
+                if ((rc = dmalloc(h, &S.ms.wx, c))) return rc;
+                if ((rc = dmalloc(h, &S.ms.wyz, 16 * c))) return rc;
+                S.step = -1;
+            }
+        }
     return LBM_OK;
 }
 
@@ -317,7 +370,8 @@ int flush_set(lbm *h, PrepSet &S)
     if (!S.dirty) return LBM_OK;
     k_clear_prev<<<LIST_GRID, 256, 0, h->stream>>>(sorted_keys(h, S), &S.scal->n_prev, S.bin_first, S.amask, S.words,
                                                     &S.scal->n_words, S.chunk_of, S.ct.slot, &S.scal->n_chunks,
-                                                    h->chunk_cap, S.tt.mask, S.tt.slot, &S.scal->n_tiles, h->tile_cap);
+                                                    h->chunk_cap, S.tt.mask, S.tt.slot, &S.scal->n_tiles, h->tile_cap,
+                                                    S.ovf_slot, &S.scal->n_ovf, OVF_CAP, (int)h->tile_slots);
     CK(cudaMemsetAsync(S.scal, 0, sizeof(SetScalars), h->stream));
     CK(cudaGetLastError());
     h->launches += 1;
@@ -336,6 +390,64 @@ int flush_ibm(lbm *h)
     return LBM_OK;
 }
 
+// ---- the fused MDF kernels for a tile edge and a lattice ---------------------------------------------
+struct MdfKernels {
+    void (*tiles)(const MdfArgs, int *, int, int);
+    void (*plan)(const MdfArgs);
+    void (*persistent)(const MdfArgs, const float *, const PlaneOffsets, int *, unsigned *, int, int);
+};
+
+// How many (tile, footprint coordinate) candidates a cell can have per axis: two unless a 4-cell span can wrap
+// onto its own tile or meet a third, narrow one (tiny or odd-sized periodic lattices); single-row and two-row
+// tiles meet up to four tiles in y and z.
+MdfKernels mdf_kernels(const lbm *h)
+{
+    const Geom &g = h->g;
+    const bool two_x = g.wallx || g.nx >= CHUNK_ENT_MAX;
+    const bool two_yz = (g.wally || g.ny % TILE_R == 0) && (g.wallz || g.nz % TILE_R == 0);
+    switch (h->tr) {
+        case 1:
+            if (two_x) return MdfKernels{k_mdf_tiles<1>, k_collect_plan<1, 2, 4>, k_mdf_persistent<1>};
+            return MdfKernels{k_mdf_tiles<1>, k_collect_plan<1, 4, 4>, k_mdf_persistent<1>};
+        case 2:
+            if (two_x) return MdfKernels{k_mdf_tiles<2>, k_collect_plan<2, 2, 4>, k_mdf_persistent<2>};
+            return MdfKernels{k_mdf_tiles<2>, k_collect_plan<2, 4, 4>, k_mdf_persistent<2>};
+        default:
+            if (two_x && two_yz) return MdfKernels{k_mdf_tiles<4>, k_collect_plan<4, 2, 2>, k_mdf_persistent<4>};
+            return MdfKernels{k_mdf_tiles<4>, k_collect_plan<4, 4, 4>, k_mdf_persistent<4>};
+    }
+}
+
+constexpr int MDFP_BLOCKS_PER_SM = 2;   // the persistent kernel leaves room for the bulk stream-collide beside it
+
+int mdf_launch_geometry(lbm *h)
+{
+    const MdfKernels K = mdf_kernels(h);
+    const size_t smem_t = (size_t)MDF_WARPS * h->mdf_wsmem, smem_p = (size_t)MDFP_WARPS * h->mdf_wsmem;
+    CK(cudaFuncSetAttribute((const void *)K.tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t));
+    CK(cudaFuncSetAttribute((const void *)K.persistent, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p));
+    int per_sm = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, K.tiles, MDF_WARPS * 32, smem_t));
+    h->mdf_grid = std::max(1, per_sm) * h->sms;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, K.persistent, MDFP_WARPS * 32, smem_p));
+    if (per_sm < 1) return fail(LBM_ECUDA, "the persistent MDF kernel does not fit on an SM (%zu bytes of shared memory)", smem_p);
+    h->mdfp_grid = std::min(per_sm, MDFP_BLOCKS_PER_SM) * h->sms;
+    return LBM_OK;
+}
+
+MdfArgs mdf_args(const lbm *h, const PrepSet &S)
+{
+    MdfArgs a{};
+    a.g = h->g; a.cg = h->cg; a.tg = h->tg;
+    a.tile_rec = S.tt.rec; a.tile_slot = S.tt.slot; a.tile_mask = S.tt.mask; a.tile_id = S.tt.id;
+    a.tile_order = S.tile_order; a.n_tiles = &S.scal->n_tiles; a.tile_cap = h->tile_cap;
+    a.fdst = S.fdst; a.cell_run = S.cell_run; a.n_felem = &S.scal->n_felem;
+    a.fs = S.ms.fs; a.uk = S.ms.uk; a.du = S.ms.du;
+    a.U = h->U; a.G = h->G; a.F = h->F;
+    a.cells = S.cells; a.n_cells = &S.scal->n_cells;
+    return a;
+}
+
 // ---- (re)build the device copies of the markers -------------------------------------------------
 int upload_markers(lbm *h)
 {
@@ -346,8 +458,13 @@ int upload_markers(lbm *h)
     drop_graphs(h);
     const int n = (int)h->h_area.size();
     const int nb = (int)h->bodies.size();
-    if (n > h->nm_cap || nb > h->nb_cap) {
+    const int tr = effective_tr(h);
+    if (n > h->nm_cap || nb > h->nb_cap || tr != h->tr || h->realloc_tables) {
         free_markers_dev(h);
+        h->realloc_tables = false;
+        h->tr = tr;
+        h->tg = tile_geom(h->g.ny, h->g.nz, tr);
+        h->tile_slots = (size_t)h->cg.nbx * h->tg.nty * h->tg.ntz;
         const size_t c = (size_t)n;
         for (int a = 0; a < 3; ++a) {
             if ((rc = dmalloc(h, &h->d_q[a], c))) return rc;
@@ -359,9 +476,9 @@ int upload_markers(lbm *h)
         // F has room for every tile that can exist up to 12 GB, beyond that the capacity is capped and an
         // overflow is flagged on the device (LBM_ENOMEM at lbm_sync)
         const size_t ccap = std::max((size_t)1, std::min(std::min(c, h->chunk_slots), (size_t)CHUNK_ID_MAX));
-        const size_t tile_bytes = (size_t)(TILE_F * TILE_F) * (size_t)h->cg.ent * sizeof(float4);
-        size_t tcap = std::max((size_t)1, std::min(std::min(c, h->tile_slots), ((size_t)12 << 30) / tile_bytes));
-        if (const char *e = std::getenv("LBM_TEST_TILE_CAP")) tcap = std::max((size_t)1, std::min(tcap, (size_t)std::atoll(e)));   // tests: force the overflow path
+        const size_t tile_elems = (size_t)((tr + 3) * (tr + 3)) * (size_t)h->cg.ent;
+        size_t tcap = std::max((size_t)1, std::min(std::min(c, h->tile_slots), ((size_t)12 << 30) / (tile_elems * sizeof(float4))));
+        if (h->opt_tile_cap > 0) tcap = std::max((size_t)1, std::min(tcap, (size_t)h->opt_tile_cap));   // LBM_OPT_TILE_CAP
         h->cells_cap = std::min((size_t)64 * c, (size_t)h->g.cells);
         h->headbits_cap = c / 32 + 16;
         for (PrepSet &S : h->set) {
@@ -370,22 +487,28 @@ int upload_markers(lbm *h)
                 if ((rc = dmalloc(h, &S.vals[a], c))) return rc;
             }
             if ((rc = dmalloc(h, &S.ms.fs, c))) return rc;
-            if ((rc = dmalloc(h, &S.ms.wx, c))) return rc;
-            if ((rc = dmalloc(h, &S.ms.wyz, 16 * c))) return rc;
             if ((rc = dmalloc(h, &S.ms.uk, c))) return rc;
-            if ((rc = dmalloc(h, &S.ms.sg, c))) return rc;
-            if ((rc = dmalloc(h, &S.ms.du, c))) return rc;
+            if ((rc = dmalloc(h, &S.ms.du, c))) return rc;      // wx, wyz, sg: comparison paths only (ensure_comparison_arrays)
             if ((rc = dmalloc(h, &S.ct.first, (size_t)ccap))) return rc;
             if ((rc = dmalloc(h, &S.ct.end, (size_t)ccap))) return rc;
             if ((rc = dmalloc(h, &S.ct.slot, (size_t)ccap))) return rc;
             if ((rc = dmalloc(h, &S.tt.slot, tcap))) return rc;
-            if ((rc = dmalloc(h, &S.tt.rec, tcap * 16))) return rc;
+            if ((rc = dmalloc(h, &S.tt.rec, tcap * (size_t)(tr * tr)))) return rc;
             if ((rc = dmalloc(h, &S.tile_order, tcap))) return rc;
+            if ((rc = dmalloc(h, &S.ovf_slot, (size_t)OVF_CAP))) return rc;
+            if ((rc = dmalloc(h, &S.fdst, tcap * tile_elems))) return rc;
+            if ((rc = dmalloc(h, &S.cell_run, h->cells_cap))) return rc;
+            if ((rc = dmalloc(h, &S.tt.mask, h->tile_slots))) return rc;
+            if ((rc = dmalloc(h, &S.tt.id, h->tile_slots))) return rc;
+            CK(cudaMemsetAsync(S.tt.mask, 0, h->tile_slots * sizeof(unsigned), h->stream));
             if ((rc = dmalloc(h, &S.cells, h->cells_cap))) return rc;
             if ((rc = dmalloc(h, &S.headbits, h->headbits_cap))) return rc;
         }
-        if ((rc = dmalloc(h, &h->F, tcap * (TILE_F * TILE_F) * (size_t)h->cg.ent))) return rc;
+        if ((rc = dmalloc(h, &h->F, tcap * tile_elems))) return rc;
         h->chunk_cap = (int)ccap; h->tile_cap = (int)tcap;
+        // launch geometry of the fused tile pass and of the persistent MDF kernel for (tr, cg)
+        h->mdf_wsmem = mdf_warp_smem(tr, h->cg);
+        if ((rc = mdf_launch_geometry(h))) return rc;
         if ((rc = dmalloc(h, &h->d_total, (size_t)RADIX))) return rc;
         if ((rc = dmalloc(h, &h->d_defs, (size_t)nb))) return rc;
         if ((rc = dmalloc(h, &h->d_tabs, (size_t)nb))) return rc;
@@ -438,7 +561,6 @@ int upload_markers(lbm *h)
     CK(cudaMemcpyAsync(h->d_defs, defs.data(), sizeof(BodyDef) * (size_t)nb, cudaMemcpyHostToDevice, h->stream));
     CK(cudaStreamSynchronize(h->stream));   // staging vectors die here
     h->markers_stale = false;
-    h->tiles_hint = -1;
     return LBM_OK;
 }
 
@@ -458,7 +580,8 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
 
     if (pt) pt->mark(PH_KEYS, s);
     k_clear_prev<<<LIST_GRID, 256, 0, s>>>(skey, &sc->n_prev, S.bin_first, S.amask, S.words, &sc->n_words, S.chunk_of,
-                                           S.ct.slot, &sc->n_chunks, h->chunk_cap, S.tt.mask, S.tt.slot, &sc->n_tiles, h->tile_cap);
+                                           S.ct.slot, &sc->n_chunks, h->chunk_cap, S.tt.mask, S.tt.slot, &sc->n_tiles, h->tile_cap,
+                                           S.ovf_slot, &sc->n_ovf, OVF_CAP, (int)h->tile_slots);
     const int nb = (int)h->bodies.size();
     k_kinematics<<<(std::max(nb, N_STEP_COUNTERS) + 127) / 128, 128, 0, s>>>(h->d_defs, h->d_tabs, nb, &h->scal->step_ctr,
                                                                               step_offset, &sc->n_words, N_STEP_COUNTERS);
@@ -487,10 +610,10 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
                                     S.chunk_of, &h->scal->status);
         k_chunk_publish<<<LIST_GRID, 256, 0, s>>>(g, h->cg, S.ct, &sc->n_chunks, h->chunk_cap, S.chunk_of, S.amask);
         k_tiles<<<LIST_GRID, 256, 0, s>>>(g, h->cg, h->tg, S.ct, &sc->n_chunks, h->chunk_cap, S.chunk_of, S.tt, h->tile_cap,
-                                          &sc->n_tiles, &h->scal->status);
+                                          &sc->n_tiles, S.ovf_slot, OVF_CAP, &sc->n_ovf, &h->scal->status);
         k_tile_fill<<<LIST_GRID, 256, 0, s>>>(g, h->cg, h->tg, S.ct, &sc->n_chunks, h->chunk_cap, S.tt);
-        k_tile_count<<<LIST_GRID, 256, 0, s>>>(S.tt, &sc->n_tiles, h->tile_cap, sc->bucket);
-        k_tile_place<<<LIST_GRID, 256, 0, s>>>(S.tt, &sc->n_tiles, h->tile_cap, sc->bucket, S.tile_order);
+        k_tile_count<<<LIST_GRID, 256, 0, s>>>(S.tt, h->tr * h->tr, &sc->n_tiles, h->tile_cap, sc->bucket);
+        k_tile_place<<<LIST_GRID, 256, 0, s>>>(S.tt, h->tr * h->tr, &sc->n_tiles, h->tile_cap, sc->bucket, S.tile_order);
         nk += 7;
     } else {
         k_bins<<<mb, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask);
@@ -498,6 +621,13 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
     }
     k_compact_words<<<LIST_GRID, 256, 0, s>>>(S.amask, (int)h->n_mask_words, S.words, &sc->n_words);
     k_active_cells<<<LIST_GRID, 256, 0, s>>>(g, S.amask, S.words, &sc->n_words, S.cells, &sc->n_cells);
+    if (h->opt_spread == 0) {
+        // collect plan: which footprint elements every active cell adds up, and where the tile pass puts them
+        const int elems = (h->tr + 3) * (h->tr + 3) * h->cg.ent;
+        k_fill_tiles<<<LIST_GRID, 256, 0, s>>>(S.fdst, &sc->n_tiles, h->tile_cap, elems);
+        mdf_kernels(h).plan<<<LIST_GRID, 256, 0, s>>>(mdf_args(h, S));
+        nk += 2;
+    }
     k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, &sc->n_prev, n, 2);
     nk += 3;
     CK(cudaGetLastError());
@@ -513,6 +643,18 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
     SetScalars *sc = S.scal;
     const unsigned *skey = sorted_keys(h, S);
     int nk = 0;
+    const bool fused = fused_path(h);
+    const MdfKernels K = mdf_kernels(h);
+    const MdfArgs ma = mdf_args(h, S);
+    const int wsmem = (int)h->mdf_wsmem;
+    if (use_persistent(h)) {
+        // a4 + the whole loop in one kernel: grid-wide barriers instead of 2 N + 1 dependent launches
+        K.persistent<<<h->mdfp_grid, MDFP_WARPS * 32, (size_t)MDFP_WARPS * h->mdf_wsmem, s>>>(
+            ma, src, h->po, sc->cursor, &sc->gbar, mdf_iters, wsmem);
+        CK(cudaGetLastError());
+        *n_kernels += 1;
+        return LBM_OK;
+    }
     if (pt) pt->mark(PH_MOMENTS, s);
     if (h->opt_moments == 1) {
         // the paper's box strategy: U on the bounding box of every body
@@ -533,6 +675,14 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
     for (int m = 0; m < mdf_iters; ++m) {
         const bool last = (m == mdf_iters - 1);
         if (pt) pt->mark(PH_INTERP, s);
+        if (fused) {
+            // product path: interpolate + correct + sweep in one tile pass, then the collect
+            K.tiles<<<h->mdf_grid, MDF_WARPS * 32, (size_t)MDF_WARPS * h->mdf_wsmem, s>>>(ma, &sc->cursor[m], last ? 1 : 0, wsmem);
+            if (pt) pt->mark(PH_SPREAD, s);
+            k_mdf_collect<<<LIST_GRID, 256, 0, s>>>(ma, last ? 1 : 0);
+            nk += 2;
+            continue;
+        }
         if (h->opt_interp == 1) k_interp_caller_order<<<(n + 127) / 128, 128, 0, s>>>(skey, S.inv, n, g, h->U, S.ms);
         else if (h->opt_interp == 2) k_interp_warp_per_marker<<<(int)(((long long)n * 32 + 255) / 256), 256, 0, s>>>(skey, n, g, h->U, S.ms);
         else if (h->opt_interp == 3 && h->opt_spread == 0)
@@ -542,21 +692,11 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
         ++nk;
         if (pt) pt->mark(PH_SPREAD, s);
         if (h->opt_spread == 0) {
-            // few tiles (a single propeller): one block per tile keeps all SMs busy; many: one warp per tile
-            // (tiles_hint = the tile count read back once after the first preparation of the current markers)
-            if (h->tiles_hint >= 0 && h->tiles_hint < SPREAD_WARP_FROM_TILES)
-                k_spread_tiles_block<<<h->rows_block_grid, BTILE_WARPS * 32, spread_tiles_block_smem(h->cg), s>>>(
-                    h->cg, S.tt.rec, S.tt.slot, S.tt.mask, &sc->n_tiles, h->tile_cap, &sc->cursor[m], S.ms.wx, S.ms.wyz,
-                    last ? S.ms.du : S.ms.sg, h->F);
-            else
-                k_spread_tiles<<<h->rows_grid, TILE_WARPS * 32, spread_tiles_smem(h->cg), s>>>(
-                    h->cg, S.tt.rec, S.tt.slot, S.tt.mask, &sc->n_tiles, h->tile_cap, &sc->cursor[m], S.tile_order, S.ms.wx,
-                    S.ms.wyz, last ? S.ms.du : S.ms.sg, h->F, (int)spread_warp_smem(h->cg));
-            const bool two = (g.wallx || g.nx >= CHUNK_ENT_MAX) && (g.wally || g.ny % TILE_R == 0) &&
-                             (g.wallz || g.nz % TILE_R == 0);
-            auto collect = last ? (two ? k_collect_tiles<true, 2> : k_collect_tiles<true, 4>)
-                                : (two ? k_collect_tiles<false, 2> : k_collect_tiles<false, 4>);
-            collect<<<LIST_GRID, 256, 0, s>>>(g, h->cg, h->tg, S.tt, h->F, S.cells, &sc->n_cells, last ? h->G : h->U);
+            // the round-1 pipeline (LBM_OPT_FUSED = 0): separate interpolation kernel, TMA-fed warp-per-tile sweep
+            k_spread_tiles<<<h->rows_grid, TILE_WARPS * 32, spread_tiles_smem(h->cg), s>>>(
+                h->cg, S.tt.rec, S.tt.slot, S.tt.mask, &sc->n_tiles, h->tile_cap, &sc->cursor[m], S.tile_order, S.ms.wx,
+                S.ms.wyz, last ? S.ms.du : S.ms.sg, S.fdst, h->F, (int)spread_warp_smem(h->cg));
+            k_mdf_collect<<<LIST_GRID, 256, 0, s>>>(ma, last ? 1 : 0);
             nk += 2;
         } else if (h->opt_spread == 2) {
             if (last)
@@ -691,7 +831,7 @@ int get_graph(lbm *h, int kind, int parity, int set, int mdf_iters, cudaGraphExe
                           ((long long)h->opt_spread << 40) | ((long long)h->opt_forcing << 44) |
                           ((long long)h->opt_lbm_kernel << 48) | ((long long)h->opt_interp << 52) |
                           ((long long)h->opt_overlap << 56) | ((long long)h->opt_moments << 58) |
-                          ((long long)(h->tiles_hint >= 0 && h->tiles_hint < SPREAD_WARP_FROM_TILES) << 60);
+                          ((long long)h->opt_fused << 60) | ((long long)h->tr << 16) | ((long long)use_persistent(h) << 20);
     auto it = h->graphs.find(key);
     if (it != h->graphs.end()) { *exec = it->second.first; *n_kernels = it->second.second; return LBM_OK; }
     cudaGraph_t graph = nullptr;
@@ -786,14 +926,7 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
     h->g.nx = nx; h->g.ny = ny; h->g.nz = nz;
     h->g.nxw = (nx + 31) / 32;
     h->g.cells = (long long)nx * ny * nz;
-    {
-        // plane padding: 0 by default; LBM_PLANE_PAD (floats, multiple of 4) for experiments
-        long long pad = 0;
-        if (const char *e = std::getenv("LBM_PLANE_PAD")) pad = std::atoll(e);
-        if (pad < 0) pad = 0;
-        pad = (pad + 3) / 4 * 4;
-        h->g.pitch = (h->g.cells + 3) / 4 * 4 + pad;
-    }
+    h->g.pitch = (h->g.cells + 3) / 4 * 4;   // plane padding was measured to make no difference (profiles/lbm_variants_r1.md)
     h->g.wallx = bc ? (bc->wall_x != 0) : 0;
     h->g.wally = bc ? (bc->wall_y != 0) : 0;
     h->g.wallz = bc ? (bc->wall_z != 0) : 0;
@@ -828,17 +961,14 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
     if (dmalloc(h, &h->scal, (size_t)1)) return bail("scalars");
     h->cg = chunk_geom(nx);
     h->chunk_slots = (size_t)h->cg.nbx * ny * nz;
-    h->tg = tile_geom(ny, nz);
-    h->tile_slots = (size_t)h->cg.nbx * h->tg.nty * h->tg.ntz;
+    h->tg = tile_geom(ny, nz);          // the tile tables are allocated with the markers (their edge depends on the set)
     bool ok = true;
     for (PrepSet &S : h->set) {
         if (dmalloc(h, &S.amask, h->n_mask_words) || dmalloc(h, &S.words, h->n_mask_words)) return bail("active mask");
         if (dmalloc(h, &S.chunk_of, h->chunk_slots)) return bail("chunk map");
-        if (dmalloc(h, &S.tt.mask, h->tile_slots) || dmalloc(h, &S.tt.id, h->tile_slots)) return bail("tile maps");
         if (dmalloc(h, &S.scal, (size_t)1)) return bail("set scalars");
         ok &= cudaMemset(S.amask, 0, h->n_mask_words * sizeof(unsigned)) == cudaSuccess;
         ok &= cudaMemset(S.chunk_of, 0xff, h->chunk_slots * sizeof(int)) == cudaSuccess;
-        ok &= cudaMemset(S.tt.mask, 0, h->tile_slots * sizeof(unsigned)) == cudaSuccess;
         ok &= cudaMemset(S.scal, 0, sizeof(SetScalars)) == cudaSuccess;
     }
     ok &= cudaMemset(h->f[0], 0, fcount * sizeof(float)) == cudaSuccess;   // rest state: f_i - t_i = 0
@@ -849,15 +979,11 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
     {
         int per_sm = 0, sms = 148;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device);
+        h->sms = sms;
         cudaFuncSetAttribute(k_spread_tiles, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)spread_tiles_smem(ChunkGeom{1, CHUNK_ENT_MAX}));
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spread_tiles, TILE_WARPS * 32, spread_tiles_smem(h->cg));
         h->rows_grid = std::max(1, per_sm) * sms;
-        cudaFuncSetAttribute(k_spread_tiles_block, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)spread_tiles_block_smem(ChunkGeom{1, CHUNK_ENT_MAX}));
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_spread_tiles_block, BTILE_WARPS * 32,
-                                                      spread_tiles_block_smem(h->cg));
-        h->rows_block_grid = std::max(1, per_sm) * sms;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_stream_collide_words, 256, 0);
         h->words_grid = std::max(1, per_sm) * sms;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moments_active, 256, 0);
@@ -876,7 +1002,6 @@ void lbm_destroy(lbm_t *h)
     cudaFree(h->f[0]); cudaFree(h->f[1]); cudaFree(h->U); cudaFree(h->G); cudaFree(h->scal);
     for (PrepSet &S : h->set) {
         cudaFree(S.amask); cudaFree(S.words); cudaFree(S.chunk_of); cudaFree(S.bin_first); cudaFree(S.scal);
-        cudaFree(S.tt.mask); cudaFree(S.tt.id);
     }
     for (int a = 0; a < 3; ++a) cudaFree(h->stage[a]);
     cudaFree(h->async_stage);
@@ -896,7 +1021,7 @@ int lbm_query_layout(int nx, int ny, int nz, int *out)
 {
     if (nx < 1 || ny < 1 || nz < 1 || !out) return fail(LBM_EINVAL, "lbm_query_layout: bad arguments");
     const ChunkGeom cg = chunk_geom(nx);
-    const TileGeom tg = tile_geom(ny, nz);
+    const TileGeom tg = tile_geom(ny, nz);   // for the 4 x 4-row tiles of large marker sets
     out[0] = cg.nbx; out[1] = cg.ent; out[2] = tg.nty; out[3] = tg.ntz; out[4] = (nx + 31) / 32;
     out[5] = CHUNK_W; out[6] = TILE_R; out[7] = CHUNK_ENT_MAX;
     return LBM_OK;
@@ -922,6 +1047,13 @@ int lbm_set_option(lbm_t *h, int key, int value)
         case LBM_OPT_MOMENTS: if (value < 0 || value > 2) break; h->opt_moments = value; return LBM_OK;
         case LBM_OPT_INTERP: if (value < 0 || value > 3) break; h->opt_interp = value; return LBM_OK;
         case LBM_OPT_TIMING: if (value < 0 || value > 1) break; h->opt_timing = value; h->timer.reset(); return LBM_OK;
+        case LBM_OPT_FUSED: if (value < 0 || value > 1) break; h->opt_fused = value; return LBM_OK;
+        case LBM_OPT_TILE_ROWS: if (value != 0 && value != 1 && value != 2 && value != 4) break; h->opt_tile_rows = value; return LBM_OK;
+        case LBM_OPT_PERSISTENT: if (value < 0 || value > 2) break; h->opt_persistent = value; return LBM_OK;
+        case LBM_OPT_TILE_CAP:
+            if (value < 0) break;
+            if (value != h->opt_tile_cap) { h->opt_tile_cap = value; h->realloc_tables = true; h->markers_stale = true; }
+            return LBM_OK;
         default: return fail(LBM_EINVAL, "lbm_set_option: unknown key %d", key);
     }
     return fail(LBM_EINVAL, "lbm_set_option: value %d out of range for key %d", value, key);
@@ -1130,6 +1262,7 @@ int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
     if (nsteps < 0 || mdf_iters < 0) return fail(LBM_EINVAL, "lbm_ibm_step: negative count");
     if (mdf_iters > MAX_MDF) return fail(LBM_EINVAL, "lbm_ibm_step: at most %d MDF iterations", MAX_MDF);
     if (nsteps == 0) return LBM_OK;
+    if (effective_tr(h) != h->tr) h->markers_stale = true;      // an option changed the tile edge: rebuild the tables
     int rc = upload_markers(h);
     if (rc) return rc;
     const bool ibm = (h->nm > 0 && mdf_iters > 0);
@@ -1142,18 +1275,6 @@ int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
         if ((rc = ensure_comparison_arrays(h))) return rc;
     }
     const bool overlapped = ibm && h->opt_overlap && h->opt_graph && !h->opt_timing;
-    if (ibm && h->opt_spread == 0 && h->tiles_hint < 0) {
-        // once per marker upload: prepare the first step now and read the tile count back (one stream
-        // synchronise); it only picks the sweep variant, results do not depend on it
-        PrepSet &S = h->set[h->cur_set];
-        int np = 0, nt = 0;
-        if ((rc = enqueue_prep(h, h->stream, S, 0, &np, nullptr))) return rc;
-        h->launches += np;
-        S.step = h->steps_done; S.spread = prep_signature(h); S.dirty = true;
-        CK(cudaMemcpyAsync(&nt, &S.scal->n_tiles, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
-        CK(cudaStreamSynchronize(h->stream));
-        h->tiles_hint = nt;
-    }
     for (int s = 0; s < nsteps; ++s) {
         int nk = 0;
         cudaGraphExec_t ex = nullptr;

@@ -1,0 +1,501 @@
+// The multi-direct-forcing loop as the product path runs it: per iteration ONE tile pass
+// that interpolates (a5), corrects (a6) and spreads (a7, stage A) and one collect pass (a7, stage B).
+//
+//   tile pass   one warp per tile (the chunks of one 8-cell x block whose source rows lie in one aligned
+//               TR x TR block of (y, z), see ibm_kernels.cuh).  The warp stages the tile's window of U^m
+//               -- (TR+3)^2 rows x (8+3) cells, every cell some marker of the tile can reach -- in ITS OWN
+//               shared memory, then takes the tile's markers 32 at a time:
+//                 phase 1, lane = marker: Peskin weights from the fractional position (3 square roots),
+//                   u^m(k) from the window (64 shared-memory reads instead of 64 global gathers),
+//                   g = u_k - u^m(k), Delta u += s g, and the marker's sweep record (value, x weights,
+//                   16 y-z weights) goes to the warp's staging buffer;
+//                 phase 2, lane = (half of the 4-cell x window, target-row offset (jy, jz)): the warp
+//                   sweeps the 32 staged markers in sorted order; the window slides along x, finished
+//                   cells are added to the tile's footprint in shared memory.
+//               Every sum has a fixed order: no atomics, no block-level barrier, bitwise reproducible.
+//               The value s g (or Delta u in the last iteration) never leaves the SM: the interpolation
+//               kernel, its `sg` round trip and the per-marker weight tables of the round-1 pipeline
+//               (96 B per marker and iteration) are gone; a marker costs 48 B read + 16 B written.
+//   collect     one thread per active cell adds the footprint elements that hold the cell (fixed order).
+//
+// Small marker sets (a single propeller) run the whole loop -- moments, N x (tile pass, collect) -- as
+// ONE persistent kernel with grid-wide barriers instead of 2N + 1 dependent launches, on tiles of a
+// single source row (TR = 1) so that a few thousand markers still spread over all SMs.
+#pragma once
+#include "ibm_kernels.cuh"
+
+namespace lbmk {
+
+constexpr int MDF_WARPS = 4;            // warps per block of the tile pass
+constexpr int MDF_BATCH = 32;           // markers per phase-1 / phase-2 round (= lanes)
+constexpr int MDF_STAGE_BYTES = MDF_BATCH * 96;
+
+struct MdfArgs {
+    Geom g;
+    ChunkGeom cg;
+    TileGeom tg;
+    // tiles of the marker set
+    const int2 *tile_rec;        // [tile][TR*TR] sorted-marker range of the chunk in source row sy + TR sz
+    const int *tile_slot;        // [tile] -> tile slot
+    const unsigned *tile_mask;   // [tile slot]
+    const int *tile_id;          // [tile slot] -> tile
+    const int *tile_order;       // tiles, longest first
+    const int *n_tiles;
+    int tile_cap;
+    // collect plan of the marker set (k_collect_plan): where every footprint element goes, and per active cell
+    // the run of elements it adds up
+    int *fdst;                   // [tile][(TR+3)^2 * ent] -> index into F, or -1 (no cell consumes the element)
+    int2 *cell_run;              // [active cell k] (first element in F, number of elements)
+    int *n_felem;                // elements handed out so far (plan construction)
+    // markers in sorted order
+    const float4 *fs;            // (fx, fy, fz, s)
+    const float4 *uk;            // u_k
+    float4 *du;                  // Delta u, w = cell x index
+    // fields
+    float4 *U, *G;
+    float4 *F;                   // footprint elements, grouped by the cell that consumes them
+    const int *cells;            // active-cell list
+    const int *n_cells;
+};
+
+inline size_t mdf_warp_smem(int tr, const ChunkGeom &cg)
+{
+    const size_t tf = (size_t)tr + 3;
+    const size_t win = (tf * tf * (size_t)cg.ent * 16 + 127) / 128 * 128;
+    const size_t foot = (tf * tf * (size_t)cg.ent * 12 + 127) / 128 * 128;
+    return win + foot + MDF_STAGE_BYTES;
+}
+
+__device__ __forceinline__ int mod_wrap(int i, int n)
+{
+    i %= n;
+    return i < 0 ? i + n : i;
+}
+
+__device__ __forceinline__ void cp_async16_cg(void *smem_dst, const void *gsrc)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// One tile, one warp.  wsm = the warp's shared memory (mdf_warp_smem bytes).
+template <int TR>
+__device__ __forceinline__ void mdf_tile_pass(const MdfArgs &a, const int t, const bool last, char *wsm, const int lane)
+{
+    constexpr int NR = TR * TR, TF = TR + 3, NROWS = TF * TF;
+    constexpr unsigned FULL = 0xffffffffu;
+    const int ent = a.cg.ent;
+    const int l = lane & 15, h = lane >> 4;
+    const int jy = l >> 2, jz = l & 3;
+    const size_t win_bytes = ((size_t)NROWS * ent * 16 + 127) / 128 * 128;
+    const size_t foot_bytes = ((size_t)NROWS * ent * 12 + 127) / 128 * 128;
+    float4 *win = reinterpret_cast<float4 *>(wsm);                       // [NROWS][ent] U^m (w unused)
+    float *foot = reinterpret_cast<float *>(wsm + win_bytes);            // [NROWS][ent][3]
+    float4 *sv = reinterpret_cast<float4 *>(wsm + win_bytes + foot_bytes);   // staged value + tag
+    float4 *swx = sv + MDF_BATCH;                                        // staged x weights
+    float *swyz = reinterpret_cast<float *>(swx + MDF_BATCH);            // staged y-z weights [32][16]
+
+    // ---- tile header: chunk ranges, their inclusive prefix, geometry ------------------------------
+    int2 rec = make_int2(0, 0);
+    if (lane < NR) rec = __ldg(a.tile_rec + (size_t)t * NR + lane);
+    const int ts = __ldg(a.tile_slot + t);
+    const unsigned m = __ldg(a.tile_mask + ts);
+    const int cnt = rec.y - rec.x;
+    int incl = cnt;
+#pragma unroll
+    for (int o = 1; o < NR; o <<= 1) {
+        const int v = __shfl_up_sync(FULL, incl, o);
+        if (lane >= o) incl += v;
+    }
+    const int total = __shfl_sync(FULL, incl, NR - 1);
+    const int blk = ts % a.cg.nbx, tyz = ts / a.cg.nbx;
+    const int ty = tyz % a.tg.nty, tz = tyz / a.tg.nty;
+    const int x0 = blk * CHUNK_W;
+    const bool ex = l < ent && ((m >> l) & 1u);              // this lane's window entry is reachable
+
+    // ---- stage the window of U^m: asynchronous 16-byte copies, half a warp per row ---------------------
+    // (row coordinates: ty TR - 1 + fy lies in [-1, ny + 4], so one conditional wrap is enough for ny >= 4)
+    {
+        const int x = mod_wrap(x0 - 1 + l, a.g.nx);
+        const int ybase = ty * TR - 1, zbase = tz * TR - 1;
+#pragma unroll 1
+        for (int fyz = h; fyz < NROWS; fyz += 2) {
+            const int fy = fyz / TF, fz = fyz - fy * TF;
+            if (ex && ((m >> (14 + fy)) & (m >> (21 + fz)) & 1u)) {
+                int y = ybase + fy, z = zbase + fz;
+                if (a.g.wally) y = min(max(y, 0), a.g.ny - 1); else { if (y < 0) y += a.g.ny; else if (y >= a.g.ny) y -= a.g.ny; }
+                if (a.g.wallz) z = min(max(z, 0), a.g.nz - 1); else { if (z < 0) z += a.g.nz; else if (z >= a.g.nz) z -= a.g.nz; }
+                cp_async16_cg(win + fyz * ent + l, a.U + (size_t)(z * a.g.ny + y) * a.g.nx + x);
+            }
+        }
+    }
+
+    // the markers of one batch: (source row, sorted index) of this lane's marker, its data in registers
+    struct Pre { float4 fs, uk, du; int r, i; };
+    auto fetch = [&](int base, Pre &pf) {
+        const int j = base + lane;
+        int r = 0;
+#pragma unroll
+        for (int step = NR / 2; step >= 1; step >>= 1) {     // the first r with incl[r] > j
+            const int v = __shfl_sync(FULL, incl, r + step - 1);
+            if (j >= v) r += step;
+        }
+        const int r_first = __shfl_sync(FULL, rec.x, r);
+        const int r_incl = __shfl_sync(FULL, incl, r), r_cnt = __shfl_sync(FULL, cnt, r);
+        pf.r = r;
+        pf.i = r_first + (j - (r_incl - r_cnt));
+        if (j < total) {
+            pf.fs = __ldg(a.fs + pf.i);
+            pf.uk = __ldg(a.uk + pf.i);
+            pf.du = __ldcg(a.du + pf.i);
+        }
+    };
+    Pre cur;
+    fetch(0, cur);                                       // in flight together with the window copies
+
+    // zero the footprint meanwhile
+    {
+        float4 *f4 = reinterpret_cast<float4 *>(foot);
+        const int n4 = (int)(foot_bytes / 16);
+        for (int i = lane; i < n4; i += 32) f4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    cp_async_wait_all();
+    __syncwarp();
+
+    // ---- the tile's markers, 32 at a time -------------------------------------------------------------
+    int tag_cur = -1;                            // (source row << 8) | window start of the sweep, -1 = none yet
+    int e = 0;
+    float *frow = foot;
+    Acc3 p{0.f, 0.f, 0.f}, q{0.f, 0.f, 0.f};     // window cells (e + 2h, e + 2h + 1)
+    auto flush = [&](int ee, const Acc3 &acc) {
+        float *d = frow + ee * 3;
+        d[0] += acc.x; d[1] += acc.y; d[2] += acc.z;
+    };
+    const float2 *sw2 = reinterpret_cast<const float2 *>(swx) + h;
+    const float *swz = swyz + l;
+    for (int base = 0; base < total; base += MDF_BATCH) {
+        const int nb = min(MDF_BATCH, total - base);
+        if (lane < nb) {
+            // ---- phase 1: interpolate, correct, stage ----------------
+            const float4 fs = cur.fs, uk = cur.uk;
+            float4 d = cur.du;
+            const int e0 = __float_as_int(d.w) - x0;             // window entry of cell cx - 1
+            const int sy = cur.r % TR, sz = cur.r / TR;
+            float wx[4], wy[4], wz[4];
+            peskin4(fs.x, wx);
+            peskin4(fs.y, wy);
+            peskin4(fs.z, wz);
+            const float4 *w0 = win + (sy * TF + sz) * ent + e0;
+            float ux = 0.f, uy = 0.f, uz = 0.f;
+            float4 *my_wyz = reinterpret_cast<float4 *>(swyz + lane * 16);
+#pragma unroll
+            for (int ky = 0; ky < 4; ++ky) {
+                float wyz[4];
+#pragma unroll
+                for (int kz = 0; kz < 4; ++kz) {
+                    wyz[kz] = wy[ky] * wz[kz];
+                    const float4 *rowp = w0 + (ky * TF + kz) * ent;
+                    const float4 c0 = rowp[0], c1 = rowp[1], c2 = rowp[2], c3 = rowp[3];
+                    const float tx = fmaf(wx[3], c3.x, fmaf(wx[2], c2.x, fmaf(wx[1], c1.x, wx[0] * c0.x)));
+                    const float ty_ = fmaf(wx[3], c3.y, fmaf(wx[2], c2.y, fmaf(wx[1], c1.y, wx[0] * c0.y)));
+                    const float tz_ = fmaf(wx[3], c3.z, fmaf(wx[2], c2.z, fmaf(wx[1], c1.z, wx[0] * c0.z)));
+                    ux = fmaf(wyz[kz], tx, ux);
+                    uy = fmaf(wyz[kz], ty_, uy);
+                    uz = fmaf(wyz[kz], tz_, uz);
+                }
+                my_wyz[ky] = make_float4(wyz[0], wyz[1], wyz[2], wyz[3]);
+            }
+            const float gx = uk.x - ux, gy = uk.y - uy, gz = uk.z - uz;
+            d.x = fmaf(fs.w, gx, d.x);
+            d.y = fmaf(fs.w, gy, d.y);
+            d.z = fmaf(fs.w, gz, d.z);
+            a.du[cur.i] = d;
+            const float tagf = __int_as_float((cur.r << 8) | e0);
+            sv[lane] = last ? make_float4(d.x, d.y, d.z, tagf) : make_float4(fs.w * gx, fs.w * gy, fs.w * gz, tagf);
+            swx[lane] = make_float4(wx[0], wx[1], wx[2], wx[3]);
+        }
+        if (base + MDF_BATCH < total) fetch(base + MDF_BATCH, cur);          // in flight during the sweep
+        __syncwarp();
+
+        // ---- phase 2: sweep the staged markers in sorted order (warp-uniform control flow) ----------------
+#pragma unroll 2
+        for (int jj = 0; jj < nb; ++jj) {
+            const float4 v = sv[jj];
+            const float2 w = sw2[2 * jj];
+            const float wz_ = swz[16 * jj];
+            const int tg_ = __float_as_int(v.w);
+            if (tg_ != tag_cur) {                        // the sweep moves on to another cell or another source row
+                const int rn = tg_ >> 8, en = tg_ & 0xff;
+                if ((tg_ ^ tag_cur) >> 8) {              // another source row (or the first marker of the tile)
+                    if (tag_cur >= 0) { flush(e + 2 * h, p); flush(e + 2 * h + 1, q); }
+                    frow = foot + (((rn % TR) + jy) * TF + ((rn / TR) + jz)) * ent * 3;
+                    p = Acc3{0.f, 0.f, 0.f}; q = Acc3{0.f, 0.f, 0.f};
+                    e = en;
+                } else {
+#pragma unroll 1
+                    do {                                 // the leftmost window cell is complete
+                        if (h == 0) flush(e, p);
+                        const float tx = __shfl_down_sync(FULL, p.x, 16);
+                        const float ty_ = __shfl_down_sync(FULL, p.y, 16);
+                        const float tz_ = __shfl_down_sync(FULL, p.z, 16);
+                        p = q;
+                        q.x = h ? 0.f : tx; q.y = h ? 0.f : ty_; q.z = h ? 0.f : tz_;
+                    } while (++e < en);
+                }
+                tag_cur = tg_;
+            }
+            const float vx = v.x * wz_, vy = v.y * wz_, vz = v.z * wz_;
+            p.x = fmaf(w.x, vx, p.x); p.y = fmaf(w.x, vy, p.y); p.z = fmaf(w.x, vz, p.z);
+            q.x = fmaf(w.y, vx, q.x); q.y = fmaf(w.y, vy, q.y); q.z = fmaf(w.y, vz, q.z);
+        }
+        __syncwarp();                                    // every lane is done with the staging buffer
+    }
+    if (tag_cur >= 0) { flush(e + 2 * h, p); flush(e + 2 * h + 1, q); }
+    __syncwarp();
+
+    // ---- hand every footprint element to the cell that consumes it (plan: fdst) ------------------------
+    {
+        const int *__restrict__ dst = a.fdst + (size_t)t * (NROWS * ent);
+#pragma unroll 1
+        for (int fyz = h; fyz < NROWS; fyz += 2) {
+            const int fy = fyz / TF, fz = fyz - fy * TF;
+            if (ex && ((m >> (14 + fy)) & (m >> (21 + fz)) & 1u)) {
+                const int o = __ldg(dst + fyz * ent + l);
+                if (o >= 0) {
+                    const float *s = foot + (fyz * ent + l) * 3;
+                    __stcg(a.F + o, make_float4(s[0], s[1], s[2], 0.f));
+                }
+            }
+        }
+    }
+    __syncwarp();
+}
+
+// tile pass as a kernel of its own: persistent grid, tiles handed out longest first through a cursor
+template <int TR>
+__global__ void __launch_bounds__(MDF_WARPS * 32)
+k_mdf_tiles(const __grid_constant__ MdfArgs a, int *__restrict__ cursor, int last, int warp_smem)
+{
+    extern __shared__ __align__(128) char smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int nt = min(*a.n_tiles, a.tile_cap);
+    char *wsm = smem + (size_t)warp * warp_smem;
+    for (;;) {
+        int t = 0;
+        if (lane == 0) { t = atomicAdd(cursor, 1); t = t < nt ? __ldg(a.tile_order + t) : nt; }
+        t = __shfl_sync(0xffffffffu, t, 0);
+        if (t >= nt) break;
+        mdf_tile_pass<TR>(a, t, last != 0, wsm, lane);
+    }
+}
+
+// ---- stage B ---------------------------------------------------------------------------------------
+// Candidates along one axis for the cell coordinate X: source coordinate c = X + 1 - j (wrapped, or
+// skipped outside a wall axis); tile = c / tile width (blocks in x: chunk_block); footprint coordinate =
+// offset of c in its tile + j.  Distinct (tile, coordinate) pairs only.
+template <int MAXC>
+struct AxisCandT { int t[MAXC], f[MAXC], n; };
+
+template <bool IS_X, int TR, int MAXC>
+__device__ __forceinline__ void axis_candidates_t(int X, int n, int wall, int nbx, AxisCandT<MAXC> &a)
+{
+    a.n = 0;
+    int pt = -1, pf = -1;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        int c = X + 1 - j;
+        if (wall) { if (c < 0 || c >= n) continue; } else c = wrap(c, n);
+        const int t = IS_X ? chunk_block(c, nbx) : c / TR;
+        const int f = c - t * (IS_X ? CHUNK_W : TR) + j;
+        if (t != pt || f != pf) {
+#pragma unroll
+            for (int i = 0; i < MAXC; ++i) if (i == a.n) { a.t[i] = t; a.f[i] = f; }
+            ++a.n; pt = t; pf = f;
+        }
+    }
+}
+
+// Collect plan, once per time step (binning stage): every active cell finds the footprint elements of the
+// tiles that hold it -- the markers that reach cell X sit in the source cells (X+1-jx, y+1-jy, z+1-jz); per
+// axis these four coordinates meet one or two tiles (up to four for single-row tiles and tiny lattices) --
+// takes a run of that many slots of F and tells each element where to go (fdst).  The order inside a run is
+// fixed (z, y, x candidates ascending), so the sum a cell forms is bitwise reproducible although the position of
+// its run is not.  fdst of the tiles in use is pre-set to -1 (k_fill_tiles).
+template <int TR, int MAXCX, int MAXCYZ>
+__global__ void __launch_bounds__(256)
+k_collect_plan(const __grid_constant__ MdfArgs a)
+{
+    constexpr int TF = TR + 3;
+    const Geom &g = a.g;
+    const int lane = threadIdx.x & 31;
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int stride = gridDim.x * blockDim.x;
+    const int nc = *a.n_cells;
+    for (int k0 = tid - lane; k0 < nc; k0 += stride) {
+        const int k = k0 + lane;
+        AxisCandT<MAXCX> ax;
+        AxisCandT<MAXCYZ> ay, az;
+        ax.n = ay.n = az.n = 0;
+        if (k < nc) {
+            const int cell = __ldg(a.cells + k);
+            const int row = cell / g.nx;
+            const int x = cell - row * g.nx;
+            const int z = row / g.ny, y = row - z * g.ny;
+            axis_candidates_t<true, TR, MAXCX>(x, g.nx, g.wallx, a.cg.nbx, ax);
+            axis_candidates_t<false, TR, MAXCYZ>(y, g.ny, g.wally, 0, ay);
+            axis_candidates_t<false, TR, MAXCYZ>(z, g.nz, g.wallz, 0, az);
+        }
+        auto for_each = [&](auto &&f) {
+#pragma unroll
+            for (int iz = 0; iz < MAXCYZ; ++iz)
+#pragma unroll
+                for (int iy = 0; iy < MAXCYZ; ++iy)
+#pragma unroll
+                    for (int ix = 0; ix < MAXCX; ++ix) {
+                        if (iz >= az.n || iy >= ay.n || ix >= ax.n) continue;
+                        const int ts = tile_slot_of(ax.t[ix], ay.t[iy], az.t[iz], a.cg, a.tg);
+                        const unsigned m = __ldg(a.tile_mask + ts);
+                        if (!((m >> ax.f[ix]) & (m >> (14 + ay.f[iy])) & (m >> (21 + az.f[iz])) & 1u)) continue;
+                        const int id = __ldg(a.tile_id + ts);
+                        if (id < 0 || id >= a.tile_cap) continue;
+                        f(((size_t)id * (TF * TF) + ay.f[iy] * TF + az.f[iz]) * a.cg.ent + ax.f[ix]);
+                    }
+        };
+        int cnt = 0;
+        for_each([&](size_t) { ++cnt; });
+        int incl = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        const int total = __shfl_sync(0xffffffffu, incl, 31);
+        int base = 0;
+        if (lane == 31 && total) base = atomicAdd(a.n_felem, total);
+        base = __shfl_sync(0xffffffffu, base, 31);
+        if (k < nc) {
+            int o = base + incl - cnt;
+            a.cell_run[k] = make_int2(o, cnt);
+            for_each([&](size_t el) { a.fdst[el] = o++; });
+        }
+    }
+}
+
+// fdst of every tile in use := -1 (elements of the mask product that no active cell consumes stay there)
+__global__ void __launch_bounds__(256)
+k_fill_tiles(int *__restrict__ fdst, const int *__restrict__ n_tiles, int tile_cap, int elems_per_tile)
+{
+    const size_t n = (size_t)min(*n_tiles, tile_cap) * (size_t)elems_per_tile;
+    int4 *d4 = reinterpret_cast<int4 *>(fdst);
+    const size_t n4 = n / 4;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x)
+        d4[i] = make_int4(-1, -1, -1, -1);
+    if (blockIdx.x == 0 && threadIdx.x < (int)(n - 4 * n4)) fdst[4 * n4 + threadIdx.x] = -1;
+}
+
+// One active cell adds up its run of footprint elements, in order.
+//   last = false:  U^{m+1}(X) = U^m(X) + sum   (R8)      last = true:  G(X) = sum
+__device__ __forceinline__ void mdf_collect_cell(const MdfArgs &a, const int k, const bool last)
+{
+    const int cell = __ldg(a.cells + k);
+    const int2 run = __ldg(a.cell_run + k);
+    const float4 *__restrict__ f = a.F + run.x;
+    float sx = 0.f, sy = 0.f, sz = 0.f;
+    for (int i0 = 0; i0 < run.y; i0 += 8) {
+        float4 v[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) v[i] = (i0 + i < run.y) ? __ldcg(f + i0 + i) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { sx += v[i].x; sy += v[i].y; sz += v[i].z; }
+    }
+    if (last) {
+        a.G[cell] = make_float4(sx, sy, sz, 0.f);
+    } else {
+        float4 u = __ldcg(a.U + cell);
+        u.x += sx; u.y += sy; u.z += sz;
+        a.U[cell] = u;
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_mdf_collect(const __grid_constant__ MdfArgs a, int last)
+{
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int stride = gridDim.x * blockDim.x;
+    const int nc = *a.n_cells;
+    for (int k = tid; k < nc; k += stride) mdf_collect_cell(a, k, last != 0);
+}
+
+// ---- the whole loop as one persistent kernel ---------------------------------------------------------
+// Grid-wide barrier on a monotonic counter (re-armed by the set's next preparation).  All blocks of the
+// grid are resident (the host sizes the grid from the occupancy query); blocks of other kernels that
+// share the SMs always retire, so the barrier cannot dead-lock.
+__device__ __forceinline__ void grid_barrier(unsigned *bar, unsigned &target)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        target += gridDim.x;
+        __threadfence();
+        atomicAdd(bar, 1u);
+        unsigned v;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(bar) : "memory");
+        } while (v < target);
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+// a4 for one cell of the active list (same arithmetic as k_moments_active)
+__device__ __forceinline__ void moments_cell(const float *__restrict__ src, const Geom &g, const PlaneOffsets &po,
+                                             const int cell, float4 *__restrict__ U)
+{
+    const int row = cell / g.nx;
+    const int x = cell - row * g.nx;
+    const int z = row / g.ny, y = row - z * g.ny;
+    float df[NQ], drho, ux, uy, uz;
+    const bool xwall = g.wallx && (x == 0 || x == g.nx - 1);
+    if (y > 0 && y < g.ny - 1 && z > 0 && z < g.nz - 1 && !xwall) {
+        pull_cell_inner(src, g, po, x, cell, df);
+    } else {
+        const Nbr n = neighbours(g, x, y, z);
+        pull_cell(src, g, n, x, y, z, df);
+    }
+    moments(df, drho, ux, uy, uz);
+    U[cell] = make_float4(ux, uy, uz, 1.0f + drho);
+}
+
+constexpr int MDFP_WARPS = 8;           // warps per block of the persistent kernel
+
+template <int TR>
+__global__ void __launch_bounds__(MDFP_WARPS * 32)
+k_mdf_persistent(const __grid_constant__ MdfArgs a, const float *__restrict__ src, const __grid_constant__ PlaneOffsets po,
+                 int *__restrict__ cursors, unsigned *__restrict__ bar, int mdf_iters, int warp_smem)
+{
+    extern __shared__ __align__(128) char smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int stride = gridDim.x * blockDim.x;
+    char *wsm = smem + (size_t)warp * warp_smem;
+    const int nt = min(*a.n_tiles, a.tile_cap);
+    const int nc = *a.n_cells;
+    unsigned target = 0u;
+    // a4: rho, U of eq. (1) on the active cells
+    for (int k = tid; k < nc; k += stride) moments_cell(src, a.g, po, __ldg(a.cells + k), a.U);
+    grid_barrier(bar, target);
+    for (int it = 0; it < mdf_iters; ++it) {
+        const bool last = (it == mdf_iters - 1);
+        for (;;) {
+            int t = 0;
+            if (lane == 0) { t = atomicAdd(cursors + it, 1); t = t < nt ? __ldg(a.tile_order + t) : nt; }
+            t = __shfl_sync(0xffffffffu, t, 0);
+            if (t >= nt) break;
+            mdf_tile_pass<TR>(a, t, last, wsm, lane);
+        }
+        grid_barrier(bar, target);
+        for (int k = tid; k < nc; k += stride) mdf_collect_cell(a, k, last);
+        if (!last) grid_barrier(bar, target);
+    }
+}
+
+}  // namespace lbmk
