@@ -189,6 +189,9 @@ def run_ours(args):
     sim = api.from_workload(wl, stream=stream)
     sim.set_option(api.OPT_SPREAD, {"gather": 0, "atomic": 1, "plain": 2}[args.spread])
     sim.set_option(api.OPT_LBM_KERNEL, {"auto": 0, "scalar": 1, "vec4": 2}[args.lbm_kernel])
+    for kv in args.opt:
+        name, val = kv.split("=")
+        sim.set_option(getattr(api, "OPT_" + name.upper()), int(val))
 
     def barrier():
         torch.cuda.synchronize()
@@ -409,6 +412,8 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=10)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--quick", action="store_true", help="skip the extra W2 pure-LBM run")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="set a library option (lbm_set_option), e.g. --opt tile_rows=2 --opt persistent=2")
     ap.add_argument("--compare", action="store_true",
                     help="also time the paper's own kernel designs (box / per-marker U precompute, ib_force1, ib_force2)")
     args = ap.parse_args()

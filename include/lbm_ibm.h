@@ -97,10 +97,13 @@ enum {
     LBM_OPT_PERSISTENT = 11, /* the fused MDF loop (moments + N x (tile pass, collect)) as ONE persistent kernel
                              with grid-wide barriers instead of 2 N + 1 launches: 0 = automatic (marker sets up
                              to 100,000 points), 1 = always, 2 = never.  Results are bit-identical.         */
-    LBM_OPT_TILE_CAP = 12 /* > 0: cap the number of tile footprints (default 0 = room for every tile that can
+    LBM_OPT_TILE_CAP = 12, /* > 0: cap the number of tile footprints (default 0 = room for every tile that can
                              exist, up to 12 GB).  More tiles than the cap are dropped for that step and
                              lbm_sync reports LBM_ENOMEM; later steps that fit are complete again.  Takes
                              effect at the next step (the tables are re-allocated).                    */
+    LBM_OPT_MDF_BLOCKS = 13 /* tuning: blocks per SM of the tile pass / of the persistent MDF kernel (0 = default:
+                             as many as fit / one); fewer blocks leave more of every SM to the stream-collide
+                             pass that runs beside the MDF loop.  Results do not depend on it.           */
 };
 
 /* Keys for lbm_get_info. */

@@ -698,6 +698,10 @@ struct TileTable {
     int *id;             // [tile slots] dense: footprint index of the tile (valid where mask != 0)
     int *slot;           // [tile ids] -> tile slot
     int2 *rec;           // [tile ids][tr*tr]: sorted-marker range [first, end) of the chunk in source row sy + tr sz, (0,0) = none
+    // the same records in processing order (longest tile first), so that a warp that draws position k from the work
+    // cursor finds everything about its tile with one round of loads
+    int4 *ohdr;          // [position] (tile slot, reach mask, tile id, markers of the tile)
+    int2 *orec;          // [position][tr*tr] as rec
 };
 
 __device__ __forceinline__ int tile_slot_of(int blk, int ty, int tz, const ChunkGeom &cg, const TileGeom &tg)
@@ -786,7 +790,12 @@ k_tile_place(TileTable tt, int nr, const int *__restrict__ n_tiles, int tile_cap
         const int c = tile_size_class(tt.rec + (size_t)t * nr, nr);
         int base = 0;
         for (int q = 0; q < c; ++q) base += bucket[q];
-        order[base + atomicAdd(bucket + 8 + c, 1)] = t;
+        const int pos = base + atomicAdd(bucket + 8 + c, 1);
+        order[pos] = t;
+        int n = 0;
+        for (int r = 0; r < nr; ++r) { const int2 v = tt.rec[(size_t)t * nr + r]; tt.orec[(size_t)pos * nr + r] = v; n += v.y - v.x; }
+        const int ts = tt.slot[t];
+        tt.ohdr[pos] = make_int4(ts, (int)tt.mask[ts], t, n);
     }
 }
 

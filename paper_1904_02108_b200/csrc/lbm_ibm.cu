@@ -121,11 +121,12 @@ struct PrepSet {
     int *vals[2] = {nullptr, nullptr};        // the permutation, same ping-pong
     MarkerSorted ms{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     ChunkTable ct{nullptr, nullptr, nullptr};
-    TileTable tt{nullptr, nullptr, nullptr, nullptr};  // mask, id: dense over the tile slots; slot, rec: per tile
+    TileTable tt{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};  // mask, id: dense over the tile slots; slot, rec: per tile; ohdr, orec: per position
     int *tile_order = nullptr;                // tiles by decreasing marker count (size classes)
     int *ovf_slot = nullptr;                  // tile slots registered without a footprint (table overflow), OVF_CAP entries
     int *fdst = nullptr;                      // collect plan: [tile][footprint element] -> index into F or -1
     int2 *cell_run = nullptr;                 // collect plan: [active cell] (first element in F, count)
+    BodyStep *tabs = nullptr;                 // per-body rotation tables of the time step the set is prepared for (a1)
     int *inv = nullptr;                       // inverse permutation (comparison LBM_OPT_INTERP = 1 only; lazy)
     unsigned *headbits = nullptr;             // one bit per sorted marker: starts a run
     int *cells = nullptr;                     // active-cell list
@@ -172,7 +173,6 @@ struct lbm {
     float *d_q[3] = {nullptr, nullptr, nullptr}, *d_v[3] = {nullptr, nullptr, nullptr}, *d_s = nullptr;
     int *d_body = nullptr;
     BodyDef *d_defs = nullptr;
-    BodyStep *d_tabs = nullptr;
     int *d_hist = nullptr, *d_total = nullptr;
     size_t cells_cap = 0, headbits_cap = 0;
     float4 *F = nullptr;                // tile footprints [tile][7][7][cg.ent]
@@ -190,7 +190,7 @@ struct lbm {
 
     int opt_spread = 0, opt_forcing = 0, opt_graph = 1, opt_lbm_kernel = 0, opt_interp = 0, opt_timing = 0;
     int opt_overlap = 1, opt_moments = 0;
-    int opt_fused = 1, opt_tile_rows = 0, opt_persistent = 0, opt_tile_cap = 0;
+    int opt_fused = 1, opt_tile_rows = 0, opt_persistent = 0, opt_tile_cap = 0, opt_mdf_blocks = 0;
     bool realloc_tables = false;        // LBM_OPT_TILE_CAP changed: the tile tables are re-allocated at the next step
     int *d_box = nullptr;               // per-body bounding boxes (comparison LBM_OPT_MOMENTS = 1 only; lazy)
     PhaseTimer timer;
@@ -268,11 +268,14 @@ void free_set(lbm *h, PrepSet &S)
     dfree(h, S.ct.first, (size_t)h->chunk_cap); dfree(h, S.ct.end, (size_t)h->chunk_cap);
     dfree(h, S.ct.slot, (size_t)h->chunk_cap);
     dfree(h, S.tt.slot, (size_t)h->tile_cap);
+    dfree(h, S.tt.ohdr, (size_t)h->tile_cap);
+    dfree(h, S.tt.orec, (size_t)h->tile_cap * (size_t)(h->tr * h->tr));
     dfree(h, S.tt.rec, (size_t)h->tile_cap * (size_t)(h->tr * h->tr));
     dfree(h, S.tile_order, (size_t)h->tile_cap);
     dfree(h, S.ovf_slot, (size_t)OVF_CAP);
     dfree(h, S.fdst, (size_t)h->tile_cap * (size_t)((h->tr + 3) * (h->tr + 3)) * (size_t)h->cg.ent);
     dfree(h, S.cell_run, h->cells_cap);
+    dfree(h, S.tabs, (size_t)h->nb_cap);
     dfree(h, S.tt.mask, h->tile_slots); dfree(h, S.tt.id, h->tile_slots);
     dfree(h, S.inv, c);
     dfree(h, S.cells, h->cells_cap);
@@ -294,7 +297,6 @@ void free_markers_dev(lbm *h)
     dfree(h, h->d_total, (size_t)RADIX);
     dfree(h, h->d_box, (size_t)6 * (size_t)h->nb_cap);
     dfree(h, h->d_defs, (size_t)h->nb_cap);
-    dfree(h, h->d_tabs, (size_t)h->nb_cap);
     h->nm_cap = 0; h->nb_cap = 0; h->sort_tiles = 0;
 }
 
@@ -418,7 +420,7 @@ MdfKernels mdf_kernels(const lbm *h)
     }
 }
 
-constexpr int MDFP_BLOCKS_PER_SM = 2;   // the persistent kernel leaves room for the bulk stream-collide beside it
+constexpr int MDFP_BLOCKS_PER_SM = 1;   // the persistent kernel leaves room for the bulk stream-collide beside it
 
 int mdf_launch_geometry(lbm *h)
 {
@@ -428,10 +430,11 @@ int mdf_launch_geometry(lbm *h)
     CK(cudaFuncSetAttribute((const void *)K.persistent, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p));
     int per_sm = 0;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, K.tiles, MDF_WARPS * 32, smem_t));
+    if (h->opt_mdf_blocks > 0) per_sm = std::min(per_sm, h->opt_mdf_blocks);
     h->mdf_grid = std::max(1, per_sm) * h->sms;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, K.persistent, MDFP_WARPS * 32, smem_p));
     if (per_sm < 1) return fail(LBM_ECUDA, "the persistent MDF kernel does not fit on an SM (%zu bytes of shared memory)", smem_p);
-    h->mdfp_grid = std::min(per_sm, MDFP_BLOCKS_PER_SM) * h->sms;
+    h->mdfp_grid = std::min(per_sm, h->opt_mdf_blocks > 0 ? h->opt_mdf_blocks : MDFP_BLOCKS_PER_SM) * h->sms;
     return LBM_OK;
 }
 
@@ -439,7 +442,7 @@ MdfArgs mdf_args(const lbm *h, const PrepSet &S)
 {
     MdfArgs a{};
     a.g = h->g; a.cg = h->cg; a.tg = h->tg;
-    a.tile_rec = S.tt.rec; a.tile_slot = S.tt.slot; a.tile_mask = S.tt.mask; a.tile_id = S.tt.id;
+    a.tile_rec = S.tt.rec; a.tile_slot = S.tt.slot; a.tile_mask = S.tt.mask; a.tile_id = S.tt.id; a.tile_ohdr = S.tt.ohdr; a.tile_orec = S.tt.orec;
     a.tile_order = S.tile_order; a.n_tiles = &S.scal->n_tiles; a.tile_cap = h->tile_cap;
     a.fdst = S.fdst; a.cell_run = S.cell_run; a.n_felem = &S.scal->n_felem;
     a.fs = S.ms.fs; a.uk = S.ms.uk; a.du = S.ms.du;
@@ -493,6 +496,8 @@ int upload_markers(lbm *h)
             if ((rc = dmalloc(h, &S.ct.end, (size_t)ccap))) return rc;
             if ((rc = dmalloc(h, &S.ct.slot, (size_t)ccap))) return rc;
             if ((rc = dmalloc(h, &S.tt.slot, tcap))) return rc;
+            if ((rc = dmalloc(h, &S.tt.ohdr, tcap))) return rc;
+            if ((rc = dmalloc(h, &S.tt.orec, tcap * (size_t)(tr * tr)))) return rc;
             if ((rc = dmalloc(h, &S.tt.rec, tcap * (size_t)(tr * tr)))) return rc;
             if ((rc = dmalloc(h, &S.tile_order, tcap))) return rc;
             if ((rc = dmalloc(h, &S.ovf_slot, (size_t)OVF_CAP))) return rc;
@@ -511,7 +516,7 @@ int upload_markers(lbm *h)
         if ((rc = mdf_launch_geometry(h))) return rc;
         if ((rc = dmalloc(h, &h->d_total, (size_t)RADIX))) return rc;
         if ((rc = dmalloc(h, &h->d_defs, (size_t)nb))) return rc;
-        if ((rc = dmalloc(h, &h->d_tabs, (size_t)nb))) return rc;
+        for (PrepSet &S : h->set) if ((rc = dmalloc(h, &S.tabs, (size_t)nb))) return rc;
         h->nm_cap = n; h->nb_cap = nb;
     }
     h->nm = n;
@@ -583,9 +588,9 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
                                            S.ct.slot, &sc->n_chunks, h->chunk_cap, S.tt.mask, S.tt.slot, &sc->n_tiles, h->tile_cap,
                                            S.ovf_slot, &sc->n_ovf, OVF_CAP, (int)h->tile_slots);
     const int nb = (int)h->bodies.size();
-    k_kinematics<<<(std::max(nb, N_STEP_COUNTERS) + 127) / 128, 128, 0, s>>>(h->d_defs, h->d_tabs, nb, &h->scal->step_ctr,
+    k_kinematics<<<(std::max(nb, N_STEP_COUNTERS) + 127) / 128, 128, 0, s>>>(h->d_defs, S.tabs, nb, &h->scal->step_ctr,
                                                                               step_offset, &sc->n_words, N_STEP_COUNTERS);
-    k_marker_keys<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, S.keys[0], &h->scal->status);
+    k_marker_keys<<<mb, 256, 0, s>>>(mi, h->d_defs, S.tabs, g, S.keys[0], &h->scal->status);
     nk += 3;
     if (pt) pt->mark(PH_SORT, s);
     const int sb = (h->sort_tiles + SORT_WARPS - 1) / SORT_WARPS;
@@ -601,7 +606,7 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
         nk += 3;
     }
     if (pt) pt->mark(PH_BINS, s);
-    k_marker_gather<<<mb, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, g, perm, S.ms);
+    k_marker_gather<<<mb, 256, 0, s>>>(mi, h->d_defs, S.tabs, g, perm, S.ms);
     ++nk;
     if (h->opt_interp == 1) { k_invert_perm<<<mb, 256, 0, s>>>(perm, n, S.inv); ++nk; }
     if (h->opt_spread == 0) {
@@ -661,7 +666,7 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
         const int nb = (int)h->bodies.size();
         MarkerIn mi{h->d_q[0], h->d_q[1], h->d_q[2], h->d_v[0], h->d_v[1], h->d_v[2], h->d_s, h->d_body, n};
         k_reset_boxes<<<(nb + 127) / 128, 128, 0, s>>>(h->d_box, nb);
-        k_body_boxes<<<(n + 255) / 256, 256, 0, s>>>(mi, h->d_defs, h->d_tabs, h->d_box);
+        k_body_boxes<<<(n + 255) / 256, 256, 0, s>>>(mi, h->d_defs, S.tabs, h->d_box);   // the set's own tables
         k_moments_box<<<dim3(64, nb), 256, 0, s>>>(src, g, h->d_box, h->U);
         nk += 3;
     } else if (h->opt_moments == 2) {
@@ -1050,6 +1055,16 @@ int lbm_set_option(lbm_t *h, int key, int value)
         case LBM_OPT_FUSED: if (value < 0 || value > 1) break; h->opt_fused = value; return LBM_OK;
         case LBM_OPT_TILE_ROWS: if (value != 0 && value != 1 && value != 2 && value != 4) break; h->opt_tile_rows = value; return LBM_OK;
         case LBM_OPT_PERSISTENT: if (value < 0 || value > 2) break; h->opt_persistent = value; return LBM_OK;
+        case LBM_OPT_MDF_BLOCKS:
+            if (value < 0 || value > 32) break;
+            h->opt_mdf_blocks = value;
+            if (h->tr > 0) {                       // cached graphs hold the old grids
+                CK(cudaStreamSynchronize(h->stream));
+                drop_graphs(h);
+                int rc = mdf_launch_geometry(h);
+                if (rc) return rc;
+            }
+            return LBM_OK;
         case LBM_OPT_TILE_CAP:
             if (value < 0) break;
             if (value != h->opt_tile_cap) { h->opt_tile_cap = value; h->realloc_tables = true; h->markers_stale = true; }

@@ -26,9 +26,14 @@
 
 namespace lbmk {
 
+#ifndef MDF_MIN_BLOCKS_CFG
+#define MDF_MIN_BLOCKS_CFG 4
+#endif
 constexpr int MDF_WARPS = 4;            // warps per block of the tile pass
+constexpr int MDF_MIN_BLOCKS = MDF_MIN_BLOCKS_CFG;   // register cap of the tile pass: 65536 / (128 threads x MDF_MIN_BLOCKS)
 constexpr int MDF_BATCH = 32;           // markers per phase-1 / phase-2 round (= lanes)
-constexpr int MDF_STAGE_BYTES = MDF_BATCH * 96;
+constexpr int MDF_STAGE_RECS = MDF_BATCH + 1;        // one padding record: the sweep reads one record ahead
+constexpr int MDF_STAGE_BYTES = (MDF_STAGE_RECS * 96 + 127) / 128 * 128;
 
 struct MdfArgs {
     Geom g;
@@ -38,6 +43,8 @@ struct MdfArgs {
     const int2 *tile_rec;        // [tile][TR*TR] sorted-marker range of the chunk in source row sy + TR sz
     const int *tile_slot;        // [tile] -> tile slot
     const unsigned *tile_mask;   // [tile slot]
+    const int4 *tile_ohdr;       // [position, longest tile first] (tile slot, reach mask, tile id, markers)
+    const int2 *tile_orec;       // [position][TR*TR] chunk ranges
     const int *tile_id;          // [tile slot] -> tile
     const int *tile_order;       // tiles, longest first
     const int *n_tiles;
@@ -78,11 +85,28 @@ __device__ __forceinline__ void cp_async16_cg(void *smem_dst, const void *gsrc)
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-// One tile, one warp.  wsm = the warp's shared memory (mdf_warp_smem bytes).
-template <int TR>
-__device__ __forceinline__ void mdf_tile_pass(const MdfArgs &a, const int t, const bool last, char *wsm, const int lane)
+// What a warp needs to know about a tile before it touches the tile's markers.
+struct TileHdr {
+    int t;               // tile id, < 0: none
+    int2 rec;            // lane r < TR*TR: sorted-marker range of the chunk in source row r
+    int cnt, incl;       // lane r: markers of row r, inclusive prefix over the rows
+    int total;           // markers of the tile
+    int x0, ty, tz;      // first x cell of the block, tile coordinates in y and z
+    unsigned m;          // reach mask: x entries (bits 0..13) | y rows (14..20) | z rows (21..27)
+};
+
+// The tile pass of one warp over a stream of tiles (next() hands out positions in the longest-first order, < 0 =
+// no more).  Software pipeline across tiles: the warp draws its next tile when it starts on the last 32 markers
+// of the current one (late, so that the dynamic balance is kept), and as soon as those are interpolated (the
+// window is dead from then on) it requests the next tile's window and first 32 markers, which arrive during
+// the last sweep and the write-out of the current tile.  wsm = the warp's shared
+// memory (mdf_warp_smem bytes).
+template <int TR, class Next>
+__device__ __forceinline__ void mdf_tile_loop(const MdfArgs &a, const bool last, char *wsm, const int lane, Next &&next)
 {
     constexpr int NR = TR * TR, TF = TR + 3, NROWS = TF * TF;
+    constexpr int NRP = NR <= 1 ? 1 : (NR <= 4 ? 4 : 16);        // rows rounded up to a power of two (prefix / search)
+    constexpr int KZ = (TF + 1) / 2;
     constexpr unsigned FULL = 0xffffffffu;
     const int ent = a.cg.ent;
     const int l = lane & 15, h = lane >> 4;
@@ -92,201 +116,262 @@ __device__ __forceinline__ void mdf_tile_pass(const MdfArgs &a, const int t, con
     float4 *win = reinterpret_cast<float4 *>(wsm);                       // [NROWS][ent] U^m (w unused)
     float *foot = reinterpret_cast<float *>(wsm + win_bytes);            // [NROWS][ent][3]
     float4 *sv = reinterpret_cast<float4 *>(wsm + win_bytes + foot_bytes);   // staged value + tag
-    float4 *swx = sv + MDF_BATCH;                                        // staged x weights
-    float *swyz = reinterpret_cast<float *>(swx + MDF_BATCH);            // staged y-z weights [32][16]
+    float4 *swx = sv + MDF_STAGE_RECS;                                   // staged x weights
+    float *swyz = reinterpret_cast<float *>(swx + MDF_STAGE_RECS);       // staged y-z weights [33][16]
+    const float2 *sw2 = reinterpret_cast<const float2 *>(swx) + h;
+    const float *swz = swyz + l;
 
-    // ---- tile header: chunk ranges, their inclusive prefix, geometry ------------------------------
-    int2 rec = make_int2(0, 0);
-    if (lane < NR) rec = __ldg(a.tile_rec + (size_t)t * NR + lane);
-    const int ts = __ldg(a.tile_slot + t);
-    const unsigned m = __ldg(a.tile_mask + ts);
-    const int cnt = rec.y - rec.x;
-    int incl = cnt;
+    // ---- tile header: chunk ranges, their inclusive prefix, geometry (one round trip: all indexed by the tile id)
+    auto load_hdr = [&](int pos, TileHdr &H) {
+        H.t = -1;
+        H.rec = make_int2(0, 0);
+        H.total = 0;
+        if (pos < 0) return;
+        if (lane < NR) H.rec = __ldg(a.tile_orec + (size_t)pos * NR + lane);
+        const int4 hd = __ldg(a.tile_ohdr + pos);
+        const int ts = hd.x;
+        H.m = (unsigned)hd.y;
+        H.t = hd.z;
+        H.cnt = H.rec.y - H.rec.x;
+        H.incl = H.cnt;
 #pragma unroll
-    for (int o = 1; o < NR; o <<= 1) {
-        const int v = __shfl_up_sync(FULL, incl, o);
-        if (lane >= o) incl += v;
-    }
-    const int total = __shfl_sync(FULL, incl, NR - 1);
-    const int blk = ts % a.cg.nbx, tyz = ts / a.cg.nbx;
-    const int ty = tyz % a.tg.nty, tz = tyz / a.tg.nty;
-    const int x0 = blk * CHUNK_W;
-    const bool ex = l < ent && ((m >> l) & 1u);              // this lane's window entry is reachable
+        for (int o = 1; o < NRP; o <<= 1) {
+            const int v = __shfl_up_sync(FULL, H.incl, o);
+            if (lane >= o) H.incl += v;
+        }
+        H.total = __shfl_sync(FULL, H.incl, NRP - 1);
+        const int blk = ts % a.cg.nbx, tyz = ts / a.cg.nbx;
+        H.ty = tyz % a.tg.nty; H.tz = tyz / a.tg.nty;
+        H.x0 = blk * CHUNK_W;
+    };
 
     // ---- stage the window of U^m: asynchronous 16-byte copies, half a warp per row ---------------------
-    // (row coordinates: ty TR - 1 + fy lies in [-1, ny + 4], so one conditional wrap is enough for ny >= 4)
-    {
-        const int x = mod_wrap(x0 - 1 + l, a.g.nx);
-        const int ybase = ty * TR - 1, zbase = tz * TR - 1;
-#pragma unroll 1
-        for (int fyz = h; fyz < NROWS; fyz += 2) {
-            const int fy = fyz / TF, fz = fyz - fy * TF;
-            if (ex && ((m >> (14 + fy)) & (m >> (21 + fz)) & 1u)) {
-                int y = ybase + fy, z = zbase + fz;
-                if (a.g.wally) y = min(max(y, 0), a.g.ny - 1); else { if (y < 0) y += a.g.ny; else if (y >= a.g.ny) y -= a.g.ny; }
-                if (a.g.wallz) z = min(max(z, 0), a.g.nz - 1); else { if (z < 0) z += a.g.nz; else if (z >= a.g.nz) z -= a.g.nz; }
-                cp_async16_cg(win + fyz * ent + l, a.U + (size_t)(z * a.g.ny + y) * a.g.nx + x);
+    // Rows: fy = 0 .. TF-1 (unrolled), fz = 2 k + h.  Row coordinates ty TR - 1 + fy lie in [-1, ny + 4], so one
+    // conditional wrap is enough for ny >= 4; rows outside a wall axis are never in the mask product.
+    auto issue_window = [&](const TileHdr &H) {
+        const unsigned my = H.m >> 14, mz = H.m >> (21 + h);         // bit fy / bit 2 k: the row is reachable
+        const bool ex = l < ent && ((H.m >> l) & 1u);                // this lane's window entry is reachable
+        const int x = mod_wrap(H.x0 - 1 + l, a.g.nx);
+        int zoff[KZ];
+#pragma unroll
+        for (int k = 0; k < KZ; ++k) {
+            int z = H.tz * TR - 1 + 2 * k + h;
+            if (a.g.wallz) z = min(max(z, 0), a.g.nz - 1); else { if (z < 0) z += a.g.nz; else if (z >= a.g.nz) z -= a.g.nz; }
+            zoff[k] = z * a.g.ny;
+        }
+#pragma unroll
+        for (int fy = 0; fy < TF; ++fy) {
+            int y = H.ty * TR - 1 + fy;
+            if (a.g.wally) y = min(max(y, 0), a.g.ny - 1); else { if (y < 0) y += a.g.ny; else if (y >= a.g.ny) y -= a.g.ny; }
+#pragma unroll
+            for (int k = 0; k < KZ; ++k) {
+                if (2 * k + 1 >= TF && h) continue;              // fz = 2 k + h < TF
+                if (ex && ((my >> fy) & (mz >> (2 * k)) & 1u))
+                    cp_async16_cg(win + (fy * TF + 2 * k + h) * ent + l, a.U + (size_t)(zoff[k] + y) * a.g.nx + x);
             }
         }
-    }
+    };
 
     // the markers of one batch: (source row, sorted index) of this lane's marker, its data in registers
     struct Pre { float4 fs, uk, du; int r, i; };
-    auto fetch = [&](int base, Pre &pf) {
+    auto fetch = [&](const TileHdr &H, int base, Pre &pf) {
         const int j = base + lane;
         int r = 0;
 #pragma unroll
-        for (int step = NR / 2; step >= 1; step >>= 1) {     // the first r with incl[r] > j
-            const int v = __shfl_sync(FULL, incl, r + step - 1);
+        for (int step = NRP / 2; step >= 1; step >>= 1) {    // the first r with incl[r] > j
+            const int v = __shfl_sync(FULL, H.incl, r + step - 1);
             if (j >= v) r += step;
         }
-        const int r_first = __shfl_sync(FULL, rec.x, r);
-        const int r_incl = __shfl_sync(FULL, incl, r), r_cnt = __shfl_sync(FULL, cnt, r);
+        const int r_first = __shfl_sync(FULL, H.rec.x, r);
+        const int r_incl = __shfl_sync(FULL, H.incl, r), r_cnt = __shfl_sync(FULL, H.cnt, r);
         pf.r = r;
         pf.i = r_first + (j - (r_incl - r_cnt));
-        if (j < total) {
+        if (j < H.total) {
             pf.fs = __ldg(a.fs + pf.i);
             pf.uk = __ldg(a.uk + pf.i);
             pf.du = __ldcg(a.du + pf.i);
         }
     };
+
+    TileHdr H, Hn;
     Pre cur;
-    fetch(0, cur);                                       // in flight together with the window copies
+    load_hdr(next(), H);
+    if (H.t < 0) return;
+    issue_window(H);
+    fetch(H, 0, cur);
 
-    // zero the footprint meanwhile
-    {
-        float4 *f4 = reinterpret_cast<float4 *>(foot);
-        const int n4 = (int)(foot_bytes / 16);
-        for (int i = lane; i < n4; i += 32) f4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-    }
-    cp_async_wait_all();
-    __syncwarp();
-
-    // ---- the tile's markers, 32 at a time -------------------------------------------------------------
-    int tag_cur = -1;                            // (source row << 8) | window start of the sweep, -1 = none yet
-    int e = 0;
-    float *frow = foot;
-    Acc3 p{0.f, 0.f, 0.f}, q{0.f, 0.f, 0.f};     // window cells (e + 2h, e + 2h + 1)
-    auto flush = [&](int ee, const Acc3 &acc) {
-        float *d = frow + ee * 3;
-        d[0] += acc.x; d[1] += acc.y; d[2] += acc.z;
-    };
-    const float2 *sw2 = reinterpret_cast<const float2 *>(swx) + h;
-    const float *swz = swyz + l;
-    for (int base = 0; base < total; base += MDF_BATCH) {
-        const int nb = min(MDF_BATCH, total - base);
-        if (lane < nb) {
-            // ---- phase 1: interpolate, correct, stage ----------------
-            const float4 fs = cur.fs, uk = cur.uk;
-            float4 d = cur.du;
-            const int e0 = __float_as_int(d.w) - x0;             // window entry of cell cx - 1
-            const int sy = cur.r % TR, sz = cur.r / TR;
-            float wx[4], wy[4], wz[4];
-            peskin4(fs.x, wx);
-            peskin4(fs.y, wy);
-            peskin4(fs.z, wz);
-            const float4 *w0 = win + (sy * TF + sz) * ent + e0;
-            float ux = 0.f, uy = 0.f, uz = 0.f;
-            float4 *my_wyz = reinterpret_cast<float4 *>(swyz + lane * 16);
-#pragma unroll
-            for (int ky = 0; ky < 4; ++ky) {
-                float wyz[4];
-#pragma unroll
-                for (int kz = 0; kz < 4; ++kz) {
-                    wyz[kz] = wy[ky] * wz[kz];
-                    const float4 *rowp = w0 + (ky * TF + kz) * ent;
-                    const float4 c0 = rowp[0], c1 = rowp[1], c2 = rowp[2], c3 = rowp[3];
-                    const float tx = fmaf(wx[3], c3.x, fmaf(wx[2], c2.x, fmaf(wx[1], c1.x, wx[0] * c0.x)));
-                    const float ty_ = fmaf(wx[3], c3.y, fmaf(wx[2], c2.y, fmaf(wx[1], c1.y, wx[0] * c0.y)));
-                    const float tz_ = fmaf(wx[3], c3.z, fmaf(wx[2], c2.z, fmaf(wx[1], c1.z, wx[0] * c0.z)));
-                    ux = fmaf(wyz[kz], tx, ux);
-                    uy = fmaf(wyz[kz], ty_, uy);
-                    uz = fmaf(wyz[kz], tz_, uz);
-                }
-                my_wyz[ky] = make_float4(wyz[0], wyz[1], wyz[2], wyz[3]);
-            }
-            const float gx = uk.x - ux, gy = uk.y - uy, gz = uk.z - uz;
-            d.x = fmaf(fs.w, gx, d.x);
-            d.y = fmaf(fs.w, gy, d.y);
-            d.z = fmaf(fs.w, gz, d.z);
-            a.du[cur.i] = d;
-            const float tagf = __int_as_float((cur.r << 8) | e0);
-            sv[lane] = last ? make_float4(d.x, d.y, d.z, tagf) : make_float4(fs.w * gx, fs.w * gy, fs.w * gz, tagf);
-            swx[lane] = make_float4(wx[0], wx[1], wx[2], wx[3]);
+    while (H.t >= 0) {
+        const int total = H.total, x0 = H.x0;
+        // zero the footprint while the window copies and the first markers are in flight
+        {
+            float4 *f4 = reinterpret_cast<float4 *>(foot);
+            const int n4 = (int)(foot_bytes / 16);
+            for (int i = lane; i < n4; i += 32) f4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
-        if (base + MDF_BATCH < total) fetch(base + MDF_BATCH, cur);          // in flight during the sweep
+        cp_async_wait_all();
         __syncwarp();
 
-        // ---- phase 2: sweep the staged markers in sorted order (warp-uniform control flow) ----------------
-#pragma unroll 2
-        for (int jj = 0; jj < nb; ++jj) {
-            const float4 v = sv[jj];
-            const float2 w = sw2[2 * jj];
-            const float wz_ = swz[16 * jj];
-            const int tg_ = __float_as_int(v.w);
-            if (tg_ != tag_cur) {                        // the sweep moves on to another cell or another source row
-                const int rn = tg_ >> 8, en = tg_ & 0xff;
-                if ((tg_ ^ tag_cur) >> 8) {              // another source row (or the first marker of the tile)
-                    if (tag_cur >= 0) { flush(e + 2 * h, p); flush(e + 2 * h + 1, q); }
-                    frow = foot + (((rn % TR) + jy) * TF + ((rn / TR) + jz)) * ent * 3;
-                    p = Acc3{0.f, 0.f, 0.f}; q = Acc3{0.f, 0.f, 0.f};
-                    e = en;
-                } else {
-#pragma unroll 1
-                    do {                                 // the leftmost window cell is complete
-                        if (h == 0) flush(e, p);
-                        const float tx = __shfl_down_sync(FULL, p.x, 16);
-                        const float ty_ = __shfl_down_sync(FULL, p.y, 16);
-                        const float tz_ = __shfl_down_sync(FULL, p.z, 16);
-                        p = q;
-                        q.x = h ? 0.f : tx; q.y = h ? 0.f : ty_; q.z = h ? 0.f : tz_;
-                    } while (++e < en);
+        // ---- the tile's markers, 32 at a time -------------------------------------------------------------
+        int tag_cur = -1;                            // (source row << 8) | cell of the last marker swept, -1 = none yet
+        int e = 0;
+        float *frow = foot;
+        Acc3 p{0.f, 0.f, 0.f}, q{0.f, 0.f, 0.f};     // window cells (e + 2h, e + 2h + 1)
+        auto flush = [&](int ee, const Acc3 &acc) {
+            float *d = frow + ee * 3;
+            d[0] += acc.x; d[1] += acc.y; d[2] += acc.z;
+        };
+        Hn.t = -1;
+        if (total <= 0) load_hdr(next(), Hn);
+        for (int base = 0; base < total; base += MDF_BATCH) {
+            const int nb = min(MDF_BATCH, total - base);
+            const bool last_batch = base + MDF_BATCH >= total;
+            if (last_batch) load_hdr(next(), Hn);
+            int tag = -2;
+            if (lane < nb) {
+                // ---- phase 1: interpolate, correct, stage ----------------
+                const float4 fs = cur.fs, uk = cur.uk;
+                float4 d = cur.du;
+                const int e0 = __float_as_int(d.w) - x0;             // window entry of cell cx - 1
+                const int sy = cur.r % TR, sz = cur.r / TR;
+                float wx[4], wy[4], wz[4];
+                peskin4(fs.x, wx);
+                peskin4(fs.y, wy);
+                peskin4(fs.z, wz);
+                const float4 *w0 = win + (sy * TF + sz) * ent + e0;
+                float ux = 0.f, uy = 0.f, uz = 0.f;
+                float4 *my_wyz = reinterpret_cast<float4 *>(swyz + lane * 16);
+#pragma unroll
+                for (int ky = 0; ky < 4; ++ky) {
+                    float wyz[4];
+#pragma unroll
+                    for (int kz = 0; kz < 4; ++kz) {
+                        wyz[kz] = wy[ky] * wz[kz];
+                        const float4 *rowp = w0 + (ky * TF + kz) * ent;
+                        const float4 c0 = rowp[0], c1 = rowp[1], c2 = rowp[2], c3 = rowp[3];
+                        const float tx = fmaf(wx[3], c3.x, fmaf(wx[2], c2.x, fmaf(wx[1], c1.x, wx[0] * c0.x)));
+                        const float ty_ = fmaf(wx[3], c3.y, fmaf(wx[2], c2.y, fmaf(wx[1], c1.y, wx[0] * c0.y)));
+                        const float tz_ = fmaf(wx[3], c3.z, fmaf(wx[2], c2.z, fmaf(wx[1], c1.z, wx[0] * c0.z)));
+                        ux = fmaf(wyz[kz], tx, ux);
+                        uy = fmaf(wyz[kz], ty_, uy);
+                        uz = fmaf(wyz[kz], tz_, uz);
+                    }
+                    my_wyz[ky] = make_float4(wyz[0], wyz[1], wyz[2], wyz[3]);
                 }
-                tag_cur = tg_;
+                const float gx = uk.x - ux, gy = uk.y - uy, gz = uk.z - uz;
+                d.x = fmaf(fs.w, gx, d.x);
+                d.y = fmaf(fs.w, gy, d.y);
+                d.z = fmaf(fs.w, gz, d.z);
+                a.du[cur.i] = d;
+                tag = (cur.r << 8) | e0;
+                const float tagf = __int_as_float(tag);
+                sv[lane] = last ? make_float4(d.x, d.y, d.z, tagf) : make_float4(fs.w * gx, fs.w * gy, fs.w * gz, tagf);
+                swx[lane] = make_float4(wx[0], wx[1], wx[2], wx[3]);
             }
-            const float vx = v.x * wz_, vy = v.y * wz_, vz = v.z * wz_;
-            p.x = fmaf(w.x, vx, p.x); p.y = fmaf(w.x, vy, p.y); p.z = fmaf(w.x, vz, p.z);
-            q.x = fmaf(w.y, vx, q.x); q.y = fmaf(w.y, vy, q.y); q.z = fmaf(w.y, vz, q.z);
-        }
-        __syncwarp();                                    // every lane is done with the staging buffer
-    }
-    if (tag_cur >= 0) { flush(e + 2 * h, p); flush(e + 2 * h + 1, q); }
-    __syncwarp();
+            // which staged markers start another cell / another source row (warp-uniform bit masks: the sweep below
+            // branches on registers, not on a value it has just loaded)
+            const int prev_tag = __shfl_up_sync(FULL, tag, 1);
+            const int before = lane == 0 ? tag_cur : prev_tag;
+            const unsigned chg = __ballot_sync(FULL, lane < nb && tag != before);
+            const unsigned rowchg = __ballot_sync(FULL, lane < nb && ((tag ^ before) >> 8) != 0);
+            const int tag_last = __shfl_sync(FULL, tag, nb - 1);
+            __syncwarp();                                // staging buffer complete; nobody reads the window any more
+            if (!last_batch) {
+                fetch(H, base + MDF_BATCH, cur);         // in flight during the sweep
+            } else if (Hn.t >= 0) {
+                issue_window(Hn);                        // the window is dead: bring in the next tile's, and its first markers
+                fetch(Hn, 0, cur);
+            }
 
-    // ---- hand every footprint element to the cell that consumes it (plan: fdst) ------------------------
-    {
-        const int *__restrict__ dst = a.fdst + (size_t)t * (NROWS * ent);
+            // ---- phase 2: sweep the staged markers in sorted order (warp-uniform control flow); the staged record
+            // of marker jj + 1 is read while marker jj is processed
+            float4 v = sv[0];
+            float2 w = sw2[0];
+            float wz_ = swz[0];
+            const float4 *pv = sv + 1;                       // record jj + 1 (the last read lands on the padding record)
+            const float2 *pw = sw2 + 2;
+            const float *pz = swz + 16;
+            unsigned cbits = chg, rbits = rowchg;
+#pragma unroll 4
+            for (int jj = 0; jj < nb; ++jj, ++pv, pw += 2, pz += 16, cbits >>= 1, rbits >>= 1) {
+                const float4 vn = *pv;
+                const float2 wn = *pw;
+                const float wzn = *pz;
+                if (cbits & 1u) {                            // the sweep moves on to another cell or another source row
+                    const int tg_ = __float_as_int(v.w);
+                    const int en = tg_ & 0xff;
+                    if (rbits & 1u) {                        // another source row (or the first marker of the tile)
+                        const int rn = tg_ >> 8;
+                        if (tag_cur >= 0) { flush(e + 2 * h, p); flush(e + 2 * h + 1, q); }
+                        frow = foot + (((rn % TR) + jy) * TF + ((rn / TR) + jz)) * ent * 3;
+                        p = Acc3{0.f, 0.f, 0.f}; q = Acc3{0.f, 0.f, 0.f};
+                        e = en;
+                        tag_cur = tg_;
+                    } else {
 #pragma unroll 1
-        for (int fyz = h; fyz < NROWS; fyz += 2) {
-            const int fy = fyz / TF, fz = fyz - fy * TF;
-            if (ex && ((m >> (14 + fy)) & (m >> (21 + fz)) & 1u)) {
-                const int o = __ldg(dst + fyz * ent + l);
-                if (o >= 0) {
-                    const float *s = foot + (fyz * ent + l) * 3;
-                    __stcg(a.F + o, make_float4(s[0], s[1], s[2], 0.f));
+                        do {                                 // the leftmost window cell is complete
+                            if (h == 0) flush(e, p);
+                            const float tx = __shfl_down_sync(FULL, p.x, 16);
+                            const float ty_ = __shfl_down_sync(FULL, p.y, 16);
+                            const float tz_ = __shfl_down_sync(FULL, p.z, 16);
+                            p = q;
+                            q.x = h ? 0.f : tx; q.y = h ? 0.f : ty_; q.z = h ? 0.f : tz_;
+                        } while (++e < en);
+                    }
                 }
+                const float vx = v.x * wz_, vy = v.y * wz_, vz = v.z * wz_;
+                p.x = fmaf(w.x, vx, p.x); p.y = fmaf(w.x, vy, p.y); p.z = fmaf(w.x, vz, p.z);
+                q.x = fmaf(w.y, vx, q.x); q.y = fmaf(w.y, vy, q.y); q.z = fmaf(w.y, vz, q.z);
+                v = vn; w = wn; wz_ = wzn;
             }
+            tag_cur = tag_last;
+            __syncwarp();                                    // every lane is done with the staging buffer
         }
+        if (tag_cur >= 0) { flush(e + 2 * h, p); flush(e + 2 * h + 1, q); }
+        __syncwarp();
+
+        // ---- hand every footprint element to the cell that consumes it (plan: fdst) ------------------------
+        // all the destinations first (independent loads), then the stores
+        {
+            const unsigned my = H.m >> 14, mz = H.m >> (21 + h);
+            const bool ex = l < ent && ((H.m >> l) & 1u);
+            const int *__restrict__ dst = a.fdst + (size_t)H.t * (NROWS * ent) + l;
+            int o[TF][KZ];
+#pragma unroll
+            for (int fy = 0; fy < TF; ++fy)
+#pragma unroll
+                for (int k = 0; k < KZ; ++k) {
+                    o[fy][k] = -1;
+                    if (2 * k + 1 >= TF && h) continue;
+                    if (ex && ((my >> fy) & (mz >> (2 * k)) & 1u)) o[fy][k] = __ldg(dst + (fy * TF + 2 * k + h) * ent);
+                }
+#pragma unroll
+            for (int fy = 0; fy < TF; ++fy)
+#pragma unroll
+                for (int k = 0; k < KZ; ++k)
+                    if (o[fy][k] >= 0) {
+                        const float *sp = foot + ((fy * TF + 2 * k + h) * ent + l) * 3;
+                        __stcg(a.F + o[fy][k], make_float4(sp[0], sp[1], sp[2], 0.f));
+                    }
+        }
+        __syncwarp();
+        H = Hn;
     }
-    __syncwarp();
 }
 
 // tile pass as a kernel of its own: persistent grid, tiles handed out longest first through a cursor
 template <int TR>
-__global__ void __launch_bounds__(MDF_WARPS * 32)
+__global__ void __launch_bounds__(MDF_WARPS * 32, MDF_MIN_BLOCKS)
 k_mdf_tiles(const __grid_constant__ MdfArgs a, int *__restrict__ cursor, int last, int warp_smem)
 {
     extern __shared__ __align__(128) char smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int nt = min(*a.n_tiles, a.tile_cap);
     char *wsm = smem + (size_t)warp * warp_smem;
-    for (;;) {
+    mdf_tile_loop<TR>(a, last != 0, wsm, lane, [&]() {
         int t = 0;
-        if (lane == 0) { t = atomicAdd(cursor, 1); t = t < nt ? __ldg(a.tile_order + t) : nt; }
-        t = __shfl_sync(0xffffffffu, t, 0);
-        if (t >= nt) break;
-        mdf_tile_pass<TR>(a, t, last != 0, wsm, lane);
-    }
+        if (lane == 0) { t = atomicAdd(cursor, 1); t = t < nt ? t : -1; }
+        return __shfl_sync(0xffffffffu, t, 0);
+    });
 }
 
 // ---- stage B ---------------------------------------------------------------------------------------
@@ -468,7 +553,7 @@ __device__ __forceinline__ void moments_cell(const float *__restrict__ src, cons
 constexpr int MDFP_WARPS = 8;           // warps per block of the persistent kernel
 
 template <int TR>
-__global__ void __launch_bounds__(MDFP_WARPS * 32)
+__global__ void __launch_bounds__(MDFP_WARPS * 32, 2)
 k_mdf_persistent(const __grid_constant__ MdfArgs a, const float *__restrict__ src, const __grid_constant__ PlaneOffsets po,
                  int *__restrict__ cursors, unsigned *__restrict__ bar, int mdf_iters, int warp_smem)
 {
@@ -479,18 +564,23 @@ k_mdf_persistent(const __grid_constant__ MdfArgs a, const float *__restrict__ sr
     char *wsm = smem + (size_t)warp * warp_smem;
     const int nt = min(*a.n_tiles, a.tile_cap);
     const int nc = *a.n_cells;
+    const int gwarp = warp * gridDim.x + blockIdx.x, nwarps = gridDim.x * MDFP_WARPS;   // consecutive tiles go to different SMs
     unsigned target = 0u;
     // a4: rho, U of eq. (1) on the active cells
     for (int k = tid; k < nc; k += stride) moments_cell(src, a.g, po, __ldg(a.cells + k), a.U);
     grid_barrier(bar, target);
     for (int it = 0; it < mdf_iters; ++it) {
         const bool last = (it == mdf_iters - 1);
-        for (;;) {
-            int t = 0;
-            if (lane == 0) { t = atomicAdd(cursors + it, 1); t = t < nt ? __ldg(a.tile_order + t) : nt; }
-            t = __shfl_sync(0xffffffffu, t, 0);
-            if (t >= nt) break;
-            mdf_tile_pass<TR>(a, t, last, wsm, lane);
+        if (nt <= 2 * nwarps) {
+            // few tiles: dealt statically, longest first (no cursor round trips on the critical path)
+            int k = gwarp - nwarps;
+            mdf_tile_loop<TR>(a, last, wsm, lane, [&]() { k += nwarps; return k < nt ? k : -1; });
+        } else {
+            mdf_tile_loop<TR>(a, last, wsm, lane, [&]() {
+                int t = 0;
+                if (lane == 0) { t = atomicAdd(cursors + it, 1); t = t < nt ? t : -1; }
+                return __shfl_sync(0xffffffffu, t, 0);
+            });
         }
         grid_barrier(bar, target);
         for (int k = tid; k < nc; k += stride) mdf_collect_cell(a, k, last);
