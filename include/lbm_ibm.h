@@ -77,12 +77,14 @@ enum {
     LBM_OPT_TIMING = 6,   /* 1 = run steps as plain launches with CUDA events between the phases and
                              accumulate per-phase device time (LBM_INFO_PHASE_NS); setting it resets
                              the accumulators.  Each step then ends with a stream synchronise.     */
-    LBM_OPT_OVERLAP = 7,  /* 1 (default) = a coupled step runs as three concurrent graph branches: the
-                             MDF loop, the stream-collide of every cell outside the marker stencils
-                             (it needs no IBM force), and the binning of the NEXT step's markers (P:154:
-                             positions depend on time only); the cells inside the stencils are updated
-                             after the join.  0 = the same step as one serial chain with a single fused
-                             stream-collide pass (measured comparison).  Results are identical.        */
+    LBM_OPT_OVERLAP = 7,  /* how a coupled step is laid out in its CUDA graph.  1 = three concurrent branches: the MDF
+                             loop, the stream-collide of every cell outside the marker stencils (it needs no
+                             IBM force), and the binning of the NEXT step's markers (positions depend on
+                             time only); the cells inside the stencils are updated after the join.  2 = two
+                             branches (MDF loop, binning of the next step), then ONE fused stream-collide
+                             pass over the whole lattice.  0 = one serial chain with a single fused
+                             stream-collide pass (measured comparison).  3 (default) = 2 on lattices above
+                             64 Mi cells or above 1,000,000 markers, else 1.  Results are bit-identical.      */
     LBM_OPT_MOMENTS = 8,  /* where U is precomputed for the IBM: 0 = the de-duplicated list of
                              cells inside a marker stencil (default), 1 = the paper's box strategy (bounding
                              box of every body), 2 = the paper's kernel strategy (a block per Lagrangian
@@ -91,16 +93,21 @@ enum {
                              corrects and spreads (s g never leaves the SM) plus the collect; 0 = the
                              round-1 pipeline: interpolation kernel, TMA-fed tile sweep, collect (measured
                              comparison).  Only with LBM_OPT_SPREAD = 0 and LBM_OPT_INTERP = 0.           */
-    LBM_OPT_TILE_ROWS = 10, /* source rows per tile in y and z for the fused path: 0 = automatic (1 for marker
-                             sets up to 100,000 points, else 4), or 1, 2, 4.  Changing it rebuilds the
-                             tile tables at the next step.  Results agree to rounding (summation order).  */
+    LBM_OPT_TILE_ROWS = 10, /* source rows per tile in y and z for the fused path: 0 = automatic (1 up to 20,000
+                             markers, 2 up to 400,000, else 4), or 1, 2, 4.  Changing it rebuilds the tile
+                             tables at the next step.  Results agree to rounding (summation order).        */
     LBM_OPT_PERSISTENT = 11, /* the fused MDF loop (moments + N x (tile pass, collect)) as ONE persistent kernel
-                             with grid-wide barriers instead of 2 N + 1 launches: 0 = automatic (marker sets up
-                             to 100,000 points), 1 = always, 2 = never.  Results are bit-identical.         */
+                             with grid-wide barriers instead of 2 N + 1 launches: 1 = on, 0 / 2 = off (default;
+                             measured slower on B200).  Results are bit-identical.       */
     LBM_OPT_TILE_CAP = 12, /* > 0: cap the number of tile footprints (default 0 = room for every tile that can
                              exist, up to 12 GB).  More tiles than the cap are dropped for that step and
                              lbm_sync reports LBM_ENOMEM; later steps that fit are complete again.  Takes
                              effect at the next step (the tables are re-allocated).                    */
+    LBM_OPT_TILE_WARPS = 14, /* warps that work on one tile in the tile pass: 0 / 1 = one warp per tile (default),
+                             2 = a pair of warps shares the tile's window and footprint
+                             and alternates between interpolating one batch of 32 markers and sweeping the
+                             previous one (measured comparison: more warps per SM, no faster).  Results agree
+                             to rounding (each batch's sweep is flushed).                                   */
     LBM_OPT_MDF_BLOCKS = 13 /* tuning: blocks per SM of the tile pass / of the persistent MDF kernel (0 = default:
                              as many as fit / one); fewer blocks leave more of every SM to the stream-collide
                              pass that runs beside the MDF loop.  Results do not depend on it.           */

@@ -81,9 +81,15 @@ struct HostBody {
 };
 
 constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driven kernels
-// Marker sets up to this size run the MDF loop as one persistent kernel on single-row tiles (LBM_OPT_TILE_ROWS,
-// LBM_OPT_PERSISTENT = 0): W1 / W3 / P1-P18 (<= 70,848 markers) fall below, W4lit (147,456) and up above.
-constexpr int SMALL_SET_MARKERS = 100000;
+// Tile edge by marker count (LBM_OPT_TILE_ROWS = 0), measured on B200: single-row tiles while
+// the set is so small that larger tiles would not fill the SMs (W1, W3: 15,360 markers), two-row tiles up to a few
+// hundred thousand markers (P6, P18, W4lit), 4 x 4-row tiles beyond (W4, W5lit, W5).
+constexpr int TR1_MAX_MARKERS = 20000;
+constexpr int TR2_MAX_MARKERS = 400000;
+// Step layout (LBM_OPT_OVERLAP = 3): on large lattices / marker sets the split of the stream-collide into a bulk
+// pass beside the MDF loop and a pass over the stencil cells costs more than the overlap hides
+constexpr long long SPLIT_MAX_CELLS = 64LL << 20;
+constexpr int SPLIT_MAX_MARKERS = 1000000;
 
 // Optional per-phase device timing (LBM_OPT_TIMING): CUDA events recorded on the launching stream
 // between the phases of a step; durations are accumulated after a stream synchronise.
@@ -183,14 +189,14 @@ struct lbm {
     int rows_grid = 148;                // persistent grid of the round-1 tile sweep (blocks resident at once)
     int sms = 148;
     int tr = 0;                         // tile edge (source rows in y and z) the tile tables are built for; 0 = none yet
-    int mdf_grid = 148, mdfp_grid = 148;   // grids of the fused tile pass / of the persistent MDF kernel
+    int mdf_grid = 148, mdf2_grid = 148, mdfp_grid = 148;   // grids of the fused tile pass (one / two warps per tile) / of the persistent MDF kernel
     size_t mdf_wsmem = 0;               // shared memory per warp of the tile pass for (tr, cg)
     int words_grid = 148, moments_grid = 148;   // same for the active-word stream-collide and the moments kernel
     int sort_ipw = 64, sort_tiles = 0, sort_passes = 1;
 
     int opt_spread = 0, opt_forcing = 0, opt_graph = 1, opt_lbm_kernel = 0, opt_interp = 0, opt_timing = 0;
-    int opt_overlap = 1, opt_moments = 0;
-    int opt_fused = 1, opt_tile_rows = 0, opt_persistent = 0, opt_tile_cap = 0, opt_mdf_blocks = 0;
+    int opt_overlap = 3, opt_moments = 0;
+    int opt_fused = 1, opt_tile_rows = 0, opt_persistent = 0, opt_tile_cap = 0, opt_mdf_blocks = 0, opt_tile_warps = 0;
     bool realloc_tables = false;        // LBM_OPT_TILE_CAP changed: the tile tables are re-allocated at the next step
     int *d_box = nullptr;               // per-body bounding boxes (comparison LBM_OPT_MOMENTS = 1 only; lazy)
     PhaseTimer timer;
@@ -317,15 +323,31 @@ int effective_tr(const lbm *h)
 {
     if (!fused_path(h)) return TILE_R;
     if (h->opt_tile_rows) return h->opt_tile_rows;
-    return (int)h->h_area.size() <= SMALL_SET_MARKERS ? 1 : TILE_R;
+    const size_t n = h->h_area.size();
+    return n <= (size_t)TR1_MAX_MARKERS ? 1 : (n <= (size_t)TR2_MAX_MARKERS ? 2 : TILE_R);
+}
+
+// how a coupled step is laid out (LBM_OPT_OVERLAP): 0 = one serial chain; 1 = three branches (MDF loop, bulk
+// stream-collide of the cells outside the stencils, binning of the next step), then the cells inside the stencils;
+// 2 = two branches (MDF loop, binning of the next step), then ONE fused stream-collide pass over the lattice
+int overlap_mode(const lbm *h)
+{
+    if (h->opt_overlap != 3) return h->opt_overlap;
+    return (h->g.cells > SPLIT_MAX_CELLS || h->nm > SPLIT_MAX_MARKERS) ? 2 : 1;
+}
+
+// warps per tile of the tile pass: two share a tile's window and footprint where tiles hold several batches of 32
+// markers (4 x 4-row tiles), one otherwise
+int tile_warps(const lbm *h)
+{
+    return h->opt_tile_warps == 2 ? 2 : 1;
 }
 
 // the whole MDF loop as one persistent kernel (small marker sets: launch latency dominates otherwise)
 bool use_persistent(const lbm *h)
 {
     if (!fused_path(h) || h->opt_moments != 0 || h->opt_timing) return false;
-    if (h->opt_persistent) return h->opt_persistent == 1;
-    return h->nm <= SMALL_SET_MARKERS;
+    return h->opt_persistent == 1;
 }
 
 // the options a preparation depends on (which tables it builds)
@@ -395,6 +417,7 @@ int flush_ibm(lbm *h)
 // ---- the fused MDF kernels for a tile edge and a lattice ---------------------------------------------
 struct MdfKernels {
     void (*tiles)(const MdfArgs, int *, int, int);
+    void (*pairs)(const MdfArgs, int *, int);
     void (*plan)(const MdfArgs);
     void (*persistent)(const MdfArgs, const float *, const PlaneOffsets, int *, unsigned *, int, int);
 };
@@ -409,14 +432,14 @@ MdfKernels mdf_kernels(const lbm *h)
     const bool two_yz = (g.wally || g.ny % TILE_R == 0) && (g.wallz || g.nz % TILE_R == 0);
     switch (h->tr) {
         case 1:
-            if (two_x) return MdfKernels{k_mdf_tiles<1>, k_collect_plan<1, 2, 4>, k_mdf_persistent<1>};
-            return MdfKernels{k_mdf_tiles<1>, k_collect_plan<1, 4, 4>, k_mdf_persistent<1>};
+            if (two_x) return MdfKernels{k_mdf_tiles<1>, k_mdf_pairs<1>, k_collect_plan<1, 2, 4>, k_mdf_persistent<1>};
+            return MdfKernels{k_mdf_tiles<1>, k_mdf_pairs<1>, k_collect_plan<1, 4, 4>, k_mdf_persistent<1>};
         case 2:
-            if (two_x) return MdfKernels{k_mdf_tiles<2>, k_collect_plan<2, 2, 4>, k_mdf_persistent<2>};
-            return MdfKernels{k_mdf_tiles<2>, k_collect_plan<2, 4, 4>, k_mdf_persistent<2>};
+            if (two_x) return MdfKernels{k_mdf_tiles<2>, k_mdf_pairs<2>, k_collect_plan<2, 2, 4>, k_mdf_persistent<2>};
+            return MdfKernels{k_mdf_tiles<2>, k_mdf_pairs<2>, k_collect_plan<2, 4, 4>, k_mdf_persistent<2>};
         default:
-            if (two_x && two_yz) return MdfKernels{k_mdf_tiles<4>, k_collect_plan<4, 2, 2>, k_mdf_persistent<4>};
-            return MdfKernels{k_mdf_tiles<4>, k_collect_plan<4, 4, 4>, k_mdf_persistent<4>};
+            if (two_x && two_yz) return MdfKernels{k_mdf_tiles<4>, k_mdf_pairs<4>, k_collect_plan<4, 2, 2>, k_mdf_persistent<4>};
+            return MdfKernels{k_mdf_tiles<4>, k_mdf_pairs<4>, k_collect_plan<4, 4, 4>, k_mdf_persistent<4>};
     }
 }
 
@@ -432,6 +455,11 @@ int mdf_launch_geometry(lbm *h)
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, K.tiles, MDF_WARPS * 32, smem_t));
     if (h->opt_mdf_blocks > 0) per_sm = std::min(per_sm, h->opt_mdf_blocks);
     h->mdf_grid = std::max(1, per_sm) * h->sms;
+    const size_t smem_2 = mdf_pair_smem(h->tr, h->cg);
+    CK(cudaFuncSetAttribute((const void *)K.pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_2));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, K.pairs, 64, smem_2));
+    if (h->opt_mdf_blocks > 0) per_sm = std::min(per_sm, h->opt_mdf_blocks);
+    h->mdf2_grid = std::max(1, per_sm) * h->sms;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, K.persistent, MDFP_WARPS * 32, smem_p));
     if (per_sm < 1) return fail(LBM_ECUDA, "the persistent MDF kernel does not fit on an SM (%zu bytes of shared memory)", smem_p);
     h->mdfp_grid = std::min(per_sm, h->opt_mdf_blocks > 0 ? h->opt_mdf_blocks : MDFP_BLOCKS_PER_SM) * h->sms;
@@ -682,7 +710,10 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
         if (pt) pt->mark(PH_INTERP, s);
         if (fused) {
             // product path: interpolate + correct + sweep in one tile pass, then the collect
-            K.tiles<<<h->mdf_grid, MDF_WARPS * 32, (size_t)MDF_WARPS * h->mdf_wsmem, s>>>(ma, &sc->cursor[m], last ? 1 : 0, wsmem);
+            if (tile_warps(h) == 2)
+                K.pairs<<<h->mdf2_grid, 64, mdf_pair_smem(h->tr, h->cg), s>>>(ma, &sc->cursor[m], last ? 1 : 0);
+            else
+                K.tiles<<<h->mdf_grid, MDF_WARPS * 32, (size_t)MDF_WARPS * h->mdf_wsmem, s>>>(ma, &sc->cursor[m], last ? 1 : 0, wsmem);
             if (pt) pt->mark(PH_SPREAD, s);
             k_mdf_collect<<<LIST_GRID, 256, 0, s>>>(ma, last ? 1 : 0);
             nk += 2;
@@ -777,7 +808,7 @@ int enqueue_step_serial(lbm *h, cudaStream_t s, int parity, PrepSet *S, bool pre
     if (S) {
         if (prep && (rc = enqueue_prep(h, s, *S, 0, &nk, pt))) return rc;
         if ((rc = enqueue_mdf(h, s, *S, src, mdf_iters, &nk, pt))) return rc;
-        if (h->opt_overlap) {
+        if (overlap_mode(h) == 1) {
             if (pt) pt->mark(PH_LBM, s);
             if ((rc = enqueue_lbm_pass(h, s, src, dst, LBM_BULK, S->amask))) return rc;
             if (pt) pt->mark(PH_LBM_ACTIVE, s);
@@ -811,19 +842,28 @@ int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, int mdf_
     float *dst = h->f[parity ^ 1];
     cudaStream_t s = h->cap_stream;
     int nk = 0, rc;
+    const bool split = overlap_mode(h) == 1;    // 1: bulk stream-collide beside the MDF loop; 2: one fused pass after it
     CK(cudaEventRecord(h->ev_fork, s));
-    CK(cudaStreamWaitEvent(h->cap_bulk, h->ev_fork, 0));
+    if (split) CK(cudaStreamWaitEvent(h->cap_bulk, h->ev_fork, 0));
     CK(cudaStreamWaitEvent(h->cap_prep, h->ev_fork, 0));
-    if ((rc = enqueue_lbm_pass(h, h->cap_bulk, src, dst, LBM_BULK, S.amask))) return rc;
-    ++nk;
+    if (split) {
+        if ((rc = enqueue_lbm_pass(h, h->cap_bulk, src, dst, LBM_BULK, S.amask))) return rc;
+        ++nk;
+    }
     if ((rc = enqueue_mdf(h, s, S, src, mdf_iters, &nk, nullptr))) return rc;
     if ((rc = enqueue_prep(h, h->cap_prep, N, 1, &nk, nullptr))) return rc;
-    CK(cudaEventRecord(h->ev_bulk, h->cap_bulk));
+    if (split) CK(cudaEventRecord(h->ev_bulk, h->cap_bulk));
     CK(cudaEventRecord(h->ev_prep, h->cap_prep));
-    CK(cudaStreamWaitEvent(s, h->ev_bulk, 0));
+    if (split) CK(cudaStreamWaitEvent(s, h->ev_bulk, 0));
     CK(cudaStreamWaitEvent(s, h->ev_prep, 0));
-    if ((rc = enqueue_lbm_active(h, s, src, dst, S))) return rc;               // also advances the step counter
-    ++nk;
+    if (split) {
+        if ((rc = enqueue_lbm_active(h, s, src, dst, S))) return rc;           // also advances the step counter
+        ++nk;
+    } else {
+        if ((rc = enqueue_lbm_pass(h, s, src, dst, LBM_FUSED, S.amask))) return rc;
+        k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, nullptr, 0, 4);
+        nk += 2;
+    }
     CK(cudaGetLastError());
     *n_kernels = nk;
     return LBM_OK;
@@ -835,8 +875,9 @@ int get_graph(lbm *h, int kind, int parity, int set, int mdf_iters, cudaGraphExe
     const long long key = ((long long)mdf_iters << 8) | ((long long)kind << 4) | (set << 1) | parity |
                           ((long long)h->opt_spread << 40) | ((long long)h->opt_forcing << 44) |
                           ((long long)h->opt_lbm_kernel << 48) | ((long long)h->opt_interp << 52) |
-                          ((long long)h->opt_overlap << 56) | ((long long)h->opt_moments << 58) |
-                          ((long long)h->opt_fused << 60) | ((long long)h->tr << 16) | ((long long)use_persistent(h) << 20);
+                          ((long long)overlap_mode(h) << 56) | ((long long)h->opt_moments << 58) |
+                          ((long long)h->opt_fused << 60) | ((long long)h->tr << 16) | ((long long)use_persistent(h) << 20) |
+                          ((long long)tile_warps(h) << 21);
     auto it = h->graphs.find(key);
     if (it != h->graphs.end()) { *exec = it->second.first; *n_kernels = it->second.second; return LBM_OK; }
     cudaGraph_t graph = nullptr;
@@ -1048,7 +1089,7 @@ int lbm_set_option(lbm_t *h, int key, int value)
         case LBM_OPT_FORCING: if (value < 0 || value > 1) break; h->opt_forcing = value; return LBM_OK;
         case LBM_OPT_GRAPH: if (value < 0 || value > 1) break; h->opt_graph = value; return LBM_OK;
         case LBM_OPT_LBM_KERNEL: if (value < 0 || value > 2) break; h->opt_lbm_kernel = value; return LBM_OK;
-        case LBM_OPT_OVERLAP: if (value < 0 || value > 1) break; h->opt_overlap = value; return LBM_OK;
+        case LBM_OPT_OVERLAP: if (value < 0 || value > 3) break; h->opt_overlap = value; return LBM_OK;
         case LBM_OPT_MOMENTS: if (value < 0 || value > 2) break; h->opt_moments = value; return LBM_OK;
         case LBM_OPT_INTERP: if (value < 0 || value > 3) break; h->opt_interp = value; return LBM_OK;
         case LBM_OPT_TIMING: if (value < 0 || value > 1) break; h->opt_timing = value; h->timer.reset(); return LBM_OK;
@@ -1065,6 +1106,7 @@ int lbm_set_option(lbm_t *h, int key, int value)
                 if (rc) return rc;
             }
             return LBM_OK;
+        case LBM_OPT_TILE_WARPS: if (value < 0 || value > 2) break; h->opt_tile_warps = value; return LBM_OK;
         case LBM_OPT_TILE_CAP:
             if (value < 0) break;
             if (value != h->opt_tile_cap) { h->opt_tile_cap = value; h->realloc_tables = true; h->markers_stale = true; }

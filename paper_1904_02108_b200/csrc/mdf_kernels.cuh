@@ -95,116 +95,309 @@ struct TileHdr {
     unsigned m;          // reach mask: x entries (bits 0..13) | y rows (14..20) | z rows (21..27)
 };
 
-// The tile pass of one warp over a stream of tiles (next() hands out positions in the longest-first order, < 0 =
+template <int TR>
+struct TileDims {
+    static constexpr int NR = TR * TR, TF = TR + 3, NROWS = TF * TF;
+    static constexpr int NRP = NR <= 1 ? 1 : (NR <= 4 ? 4 : 16);     // rows rounded up to a power of two (prefix / search)
+    static constexpr int KZ = (TF + 1) / 2;
+};
+
+// the shared-memory areas a tile is processed in
+struct TileSmem {
+    float4 *win;         // [NROWS][ent] window of U^m (w unused)
+    float *foot;         // [NROWS][ent][3] footprint
+    float4 *sv;          // staging: value + tag of 32 markers (+ 1 padding record)
+    float4 *swx;         // staging: x weights
+    float *swyz;         // staging: y-z weights [16][33] (weight index major: conflict-free stores by marker, loads by weight)
+};
+
+__device__ __forceinline__ size_t tile_win_bytes(int nrows, int ent) { return ((size_t)nrows * ent * 16 + 127) / 128 * 128; }
+__device__ __forceinline__ size_t tile_foot_bytes(int nrows, int ent) { return ((size_t)nrows * ent * 12 + 127) / 128 * 128; }
+
+__device__ __forceinline__ TileSmem stage_at(float4 *win, float *foot, char *stage)
+{
+    TileSmem s;
+    s.win = win; s.foot = foot;
+    s.sv = reinterpret_cast<float4 *>(stage);
+    s.swx = s.sv + MDF_STAGE_RECS;
+    s.swyz = reinterpret_cast<float *>(s.swx + MDF_STAGE_RECS);
+    return s;
+}
+
+// ---- tile header: chunk ranges, their inclusive prefix, geometry (one round trip: all indexed by the position) ----
+template <int TR>
+__device__ __forceinline__ void tile_load_hdr(const MdfArgs &a, const int pos, const int lane, TileHdr &H)
+{
+    using D = TileDims<TR>;
+    constexpr unsigned FULL = 0xffffffffu;
+    H.t = -1;
+    H.rec = make_int2(0, 0);
+    H.total = 0;
+    if (pos < 0) return;
+    if (lane < D::NR) H.rec = __ldg(a.tile_orec + (size_t)pos * D::NR + lane);
+    const int4 hd = __ldg(a.tile_ohdr + pos);
+    const int ts = hd.x;
+    H.m = (unsigned)hd.y;
+    H.t = hd.z;
+    H.cnt = H.rec.y - H.rec.x;
+    H.incl = H.cnt;
+#pragma unroll
+    for (int o = 1; o < D::NRP; o <<= 1) {
+        const int v = __shfl_up_sync(FULL, H.incl, o);
+        if (lane >= o) H.incl += v;
+    }
+    H.total = __shfl_sync(FULL, H.incl, D::NRP - 1);
+    const int blk = ts % a.cg.nbx, tyz = ts / a.cg.nbx;
+    H.ty = tyz % a.tg.nty; H.tz = tyz / a.tg.nty;
+    H.x0 = blk * CHUNK_W;
+}
+
+// ---- stage the window of U^m: asynchronous 16-byte copies, half a warp per row ------------------------------
+// Rows: fy = 0 .. TF-1 (unrolled; with two warps on a tile, `part` takes the rows fy = part, part + nparts, ...),
+// fz = 2 k + h.  Row coordinates ty TR - 1 + fy lie in [-1, ny + 4], so one conditional wrap is enough for
+// ny >= 4; rows outside a wall axis are never in the mask product.
+template <int TR>
+__device__ __forceinline__ void tile_issue_window(const MdfArgs &a, const TileHdr &H, float4 *win, const int lane,
+                                                  const int part, const int nparts)
+{
+    using D = TileDims<TR>;
+    const int ent = a.cg.ent;
+    const int l = lane & 15, h = lane >> 4;
+    const unsigned my = H.m >> 14, mz = H.m >> (21 + h);         // bit fy / bit 2 k: the row is reachable
+    const bool ex = l < ent && ((H.m >> l) & 1u);                // this lane's window entry is reachable
+    const int x = mod_wrap(H.x0 - 1 + l, a.g.nx);
+    int zoff[D::KZ];
+#pragma unroll
+    for (int k = 0; k < D::KZ; ++k) {
+        int z = H.tz * TR - 1 + 2 * k + h;
+        if (a.g.wallz) z = min(max(z, 0), a.g.nz - 1); else { if (z < 0) z += a.g.nz; else if (z >= a.g.nz) z -= a.g.nz; }
+        zoff[k] = z * a.g.ny;
+    }
+#pragma unroll
+    for (int fy = 0; fy < D::TF; ++fy) {
+        if (nparts > 1 && (fy % nparts) != part) continue;
+        int y = H.ty * TR - 1 + fy;
+        if (a.g.wally) y = min(max(y, 0), a.g.ny - 1); else { if (y < 0) y += a.g.ny; else if (y >= a.g.ny) y -= a.g.ny; }
+#pragma unroll
+        for (int k = 0; k < D::KZ; ++k) {
+            if (2 * k + 1 >= D::TF && h) continue;               // fz = 2 k + h < TF
+            if (ex && ((my >> fy) & (mz >> (2 * k)) & 1u))
+                cp_async16_cg(win + (fy * D::TF + 2 * k + h) * ent + l, a.U + (size_t)(zoff[k] + y) * a.g.nx + x);
+        }
+    }
+}
+
+// the markers of one batch: (source row, sorted index) of this lane's marker, its data in registers
+struct MarkerRegs { float4 fs, uk, du; int r, i; };
+
+template <int TR>
+__device__ __forceinline__ void tile_fetch(const MdfArgs &a, const TileHdr &H, const int base, const int lane, MarkerRegs &pf)
+{
+    using D = TileDims<TR>;
+    constexpr unsigned FULL = 0xffffffffu;
+    const int j = base + lane;
+    int r = 0;
+#pragma unroll
+    for (int step = D::NRP / 2; step >= 1; step >>= 1) {     // the first r with incl[r] > j
+        const int v = __shfl_sync(FULL, H.incl, r + step - 1);
+        if (j >= v) r += step;
+    }
+    const int r_first = __shfl_sync(FULL, H.rec.x, r);
+    const int r_incl = __shfl_sync(FULL, H.incl, r), r_cnt = __shfl_sync(FULL, H.cnt, r);
+    pf.r = r;
+    pf.i = r_first + (j - (r_incl - r_cnt));
+    if (j < H.total) {
+        pf.fs = __ldg(a.fs + pf.i);
+        pf.uk = __ldg(a.uk + pf.i);
+        pf.du = __ldcg(a.du + pf.i);
+    }
+}
+
+// ---- phase 1, lane = marker: interpolate, correct, stage the sweep record.
+// Returns the marker's tag (source row << 8) | window entry of cell cx - 1.
+template <int TR>
+__device__ __forceinline__ int tile_phase1(const MdfArgs &a, const TileHdr &H, const MarkerRegs &cur, const bool last,
+                                           const TileSmem &sm, const int lane)
+{
+    using D = TileDims<TR>;
+    const int ent = a.cg.ent;
+    const float4 fs = cur.fs, uk = cur.uk;
+    float4 d = cur.du;
+    const int e0 = __float_as_int(d.w) - H.x0;               // window entry of cell cx - 1
+    const int sy = cur.r % TR, sz = cur.r / TR;
+    float wx[4], wy[4], wz[4];
+    peskin4(fs.x, wx);
+    peskin4(fs.y, wy);
+    peskin4(fs.z, wz);
+    const float4 *w0 = sm.win + (sy * D::TF + sz) * ent + e0;
+    float ux = 0.f, uy = 0.f, uz = 0.f;
+    float *my_wyz = sm.swyz + lane;                  // [ky*4 + kz][marker]
+#pragma unroll
+    for (int ky = 0; ky < 4; ++ky) {
+        float wyz[4];
+#pragma unroll
+        for (int kz = 0; kz < 4; ++kz) {
+            wyz[kz] = wy[ky] * wz[kz];
+            const float4 *rowp = w0 + (ky * D::TF + kz) * ent;
+            const float4 c0 = rowp[0], c1 = rowp[1], c2 = rowp[2], c3 = rowp[3];
+            const float tx = fmaf(wx[3], c3.x, fmaf(wx[2], c2.x, fmaf(wx[1], c1.x, wx[0] * c0.x)));
+            const float ty_ = fmaf(wx[3], c3.y, fmaf(wx[2], c2.y, fmaf(wx[1], c1.y, wx[0] * c0.y)));
+            const float tz_ = fmaf(wx[3], c3.z, fmaf(wx[2], c2.z, fmaf(wx[1], c1.z, wx[0] * c0.z)));
+            ux = fmaf(wyz[kz], tx, ux);
+            uy = fmaf(wyz[kz], ty_, uy);
+            uz = fmaf(wyz[kz], tz_, uz);
+        }
+#pragma unroll
+        for (int kz = 0; kz < 4; ++kz) my_wyz[(ky * 4 + kz) * MDF_STAGE_RECS] = wyz[kz];
+    }
+    const float gx = uk.x - ux, gy = uk.y - uy, gz = uk.z - uz;
+    d.x = fmaf(fs.w, gx, d.x);
+    d.y = fmaf(fs.w, gy, d.y);
+    d.z = fmaf(fs.w, gz, d.z);
+    a.du[cur.i] = d;
+    const int tag = (cur.r << 8) | e0;
+    const float tagf = __int_as_float(tag);
+    sm.sv[lane] = last ? make_float4(d.x, d.y, d.z, tagf) : make_float4(fs.w * gx, fs.w * gy, fs.w * gz, tagf);
+    sm.swx[lane] = make_float4(wx[0], wx[1], wx[2], wx[3]);
+    return tag;
+}
+
+// ---- phase 2, lane = (half h of the 4-cell x window, target-row offset (jy, jz)): sweep the nb staged markers in
+// sorted order (warp-uniform control flow); the staged record of marker jj + 1 is read while marker jj is
+// processed.  chg / rowchg: bit jj set = marker jj starts another cell / another source row.
+struct SweepState {
+    int started;         // a window is open
+    int e;               // its first entry
+    float *frow;         // footprint row of this lane for the source row being swept
+    Acc3 p, q;           // window cells (e + 2h, e + 2h + 1)
+};
+
+__device__ __forceinline__ void sweep_flush(float *frow, int ee, const Acc3 &acc)
+{
+    float *d = frow + ee * 3;
+    d[0] += acc.x; d[1] += acc.y; d[2] += acc.z;
+}
+
+template <int TR>
+__device__ __forceinline__ void tile_sweep(const TileSmem &sm, const int ent, const int nb, const unsigned chg,
+                                           const unsigned rowchg, SweepState &st, const int lane)
+{
+    using D = TileDims<TR>;
+    constexpr unsigned FULL = 0xffffffffu;
+    const int l = lane & 15, h = lane >> 4;
+    const int jy = l >> 2, jz = l & 3;
+    const float2 *sw2 = reinterpret_cast<const float2 *>(sm.swx) + h;
+    const float *swz = sm.swyz + l * MDF_STAGE_RECS;
+    float4 v = sm.sv[0];
+    float2 w = sw2[0];
+    float wz_ = swz[0];
+    const float4 *pv = sm.sv + 1;                    // record jj + 1 (the last read lands on the padding record)
+    const float2 *pw = sw2 + 2;
+    const float *pz = swz + 1;
+    unsigned cbits = chg, rbits = rowchg;
+    Acc3 p = st.p, q = st.q;
+    int e = st.e, started = st.started;
+    float *frow = st.frow;
+#pragma unroll 4
+    for (int jj = 0; jj < nb; ++jj, ++pv, pw += 2, ++pz, cbits >>= 1, rbits >>= 1) {
+        const float4 vn = *pv;
+        const float2 wn = *pw;
+        const float wzn = *pz;
+        if (cbits & 1u) {                            // the sweep moves on to another cell or another source row
+            const int tg_ = __float_as_int(v.w);
+            const int en = tg_ & 0xff;
+            if (rbits & 1u) {                        // another source row (or the first marker of the tile)
+                const int rn = tg_ >> 8;
+                if (started) { sweep_flush(frow, e + 2 * h, p); sweep_flush(frow, e + 2 * h + 1, q); }
+                frow = sm.foot + (((rn % TR) + jy) * D::TF + ((rn / TR) + jz)) * ent * 3;
+                p = Acc3{0.f, 0.f, 0.f}; q = Acc3{0.f, 0.f, 0.f};
+                e = en;
+                started = 1;
+            } else {
+#pragma unroll 1
+                do {                                 // the leftmost window cell is complete
+                    if (h == 0) sweep_flush(frow, e, p);
+                    const float tx = __shfl_down_sync(FULL, p.x, 16);
+                    const float ty_ = __shfl_down_sync(FULL, p.y, 16);
+                    const float tz_ = __shfl_down_sync(FULL, p.z, 16);
+                    p = q;
+                    q.x = h ? 0.f : tx; q.y = h ? 0.f : ty_; q.z = h ? 0.f : tz_;
+                } while (++e < en);
+            }
+        }
+        const float vx = v.x * wz_, vy = v.y * wz_, vz = v.z * wz_;
+        p.x = fmaf(w.x, vx, p.x); p.y = fmaf(w.x, vy, p.y); p.z = fmaf(w.x, vz, p.z);
+        q.x = fmaf(w.y, vx, q.x); q.y = fmaf(w.y, vy, q.y); q.z = fmaf(w.y, vz, q.z);
+        v = vn; w = wn; wz_ = wzn;
+    }
+    st.p = p; st.q = q; st.e = e; st.started = started; st.frow = frow;
+}
+
+__device__ __forceinline__ void sweep_close(SweepState &st, const int lane)
+{
+    const int h = lane >> 4;
+    if (st.started) { sweep_flush(st.frow, st.e + 2 * h, st.p); sweep_flush(st.frow, st.e + 2 * h + 1, st.q); }
+    st.started = 0;
+}
+
+// ---- hand every footprint element to the cell that consumes it (plan: fdst): all the destinations first
+// (independent loads), then the stores.  With two warps on a tile, `part` takes the rows fy = part, part + nparts, ...
+template <int TR>
+__device__ __forceinline__ void tile_writeout(const MdfArgs &a, const TileHdr &H, const float *foot, const int lane,
+                                              const int part, const int nparts)
+{
+    using D = TileDims<TR>;
+    const int ent = a.cg.ent;
+    const int l = lane & 15, h = lane >> 4;
+    const unsigned my = H.m >> 14, mz = H.m >> (21 + h);
+    const bool ex = l < ent && ((H.m >> l) & 1u);
+    const int *__restrict__ dst = a.fdst + (size_t)H.t * (D::NROWS * ent) + l;
+    int o[D::TF][D::KZ];
+#pragma unroll
+    for (int fy = 0; fy < D::TF; ++fy)
+#pragma unroll
+        for (int k = 0; k < D::KZ; ++k) {
+            o[fy][k] = -1;
+            if (nparts > 1 && (fy % nparts) != part) continue;
+            if (2 * k + 1 >= D::TF && h) continue;
+            if (ex && ((my >> fy) & (mz >> (2 * k)) & 1u)) o[fy][k] = __ldg(dst + (fy * D::TF + 2 * k + h) * ent);
+        }
+#pragma unroll
+    for (int fy = 0; fy < D::TF; ++fy)
+#pragma unroll
+        for (int k = 0; k < D::KZ; ++k)
+            if (o[fy][k] >= 0) {
+                const float *sp = foot + ((fy * D::TF + 2 * k + h) * ent + l) * 3;
+                __stcg(a.F + o[fy][k], make_float4(sp[0], sp[1], sp[2], 0.f));
+            }
+}
+
+// The tile pass of ONE warp over a stream of tiles (next() hands out positions in the longest-first order, < 0 =
 // no more).  Software pipeline across tiles: the warp draws its next tile when it starts on the last 32 markers
 // of the current one (late, so that the dynamic balance is kept), and as soon as those are interpolated (the
 // window is dead from then on) it requests the next tile's window and first 32 markers, which arrive during
-// the last sweep and the write-out of the current tile.  wsm = the warp's shared
-// memory (mdf_warp_smem bytes).
+// the last sweep and the write-out of the current tile.  wsm = the warp's shared memory (mdf_warp_smem bytes).
 template <int TR, class Next>
 __device__ __forceinline__ void mdf_tile_loop(const MdfArgs &a, const bool last, char *wsm, const int lane, Next &&next)
 {
-    constexpr int NR = TR * TR, TF = TR + 3, NROWS = TF * TF;
-    constexpr int NRP = NR <= 1 ? 1 : (NR <= 4 ? 4 : 16);        // rows rounded up to a power of two (prefix / search)
-    constexpr int KZ = (TF + 1) / 2;
+    using D = TileDims<TR>;
     constexpr unsigned FULL = 0xffffffffu;
     const int ent = a.cg.ent;
-    const int l = lane & 15, h = lane >> 4;
-    const int jy = l >> 2, jz = l & 3;
-    const size_t win_bytes = ((size_t)NROWS * ent * 16 + 127) / 128 * 128;
-    const size_t foot_bytes = ((size_t)NROWS * ent * 12 + 127) / 128 * 128;
-    float4 *win = reinterpret_cast<float4 *>(wsm);                       // [NROWS][ent] U^m (w unused)
-    float *foot = reinterpret_cast<float *>(wsm + win_bytes);            // [NROWS][ent][3]
-    float4 *sv = reinterpret_cast<float4 *>(wsm + win_bytes + foot_bytes);   // staged value + tag
-    float4 *swx = sv + MDF_STAGE_RECS;                                   // staged x weights
-    float *swyz = reinterpret_cast<float *>(swx + MDF_STAGE_RECS);       // staged y-z weights [33][16]
-    const float2 *sw2 = reinterpret_cast<const float2 *>(swx) + h;
-    const float *swz = swyz + l;
-
-    // ---- tile header: chunk ranges, their inclusive prefix, geometry (one round trip: all indexed by the tile id)
-    auto load_hdr = [&](int pos, TileHdr &H) {
-        H.t = -1;
-        H.rec = make_int2(0, 0);
-        H.total = 0;
-        if (pos < 0) return;
-        if (lane < NR) H.rec = __ldg(a.tile_orec + (size_t)pos * NR + lane);
-        const int4 hd = __ldg(a.tile_ohdr + pos);
-        const int ts = hd.x;
-        H.m = (unsigned)hd.y;
-        H.t = hd.z;
-        H.cnt = H.rec.y - H.rec.x;
-        H.incl = H.cnt;
-#pragma unroll
-        for (int o = 1; o < NRP; o <<= 1) {
-            const int v = __shfl_up_sync(FULL, H.incl, o);
-            if (lane >= o) H.incl += v;
-        }
-        H.total = __shfl_sync(FULL, H.incl, NRP - 1);
-        const int blk = ts % a.cg.nbx, tyz = ts / a.cg.nbx;
-        H.ty = tyz % a.tg.nty; H.tz = tyz / a.tg.nty;
-        H.x0 = blk * CHUNK_W;
-    };
-
-    // ---- stage the window of U^m: asynchronous 16-byte copies, half a warp per row ---------------------
-    // Rows: fy = 0 .. TF-1 (unrolled), fz = 2 k + h.  Row coordinates ty TR - 1 + fy lie in [-1, ny + 4], so one
-    // conditional wrap is enough for ny >= 4; rows outside a wall axis are never in the mask product.
-    auto issue_window = [&](const TileHdr &H) {
-        const unsigned my = H.m >> 14, mz = H.m >> (21 + h);         // bit fy / bit 2 k: the row is reachable
-        const bool ex = l < ent && ((H.m >> l) & 1u);                // this lane's window entry is reachable
-        const int x = mod_wrap(H.x0 - 1 + l, a.g.nx);
-        int zoff[KZ];
-#pragma unroll
-        for (int k = 0; k < KZ; ++k) {
-            int z = H.tz * TR - 1 + 2 * k + h;
-            if (a.g.wallz) z = min(max(z, 0), a.g.nz - 1); else { if (z < 0) z += a.g.nz; else if (z >= a.g.nz) z -= a.g.nz; }
-            zoff[k] = z * a.g.ny;
-        }
-#pragma unroll
-        for (int fy = 0; fy < TF; ++fy) {
-            int y = H.ty * TR - 1 + fy;
-            if (a.g.wally) y = min(max(y, 0), a.g.ny - 1); else { if (y < 0) y += a.g.ny; else if (y >= a.g.ny) y -= a.g.ny; }
-#pragma unroll
-            for (int k = 0; k < KZ; ++k) {
-                if (2 * k + 1 >= TF && h) continue;              // fz = 2 k + h < TF
-                if (ex && ((my >> fy) & (mz >> (2 * k)) & 1u))
-                    cp_async16_cg(win + (fy * TF + 2 * k + h) * ent + l, a.U + (size_t)(zoff[k] + y) * a.g.nx + x);
-            }
-        }
-    };
-
-    // the markers of one batch: (source row, sorted index) of this lane's marker, its data in registers
-    struct Pre { float4 fs, uk, du; int r, i; };
-    auto fetch = [&](const TileHdr &H, int base, Pre &pf) {
-        const int j = base + lane;
-        int r = 0;
-#pragma unroll
-        for (int step = NRP / 2; step >= 1; step >>= 1) {    // the first r with incl[r] > j
-            const int v = __shfl_sync(FULL, H.incl, r + step - 1);
-            if (j >= v) r += step;
-        }
-        const int r_first = __shfl_sync(FULL, H.rec.x, r);
-        const int r_incl = __shfl_sync(FULL, H.incl, r), r_cnt = __shfl_sync(FULL, H.cnt, r);
-        pf.r = r;
-        pf.i = r_first + (j - (r_incl - r_cnt));
-        if (j < H.total) {
-            pf.fs = __ldg(a.fs + pf.i);
-            pf.uk = __ldg(a.uk + pf.i);
-            pf.du = __ldcg(a.du + pf.i);
-        }
-    };
-
+    const size_t win_bytes = tile_win_bytes(D::NROWS, ent), foot_bytes = tile_foot_bytes(D::NROWS, ent);
+    const TileSmem sm = stage_at(reinterpret_cast<float4 *>(wsm), reinterpret_cast<float *>(wsm + win_bytes),
+                                 wsm + win_bytes + foot_bytes);
     TileHdr H, Hn;
-    Pre cur;
-    load_hdr(next(), H);
+    MarkerRegs cur;
+    tile_load_hdr<TR>(a, next(), lane, H);
     if (H.t < 0) return;
-    issue_window(H);
-    fetch(H, 0, cur);
+    tile_issue_window<TR>(a, H, sm.win, lane, 0, 1);
+    tile_fetch<TR>(a, H, 0, lane, cur);
 
     while (H.t >= 0) {
-        const int total = H.total, x0 = H.x0;
+        const int total = H.total;
         // zero the footprint while the window copies and the first markers are in flight
         {
-            float4 *f4 = reinterpret_cast<float4 *>(foot);
+            float4 *f4 = reinterpret_cast<float4 *>(sm.foot);
             const int n4 = (int)(foot_bytes / 16);
             for (int i = lane; i < n4; i += 32) f4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
@@ -212,147 +405,38 @@ __device__ __forceinline__ void mdf_tile_loop(const MdfArgs &a, const bool last,
         __syncwarp();
 
         // ---- the tile's markers, 32 at a time -------------------------------------------------------------
-        int tag_cur = -1;                            // (source row << 8) | cell of the last marker swept, -1 = none yet
-        int e = 0;
-        float *frow = foot;
-        Acc3 p{0.f, 0.f, 0.f}, q{0.f, 0.f, 0.f};     // window cells (e + 2h, e + 2h + 1)
-        auto flush = [&](int ee, const Acc3 &acc) {
-            float *d = frow + ee * 3;
-            d[0] += acc.x; d[1] += acc.y; d[2] += acc.z;
-        };
+        SweepState st;
+        st.started = 0; st.e = 0; st.frow = sm.foot;
+        st.p = Acc3{0.f, 0.f, 0.f}; st.q = Acc3{0.f, 0.f, 0.f};
+        int tag_cur = -1;                            // tag of the last marker swept, -1 = none yet
         Hn.t = -1;
-        if (total <= 0) load_hdr(next(), Hn);
+        if (total <= 0) tile_load_hdr<TR>(a, next(), lane, Hn);
         for (int base = 0; base < total; base += MDF_BATCH) {
             const int nb = min(MDF_BATCH, total - base);
             const bool last_batch = base + MDF_BATCH >= total;
-            if (last_batch) load_hdr(next(), Hn);
+            if (last_batch) tile_load_hdr<TR>(a, next(), lane, Hn);
             int tag = -2;
-            if (lane < nb) {
-                // ---- phase 1: interpolate, correct, stage ----------------
-                const float4 fs = cur.fs, uk = cur.uk;
-                float4 d = cur.du;
-                const int e0 = __float_as_int(d.w) - x0;             // window entry of cell cx - 1
-                const int sy = cur.r % TR, sz = cur.r / TR;
-                float wx[4], wy[4], wz[4];
-                peskin4(fs.x, wx);
-                peskin4(fs.y, wy);
-                peskin4(fs.z, wz);
-                const float4 *w0 = win + (sy * TF + sz) * ent + e0;
-                float ux = 0.f, uy = 0.f, uz = 0.f;
-                float4 *my_wyz = reinterpret_cast<float4 *>(swyz + lane * 16);
-#pragma unroll
-                for (int ky = 0; ky < 4; ++ky) {
-                    float wyz[4];
-#pragma unroll
-                    for (int kz = 0; kz < 4; ++kz) {
-                        wyz[kz] = wy[ky] * wz[kz];
-                        const float4 *rowp = w0 + (ky * TF + kz) * ent;
-                        const float4 c0 = rowp[0], c1 = rowp[1], c2 = rowp[2], c3 = rowp[3];
-                        const float tx = fmaf(wx[3], c3.x, fmaf(wx[2], c2.x, fmaf(wx[1], c1.x, wx[0] * c0.x)));
-                        const float ty_ = fmaf(wx[3], c3.y, fmaf(wx[2], c2.y, fmaf(wx[1], c1.y, wx[0] * c0.y)));
-                        const float tz_ = fmaf(wx[3], c3.z, fmaf(wx[2], c2.z, fmaf(wx[1], c1.z, wx[0] * c0.z)));
-                        ux = fmaf(wyz[kz], tx, ux);
-                        uy = fmaf(wyz[kz], ty_, uy);
-                        uz = fmaf(wyz[kz], tz_, uz);
-                    }
-                    my_wyz[ky] = make_float4(wyz[0], wyz[1], wyz[2], wyz[3]);
-                }
-                const float gx = uk.x - ux, gy = uk.y - uy, gz = uk.z - uz;
-                d.x = fmaf(fs.w, gx, d.x);
-                d.y = fmaf(fs.w, gy, d.y);
-                d.z = fmaf(fs.w, gz, d.z);
-                a.du[cur.i] = d;
-                tag = (cur.r << 8) | e0;
-                const float tagf = __int_as_float(tag);
-                sv[lane] = last ? make_float4(d.x, d.y, d.z, tagf) : make_float4(fs.w * gx, fs.w * gy, fs.w * gz, tagf);
-                swx[lane] = make_float4(wx[0], wx[1], wx[2], wx[3]);
-            }
-            // which staged markers start another cell / another source row (warp-uniform bit masks: the sweep below
+            if (lane < nb) tag = tile_phase1<TR>(a, H, cur, last, sm, lane);
+            // which staged markers start another cell / another source row (warp-uniform bit masks: the sweep
             // branches on registers, not on a value it has just loaded)
             const int prev_tag = __shfl_up_sync(FULL, tag, 1);
             const int before = lane == 0 ? tag_cur : prev_tag;
             const unsigned chg = __ballot_sync(FULL, lane < nb && tag != before);
             const unsigned rowchg = __ballot_sync(FULL, lane < nb && ((tag ^ before) >> 8) != 0);
-            const int tag_last = __shfl_sync(FULL, tag, nb - 1);
+            tag_cur = __shfl_sync(FULL, tag, nb - 1);
             __syncwarp();                                // staging buffer complete; nobody reads the window any more
             if (!last_batch) {
-                fetch(H, base + MDF_BATCH, cur);         // in flight during the sweep
+                tile_fetch<TR>(a, H, base + MDF_BATCH, lane, cur);     // in flight during the sweep
             } else if (Hn.t >= 0) {
-                issue_window(Hn);                        // the window is dead: bring in the next tile's, and its first markers
-                fetch(Hn, 0, cur);
+                tile_issue_window<TR>(a, Hn, sm.win, lane, 0, 1);      // the window is dead: bring in the next tile's,
+                tile_fetch<TR>(a, Hn, 0, lane, cur);                   // and its first markers
             }
-
-            // ---- phase 2: sweep the staged markers in sorted order (warp-uniform control flow); the staged record
-            // of marker jj + 1 is read while marker jj is processed
-            float4 v = sv[0];
-            float2 w = sw2[0];
-            float wz_ = swz[0];
-            const float4 *pv = sv + 1;                       // record jj + 1 (the last read lands on the padding record)
-            const float2 *pw = sw2 + 2;
-            const float *pz = swz + 16;
-            unsigned cbits = chg, rbits = rowchg;
-#pragma unroll 4
-            for (int jj = 0; jj < nb; ++jj, ++pv, pw += 2, pz += 16, cbits >>= 1, rbits >>= 1) {
-                const float4 vn = *pv;
-                const float2 wn = *pw;
-                const float wzn = *pz;
-                if (cbits & 1u) {                            // the sweep moves on to another cell or another source row
-                    const int tg_ = __float_as_int(v.w);
-                    const int en = tg_ & 0xff;
-                    if (rbits & 1u) {                        // another source row (or the first marker of the tile)
-                        const int rn = tg_ >> 8;
-                        if (tag_cur >= 0) { flush(e + 2 * h, p); flush(e + 2 * h + 1, q); }
-                        frow = foot + (((rn % TR) + jy) * TF + ((rn / TR) + jz)) * ent * 3;
-                        p = Acc3{0.f, 0.f, 0.f}; q = Acc3{0.f, 0.f, 0.f};
-                        e = en;
-                        tag_cur = tg_;
-                    } else {
-#pragma unroll 1
-                        do {                                 // the leftmost window cell is complete
-                            if (h == 0) flush(e, p);
-                            const float tx = __shfl_down_sync(FULL, p.x, 16);
-                            const float ty_ = __shfl_down_sync(FULL, p.y, 16);
-                            const float tz_ = __shfl_down_sync(FULL, p.z, 16);
-                            p = q;
-                            q.x = h ? 0.f : tx; q.y = h ? 0.f : ty_; q.z = h ? 0.f : tz_;
-                        } while (++e < en);
-                    }
-                }
-                const float vx = v.x * wz_, vy = v.y * wz_, vz = v.z * wz_;
-                p.x = fmaf(w.x, vx, p.x); p.y = fmaf(w.x, vy, p.y); p.z = fmaf(w.x, vz, p.z);
-                q.x = fmaf(w.y, vx, q.x); q.y = fmaf(w.y, vy, q.y); q.z = fmaf(w.y, vz, q.z);
-                v = vn; w = wn; wz_ = wzn;
-            }
-            tag_cur = tag_last;
-            __syncwarp();                                    // every lane is done with the staging buffer
+            tile_sweep<TR>(sm, ent, nb, chg, rowchg, st, lane);
+            __syncwarp();                                // every lane is done with the staging buffer
         }
-        if (tag_cur >= 0) { flush(e + 2 * h, p); flush(e + 2 * h + 1, q); }
+        sweep_close(st, lane);
         __syncwarp();
-
-        // ---- hand every footprint element to the cell that consumes it (plan: fdst) ------------------------
-        // all the destinations first (independent loads), then the stores
-        {
-            const unsigned my = H.m >> 14, mz = H.m >> (21 + h);
-            const bool ex = l < ent && ((H.m >> l) & 1u);
-            const int *__restrict__ dst = a.fdst + (size_t)H.t * (NROWS * ent) + l;
-            int o[TF][KZ];
-#pragma unroll
-            for (int fy = 0; fy < TF; ++fy)
-#pragma unroll
-                for (int k = 0; k < KZ; ++k) {
-                    o[fy][k] = -1;
-                    if (2 * k + 1 >= TF && h) continue;
-                    if (ex && ((my >> fy) & (mz >> (2 * k)) & 1u)) o[fy][k] = __ldg(dst + (fy * TF + 2 * k + h) * ent);
-                }
-#pragma unroll
-            for (int fy = 0; fy < TF; ++fy)
-#pragma unroll
-                for (int k = 0; k < KZ; ++k)
-                    if (o[fy][k] >= 0) {
-                        const float *sp = foot + ((fy * TF + 2 * k + h) * ent + l) * 3;
-                        __stcg(a.F + o[fy][k], make_float4(sp[0], sp[1], sp[2], 0.f));
-                    }
-        }
+        tile_writeout<TR>(a, H, sm.foot, lane, 0, 1);
         __syncwarp();
         H = Hn;
     }
@@ -372,6 +456,93 @@ k_mdf_tiles(const __grid_constant__ MdfArgs a, int *__restrict__ cursor, int las
         if (lane == 0) { t = atomicAdd(cursor, 1); t = t < nt ? t : -1; }
         return __shfl_sync(0xffffffffu, t, 0);
     });
+}
+
+// ---- two warps per tile -------------------------------------------------------------------------------------
+// A block is ONE pair of warps that share a tile's window and footprint (half the shared memory per warp of the
+// one-warp pass, so 20 instead of 12 warps fit on an SM) and take its batches of 32 markers in turn: in time
+// slot s the warp that owns batch s interpolates it (phase 1, into its own staging buffer) while the other warp
+// sweeps batch s - 1 (phase 2) into the shared footprint; a block barrier ends the slot.  The sweeps therefore
+// still follow one another in sorted order -- every sum keeps its fixed order -- and the shared-memory-heavy
+// interpolation of one warp overlaps the FMA-heavy sweep of the other.  Each sweep starts with an empty window
+// and ends with a full flush.
+inline size_t mdf_pair_smem(int tr, const ChunkGeom &cg)
+{
+    const size_t tf = (size_t)tr + 3;
+    const size_t win = (tf * tf * (size_t)cg.ent * 16 + 127) / 128 * 128;
+    const size_t foot = (tf * tf * (size_t)cg.ent * 12 + 127) / 128 * 128;
+    return win + foot + 2 * MDF_STAGE_BYTES;
+}
+
+#ifndef MDF_PAIR_MIN_BLOCKS_CFG
+#define MDF_PAIR_MIN_BLOCKS_CFG 10
+#endif
+
+template <int TR>
+__global__ void __launch_bounds__(64, MDF_PAIR_MIN_BLOCKS_CFG)
+k_mdf_pairs(const __grid_constant__ MdfArgs a, int *__restrict__ cursor, int last_i)
+{
+    using D = TileDims<TR>;
+    constexpr unsigned FULL = 0xffffffffu;
+    extern __shared__ __align__(128) char smem[];
+    __shared__ int s_pos[2];
+    const bool last = last_i != 0;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int nt = min(*a.n_tiles, a.tile_cap);
+    const int ent = a.cg.ent;
+    const size_t win_bytes = tile_win_bytes(D::NROWS, ent), foot_bytes = tile_foot_bytes(D::NROWS, ent);
+    const TileSmem sm = stage_at(reinterpret_cast<float4 *>(smem), reinterpret_cast<float *>(smem + win_bytes),
+                                 smem + win_bytes + foot_bytes + (size_t)w * MDF_STAGE_BYTES);
+    if (threadIdx.x == 0) { const int t = atomicAdd(cursor, 1); s_pos[0] = t < nt ? t : -1; }
+    __syncthreads();
+    for (int it = 0;; ++it) {
+        const int pos = s_pos[it & 1];
+        if (pos < 0) break;
+        // the next tile is drawn now; its position is read after the barriers of this tile
+        if (threadIdx.x == 0) { const int t = atomicAdd(cursor, 1); s_pos[(it + 1) & 1] = t < nt ? t : -1; }
+        TileHdr H;
+        tile_load_hdr<TR>(a, pos, lane, H);
+        const int total = H.total;
+        const int nbatch = (total + MDF_BATCH - 1) / MDF_BATCH;
+        tile_issue_window<TR>(a, H, sm.win, lane, w, 2);
+        MarkerRegs cur;
+        if (w < nbatch) tile_fetch<TR>(a, H, w * MDF_BATCH, lane, cur);      // this warp's first batch
+        {
+            float4 *f4 = reinterpret_cast<float4 *>(sm.foot);
+            const int n4 = (int)(foot_bytes / 16);
+            for (int i = threadIdx.x; i < n4; i += 64) f4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        cp_async_wait_all();
+        __syncthreads();
+        unsigned chg = 0u, rowchg = 0u;
+        int nb_staged = 0;
+        for (int s = 0; s <= nbatch; ++s) {
+            if ((s & 1) == w) {
+                if (s < nbatch) {
+                    // phase 1 of batch s
+                    const int base = s * MDF_BATCH;
+                    const int nb = min(MDF_BATCH, total - base);
+                    int tag = -2;
+                    if (lane < nb) tag = tile_phase1<TR>(a, H, cur, last, sm, lane);
+                    const int prev_tag = __shfl_up_sync(FULL, tag, 1);
+                    chg = __ballot_sync(FULL, lane < nb && (lane == 0 || tag != prev_tag));
+                    rowchg = __ballot_sync(FULL, lane < nb && (lane == 0 || ((tag ^ prev_tag) >> 8) != 0));
+                    nb_staged = nb;
+                    if (s + 2 < nbatch) tile_fetch<TR>(a, H, base + 2 * MDF_BATCH, lane, cur);   // this warp's next batch
+                }
+            } else if (s >= 1) {
+                // phase 2 of batch s - 1 (staged by this warp in the previous slot)
+                SweepState st;
+                st.started = 0; st.e = 0; st.frow = sm.foot;
+                st.p = Acc3{0.f, 0.f, 0.f}; st.q = Acc3{0.f, 0.f, 0.f};
+                tile_sweep<TR>(sm, ent, nb_staged, chg, rowchg, st, lane);
+                sweep_close(st, lane);
+            }
+            __syncthreads();
+        }
+        tile_writeout<TR>(a, H, sm.foot, lane, w, 2);
+        __syncthreads();
+    }
 }
 
 // ---- stage B ---------------------------------------------------------------------------------------

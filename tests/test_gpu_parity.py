@@ -240,7 +240,9 @@ def _variants(api):
         ("default", {}),
         ("tile_rows_1_launches", {api.OPT_TILE_ROWS: 1, api.OPT_PERSISTENT: api.PERSISTENT_OFF}),
         ("tile_rows_2_persistent", {api.OPT_TILE_ROWS: 2, api.OPT_PERSISTENT: api.PERSISTENT_ON}),
-        ("tile_rows_4_launches", {api.OPT_TILE_ROWS: 4, api.OPT_PERSISTENT: api.PERSISTENT_OFF}),
+        ("tile_rows_4_launches", {api.OPT_TILE_ROWS: 4, api.OPT_PERSISTENT: api.PERSISTENT_OFF, api.OPT_TILE_WARPS: 1}),
+        ("tile_rows_4_warp_pairs", {api.OPT_TILE_ROWS: 4, api.OPT_PERSISTENT: api.PERSISTENT_OFF, api.OPT_TILE_WARPS: 2}),
+        ("tile_rows_2_warp_pairs", {api.OPT_TILE_ROWS: 2, api.OPT_PERSISTENT: api.PERSISTENT_OFF, api.OPT_TILE_WARPS: 2}),
         ("tile_rows_4_persistent", {api.OPT_TILE_ROWS: 4, api.OPT_PERSISTENT: api.PERSISTENT_ON}),
         ("serial_plain_launches", {api.OPT_OVERLAP: 0, api.OPT_GRAPH: 0}),
         ("unfused_round1_pipeline", {api.OPT_FUSED: 0}),
@@ -366,7 +368,9 @@ def test_odd_lattices_chunk_and_tile_edges(api, orc, shape, wall):
     r_fields = r_du = None
     variants = [{api.OPT_SPREAD: api.SPREAD_GATHER}, {api.OPT_SPREAD: api.SPREAD_ATOMIC},
                 {api.OPT_TILE_ROWS: 4}, {api.OPT_TILE_ROWS: 2, api.OPT_PERSISTENT: api.PERSISTENT_OFF},
-                {api.OPT_TILE_ROWS: 4, api.OPT_PERSISTENT: api.PERSISTENT_OFF}, {api.OPT_FUSED: 0},
+                {api.OPT_TILE_ROWS: 4, api.OPT_PERSISTENT: api.PERSISTENT_OFF, api.OPT_TILE_WARPS: 1},
+                {api.OPT_TILE_ROWS: 4, api.OPT_PERSISTENT: api.PERSISTENT_OFF, api.OPT_TILE_WARPS: 2},
+                {api.OPT_TILE_ROWS: 1, api.OPT_PERSISTENT: api.PERSISTENT_OFF, api.OPT_TILE_WARPS: 2}, {api.OPT_FUSED: 0},
                 {api.OPT_INTERP: api.INTERP_CHUNK_SMEM}, {api.OPT_SPREAD: api.SPREAD_BLOCK125}]
     for opts in variants:
         sim = api.LbmIbm(nx, ny, nz, 0.8, wall=wall, stream=_stream())

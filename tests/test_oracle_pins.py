@@ -289,6 +289,86 @@ def test_K9_poiseuille_exact_discrete_profile(tau, forcing):
     assert np.allclose(rho, 1.0, atol=1e-12)
 
 
+def test_K9_poiseuille_from_rest_converges_to_the_exact_profile():
+    """K9 started from rest (u0 = 0) instead of from the answer: the profile must be REACHED, not merely held.
+    tau = 1 makes the diffusive time short (nu = 1/6): H^2 / nu = 384 steps for H = 8; 40 diffusive times."""
+    H, g, tau = 8, 1e-5, 1.0
+    nu = (tau - 0.5) / 3.0
+    for forcing in ("guo", "shift"):
+        o = Oracle(2, 2, H, tau, wall=(0, 0, 1), g=(g, 0.0, 0.0), forcing=forcing)
+        z = np.arange(H, dtype=np.float64)
+        slip = g * (16 * tau * tau - 20 * tau + 3) / (4 * (2 * tau - 1))
+        exact = g / (2 * nu) * (z + 0.5) * (H - 0.5 - z) + slip
+        o.step(int(40 * H * H / nu), 0)
+        rho, u, _ = o.read_fields()
+        prof = u[0].mean(axis=(1, 2))
+        assert prof.max() > 0.9 * exact.max()                  # it did move away from rest
+        assert np.abs(prof - exact).max() < 1e-8 * g
+
+
+# ----------------------------------------------------------------------------------------------
+# K14: second moment of the forced collision (the part of the Guo source term K8 / K9 do not see)
+_E = np.array([[0, 0, 0], [1, 0, 0], [-1, 0, 0], [0, 1, 0], [0, -1, 0], [0, 0, 1], [0, 0, -1],
+               [1, 1, 0], [-1, -1, 0], [1, -1, 0], [-1, 1, 0], [1, 0, 1], [-1, 0, -1], [1, 0, -1],
+               [-1, 0, 1], [0, 1, 1], [0, -1, -1], [0, 1, -1], [0, -1, 1]], dtype=np.float64)
+
+
+def test_K14_guo_source_second_moment_closed_form():
+    """Uniform periodic box, rho = 1, uniform u0 and uniform acceleration a: streaming maps a uniform state onto
+    itself, so a step is the collision alone and every moment follows a closed recurrence.
+
+    Moments of the D3Q19 equilibrium and of the Guo source S_i = t_i rho [3 (e_i - u*).a + 9 (e_i.u*)(e_i.a)]
+    (P:56 force inclusion, reading R3; u* = U + a/2):
+        sum_i e e^T Eq_i(rho, u) = rho (I/3 + u u^T),      sum_i e e^T S_i = rho (u* a^T + a u*^T),
+        sum_i e Eq_i = rho u,  sum_i e S_i = rho a,  sum_i S_i = 0.
+    With f' = f - (f - Eq(rho, u*))/tau + (1 - 1/(2 tau)) S the momentum gains rho a per step (U_{n+1} = U_n + a)
+    and the second moment Pi = sum_i e e^T f_i obeys
+        Pi_{n+1} = (1 - 1/tau) Pi_n + (1/tau) rho (I/3 + u* u*^T) + (1 - 1/(2 tau)) rho (u* a^T + a u*^T),
+    whose solution from Pi_0 = rho (I/3 + u0 u0^T) is
+        Pi_n = rho [ I/3 + U_n U_n^T - (1/4) a a^T (1 - (1 - 1/tau)^n) ].
+    (Check: insert, use u* = U_n + a/2 and U_{n+1} = U_n + a; the a a^T terms give -1/4 + (1/tau)(1/4) ... = the
+    stated factor.)  Dropping the 9 (e.u*)(e.a) term, or writing U for u* in the source, changes Pi at O(|u||a|)
+    and O(|a|^2): the mutated recurrences below miss the oracle by many orders of magnitude more than the pin allows."""
+    tau = 0.8
+    u0 = np.array([0.021, -0.013, 0.008])
+    a = np.array([0.011, 0.007, -0.009])
+    nx, ny, nz = 3, 4, 5
+    o = Oracle(nx, ny, nz, tau, g=tuple(a))
+    o.set_fields(None, np.broadcast_to(u0[:, None, None, None], (3, nz, ny, nx)).copy())
+
+    def second_moment():
+        f = o.populations()
+        assert np.abs(f - f[:, :1, :1, :1]).max() < 1e-15            # stays uniform
+        return np.einsum("ia,ib,i->ab", _E, _E, f[:, 0, 0, 0])
+
+    def recurrence(P, U, variant):
+        us = U + 0.5 * a
+        uv = U if variant == "U_for_ustar" else us
+        src = np.outer(uv, a) + np.outer(a, uv)
+        if variant == "no_second_order":                              # only 3 (e - u*).a kept: -(u*.a) I
+            src = -np.dot(us, a) * np.eye(3)
+        return (1 - 1 / tau) * P + (1 / tau) * (np.eye(3) / 3 + np.outer(us, us)) + (1 - 0.5 / tau) * src
+
+    P = {v: np.eye(3) / 3 + np.outer(u0, u0) for v in ("exact", "no_second_order", "U_for_ustar")}
+    U = u0.copy()
+    assert np.abs(second_moment() - P["exact"]).max() < 1e-15
+    worst = {v: 0.0 for v in P}
+    for n in range(1, 8):
+        o.step(1, 0)
+        for v in P:
+            P[v] = recurrence(P[v], U, v)
+        U = U + a
+        got = second_moment()
+        closed = np.eye(3) / 3 + np.outer(U, U) - 0.25 * np.outer(a, a) * (1 - (1 - 1 / tau) ** n)
+        assert np.abs(got - closed).max() < 1e-14, n
+        assert np.abs(got - P["exact"]).max() < 1e-14, n
+        for v in P:
+            worst[v] = max(worst[v], np.abs(got - P[v]).max())
+        rho, u, _ = o.read_fields()
+        assert np.abs(u[:, 0, 0, 0] - U).max() < 1e-15 and abs(rho[0, 0, 0] - 1) < 1e-15
+    assert worst["no_second_order"] > 1e-5 and worst["U_for_ustar"] > 1e-5      # the pin discriminates
+
+
 # K10: tau <-> nu through the decay of a periodic shear wave
 def test_K10_shear_wave_decay():
     L, tau, A = 32, 0.8, 1e-4
