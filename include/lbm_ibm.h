@@ -108,6 +108,11 @@ enum {
                              and alternates between interpolating one batch of 32 markers and sweeping the
                              previous one (measured comparison: more warps per SM, no faster).  Results agree
                              to rounding (each batch's sweep is flushed).                                   */
+    LBM_OPT_TRACE = 15,   /* 1 = the graph of the overlapped step also records a timing event after every kernel of
+                             the MDF branch, after the bulk stream-collide and after the binning branch; after
+                             lbm_sync, lbm_get_info(LBM_INFO_TRACE_NS + i) is the device time in ns from the fork
+                             of the LAST step to event i and lbm_trace_label(i) names it.  A profiling aid
+                             (the timeline of the concurrent branches); results do not depend on it.          */
     LBM_OPT_MDF_BLOCKS = 13 /* tuning: blocks per SM of the tile pass / of the persistent MDF kernel (0 = default:
                              as many as fit / one); fewer blocks leave more of every SM to the stream-collide
                              pass that runs beside the MDF loop.  Results do not depend on it.           */
@@ -127,6 +132,8 @@ enum {
     LBM_INFO_TILES = 10,        /* tiles (chunks of one x block and one block of tile-rows x tile-rows source rows) in the last step */
     LBM_INFO_ACTIVE_WORDS = 11, /* 32-cell words of the active mask that hold an active cell (the cells the
                                    second stream-collide pass of the overlapped step updates)          */
+    LBM_INFO_TRACE_COUNT = 12,  /* number of trace events of a step (LBM_OPT_TRACE)                  */
+    LBM_INFO_TRACE_NS = 200,    /* + i: device time in ns from the fork of the last step to trace event i */
     LBM_INFO_PHASE_NS = 100     /* + phase: accumulated device time in ns under LBM_OPT_TIMING.
                                    phases: 0 kinematics+keys, 1 sort, 2 gather+bins, 3 moments on
                                    active cells, 4 interpolation+correction (fused path: the whole tile
@@ -221,6 +228,10 @@ int lbm_sync(lbm_t *h);
 
 /* Text of the last error raised on the calling thread ("" if none). */
 const char *lbm_last_error(void);
+
+/* Label of trace event i of the last step (LBM_OPT_TRACE), "" when out of range.  The string is owned
+ * by the handle and valid until the next step. */
+const char *lbm_trace_label(lbm_t *h, int i);
 
 #ifdef __cplusplus
 }

@@ -22,10 +22,11 @@ if not os.path.exists(LIB_PATH):
 _L = C.CDLL(LIB_PATH)
 
 OPT_SPREAD, OPT_FORCING, OPT_GRAPH, OPT_LBM_KERNEL, OPT_INTERP, OPT_TIMING, OPT_OVERLAP, OPT_MOMENTS = 1, 2, 3, 4, 5, 6, 7, 8
-OPT_FUSED, OPT_TILE_ROWS, OPT_PERSISTENT, OPT_TILE_CAP, OPT_MDF_BLOCKS, OPT_TILE_WARPS = 9, 10, 11, 12, 13, 14
+OPT_FUSED, OPT_TILE_ROWS, OPT_PERSISTENT, OPT_TILE_CAP, OPT_MDF_BLOCKS, OPT_TILE_WARPS, OPT_TRACE = 9, 10, 11, 12, 13, 14, 15
 PERSISTENT_AUTO, PERSISTENT_ON, PERSISTENT_OFF = 0, 1, 2
 INFO_MARKERS, INFO_BODIES, INFO_STEPS, INFO_LAUNCHES, INFO_ACTIVE_CELLS, INFO_DEVICE_BYTES, INFO_STATUS = range(1, 8)
 INFO_RUNS, INFO_RUN_ENTRIES, INFO_TILES, INFO_ACTIVE_WORDS = 8, 9, 10, 11
+INFO_TRACE_COUNT, INFO_TRACE_NS = 12, 200
 INFO_PHASE_NS = 100
 PHASES = ["keys", "sort", "bins", "moments", "interp", "spread", "lbm", "lbm_active"]
 SPREAD_GATHER, SPREAD_ATOMIC, SPREAD_GATHER_PLAIN, SPREAD_BLOCK125 = 0, 1, 2, 3
@@ -35,7 +36,8 @@ FORCING_GUO, FORCING_SHIFT = 0, 1
 
 EXPORTS = ["lbm_create", "lbm_destroy", "lbm_query_layout", "lbm_set_stream", "lbm_set_option", "lbm_get_info", "lbm_set_fields",
            "ibm_set_markers", "ibm_set_kinematics", "ibm_update_kinematics", "ibm_clear", "lbm_ibm_step", "lbm_read_fields",
-           "ibm_read_markers", "ibm_read_markers_async", "ibm_wait_markers", "lbm_sync", "lbm_last_error"]
+           "ibm_read_markers", "ibm_read_markers_async", "ibm_wait_markers", "lbm_sync", "lbm_last_error",
+           "lbm_trace_label"]
 
 
 class _Bc(C.Structure):
@@ -65,6 +67,8 @@ _L.ibm_wait_markers.argtypes = [_vp]
 _L.lbm_sync.argtypes = [_vp]
 _L.lbm_last_error.restype = C.c_char_p
 _L.lbm_last_error.argtypes = []
+_L.lbm_trace_label.restype = C.c_char_p
+_L.lbm_trace_label.argtypes = [_vp, C.c_int]
 
 
 class LbmError(RuntimeError):
@@ -190,6 +194,11 @@ class LbmIbm:
     def phase_ms(self) -> dict:
         """per-phase device time accumulated under OPT_TIMING, in ms"""
         return {n: self.get_info(INFO_PHASE_NS + i) * 1e-6 for i, n in enumerate(PHASES)}
+
+    def trace(self) -> list:
+        """[(label, ms since the fork of the last step)] of the trace events (OPT_TRACE)"""
+        n = self.get_info(INFO_TRACE_COUNT)
+        return [(_L.lbm_trace_label(self._h, i).decode(), self.get_info(INFO_TRACE_NS + i) * 1e-6) for i in range(n)]
 
     def sync(self):
         _check(_L.lbm_sync(self._h), "lbm_sync")

@@ -200,6 +200,11 @@ struct lbm {
     bool realloc_tables = false;        // LBM_OPT_TILE_CAP changed: the tile tables are re-allocated at the next step
     int *d_box = nullptr;               // per-body bounding boxes (comparison LBM_OPT_MOMENTS = 1 only; lazy)
     PhaseTimer timer;
+    // LBM_OPT_TRACE: timing events recorded inside the step graph after every kernel of every branch
+    int opt_trace = 0;
+    std::vector<cudaEvent_t> trace_ev;
+    std::vector<std::string> trace_label;
+    size_t trace_used = 0;
     std::map<long long, std::pair<cudaGraphExec_t, int>> graphs;   // key -> (exec, kernel nodes)
     long long launches = 0;
     size_t dev_bytes = 0;
@@ -263,6 +268,22 @@ void drop_graphs(lbm *h)
 {
     for (auto &kv : h->graphs) cudaGraphExecDestroy(kv.second.first);
     h->graphs.clear();
+}
+
+// LBM_OPT_TRACE: record a timing event on (capture) stream s; slot order = enqueue order, fixed per graph
+void trace_mark(lbm *h, cudaStream_t s, const char *label, int idx = -1)
+{
+    if (!h->opt_trace) return;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(s, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusActive) return;   // graph nodes only
+    if (h->trace_used == h->trace_ev.size()) {
+        cudaEvent_t e; cudaEventCreate(&e);
+        h->trace_ev.push_back(e); h->trace_label.emplace_back();
+    }
+    char buf[64];
+    if (idx >= 0) snprintf(buf, sizeof buf, "%s[%d]", label, idx); else snprintf(buf, sizeof buf, "%s", label);
+    h->trace_label[h->trace_used] = buf;
+    cudaEventRecordWithFlags(h->trace_ev[h->trace_used++], s, cudaEventRecordExternal);
 }
 
 void free_set(lbm *h, PrepSet &S)
@@ -633,6 +654,7 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
                                                    h->d_total);
         nk += 3;
     }
+    trace_mark(h, s, "prep.sort");
     if (pt) pt->mark(PH_BINS, s);
     k_marker_gather<<<mb, 256, 0, s>>>(mi, h->d_defs, S.tabs, g, perm, S.ms);
     ++nk;
@@ -684,6 +706,7 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
         // a4 + the whole loop in one kernel: grid-wide barriers instead of 2 N + 1 dependent launches
         K.persistent<<<h->mdfp_grid, MDFP_WARPS * 32, (size_t)MDFP_WARPS * h->mdf_wsmem, s>>>(
             ma, src, h->po, sc->cursor, &sc->gbar, mdf_iters, wsmem);
+        trace_mark(h, s, "mdf_persistent");
         CK(cudaGetLastError());
         *n_kernels += 1;
         return LBM_OK;
@@ -705,6 +728,7 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
         k_moments_active<<<h->moments_grid, 256, 0, s>>>(src, g, h->po, S.cells, &sc->n_cells, h->U);
         ++nk;
     }
+    trace_mark(h, s, "moments");
     for (int m = 0; m < mdf_iters; ++m) {
         const bool last = (m == mdf_iters - 1);
         if (pt) pt->mark(PH_INTERP, s);
@@ -714,8 +738,10 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
                 K.pairs<<<h->mdf2_grid, 64, mdf_pair_smem(h->tr, h->cg), s>>>(ma, &sc->cursor[m], last ? 1 : 0);
             else
                 K.tiles<<<h->mdf_grid, MDF_WARPS * 32, (size_t)MDF_WARPS * h->mdf_wsmem, s>>>(ma, &sc->cursor[m], last ? 1 : 0, wsmem);
+            trace_mark(h, s, "tiles", m);
             if (pt) pt->mark(PH_SPREAD, s);
             k_mdf_collect<<<LIST_GRID, 256, 0, s>>>(ma, last ? 1 : 0);
+            trace_mark(h, s, "collect", m);
             nk += 2;
             continue;
         }
@@ -843,27 +869,34 @@ int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, int mdf_
     cudaStream_t s = h->cap_stream;
     int nk = 0, rc;
     const bool split = overlap_mode(h) == 1;    // 1: bulk stream-collide beside the MDF loop; 2: one fused pass after it
+    h->trace_used = 0;
+    trace_mark(h, s, "fork");
     CK(cudaEventRecord(h->ev_fork, s));
     if (split) CK(cudaStreamWaitEvent(h->cap_bulk, h->ev_fork, 0));
     CK(cudaStreamWaitEvent(h->cap_prep, h->ev_fork, 0));
     if (split) {
         if ((rc = enqueue_lbm_pass(h, h->cap_bulk, src, dst, LBM_BULK, S.amask))) return rc;
+        trace_mark(h, h->cap_bulk, "bulk");
         ++nk;
     }
     if ((rc = enqueue_mdf(h, s, S, src, mdf_iters, &nk, nullptr))) return rc;
     if ((rc = enqueue_prep(h, h->cap_prep, N, 1, &nk, nullptr))) return rc;
+    trace_mark(h, h->cap_prep, "prep");
     if (split) CK(cudaEventRecord(h->ev_bulk, h->cap_bulk));
     CK(cudaEventRecord(h->ev_prep, h->cap_prep));
     if (split) CK(cudaStreamWaitEvent(s, h->ev_bulk, 0));
     CK(cudaStreamWaitEvent(s, h->ev_prep, 0));
     if (split) {
+        trace_mark(h, s, "join");
         if ((rc = enqueue_lbm_active(h, s, src, dst, S))) return rc;           // also advances the step counter
         ++nk;
     } else {
+        trace_mark(h, s, "join");
         if ((rc = enqueue_lbm_pass(h, s, src, dst, LBM_FUSED, S.amask))) return rc;
         k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, nullptr, 0, 4);
         nk += 2;
     }
+    trace_mark(h, s, "end");
     CK(cudaGetLastError());
     *n_kernels = nk;
     return LBM_OK;
@@ -877,7 +910,7 @@ int get_graph(lbm *h, int kind, int parity, int set, int mdf_iters, cudaGraphExe
                           ((long long)h->opt_lbm_kernel << 48) | ((long long)h->opt_interp << 52) |
                           ((long long)overlap_mode(h) << 56) | ((long long)h->opt_moments << 58) |
                           ((long long)h->opt_fused << 60) | ((long long)h->tr << 16) | ((long long)use_persistent(h) << 20) |
-                          ((long long)tile_warps(h) << 21);
+                          ((long long)tile_warps(h) << 21) | ((long long)h->opt_trace << 23);
     auto it = h->graphs.find(key);
     if (it != h->graphs.end()) { *exec = it->second.first; *n_kernels = it->second.second; return LBM_OK; }
     cudaGraph_t graph = nullptr;
@@ -1060,7 +1093,14 @@ void lbm_destroy(lbm_t *h)
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->ev_bulk) cudaEventDestroy(h->ev_bulk);
     if (h->ev_prep) cudaEventDestroy(h->ev_prep);
+    for (cudaEvent_t e : h->trace_ev) cudaEventDestroy(e);
     delete h;
+}
+
+const char *lbm_trace_label(lbm_t *h, int i)
+{
+    if (!h || i < 0 || (size_t)i >= h->trace_used) return "";
+    return h->trace_label[(size_t)i].c_str();
 }
 
 int lbm_query_layout(int nx, int ny, int nz, int *out)
@@ -1107,6 +1147,10 @@ int lbm_set_option(lbm_t *h, int key, int value)
             }
             return LBM_OK;
         case LBM_OPT_TILE_WARPS: if (value < 0 || value > 2) break; h->opt_tile_warps = value; return LBM_OK;
+        case LBM_OPT_TRACE:
+            if (value < 0 || value > 1) break;
+            if (value != h->opt_trace) { CK(cudaStreamSynchronize(h->stream)); drop_graphs(h); h->opt_trace = value; h->trace_used = 0; }
+            return LBM_OK;
         case LBM_OPT_TILE_CAP:
             if (value < 0) break;
             if (value != h->opt_tile_cap) { h->opt_tile_cap = value; h->realloc_tables = true; h->markers_stale = true; }
@@ -1144,7 +1188,16 @@ int lbm_get_info(lbm_t *h, int key, long long *value)
             *value = st;
             return LBM_OK;
         }
+        case LBM_INFO_TRACE_COUNT: *value = (long long)h->trace_used; return LBM_OK;
         default:
+            if (key >= LBM_INFO_TRACE_NS && key < LBM_INFO_TRACE_NS + (int)h->trace_used) {
+                // device time from the first trace event of the last step (the fork) to event key - LBM_INFO_TRACE_NS
+                CK(cudaStreamSynchronize(h->stream));
+                float ms = 0.f;
+                CK(cudaEventElapsedTime(&ms, h->trace_ev[0], h->trace_ev[(size_t)(key - LBM_INFO_TRACE_NS)]));
+                *value = (long long)(1e6 * (double)ms);
+                return LBM_OK;
+            }
             if (key >= LBM_INFO_PHASE_NS && key < LBM_INFO_PHASE_NS + PH_COUNT) {
                 *value = (long long)h->timer.ns[key - LBM_INFO_PHASE_NS];
                 return LBM_OK;
