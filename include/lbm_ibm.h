@@ -132,6 +132,9 @@ enum {
     LBM_INFO_TILES = 10,        /* tiles (chunks of one x block and one block of tile-rows x tile-rows source rows) in the last step */
     LBM_INFO_ACTIVE_WORDS = 11, /* 32-cell words of the active mask that hold an active cell (the cells the
                                    second stream-collide pass of the overlapped step updates)          */
+    LBM_INFO_LAYOUT = 13,       /* step layout in effect for the current markers (LBM_OPT_OVERLAP resolved: 0, 1, 2)   */
+    LBM_INFO_TILE_ROWS = 14,    /* tile edge in effect (LBM_OPT_TILE_ROWS resolved: 1, 2, 4; 0 before the first step) */
+    LBM_INFO_SORT_PASSES = 15,  /* 8-bit radix passes of the marker sort (ceil(log2(cells) / 8))                     */
     LBM_INFO_TRACE_COUNT = 12,  /* number of trace events of a step (LBM_OPT_TRACE)                  */
     LBM_INFO_TRACE_NS = 200,    /* + i: device time in ns from the fork of the last step to trace event i */
     LBM_INFO_PHASE_NS = 100     /* + phase: accumulated device time in ns under LBM_OPT_TIMING.

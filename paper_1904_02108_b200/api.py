@@ -27,6 +27,7 @@ PERSISTENT_AUTO, PERSISTENT_ON, PERSISTENT_OFF = 0, 1, 2
 INFO_MARKERS, INFO_BODIES, INFO_STEPS, INFO_LAUNCHES, INFO_ACTIVE_CELLS, INFO_DEVICE_BYTES, INFO_STATUS = range(1, 8)
 INFO_RUNS, INFO_RUN_ENTRIES, INFO_TILES, INFO_ACTIVE_WORDS = 8, 9, 10, 11
 INFO_TRACE_COUNT, INFO_TRACE_NS = 12, 200
+INFO_LAYOUT, INFO_TILE_ROWS, INFO_SORT_PASSES = 13, 14, 15
 INFO_PHASE_NS = 100
 PHASES = ["keys", "sort", "bins", "moments", "interp", "spread", "lbm", "lbm_active"]
 SPREAD_GATHER, SPREAD_ATOMIC, SPREAD_GATHER_PLAIN, SPREAD_BLOCK125 = 0, 1, 2, 3

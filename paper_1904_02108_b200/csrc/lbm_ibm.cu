@@ -1189,6 +1189,9 @@ int lbm_get_info(lbm_t *h, int key, long long *value)
             return LBM_OK;
         }
         case LBM_INFO_TRACE_COUNT: *value = (long long)h->trace_used; return LBM_OK;
+        case LBM_INFO_LAYOUT: *value = (h->nm > 0) ? overlap_mode(h) : 0; return LBM_OK;
+        case LBM_INFO_TILE_ROWS: *value = h->tr; return LBM_OK;
+        case LBM_INFO_SORT_PASSES: *value = h->sort_passes; return LBM_OK;
         default:
             if (key >= LBM_INFO_TRACE_NS && key < LBM_INFO_TRACE_NS + (int)h->trace_used) {
                 // device time from the first trace event of the last step (the fork) to event key - LBM_INFO_TRACE_NS

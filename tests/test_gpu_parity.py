@@ -153,6 +153,73 @@ def test_w1_coupled_parity_100_steps(api, orc):
     sim.close()
 
 
+@pytest.mark.parametrize("forcing", [0, 1])
+def test_thin_channel_from_rest_reaches_the_exact_poiseuille_profile(api, forcing):
+    """K9 on the GPU, from rest: a 4 x 4 x 16 channel (walls in z, R16) driven by g_x converges to the exact discrete
+    profile u_x(z) = g/(2 nu) (z + 1/2)(H - 1/2 - z) + g (16 tau^2 - 20 tau + 3) / (4 (2 tau - 1)) for both forcings.
+    Unlike "the profile is held", this fails for a missing or mis-scaled body force, a wrong wall or a wrong tau."""
+    tau, g, H = 0.8, 1e-5, 16
+    nu = (tau - 0.5) / 3.0
+    sim = api.LbmIbm(4, 4, H, tau, wall=(0, 0, 1), g=(g, 0.0, 0.0), stream=_stream())
+    sim.set_option(api.OPT_FORCING, forcing)
+    sim.step(6000, 0)                                   # e-folding time H^2 / (pi^2 nu) = 260 steps
+    sim.sync()
+    rho, u, _ = sim.read_fields(force=False)
+    z = np.arange(H, dtype=np.float64)
+    exact = g / (2 * nu) * (z + 0.5) * (H - 0.5 - z) + g * (16 * tau * tau - 20 * tau + 3) / (4 * (2 * tau - 1))
+    prof = u[0].astype(np.float64)
+    assert np.abs(prof - exact[:, None, None]).max() <= 2e-4 * exact.max()
+    assert np.abs(u[1:]).max() <= 1e-9 and abs(rho.astype(np.float64).mean() - 1.0) < 1e-6
+    sim.close()
+
+
+def test_w1_coupled_with_the_papers_shift_forcing_100_steps(api, orc):
+    """the paper's own forcing (equilibrium velocity shifted by tau G) coupled to the markers, the
+    whole of configs[0] against the oracle's forcing="shift" at north_star's tolerances."""
+    from paper_1904_02108_b200 import workloads
+    wl = workloads.get("W1")
+    sim = api.from_workload(wl, stream=_stream())
+    sim.set_option(api.OPT_FORCING, api.FORCING_SHIFT)
+    ref = orc.from_workload(wl, forcing="shift")
+    sim.step(100, wl.mdf_iters)
+    ref.step(100, wl.mdf_iters)
+    sim.sync()
+    e = _compare_fields(sim, ref)
+    _check_markers(sim, ref, orc, wl)
+    # and the two forcings do differ by more than the tolerance (SURVEY R3: 3.9e-6 in u on W1), so the option is live
+    guo = orc.from_workload(wl)
+    guo.step(100, wl.mdf_iters)
+    assert np.abs(guo.read_fields()[1] - ref.read_fields()[1]).max() > TOL_U
+    print("W1 shift-forcing errors (u, rho, G):", e)
+    sim.close()
+
+
+def test_trace_option_reports_a_timeline_and_changes_nothing(api):
+    """LBM_OPT_TRACE: event-record nodes in the step graph; the fields stay bit-identical and the labels / times
+    describe one step (fork first, end last, every MDF kernel in between)."""
+    from paper_1904_02108_b200 import workloads
+    wl = workloads.get("W1")
+    outs = []
+    for trace in (0, 1):
+        sim = api.from_workload(wl, stream=_stream())
+        sim.set_option(api.OPT_TRACE, trace)
+        sim.step(12, wl.mdf_iters)
+        sim.sync()
+        outs.append(sim.read_fields())
+        if trace:
+            tr = sim.trace()
+            labels = [l for l, _ in tr]
+            assert labels[0] == "fork" and labels[-1] == "end" and "prep" in labels and "join" in labels
+            assert sum(l.startswith("tiles[") for l in labels) == wl.mdf_iters or "mdf_persistent" in labels
+            t = dict(tr)
+            assert t["fork"] == 0.0 and 0.0 < t["join"] <= t["end"] < 50.0       # ms
+        else:
+            assert sim.trace() == []
+        sim.close()
+    for a, b in zip(*outs):
+        assert np.array_equal(a, b)
+
+
 def test_w1_atomic_variant_matches_and_gather_is_deterministic(api, orc):
     from paper_1904_02108_b200 import workloads
     wl = workloads.get("W1")
