@@ -97,8 +97,9 @@ enum {
                              markers, 2 up to 400,000, else 4), or 1, 2, 4.  Changing it rebuilds the tile
                              tables at the next step.  Results agree to rounding (summation order).        */
     LBM_OPT_PERSISTENT = 11, /* the fused MDF loop (moments + N x (tile pass, collect)) as ONE persistent kernel
-                             with grid-wide barriers instead of 2 N + 1 launches: 1 = on, 0 / 2 = off (default;
-                             measured slower on B200).  Results are bit-identical.       */
+                             with grid-wide barriers instead of 2 N + 1 launches: 1 = on, 2 = off, 0 (default) =
+                             on for marker sets of up to 20,000 markers on lattices of up to 4 Mi cells (where the
+                             chain of launches is the critical path of the step).  Results are bit-identical.   */
     LBM_OPT_TILE_CAP = 12, /* > 0: cap the number of tile footprints (default 0 = room for every tile that can
                              exist, up to 12 GB).  More tiles than the cap are dropped for that step and
                              lbm_sync reports LBM_ENOMEM; later steps that fit are complete again.  Takes
@@ -108,6 +109,11 @@ enum {
                              and alternates between interpolating one batch of 32 markers and sweeping the
                              previous one (measured comparison: more warps per SM, no faster).  Results agree
                              to rounding (each batch's sweep is flushed).                                   */
+    LBM_OPT_PIPELINE = 16, /* depth of the binning pipeline of the overlapped step (three marker sets are used in
+                             turn): 2 = the step's graph bins the second half of step n + 1 (gather, chunks, tiles,
+                             active cells, collect plan) and, in a branch of its own, the first half of step n + 2
+                             (kinematics, keys, sort); 1 = it bins all of step n + 1 in one branch; 0 (default) = 2
+                             up to 400,000 markers, else 1.  Results are bit-identical.                         */
     LBM_OPT_TRACE = 15,   /* 1 = the graph of the overlapped step also records a timing event after every kernel of
                              the MDF branch, after the bulk stream-collide and after the binning branch; after
                              lbm_sync, lbm_get_info(LBM_INFO_TRACE_NS + i) is the device time in ns from the fork

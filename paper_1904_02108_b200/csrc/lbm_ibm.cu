@@ -80,7 +80,7 @@ struct HostBody {
     bool has_kin;
 };
 
-constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driven kernels
+constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driven kernels (grid-stride loops over device-side lists)
 // Tile edge by marker count (LBM_OPT_TILE_ROWS = 0), measured on B200: single-row tiles while
 // the set is so small that larger tiles would not fill the SMs (W1, W3: 15,360 markers), two-row tiles up to a few
 // hundred thousand markers (P6, P18, W4lit), 4 x 4-row tiles beyond (W4, W5lit, W5).
@@ -119,9 +119,13 @@ struct PhaseTimer {
 
 }  // namespace
 
-// Everything the binning stage (a1-a3) produces for ONE time step.  There are two sets: while the
-// MDF loop and the stream-collide of step n use set n & 1, the side stream prepares step n + 1 in
-// the other set (the marker positions depend on time only, not on the fluid).
+// Everything the binning stage (a1-a3) produces for ONE time step.  There are three sets, used in turn: while the
+// MDF loop and the stream-collide of step n use set n % 3, two side branches of the step's graph prepare the steps to
+// come (the marker positions depend on time only, not on the fluid): the second half of the binning of step
+// n + 1 (gather, chunks, tiles, active cells, collect plan) and the first half of the binning of step n + 2
+// (kinematics, keys, sort).  The binning is a chain of ~25 small dependent kernels; split over two steps its length
+// stays below that of the MDF loop also for small marker sets, where every kernel costs its launch latency.
+constexpr int N_SETS = 3;
 struct PrepSet {
     unsigned *keys[2] = {nullptr, nullptr};   // radix ping-pong; the sorted keys end in keys[sort_passes & 1]
     int *vals[2] = {nullptr, nullptr};        // the permutation, same ping-pong
@@ -144,6 +148,7 @@ struct PrepSet {
     SetScalars *scal = nullptr;
     bool dirty = false;                       // the dense maps hold entries of a preparation
     long long step = -1;                      // time step the set is prepared for (-1: none)
+    int stage = 0;                            // how far: 1 = first half (kinematics, keys, sort), 2 = complete
     int spread = -1;                          // prep_signature() the preparation was made for
 };
 
@@ -152,8 +157,9 @@ struct lbm {
     cudaStream_t stream = nullptr;      // where work is enqueued
     cudaStream_t cap_stream = nullptr;  // capture-only streams for building graphs: the MDF chain (high priority),
     cudaStream_t cap_bulk = nullptr;    //   the bulk stream-collide (low priority),
-    cudaStream_t cap_prep = nullptr;    //   the preparation of the next step
-    cudaEvent_t ev_fork = nullptr, ev_bulk = nullptr, ev_prep = nullptr;
+    cudaStream_t cap_prep = nullptr;    //   the second half of the binning of the next step
+    cudaStream_t cap_prep2 = nullptr;   //   the first half of the binning of the step after that
+    cudaEvent_t ev_fork = nullptr, ev_bulk = nullptr, ev_prep = nullptr, ev_prep2 = nullptr;
     Geom g{};
     CollisionConst cc{};
     PlaneOffsets po{};
@@ -164,7 +170,7 @@ struct lbm {
     DevScalars *scal = nullptr;
     long long steps_done = 0;
     size_t n_mask_words = 0;
-    PrepSet set[2];
+    PrepSet set[N_SETS];
     int cur_set = 0;                    // set the next IBM step uses
     int last_set = -1;                  // set of the last completed IBM step (G, mask, marker read-out), -1: none
     bool force_valid = false;           // G + mask of last_set describe the last completed step
@@ -179,7 +185,7 @@ struct lbm {
     float *d_q[3] = {nullptr, nullptr, nullptr}, *d_v[3] = {nullptr, nullptr, nullptr}, *d_s = nullptr;
     int *d_body = nullptr;
     BodyDef *d_defs = nullptr;
-    int *d_hist = nullptr, *d_total = nullptr;
+    int *d_hist[N_SETS] = {nullptr, nullptr, nullptr}, *d_total[N_SETS] = {nullptr, nullptr, nullptr};   // radix scratch, one per marker set (two binnings run side by side)
     size_t cells_cap = 0, headbits_cap = 0;
     float4 *F = nullptr;                // tile footprints [tile][7][7][cg.ent]
     ChunkGeom cg{1, CHUNK_W + 3};
@@ -196,6 +202,7 @@ struct lbm {
 
     int opt_spread = 0, opt_forcing = 0, opt_graph = 1, opt_lbm_kernel = 0, opt_interp = 0, opt_timing = 0;
     int opt_overlap = 3, opt_moments = 0;
+    int opt_pipeline = 0;
     int opt_fused = 1, opt_tile_rows = 0, opt_persistent = 0, opt_tile_cap = 0, opt_mdf_blocks = 0, opt_tile_warps = 0;
     bool realloc_tables = false;        // LBM_OPT_TILE_CAP changed: the tile tables are re-allocated at the next step
     int *d_box = nullptr;               // per-body bounding boxes (comparison LBM_OPT_MOMENTS = 1 only; lazy)
@@ -307,7 +314,7 @@ void free_set(lbm *h, PrepSet &S)
     dfree(h, S.inv, c);
     dfree(h, S.cells, h->cells_cap);
     dfree(h, S.headbits, h->headbits_cap);
-    S.step = -1;
+    S.step = -1; S.stage = 0;
 }
 
 void free_markers_dev(lbm *h)
@@ -320,8 +327,10 @@ void free_markers_dev(lbm *h)
     h->cells_cap = 0; h->headbits_cap = 0;
     dfree(h, h->F, (size_t)h->tile_cap * (size_t)((h->tr + 3) * (h->tr + 3)) * (size_t)h->cg.ent);
     h->chunk_cap = 0; h->tile_cap = 0; h->tile_slots = 0; h->tr = 0;
-    dfree(h, h->d_hist, (size_t)RADIX * (size_t)h->sort_tiles);
-    dfree(h, h->d_total, (size_t)RADIX);
+    for (int i = 0; i < N_SETS; ++i) {
+        dfree(h, h->d_hist[i], (size_t)RADIX * (size_t)h->sort_tiles);
+        dfree(h, h->d_total[i], (size_t)RADIX);
+    }
     dfree(h, h->d_box, (size_t)6 * (size_t)h->nb_cap);
     dfree(h, h->d_defs, (size_t)h->nb_cap);
     h->nm_cap = 0; h->nb_cap = 0; h->sort_tiles = 0;
@@ -337,6 +346,14 @@ dim3 cell_grid(const Geom &g, dim3 b) { return dim3((g.nx + b.x - 1) / b.x, (g.n
 
 // the product path: fused tile pass + collect (mdf_kernels.cuh); everything else is a measured comparison
 bool fused_path(const lbm *h) { return h->opt_fused && h->opt_spread == 0 && h->opt_interp == 0; }
+
+// grid of a list-driven kernel: the lists (chunks, tiles, words, active cells) grow with the marker count, and a small
+// marker set should not pay for scheduling 1184 mostly empty blocks in every one of its ~30 dependent kernels
+int list_grid(const lbm *h)
+{
+    const long long want = (4LL * h->nm + 255) / 256;
+    return (int)std::min<long long>(LIST_GRID, std::max<long long>(h->sms, want));
+}
 
 // tile edge for the current markers and options: the comparison paths are written for 4 x 4 rows; the fused
 // path uses single-row tiles for small marker sets (enough tiles for all SMs) unless LBM_OPT_TILE_ROWS says otherwise
@@ -364,11 +381,27 @@ int tile_warps(const lbm *h)
     return h->opt_tile_warps == 2 ? 2 : 1;
 }
 
-// the whole MDF loop as one persistent kernel (small marker sets: launch latency dominates otherwise)
+// The whole MDF loop as one persistent kernel (LBM_OPT_PERSISTENT; automatic: small marker sets on small lattices).
+// With few markers every tile pass and collect costs its launch latency, and the chain of 2 N + 1 dependent launches
+// is the critical path of the step as long as the lattice-wide stream-collide beside it is shorter; on larger
+// lattices the stream-collide is the critical path and a persistent kernel only takes SM resources from it
+// (measured on B200: W3 0.107 against 0.140 ms per step, P1 0.251 against 0.241, P6 0.338 against 0.322).
+constexpr long long PERSISTENT_MAX_CELLS = 4LL << 20;
 bool use_persistent(const lbm *h)
 {
     if (!fused_path(h) || h->opt_moments != 0 || h->opt_timing) return false;
-    return h->opt_persistent == 1;
+    if (h->opt_persistent) return h->opt_persistent == 1;
+    return h->nm <= TR1_MAX_MARKERS && h->g.cells <= PERSISTENT_MAX_CELLS;
+}
+
+// Depth of the binning pipeline (LBM_OPT_PIPELINE): 2 = the binning of a step is spread over the two steps before it
+// (small marker sets: the chain of ~25 dependent launches is longer than the MDF loop); 1 = all of it during the
+// step before (large sets: the binning is short beside the MDF loop and a second branch only adds contention)
+constexpr int PIPE2_MAX_MARKERS = 400000;
+int pipeline_depth(const lbm *h)
+{
+    if (h->opt_pipeline) return h->opt_pipeline;
+    return h->nm <= PIPE2_MAX_MARKERS ? 2 : 1;
 }
 
 // the options a preparation depends on (which tables it builds)
@@ -411,7 +444,7 @@ int ensure_comparison_arrays(lbm *h)
 // ---- remove what the preparations registered in the dense maps (outside any graph) -------------
 int flush_set(lbm *h, PrepSet &S)
 {
-    S.step = -1;
+    S.step = -1; S.stage = 0;
     if (!S.dirty) return LBM_OK;
     k_clear_prev<<<LIST_GRID, 256, 0, h->stream>>>(sorted_keys(h, S), &S.scal->n_prev, S.bin_first, S.amask, S.words,
                                                     &S.scal->n_words, S.chunk_of, S.ct.slot, &S.scal->n_chunks,
@@ -563,7 +596,7 @@ int upload_markers(lbm *h)
         // launch geometry of the fused tile pass and of the persistent MDF kernel for (tr, cg)
         h->mdf_wsmem = mdf_warp_smem(tr, h->cg);
         if ((rc = mdf_launch_geometry(h))) return rc;
-        if ((rc = dmalloc(h, &h->d_total, (size_t)RADIX))) return rc;
+        for (int i = 0; i < N_SETS; ++i) if ((rc = dmalloc(h, &h->d_total[i], (size_t)RADIX))) return rc;
         if ((rc = dmalloc(h, &h->d_defs, (size_t)nb))) return rc;
         for (PrepSet &S : h->set) if ((rc = dmalloc(h, &S.tabs, (size_t)nb))) return rc;
         h->nm_cap = n; h->nb_cap = nb;
@@ -575,8 +608,10 @@ int upload_markers(lbm *h)
     if (ipw > 2048) ipw = 2048;
     const int tiles = n > 0 ? (n + ipw - 1) / ipw : 0;
     if (tiles > h->sort_tiles) {
-        dfree(h, h->d_hist, (size_t)RADIX * (size_t)h->sort_tiles);
-        if ((rc = dmalloc(h, &h->d_hist, (size_t)RADIX * (size_t)tiles))) return rc;
+        for (int i = 0; i < N_SETS; ++i) {
+            dfree(h, h->d_hist[i], (size_t)RADIX * (size_t)h->sort_tiles);
+            if ((rc = dmalloc(h, &h->d_hist[i], (size_t)RADIX * (size_t)tiles))) return rc;
+        }
     }
     h->sort_ipw = ipw; h->sort_tiles = tiles;
     int bits = 1;
@@ -620,8 +655,10 @@ int upload_markers(lbm *h)
 
 // ---- launch helpers (plain launches on stream s; also what graph capture records) --------------
 
-// a1-a3 for the time step (device step counter + step_offset) into marker set S.
-int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_kernels, PhaseTimer *pt)
+// a1-a3 for the time step (device step counter + step_offset) into marker set S.  parts: bit 0 = first half
+// (kinematics tables, keys, sort), bit 1 = second half (gather, chunks, tiles, active cells, collect plan).
+enum { PREP_SORT = 1, PREP_BINS = 2, PREP_ALL = 3 };
+int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_kernels, PhaseTimer *pt, int parts = PREP_ALL)
 {
     const Geom &g = h->g;
     const int n = h->nm;
@@ -631,9 +668,11 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
     int *perm = S.vals[h->sort_passes & 1];
     MarkerIn mi{h->d_q[0], h->d_q[1], h->d_q[2], h->d_v[0], h->d_v[1], h->d_v[2], h->d_s, h->d_body, n};
     int nk = 0;
+    const int lg = list_grid(h);
 
+    if (parts & PREP_SORT) {
     if (pt) pt->mark(PH_KEYS, s);
-    k_clear_prev<<<LIST_GRID, 256, 0, s>>>(skey, &sc->n_prev, S.bin_first, S.amask, S.words, &sc->n_words, S.chunk_of,
+    k_clear_prev<<<lg, 256, 0, s>>>(skey, &sc->n_prev, S.bin_first, S.amask, S.words, &sc->n_words, S.chunk_of,
                                            S.ct.slot, &sc->n_chunks, h->chunk_cap, S.tt.mask, S.tt.slot, &sc->n_tiles, h->tile_cap,
                                            S.ovf_slot, &sc->n_ovf, OVF_CAP, (int)h->tile_slots);
     const int nb = (int)h->bodies.size();
@@ -642,19 +681,28 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
     k_marker_keys<<<mb, 256, 0, s>>>(mi, h->d_defs, S.tabs, g, S.keys[0], &h->scal->status);
     nk += 3;
     if (pt) pt->mark(PH_SORT, s);
-    const int sb = (h->sort_tiles + SORT_WARPS - 1) / SORT_WARPS;
-    for (int p = 0; p < h->sort_passes; ++p) {
-        const unsigned *kin = S.keys[p & 1];
-        unsigned *kout = S.keys[(p + 1) & 1];
-        const int *vin = p == 0 ? nullptr : S.vals[p & 1];
-        int *vout = S.vals[(p + 1) & 1];
-        k_radix_hist<<<sb, SORT_BLOCK, 0, s>>>(kin, n, h->sort_ipw, h->sort_tiles, 8 * p, h->d_hist);
-        k_radix_scan<<<RADIX, SORT_BLOCK, 0, s>>>(h->d_hist, h->sort_tiles, h->d_total);
-        k_radix_scatter<<<sb, SORT_BLOCK, 0, s>>>(kin, vin, kout, vout, n, h->sort_ipw, h->sort_tiles, 8 * p, h->d_hist,
-                                                   h->d_total);
-        nk += 3;
+    if (n <= SORT_SMALL_MAX) {
+        // small marker sets: every pass in one single-block kernel (same result, 3 launches instead of 3 per pass)
+        k_radix_sort_small<<<1, SORT_SMALL_BLOCK, 0, s>>>(S.keys[0], S.keys[1], S.vals[0], S.vals[1], n, h->sort_passes);
+        ++nk;
+    } else {
+        const int sb = (h->sort_tiles + SORT_WARPS - 1) / SORT_WARPS;
+        const int si = (int)(&S - h->set);
+        int *hist = h->d_hist[si], *total = h->d_total[si];
+        for (int p = 0; p < h->sort_passes; ++p) {
+            const unsigned *kin = S.keys[p & 1];
+            unsigned *kout = S.keys[(p + 1) & 1];
+            const int *vin = p == 0 ? nullptr : S.vals[p & 1];
+            int *vout = S.vals[(p + 1) & 1];
+            k_radix_hist<<<sb, SORT_BLOCK, 0, s>>>(kin, n, h->sort_ipw, h->sort_tiles, 8 * p, hist);
+            k_radix_scan<<<RADIX, SORT_BLOCK, 0, s>>>(hist, h->sort_tiles, total);
+            k_radix_scatter<<<sb, SORT_BLOCK, 0, s>>>(kin, vin, kout, vout, n, h->sort_ipw, h->sort_tiles, 8 * p, hist, total);
+            nk += 3;
+        }
     }
     trace_mark(h, s, "prep.sort");
+    }
+    if (!(parts & PREP_BINS)) { CK(cudaGetLastError()); *n_kernels += nk; return LBM_OK; }
     if (pt) pt->mark(PH_BINS, s);
     k_marker_gather<<<mb, 256, 0, s>>>(mi, h->d_defs, S.tabs, g, perm, S.ms);
     ++nk;
@@ -663,24 +711,24 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
         k_chunk_heads<<<(n + 32 + 255) / 256, 256, 0, s>>>(skey, n, g, h->cg, S.headbits);
         k_chunks<<<mb, 256, 0, s>>>(skey, n, g, h->cg, S.headbits, S.ct, h->chunk_cap, &sc->n_chunks, &sc->n_entries,
                                     S.chunk_of, &h->scal->status);
-        k_chunk_publish<<<LIST_GRID, 256, 0, s>>>(g, h->cg, S.ct, &sc->n_chunks, h->chunk_cap, S.chunk_of, S.amask);
-        k_tiles<<<LIST_GRID, 256, 0, s>>>(g, h->cg, h->tg, S.ct, &sc->n_chunks, h->chunk_cap, S.chunk_of, S.tt, h->tile_cap,
+        k_chunk_publish<<<lg, 256, 0, s>>>(g, h->cg, S.ct, &sc->n_chunks, h->chunk_cap, S.chunk_of, S.amask);
+        k_tiles<<<lg, 256, 0, s>>>(g, h->cg, h->tg, S.ct, &sc->n_chunks, h->chunk_cap, S.chunk_of, S.tt, h->tile_cap,
                                           &sc->n_tiles, S.ovf_slot, OVF_CAP, &sc->n_ovf, &h->scal->status);
-        k_tile_fill<<<LIST_GRID, 256, 0, s>>>(g, h->cg, h->tg, S.ct, &sc->n_chunks, h->chunk_cap, S.tt);
-        k_tile_count<<<LIST_GRID, 256, 0, s>>>(S.tt, h->tr * h->tr, &sc->n_tiles, h->tile_cap, sc->bucket);
-        k_tile_place<<<LIST_GRID, 256, 0, s>>>(S.tt, h->tr * h->tr, &sc->n_tiles, h->tile_cap, sc->bucket, S.tile_order);
+        k_tile_fill<<<lg, 256, 0, s>>>(g, h->cg, h->tg, S.ct, &sc->n_chunks, h->chunk_cap, S.tt);
+        k_tile_count<<<lg, 256, 0, s>>>(S.tt, h->tr * h->tr, &sc->n_tiles, h->tile_cap, sc->bucket);
+        k_tile_place<<<lg, 256, 0, s>>>(S.tt, h->tr * h->tr, &sc->n_tiles, h->tile_cap, sc->bucket, S.tile_order);
         nk += 7;
     } else {
         k_bins<<<mb, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask);
         ++nk;
     }
-    k_compact_words<<<LIST_GRID, 256, 0, s>>>(S.amask, (int)h->n_mask_words, S.words, &sc->n_words);
-    k_active_cells<<<LIST_GRID, 256, 0, s>>>(g, S.amask, S.words, &sc->n_words, S.cells, &sc->n_cells);
+    k_compact_words<<<(int)std::min<size_t>(LIST_GRID, (h->n_mask_words + 255) / 256), 256, 0, s>>>(S.amask, (int)h->n_mask_words, S.words, &sc->n_words);
+    k_active_cells<<<lg, 256, 0, s>>>(g, S.amask, S.words, &sc->n_words, S.cells, &sc->n_cells);
     if (h->opt_spread == 0) {
         // collect plan: which footprint elements every active cell adds up, and where the tile pass puts them
         const int elems = (h->tr + 3) * (h->tr + 3) * h->cg.ent;
-        k_fill_tiles<<<LIST_GRID, 256, 0, s>>>(S.fdst, &sc->n_tiles, h->tile_cap, elems);
-        mdf_kernels(h).plan<<<LIST_GRID, 256, 0, s>>>(mdf_args(h, S));
+        k_fill_tiles<<<lg, 256, 0, s>>>(S.fdst, &sc->n_tiles, h->tile_cap, elems);
+        mdf_kernels(h).plan<<<lg, 256, 0, s>>>(mdf_args(h, S));
         nk += 2;
     }
     k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, &sc->n_prev, n, 2);
@@ -699,6 +747,7 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
     const unsigned *skey = sorted_keys(h, S);
     int nk = 0;
     const bool fused = fused_path(h);
+    const int lg = list_grid(h);
     const MdfKernels K = mdf_kernels(h);
     const MdfArgs ma = mdf_args(h, S);
     const int wsmem = (int)h->mdf_wsmem;
@@ -740,7 +789,7 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
                 K.tiles<<<h->mdf_grid, MDF_WARPS * 32, (size_t)MDF_WARPS * h->mdf_wsmem, s>>>(ma, &sc->cursor[m], last ? 1 : 0, wsmem);
             trace_mark(h, s, "tiles", m);
             if (pt) pt->mark(PH_SPREAD, s);
-            k_mdf_collect<<<LIST_GRID, 256, 0, s>>>(ma, last ? 1 : 0);
+            k_mdf_collect<<<lg, 256, 0, s>>>(ma, last ? 1 : 0);
             trace_mark(h, s, "collect", m);
             nk += 2;
             continue;
@@ -758,19 +807,19 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
             k_spread_tiles<<<h->rows_grid, TILE_WARPS * 32, spread_tiles_smem(h->cg), s>>>(
                 h->cg, S.tt.rec, S.tt.slot, S.tt.mask, &sc->n_tiles, h->tile_cap, &sc->cursor[m], S.tile_order, S.ms.wx,
                 S.ms.wyz, last ? S.ms.du : S.ms.sg, S.fdst, h->F, (int)spread_warp_smem(h->cg));
-            k_mdf_collect<<<LIST_GRID, 256, 0, s>>>(ma, last ? 1 : 0);
+            k_mdf_collect<<<lg, 256, 0, s>>>(ma, last ? 1 : 0);
             nk += 2;
         } else if (h->opt_spread == 2) {
             if (last)
-                k_spread_gather<true><<<LIST_GRID, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask, S.words, &sc->n_words,
+                k_spread_gather<true><<<lg, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask, S.words, &sc->n_words,
                                                                  S.ms.fs, S.ms.du, h->G);
             else
-                k_spread_gather<false><<<LIST_GRID, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask, S.words, &sc->n_words,
+                k_spread_gather<false><<<lg, 256, 0, s>>>(skey, n, g, S.bin_first, S.amask, S.words, &sc->n_words,
                                                                   S.ms.fs, S.ms.sg, h->U);
             ++nk;
         } else {
             // global atomics: thread per marker (1) or the paper's block of 5^3 threads per marker (3)
-            if (last) { k_zero_active<<<LIST_GRID, 256, 0, s>>>(g, S.amask, S.words, &sc->n_words, h->G); ++nk; }
+            if (last) { k_zero_active<<<lg, 256, 0, s>>>(g, S.amask, S.words, &sc->n_words, h->G); ++nk; }
             const float4 *v = last ? S.ms.du : S.ms.sg;
             float4 *field = last ? h->G : h->U;
             if (h->opt_spread == 3) k_spread_block125<<<n, 125, 0, s>>>(skey, n, g, S.ms.fs, v, field);
@@ -857,12 +906,15 @@ int enqueue_step_serial(lbm *h, cudaStream_t s, int parity, PrepSet *S, bool pre
     return LBM_OK;
 }
 
-// ---- one time step as three concurrent branches (captured into a graph) --------------------------
+// ---- one time step as concurrent branches (captured into a graph) ------------------------------------
 //   main (high priority): moments + MDF loop on set S          -> G
-//   bulk (low priority) : stream-collide of every cell outside S's active mask (needs no G)
-//   prep                : a1-a3 of the NEXT step into the other set (depends on time only)
-//   join, then the stream-collide of the active cells with G, then step counter + 1.
-int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, int mdf_iters, int *n_kernels)
+//   bulk (low priority) : stream-collide of every cell outside S's active mask (needs no G); layout 1 only
+//   prep                : binning of step n + 1 into set N: its second half if the first was done during step n - 1
+//                         (n_has_sort), else all of it
+//   prep2               : first half of the binning of step n + 2 into set N2 (pipeline depth 2 only, N2 != NULL)
+//   join, then the stream-collide of the active cells with G (layout 2: of all cells), then step counter + 1.
+int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, PrepSet *N2, bool n_has_sort, int mdf_iters,
+                            int *n_kernels)
 {
     const float *src = h->f[parity];
     float *dst = h->f[parity ^ 1];
@@ -874,18 +926,25 @@ int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, int mdf_
     CK(cudaEventRecord(h->ev_fork, s));
     if (split) CK(cudaStreamWaitEvent(h->cap_bulk, h->ev_fork, 0));
     CK(cudaStreamWaitEvent(h->cap_prep, h->ev_fork, 0));
+    if (N2) CK(cudaStreamWaitEvent(h->cap_prep2, h->ev_fork, 0));
     if (split) {
         if ((rc = enqueue_lbm_pass(h, h->cap_bulk, src, dst, LBM_BULK, S.amask))) return rc;
         trace_mark(h, h->cap_bulk, "bulk");
         ++nk;
     }
     if ((rc = enqueue_mdf(h, s, S, src, mdf_iters, &nk, nullptr))) return rc;
-    if ((rc = enqueue_prep(h, h->cap_prep, N, 1, &nk, nullptr))) return rc;
+    if ((rc = enqueue_prep(h, h->cap_prep, N, 1, &nk, nullptr, n_has_sort ? PREP_BINS : PREP_ALL))) return rc;
     trace_mark(h, h->cap_prep, "prep");
+    if (N2) {
+        if ((rc = enqueue_prep(h, h->cap_prep2, *N2, 2, &nk, nullptr, PREP_SORT))) return rc;
+        trace_mark(h, h->cap_prep2, "prep2");
+    }
     if (split) CK(cudaEventRecord(h->ev_bulk, h->cap_bulk));
     CK(cudaEventRecord(h->ev_prep, h->cap_prep));
+    if (N2) CK(cudaEventRecord(h->ev_prep2, h->cap_prep2));
     if (split) CK(cudaStreamWaitEvent(s, h->ev_bulk, 0));
     CK(cudaStreamWaitEvent(s, h->ev_prep, 0));
+    if (N2) CK(cudaStreamWaitEvent(s, h->ev_prep2, 0));
     if (split) {
         trace_mark(h, s, "join");
         if ((rc = enqueue_lbm_active(h, s, src, dst, S))) return rc;           // also advances the step counter
@@ -903,20 +962,23 @@ int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, int mdf_
 }
 
 // kind: 0 = pure LBM, 1 = serial IBM step that prepares its own set, 2 = overlapped IBM step
-int get_graph(lbm *h, int kind, int parity, int set, int mdf_iters, cudaGraphExec_t *exec, int *n_kernels)
+// pipe: for kind 2, bit 0 = the next step's set already holds its sorted keys, bit 1 = pipeline depth 2
+int get_graph(lbm *h, int kind, int parity, int set, int mdf_iters, cudaGraphExec_t *exec, int *n_kernels, int pipe = 0)
 {
     const long long key = ((long long)mdf_iters << 8) | ((long long)kind << 4) | (set << 1) | parity |
                           ((long long)h->opt_spread << 40) | ((long long)h->opt_forcing << 44) |
                           ((long long)h->opt_lbm_kernel << 48) | ((long long)h->opt_interp << 52) |
                           ((long long)overlap_mode(h) << 56) | ((long long)h->opt_moments << 58) |
                           ((long long)h->opt_fused << 60) | ((long long)h->tr << 16) | ((long long)use_persistent(h) << 20) |
-                          ((long long)tile_warps(h) << 21) | ((long long)h->opt_trace << 23);
+                          ((long long)tile_warps(h) << 21) | ((long long)h->opt_trace << 23) | ((long long)pipe << 24);
     auto it = h->graphs.find(key);
     if (it != h->graphs.end()) { *exec = it->second.first; *n_kernels = it->second.second; return LBM_OK; }
     cudaGraph_t graph = nullptr;
     CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
     int nk = 0, rc;
-    if (kind == 2) rc = enqueue_step_overlapped(h, parity, h->set[set], h->set[set ^ 1], mdf_iters, &nk);
+    if (kind == 2)
+        rc = enqueue_step_overlapped(h, parity, h->set[set], h->set[(set + 1) % N_SETS],
+                                     (pipe & 2) ? &h->set[(set + 2) % N_SETS] : nullptr, (pipe & 1) != 0, mdf_iters, &nk);
     else rc = enqueue_step_serial(h, h->cap_stream, parity, kind ? &h->set[set] : nullptr, true, mdf_iters, &nk);
     cudaError_t e = cudaStreamEndCapture(h->cap_stream, &graph);
     if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
@@ -1027,10 +1089,12 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
         cudaDeviceGetStreamPriorityRange(&lo, &hi);
         bool ok = cudaStreamCreateWithPriority(&h->cap_stream, cudaStreamNonBlocking, hi) == cudaSuccess;
         ok &= cudaStreamCreateWithPriority(&h->cap_prep, cudaStreamNonBlocking, hi) == cudaSuccess;
+        ok &= cudaStreamCreateWithPriority(&h->cap_prep2, cudaStreamNonBlocking, hi) == cudaSuccess;
         ok &= cudaStreamCreateWithPriority(&h->cap_bulk, cudaStreamNonBlocking, lo) == cudaSuccess;
         ok &= cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) == cudaSuccess;
         ok &= cudaEventCreateWithFlags(&h->ev_bulk, cudaEventDisableTiming) == cudaSuccess;
         ok &= cudaEventCreateWithFlags(&h->ev_prep, cudaEventDisableTiming) == cudaSuccess;
+        ok &= cudaEventCreateWithFlags(&h->ev_prep2, cudaEventDisableTiming) == cudaSuccess;
         if (!ok) { fail(LBM_ECUDA, "%s", cudaGetErrorString(cudaGetLastError())); return bail("streams"); }
     }
     h->po = plane_offsets(h->g);
@@ -1090,9 +1154,11 @@ void lbm_destroy(lbm_t *h)
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     if (h->cap_bulk) cudaStreamDestroy(h->cap_bulk);
     if (h->cap_prep) cudaStreamDestroy(h->cap_prep);
+    if (h->cap_prep2) cudaStreamDestroy(h->cap_prep2);
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->ev_bulk) cudaEventDestroy(h->ev_bulk);
     if (h->ev_prep) cudaEventDestroy(h->ev_prep);
+    if (h->ev_prep2) cudaEventDestroy(h->ev_prep2);
     for (cudaEvent_t e : h->trace_ev) cudaEventDestroy(e);
     delete h;
 }
@@ -1147,6 +1213,7 @@ int lbm_set_option(lbm_t *h, int key, int value)
             }
             return LBM_OK;
         case LBM_OPT_TILE_WARPS: if (value < 0 || value > 2) break; h->opt_tile_warps = value; return LBM_OK;
+        case LBM_OPT_PIPELINE: if (value < 0 || value > 2) break; h->opt_pipeline = value; return LBM_OK;
         case LBM_OPT_TRACE:
             if (value < 0 || value > 1) break;
             if (value != h->opt_trace) { CK(cudaStreamSynchronize(h->stream)); drop_graphs(h); h->opt_trace = value; h->trace_used = 0; }
@@ -1347,7 +1414,7 @@ int ibm_update_kinematics(lbm_t *h, int first_body, int count, const double *ome
     std::copy(nb.begin(), nb.end(), h->bodies.begin() + first_body);
     if (moved || h->markers_stale) { h->markers_stale = true; return LBM_OK; }
     // a set prepared ahead for the next step used the old table
-    if (changed) for (PrepSet &S : h->set) if (S.step >= h->steps_done) S.step = -1;
+    if (changed) for (PrepSet &S : h->set) if (S.step >= h->steps_done) { S.step = -1; S.stage = 0; }
     // centres unchanged: only the small per-body table changes; graphs and marker arrays stay valid
     for (int b = 0; b < count; ++b) {
         const HostBody &B = h->bodies[(size_t)(first_body + b)];
@@ -1393,19 +1460,28 @@ int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
         cudaGraphExec_t ex = nullptr;
         PrepSet *S = ibm ? &h->set[h->cur_set] : nullptr;
         if (overlapped) {
-            if (S->step != h->steps_done || S->spread != prep_signature(h)) {
-                // first step of a run (or the kinematics changed): prepare this step's set in line
+            const int sig = prep_signature(h);
+            const int depth2 = pipeline_depth(h) == 2;
+            if (S->step != h->steps_done || S->spread != sig || S->stage != 2) {
+                // first step of a run (or the kinematics changed): bin this step's markers in line -- all of it, or the
+                // second half if the set already holds this step's sorted keys
+                const bool half = S->step == h->steps_done && S->spread == sig && S->stage == 1;
                 int np = 0;
-                if ((rc = enqueue_prep(h, h->stream, *S, 0, &np, nullptr))) return rc;
+                if ((rc = enqueue_prep(h, h->stream, *S, 0, &np, nullptr, half ? PREP_BINS : PREP_ALL))) return rc;
                 h->launches += np;
-                S->step = h->steps_done; S->spread = prep_signature(h); S->dirty = true;
+                S->step = h->steps_done; S->spread = sig; S->stage = 2; S->dirty = true;
             }
-            if ((rc = get_graph(h, 2, h->cur, h->cur_set, mdf_iters, &ex, &nk))) return rc;
+            PrepSet &N = h->set[(h->cur_set + 1) % N_SETS];
+            const bool n_has_sort = N.step == h->steps_done + 1 && N.spread == sig && N.stage == 1;
+            if ((rc = get_graph(h, 2, h->cur, h->cur_set, mdf_iters, &ex, &nk, (n_has_sort ? 1 : 0) | (depth2 ? 2 : 0)))) return rc;
             CK(cudaGraphLaunch(ex, h->stream));
-            PrepSet &N = h->set[h->cur_set ^ 1];
-            N.step = h->steps_done + 1; N.spread = prep_signature(h); N.dirty = true;
+            N.step = h->steps_done + 1; N.spread = sig; N.stage = 2; N.dirty = true;
+            if (depth2) {
+                PrepSet &N2 = h->set[(h->cur_set + 2) % N_SETS];
+                N2.step = h->steps_done + 2; N2.spread = sig; N2.stage = 1; N2.dirty = true;
+            }
             h->last_set = h->cur_set;
-            h->cur_set ^= 1;
+            h->cur_set = (h->cur_set + 1) % N_SETS;
         } else {
             if (h->opt_timing) {
                 if ((rc = enqueue_step_serial(h, h->stream, h->cur, S, true, mdf_iters, &nk, &h->timer))) return rc;
@@ -1417,7 +1493,7 @@ int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
             } else {
                 if ((rc = enqueue_step_serial(h, h->stream, h->cur, S, true, mdf_iters, &nk))) return rc;
             }
-            if (S) { S->step = h->steps_done; S->spread = prep_signature(h); S->dirty = true; h->last_set = h->cur_set; }
+            if (S) { S->step = h->steps_done; S->spread = prep_signature(h); S->stage = 2; S->dirty = true; h->last_set = h->cur_set; }
         }
         h->launches += nk;
         h->cur ^= 1;

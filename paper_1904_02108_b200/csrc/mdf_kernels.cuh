@@ -584,11 +584,12 @@ k_collect_plan(const __grid_constant__ MdfArgs a)
     constexpr int TF = TR + 3;
     const Geom &g = a.g;
     const int lane = threadIdx.x & 31;
+    const int sub = lane & 3, cl = lane >> 2;        // four lanes per cell: lane `sub` takes the z candidate iz = sub
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     const int stride = gridDim.x * blockDim.x;
     const int nc = *a.n_cells;
-    for (int k0 = tid - lane; k0 < nc; k0 += stride) {
-        const int k = k0 + lane;
+    for (int c0 = (tid - lane) >> 2; c0 < nc; c0 += stride >> 2) {
+        const int k = c0 + cl;
         AxisCandT<MAXCX> ax;
         AxisCandT<MAXCYZ> ay, az;
         ax.n = ay.n = az.n = 0;
@@ -601,24 +602,30 @@ k_collect_plan(const __grid_constant__ MdfArgs a)
             axis_candidates_t<false, TR, MAXCYZ>(y, g.ny, g.wally, 0, ay);
             axis_candidates_t<false, TR, MAXCYZ>(z, g.nz, g.wallz, 0, az);
         }
+        // this lane's z candidate (none when sub >= az.n); selected without dynamic indexing
+        int zt = 0, zf = 0;
+        bool zok = false;
+#pragma unroll
+        for (int iz = 0; iz < MAXCYZ; ++iz) if (iz == sub && iz < az.n) { zt = az.t[iz]; zf = az.f[iz]; zok = true; }
         auto for_each = [&](auto &&f) {
+            if (!zok) return;
 #pragma unroll
-            for (int iz = 0; iz < MAXCYZ; ++iz)
+            for (int iy = 0; iy < MAXCYZ; ++iy)
 #pragma unroll
-                for (int iy = 0; iy < MAXCYZ; ++iy)
-#pragma unroll
-                    for (int ix = 0; ix < MAXCX; ++ix) {
-                        if (iz >= az.n || iy >= ay.n || ix >= ax.n) continue;
-                        const int ts = tile_slot_of(ax.t[ix], ay.t[iy], az.t[iz], a.cg, a.tg);
-                        const unsigned m = __ldg(a.tile_mask + ts);
-                        if (!((m >> ax.f[ix]) & (m >> (14 + ay.f[iy])) & (m >> (21 + az.f[iz])) & 1u)) continue;
-                        const int id = __ldg(a.tile_id + ts);
-                        if (id < 0 || id >= a.tile_cap) continue;
-                        f(((size_t)id * (TF * TF) + ay.f[iy] * TF + az.f[iz]) * a.cg.ent + ax.f[ix]);
-                    }
+                for (int ix = 0; ix < MAXCX; ++ix) {
+                    if (iy >= ay.n || ix >= ax.n) continue;
+                    const int ts = tile_slot_of(ax.t[ix], ay.t[iy], zt, a.cg, a.tg);
+                    const unsigned m = __ldg(a.tile_mask + ts);
+                    if (!((m >> ax.f[ix]) & (m >> (14 + ay.f[iy])) & (m >> (21 + zf)) & 1u)) continue;
+                    const int id = __ldg(a.tile_id + ts);
+                    if (id < 0 || id >= a.tile_cap) continue;
+                    f(((size_t)id * (TF * TF) + ay.f[iy] * TF + zf) * a.cg.ent + ax.f[ix]);
+                }
         };
         int cnt = 0;
         for_each([&](size_t) { ++cnt; });
+        // lanes in order = cells in order, z candidates ascending inside a cell: the inclusive scan over the warp
+        // lays the runs out back to back with their elements in (z, y, x) order
         int incl = cnt;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -629,11 +636,10 @@ k_collect_plan(const __grid_constant__ MdfArgs a)
         int base = 0;
         if (lane == 31 && total) base = atomicAdd(a.n_felem, total);
         base = __shfl_sync(0xffffffffu, base, 31);
-        if (k < nc) {
-            int o = base + incl - cnt;
-            a.cell_run[k] = make_int2(o, cnt);
-            for_each([&](size_t el) { a.fdst[el] = o++; });
-        }
+        int o = base + incl - cnt;
+        const int run_len = __shfl_sync(0xffffffffu, incl, lane | 3) - (incl - cnt) ;      // sub == 0: elements of the cell
+        if (k < nc && sub == 0) a.cell_run[k] = make_int2(o, run_len);
+        for_each([&](size_t el) { a.fdst[el] = o++; });
     }
 }
 

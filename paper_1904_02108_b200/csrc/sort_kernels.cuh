@@ -124,4 +124,80 @@ k_radix_scatter(const unsigned *__restrict__ keys_in, const int *__restrict__ va
     }
 }
 
+// Small marker sets: all passes in ONE kernel of ONE block (32 warps; warp w owns the w-th contiguous stretch of the
+// array).  Per pass: per-warp digit histograms in shared memory, one thread per digit turns them into the warps'
+// start offsets (digit-major, warp-minor: the same order as the three-kernel pass), the warps scatter their items
+// 32 at a time with the same __match_any_sync ranking; block barriers order the passes (one block: no grid-wide
+// synchronisation is needed).  Same result as the three-kernel passes, nine launches fewer for a 24-bit key.
+constexpr int SORT_SMALL_BLOCK = 1024;
+constexpr int SORT_SMALL_WARPS = SORT_SMALL_BLOCK / 32;
+constexpr int SORT_SMALL_MAX = 32768;       // markers up to which the single-block sort is used
+
+__global__ void __launch_bounds__(SORT_SMALL_BLOCK, 1)
+k_radix_sort_small(unsigned *keys0, unsigned *keys1, int *vals0, int *vals1, int n, int npasses)
+{
+    __shared__ int cnt[SORT_SMALL_WARPS][RADIX];
+    __shared__ int dsum[RADIX];
+    __shared__ int wsum[RADIX / 32];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int per = ((n + SORT_SMALL_WARPS - 1) / SORT_SMALL_WARPS + 31) & ~31;
+    const int beg = min(n, wib * per), end = min(n, beg + per);
+    const unsigned lt = (1u << lane) - 1u;
+    for (int p = 0; p < npasses; ++p) {
+        // plain pointers: a pass reads what the pass before wrote (no read-only data path)
+        const unsigned *kin = (p & 1) ? keys1 : keys0;
+        unsigned *kout = (p & 1) ? keys0 : keys1;
+        const int *vin = p == 0 ? nullptr : ((p & 1) ? vals1 : vals0);
+        int *vout = (p & 1) ? vals0 : vals1;
+        const int shift = 8 * p;
+        for (int d = lane; d < RADIX; d += 32) cnt[wib][d] = 0;
+        __syncwarp();
+        for (int i = beg + lane; i < end; i += 32) atomicAdd(&cnt[wib][(kin[i] >> shift) & (RADIX - 1)], 1);
+        __syncthreads();
+        // thread d < 256: exclusive prefix of digit d over the warps, digit total
+        if (threadIdx.x < RADIX) {
+            int run = 0;
+#pragma unroll 8
+            for (int w = 0; w < SORT_SMALL_WARPS; ++w) { const int v = cnt[w][threadIdx.x]; cnt[w][threadIdx.x] = run; run += v; }
+            int incl = run;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int v = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += v;
+            }
+            if (lane == 31) wsum[wib] = incl;
+            dsum[threadIdx.x] = incl - run;          // exclusive inside the warp of 32 digits
+        }
+        __syncthreads();
+        if (threadIdx.x < RADIX) {
+            int base = dsum[threadIdx.x];
+            for (int w = 0; w < wib; ++w) base += wsum[w];
+#pragma unroll 8
+            for (int w = 0; w < SORT_SMALL_WARPS; ++w) cnt[w][threadIdx.x] += base;
+        }
+        __syncthreads();
+        for (int r = beg; r < end; r += 32) {
+            const int i = r + lane;
+            const bool valid = i < end;
+            const unsigned key = valid ? kin[i] : 0u;
+            const int val = valid ? (vin ? vin[i] : i) : 0;
+            const unsigned d = valid ? ((key >> shift) & (RADIX - 1)) : 0xffffffffu;
+            const unsigned peers = __match_any_sync(0xffffffffu, d);
+            const int leader = __ffs(peers) - 1;
+            int old = 0;
+            if (valid && lane == leader) old = cnt[wib][d];
+            __syncwarp();
+            if (valid && lane == leader) cnt[wib][d] = old + __popc(peers);
+            old = __shfl_sync(0xffffffffu, old, leader);
+            __syncwarp();
+            if (valid) {
+                const int pos = old + __popc(peers & lt);
+                kout[pos] = key;
+                vout[pos] = val;
+            }
+        }
+        __syncthreads();                             // the pass's output is complete (and visible) for the whole block
+    }
+}
+
 }  // namespace lbmk

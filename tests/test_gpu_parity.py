@@ -311,6 +311,8 @@ def _variants(api):
         ("tile_rows_4_warp_pairs", {api.OPT_TILE_ROWS: 4, api.OPT_PERSISTENT: api.PERSISTENT_OFF, api.OPT_TILE_WARPS: 2}),
         ("tile_rows_2_warp_pairs", {api.OPT_TILE_ROWS: 2, api.OPT_PERSISTENT: api.PERSISTENT_OFF, api.OPT_TILE_WARPS: 2}),
         ("tile_rows_4_persistent", {api.OPT_TILE_ROWS: 4, api.OPT_PERSISTENT: api.PERSISTENT_ON}),
+        ("binning_pipeline_depth_1", {api.OPT_PIPELINE: 1, api.OPT_PERSISTENT: api.PERSISTENT_OFF}),
+        ("binning_pipeline_depth_2_fused_pass", {api.OPT_PIPELINE: 2, api.OPT_OVERLAP: 2}),
         ("serial_plain_launches", {api.OPT_OVERLAP: 0, api.OPT_GRAPH: 0}),
         ("unfused_round1_pipeline", {api.OPT_FUSED: 0}),
         ("moments_box(P:209)", {api.OPT_MOMENTS: api.MOMENTS_BOX}),
