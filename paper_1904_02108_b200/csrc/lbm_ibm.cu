@@ -159,7 +159,7 @@ struct lbm {
     cudaStream_t cap_bulk = nullptr;    //   the bulk stream-collide (low priority),
     cudaStream_t cap_prep = nullptr;    //   the second half of the binning of the next step
     cudaStream_t cap_prep2 = nullptr;   //   the first half of the binning of the step after that
-    cudaEvent_t ev_fork = nullptr, ev_bulk = nullptr, ev_prep = nullptr, ev_prep2 = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_bulk = nullptr, ev_prep = nullptr, ev_prep2 = nullptr, ev_mdf = nullptr;
     Geom g{};
     CollisionConst cc{};
     PlaneOffsets po{};
@@ -473,7 +473,7 @@ struct MdfKernels {
     void (*tiles)(const MdfArgs, int *, int, int);
     void (*pairs)(const MdfArgs, int *, int);
     void (*plan)(const MdfArgs);
-    void (*persistent)(const MdfArgs, const float *, const PlaneOffsets, int *, unsigned *, int, int);
+    void (*persistent)(const MdfArgs, const float *, const PlaneOffsets, int *, unsigned *, int, int, const WordsArgs);
 };
 
 // How many (tile, footprint coordinate) candidates a cell can have per axis: two unless a 4-cell span can wrap
@@ -738,8 +738,13 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
     return LBM_OK;
 }
 
+CollisionConst collision_const(const lbm *h);
+
 // a4-a7: moments on the active cells of set S, then the MDF loop; leaves G on the active cells.
-int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_iters, int *n_kernels, PhaseTimer *pt)
+// words_dst != NULL (persistent kernel only): the kernel also runs the stream-collide of the cells inside the stencils
+// into that buffer once G is complete.
+int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_iters, int *n_kernels, PhaseTimer *pt,
+                float *words_dst = nullptr)
 {
     const Geom &g = h->g;
     const int n = h->nm;
@@ -753,8 +758,11 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
     const int wsmem = (int)h->mdf_wsmem;
     if (use_persistent(h)) {
         // a4 + the whole loop in one kernel: grid-wide barriers instead of 2 N + 1 dependent launches
+        WordsArgs wa{};
+        wa.dst = words_dst; wa.cc = collision_const(h); wa.amask = S.amask; wa.words = S.words; wa.n_words = &sc->n_words;
+        wa.enabled = words_dst ? 1 : 0;
         K.persistent<<<h->mdfp_grid, MDFP_WARPS * 32, (size_t)MDFP_WARPS * h->mdf_wsmem, s>>>(
-            ma, src, h->po, sc->cursor, &sc->gbar, mdf_iters, wsmem);
+            ma, src, h->po, sc->cursor, &sc->gbar, mdf_iters, wsmem, wa);
         trace_mark(h, s, "mdf_persistent");
         CK(cudaGetLastError());
         *n_kernels += 1;
@@ -924,28 +932,55 @@ int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, PrepSet 
     h->trace_used = 0;
     trace_mark(h, s, "fork");
     CK(cudaEventRecord(h->ev_fork, s));
-    if (split) CK(cudaStreamWaitEvent(h->cap_bulk, h->ev_fork, 0));
+    const bool pdl = split && use_persistent(h);
+    if (split && !pdl) CK(cudaStreamWaitEvent(h->cap_bulk, h->ev_fork, 0));
     CK(cudaStreamWaitEvent(h->cap_prep, h->ev_fork, 0));
     if (N2) CK(cudaStreamWaitEvent(h->cap_prep2, h->ev_fork, 0));
-    if (split) {
+    if (split && !pdl) {
         if ((rc = enqueue_lbm_pass(h, h->cap_bulk, src, dst, LBM_BULK, S.amask))) return rc;
         trace_mark(h, h->cap_bulk, "bulk");
         ++nk;
     }
-    if ((rc = enqueue_mdf(h, s, S, src, mdf_iters, &nk, nullptr))) return rc;
+    // with the persistent MDF kernel the cells inside the stencils are updated by that kernel itself (it needs G, not
+    // the bulk pass: the two passes write disjoint cells); the step counter then advances in a kernel of its own
+    const bool fold = split && use_persistent(h);
+    if ((rc = enqueue_mdf(h, s, S, src, mdf_iters, &nk, nullptr, fold ? dst : nullptr))) return rc;
+    if (pdl) {
+        // the bulk pass as a programmatic dependent of the persistent kernel: it starts when every block of that
+        // grid is resident (griddepcontrol.launch_dependents at its top), not before
+        CK(cudaEventRecord(h->ev_mdf, s));
+        const dim3 b = cell_block(h->g);
+        const dim3 gr = cell_grid(h->g, b);
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = gr; cfg.blockDim = b; cfg.dynamicSmemBytes = 0; cfg.stream = s;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        const CollisionConst cc = collision_const(h);
+        CK(cudaLaunchKernelEx(&cfg, k_stream_collide_scalar<LBM_BULK, 256, 5>, src, dst, h->g, cc, h->po,
+                              (const unsigned *)S.amask, (const float4 *)nullptr));
+        trace_mark(h, s, "bulk");
+        ++nk;
+    }
     if ((rc = enqueue_prep(h, h->cap_prep, N, 1, &nk, nullptr, n_has_sort ? PREP_BINS : PREP_ALL))) return rc;
     trace_mark(h, h->cap_prep, "prep");
     if (N2) {
         if ((rc = enqueue_prep(h, h->cap_prep2, *N2, 2, &nk, nullptr, PREP_SORT))) return rc;
         trace_mark(h, h->cap_prep2, "prep2");
     }
-    if (split) CK(cudaEventRecord(h->ev_bulk, h->cap_bulk));
+    if (split && !pdl) CK(cudaEventRecord(h->ev_bulk, h->cap_bulk));
     CK(cudaEventRecord(h->ev_prep, h->cap_prep));
     if (N2) CK(cudaEventRecord(h->ev_prep2, h->cap_prep2));
-    if (split) CK(cudaStreamWaitEvent(s, h->ev_bulk, 0));
+    if (split && !pdl) CK(cudaStreamWaitEvent(s, h->ev_bulk, 0));
+    if (pdl) CK(cudaStreamWaitEvent(s, h->ev_mdf, 0));
     CK(cudaStreamWaitEvent(s, h->ev_prep, 0));
     if (N2) CK(cudaStreamWaitEvent(s, h->ev_prep2, 0));
-    if (split) {
+    if (fold) {
+        trace_mark(h, s, "join");
+        k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, nullptr, 0, 4);
+        ++nk;
+    } else if (split) {
         trace_mark(h, s, "join");
         if ((rc = enqueue_lbm_active(h, s, src, dst, S))) return rc;           // also advances the step counter
         ++nk;
@@ -1095,6 +1130,7 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
         ok &= cudaEventCreateWithFlags(&h->ev_bulk, cudaEventDisableTiming) == cudaSuccess;
         ok &= cudaEventCreateWithFlags(&h->ev_prep, cudaEventDisableTiming) == cudaSuccess;
         ok &= cudaEventCreateWithFlags(&h->ev_prep2, cudaEventDisableTiming) == cudaSuccess;
+        ok &= cudaEventCreateWithFlags(&h->ev_mdf, cudaEventDisableTiming) == cudaSuccess;
         if (!ok) { fail(LBM_ECUDA, "%s", cudaGetErrorString(cudaGetLastError())); return bail("streams"); }
     }
     h->po = plane_offsets(h->g);
@@ -1159,6 +1195,7 @@ void lbm_destroy(lbm_t *h)
     if (h->ev_bulk) cudaEventDestroy(h->ev_bulk);
     if (h->ev_prep) cudaEventDestroy(h->ev_prep);
     if (h->ev_prep2) cudaEventDestroy(h->ev_prep2);
+    if (h->ev_mdf) cudaEventDestroy(h->ev_mdf);
     for (cudaEvent_t e : h->trace_ev) cudaEventDestroy(e);
     delete h;
 }

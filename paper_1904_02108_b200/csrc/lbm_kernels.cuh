@@ -190,18 +190,13 @@ k_stream_collide_scalar(const float *__restrict__ src, float *__restrict__ dst, 
 // a8 on the words the bulk pass skipped (second pass of the overlapped step): one warp per entry of
 // the active-word list, lane = cell of the word; a = G + g_body where the cell's bit is set, g_body
 // on the other cells of the word.
-__global__ void __launch_bounds__(256)
-k_stream_collide_words(const float *__restrict__ src, float *__restrict__ dst, const __grid_constant__ Geom g,
-                       const __grid_constant__ CollisionConst cc, const __grid_constant__ PlaneOffsets po,
-                       const unsigned *__restrict__ amask, const int *__restrict__ words,
-                       const int *__restrict__ n_words, const float4 *__restrict__ G, long long *__restrict__ step_ctr)
+// the words pass of one warp team: warp `warp` of `nwarps` takes the entries warp, warp + nwarps, ... of the list
+__device__ __forceinline__ void stream_collide_words(const float *__restrict__ src, float *__restrict__ dst, const Geom &g,
+                                                     const CollisionConst &cc, const PlaneOffsets &po,
+                                                     const unsigned *__restrict__ amask, const int *__restrict__ words,
+                                                     const int nw, const float4 *__restrict__ G, const int warp,
+                                                     const int nwarps, const int lane)
 {
-    // last kernel of a coupled step: advance the device-side time-step counter (read by k_kinematics)
-    if (step_ctr && blockIdx.x == 0 && threadIdx.x == 0) *step_ctr += 1;
-    const int lane = threadIdx.x & 31;
-    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int nwarps = (gridDim.x * blockDim.x) >> 5;
-    const int nw = *n_words;
     // the word and its mask bits of the next round are fetched while this round's cells are updated
     int w_next = warp < nw ? __ldg(words + warp) : 0;
     unsigned bits_next = warp < nw ? __ldg(amask + w_next) : 0u;
@@ -219,7 +214,7 @@ k_stream_collide_words(const float *__restrict__ src, float *__restrict__ dst, c
         const int self = row * g.nx + x;
         float ax = cc.gbx, ay = cc.gby, az = cc.gbz;
         if ((bits >> lane) & 1u) {
-            const float4 gv = __ldg(G + self);
+            const float4 gv = __ldcg(G + self);          // written earlier in the step, possibly by this very kernel
             ax += gv.x; ay += gv.y; az += gv.z;
         }
         float df[NQ];
@@ -235,6 +230,18 @@ k_stream_collide_words(const float *__restrict__ src, float *__restrict__ dst, c
 #pragma unroll
         for (int i = 0; i < NQ; ++i) LBM_STORE(reinterpret_cast<float *>(q + po.st[i]), df[i]);
     }
+}
+
+__global__ void __launch_bounds__(256)
+k_stream_collide_words(const float *__restrict__ src, float *__restrict__ dst, const __grid_constant__ Geom g,
+                       const __grid_constant__ CollisionConst cc, const __grid_constant__ PlaneOffsets po,
+                       const unsigned *__restrict__ amask, const int *__restrict__ words,
+                       const int *__restrict__ n_words, const float4 *__restrict__ G, long long *__restrict__ step_ctr)
+{
+    // last kernel of a coupled step: advance the device-side time-step counter (read by k_kinematics)
+    if (step_ctr && blockIdx.x == 0 && threadIdx.x == 0) *step_ctr += 1;
+    stream_collide_words(src, dst, g, cc, po, amask, words, *n_words, G, (blockIdx.x * blockDim.x + threadIdx.x) >> 5,
+                         (gridDim.x * blockDim.x) >> 5, threadIdx.x & 31);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -343,8 +343,12 @@ __device__ __forceinline__ void sweep_close(SweepState &st, const int lane)
 // ---- hand every footprint element to the cell that consumes it (plan: fdst): all the destinations first
 // (independent loads), then the stores.  With two warps on a tile, `part` takes the rows fy = part, part + nparts, ...
 template <int TR>
-__device__ __forceinline__ void tile_writeout(const MdfArgs &a, const TileHdr &H, const float *foot, const int lane,
-                                              const int part, const int nparts)
+struct TileDst { int o[TileDims<TR>::TF][TileDims<TR>::KZ]; };
+
+// where this lane's footprint elements go (collect plan), -1 = nowhere
+template <int TR>
+__device__ __forceinline__ void tile_load_dst(const MdfArgs &a, const TileHdr &H, const int lane, const int part,
+                                              const int nparts, TileDst<TR> &d)
 {
     using D = TileDims<TR>;
     const int ent = a.cg.ent;
@@ -352,24 +356,40 @@ __device__ __forceinline__ void tile_writeout(const MdfArgs &a, const TileHdr &H
     const unsigned my = H.m >> 14, mz = H.m >> (21 + h);
     const bool ex = l < ent && ((H.m >> l) & 1u);
     const int *__restrict__ dst = a.fdst + (size_t)H.t * (D::NROWS * ent) + l;
-    int o[D::TF][D::KZ];
 #pragma unroll
     for (int fy = 0; fy < D::TF; ++fy)
 #pragma unroll
         for (int k = 0; k < D::KZ; ++k) {
-            o[fy][k] = -1;
+            d.o[fy][k] = -1;
             if (nparts > 1 && (fy % nparts) != part) continue;
             if (2 * k + 1 >= D::TF && h) continue;
-            if (ex && ((my >> fy) & (mz >> (2 * k)) & 1u)) o[fy][k] = __ldg(dst + (fy * D::TF + 2 * k + h) * ent);
+            if (ex && ((my >> fy) & (mz >> (2 * k)) & 1u)) d.o[fy][k] = __ldg(dst + (fy * D::TF + 2 * k + h) * ent);
         }
+}
+
+template <int TR>
+__device__ __forceinline__ void tile_store(const MdfArgs &a, const float *foot, const int lane, const TileDst<TR> &d)
+{
+    using D = TileDims<TR>;
+    const int ent = a.cg.ent;
+    const int l = lane & 15, h = lane >> 4;
 #pragma unroll
     for (int fy = 0; fy < D::TF; ++fy)
 #pragma unroll
         for (int k = 0; k < D::KZ; ++k)
-            if (o[fy][k] >= 0) {
+            if (d.o[fy][k] >= 0) {
                 const float *sp = foot + ((fy * D::TF + 2 * k + h) * ent + l) * 3;
-                __stcg(a.F + o[fy][k], make_float4(sp[0], sp[1], sp[2], 0.f));
+                __stcg(a.F + d.o[fy][k], make_float4(sp[0], sp[1], sp[2], 0.f));
             }
+}
+
+template <int TR>
+__device__ __forceinline__ void tile_writeout(const MdfArgs &a, const TileHdr &H, const float *foot, const int lane,
+                                              const int part, const int nparts)
+{
+    TileDst<TR> d;
+    tile_load_dst<TR>(a, H, lane, part, nparts, d);
+    tile_store<TR>(a, foot, lane, d);
 }
 
 // The tile pass of ONE warp over a stream of tiles (next() hands out positions in the longest-first order, < 0 =
@@ -377,8 +397,20 @@ __device__ __forceinline__ void tile_writeout(const MdfArgs &a, const TileHdr &H
 // of the current one (late, so that the dynamic balance is kept), and as soon as those are interpolated (the
 // window is dead from then on) it requests the next tile's window and first 32 markers, which arrive during
 // the last sweep and the write-out of the current tile.  wsm = the warp's shared memory (mdf_warp_smem bytes).
+// first tile of a warp's stream, loaded ahead of time: header and the first 32 markers do not depend on U, so the
+// persistent kernel requests them BEFORE the grid barrier that ends the previous phase
+struct TilePre { TileHdr H; MarkerRegs cur; };
+
 template <int TR, class Next>
-__device__ __forceinline__ void mdf_tile_loop(const MdfArgs &a, const bool last, char *wsm, const int lane, Next &&next)
+__device__ __forceinline__ void mdf_tile_prefetch(const MdfArgs &a, const int lane, TilePre &P, Next &&next)
+{
+    tile_load_hdr<TR>(a, next(), lane, P.H);
+    if (P.H.t >= 0) tile_fetch<TR>(a, P.H, 0, lane, P.cur);
+}
+
+template <int TR, class Next>
+__device__ __forceinline__ void mdf_tile_loop(const MdfArgs &a, const bool last, char *wsm, const int lane, Next &&next,
+                                              const TilePre *pre = nullptr)
 {
     using D = TileDims<TR>;
     constexpr unsigned FULL = 0xffffffffu;
@@ -388,10 +420,16 @@ __device__ __forceinline__ void mdf_tile_loop(const MdfArgs &a, const bool last,
                                  wsm + win_bytes + foot_bytes);
     TileHdr H, Hn;
     MarkerRegs cur;
-    tile_load_hdr<TR>(a, next(), lane, H);
-    if (H.t < 0) return;
-    tile_issue_window<TR>(a, H, sm.win, lane, 0, 1);
-    tile_fetch<TR>(a, H, 0, lane, cur);
+    if (pre) {
+        H = pre->H; cur = pre->cur;
+        if (H.t < 0) return;
+        tile_issue_window<TR>(a, H, sm.win, lane, 0, 1);
+    } else {
+        tile_load_hdr<TR>(a, next(), lane, H);
+        if (H.t < 0) return;
+        tile_issue_window<TR>(a, H, sm.win, lane, 0, 1);
+        tile_fetch<TR>(a, H, 0, lane, cur);
+    }
 
     while (H.t >= 0) {
         const int total = H.total;
@@ -405,6 +443,9 @@ __device__ __forceinline__ void mdf_tile_loop(const MdfArgs &a, const bool last,
         __syncwarp();
 
         // ---- the tile's markers, 32 at a time -------------------------------------------------------------
+        // single-row tiles (small marker sets, latency-bound): the destinations are requested now, not after the sweep
+        TileDst<TR> dst_early;
+        if (TR == 1) tile_load_dst<TR>(a, H, lane, 0, 1, dst_early);
         SweepState st;
         st.started = 0; st.e = 0; st.frow = sm.foot;
         st.p = Acc3{0.f, 0.f, 0.f}; st.q = Acc3{0.f, 0.f, 0.f};
@@ -436,7 +477,8 @@ __device__ __forceinline__ void mdf_tile_loop(const MdfArgs &a, const bool last,
         }
         sweep_close(st, lane);
         __syncwarp();
-        tile_writeout<TR>(a, H, sm.foot, lane, 0, 1);
+        if (TR == 1) tile_store<TR>(a, sm.foot, lane, dst_early);
+        else tile_writeout<TR>(a, H, sm.foot, lane, 0, 1);
         __syncwarp();
         H = Hn;
     }
@@ -584,11 +626,14 @@ k_collect_plan(const __grid_constant__ MdfArgs a)
     constexpr int TF = TR + 3;
     const Geom &g = a.g;
     const int lane = threadIdx.x & 31;
-    const int sub = lane & 3, cl = lane >> 2;        // four lanes per cell: lane `sub` takes the z candidate iz = sub
+    constexpr int LPC = MAXCYZ;                      // lanes per cell: lane `sub` of a cell takes the z candidate iz = sub
+    constexpr int LSH = LPC == 4 ? 2 : 1;
+    static_assert(LPC == 2 || LPC == 4, "two or four z candidates");
+    const int sub = lane & (LPC - 1), cl = lane >> LSH;
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     const int stride = gridDim.x * blockDim.x;
     const int nc = *a.n_cells;
-    for (int c0 = (tid - lane) >> 2; c0 < nc; c0 += stride >> 2) {
+    for (int c0 = (tid - lane) >> LSH; c0 < nc; c0 += stride >> LSH) {
         const int k = c0 + cl;
         AxisCandT<MAXCX> ax;
         AxisCandT<MAXCYZ> ay, az;
@@ -637,7 +682,7 @@ k_collect_plan(const __grid_constant__ MdfArgs a)
         if (lane == 31 && total) base = atomicAdd(a.n_felem, total);
         base = __shfl_sync(0xffffffffu, base, 31);
         int o = base + incl - cnt;
-        const int run_len = __shfl_sync(0xffffffffu, incl, lane | 3) - (incl - cnt) ;      // sub == 0: elements of the cell
+        const int run_len = __shfl_sync(0xffffffffu, incl, lane | (LPC - 1)) - (incl - cnt);   // sub == 0: elements of the cell
         if (k < nc && sub == 0) a.cell_run[k] = make_int2(o, run_len);
         for_each([&](size_t el) { a.fdst[el] = o++; });
     }
@@ -657,10 +702,8 @@ k_fill_tiles(int *__restrict__ fdst, const int *__restrict__ n_tiles, int tile_c
 
 // One active cell adds up its run of footprint elements, in order.
 //   last = false:  U^{m+1}(X) = U^m(X) + sum   (R8)      last = true:  G(X) = sum
-__device__ __forceinline__ void mdf_collect_cell(const MdfArgs &a, const int k, const bool last)
+__device__ __forceinline__ void mdf_collect_run(const MdfArgs &a, const int cell, const int2 run, const bool last)
 {
-    const int cell = __ldg(a.cells + k);
-    const int2 run = __ldg(a.cell_run + k);
     const float4 *__restrict__ f = a.F + run.x;
     float sx = 0.f, sy = 0.f, sz = 0.f;
     for (int i0 = 0; i0 < run.y; i0 += 8) {
@@ -677,6 +720,11 @@ __device__ __forceinline__ void mdf_collect_cell(const MdfArgs &a, const int k, 
         u.x += sx; u.y += sy; u.z += sz;
         a.U[cell] = u;
     }
+}
+
+__device__ __forceinline__ void mdf_collect_cell(const MdfArgs &a, const int k, const bool last)
+{
+    mdf_collect_run(a, __ldg(a.cells + k), __ldg(a.cell_run + k), last);
 }
 
 __global__ void __launch_bounds__(256)
@@ -729,10 +777,22 @@ __device__ __forceinline__ void moments_cell(const float *__restrict__ src, cons
 
 constexpr int MDFP_WARPS = 8;           // warps per block of the persistent kernel
 
+// What the persistent kernel needs for the stream-collide of the cells inside the stencils (the words pass), which
+// it runs itself once G is complete: one launch and one graph dependency fewer at the end of the step.
+struct WordsArgs {
+    float *dst;
+    CollisionConst cc;
+    const unsigned *amask;
+    const int *words;
+    const int *n_words;
+    int enabled;
+};
+
 template <int TR>
 __global__ void __launch_bounds__(MDFP_WARPS * 32, 2)
 k_mdf_persistent(const __grid_constant__ MdfArgs a, const float *__restrict__ src, const __grid_constant__ PlaneOffsets po,
-                 int *__restrict__ cursors, unsigned *__restrict__ bar, int mdf_iters, int warp_smem)
+                 int *__restrict__ cursors, unsigned *__restrict__ bar, int mdf_iters, int warp_smem,
+                 const __grid_constant__ WordsArgs wa)
 {
     extern __shared__ __align__(128) char smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -742,27 +802,48 @@ k_mdf_persistent(const __grid_constant__ MdfArgs a, const float *__restrict__ sr
     const int nt = min(*a.n_tiles, a.tile_cap);
     const int nc = *a.n_cells;
     const int gwarp = warp * gridDim.x + blockIdx.x, nwarps = gridDim.x * MDFP_WARPS;   // consecutive tiles go to different SMs
+    const bool dealt = nt <= 2 * nwarps;     // few tiles: dealt statically, longest first (no cursor round trips)
     unsigned target = 0u;
+    // every block of this grid is resident now: let the stream-collide pass that runs beside the loop start (it is
+    // launched as a programmatic dependent, so that it cannot take the SMs before this grid holds its share)
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    // the first cell this thread collects is the same in every iteration: its index and run stay in registers
+    int my_cell = -1;
+    int2 my_run = make_int2(0, 0);
+    if (tid < nc) { my_cell = __ldg(a.cells + tid); my_run = __ldg(a.cell_run + tid); }
     // a4: rho, U of eq. (1) on the active cells
-    for (int k = tid; k < nc; k += stride) moments_cell(src, a.g, po, __ldg(a.cells + k), a.U);
+    if (my_cell >= 0) moments_cell(src, a.g, po, my_cell, a.U);
+    for (int k = tid + stride; k < nc; k += stride) moments_cell(src, a.g, po, __ldg(a.cells + k), a.U);
+    // header and first markers of this warp's first tile: requested before the barrier, they arrive behind it
+    TilePre P;
+    int kd = gwarp - nwarps;
+    auto next_dealt = [&]() { kd += nwarps; return kd < nt ? kd : -1; };
+    int itc = 0;
+    auto next_drawn = [&]() {
+        int t = 0;
+        if (lane == 0) { t = atomicAdd(cursors + itc, 1); t = t < nt ? t : -1; }
+        return __shfl_sync(0xffffffffu, t, 0);
+    };
+    if (dealt) mdf_tile_prefetch<TR>(a, lane, P, next_dealt); else mdf_tile_prefetch<TR>(a, lane, P, next_drawn);
     grid_barrier(bar, target);
     for (int it = 0; it < mdf_iters; ++it) {
         const bool last = (it == mdf_iters - 1);
-        if (nt <= 2 * nwarps) {
-            // few tiles: dealt statically, longest first (no cursor round trips on the critical path)
-            int k = gwarp - nwarps;
-            mdf_tile_loop<TR>(a, last, wsm, lane, [&]() { k += nwarps; return k < nt ? k : -1; });
-        } else {
-            mdf_tile_loop<TR>(a, last, wsm, lane, [&]() {
-                int t = 0;
-                if (lane == 0) { t = atomicAdd(cursors + it, 1); t = t < nt ? t : -1; }
-                return __shfl_sync(0xffffffffu, t, 0);
-            });
-        }
+        if (dealt) mdf_tile_loop<TR>(a, last, wsm, lane, next_dealt, &P);
+        else mdf_tile_loop<TR>(a, last, wsm, lane, next_drawn, &P);
         grid_barrier(bar, target);
-        for (int k = tid; k < nc; k += stride) mdf_collect_cell(a, k, last);
-        if (!last) grid_barrier(bar, target);
+        if (my_cell >= 0) mdf_collect_run(a, my_cell, my_run, last);
+        for (int k = tid + stride; k < nc; k += stride) mdf_collect_cell(a, k, last);
+        if (!last) {
+            // the next iteration's first tile (Delta u of its markers was written by this very thread: program order)
+            kd = gwarp - nwarps; itc = it + 1;
+            if (dealt) mdf_tile_prefetch<TR>(a, lane, P, next_dealt); else mdf_tile_prefetch<TR>(a, lane, P, next_drawn);
+            grid_barrier(bar, target);
+        }
     }
+    if (!wa.enabled) return;
+    // a8 on the cells inside the stencils: needs the complete G of every active cell
+    grid_barrier(bar, target);
+    stream_collide_words(src, wa.dst, a.g, wa.cc, po, wa.amask, wa.words, *wa.n_words, a.G, gwarp, nwarps, lane);
 }
 
 }  // namespace lbmk
