@@ -504,7 +504,7 @@ k_chunks(const unsigned *__restrict__ skey, int n, Geom g, ChunkGeom cg, const u
     __syncthreads();
     if (threadIdx.x == 0) {
         int tc = 0, te = 0;
-        for (int w = 0; w < 8; ++w) { const int t = s_cnt[w]; s_cnt[w] = tc; tc += t; te += s_ent[w]; }
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { const int t = s_cnt[w]; s_cnt[w] = tc; tc += t; te += s_ent[w]; }
         s_base = tc ? atomicAdd(n_chunks, tc) : 0;
         if (te) atomicAdd(n_entries, te);
     }

@@ -763,7 +763,7 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
         wa.enabled = words_dst ? 1 : 0;
         K.persistent<<<h->mdfp_grid, MDFP_WARPS * 32, (size_t)MDFP_WARPS * h->mdf_wsmem, s>>>(
             ma, src, h->po, sc->cursor, &sc->gbar, mdf_iters, wsmem, wa);
-        trace_mark(h, s, "mdf_persistent");
+        if (!words_dst) trace_mark(h, s, "mdf_persistent");   // with the words pass inside: marked by the caller, off this stream
         CK(cudaGetLastError());
         *n_kernels += 1;
         return LBM_OK;
@@ -949,6 +949,13 @@ int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, PrepSet 
         // the bulk pass as a programmatic dependent of the persistent kernel: it starts when every block of that
         // grid is resident (griddepcontrol.launch_dependents at its top), not before
         CK(cudaEventRecord(h->ev_mdf, s));
+        if (h->opt_trace) {
+            // the trace event of the persistent kernel goes to a side stream: an event node between the two kernels
+            // would turn the programmatic edge into a full dependency
+            CK(cudaStreamWaitEvent(h->cap_bulk, h->ev_mdf, 0));
+            trace_mark(h, h->cap_bulk, "mdf_persistent");
+            CK(cudaEventRecord(h->ev_bulk, h->cap_bulk));
+        }
         const dim3 b = cell_block(h->g);
         const dim3 gr = cell_grid(h->g, b);
         cudaLaunchConfig_t cfg{};
@@ -974,6 +981,7 @@ int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, PrepSet 
     if (N2) CK(cudaEventRecord(h->ev_prep2, h->cap_prep2));
     if (split && !pdl) CK(cudaStreamWaitEvent(s, h->ev_bulk, 0));
     if (pdl) CK(cudaStreamWaitEvent(s, h->ev_mdf, 0));
+    if (pdl && h->opt_trace) CK(cudaStreamWaitEvent(s, h->ev_bulk, 0));
     CK(cudaStreamWaitEvent(s, h->ev_prep, 0));
     if (N2) CK(cudaStreamWaitEvent(s, h->ev_prep2, 0));
     if (fold) {

@@ -775,7 +775,10 @@ __device__ __forceinline__ void moments_cell(const float *__restrict__ src, cons
     U[cell] = make_float4(ux, uy, uz, 1.0f + drho);
 }
 
-constexpr int MDFP_WARPS = 8;           // warps per block of the persistent kernel
+#ifndef MDFP_WARPS_CFG
+#define MDFP_WARPS_CFG 8
+#endif
+constexpr int MDFP_WARPS = MDFP_WARPS_CFG;   // warps per block of the persistent kernel
 
 // What the persistent kernel needs for the stream-collide of the cells inside the stencils (the words pass), which
 // it runs itself once G is complete: one launch and one graph dependency fewer at the end of the step.

@@ -124,21 +124,23 @@ k_radix_scatter(const unsigned *__restrict__ keys_in, const int *__restrict__ va
     }
 }
 
-// Small marker sets: all passes in ONE kernel of ONE block (32 warps; warp w owns the w-th contiguous stretch of the
-// array).  Per pass: per-warp digit histograms in shared memory, one thread per digit turns them into the warps'
+// Small marker sets: all passes in ONE kernel of ONE block (16 warps; warp w owns the w-th contiguous stretch of the
+// array; 512 threads so that the block finds room on an SM that already holds a block of the persistent MDF kernel).  Per pass: per-warp digit histograms in shared memory, one thread per digit turns them into the warps'
 // start offsets (digit-major, warp-minor: the same order as the three-kernel pass), the warps scatter their items
 // 32 at a time with the same __match_any_sync ranking; block barriers order the passes (one block: no grid-wide
 // synchronisation is needed).  Same result as the three-kernel passes, nine launches fewer for a 24-bit key.
-constexpr int SORT_SMALL_BLOCK = 1024;
+#ifndef SORT_SMALL_BLOCK_CFG
+#define SORT_SMALL_BLOCK_CFG 512
+#endif
+constexpr int SORT_SMALL_BLOCK = SORT_SMALL_BLOCK_CFG;
 constexpr int SORT_SMALL_WARPS = SORT_SMALL_BLOCK / 32;
 constexpr int SORT_SMALL_MAX = 32768;       // markers up to which the single-block sort is used
 
-__global__ void __launch_bounds__(SORT_SMALL_BLOCK, 1)
+__global__ void __launch_bounds__(SORT_SMALL_BLOCK, 2)
 k_radix_sort_small(unsigned *keys0, unsigned *keys1, int *vals0, int *vals1, int n, int npasses)
 {
     __shared__ int cnt[SORT_SMALL_WARPS][RADIX];
     __shared__ int dsum[RADIX];
-    __shared__ int wsum[RADIX / 32];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const int per = ((n + SORT_SMALL_WARPS - 1) / SORT_SMALL_WARPS + 31) & ~31;
     const int beg = min(n, wib * per), end = min(n, beg + per);
@@ -154,33 +156,46 @@ k_radix_sort_small(unsigned *keys0, unsigned *keys1, int *vals0, int *vals1, int
         __syncwarp();
         for (int i = beg + lane; i < end; i += 32) atomicAdd(&cnt[wib][(kin[i] >> shift) & (RADIX - 1)], 1);
         __syncthreads();
-        // thread d < 256: exclusive prefix of digit d over the warps, digit total
-        if (threadIdx.x < RADIX) {
+        // one thread per digit (in rounds): exclusive prefix of the digit over the warps, digit total
+        for (int d = threadIdx.x; d < RADIX; d += SORT_SMALL_BLOCK) {
             int run = 0;
-#pragma unroll 8
-            for (int w = 0; w < SORT_SMALL_WARPS; ++w) { const int v = cnt[w][threadIdx.x]; cnt[w][threadIdx.x] = run; run += v; }
+#pragma unroll 4
+            for (int w = 0; w < SORT_SMALL_WARPS; ++w) { const int v = cnt[w][d]; cnt[w][d] = run; run += v; }
+            dsum[d] = run;
+        }
+        __syncthreads();
+        // warp 0: exclusive scan of the 256 digit totals, lane holds digits 8 lane .. 8 lane + 7
+        if (wib == 0) {
+            int t[8], run = 0;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) { t[j] = dsum[lane * 8 + j]; run += t[j]; }
             int incl = run;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
                 const int v = __shfl_up_sync(0xffffffffu, incl, o);
                 if (lane >= o) incl += v;
             }
-            if (lane == 31) wsum[wib] = incl;
-            dsum[threadIdx.x] = incl - run;          // exclusive inside the warp of 32 digits
+            int base = incl - run;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) { dsum[lane * 8 + j] = base; base += t[j]; }
         }
         __syncthreads();
-        if (threadIdx.x < RADIX) {
-            int base = dsum[threadIdx.x];
-            for (int w = 0; w < wib; ++w) base += wsum[w];
-#pragma unroll 8
-            for (int w = 0; w < SORT_SMALL_WARPS; ++w) cnt[w][threadIdx.x] += base;
+        for (int d = threadIdx.x; d < RADIX; d += SORT_SMALL_BLOCK) {
+            const int base = dsum[d];
+#pragma unroll 4
+            for (int w = 0; w < SORT_SMALL_WARPS; ++w) cnt[w][d] += base;
         }
         __syncthreads();
+        // the items of round r + 1 are requested while round r is ranked (one warp per stretch: nothing else hides
+        // the load latency)
+        unsigned key_n = (beg + lane < end) ? kin[beg + lane] : 0u;
+        int val_n = (beg + lane < end) ? (vin ? vin[beg + lane] : beg + lane) : 0;
         for (int r = beg; r < end; r += 32) {
             const int i = r + lane;
             const bool valid = i < end;
-            const unsigned key = valid ? kin[i] : 0u;
-            const int val = valid ? (vin ? vin[i] : i) : 0;
+            const unsigned key = key_n;
+            const int val = val_n;
+            if (i + 32 < end) { key_n = kin[i + 32]; val_n = vin ? vin[i + 32] : i + 32; }
             const unsigned d = valid ? ((key >> shift) & (RADIX - 1)) : 0xffffffffu;
             const unsigned peers = __match_any_sync(0xffffffffu, d);
             const int leader = __ffs(peers) - 1;
