@@ -18,6 +18,10 @@
  *  - Every pointer argument marked "host or device" may point to pageable/pinned host memory or
  *    to device memory of the handle's GPU (detected with cudaPointerGetAttributes).  Pointers
  *    marked "host" are read on the CPU during the call.
+ *  - Device INPUTS are read on the handle's stream (ibm_set_markers: by a blocking copy): what they
+ *    hold must be complete before the call, i.e. produced on the handle's stream or on a stream the
+ *    caller has synchronised with it.  Device OUTPUTS are written on the handle's stream and are
+ *    valid for work enqueued behind it on that stream (or after lbm_sync).
  *  - The caller owns every buffer it passes; inputs are copied during the call and may be freed
  *    at once.  The library owns lattice and marker state (device memory of the current device at
  *    lbm_create time).

@@ -1327,24 +1327,28 @@ int lbm_set_fields(lbm_t *h, const float *rho, const float *u)
     int rc = flush_ibm(h);
     if (rc) return rc;
     const size_t cells = (size_t)h->g.cells;
-    float *d_rho = nullptr, *d_u = nullptr;
     const float *p_rho = rho, *p_u = u;
+    // host sources go through the handle's staging buffers (kept between calls: no cudaMalloc / cudaFree, which
+    // synchronise the device, on the path of a host loop that resets the fields)
     if (rho && !is_device_ptr(rho)) {
-        CK(cudaMalloc((void **)&d_rho, cells * sizeof(float)));
-        CK(cudaMemcpyAsync(d_rho, rho, cells * sizeof(float), cudaMemcpyHostToDevice, h->stream));
-        p_rho = d_rho;
+        float *d = (float *)stage_get(h, 0, cells * sizeof(float));
+        if (!d) return fail(LBM_ENOMEM, "lbm_set_fields: staging allocation failed");
+        CK(cudaMemcpyAsync(d, rho, cells * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+        p_rho = d;
     }
     if (u && !is_device_ptr(u)) {
-        CK(cudaMalloc((void **)&d_u, 3 * cells * sizeof(float)));
-        CK(cudaMemcpyAsync(d_u, u, 3 * cells * sizeof(float), cudaMemcpyHostToDevice, h->stream));
-        p_u = d_u;
+        float *d = (float *)stage_get(h, 1, 3 * cells * sizeof(float));
+        if (!d) return fail(LBM_ENOMEM, "lbm_set_fields: staging allocation failed");
+        CK(cudaMemcpyAsync(d, u, 3 * cells * sizeof(float), cudaMemcpyHostToDevice, h->stream));
+        p_u = d;
     }
     dim3 b = cell_block(h->g);
     k_init_fields<<<cell_grid(h->g, b), b, 0, h->stream>>>(h->f[h->cur], h->g, p_rho, p_u);
     h->launches += 1;
-    cudaError_t e = cudaStreamSynchronize(h->stream);
-    if (d_rho) cudaFree(d_rho);
-    if (d_u) cudaFree(d_u);
+    cudaError_t e = cudaGetLastError();
+    // the caller's host buffers may be reused when the call returns
+    if (e == cudaSuccess && (p_rho != rho || p_u != u)) e = cudaStreamSynchronize(h->stream);
+    stage_release(h);
     if (e != cudaSuccess) return fail(LBM_ECUDA, "lbm_set_fields: %s", cudaGetErrorString(e));
     h->steps_done = 0;
     h->force_valid = false;
