@@ -88,7 +88,7 @@ enum {
                              branches (MDF loop, binning of the next step), then ONE fused stream-collide
                              pass over the whole lattice.  0 = one serial chain with a single fused
                              stream-collide pass (measured comparison).  3 (default) = 2 on lattices above
-                             64 Mi cells or above 1,000,000 markers, else 1.  Results are bit-identical.      */
+                             64 Mi cells or above 40,000 markers, else 1.  Results are bit-identical.      */
     LBM_OPT_MOMENTS = 8,  /* where U is precomputed for the IBM: 0 = the de-duplicated list of
                              cells inside a marker stencil (default), 1 = the paper's box strategy (bounding
                              box of every body), 2 = the paper's kernel strategy (a block per Lagrangian
@@ -98,7 +98,7 @@ enum {
                              round-1 pipeline: interpolation kernel, TMA-fed tile sweep, collect (measured
                              comparison).  Only with LBM_OPT_SPREAD = 0 and LBM_OPT_INTERP = 0.           */
     LBM_OPT_TILE_ROWS = 10, /* source rows per tile in y and z for the fused path: 0 = automatic (1 up to 20,000
-                             markers, 2 up to 400,000, else 4), or 1, 2, 4.  Changing it rebuilds the tile
+                             markers, 2 up to 40,000, else 4), or 1, 2, 4.  Changing it rebuilds the tile
                              tables at the next step.  Results agree to rounding (summation order).        */
     LBM_OPT_PERSISTENT = 11, /* the fused MDF loop (moments + N x (tile pass, collect)) as ONE persistent kernel
                              with grid-wide barriers instead of 2 N + 1 launches: 1 = on, 2 = off, 0 (default) =

@@ -83,13 +83,15 @@ struct HostBody {
 constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driven kernels (grid-stride loops over device-side lists)
 // Tile edge by marker count (LBM_OPT_TILE_ROWS = 0), measured on B200: single-row tiles while
 // the set is so small that larger tiles would not fill the SMs (W1, W3: 15,360 markers), two-row tiles up to a few
-// hundred thousand markers (P6, P18, W4lit), 4 x 4-row tiles beyond (W4, W5lit, W5).
+// ten thousand markers (P6), 4 x 4-row tiles beyond (P18, W4lit, W4, W5lit, W5).
 constexpr int TR1_MAX_MARKERS = 20000;
-constexpr int TR2_MAX_MARKERS = 400000;
-// Step layout (LBM_OPT_OVERLAP = 3): on large lattices / marker sets the split of the stream-collide into a bulk
-// pass beside the MDF loop and a pass over the stencil cells costs more than the overlap hides
+constexpr int TR2_MAX_MARKERS = 40000;
+// Step layout (LBM_OPT_OVERLAP = 3): the split of the stream-collide into a bulk pass beside the MDF loop and a pass
+// over the stencil cells pays while the MDF loop is a chain of short, latency-bound kernels that leave the SMs mostly
+// idle (small marker sets); beyond that the tile pass fills the SMs itself and one fused pass after it is faster
+// (measured: P18 0.469 against 0.552 ms per step, W4lit 0.683 against 0.740, W4 1.245 against 1.262)
 constexpr long long SPLIT_MAX_CELLS = 64LL << 20;
-constexpr int SPLIT_MAX_MARKERS = 1000000;
+constexpr int SPLIT_MAX_MARKERS = 40000;
 
 // Optional per-phase device timing (LBM_OPT_TIMING): CUDA events recorded on the launching stream
 // between the phases of a step; durations are accumulated after a stream synchronise.
@@ -209,9 +211,11 @@ struct lbm {
     PhaseTimer timer;
     // LBM_OPT_TRACE: timing events recorded inside the step graph after every kernel of every branch
     int opt_trace = 0;
-    std::vector<cudaEvent_t> trace_ev;
-    std::vector<std::string> trace_label;
-    size_t trace_used = 0;
+    struct TraceList { std::vector<cudaEvent_t> ev; std::vector<std::string> label; };
+    std::map<long long, TraceList> traces;      // one list per step graph (the variants differ in their kernels)
+    TraceList *trace_cap = nullptr;             // list of the graph being captured
+    const TraceList *trace_last = nullptr;      // list of the graph launched last
+    long long last_key = 0;                     // key of the graph get_graph returned last
     std::map<long long, std::pair<cudaGraphExec_t, int>> graphs;   // key -> (exec, kernel nodes)
     long long launches = 0;
     size_t dev_bytes = 0;
@@ -271,26 +275,34 @@ bool is_device_ptr(const void *p)
     return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
 }
 
+void drop_traces(lbm *h);
 void drop_graphs(lbm *h)
 {
     for (auto &kv : h->graphs) cudaGraphExecDestroy(kv.second.first);
     h->graphs.clear();
+    drop_traces(h);
 }
 
 // LBM_OPT_TRACE: record a timing event on (capture) stream s; slot order = enqueue order, fixed per graph
 void trace_mark(lbm *h, cudaStream_t s, const char *label, int idx = -1)
 {
-    if (!h->opt_trace) return;
+    if (!h->opt_trace || !h->trace_cap) return;
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     if (cudaStreamIsCapturing(s, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusActive) return;   // graph nodes only
-    if (h->trace_used == h->trace_ev.size()) {
-        cudaEvent_t e; cudaEventCreate(&e);
-        h->trace_ev.push_back(e); h->trace_label.emplace_back();
-    }
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) return;
     char buf[64];
     if (idx >= 0) snprintf(buf, sizeof buf, "%s[%d]", label, idx); else snprintf(buf, sizeof buf, "%s", label);
-    h->trace_label[h->trace_used] = buf;
-    cudaEventRecordWithFlags(h->trace_ev[h->trace_used++], s, cudaEventRecordExternal);
+    h->trace_cap->ev.push_back(e);
+    h->trace_cap->label.emplace_back(buf);
+    cudaEventRecordWithFlags(e, s, cudaEventRecordExternal);
+}
+
+void drop_traces(lbm *h)
+{
+    for (auto &kv : h->traces) for (cudaEvent_t e : kv.second.ev) cudaEventDestroy(e);
+    h->traces.clear();
+    h->trace_cap = nullptr; h->trace_last = nullptr;
 }
 
 void free_set(lbm *h, PrepSet &S)
@@ -700,7 +712,7 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
             nk += 3;
         }
     }
-    trace_mark(h, s, "prep.sort");
+    trace_mark(h, s, step_offset == 2 ? "prep2.sort" : "prep.sort");
     }
     if (!(parts & PREP_BINS)) { CK(cudaGetLastError()); *n_kernels += nk; return LBM_OK; }
     if (pt) pt->mark(PH_BINS, s);
@@ -929,7 +941,6 @@ int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, PrepSet 
     cudaStream_t s = h->cap_stream;
     int nk = 0, rc;
     const bool split = overlap_mode(h) == 1;    // 1: bulk stream-collide beside the MDF loop; 2: one fused pass after it
-    h->trace_used = 0;
     trace_mark(h, s, "fork");
     CK(cudaEventRecord(h->ev_fork, s));
     const bool pdl = split && use_persistent(h);
@@ -1014,9 +1025,11 @@ int get_graph(lbm *h, int kind, int parity, int set, int mdf_iters, cudaGraphExe
                           ((long long)overlap_mode(h) << 56) | ((long long)h->opt_moments << 58) |
                           ((long long)h->opt_fused << 60) | ((long long)h->tr << 16) | ((long long)use_persistent(h) << 20) |
                           ((long long)tile_warps(h) << 21) | ((long long)h->opt_trace << 23) | ((long long)pipe << 24);
+    h->last_key = key;
     auto it = h->graphs.find(key);
     if (it != h->graphs.end()) { *exec = it->second.first; *n_kernels = it->second.second; return LBM_OK; }
     cudaGraph_t graph = nullptr;
+    if (h->opt_trace && kind == 2) h->trace_cap = &h->traces[key];
     CK(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
     int nk = 0, rc;
     if (kind == 2)
@@ -1024,6 +1037,7 @@ int get_graph(lbm *h, int kind, int parity, int set, int mdf_iters, cudaGraphExe
                                      (pipe & 2) ? &h->set[(set + 2) % N_SETS] : nullptr, (pipe & 1) != 0, mdf_iters, &nk);
     else rc = enqueue_step_serial(h, h->cap_stream, parity, kind ? &h->set[set] : nullptr, true, mdf_iters, &nk);
     cudaError_t e = cudaStreamEndCapture(h->cap_stream, &graph);
+    h->trace_cap = nullptr;
     if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
     if (e != cudaSuccess) return fail(LBM_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
     if (kind == 2) {
@@ -1204,14 +1218,14 @@ void lbm_destroy(lbm_t *h)
     if (h->ev_prep) cudaEventDestroy(h->ev_prep);
     if (h->ev_prep2) cudaEventDestroy(h->ev_prep2);
     if (h->ev_mdf) cudaEventDestroy(h->ev_mdf);
-    for (cudaEvent_t e : h->trace_ev) cudaEventDestroy(e);
+    drop_traces(h);
     delete h;
 }
 
 const char *lbm_trace_label(lbm_t *h, int i)
 {
-    if (!h || i < 0 || (size_t)i >= h->trace_used) return "";
-    return h->trace_label[(size_t)i].c_str();
+    if (!h || !h->trace_last || i < 0 || (size_t)i >= h->trace_last->label.size()) return "";
+    return h->trace_last->label[(size_t)i].c_str();
 }
 
 int lbm_query_layout(int nx, int ny, int nz, int *out)
@@ -1261,7 +1275,7 @@ int lbm_set_option(lbm_t *h, int key, int value)
         case LBM_OPT_PIPELINE: if (value < 0 || value > 2) break; h->opt_pipeline = value; return LBM_OK;
         case LBM_OPT_TRACE:
             if (value < 0 || value > 1) break;
-            if (value != h->opt_trace) { CK(cudaStreamSynchronize(h->stream)); drop_graphs(h); h->opt_trace = value; h->trace_used = 0; }
+            if (value != h->opt_trace) { CK(cudaStreamSynchronize(h->stream)); drop_graphs(h); h->opt_trace = value; }
             return LBM_OK;
         case LBM_OPT_TILE_CAP:
             if (value < 0) break;
@@ -1300,16 +1314,16 @@ int lbm_get_info(lbm_t *h, int key, long long *value)
             *value = st;
             return LBM_OK;
         }
-        case LBM_INFO_TRACE_COUNT: *value = (long long)h->trace_used; return LBM_OK;
+        case LBM_INFO_TRACE_COUNT: *value = h->trace_last ? (long long)h->trace_last->ev.size() : 0; return LBM_OK;
         case LBM_INFO_LAYOUT: *value = (h->nm > 0) ? overlap_mode(h) : 0; return LBM_OK;
         case LBM_INFO_TILE_ROWS: *value = h->tr; return LBM_OK;
         case LBM_INFO_SORT_PASSES: *value = h->sort_passes; return LBM_OK;
         default:
-            if (key >= LBM_INFO_TRACE_NS && key < LBM_INFO_TRACE_NS + (int)h->trace_used) {
+            if (h->trace_last && key >= LBM_INFO_TRACE_NS && key < LBM_INFO_TRACE_NS + (int)h->trace_last->ev.size()) {
                 // device time from the first trace event of the last step (the fork) to event key - LBM_INFO_TRACE_NS
                 CK(cudaStreamSynchronize(h->stream));
                 float ms = 0.f;
-                CK(cudaEventElapsedTime(&ms, h->trace_ev[0], h->trace_ev[(size_t)(key - LBM_INFO_TRACE_NS)]));
+                CK(cudaEventElapsedTime(&ms, h->trace_last->ev[0], h->trace_last->ev[(size_t)(key - LBM_INFO_TRACE_NS)]));
                 *value = (long long)(1e6 * (double)ms);
                 return LBM_OK;
             }
@@ -1504,6 +1518,17 @@ int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
         if ((rc = ensure_comparison_arrays(h))) return rc;
     }
     const bool overlapped = ibm && h->opt_overlap && h->opt_graph && !h->opt_timing;
+    if (overlapped) {
+        // the steady-state graphs of every (buffer parity, marker set) combination are built now, not one by one
+        // during the first six steps of a run
+        const int pipe = pipeline_depth(h) == 2 ? 3 : 0;
+        for (int par = 0; par < 2; ++par)
+            for (int st = 0; st < N_SETS; ++st) {
+                cudaGraphExec_t ex = nullptr;
+                int nk = 0;
+                if ((rc = get_graph(h, 2, par, st, mdf_iters, &ex, &nk, pipe))) return rc;
+            }
+    }
     for (int s = 0; s < nsteps; ++s) {
         int nk = 0;
         cudaGraphExec_t ex = nullptr;
@@ -1524,6 +1549,7 @@ int lbm_ibm_step(lbm_t *h, int nsteps, int mdf_iters)
             const bool n_has_sort = N.step == h->steps_done + 1 && N.spread == sig && N.stage == 1;
             if ((rc = get_graph(h, 2, h->cur, h->cur_set, mdf_iters, &ex, &nk, (n_has_sort ? 1 : 0) | (depth2 ? 2 : 0)))) return rc;
             CK(cudaGraphLaunch(ex, h->stream));
+            if (h->opt_trace) { auto tr = h->traces.find(h->last_key); h->trace_last = tr == h->traces.end() ? nullptr : &tr->second; }
             N.step = h->steps_done + 1; N.spread = sig; N.stage = 2; N.dirty = true;
             if (depth2) {
                 PrepSet &N2 = h->set[(h->cur_set + 2) % N_SETS];
