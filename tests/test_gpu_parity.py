@@ -285,6 +285,35 @@ def test_kinematics_change_discards_the_set_prepared_ahead(api):
     assert not np.array_equal(same[3], got[3])
 
 
+@pytest.mark.parametrize("opts", [{}, {"pipeline": 1}, {"persistent": 2}, {"pipeline": 1, "persistent": 2, "overlap": 2}])
+def test_controller_that_retunes_every_step_matches_the_serial_chain(api, opts):
+    """A host controller that changes the rotation rate before every step: everything binned ahead (the second half
+    of step n + 1 and the first half of step n + 2, three marker sets) is discarded each time and the step bins in
+    line; in between, runs of unchanged steps let the pipeline fill again.  Bit-identical to the serial chain."""
+    from paper_1904_02108_b200 import workloads
+    wl = workloads.get("W1")
+    b = wl.bodies[0]
+    plan = [(1, 1.5), (1, 0.5), (1, None), (3, 2.0), (1, 1.0), (4, None), (1, 3.0), (2, None)]   # (steps, omega factor or None)
+    outs = []
+    for serial in (True, False):
+        sim = api.from_workload(wl, stream=_stream())
+        if serial:
+            sim.set_option(api.OPT_OVERLAP, 0)
+        else:
+            for k, v in opts.items():
+                sim.set_option(getattr(api, "OPT_" + k.upper()), v)
+        for n, fac in plan:
+            if fac is not None:
+                sim.update_kinematics(0, np.array([fac * b.omega]), np.array([b.axis]))
+            sim.step(n, wl.mdf_iters)
+        mk = sim.read_markers()
+        outs.append(sim.read_fields() + (mk["force"], mk["perm"], mk["pos"]))
+        sim.sync()
+        sim.close()
+    for a, c in zip(*outs):
+        assert np.array_equal(a, c)
+
+
 def test_pure_and_coupled_steps_interleave(api, orc):
     """mdf_iters = 0 calls between coupled calls (flushes the marker sets, flips the buffer parity)."""
     from paper_1904_02108_b200 import workloads
