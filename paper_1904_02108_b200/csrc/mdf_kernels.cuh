@@ -775,6 +775,9 @@ __device__ __forceinline__ void moments_cell(const float *__restrict__ src, cons
     U[cell] = make_float4(ux, uy, uz, 1.0f + drho);
 }
 
+#ifndef MDFP_MINB_CFG
+#define MDFP_MINB_CFG 2
+#endif
 #ifndef MDFP_WARPS_CFG
 #define MDFP_WARPS_CFG 8
 #endif
@@ -792,7 +795,7 @@ struct WordsArgs {
 };
 
 template <int TR>
-__global__ void __launch_bounds__(MDFP_WARPS * 32, 2)
+__global__ void __launch_bounds__(MDFP_WARPS * 32, MDFP_MINB_CFG)
 k_mdf_persistent(const __grid_constant__ MdfArgs a, const float *__restrict__ src, const __grid_constant__ PlaneOffsets po,
                  int *__restrict__ cursors, unsigned *__restrict__ bar, int mdf_iters, int warp_smem,
                  const __grid_constant__ WordsArgs wa)
