@@ -100,8 +100,11 @@ __device__ __forceinline__ Placed place_marker(const BodyDef &d, const BodyStep 
 // a2: cell key of every marker (original order): key = (cz ny + cy) nx + cx  (O3).
 __global__ void __launch_bounds__(256)
 k_marker_keys(MarkerIn m, const BodyDef *__restrict__ defs, const BodyStep *__restrict__ tabs, Geom g,
-              unsigned *__restrict__ keys, int *__restrict__ status)
+              unsigned *__restrict__ keys, int *__restrict__ status, long long *__restrict__ advance_ctr)
 {
+    // advance_ctr != NULL: this launch follows the only k_kinematics of its step graph in the same chain, so the
+    // device-side time-step counter (read by k_kinematics alone) can advance here instead of in a kernel of its own
+    if (advance_ctr && blockIdx.x == 0 && threadIdx.x == 0) *advance_ctr += 1;
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= m.n) return;
     const int b = m.body[k];

@@ -670,7 +670,8 @@ int upload_markers(lbm *h)
 // a1-a3 for the time step (device step counter + step_offset) into marker set S.  parts: bit 0 = first half
 // (kinematics tables, keys, sort), bit 1 = second half (gather, chunks, tiles, active cells, collect plan).
 enum { PREP_SORT = 1, PREP_BINS = 2, PREP_ALL = 3 };
-int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_kernels, PhaseTimer *pt, int parts = PREP_ALL)
+int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_kernels, PhaseTimer *pt, int parts = PREP_ALL,
+                 bool advance_step = false)
 {
     const Geom &g = h->g;
     const int n = h->nm;
@@ -690,7 +691,8 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
     const int nb = (int)h->bodies.size();
     k_kinematics<<<(std::max(nb, N_STEP_COUNTERS) + 127) / 128, 128, 0, s>>>(h->d_defs, S.tabs, nb, &h->scal->step_ctr,
                                                                               step_offset, &sc->n_words, N_STEP_COUNTERS);
-    k_marker_keys<<<mb, 256, 0, s>>>(mi, h->d_defs, S.tabs, g, S.keys[0], &h->scal->status);
+    k_marker_keys<<<mb, 256, 0, s>>>(mi, h->d_defs, S.tabs, g, S.keys[0], &h->scal->status,
+                                     advance_step ? &h->scal->step_ctr : nullptr);
     nk += 3;
     if (pt) pt->mark(PH_SORT, s);
     if (n <= SORT_SMALL_MAX) {
@@ -983,8 +985,11 @@ int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, PrepSet 
     }
     if ((rc = enqueue_prep(h, h->cap_prep, N, 1, &nk, nullptr, n_has_sort ? PREP_BINS : PREP_ALL))) return rc;
     trace_mark(h, h->cap_prep, "prep");
+    // steady state of the depth-2 pipeline with the persistent kernel: the only reader of the step counter in this
+    // graph is the k_kinematics of the prep2 chain, and the counter advances right behind it in that chain
+    const bool ctr_in_prep2 = fold && N2 && n_has_sort;
     if (N2) {
-        if ((rc = enqueue_prep(h, h->cap_prep2, *N2, 2, &nk, nullptr, PREP_SORT))) return rc;
+        if ((rc = enqueue_prep(h, h->cap_prep2, *N2, 2, &nk, nullptr, PREP_SORT, ctr_in_prep2))) return rc;
         trace_mark(h, h->cap_prep2, "prep2");
     }
     if (split && !pdl) CK(cudaEventRecord(h->ev_bulk, h->cap_bulk));
@@ -997,8 +1002,7 @@ int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, PrepSet 
     if (N2) CK(cudaStreamWaitEvent(s, h->ev_prep2, 0));
     if (fold) {
         trace_mark(h, s, "join");
-        k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, nullptr, 0, 4);
-        ++nk;
+        if (!ctr_in_prep2) { k_set_scalars<<<1, 1, 0, s>>>(&h->scal->step_ctr, 0, nullptr, 0, 4); ++nk; }
     } else if (split) {
         trace_mark(h, s, "join");
         if ((rc = enqueue_lbm_active(h, s, src, dst, S))) return rc;           // also advances the step counter
