@@ -20,7 +20,9 @@
 //
 // Small marker sets (a single propeller) run the whole loop -- moments, N x (tile pass, collect) -- as
 // ONE persistent kernel with grid-wide barriers instead of 2N + 1 dependent launches, on tiles of a
-// single source row (TR = 1) so that a few thousand markers still spread over all SMs.
+// single source row (TR = 1) so that a few thousand markers still spread over all SMs.  That kernel also
+// updates the lattice cells inside the stencils once G is complete, and it releases the lattice-wide
+// stream-collide pass that runs beside it (its programmatic dependent) as soon as all its blocks are resident.
 #pragma once
 #include "ibm_kernels.cuh"
 
