@@ -20,13 +20,12 @@ struct BodyStep {
     float dR[9];   // R(omega (n+1)) - R(omega n), formed in fp64 (R12)
 };
 
-struct MarkerIn {                  // original (caller) order, SoA
-    const float *qx, *qy, *qz;     // rest position relative to the body centre, p_k - c (fp64 -> fp32)
-    const float *vx, *vy, *vz;     // extra velocity vel_k (R14)
-    const float *s;                // area s(k)
-    const int *body;
-    int n;
-};
+struct MarkerIn {                  // original (caller) order
+    const float4 *qs;              // (rest position relative to the body centre p_k - c (fp64 -> fp32), area s(k))
+    const float4 *vb;              // (extra velocity vel_k (R14), body id as int bits)
+    const int *body;               // body id once more, for the kernels that read in caller order
+    int n;                         // two 16-byte records per marker: the gather by the sort permutation touches
+};                                 // two sectors per marker instead of eight
 
 // a1: Rodrigues rotation tables of every body for step n -> n+1, in fp64 (R12, R13).
 // Also re-arms the per-step device counters of the marker set being prepared.  step_offset = 1
@@ -108,7 +107,8 @@ k_marker_keys(MarkerIn m, const BodyDef *__restrict__ defs, const BodyStep *__re
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= m.n) return;
     const int b = m.body[k];
-    const Placed p = place_marker(defs[b], tabs[b], m.qx[k], m.qy[k], m.qz[k], g);
+    const float4 q = __ldg(m.qs + k);
+    const Placed p = place_marker(defs[b], tabs[b], q.x, q.y, q.z, g);
     if (p.bad) *status = 1;
     keys[k] = (unsigned)((p.cz * g.ny + p.cy) * g.nx + p.cx);
 }
@@ -145,15 +145,16 @@ k_marker_gather(MarkerIn m, const BodyDef *__restrict__ defs, const BodyStep *__
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m.n) return;
     const int k = perm[i];
-    const int b = m.body[k];
+    const float4 q = __ldg(m.qs + k), v = __ldg(m.vb + k);
+    const int b = __float_as_int(v.w);
     const BodyStep t = tabs[b];
-    const float qx = m.qx[k], qy = m.qy[k], qz = m.qz[k];
+    const float qx = q.x, qy = q.y, qz = q.z;
     const Placed p = place_marker(defs[b], t, qx, qy, qz, g);
-    out.fs[i] = make_float4(p.fx, p.fy, p.fz, m.s[k]);
+    out.fs[i] = make_float4(p.fx, p.fy, p.fz, q.w);
 
-    const float ux = fmaf(t.dR[0], qx, fmaf(t.dR[1], qy, fmaf(t.dR[2], qz, m.vx[k])));
-    const float uy = fmaf(t.dR[3], qx, fmaf(t.dR[4], qy, fmaf(t.dR[5], qz, m.vy[k])));
-    const float uz = fmaf(t.dR[6], qx, fmaf(t.dR[7], qy, fmaf(t.dR[8], qz, m.vz[k])));
+    const float ux = fmaf(t.dR[0], qx, fmaf(t.dR[1], qy, fmaf(t.dR[2], qz, v.x)));
+    const float uy = fmaf(t.dR[3], qx, fmaf(t.dR[4], qy, fmaf(t.dR[5], qz, v.y)));
+    const float uz = fmaf(t.dR[6], qx, fmaf(t.dR[7], qy, fmaf(t.dR[8], qz, v.z)));
     out.uk[i] = make_float4(ux, uy, uz, 0.f);
     out.du[i] = make_float4(0.f, 0.f, 0.f, __int_as_float(p.cx));
     if (!out.sg) return;                             // the fused tile pass (mdf_kernels.cuh) needs no tables
@@ -1252,7 +1253,8 @@ k_body_boxes(MarkerIn m, const BodyDef *__restrict__ defs, const BodyStep *__res
     const int b = m.body[k];
     const BodyDef d = defs[b];
     const BodyStep t = tabs[b];
-    const float qx = m.qx[k], qy = m.qy[k], qz = m.qz[k];
+    const float4 q4 = __ldg(m.qs + k);
+    const float qx = q4.x, qy = q4.y, qz = q4.z;
     const float dx = fmaf(t.R[0], qx, fmaf(t.R[1], qy, fmaf(t.R[2], qz, d.cf[0])));
     const float dy = fmaf(t.R[3], qx, fmaf(t.R[4], qy, fmaf(t.R[5], qz, d.cf[1])));
     const float dz = fmaf(t.R[6], qx, fmaf(t.R[7], qy, fmaf(t.R[8], qz, d.cf[2])));

@@ -184,7 +184,7 @@ struct lbm {
     std::vector<BodyDef> h_defs;        // host copy of the per-body device table
     bool markers_stale = true;          // device copies / graphs need rebuilding
     int nm = 0, nm_cap = 0, nb_cap = 0;
-    float *d_q[3] = {nullptr, nullptr, nullptr}, *d_v[3] = {nullptr, nullptr, nullptr}, *d_s = nullptr;
+    float4 *d_qs = nullptr, *d_vb = nullptr;   // (p - c, s) and (vel, body id) per marker, caller order
     int *d_body = nullptr;
     BodyDef *d_defs = nullptr;
     int *d_hist[N_SETS] = {nullptr, nullptr, nullptr}, *d_total[N_SETS] = {nullptr, nullptr, nullptr};   // radix scratch, one per marker set (two binnings run side by side)
@@ -332,8 +332,7 @@ void free_set(lbm *h, PrepSet &S)
 void free_markers_dev(lbm *h)
 {
     const size_t c = (size_t)h->nm_cap;
-    for (int a = 0; a < 3; ++a) { dfree(h, h->d_q[a], c); dfree(h, h->d_v[a], c); }
-    dfree(h, h->d_s, c);
+    dfree(h, h->d_qs, c); dfree(h, h->d_vb, c);
     dfree(h, h->d_body, c);
     for (PrepSet &S : h->set) free_set(h, S);
     h->cells_cap = 0; h->headbits_cap = 0;
@@ -563,11 +562,8 @@ int upload_markers(lbm *h)
         h->tg = tile_geom(h->g.ny, h->g.nz, tr);
         h->tile_slots = (size_t)h->cg.nbx * h->tg.nty * h->tg.ntz;
         const size_t c = (size_t)n;
-        for (int a = 0; a < 3; ++a) {
-            if ((rc = dmalloc(h, &h->d_q[a], c))) return rc;
-            if ((rc = dmalloc(h, &h->d_v[a], c))) return rc;
-        }
-        if ((rc = dmalloc(h, &h->d_s, c))) return rc;
+        if ((rc = dmalloc(h, &h->d_qs, c))) return rc;
+        if ((rc = dmalloc(h, &h->d_vb, c))) return rc;
         if ((rc = dmalloc(h, &h->d_body, c))) return rc;
         // every chunk that can exist gets a table entry (one per marker, one per (row, block) slot, CHUNK_ID_MAX);
         // F has room for every tile that can exist up to 12 GB, beyond that the capacity is capped and an
@@ -634,8 +630,7 @@ int upload_markers(lbm *h)
     // body tables; rest positions relative to the body centre, formed in fp64
     std::vector<BodyDef> &defs = h->h_defs;
     defs.assign((size_t)nb, BodyDef{});
-    std::vector<float> q[3], v[3];
-    for (int a = 0; a < 3; ++a) { q[a].resize((size_t)n); v[a].resize((size_t)n); }
+    std::vector<float4> qs((size_t)n), vb((size_t)n);
     for (int b = 0; b < nb; ++b) {
         const HostBody &B = h->bodies[(size_t)b];
         BodyDef d{};
@@ -647,17 +642,17 @@ int upload_markers(lbm *h)
             if (d.cf[a] >= 1.0f) { d.cf[a] = 0.0f; d.ci[a] += 1; }
         }
         defs[(size_t)b] = d;
-        for (long long k = B.first; k < B.first + B.count; ++k)
-            for (int a = 0; a < 3; ++a) {
-                q[a][(size_t)k] = (float)((double)h->h_pos[(size_t)(3 * k + a)] - B.center[a]);
-                v[a][(size_t)k] = h->h_vel[(size_t)(3 * k + a)];
-            }
+        for (long long k = B.first; k < B.first + B.count; ++k) {
+            const size_t i = (size_t)k;
+            float bits;
+            std::memcpy(&bits, &b, sizeof bits);
+            qs[i] = make_float4((float)((double)h->h_pos[3 * i] - B.center[0]), (float)((double)h->h_pos[3 * i + 1] - B.center[1]),
+                                (float)((double)h->h_pos[3 * i + 2] - B.center[2]), h->h_area[i]);
+            vb[i] = make_float4(h->h_vel[3 * i], h->h_vel[3 * i + 1], h->h_vel[3 * i + 2], bits);
+        }
     }
-    for (int a = 0; a < 3; ++a) {
-        CK(cudaMemcpyAsync(h->d_q[a], q[a].data(), sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, h->stream));
-        CK(cudaMemcpyAsync(h->d_v[a], v[a].data(), sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, h->stream));
-    }
-    CK(cudaMemcpyAsync(h->d_s, h->h_area.data(), sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaMemcpyAsync(h->d_qs, qs.data(), sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, h->stream));
+    CK(cudaMemcpyAsync(h->d_vb, vb.data(), sizeof(float4) * (size_t)n, cudaMemcpyHostToDevice, h->stream));
     CK(cudaMemcpyAsync(h->d_body, h->h_body.data(), sizeof(int) * (size_t)n, cudaMemcpyHostToDevice, h->stream));
     CK(cudaMemcpyAsync(h->d_defs, defs.data(), sizeof(BodyDef) * (size_t)nb, cudaMemcpyHostToDevice, h->stream));
     CK(cudaStreamSynchronize(h->stream));   // staging vectors die here
@@ -679,7 +674,7 @@ int enqueue_prep(lbm *h, cudaStream_t s, PrepSet &S, int step_offset, int *n_ker
     SetScalars *sc = S.scal;
     unsigned *skey = S.keys[h->sort_passes & 1];
     int *perm = S.vals[h->sort_passes & 1];
-    MarkerIn mi{h->d_q[0], h->d_q[1], h->d_q[2], h->d_v[0], h->d_v[1], h->d_v[2], h->d_s, h->d_body, n};
+    MarkerIn mi{h->d_qs, h->d_vb, h->d_body, n};
     int nk = 0;
     const int lg = list_grid(h);
 
@@ -786,7 +781,7 @@ int enqueue_mdf(lbm *h, cudaStream_t s, PrepSet &S, const float *src, int mdf_it
     if (h->opt_moments == 1) {
         // the paper's box strategy: U on the bounding box of every body
         const int nb = (int)h->bodies.size();
-        MarkerIn mi{h->d_q[0], h->d_q[1], h->d_q[2], h->d_v[0], h->d_v[1], h->d_v[2], h->d_s, h->d_body, n};
+        MarkerIn mi{h->d_qs, h->d_vb, h->d_body, n};
         k_reset_boxes<<<(nb + 127) / 128, 128, 0, s>>>(h->d_box, nb);
         k_body_boxes<<<(n + 255) / 256, 256, 0, s>>>(mi, h->d_defs, S.tabs, h->d_box);   // the set's own tables
         k_moments_box<<<dim3(64, nb), 256, 0, s>>>(src, g, h->d_box, h->U);

@@ -22,7 +22,7 @@ def test_bench_line_has_the_contract_keys():
         assert k in d, k
     assert d["unit"] == "MLUPS" and d["n_gpus"] == 1 and d["steps"] == 20 and d["dtype"] == "f32" and d["vs_baseline"] is None
     assert d["config"]["workload"] == "W3" and "model" not in d["config"]
-    assert d["gpu_launches"] > 20 * 20                 # a coupled step is ~40 kernels of this library
+    assert d["gpu_launches"] > 20 * 15                 # a coupled W3 step is ~20 kernels of this library (one of them the whole MDF loop)
     r = d["roofline"]
     assert r["bound"] == "hbm" and r["unit"] == "GB/s" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
     assert 0.3 < r["frac"] < 1.2
