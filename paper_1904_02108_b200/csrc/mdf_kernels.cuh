@@ -502,25 +502,45 @@ k_mdf_tiles(const __grid_constant__ MdfArgs a, int *__restrict__ cursor, int las
     });
 }
 
-// ---- two warps per tile -------------------------------------------------------------------------------------
-// A block is ONE pair of warps that share a tile's window and footprint (half the shared memory per warp of the
-// one-warp pass, so 20 instead of 12 warps fit on an SM) and take its batches of 32 markers in turn: in time
-// slot s the warp that owns batch s interpolates it (phase 1, into its own staging buffer) while the other warp
-// sweeps batch s - 1 (phase 2) into the shared footprint; a block barrier ends the slot.  The sweeps therefore
-// still follow one another in sorted order -- every sum keeps its fixed order -- and the shared-memory-heavy
-// interpolation of one warp overlaps the FMA-heavy sweep of the other.  Each sweep starts with an empty window
-// and ends with a full flush.
+// ---- two warps per tile ---------------------------------------------------------------------------------------
+// A block is ONE pair of warps on one tile.  The tile's source rows are cut at the row where the marker count
+// reaches half the tile's: warp 0 takes the rows up to it, warp 1 the rest.  The two share the tile's window of U^m
+// (read only) and otherwise work on their own: each interpolates and sweeps ITS rows' markers, 32 at a time, into a
+// footprint of its own; the write-out adds the two footprints (warp 0's first: the order is fixed) and hands the
+// elements to the cells.  No barrier inside the tile, two around it.  Against one warp per tile: the longest tile
+// takes half as long (the tail of the pass), and 16 instead of 12 warps fit on an SM (28 KB per pair at TR = 4).
 inline size_t mdf_pair_smem(int tr, const ChunkGeom &cg)
 {
     const size_t tf = (size_t)tr + 3;
     const size_t win = (tf * tf * (size_t)cg.ent * 16 + 127) / 128 * 128;
     const size_t foot = (tf * tf * (size_t)cg.ent * 12 + 127) / 128 * 128;
-    return win + foot + 2 * MDF_STAGE_BYTES;
+    return win + 2 * (foot + MDF_STAGE_BYTES);
 }
 
 #ifndef MDF_PAIR_MIN_BLOCKS_CFG
-#define MDF_PAIR_MIN_BLOCKS_CFG 10
+#define MDF_PAIR_MIN_BLOCKS_CFG 8
 #endif
+
+// footprint elements of the rows fy = part, part + 2, ...: the sum of the two warps' footprints goes to the cells
+template <int TR>
+__device__ __forceinline__ void pair_writeout(const MdfArgs &a, const TileHdr &H, const float *foot0, const float *foot1,
+                                              const int lane, const int part)
+{
+    using D = TileDims<TR>;
+    const int ent = a.cg.ent;
+    const int l = lane & 15, h = lane >> 4;
+    TileDst<TR> d;
+    tile_load_dst<TR>(a, H, lane, part, 2, d);
+#pragma unroll
+    for (int fy = 0; fy < D::TF; ++fy)
+#pragma unroll
+        for (int k = 0; k < D::KZ; ++k)
+            if (d.o[fy][k] >= 0) {
+                const int off = ((fy * D::TF + 2 * k + h) * ent + l) * 3;
+                __stcg(a.F + d.o[fy][k], make_float4(foot0[off] + foot1[off], foot0[off + 1] + foot1[off + 1],
+                                                      foot0[off + 2] + foot1[off + 2], 0.f));
+            }
+}
 
 template <int TR>
 __global__ void __launch_bounds__(64, MDF_PAIR_MIN_BLOCKS_CFG)
@@ -535,8 +555,10 @@ k_mdf_pairs(const __grid_constant__ MdfArgs a, int *__restrict__ cursor, int las
     const int nt = min(*a.n_tiles, a.tile_cap);
     const int ent = a.cg.ent;
     const size_t win_bytes = tile_win_bytes(D::NROWS, ent), foot_bytes = tile_foot_bytes(D::NROWS, ent);
-    const TileSmem sm = stage_at(reinterpret_cast<float4 *>(smem), reinterpret_cast<float *>(smem + win_bytes),
-                                 smem + win_bytes + foot_bytes + (size_t)w * MDF_STAGE_BYTES);
+    float *foot0 = reinterpret_cast<float *>(smem + win_bytes);
+    float *foot1 = reinterpret_cast<float *>(smem + win_bytes + foot_bytes);
+    const TileSmem sm = stage_at(reinterpret_cast<float4 *>(smem), w ? foot1 : foot0,
+                                 smem + win_bytes + 2 * foot_bytes + (size_t)w * MDF_STAGE_BYTES);
     if (threadIdx.x == 0) { const int t = atomicAdd(cursor, 1); s_pos[0] = t < nt ? t : -1; }
     __syncthreads();
     for (int it = 0;; ++it) {
@@ -546,45 +568,54 @@ k_mdf_pairs(const __grid_constant__ MdfArgs a, int *__restrict__ cursor, int las
         if (threadIdx.x == 0) { const int t = atomicAdd(cursor, 1); s_pos[(it + 1) & 1] = t < nt ? t : -1; }
         TileHdr H;
         tile_load_hdr<TR>(a, pos, lane, H);
-        const int total = H.total;
-        const int nbatch = (total + MDF_BATCH - 1) / MDF_BATCH;
         tile_issue_window<TR>(a, H, sm.win, lane, w, 2);
+        // this warp's rows: up to and including the row where the inclusive count reaches half the tile (warp 0),
+        // the rows behind it (warp 1); the header keeps only those, with their prefix redone
+        {
+            const int half = (H.total + 1) >> 1;
+            const unsigned ge = __ballot_sync(FULL, lane < D::NR && H.incl >= half);
+            const int b = ge ? __ffs(ge) - 1 : D::NR - 1;
+            const bool keep = w == 0 ? lane <= b : lane > b;
+            if (!keep) { H.rec.y = H.rec.x; H.cnt = 0; }
+            H.incl = H.cnt;
+#pragma unroll
+            for (int o = 1; o < D::NRP; o <<= 1) {
+                const int v = __shfl_up_sync(FULL, H.incl, o);
+                if (lane >= o) H.incl += v;
+            }
+            H.total = __shfl_sync(FULL, H.incl, D::NRP - 1);
+        }
+        const int total = H.total;
         MarkerRegs cur;
-        if (w < nbatch) tile_fetch<TR>(a, H, w * MDF_BATCH, lane, cur);      // this warp's first batch
+        if (total > 0) tile_fetch<TR>(a, H, 0, lane, cur);
         {
             float4 *f4 = reinterpret_cast<float4 *>(sm.foot);
             const int n4 = (int)(foot_bytes / 16);
-            for (int i = threadIdx.x; i < n4; i += 64) f4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int i = lane; i < n4; i += 32) f4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
         cp_async_wait_all();
-        __syncthreads();
-        unsigned chg = 0u, rowchg = 0u;
-        int nb_staged = 0;
-        for (int s = 0; s <= nbatch; ++s) {
-            if ((s & 1) == w) {
-                if (s < nbatch) {
-                    // phase 1 of batch s
-                    const int base = s * MDF_BATCH;
-                    const int nb = min(MDF_BATCH, total - base);
-                    int tag = -2;
-                    if (lane < nb) tag = tile_phase1<TR>(a, H, cur, last, sm, lane);
-                    const int prev_tag = __shfl_up_sync(FULL, tag, 1);
-                    chg = __ballot_sync(FULL, lane < nb && (lane == 0 || tag != prev_tag));
-                    rowchg = __ballot_sync(FULL, lane < nb && (lane == 0 || ((tag ^ prev_tag) >> 8) != 0));
-                    nb_staged = nb;
-                    if (s + 2 < nbatch) tile_fetch<TR>(a, H, base + 2 * MDF_BATCH, lane, cur);   // this warp's next batch
-                }
-            } else if (s >= 1) {
-                // phase 2 of batch s - 1 (staged by this warp in the previous slot)
-                SweepState st;
-                st.started = 0; st.e = 0; st.frow = sm.foot;
-                st.p = Acc3{0.f, 0.f, 0.f}; st.q = Acc3{0.f, 0.f, 0.f};
-                tile_sweep<TR>(sm, ent, nb_staged, chg, rowchg, st, lane);
-                sweep_close(st, lane);
-            }
-            __syncthreads();
+        __syncthreads();                                 // the window is complete (both warps' copies)
+        SweepState st;
+        st.started = 0; st.e = 0; st.frow = sm.foot;
+        st.p = Acc3{0.f, 0.f, 0.f}; st.q = Acc3{0.f, 0.f, 0.f};
+        int tag_cur = -1;
+        for (int base = 0; base < total; base += MDF_BATCH) {
+            const int nb = min(MDF_BATCH, total - base);
+            int tag = -2;
+            if (lane < nb) tag = tile_phase1<TR>(a, H, cur, last, sm, lane);
+            const int prev_tag = __shfl_up_sync(FULL, tag, 1);
+            const int before = lane == 0 ? tag_cur : prev_tag;
+            const unsigned chg = __ballot_sync(FULL, lane < nb && tag != before);
+            const unsigned rowchg = __ballot_sync(FULL, lane < nb && ((tag ^ before) >> 8) != 0);
+            tag_cur = __shfl_sync(FULL, tag, nb - 1);
+            __syncwarp();
+            if (base + MDF_BATCH < total) tile_fetch<TR>(a, H, base + MDF_BATCH, lane, cur);   // in flight during the sweep
+            tile_sweep<TR>(sm, ent, nb, chg, rowchg, st, lane);
+            __syncwarp();
         }
-        tile_writeout<TR>(a, H, sm.foot, lane, w, 2);
+        sweep_close(st, lane);
+        __syncthreads();                                 // both footprints are complete, nobody reads the window any more
+        pair_writeout<TR>(a, H, foot0, foot1, lane, w);
         __syncthreads();
     }
 }
