@@ -114,6 +114,16 @@ enum {
                              footprint of its own and the write-out adds the two (measured comparison: 16 instead
                              of 12 warps per SM and half the longest tile, no faster: the pass is bound by the
                              shared-memory pipe).  Results agree to rounding (summation order).               */
+    LBM_OPT_PIPELINE = 16, /* depth of the binning pipeline of the overlapped step (three marker sets are used in
+                             turn): 2 = the step's graph bins the second half of step n + 1 (gather, chunks, tiles,
+                             active cells, collect plan) and, in a branch of its own, the first half of step n + 2
+                             (kinematics, keys, sort); 1 = it bins all of step n + 1 in one branch; 0 (default) = 2
+                             up to 400,000 markers, else 1.  Results are bit-identical.                         */
+    LBM_OPT_TRACE = 15,   /* 1 = the graph of the overlapped step also records a timing event after every kernel of
+                             the MDF branch, after the bulk stream-collide and after the binning branches; after
+                             lbm_sync, lbm_get_info(LBM_INFO_TRACE_NS + i) is the device time in ns from the fork
+                             of the LAST step to event i and lbm_trace_label(i) names it.  A profiling aid
+                             (the timeline of the concurrent branches); results do not depend on it.          */
     LBM_OPT_MDF_BLOCKS = 13 /* tuning: blocks per SM of the tile pass / of the persistent MDF kernel (0 = default:
                              as many as fit / one); fewer blocks leave more of every SM to the stream-collide
                              pass that runs beside the MDF loop.  Results do not depend on it.           */
