@@ -544,6 +544,82 @@ def test_tile_table_overflow_is_flagged_not_fatal(api, orc):
     sim.close()
 
 
+def _random_static_markers(rng, n, nx, ny, nz, area):
+    pos = np.stack([rng.uniform(0, nx, n), rng.uniform(0, ny, n), rng.uniform(0, nz, n)], axis=1).astype(np.float32)
+    vel = rng.normal(scale=0.01, size=(n, 3)).astype(np.float32)
+    return pos, vel, np.full(n, area, np.float32)
+
+
+def _pair(api, orc, nx, ny, nz):
+    return api.LbmIbm(nx, ny, nz, 0.8, wall=(0, 0, 0), stream=_stream()), orc.Oracle(nx, ny, nz, 0.8, wall=(0, 0, 0))
+
+
+def _marker_forces_agree(sim, ref):
+    mk, rm = sim.read_markers(), ref.read_markers()
+    assert np.abs(mk["force"] - rm["du"]).max() <= TOL_F * np.abs(rm["du"]).max()
+
+
+def test_degenerate_marker_sets(api, orc):
+    """The degenerate cases of the method: one marker; 1500 markers inside ONE cell (several 32-marker batches in a
+    single chunk, 100 of them exactly on a cell face); a lattice so small that every stencil wraps onto its own
+    tile; a set replaced by a larger one in mid-run, then cleared; nsteps = 0."""
+    rng = np.random.default_rng(5)
+    sim, ref = _pair(api, orc, 24, 20, 16)
+    one = (np.array([[7.3, 9.9, 4.1]], np.float32), np.array([[0.02, -0.01, 0.015]], np.float32), np.array([0.25], np.float32))
+    sim.set_markers(*one); ref.set_markers(*one)
+    sim.step(20, 3); ref.step(20, 3); sim.sync()
+    _compare_fields(sim, ref); _marker_forces_agree(sim, ref)
+    sim.close()
+
+    sim, ref = _pair(api, orc, 24, 20, 16)
+    n = 1500
+    pos = (np.array([11.0, 8.0, 6.0]) + rng.uniform(0, 1, (n, 3))).astype(np.float32)
+    pos[:50, 0] = 11.0
+    pos[50:100, 1] = 8.0
+    vel = rng.normal(scale=0.01, size=(n, 3)).astype(np.float32)
+    area = np.full(n, 0.01, np.float32)
+    sim.set_markers(pos, vel, area); ref.set_markers(pos, vel, area)
+    sim.step(10, 5); ref.step(10, 5); sim.sync()
+    _compare_fields(sim, ref); _marker_forces_agree(sim, ref)
+    sim.close()
+
+    sim, ref = _pair(api, orc, 8, 4, 4)
+    m = _random_static_markers(rng, 60, 8, 4, 4, 0.05)
+    sim.set_markers(*m); ref.set_markers(*m)
+    sim.step(20, 3); ref.step(20, 3); sim.sync()
+    _compare_fields(sim, ref); _marker_forces_agree(sim, ref)
+    sim.close()
+
+    sim, ref = _pair(api, orc, 24, 20, 16)
+    for n in (100, 3000):
+        m = _random_static_markers(rng, n, 24, 20, 16, 0.02)
+        sim.clear(); ref.clear_markers()
+        sim.set_markers(*m); ref.set_markers(*m)
+        sim.step(7, 4); ref.step(7, 4); sim.sync()
+        _compare_fields(sim, ref); _marker_forces_agree(sim, ref)
+    sim.clear(); ref.clear_markers()
+    sim.step(5, 0); ref.step(5, 0); sim.sync()
+    _compare_fields(sim, ref)
+    before = sim.read_fields()
+    sim.step(0, 3); sim.sync()
+    for a, b in zip(before, sim.read_fields()):
+        assert np.array_equal(a, b)
+    sim.close()
+
+
+@pytest.mark.parametrize("iters", [1, 17, 64])
+def test_mdf_iteration_counts_from_one_to_the_maximum(api, orc, iters):
+    """P:110 fixes 5 iterations; the loop is generic: 1 (interpolate once, spread Delta u once, R11), an odd count,
+    and the library's maximum of 64."""
+    rng = np.random.default_rng(7)
+    sim, ref = _pair(api, orc, 20, 16, 12)
+    m = _random_static_markers(rng, 200, 20, 16, 12, 0.05)
+    sim.set_markers(*m); ref.set_markers(*m)
+    sim.step(5, iters); ref.step(5, iters); sim.sync()
+    _compare_fields(sim, ref); _marker_forces_agree(sim, ref)
+    sim.close()
+
+
 def test_error_paths(api):
     with pytest.raises(api.LbmError):
         api.LbmIbm(8, 8, 8, 0.5)
