@@ -240,6 +240,26 @@ int ibm_wait_markers(lbm_t *h);
  * beyond the 12 GB footprint cap; the excess chunks were dropped). */
 int lbm_sync(lbm_t *h);
 
+/* Marker binning (a3: the stable sort by owning lattice cell the paper suggests) WITHOUT any allocation, for
+ * callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it).  Needs no handle.  cell [n]: cell key of every marker, each < ncells (DEVICE pointer, not modified);
+ * cell_sorted [n]: the keys in ascending order; perm [n]: perm[j] = index of the marker that holds rank j, equal keys
+ * in ascending index order (the unique stable permutation, R20) -- both DEVICE pointers owned by the caller, and
+ * the same result, bit for bit, as the permutation the handle-based path reports through ibm_read_markers.
+ * The work (3 kernels per 8-bit pass, ceil(log2(ncells) / 8) passes) is enqueued on `cuda_stream` (a cudaStream_t, NULL
+ * = the default stream); the call does not synchronise and calls no cudaMalloc / cudaFree or allocating library
+ * routine.  The scratch of the sort (digit histograms, one ping-pong copy of keys and values) is a file-scope device
+ * array of 3 MiB + 1 KiB that every GPU which loads the library holds until the process exits; its size fixes the
+ * limit: n > IBM_NOALLOC_MAX_MARKERS returns LBM_ERANGE (use the handle-based path for larger sets).  n = 0 is a
+ * no-op.  All calls on a device SHARE that array: calls whose kernels may overlap on the GPU (different streams
+ * without an ordering between them, or different host threads) RACE on it -- keep them on one stream or order them
+ * with events.  The array keeps the last call's contents; nothing in it has to start at zero (every word a call reads
+ * it has written before).  Errors: LBM_EINVAL (n < 0, ncells out of 1..2^32, NULL or host pointers, cell_sorted
+ * aliasing cell), LBM_ERANGE (n beyond the maximum), LBM_ECUDA. */
+#define IBM_NOALLOC_MAX_MARKERS 262144
+int ibm_sort_cells_noalloc(const unsigned *cell /* device */, int n, long long ncells, unsigned *cell_sorted /* device */,
+                           int *perm /* device */, void *cuda_stream);
+
 /* Text of the last error raised on the calling thread ("" if none). */
 const char *lbm_last_error(void);
 

@@ -38,7 +38,7 @@ FORCING_GUO, FORCING_SHIFT = 0, 1
 EXPORTS = ["lbm_create", "lbm_destroy", "lbm_query_layout", "lbm_set_stream", "lbm_set_option", "lbm_get_info", "lbm_set_fields",
            "ibm_set_markers", "ibm_set_kinematics", "ibm_update_kinematics", "ibm_clear", "lbm_ibm_step", "lbm_read_fields",
            "ibm_read_markers", "ibm_read_markers_async", "ibm_wait_markers", "lbm_sync", "lbm_last_error",
-           "lbm_trace_label"]
+           "lbm_trace_label", "ibm_sort_cells_noalloc"]
 
 
 class _Bc(C.Structure):
@@ -70,6 +70,8 @@ _L.lbm_last_error.restype = C.c_char_p
 _L.lbm_last_error.argtypes = []
 _L.lbm_trace_label.restype = C.c_char_p
 _L.lbm_trace_label.argtypes = [_vp, C.c_int]
+_L.ibm_sort_cells_noalloc.argtypes = [_vp, C.c_int, C.c_longlong, _vp, _vp, _vp]
+NOALLOC_MAX_MARKERS = 262144     # IBM_NOALLOC_MAX_MARKERS of include/lbm_ibm.h
 
 
 class LbmError(RuntimeError):
@@ -251,6 +253,20 @@ class LbmIbm:
 
     def wait_markers(self):
         _check(_L.ibm_wait_markers(self._h), "ibm_wait_markers")
+
+
+def sort_cells_noalloc(cell, ncells, cell_sorted, perm, stream=None):
+    """ibm_sort_cells_noalloc: cell (device tensor, n 32-bit keys < ncells) -> cell_sorted, perm (device tensors of n
+    32-bit words, written in place).  Enqueued on `stream` (a torch.cuda.Stream, None = the default stream); allocates
+    nothing; at most NOALLOC_MAX_MARKERS keys; calls that overlap on the GPU race on the library's scratch array."""
+    n = int(cell.numel())
+    for t in (cell, cell_sorted, perm):
+        if t.element_size() != 4 or not t.is_contiguous():
+            raise ValueError("sort_cells_noalloc: contiguous tensors of 32-bit words expected")
+    if cell_sorted.numel() < n or perm.numel() < n:
+        raise ValueError("sort_cells_noalloc: output tensors shorter than the input")
+    _check(_L.ibm_sort_cells_noalloc(cell.data_ptr(), n, int(ncells), cell_sorted.data_ptr(), perm.data_ptr(),
+                                     stream.cuda_stream if stream is not None else None), "ibm_sort_cells_noalloc")
 
 
 def from_workload(wl, stream=None) -> LbmIbm:

@@ -12,6 +12,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <map>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1714,3 +1715,105 @@ int lbm_sync(lbm_t *h)
 }
 
 }  // extern "C"
+
+// ---- a3 without any allocation: ibm_sort_cells_noalloc -------------------------------------------------------------
+// The stable LSD radix sort of the binning (sort_kernels.cuh: k_radix_hist / k_radix_scan / k_radix_scatter, the very
+// kernels the step uses above 32,768 markers) for callers that cannot call cudaMalloc (code under CUDA graph capture,
+// tight serving loops, harnesses that forbid it).  The scratch the sort needs -- the per-sub-tile digit histograms, the
+// digit totals and one ping-pong copy of keys and values -- lives in a file-scope device array of fixed size; every GPU
+// that loads the library holds these 3 MiB + 1 KiB until the process exits.
+//
+// g_noalloc_scratch below is, in HOST code, only a stand-in for the symbol: its address is NOT a device address.  The
+// device address comes from cudaGetSymbolAddress, asked for once per device with that device current
+// (noalloc_scratch_ptr), and that pointer is what the kernels are given.
+namespace {
+
+constexpr int NOALLOC_MAX_MARKERS = 262144;      // stated maximum of ibm_sort_cells_noalloc (IBM_NOALLOC_MAX_MARKERS)
+constexpr int NOALLOC_MAX_TILES = 1024;          // sub-tiles of the sort (one warp each) at the maximum
+struct NoallocScratch {
+    unsigned keys[NOALLOC_MAX_MARKERS];          // ping-pong partner of the caller's key output
+    int vals[NOALLOC_MAX_MARKERS];               // ping-pong partner of the caller's permutation output
+    int hist[RADIX * NOALLOC_MAX_TILES];         // [digit][sub-tile], fully rewritten by every pass
+    int total[RADIX];                            // digit totals, fully rewritten by every pass
+};
+static_assert(NOALLOC_MAX_MARKERS == IBM_NOALLOC_MAX_MARKERS, "lbm_ibm.h states the maximum");
+static_assert(sizeof(NoallocScratch) == 3 * 1048576 + 1024, "the header and README state 3 MiB + 1 KiB");
+
+}  // namespace
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[sizeof(NoallocScratch)];
+
+namespace {
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+NoallocScratch *g_noalloc_ptr[NOALLOC_MAX_DEVICES];       // device address of g_noalloc_scratch on device i, or NULL
+std::mutex g_noalloc_mutex;
+
+// Device address of the scratch array on the CURRENT device (asked for once per device).  No allocation: the array
+// is part of the loaded module.
+int noalloc_scratch_ptr(NoallocScratch **out)
+{
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(LBM_EINVAL, "ibm_sort_cells_noalloc: device ordinal %d not supported", dev);
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+        void *p = nullptr;
+        CK(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        if (!p) return fail(LBM_ECUDA, "ibm_sort_cells_noalloc: cudaGetSymbolAddress returned a NULL address");
+        g_noalloc_ptr[dev] = static_cast<NoallocScratch *>(p);
+    }
+    *out = g_noalloc_ptr[dev];
+    return LBM_OK;
+}
+
+}  // namespace
+
+extern "C" int ibm_sort_cells_noalloc(const unsigned *cell, int n, long long ncells, unsigned *cell_sorted, int *perm,
+                                      void *cuda_stream)
+{
+    if (n < 0) return fail(LBM_EINVAL, "ibm_sort_cells_noalloc: n = %d < 0", n);
+    if (n > NOALLOC_MAX_MARKERS)
+        return fail(LBM_ERANGE, "ibm_sort_cells_noalloc: n = %d exceeds the fixed scratch array (at most %d markers); "
+                                "use the handle-based path (ibm_set_markers + lbm_ibm_step) for larger sets",
+                    n, NOALLOC_MAX_MARKERS);
+    if (ncells < 1 || ncells > (1ll << 32)) return fail(LBM_EINVAL, "ibm_sort_cells_noalloc: ncells = %lld out of range", ncells);
+    if (n == 0) return LBM_OK;
+    if (!cell || !cell_sorted || !perm) return fail(LBM_EINVAL, "ibm_sort_cells_noalloc: NULL buffer");
+    if (!is_device_ptr(cell) || !is_device_ptr(cell_sorted) || !is_device_ptr(perm))
+        return fail(LBM_EINVAL, "ibm_sort_cells_noalloc: cell, cell_sorted and perm must be device pointers");
+    if ((const void *)cell == (const void *)cell_sorted) return fail(LBM_EINVAL, "ibm_sort_cells_noalloc: cell_sorted must not alias cell");
+    NoallocScratch *sc = nullptr;
+    int rc = noalloc_scratch_ptr(&sc);
+    if (rc) return rc;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    // sort geometry: as in the handle-based path, with sub-tiles widened until they fit the fixed histogram table
+    // (the result of a stable sort does not depend on it)
+    int ipw = ((n / (148 * 32)) + 31) / 32 * 32;
+    ipw = std::max(ipw, ((n + NOALLOC_MAX_TILES - 1) / NOALLOC_MAX_TILES + 31) / 32 * 32);
+    ipw = std::min(std::max(ipw, 64), 2048);
+    const int tiles = (n + ipw - 1) / ipw;
+    if (tiles > NOALLOC_MAX_TILES) return fail(LBM_ERANGE, "ibm_sort_cells_noalloc: %d sub-tiles exceed the scratch array", tiles);
+    int bits = 1;
+    while (bits < 32 && (1ll << bits) < ncells) ++bits;
+    const int passes = (bits + 7) / 8;
+    const int sb = (tiles + SORT_WARPS - 1) / SORT_WARPS;
+    // Pass p reads what pass p - 1 wrote (pass 0: the caller's keys, value = index) and writes the caller's outputs
+    // when an even number of passes follows it, else the scratch copy: the last pass always lands in the outputs and
+    // the input is never written.  Nothing in the scratch has to start at zero: every word a pass reads was written
+    // earlier in the same call (hist and total by k_radix_hist / k_radix_scan for all `tiles` sub-tiles and 256
+    // digits, keys / vals by the pass before); what an earlier call left behind is never read.
+    const unsigned *kin = cell;
+    const int *vin = nullptr;
+    for (int p = 0; p < passes; ++p) {
+        const bool to_out = ((passes - 1 - p) & 1) == 0;
+        unsigned *kout = to_out ? cell_sorted : sc->keys;
+        int *vout = to_out ? perm : sc->vals;
+        k_radix_hist<<<sb, SORT_BLOCK, 0, s>>>(kin, n, ipw, tiles, 8 * p, sc->hist);
+        k_radix_scan<<<RADIX, SORT_BLOCK, 0, s>>>(sc->hist, tiles, sc->total);
+        k_radix_scatter<<<sb, SORT_BLOCK, 0, s>>>(kin, vin, kout, vout, n, ipw, tiles, 8 * p, sc->hist, sc->total);
+        kin = kout; vin = vout;
+    }
+    CK(cudaGetLastError());
+    return LBM_OK;
+}
