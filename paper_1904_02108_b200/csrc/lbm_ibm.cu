@@ -573,7 +573,10 @@ int upload_markers(lbm *h)
         const size_t tile_elems = (size_t)((tr + 3) * (tr + 3)) * (size_t)h->cg.ent;
         size_t tcap = std::max((size_t)1, std::min(std::min(c, h->tile_slots), ((size_t)12 << 30) / (tile_elems * sizeof(float4))));
         if (h->opt_tile_cap > 0) tcap = std::max((size_t)1, std::min(tcap, (size_t)h->opt_tile_cap));   // LBM_OPT_TILE_CAP
-        h->cells_cap = std::min((size_t)64 * c, (size_t)h->g.cells);
+        // active cells: a chunk marks the whole x span between the windows of its first and its last marker in 16 rows,
+        // cells between two far-apart markers included: one marker alone activates 64 cells, two markers of a chunk up to
+        // CHUNK_ENT_MAX x 16, i.e. at most 8 x CHUNK_ENT_MAX cells per marker
+        h->cells_cap = std::min((size_t)(8 * CHUNK_ENT_MAX) * c, (size_t)h->g.cells);
         h->headbits_cap = c / 32 + 16;
         for (PrepSet &S : h->set) {
             for (int a = 0; a < 2; ++a) {

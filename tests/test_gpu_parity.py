@@ -607,6 +607,28 @@ def test_degenerate_marker_sets(api, orc):
     sim.close()
 
 
+@pytest.mark.parametrize("opts", [{"tile_rows": 1}, {"tile_rows": 2}, {"tile_rows": 4}, {"tile_rows": 4, "tile_warps": 2},
+                                  {"fused": 0}])
+def test_two_markers_far_apart_in_one_chunk_activate_the_cells_between_them(api, orc, opts):
+    """A chunk (one lattice row, one 8-cell x block) marks the whole x span from its first to its last marker as
+    active: two markers 5 to 7 cells apart activate up to 11 x 16 = 176 cells, more than the 64 per marker the
+    active-cell list was once sized for (found by a randomised differential run; dense propellers never leave such
+    gaps).  Every gap from 0 to 7 cells, for each tile edge and for the round-1 path."""
+    for gap in range(0, 8):
+        sim, ref = _pair(api, orc, 24, 12, 12)
+        pos = np.array([[0.24, 3.55, 2.96], [0.34 + gap, 3.36, 2.36]], np.float32)
+        vel = np.array([[0.01, -0.02, 0.015], [-0.02, 0.01, 0.005]], np.float32)
+        area = np.array([0.25, 0.2], np.float32)
+        sim.set_markers(pos, vel, area); ref.set_markers(pos, vel, area)
+        sim.set_option(api.OPT_PERSISTENT, 2)
+        for k, v in opts.items():
+            sim.set_option(getattr(api, "OPT_" + k.upper()), v)
+        sim.step(3, 3); ref.step(3, 3); sim.sync()
+        assert sim.get_info(api.INFO_ACTIVE_CELLS) == 16 * (4 + gap)
+        _compare_fields(sim, ref); _marker_forces_agree(sim, ref)
+        sim.close()
+
+
 @pytest.mark.parametrize("iters", [1, 17, 64])
 def test_mdf_iteration_counts_from_one_to_the_maximum(api, orc, iters):
     """P:110 fixes 5 iterations; the loop is generic: 1 (interpolate once, spread Delta u once, R11), an odd count,
