@@ -201,14 +201,15 @@ k_bins(const unsigned *__restrict__ skey, int n, Geom g, int *__restrict__ bin_f
             key_to_cell(key, g, cx, cy, cz);
         }
     }
-    // the four x cells cx-1..cx+2 fall into at most two words (two runs when they wrap)
+    // the four x cells cx-1..cx+2 fall into at most two words, or three when they wrap on a lattice whose last word
+    // holds one or two cells (nx % 32 = 1, 2: e.g. nx = 65, cells 63 | 64 | 0, 1)
 #pragma unroll 1
     for (int r = 0; r < 16; ++r) {
         const int y = wrap(cy - 1 + (r & 3), g.ny);
         const int z = wrap(cz - 1 + (r >> 2), g.nz);
         const int rowbase = (z * g.ny + y) * g.nxw;
-        int w0 = -1, w1 = -1;
-        unsigned b0 = 0, b1 = 0;
+        int w0 = -1, w1 = -1, w2 = -1;
+        unsigned b0 = 0, b1 = 0, b2 = 0;
         if (head) {
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
@@ -216,11 +217,13 @@ k_bins(const unsigned *__restrict__ skey, int n, Geom g, int *__restrict__ bin_f
                 const int w = rowbase + (x >> 5);
                 const unsigned bit = 1u << (x & 31);
                 if (w0 < 0 || w == w0) { w0 = w; b0 |= bit; }
-                else { w1 = w; b1 |= bit; }
+                else if (w1 < 0 || w == w1) { w1 = w; b1 |= bit; }
+                else { w2 = w; b2 |= bit; }
             }
         }
         if (w0 >= 0) atomicOr(amask + w0, b0);
         if (w1 >= 0) atomicOr(amask + w1, b1);
+        if (w2 >= 0) atomicOr(amask + w2, b2);
     }
 }
 

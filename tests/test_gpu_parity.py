@@ -629,6 +629,25 @@ def test_two_markers_far_apart_in_one_chunk_activate_the_cells_between_them(api,
         sim.close()
 
 
+@pytest.mark.parametrize("nx", [65, 66, 97])
+@pytest.mark.parametrize("opts", [{"spread": 1}, {"spread": 2}, {"spread": 3}, {"interp": 1}, {"moments": 2}, {}])
+def test_stencil_across_the_seam_of_a_lattice_whose_last_mask_word_holds_one_or_two_cells(api, orc, nx, opts):
+    """nx % 32 = 1, 2: the four x cells of a stencil that wraps (63 | 64 | 0, 1 for nx = 65) lie in THREE words of the
+    active-cell bitmask.  k_bins, the marking kernel of the comparison variants, once assumed two and lost the cell of
+    the last word (found by the randomised differential run).  One marker per seam position, so that no other marker
+    marks the cell."""
+    for cx in range(nx - 4, nx):
+        sim, ref = _pair(api, orc, nx, 8, 6)
+        m = (np.array([[cx + 0.3, 3.4, 2.6]], np.float32), np.array([[0.01, -0.02, 0.015]], np.float32), np.array([0.25], np.float32))
+        sim.set_markers(*m); ref.set_markers(*m)
+        for k, v in opts.items():
+            sim.set_option(getattr(api, "OPT_" + k.upper()), v)
+        sim.step(3, 3); ref.step(3, 3); sim.sync()
+        _compare_fields(sim, ref); _marker_forces_agree(sim, ref)
+        assert sim.get_info(api.INFO_ACTIVE_CELLS) == 64
+        sim.close()
+
+
 @pytest.mark.parametrize("iters", [1, 17, 64])
 def test_mdf_iteration_counts_from_one_to_the_maximum(api, orc, iters):
     """P:110 fixes 5 iterations; the loop is generic: 1 (interpolate once, spread Delta u once, R11), an odd count,
