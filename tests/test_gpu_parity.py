@@ -648,6 +648,53 @@ def test_stencil_across_the_seam_of_a_lattice_whose_last_mask_word_holds_one_or_
         sim.close()
 
 
+@pytest.mark.parametrize("opts", [{}, {"persistent": 2, "pipeline": 1}, {"overlap": 0}])
+def test_update_kinematics_in_mid_run_against_the_oracle(api, orc, opts):
+    """ibm_update_kinematics (new rate, then new rate and centre) between steps.  The oracle has no such call: there
+    the bodies are cleared and set again with the new values; its step counter carries on, so the phase is omega n in
+    both (R13).  What was binned ahead with the old rate has to be discarded by the library."""
+    rng = np.random.default_rng(11)
+    sim, ref = _pair(api, orc, 28, 20, 18)
+    for k, v in opts.items():
+        sim.set_option(getattr(api, "OPT_" + k.upper()), v)
+    dims = np.array([28.0, 20.0, 18.0])
+    bodies = []
+    for b in range(3):
+        n = 400
+        pos = (dims / 2 + rng.normal(scale=3.0, size=(n, 3))).astype(np.float32)
+        m = (pos, rng.normal(scale=0.005, size=(n, 3)).astype(np.float32), np.full(n, 0.05, np.float32))
+        axis = rng.normal(size=3)
+        kin = [float(rng.uniform(-0.01, 0.01)), axis / np.linalg.norm(axis), dims / 2 + rng.normal(scale=1.0, size=3)]
+        bodies.append([m, kin])
+        for o in (sim, ref):
+            o.set_markers(*m)
+            o.set_kinematics(*kin)
+
+    def oracle_reset():
+        ref.clear_markers()
+        for m, kin in bodies:
+            ref.set_markers(*m)
+            ref.set_kinematics(*kin)
+
+    sim.step(5, 3); ref.step(5, 3)
+    bodies[1][1][0] = 0.015                                          # body 1: another rate
+    sim.update_kinematics(1, [0.015], [bodies[1][1][1]])
+    oracle_reset()
+    sim.step(4, 3); ref.step(4, 3)
+    bodies[0][1][0] = -0.012                                         # body 0: another rate and centre
+    bodies[0][1][2] = bodies[0][1][2] + np.array([0.4, -0.3, 0.2])
+    bodies[2][1][0] = 0.0                                            # body 2: stopped
+    sim.update_kinematics(0, [-0.012], [bodies[0][1][1]], [bodies[0][1][2]])
+    sim.update_kinematics(2, [0.0], [bodies[2][1][1]])
+    oracle_reset()
+    sim.step(6, 3); ref.step(6, 3)
+    sim.sync()
+    _compare_fields(sim, ref); _marker_forces_agree(sim, ref)
+    mk, rm = sim.read_markers(), ref.read_markers()
+    assert np.abs(mk["pos"] - rm["x"]).max() <= 8 * np.spacing(np.float32(28))
+    sim.close()
+
+
 @pytest.mark.parametrize("iters", [1, 17, 64])
 def test_mdf_iteration_counts_from_one_to_the_maximum(api, orc, iters):
     """P:110 fixes 5 iterations; the loop is generic: 1 (interpolate once, spread Delta u once, R11), an odd count,
