@@ -695,6 +695,35 @@ def test_update_kinematics_in_mid_run_against_the_oracle(api, orc, opts):
     sim.close()
 
 
+def test_set_fields_in_mid_run_restarts_the_time(api, orc):
+    """lbm_set_fields "resets the step counter" (include/lbm_ibm.h): a rotating body returns to the phase of step 0,
+    and what the library had binned ahead for steps n + 1, n + 2 has to go.  The oracle's set_fields keeps counting,
+    so the comparison is with a FRESH oracle (step 0) that gets the same bodies and fields."""
+    import torch
+    rng = np.random.default_rng(13)
+    nx, ny, nz = 26, 18, 16
+    dims = np.array([nx, ny, nz], float)
+    n = 500
+    pos = (dims / 2 + rng.normal(scale=2.5, size=(n, 3))).astype(np.float32)
+    m = (pos, None, np.full(n, 0.05, np.float32))
+    kin = (0.02, np.array([0.3, -0.5, 0.8]) / np.linalg.norm([0.3, -0.5, 0.8]), dims / 2)
+    u0 = rng.normal(scale=0.01, size=(3, nz, ny, nx)).astype(np.float32)
+    sim = api.LbmIbm(nx, ny, nz, 0.8, stream=_stream())
+    sim.set_markers(*m); sim.set_kinematics(*kin)
+    sim.step(7, 3)                                   # the markers of steps 8 and 9 are binned by now
+    sim.set_fields(None, torch.from_numpy(u0).cuda())
+    torch.cuda.synchronize()
+    sim.step(5, 3)
+    ref = orc.Oracle(nx, ny, nz, 0.8)
+    ref.set_markers(*m); ref.set_kinematics(*kin)
+    ref.set_fields(None, u0)
+    ref.step(5, 3)
+    sim.sync()
+    _compare_fields(sim, ref); _marker_forces_agree(sim, ref)
+    assert np.abs(sim.read_markers()["pos"] - ref.read_markers()["x"]).max() <= 8 * np.spacing(np.float32(nx))
+    sim.close()
+
+
 @pytest.mark.parametrize("iters", [1, 17, 64])
 def test_mdf_iteration_counts_from_one_to_the_maximum(api, orc, iters):
     """P:110 fixes 5 iterations; the loop is generic: 1 (interpolate once, spread Delta u once, R11), an odd count,
