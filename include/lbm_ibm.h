@@ -124,6 +124,11 @@ enum {
                              lbm_sync, lbm_get_info(LBM_INFO_TRACE_NS + i) is the device time in ns from the fork
                              of the LAST step to event i and lbm_trace_label(i) names it.  A profiling aid
                              (the timeline of the concurrent branches); results do not depend on it.          */
+    LBM_OPT_BULK_STREAM = 17, /* cache policy of the bulk stream-collide pass that runs beside the MDF loop (step layout
+                             1): 1 = evict-first ("cache-streaming") loads and stores, so that the populations it
+                             streams through L2 do not evict the few MB the MDF kernels work on; 2 = the default policy;
+                             0 (default) = 1 when the persistent MDF kernel is in use, else 2.  Results are
+                             bit-identical.                                                                       */
     LBM_OPT_MDF_BLOCKS = 13 /* tuning: blocks per SM of the tile pass / of the persistent MDF kernel (0 = default:
                              as many as fit / one); fewer blocks leave more of every SM to the stream-collide
                              pass that runs beside the MDF loop.  Results do not depend on it.           */

@@ -23,6 +23,7 @@ _L = C.CDLL(LIB_PATH)
 
 OPT_SPREAD, OPT_FORCING, OPT_GRAPH, OPT_LBM_KERNEL, OPT_INTERP, OPT_TIMING, OPT_OVERLAP, OPT_MOMENTS = 1, 2, 3, 4, 5, 6, 7, 8
 OPT_FUSED, OPT_TILE_ROWS, OPT_PERSISTENT, OPT_TILE_CAP, OPT_MDF_BLOCKS, OPT_TILE_WARPS, OPT_TRACE, OPT_PIPELINE = 9, 10, 11, 12, 13, 14, 15, 16
+OPT_BULK_STREAM = 17
 PERSISTENT_AUTO, PERSISTENT_ON, PERSISTENT_OFF = 0, 1, 2
 INFO_MARKERS, INFO_BODIES, INFO_STEPS, INFO_LAUNCHES, INFO_ACTIVE_CELLS, INFO_DEVICE_BYTES, INFO_STATUS = range(1, 8)
 INFO_RUNS, INFO_RUN_ENTRIES, INFO_TILES, INFO_ACTIVE_WORDS = 8, 9, 10, 11

@@ -207,6 +207,7 @@ struct lbm {
     int opt_overlap = 3, opt_moments = 0;
     int opt_pipeline = 0;
     int opt_fused = 1, opt_tile_rows = 0, opt_persistent = 0, opt_tile_cap = 0, opt_mdf_blocks = 0, opt_tile_warps = 0;
+    int opt_bulk_stream = 0;
     bool realloc_tables = false;        // LBM_OPT_TILE_CAP changed: the tile tables are re-allocated at the next step
     int *d_box = nullptr;               // per-body bounding boxes (comparison LBM_OPT_MOMENTS = 1 only; lazy)
     PhaseTimer timer;
@@ -404,6 +405,15 @@ bool use_persistent(const lbm *h)
     if (!fused_path(h) || h->opt_moments != 0 || h->opt_timing) return false;
     if (h->opt_persistent) return h->opt_persistent == 1;
     return h->nm <= TR1_MAX_MARKERS && h->g.cells <= PERSISTENT_MAX_CELLS;
+}
+
+// Cache policy of the bulk stream-collide pass that runs beside the MDF loop (LBM_OPT_BULK_STREAM): evict-first loads
+// and stores keep the ~1 GB it streams through L2 from evicting what the MDF kernels work on.  Automatic: with the
+// persistent MDF kernel (small marker sets on small lattices, where the two kernels run side by side from start to end).
+bool bulk_stream(const lbm *h)
+{
+    if (h->opt_bulk_stream) return h->opt_bulk_stream == 1;
+    return use_persistent(h);
 }
 
 // Depth of the binning pipeline (LBM_OPT_PIPELINE): 2 = the binning of a step is spread over the two steps before it
@@ -878,6 +888,7 @@ int enqueue_lbm_pass(lbm *h, cudaStream_t s, const float *src, float *dst, int m
         const dim3 b = cell_block(g);
         const dim3 gr = cell_grid(g, b);
         if (mode == LBM_FUSED) k_stream_collide_scalar<LBM_FUSED, 256, 5><<<gr, b, 0, s>>>(src, dst, g, cc, h->po, amask, h->G);
+        else if (mode == LBM_BULK && bulk_stream(h)) k_stream_collide_scalar<LBM_BULK, 256, 5, true><<<gr, b, 0, s>>>(src, dst, g, cc, h->po, amask, nullptr);
         else if (mode == LBM_BULK) k_stream_collide_scalar<LBM_BULK, 256, 5><<<gr, b, 0, s>>>(src, dst, g, cc, h->po, amask, nullptr);
         else k_stream_collide_scalar<LBM_PURE, 256, 5><<<gr, b, 0, s>>>(src, dst, g, cc, h->po, nullptr, nullptr);
     }
@@ -977,8 +988,12 @@ int enqueue_step_overlapped(lbm *h, int parity, PrepSet &S, PrepSet &N, PrepSet 
         at[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
         const CollisionConst cc = collision_const(h);
-        CK(cudaLaunchKernelEx(&cfg, k_stream_collide_scalar<LBM_BULK, 256, 5>, src, dst, h->g, cc, h->po,
-                              (const unsigned *)S.amask, (const float4 *)nullptr));
+        if (bulk_stream(h))
+            CK(cudaLaunchKernelEx(&cfg, k_stream_collide_scalar<LBM_BULK, 256, 5, true>, src, dst, h->g, cc, h->po,
+                                  (const unsigned *)S.amask, (const float4 *)nullptr));
+        else
+            CK(cudaLaunchKernelEx(&cfg, k_stream_collide_scalar<LBM_BULK, 256, 5>, src, dst, h->g, cc, h->po,
+                                  (const unsigned *)S.amask, (const float4 *)nullptr));
         trace_mark(h, s, "bulk");
         ++nk;
     }
@@ -1027,7 +1042,8 @@ int get_graph(lbm *h, int kind, int parity, int set, int mdf_iters, cudaGraphExe
                           ((long long)h->opt_lbm_kernel << 48) | ((long long)h->opt_interp << 52) |
                           ((long long)overlap_mode(h) << 56) | ((long long)h->opt_moments << 58) |
                           ((long long)h->opt_fused << 60) | ((long long)h->tr << 16) | ((long long)use_persistent(h) << 20) |
-                          ((long long)tile_warps(h) << 21) | ((long long)h->opt_trace << 23) | ((long long)pipe << 24);
+                          ((long long)tile_warps(h) << 21) | ((long long)h->opt_trace << 23) | ((long long)pipe << 24) |
+                          ((long long)h->opt_bulk_stream << 26);
     h->last_key = key;
     auto it = h->graphs.find(key);
     if (it != h->graphs.end()) { *exec = it->second.first; *n_kernels = it->second.second; return LBM_OK; }
@@ -1053,13 +1069,14 @@ int get_graph(lbm *h, int kind, int parity, int set, int mdf_iters, cudaGraphExe
         std::vector<cudaGraphNode_t> nodes(nn);
         if (e == cudaSuccess) e = cudaGraphGetNodes(graph, nodes.data(), &nn);
         const void *bulk_fn = (const void *)k_stream_collide_scalar<LBM_BULK, 256, 5>;
+        const void *bulk_cs_fn = (const void *)k_stream_collide_scalar<LBM_BULK, 256, 5, true>;
         for (size_t i = 0; i < nn && e == cudaSuccess; ++i) {
             cudaGraphNodeType ty;
             if (cudaGraphNodeGetType(nodes[i], &ty) != cudaSuccess || ty != cudaGraphNodeTypeKernel) continue;
             cudaKernelNodeParams kp{};
             if (cudaGraphKernelNodeGetParams(nodes[i], &kp) != cudaSuccess) continue;
             cudaLaunchAttributeValue v{};
-            v.priority = (kp.func == bulk_fn) ? lo : hi;
+            v.priority = (kp.func == bulk_fn || kp.func == bulk_cs_fn) ? lo : hi;
             e = cudaGraphKernelNodeSetAttribute(nodes[i], cudaLaunchAttributePriority, &v);
         }
         if (e != cudaSuccess) {
@@ -1276,6 +1293,7 @@ int lbm_set_option(lbm_t *h, int key, int value)
             return LBM_OK;
         case LBM_OPT_TILE_WARPS: if (value < 0 || value > 2) break; h->opt_tile_warps = value; return LBM_OK;
         case LBM_OPT_PIPELINE: if (value < 0 || value > 2) break; h->opt_pipeline = value; return LBM_OK;
+        case LBM_OPT_BULK_STREAM: if (value < 0 || value > 2) break; h->opt_bulk_stream = value; return LBM_OK;
         case LBM_OPT_TRACE:
             if (value < 0 || value > 1) break;
             if (value != h->opt_trace) { CK(cudaStreamSynchronize(h->stream)); drop_graphs(h); h->opt_trace = value; }

@@ -40,6 +40,11 @@
 
 namespace lbmk {
 
+// CS = cache-streaming (evict-first) accesses: for the bulk pass that runs BESIDE the MDF loop, so that the ~1 GB it
+// streams through L2 does not evict the few MB the MDF kernels work on (U, the footprints, the markers)
+template <bool CS> __device__ __forceinline__ float lbm_load(const float *p) { return CS ? __ldcs(p) : LBM_LOAD(p); }
+template <bool CS> __device__ __forceinline__ void lbm_store(float *p, float v) { if (CS) __stcs(p, v); else LBM_STORE(p, v); }
+
 struct Geom {
     int nx, ny, nz;
     int nxw;             // 32-cell words per x-row of the active-cell bitmask
@@ -75,6 +80,7 @@ __device__ __forceinline__ Nbr neighbours(const Geom &g, int x, int y, int z)
 }
 
 // Pull the 19 canonical populations of cell (x,y,z) out of a post-collision buffer.
+template <bool CS = false>
 __device__ __forceinline__ void pull_cell(const float *__restrict__ src, const Geom &g, const Nbr &n, int x, int y,
                                           int z, float (&df)[NQ])
 {
@@ -95,7 +101,7 @@ __device__ __forceinline__ void pull_cell(const float *__restrict__ src, const G
         if (dir_ez(i) == -1) behind_wall |= n.wzp;
         const int cell = behind_wall ? self : (sz * g.ny + sy) * g.nx + sx;
         const int plane = behind_wall ? dir_opp(i) : i;
-        df[i] = LBM_LOAD(src + (size_t)plane * cells + cell);
+        df[i] = lbm_load<CS>(src + (size_t)plane * cells + cell);
     }
 }
 
@@ -125,6 +131,7 @@ inline PlaneOffsets plane_offsets(const Geom &g)
 // Pull for a cell whose y and z neighbours are plain lattice rows (no wrap, no wall) and that has
 // no x wall behind it: every source sits at a kernel-uniform byte offset (plane + row shift) from
 // one of three per-thread pointers (the cell itself, its wrapped x-1 and x+1 neighbours).
+template <bool CS = false>
 __device__ __forceinline__ void pull_cell_inner(const float *__restrict__ src, const Geom &g, const PlaneOffsets &po,
                                                 int x, int self, float (&df)[NQ])
 {
@@ -134,7 +141,7 @@ __device__ __forceinline__ void pull_cell_inner(const float *__restrict__ src, c
 #pragma unroll
     for (int i = 0; i < NQ; ++i) {
         const char *__restrict__ b = dir_ex(i) == 1 ? pm : (dir_ex(i) == -1 ? pp : p0);
-        df[i] = LBM_LOAD(reinterpret_cast<const float *>(b + po.ld[i]));
+        df[i] = lbm_load<CS>(reinterpret_cast<const float *>(b + po.ld[i]));
     }
 }
 
@@ -151,7 +158,7 @@ __device__ __forceinline__ void pull_cell_inner(const float *__restrict__ src, c
 //           Everywhere else a = g_body: this pass needs nothing from the IBM and runs beside it.
 enum { LBM_PURE = 0, LBM_FUSED = 1, LBM_BULK = 2 };
 
-template <int MODE, int THREADS, int MINB>
+template <int MODE, int THREADS, int MINB, bool CS = false>
 __global__ void __launch_bounds__(THREADS, MINB)
 k_stream_collide_scalar(const float *__restrict__ src, float *__restrict__ dst, const __grid_constant__ Geom g,
                         const __grid_constant__ CollisionConst cc, const __grid_constant__ PlaneOffsets po,
@@ -176,15 +183,15 @@ k_stream_collide_scalar(const float *__restrict__ src, float *__restrict__ dst, 
     float df[NQ];
     const bool xwall = g.wallx && (x == 0 || x == g.nx - 1);
     if (y > 0 && y < g.ny - 1 && z > 0 && z < g.nz - 1 && !xwall) {
-        pull_cell_inner(src, g, po, x, self, df);
+        pull_cell_inner<CS>(src, g, po, x, self, df);
     } else {
         const Nbr n = neighbours(g, x, y, z);
-        pull_cell(src, g, n, x, y, z, df);
+        pull_cell<CS>(src, g, n, x, y, z, df);
     }
     collide(df, ax, ay, az, cc);
     char *__restrict__ q = reinterpret_cast<char *>(dst + self);
 #pragma unroll
-    for (int i = 0; i < NQ; ++i) LBM_STORE(reinterpret_cast<float *>(q + po.st[i]), df[i]);
+    for (int i = 0; i < NQ; ++i) lbm_store<CS>(reinterpret_cast<float *>(q + po.st[i]), df[i]);
 }
 
 // a8 on the words the bulk pass skipped (second pass of the overlapped step): one warp per entry of

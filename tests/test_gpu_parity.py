@@ -238,13 +238,15 @@ def test_w1_atomic_variant_matches_and_gather_is_deterministic(api, orc):
     assert np.abs(outs[0][3] - outs[3][3]).max() <= 1e-5 * np.abs(outs[0][3]).max()
 
 
-def _run_w1(api, steps_per_call, overlap, graph=1, reads=False, retune_at=None):
+def _run_w1(api, steps_per_call, overlap, graph=1, reads=False, retune_at=None, bulk_stream=0, persistent=0):
     """W1 for sum(steps_per_call) steps; returns (rho, u, G, marker forces, perm)."""
     from paper_1904_02108_b200 import workloads
     wl = workloads.get("W1")
     sim = api.from_workload(wl, stream=_stream())
     sim.set_option(api.OPT_OVERLAP, overlap)
     sim.set_option(api.OPT_GRAPH, graph)
+    sim.set_option(api.OPT_BULK_STREAM, bulk_stream)
+    sim.set_option(api.OPT_PERSISTENT, persistent)
     done = 0
     for n in steps_per_call:
         if retune_at is not None and done == retune_at:
@@ -268,7 +270,11 @@ def test_overlapped_step_equals_serial_step_bitwise(api):
     whatever the split into calls, with read-outs in between, and with plain launches."""
     ref = _run_w1(api, [12], overlap=0)
     for kw in (dict(steps_per_call=[12], overlap=1), dict(steps_per_call=[1, 2, 1, 5, 3], overlap=1, reads=True),
-               dict(steps_per_call=[5, 7], overlap=1, graph=0), dict(steps_per_call=[3, 9], overlap=0, graph=0)):
+               dict(steps_per_call=[5, 7], overlap=1, graph=0), dict(steps_per_call=[3, 9], overlap=0, graph=0),
+               # the cache policy of the bulk pass (evict-first or default), beside the persistent kernel and beside the chain
+               dict(steps_per_call=[12], overlap=1, bulk_stream=1), dict(steps_per_call=[12], overlap=1, bulk_stream=2),
+               dict(steps_per_call=[4, 8], overlap=1, bulk_stream=1, persistent=2),
+               dict(steps_per_call=[12], overlap=1, bulk_stream=1, graph=0)):
         got = _run_w1(api, **kw)
         for a, b in zip(ref, got):
             assert np.array_equal(a, b), kw
