@@ -15,6 +15,9 @@
  *  - All entry points are extern "C"; no exceptions or aborts cross the boundary.  Functions
  *    returning int give 0 on success and a negative LBM_E* code on error; the text of the last
  *    error of the calling thread is lbm_last_error().  On error the state is unchanged.
+ *    Threads: different handles may be used from different host threads at the same time (no call synchronises
+ *    the whole device or touches the legacy default stream after lbm_create has returned its handle); one handle is
+ *    used by one thread at a time.
  *  - Every pointer argument marked "host or device" may point to pageable/pinned host memory or
  *    to device memory of the handle's GPU (detected with cudaPointerGetAttributes).  Pointers
  *    marked "host" are read on the CPU during the call.

@@ -525,14 +525,20 @@ int mdf_launch_geometry(lbm *h)
 {
     const MdfKernels K = mdf_kernels(h);
     const size_t smem_t = (size_t)MDF_WARPS * h->mdf_wsmem, smem_p = (size_t)MDFP_WARPS * h->mdf_wsmem;
-    CK(cudaFuncSetAttribute((const void *)K.tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_t));
-    CK(cudaFuncSetAttribute((const void *)K.persistent, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_p));
+    // The shared-memory cap is an attribute of the KERNEL, device-wide, shared by every handle of the process (and by
+    // every host thread): it is set to what the widest window needs (CHUNK_ENT_MAX entries), never to this handle's own
+    // size -- a handle on a lattice with a narrower window would otherwise lower the cap under the graphs another
+    // handle has still to build.
+    const ChunkGeom widest{1, CHUNK_ENT_MAX};
+    const size_t wmax = mdf_warp_smem(h->tr, widest);
+    CK(cudaFuncSetAttribute((const void *)K.tiles, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(MDF_WARPS * wmax)));
+    CK(cudaFuncSetAttribute((const void *)K.persistent, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(MDFP_WARPS * wmax)));
     int per_sm = 0;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, K.tiles, MDF_WARPS * 32, smem_t));
     if (h->opt_mdf_blocks > 0) per_sm = std::min(per_sm, h->opt_mdf_blocks);
     h->mdf_grid = std::max(1, per_sm) * h->sms;
     const size_t smem_2 = mdf_pair_smem(h->tr, h->cg);
-    CK(cudaFuncSetAttribute((const void *)K.pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_2));
+    CK(cudaFuncSetAttribute((const void *)K.pairs, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mdf_pair_smem(h->tr, widest)));
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, K.pairs, 64, smem_2));
     if (h->opt_mdf_blocks > 0) per_sm = std::min(per_sm, h->opt_mdf_blocks);
     h->mdf2_grid = std::max(1, per_sm) * h->sms;
@@ -1188,14 +1194,16 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
         if (dmalloc(h, &S.amask, h->n_mask_words) || dmalloc(h, &S.words, h->n_mask_words)) return bail("active mask");
         if (dmalloc(h, &S.chunk_of, h->chunk_slots)) return bail("chunk map");
         if (dmalloc(h, &S.scal, (size_t)1)) return bail("set scalars");
-        ok &= cudaMemset(S.amask, 0, h->n_mask_words * sizeof(unsigned)) == cudaSuccess;
-        ok &= cudaMemset(S.chunk_of, 0xff, h->chunk_slots * sizeof(int)) == cudaSuccess;
-        ok &= cudaMemset(S.scal, 0, sizeof(SetScalars)) == cudaSuccess;
+        // on a stream of the handle's own and with a stream synchronisation: a legacy-stream memset or a device-wide
+        // synchronisation would collide with a graph capture another handle has open in another host thread
+        ok &= cudaMemsetAsync(S.amask, 0, h->n_mask_words * sizeof(unsigned), h->cap_stream) == cudaSuccess;
+        ok &= cudaMemsetAsync(S.chunk_of, 0xff, h->chunk_slots * sizeof(int), h->cap_stream) == cudaSuccess;
+        ok &= cudaMemsetAsync(S.scal, 0, sizeof(SetScalars), h->cap_stream) == cudaSuccess;
     }
-    ok &= cudaMemset(h->f[0], 0, fcount * sizeof(float)) == cudaSuccess;   // rest state: f_i - t_i = 0
-    ok &= cudaMemset(h->f[1], 0, fcount * sizeof(float)) == cudaSuccess;
-    ok &= cudaMemset(h->scal, 0, sizeof(DevScalars)) == cudaSuccess;
-    ok &= cudaDeviceSynchronize() == cudaSuccess;
+    ok &= cudaMemsetAsync(h->f[0], 0, fcount * sizeof(float), h->cap_stream) == cudaSuccess;   // rest state: f_i - t_i = 0
+    ok &= cudaMemsetAsync(h->f[1], 0, fcount * sizeof(float), h->cap_stream) == cudaSuccess;
+    ok &= cudaMemsetAsync(h->scal, 0, sizeof(DevScalars), h->cap_stream) == cudaSuccess;
+    ok &= cudaStreamSynchronize(h->cap_stream) == cudaSuccess;
     if (!ok) { fail(LBM_ECUDA, "%s", cudaGetErrorString(cudaGetLastError())); return bail("memset"); }
     {
         int per_sm = 0, sms = 148;
@@ -1217,7 +1225,10 @@ lbm_t *lbm_create(int nx, int ny, int nz, double tau, const lbm_bc_t *bc)
 void lbm_destroy(lbm_t *h)
 {
     if (!h) return;
-    cudaDeviceSynchronize();
+    // wait for the handle's own work only (never the whole device: a device-wide synchronisation fails while another
+    // handle captures a graph in another host thread, and invalidates that capture)
+    cudaStreamSynchronize(h->stream);
+    if (h->copy_stream) cudaStreamSynchronize(h->copy_stream);
     drop_graphs(h);
     free_markers_dev(h);
     cudaFree(h->f[0]); cudaFree(h->f[1]); cudaFree(h->U); cudaFree(h->G); cudaFree(h->scal);

@@ -730,6 +730,70 @@ def test_set_fields_in_mid_run_restarts_the_time(api, orc):
     sim.close()
 
 
+def test_a_second_handle_with_a_narrower_window_does_not_lower_the_first_ones_shared_memory_cap(api, orc):
+    """The dynamic shared-memory cap is an attribute of a KERNEL, shared by all handles.  nx = 19 needs windows of 14
+    entries, nx = 16 of 11: a second handle that set the cap to its own need left the first one unable to launch the
+    graphs it had still to build (here: for another iteration count).  The cap is now the geometry-independent maximum."""
+    rng = np.random.default_rng(3)
+    pairs = []
+    for nx in (19, 16):
+        sim, ref = _pair(api, orc, nx, 12, 10)
+        m = _random_static_markers(rng, 300, nx, 12, 10, 0.05)
+        sim.set_markers(*m); ref.set_markers(*m)
+        sim.step(2, 3); ref.step(2, 3)
+        pairs.append((sim, ref))
+    for sim, ref in pairs:                           # another iteration count, another layout: new graphs, same tables
+        sim.step(3, 4); ref.step(3, 4)
+        sim.set_option(api.OPT_OVERLAP, 2)
+        sim.set_option(api.OPT_PERSISTENT, 2)
+        sim.step(2, 5); ref.step(2, 5)
+    for sim, ref in pairs:
+        sim.sync()
+        _compare_fields(sim, ref); _marker_forces_agree(sim, ref)
+        sim.close()
+
+
+def test_handles_driven_from_several_host_threads(api, orc):
+    """One handle per host thread, created, stepped and destroyed concurrently (ctypes releases the GIL during the
+    calls).  lbm_create and lbm_destroy once synchronised the whole device, which fails while another thread captures
+    a step graph and invalidates that capture; now every call waits for the handle's own streams only."""
+    import threading
+    import torch
+    results, errors = {}, []
+
+    def worker(tid):
+        try:
+            torch.cuda.set_device(0)
+            rng = np.random.default_rng(100 + tid)
+            worst = 0.0
+            for rep in range(8):
+                nx, ny, nz = int(rng.integers(12, 40)), int(rng.integers(8, 20)), int(rng.integers(8, 20))
+                sim, ref = _pair(api, orc, nx, ny, nz)
+                m = _random_static_markers(rng, int(rng.choice([40, 300, 1200])), nx, ny, nz, 0.05)
+                axis = rng.normal(size=3)
+                for o in (sim, ref):
+                    o.set_markers(*m)
+                    o.set_kinematics(0.01, axis / np.linalg.norm(axis), np.array([nx, ny, nz]) / 2.0)
+                for _ in range(3):
+                    k = int(rng.integers(1, 4))
+                    sim.step(k, 3); ref.step(k, 3)
+                sim.sync()
+                worst = max(worst, float(np.abs(sim.read_fields()[1] - ref.read_fields()[1]).max()))
+                _marker_forces_agree(sim, ref)
+                sim.close()
+            results[tid] = worst
+        except Exception as e:                       # noqa: BLE001 - reported by the main thread
+            errors.append(f"thread {tid}: {type(e).__name__}: {e}")
+
+    threads = [threading.Thread(target=worker, args=(i,)) for i in range(4)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    assert len(results) == 4 and max(results.values()) <= TOL_U
+
+
 @pytest.mark.parametrize("iters", [1, 17, 64])
 def test_mdf_iteration_counts_from_one_to_the_maximum(api, orc, iters):
     """P:110 fixes 5 iterations; the loop is generic: 1 (interpolate once, spread Delta u once, R11), an odd count,
