@@ -1421,7 +1421,8 @@ int ibm_set_markers(lbm_t *h, const float *pos, const float *vel, const float *a
     double c[3] = {0, 0, 0};
     for (long long k = 0; k < n; ++k) {
         double x[3] = {p[(size_t)(3 * k)], p[(size_t)(3 * k + 1)], p[(size_t)(3 * k + 2)]};
-        if (!std::isfinite(x[0]) || !std::isfinite(x[1]) || !std::isfinite(x[2]) || !std::isfinite(s[(size_t)k]))
+        if (!std::isfinite(x[0]) || !std::isfinite(x[1]) || !std::isfinite(x[2]) || !std::isfinite(s[(size_t)k]) ||
+            !std::isfinite(v[(size_t)(3 * k)]) || !std::isfinite(v[(size_t)(3 * k + 1)]) || !std::isfinite(v[(size_t)(3 * k + 2)]))
             return fail(LBM_EINVAL, "ibm_set_markers: non-finite input at marker %lld", k);
         if (!stencil_inside(h, x, x))
             return fail(LBM_ERANGE, "ibm_set_markers: stencil of marker %lld (%.3f %.3f %.3f) crosses a wall", k,
@@ -1445,6 +1446,8 @@ int ibm_set_kinematics(lbm_t *h, double omega, const double *axis, const double 
     const double nrm = std::sqrt(axis[0] * axis[0] + axis[1] * axis[1] + axis[2] * axis[2]);
     if (!(nrm > 0.0) || !std::isfinite(nrm) || !std::isfinite(omega))
         return fail(LBM_EINVAL, "ibm_set_kinematics: axis must be non-zero and finite");
+    if (!std::isfinite(center[0]) || !std::isfinite(center[1]) || !std::isfinite(center[2]))
+        return fail(LBM_EINVAL, "ibm_set_kinematics: non-finite centre");
     HostBody &B = h->bodies.back();
     if (omega != 0.0) {
         // every point stays on a sphere of radius |p - c| about c
@@ -1483,6 +1486,8 @@ int ibm_update_kinematics(lbm_t *h, int first_body, int count, const double *ome
             return fail(LBM_EINVAL, "ibm_update_kinematics: bad axis or omega for body %d", first_body + b);
         HostBody &B = nb[(size_t)b];
         const double *c = center ? center + 3 * b : B.center;
+        if (!std::isfinite(c[0]) || !std::isfinite(c[1]) || !std::isfinite(c[2]))
+            return fail(LBM_EINVAL, "ibm_update_kinematics: non-finite centre for body %d", first_body + b);
         if (center) for (int a = 0; a < 3; ++a) moved |= (c[a] != B.center[a]);
         const bool any_wall = h->g.wallx || h->g.wally || h->g.wallz;
         if (any_wall && omega[b] != 0.0 && (center || B.omega == 0.0))

@@ -824,8 +824,22 @@ def test_error_paths(api):
         sim.set_kinematics(0.01, (1, 0, 0), (8, 8, 2.0))          # sweeps through the z wall
     assert ei.value.code == -4
     sim.set_kinematics(0.01, (0, 0, 2), (8, 8, 8))
+    # non-finite inputs are refused on the host and leave the state unchanged
+    one = np.array([[8.0, 8.0, 8.0]], dtype=np.float32)
+    for bad in (dict(pos=np.array([[np.nan, 8.0, 8.0]], np.float32)), dict(vel=np.array([[0.0, np.inf, 0.0]], np.float32)),
+                dict(area=np.array([np.nan], np.float32))):
+        with pytest.raises(api.LbmError) as ei:
+            sim.set_markers(bad.get("pos", one), bad.get("vel"), bad.get("area", np.ones(1, np.float32)))
+        assert ei.value.code == -1
+    for args in ((np.nan, (0, 0, 1), (8, 8, 8)), (0.01, (0, 0, 0), (8, 8, 8)), (0.01, (0, 0, 1), (8, np.inf, 8))):
+        with pytest.raises(api.LbmError):
+            sim.set_kinematics(*args)
+    with pytest.raises(api.LbmError):
+        sim.update_kinematics(0, [0.01], [[0.0, 0.0, 1.0]], [[np.nan, 8.0, 8.0]])
+    assert sim.get_info(api.INFO_MARKERS) == 1 and sim.get_info(api.INFO_BODIES) == 1
     sim.step(2, 2)
     sim.sync()
+    assert np.isfinite(sim.read_fields()[1]).all()
     sim.close()
 
 
