@@ -41,7 +41,7 @@ UNIT = "MLUPS"
 NOMINAL_HBM_GBS = 8000.0       # north_star's denominator
 # B200 fp32 FMA peak for the ALU-bound tile pass: 148 SMs x 128 fp32 lanes x 2 flop x 1.965 GHz
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-SWEEP = ["W3", "W4lit", "W4", "W5lit", "W5", "P1", "P6", "P18"]
+SWEEP = ["W3", "W3x4", "W4lit", "W4", "W5lit", "W5", "P1", "P6", "P18"]
 PAPER_MLUPS = {"P1": 893.0, "P6": 650.0, "P18": 344.2}
 ORACLE_FULL_MAX_CELLS = 1 << 25      # the fp64 oracle at full size up to 256^3 x 2 (W5: 512^3 needs ~48 GB and minutes per step)
 
@@ -617,7 +617,7 @@ def run_ours(args):
 
 
 def workloads_names():
-    return ("W1", "W2", "W3", "W3lit", "W4", "W4lit", "W5", "W5lit", "P1", "P6", "P18")
+    return ("W1", "W2", "W3", "W3lit", "W3x4", "W4", "W4lit", "W5", "W5lit", "P1", "P6", "P18")
 
 
 def main():

@@ -91,7 +91,8 @@ enum {
                              branches (MDF loop, binning of the next step), then ONE fused stream-collide
                              pass over the whole lattice.  0 = one serial chain with a single fused
                              stream-collide pass (measured comparison).  3 (default) = 2 on lattices above
-                             64 Mi cells or above 40,000 markers, else 1.  Results are bit-identical.      */
+                             64 Mi cells or with tiles of 4 x 4 rows (the tile pass then fills the SMs by itself),
+                             else 1.  Results are bit-identical.                                         */
     LBM_OPT_MOMENTS = 8,  /* where U is precomputed for the IBM: 0 = the de-duplicated list of
                              cells inside a marker stencil (default), 1 = the paper's box strategy (bounding
                              box of every body), 2 = the paper's kernel strategy (a block per Lagrangian
@@ -100,13 +101,17 @@ enum {
                              corrects and spreads (s g never leaves the SM) plus the collect; 0 = the
                              round-1 pipeline: interpolation kernel, TMA-fed tile sweep, collect (measured
                              comparison).  Only with LBM_OPT_SPREAD = 0 and LBM_OPT_INTERP = 0.           */
-    LBM_OPT_TILE_ROWS = 10, /* source rows per tile in y and z for the fused path: 0 = automatic (1 up to 20,000
-                             markers, 2 up to 40,000, else 4), or 1, 2, 4.  Changing it rebuilds the tile
-                             tables at the next step.  Results agree to rounding (summation order).        */
+    LBM_OPT_TILE_ROWS = 10, /* source rows per tile in y and z for the fused path: 1, 2, 4, or 0 = automatic: the largest
+                             of 4, 2, 1 for which the markers, in their rest pose, occupy at least 2,500 tiles (the
+                             tile pass needs more tiles than warp slots; the number of tiles, not of markers,
+                             decides: one thin body of 60,000 markers occupies ~300 tiles of 4 x 4 rows).
+                             Changing it rebuilds the tile tables at the next step.  Results agree to rounding
+                             (summation order).                                                           */
     LBM_OPT_PERSISTENT = 11, /* the fused MDF loop (moments + N x (tile pass, collect)) as ONE persistent kernel
                              with grid-wide barriers instead of 2 N + 1 launches: 1 = on, 2 = off, 0 (default) =
-                             on for marker sets of up to 20,000 markers on lattices of up to 4 Mi cells (where the
-                             chain of launches is the critical path of the step).  Results are bit-identical.   */
+                             on for single-row tiles (see LBM_OPT_TILE_ROWS) with up to 36,000 markers on lattices
+                             of up to 4 Mi cells (where the chain of launches is the critical path of the step).
+                             Results are bit-identical.                                                   */
     LBM_OPT_TILE_CAP = 12, /* > 0: cap the number of tile footprints (default 0 = room for every tile that can
                              exist, up to 12 GB).  More tiles than the cap are dropped for that step and
                              lbm_sync reports LBM_ENOMEM; later steps that fit are complete again.  Takes

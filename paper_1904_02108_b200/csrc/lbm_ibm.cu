@@ -85,14 +85,19 @@ constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driv
 // Tile edge by marker count (LBM_OPT_TILE_ROWS = 0), measured on B200: single-row tiles while
 // the set is so small that larger tiles would not fill the SMs (W1, W3: 15,360 markers), two-row tiles up to a few
 // ten thousand markers (P6), 4 x 4-row tiles beyond (P18, W4lit, W4, W5lit, W5).
-constexpr int TR1_MAX_MARKERS = 20000;
-constexpr int TR2_MAX_MARKERS = 40000;
+// Tile edge (source rows per tile in y and z): the largest of 4, 2, 1 that still gives the tile pass enough tiles --
+// about 1.4 per warp slot of the grid (148 SMs x 12 warps).  The count, not the marker count, is what matters: 60,000
+// markers of ONE thin propeller occupy ~300 tiles of 4 x 4 rows (most warps idle, 0.67 ms per step on 128^3) but
+// ~1,200 single-row tiles (0.17 ms); the same number of markers spread over 18 bodies fills 4,400 tiles of 4 x 4 rows.
+// Measured on B200 (tiles at edge 4 / 2 / 1 and the best edge): P6 1441 / 3498 / 9807: 2; P18 4365 / 10527 / 29018: 4;
+// W4lit 3662 / 9153 / 25968: 4; P1 225 / 555 / 1621: 1 or 2.
+constexpr long long TILE_RULE_MIN_TILES = 2500;
+constexpr int PERSISTENT_MAX_MARKERS = 36000;   // persistent MDF kernel: faster than the kernel chain up to ~30 k markers, slower from ~45 k (128^3)
 // Step layout (LBM_OPT_OVERLAP = 3): the split of the stream-collide into a bulk pass beside the MDF loop and a pass
 // over the stencil cells pays while the MDF loop is a chain of short, latency-bound kernels that leave the SMs mostly
 // idle (small marker sets); beyond that the tile pass fills the SMs itself and one fused pass after it is faster
 // (measured: P18 0.469 against 0.552 ms per step, W4lit 0.683 against 0.740, W4 1.245 against 1.262)
 constexpr long long SPLIT_MAX_CELLS = 64LL << 20;
-constexpr int SPLIT_MAX_MARKERS = 40000;
 
 // Optional per-phase device timing (LBM_OPT_TIMING): CUDA events recorded on the launching stream
 // between the phases of a step; durations are accumulated after a stream synchronise.
@@ -180,6 +185,10 @@ struct lbm {
 
     // markers: host mirror (caller order) and device copies
     std::vector<float> h_pos, h_vel, h_area;   // [n][3], [n][3], [n]
+    // tiles the markers occupy in their rest pose, for tile edges 1, 2, 4 (bitmaps over the tile slots + counts): what the
+    // automatic tile edge, step layout and persistent-kernel rules go by
+    std::vector<unsigned long long> rest_map[3];
+    long long rest_tiles[3] = {0, 0, 0};
     std::vector<int> h_body;
     std::vector<HostBody> bodies;
     std::vector<BodyDef> h_defs;        // host copy of the per-body device table
@@ -375,7 +384,9 @@ int effective_tr(const lbm *h)
     if (!fused_path(h)) return TILE_R;
     if (h->opt_tile_rows) return h->opt_tile_rows;
     const size_t n = h->h_area.size();
-    return n <= (size_t)TR1_MAX_MARKERS ? 1 : (n <= (size_t)TR2_MAX_MARKERS ? 2 : TILE_R);
+    (void)n;
+    if (h->rest_tiles[2] >= TILE_RULE_MIN_TILES) return TILE_R;
+    return h->rest_tiles[1] >= TILE_RULE_MIN_TILES ? 2 : 1;
 }
 
 // how a coupled step is laid out (LBM_OPT_OVERLAP): 0 = one serial chain; 1 = three branches (MDF loop, bulk
@@ -384,7 +395,10 @@ int effective_tr(const lbm *h)
 int overlap_mode(const lbm *h)
 {
     if (h->opt_overlap != 3) return h->opt_overlap;
-    return (h->g.cells > SPLIT_MAX_CELLS || h->nm > SPLIT_MAX_MARKERS) ? 2 : 1;
+    // 4 x 4-row tiles: the tile pass fills the SMs by itself, a bulk pass beside it only gets in its way (P18 0.470
+    // against 0.522 ms, W4lit 0.68 against 0.78); smaller tiles: the MDF kernels are short and latency-bound, the
+    // bulk pass runs beside them (P6 0.324 against 0.360, P1 0.239 against 0.281)
+    return (h->g.cells > SPLIT_MAX_CELLS || effective_tr(h) == TILE_R) ? 2 : 1;
 }
 
 // warps per tile of the tile pass: two share a tile's window and footprint where tiles hold several batches of 32
@@ -404,7 +418,7 @@ bool use_persistent(const lbm *h)
 {
     if (!fused_path(h) || h->opt_moments != 0 || h->opt_timing) return false;
     if (h->opt_persistent) return h->opt_persistent == 1;
-    return h->nm <= TR1_MAX_MARKERS && h->g.cells <= PERSISTENT_MAX_CELLS;
+    return effective_tr(h) == 1 && h->nm <= PERSISTENT_MAX_MARKERS && h->g.cells <= PERSISTENT_MAX_CELLS;
 }
 
 // Cache policy of the bulk stream-collide pass that runs beside the MDF loop (LBM_OPT_BULK_STREAM): evict-first loads
@@ -1124,6 +1138,37 @@ bool stencil_inside(const lbm *h, const double lo[3], const double hi[3])
 }  // namespace
 
 // =================================================================================================
+// Register the tiles n new markers occupy in their rest pose, for the tile edges 1, 2 and 4 (see TILE_RULE_MIN_TILES).
+// Rotating bodies sweep other tiles later on, but about as many.
+void count_rest_tiles(lbm *h, const float *pos, long long n)
+{
+    static const int edge[3] = {1, 2, 4};
+    const Geom &g = h->g;
+    for (int e = 0; e < 3; ++e) {
+        const int tr = edge[e];
+        const long long nty = (g.ny + tr - 1) / tr, ntz = (g.nz + tr - 1) / tr;
+        const size_t slots = (size_t)(h->cg.nbx * nty * ntz);
+        if (h->rest_map[e].size() != (slots + 63) / 64) { h->rest_map[e].assign((slots + 63) / 64, 0ull); h->rest_tiles[e] = 0; }
+    }
+    for (long long k = 0; k < n; ++k) {
+        long long c[3];
+        const int dim[3] = {g.nx, g.ny, g.nz};
+        for (int a = 0; a < 3; ++a) {
+            c[a] = (long long)std::floor((double)pos[3 * k + a]) % dim[a];
+            if (c[a] < 0) c[a] += dim[a];
+        }
+        const long long blk = std::min<long long>(c[0] / CHUNK_W, h->cg.nbx - 1);
+        for (int e = 0; e < 3; ++e) {
+            const int tr = edge[e];
+            const long long nty = (g.ny + tr - 1) / tr;
+            const size_t slot = (size_t)(((c[2] / tr) * nty + c[1] / tr) * h->cg.nbx + blk);
+            unsigned long long &w = h->rest_map[e][slot >> 6];
+            const unsigned long long bit = 1ull << (slot & 63);
+            if (!(w & bit)) { w |= bit; h->rest_tiles[e] += 1; }
+        }
+    }
+}
+
 extern "C" {
 
 const char *lbm_last_error(void) { return g_err.c_str(); }
@@ -1430,6 +1475,7 @@ int ibm_set_markers(lbm_t *h, const float *pos, const float *vel, const float *a
         for (int a = 0; a < 3; ++a) c[a] += x[a];
     }
     for (int a = 0; a < 3; ++a) B.center[a] = n > 0 ? c[a] / (double)n : 0.0;
+    count_rest_tiles(h, p.data(), n);
     h->h_pos.insert(h->h_pos.end(), p.begin(), p.end());
     h->h_vel.insert(h->h_vel.end(), v.begin(), v.end());
     h->h_area.insert(h->h_area.end(), s.begin(), s.end());
@@ -1532,6 +1578,7 @@ int ibm_clear(lbm_t *h)
     int rc = flush_ibm(h);
     if (rc) return rc;
     h->h_pos.clear(); h->h_vel.clear(); h->h_area.clear(); h->h_body.clear(); h->bodies.clear();
+    for (int e = 0; e < 3; ++e) { h->rest_map[e].clear(); h->rest_tiles[e] = 0; }
     h->markers_stale = true;
     return LBM_OK;
 }

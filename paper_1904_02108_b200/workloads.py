@@ -214,13 +214,14 @@ def paper_case(n_bodies: int, seed: int = 0) -> Workload:
 
 
 def get(name: str, seed: int = 0) -> Workload:
-    """Named workloads: W1, W2, W3, W3lit, W4, W4lit, W5, W5lit (lit = single layer, 'literal');
+    """Named workloads: W1, W2, W3, W3lit, W3x4, W4, W4lit, W5, W5lit (lit = single layer, 'literal'; x4 = 8 layers);
     P1, P6, P18 = the paper-shaped cases of SURVEY 8(f3)."""
     table = {
         "W1": lambda: w1(seed),
         "W2": lambda: w2(seed),
         "W3": lambda: w3(seed, 2),
         "W3lit": lambda: w3(seed, 1),
+        "W3x4": lambda: w3(seed, 8),        # the same propeller with four times the marker density (61,440 markers)
         "W4": lambda: w4(seed, 8),
         "W4lit": lambda: w4(seed, 1),
         "W5": lambda: w5(seed, 12),

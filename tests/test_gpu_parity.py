@@ -794,6 +794,27 @@ def test_handles_driven_from_several_host_threads(api, orc):
     assert len(results) == 4 and max(results.values()) <= TOL_U
 
 
+def test_tile_edge_follows_the_number_of_tiles_not_of_markers(api, orc):
+    """Automatic tile edge (LBM_OPT_TILE_ROWS = 0): the largest of 4, 2, 1 that leaves >= 2,500 tiles in the rest pose.
+    One thin propeller with 61,440 markers (W3 with 8 layers instead of 2) occupies a few hundred 4 x 4-row tiles: single-row
+    tiles, layout 1; 6 and 18 paper-shaped propellers keep the edges they were tuned with (2 and 4).  The dense single
+    propeller is also compared with the oracle (it takes the kernel chain: above the persistent kernel's 36,000)."""
+    from paper_1904_02108_b200 import workloads
+    for name, rows, layout in (("W3", 1, 1), ("W3x4", 1, 1), ("P6", 2, 1), ("P18", 4, 2)):
+        wl = workloads.get(name)
+        sim = api.from_workload(wl, stream=_stream())
+        sim.step(2, wl.mdf_iters)
+        sim.sync()
+        assert (sim.get_info(api.INFO_TILE_ROWS), sim.get_info(api.INFO_LAYOUT)) == (rows, layout), name
+        if name == "W3x4":
+            ref = orc.from_workload(wl)
+            sim.step(8, wl.mdf_iters); ref.step(10, wl.mdf_iters)
+            sim.sync()
+            _compare_fields(sim, ref)
+            _check_markers(sim, ref, orc, wl)
+        sim.close()
+
+
 @pytest.mark.parametrize("iters", [1, 17, 64])
 def test_mdf_iteration_counts_from_one_to_the_maximum(api, orc, iters):
     """P:110 fixes 5 iterations; the loop is generic: 1 (interpolate once, spread Delta u once, R11), an odd count,

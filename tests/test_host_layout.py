@@ -39,7 +39,7 @@ def test_tiles_cover_the_rows():
 
 def test_workload_generators_are_seeded_and_sized():
     from paper_1904_02108_b200 import workloads
-    counts = {"W1": 240, "W3": 15360, "W3lit": 7680, "P1": 3936, "P6": 6 * 3936, "P18": 18 * 3936}
+    counts = {"W1": 240, "W3": 15360, "W3lit": 7680, "W3x4": 61440, "P1": 3936, "P6": 6 * 3936, "P18": 18 * 3936}
     for name, n in counts.items():
         a, b = workloads.get(name, 0), workloads.get(name, 0)
         assert a.n_markers == n
