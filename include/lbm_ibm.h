@@ -109,7 +109,7 @@ enum {
                              (summation order).                                                           */
     LBM_OPT_PERSISTENT = 11, /* the fused MDF loop (moments + N x (tile pass, collect)) as ONE persistent kernel
                              with grid-wide barriers instead of 2 N + 1 launches: 1 = on, 2 = off, 0 (default) =
-                             on for single-row tiles (see LBM_OPT_TILE_ROWS) with up to 36,000 markers on lattices
+                             on for single-row tiles (see LBM_OPT_TILE_ROWS) with up to 100,000 markers on lattices
                              of up to 4 Mi cells (where the chain of launches is the critical path of the step).
                              Results are bit-identical.                                                   */
     LBM_OPT_TILE_CAP = 12, /* > 0: cap the number of tile footprints (default 0 = room for every tile that can
@@ -135,7 +135,7 @@ enum {
     LBM_OPT_BULK_STREAM = 17, /* cache policy of the bulk stream-collide pass that runs beside the MDF loop (step layout
                              1): 1 = evict-first ("cache-streaming") loads and stores, so that the populations it
                              streams through L2 do not evict the few MB the MDF kernels work on; 2 = the default policy;
-                             0 (default) = 1 when the persistent MDF kernel is in use, else 2.  Results are
+                             0 (default) = 1 on lattices of up to 4 Mi cells, else 2.  Results are
                              bit-identical.                                                                       */
     LBM_OPT_MDF_BLOCKS = 13 /* tuning: blocks per SM of the tile pass / of the persistent MDF kernel (0 = default:
                              as many as fit / one); fewer blocks leave more of every SM to the stream-collide

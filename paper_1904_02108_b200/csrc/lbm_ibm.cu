@@ -92,7 +92,7 @@ constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driv
 // Measured on B200 (tiles at edge 4 / 2 / 1 and the best edge): P6 1441 / 3498 / 9807: 2; P18 4365 / 10527 / 29018: 4;
 // W4lit 3662 / 9153 / 25968: 4; P1 225 / 555 / 1621: 1 or 2.
 constexpr long long TILE_RULE_MIN_TILES = 2500;
-constexpr int PERSISTENT_MAX_MARKERS = 36000;   // persistent MDF kernel: faster than the kernel chain up to ~30 k markers, slower from ~45 k (128^3)
+constexpr int PERSISTENT_MAX_MARKERS = 100000;  // persistent MDF kernel: measured faster than the kernel chain from 7,680 to 92,160 markers (one propeller, 128^3)
 // Step layout (LBM_OPT_OVERLAP = 3): the split of the stream-collide into a bulk pass beside the MDF loop and a pass
 // over the stencil cells pays while the MDF loop is a chain of short, latency-bound kernels that leave the SMs mostly
 // idle (small marker sets); beyond that the tile pass fills the SMs itself and one fused pass after it is faster
@@ -422,12 +422,13 @@ bool use_persistent(const lbm *h)
 }
 
 // Cache policy of the bulk stream-collide pass that runs beside the MDF loop (LBM_OPT_BULK_STREAM): evict-first loads
-// and stores keep the ~1 GB it streams through L2 from evicting what the MDF kernels work on.  Automatic: with the
-// persistent MDF kernel (small marker sets on small lattices, where the two kernels run side by side from start to end).
+// and stores keep the ~1 GB it streams through L2 from evicting what the MDF kernels work on.  Automatic: on lattices
+// of up to 4 Mi cells (beside the persistent MDF kernel W3 gains 7 %, beside the kernel chain W3x4 4 %; on the 8 Mi
+// cells of P1 / P6 it costs 1 %).
 bool bulk_stream(const lbm *h)
 {
     if (h->opt_bulk_stream) return h->opt_bulk_stream == 1;
-    return use_persistent(h);
+    return use_persistent(h) || h->g.cells <= PERSISTENT_MAX_CELLS;
 }
 
 // Depth of the binning pipeline (LBM_OPT_PIPELINE): 2 = the binning of a step is spread over the two steps before it

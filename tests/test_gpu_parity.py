@@ -798,7 +798,7 @@ def test_tile_edge_follows_the_number_of_tiles_not_of_markers(api, orc):
     """Automatic tile edge (LBM_OPT_TILE_ROWS = 0): the largest of 4, 2, 1 that leaves >= 2,500 tiles in the rest pose.
     One thin propeller with 61,440 markers (W3 with 8 layers instead of 2) occupies a few hundred 4 x 4-row tiles: single-row
     tiles, layout 1; 6 and 18 paper-shaped propellers keep the edges they were tuned with (2 and 4).  The dense single
-    propeller is also compared with the oracle (it takes the kernel chain: above the persistent kernel's 36,000)."""
+    propeller is also compared with the oracle."""
     from paper_1904_02108_b200 import workloads
     for name, rows, layout in (("W3", 1, 1), ("W3x4", 1, 1), ("P6", 2, 1), ("P18", 4, 2)):
         wl = workloads.get(name)
