@@ -104,12 +104,14 @@ enum {
     LBM_OPT_TILE_ROWS = 10, /* source rows per tile in y and z for the fused path: 1, 2, 4, or 0 = automatic: the largest
                              of 4, 2, 1 for which the markers, in their rest pose, occupy at least 2,500 tiles (the
                              tile pass needs more tiles than warp slots; the number of tiles, not of markers,
-                             decides: one thin body of 60,000 markers occupies ~300 tiles of 4 x 4 rows).
+                             decides: one thin body of 60,000 markers occupies ~300 tiles of 4 x 4 rows); single-row
+                             tiles that are many and sparse (1,500 or more with fewer than 7 markers each) become
+                             two-row tiles.
                              Changing it rebuilds the tile tables at the next step.  Results agree to rounding
                              (summation order).                                                           */
     LBM_OPT_PERSISTENT = 11, /* the fused MDF loop (moments + N x (tile pass, collect)) as ONE persistent kernel
                              with grid-wide barriers instead of 2 N + 1 launches: 1 = on, 2 = off, 0 (default) =
-                             on for single-row tiles (see LBM_OPT_TILE_ROWS) with up to 100,000 markers on lattices
+                             on for up to 3,000 tiles (see LBM_OPT_TILE_ROWS) and 100,000 markers on lattices
                              of up to 4 Mi cells (where the chain of launches is the critical path of the step).
                              Results are bit-identical.                                                   */
     LBM_OPT_TILE_CAP = 12, /* > 0: cap the number of tile footprints (default 0 = room for every tile that can

@@ -85,13 +85,23 @@ constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driv
 // Tile edge by marker count (LBM_OPT_TILE_ROWS = 0), measured on B200: single-row tiles while
 // the set is so small that larger tiles would not fill the SMs (W1, W3: 15,360 markers), two-row tiles up to a few
 // ten thousand markers (P6), 4 x 4-row tiles beyond (P18, W4lit, W4, W5lit, W5).
-// Tile edge (source rows per tile in y and z): the largest of 4, 2, 1 that still gives the tile pass enough tiles --
-// about 1.4 per warp slot of the grid (148 SMs x 12 warps).  The count, not the marker count, is what matters: 60,000
-// markers of ONE thin propeller occupy ~300 tiles of 4 x 4 rows (most warps idle, 0.67 ms per step on 128^3) but
-// ~1,200 single-row tiles (0.17 ms); the same number of markers spread over 18 bodies fills 4,400 tiles of 4 x 4 rows.
-// Measured on B200 (tiles at edge 4 / 2 / 1 and the best edge): P6 1441 / 3498 / 9807: 2; P18 4365 / 10527 / 29018: 4;
-// W4lit 3662 / 9153 / 25968: 4; P1 225 / 555 / 1621: 1 or 2.
+// Tile edge (source rows per tile in y and z) and persistent kernel go by the number of TILES the markers occupy
+// (counted on the host for the rest pose, count_rest_tiles), because the marker count alone says little: 60,000 markers
+// of ONE thin propeller occupy ~230 tiles of 4 x 4 rows (most of the 1,776 warp slots idle, 0.67 ms per step on 128^3)
+// but ~2,000 single-row tiles (0.16 ms), while the same number of markers on 18 bodies fills 4,400 tiles of 4 x 4 rows.
+//   edge = the largest of 4, 2, 1 with at least TILE_RULE_MIN_TILES tiles (~1.4 per warp slot);
+//   single-row tiles that are many and sparse (>= 1,500 tiles with fewer than 7 markers each) become two-row tiles:
+//   the per-tile work then outweighs the markers';
+//   the persistent MDF kernel on small lattices up to PERSISTENT_MAX_TILES tiles.
+// Measured on B200, ms per step at edge 1 / 2 / 4 (chain unless "p"): P1 0.239 / 0.233 / 0.290; 3 paper-shaped
+// propellers 0.293 / 0.267 / 0.269p; P6 0.374 / 0.323 / 0.316p; P18 0.714 / 0.545 / 0.470; W4lit 0.89 / 0.74 / 0.68;
+// one propeller on 128^3 with 61,440 markers 0.157p / 0.244p / 0.568p; 8 propellers on 128^3 with 18,432 markers
+// 0.153p / 0.129p, with 73,728 markers 0.195 / 0.240p.  Persistent kernel against the chain on 128^3: faster with
+// 924 .. 2,679 tiles, slower with 3,921 and 4,524.
 constexpr long long TILE_RULE_MIN_TILES = 2500;
+constexpr long long SPARSE_MIN_TILES = 1500;
+constexpr double SPARSE_MAX_MARKERS_PER_TILE = 7.0;
+constexpr long long PERSISTENT_MAX_TILES = 3000;
 constexpr int PERSISTENT_MAX_MARKERS = 100000;  // persistent MDF kernel: measured faster than the kernel chain from 7,680 to 92,160 markers (one propeller, 128^3)
 // Step layout (LBM_OPT_OVERLAP = 3): the split of the stream-collide into a bulk pass beside the MDF loop and a pass
 // over the stencil cells pays while the MDF loop is a chain of short, latency-bound kernels that leave the SMs mostly
@@ -377,16 +387,34 @@ int list_grid(const lbm *h)
     return (int)std::min<long long>(LIST_GRID, std::max<long long>(h->sms, want));
 }
 
+// the persistent MDF kernel can be considered: small lattices only (on larger ones the lattice-wide stream-collide is
+// the critical path and the kernel only takes SM resources from it: P1 0.251 against 0.241 ms, P6 0.338 against 0.322)
+constexpr long long PERSISTENT_MAX_CELLS = 4LL << 20;
+bool persistent_eligible(const lbm *h, long long tiles)
+{
+    return h->g.cells <= PERSISTENT_MAX_CELLS && (long long)h->h_area.size() <= PERSISTENT_MAX_MARKERS &&
+           tiles <= PERSISTENT_MAX_TILES;
+}
+
+// the automatic choice of (tile edge, persistent kernel) for the markers as uploaded; tr_only > 0: for that edge
+struct AutoPlan { int tr; bool persistent; };
+AutoPlan auto_plan(const lbm *h, int tr_only = 0)
+{
+    int e = h->rest_tiles[2] >= TILE_RULE_MIN_TILES ? 2 : (h->rest_tiles[1] >= TILE_RULE_MIN_TILES ? 1 : 0);
+    if (e == 0 && h->rest_tiles[0] >= SPARSE_MIN_TILES &&
+        (double)h->h_area.size() < SPARSE_MAX_MARKERS_PER_TILE * (double)h->rest_tiles[0]) e = 1;
+    if (tr_only) e = tr_only == 4 ? 2 : (tr_only == 2 ? 1 : 0);
+    static const int edge[3] = {1, 2, 4};
+    return AutoPlan{edge[e], persistent_eligible(h, h->rest_tiles[e])};
+}
+
 // tile edge for the current markers and options: the comparison paths are written for 4 x 4 rows; the fused
-// path uses single-row tiles for small marker sets (enough tiles for all SMs) unless LBM_OPT_TILE_ROWS says otherwise
+// path takes the edge of the cost model above unless LBM_OPT_TILE_ROWS says otherwise
 int effective_tr(const lbm *h)
 {
     if (!fused_path(h)) return TILE_R;
     if (h->opt_tile_rows) return h->opt_tile_rows;
-    const size_t n = h->h_area.size();
-    (void)n;
-    if (h->rest_tiles[2] >= TILE_RULE_MIN_TILES) return TILE_R;
-    return h->rest_tiles[1] >= TILE_RULE_MIN_TILES ? 2 : 1;
+    return auto_plan(h).tr;
 }
 
 // how a coupled step is laid out (LBM_OPT_OVERLAP): 0 = one serial chain; 1 = three branches (MDF loop, bulk
@@ -413,12 +441,11 @@ int tile_warps(const lbm *h)
 // is the critical path of the step as long as the lattice-wide stream-collide beside it is shorter; on larger
 // lattices the stream-collide is the critical path and a persistent kernel only takes SM resources from it
 // (measured on B200: W3 0.107 against 0.140 ms per step, P1 0.251 against 0.241, P6 0.338 against 0.322).
-constexpr long long PERSISTENT_MAX_CELLS = 4LL << 20;
 bool use_persistent(const lbm *h)
 {
     if (!fused_path(h) || h->opt_moments != 0 || h->opt_timing) return false;
     if (h->opt_persistent) return h->opt_persistent == 1;
-    return effective_tr(h) == 1 && h->nm <= PERSISTENT_MAX_MARKERS && h->g.cells <= PERSISTENT_MAX_CELLS;
+    return auto_plan(h, h->opt_tile_rows).persistent;
 }
 
 // Cache policy of the bulk stream-collide pass that runs beside the MDF loop (LBM_OPT_BULK_STREAM): evict-first loads
@@ -1139,7 +1166,7 @@ bool stencil_inside(const lbm *h, const double lo[3], const double hi[3])
 }  // namespace
 
 // =================================================================================================
-// Register the tiles n new markers occupy in their rest pose, for the tile edges 1, 2 and 4 (see TILE_RULE_MIN_TILES).
+// Register the tiles n new markers occupy in their rest pose, for the tile edges 1, 2 and 4 (see auto_plan).
 // Rotating bodies sweep other tiles later on, but about as many.
 void count_rest_tiles(lbm *h, const float *pos, long long n)
 {
