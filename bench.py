@@ -11,8 +11,8 @@ stream-collide-force), replayed as one CUDA graph.
 `value` is measured on W4 (BASELINE.json configs[3]: 256^3 periodic, 64 three-blade propellers, 1,179,648 markers,
 5 MDF iterations): the coupled configuration on the SAME 256^3 lattice as the pure-LBM bandwidth case configs[1] (W2),
 so that coupled / pure is like for like.  The metric is a curve, not a point: `density_sweep` carries the same
-measurement for W3, W4lit, W4, W5lit, W5 (the largest single-GPU configuration, configs[4]) and the paper-shaped
-cases P1 / P6 / P18 (P:231-237's own sweep over 1 -> 6 -> 18 propellers).  All inputs are seeded synthetic
+measurement for W3, W3x4 (the propeller of W3 with four times the markers), W4lit, W4, W5lit, W5 (the largest single-GPU
+configuration, configs[4]) and the paper-shaped cases P1 / P6 / P18 (P:231-237's own sweep over 1 -> 6 -> 18 propellers).  All inputs are seeded synthetic
 (paper_1904_02108_b200/workloads.py).
 
 N > 1: "replicas only" (DESIGN.md): every rank runs the same workload on its own GPU, no data-path collective;
