@@ -82,9 +82,6 @@ struct HostBody {
 };
 
 constexpr int LIST_GRID = 148 * 8;   // persistent-style grids for the list-driven kernels (grid-stride loops over device-side lists)
-// Tile edge by marker count (LBM_OPT_TILE_ROWS = 0), measured on B200: single-row tiles while
-// the set is so small that larger tiles would not fill the SMs (W1, W3: 15,360 markers), two-row tiles up to a few
-// ten thousand markers (P6), 4 x 4-row tiles beyond (P18, W4lit, W4, W5lit, W5).
 // Tile edge (source rows per tile in y and z) and persistent kernel go by the number of TILES the markers occupy
 // (counted on the host for the rest pose, count_rest_tiles), because the marker count alone says little: 60,000 markers
 // of ONE thin propeller occupy ~230 tiles of 4 x 4 rows (most of the 1,776 warp slots idle, 0.67 ms per step on 128^3)
@@ -409,7 +406,7 @@ AutoPlan auto_plan(const lbm *h, int tr_only = 0)
 }
 
 // tile edge for the current markers and options: the comparison paths are written for 4 x 4 rows; the fused
-// path takes the edge of the cost model above unless LBM_OPT_TILE_ROWS says otherwise
+// path takes the edge of the rule above unless LBM_OPT_TILE_ROWS says otherwise
 int effective_tr(const lbm *h)
 {
     if (!fused_path(h)) return TILE_R;
