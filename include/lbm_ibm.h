@@ -111,7 +111,7 @@ enum {
                              (summation order).                                                           */
     LBM_OPT_PERSISTENT = 11, /* the fused MDF loop (moments + N x (tile pass, collect)) as ONE persistent kernel
                              with grid-wide barriers instead of 2 N + 1 launches: 1 = on, 2 = off, 0 (default) =
-                             on for up to 3,000 tiles (see LBM_OPT_TILE_ROWS) and 100,000 markers on lattices
+                             on for up to 3,000 single-row tiles (1,184 larger ones; see LBM_OPT_TILE_ROWS) and 100,000 markers on lattices
                              of up to 4 Mi cells (where the chain of launches is the critical path of the step).
                              Results are bit-identical.                                                   */
     LBM_OPT_TILE_CAP = 12, /* > 0: cap the number of tile footprints (default 0 = room for every tile that can

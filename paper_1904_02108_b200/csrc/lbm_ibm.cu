@@ -387,10 +387,12 @@ int list_grid(const lbm *h)
 // the persistent MDF kernel can be considered: small lattices only (on larger ones the lattice-wide stream-collide is
 // the critical path and the kernel only takes SM resources from it: P1 0.251 against 0.241 ms, P6 0.338 against 0.322)
 constexpr long long PERSISTENT_MAX_CELLS = 4LL << 20;
-bool persistent_eligible(const lbm *h, long long tiles)
+bool persistent_eligible(const lbm *h, long long tiles, int tr)
 {
-    return h->g.cells <= PERSISTENT_MAX_CELLS && (long long)h->h_area.size() <= PERSISTENT_MAX_MARKERS &&
-           tiles <= PERSISTENT_MAX_TILES;
+    // multi-row tiles are heavy: there the kernel pays only while every warp of its grid (148 x 8) gets at most one
+    // (8 propellers / 1,128 two-row tiles: 0.129 against 0.150 ms; a shell / 1,939 two-row tiles: 0.165 against 0.149)
+    const long long max_tiles = tr == 1 ? PERSISTENT_MAX_TILES : (long long)h->sms * MDFP_WARPS;
+    return h->g.cells <= PERSISTENT_MAX_CELLS && (long long)h->h_area.size() <= PERSISTENT_MAX_MARKERS && tiles <= max_tiles;
 }
 
 // the automatic choice of (tile edge, persistent kernel) for the markers as uploaded; tr_only > 0: for that edge
@@ -402,7 +404,7 @@ AutoPlan auto_plan(const lbm *h, int tr_only = 0)
         (double)h->h_area.size() < SPARSE_MAX_MARKERS_PER_TILE * (double)h->rest_tiles[0]) e = 1;
     if (tr_only) e = tr_only == 4 ? 2 : (tr_only == 2 ? 1 : 0);
     static const int edge[3] = {1, 2, 4};
-    return AutoPlan{edge[e], persistent_eligible(h, h->rest_tiles[e])};
+    return AutoPlan{edge[e], persistent_eligible(h, h->rest_tiles[e], edge[e])};
 }
 
 // tile edge for the current markers and options: the comparison paths are written for 4 x 4 rows; the fused
