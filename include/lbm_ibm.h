@@ -128,7 +128,7 @@ enum {
                              turn): 2 = the step's graph bins the second half of step n + 1 (gather, chunks, tiles,
                              active cells, collect plan) and, in a branch of its own, the first half of step n + 2
                              (kinematics, keys, sort); 1 = it bins all of step n + 1 in one branch; 0 (default) = 2
-                             up to 400,000 markers, else 1.  Results are bit-identical.                         */
+                             up to 400,000 markers or in step layout 1, else 1.  Results are bit-identical.    */
     LBM_OPT_TRACE = 15,   /* 1 = the graph of the overlapped step also records a timing event after every kernel of
                              the MDF branch, after the bulk stream-collide and after the binning branches; after
                              lbm_sync, lbm_get_info(LBM_INFO_TRACE_NS + i) is the device time in ns from the fork

@@ -464,7 +464,9 @@ constexpr int PIPE2_MAX_MARKERS = 400000;
 int pipeline_depth(const lbm *h)
 {
     if (h->opt_pipeline) return h->opt_pipeline;
-    return h->nm <= PIPE2_MAX_MARKERS ? 2 : 1;
+    // layout 1 (small tiles): the binning chain is on the critical path whatever the marker count (a shell of 420,000
+    // markers on 128^3: 0.447 against 0.507 ms)
+    return (h->nm <= PIPE2_MAX_MARKERS || overlap_mode(h) == 1) ? 2 : 1;
 }
 
 // the options a preparation depends on (which tables it builds)
